@@ -1,0 +1,16 @@
+"""Seeded synthetic metabolic-network generator (inputs only).
+
+This module serves BOTH the CPU oracle (``oracle/``) and the CUDA library
+(``paper_1804_02867_b200/``).  It holds none of the method's arithmetic: it only
+produces stoichiometric matrices, reversibility flags, internal/external masks
+and the parameter sets of the five ``BASELINE.json`` configs.
+"""
+from .networks import (  # noqa: F401
+    CONFIGS,
+    Network,
+    SplitMix64,
+    config_names,
+    hand_network,
+    make_network,
+    unimolecular_network,
+)

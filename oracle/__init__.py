@@ -1,0 +1,202 @@
+"""CPU oracle for the AND/OR-graph pathway traversal of arXiv 1804.02867 -- TEST INFRASTRUCTURE.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference``
+legs may import this package.  It shares no code with ``paper_1804_02867_b200`` (the CUDA library) and
+never imports it.  ``efm_oracle.c`` is the plain-C step-by-step procedure (SURVEY.md 8(c) O1-O9 + beam B);
+``check.py`` is the O9 self-check run on every output; ``brute_force.py`` enumerates all EFMs of tiny
+networks by subset enumeration (pin P9).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import Dict, List, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "efm_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle_efm.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile efm_oracle.c with gcc (OpenMP over the entries of a level)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [("max_support", ctypes.c_int32), ("max_loop", ctypes.c_int32), ("dep_depth", ctypes.c_int32),
+                ("max_visited", ctypes.c_int32), ("frontier_cap", ctypes.c_int64), ("threads", ctypes.c_int32),
+                ("reserved", ctypes.c_int32), ("shuffle_seed", ctypes.c_uint64)]
+
+
+STAT_FIELDS = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxloop", "discarded_nonpos",
+               "discarded_overflow", "discarded_visited", "truncated_beam", "unique_supports", "poisoned",
+               "output", "peak_frontier", "algo_bytes"]
+
+
+class _Stats(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_int64) for k in STAT_FIELDS]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.oracle_enumerate.restype = ctypes.c_int
+        lib.oracle_enumerate.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p,
+                                         ctypes.c_void_p, ctypes.POINTER(_Params), ctypes.c_void_p,
+                                         ctypes.c_void_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_void_p)]
+        lib.oracle_result_count.restype = ctypes.c_int64
+        lib.oracle_result_count.argtypes = [ctypes.c_void_p]
+        lib.oracle_result_copy.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.oracle_result_stats.argtypes = [ctypes.c_void_p, ctypes.POINTER(_Stats)]
+        lib.oracle_result_levels.restype = ctypes.c_int64
+        lib.oracle_result_levels.argtypes = [ctypes.c_void_p] + [ctypes.c_void_p] * 4 + [ctypes.c_int64]
+        lib.oracle_result_roots.restype = ctypes.c_int32
+        lib.oracle_result_roots.argtypes = [ctypes.c_void_p]
+        lib.oracle_graph_info.argtypes = [ctypes.c_void_p] + [ctypes.c_void_p] * 5
+        lib.oracle_graph_export.argtypes = [ctypes.c_void_p] + [ctypes.c_void_p] * 14
+        lib.oracle_result_free.argtypes = [ctypes.c_void_p]
+        lib.oracle_state_hash.restype = ctypes.c_uint64
+        lib.oracle_state_hash.argtypes = [ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
+                                          ctypes.c_void_p]
+        lib.oracle_max_threads.restype = ctypes.c_int32
+        lib.oracle_mix64.restype = ctypes.c_uint64
+        lib.oracle_mix64.argtypes = [ctypes.c_uint64]
+        _lib = lib
+    return _lib
+
+
+def max_threads() -> int:
+    return int(_load().oracle_max_threads())
+
+
+@dataclass
+class OracleResult:
+    flux: np.ndarray  # int64 [n_out, n], reaction space, coprime, lexicographic order
+    stats: Dict[str, int]
+    levels: Dict[str, np.ndarray]  # per level: active, done, expanded, children
+    n_roots: int
+    graph: Optional[Dict[str, np.ndarray]] = None
+
+
+def _ptr(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarray, params: Dict[str, int],
+                       seed_sets: Optional[Sequence[Sequence[int]]] = None, threads: int = 1,
+                       shuffle_seed: int = 0, export_graph: bool = False,
+                       self_check: bool = True) -> OracleResult:
+    """Run the oracle.  ``seed_sets`` holds arc codes 2*j + (dir < 0); None = default boundary arcs (O2)."""
+    lib = _load()
+    S = np.ascontiguousarray(S, dtype=np.int32)
+    rev = np.ascontiguousarray(reversible, dtype=np.uint8)
+    internal = np.ascontiguousarray(internal, dtype=np.uint8)
+    m, n = S.shape
+    p = _Params(int(params.get("max_support", 0)), int(params.get("max_loop", 8)), int(params.get("dep_depth", 4)),
+                int(params.get("max_visited", 0)), int(params.get("frontier_cap", 0)), int(threads), 0,
+                int(shuffle_seed))
+    if seed_sets:
+        ptr = np.zeros(len(seed_sets) + 1, dtype=np.int32)
+        ptr[1:] = np.cumsum([len(s) for s in seed_sets])
+        codes = np.array([c for s in seed_sets for c in s], dtype=np.int32)
+        n_sets = len(seed_sets)
+    else:
+        ptr = np.zeros(1, dtype=np.int32)
+        codes = np.zeros(1, dtype=np.int32)
+        n_sets = 0
+    handle = ctypes.c_void_p()
+    rc = lib.oracle_enumerate(_ptr(S), m, n, _ptr(rev), _ptr(internal), ctypes.byref(p), _ptr(ptr), _ptr(codes),
+                              n_sets, ctypes.byref(handle))
+    try:
+        if rc != 0:
+            raise ValueError(f"oracle_enumerate: invalid input (code {rc})")
+        k = lib.oracle_result_count(handle)
+        flux = np.zeros((k, n), dtype=np.int64)
+        if k:
+            lib.oracle_result_copy(handle, _ptr(flux))
+        st = _Stats()
+        lib.oracle_result_stats(handle, ctypes.byref(st))
+        stats = {f: int(getattr(st, f)) for f in STAT_FIELDS}
+        nl = int(stats["levels"])
+        arrs = [np.zeros(max(nl, 1), dtype=np.int64) for _ in range(4)]
+        lib.oracle_result_levels(handle, *[_ptr(a) for a in arrs], nl)
+        levels = dict(active=arrs[0][:nl], done=arrs[1][:nl], expanded=arrs[2][:nl], children=arrs[3][:nl])
+        graph = None
+        if export_graph:
+            M, A, W = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
+            nnz, depb = ctypes.c_int64(), ctypes.c_int64()
+            lib.oracle_graph_info(handle, ctypes.byref(M), ctypes.byref(A), ctypes.byref(W), ctypes.byref(nnz),
+                                  ctypes.byref(depb))
+            M, A, W, nnz, depb = M.value, A.value, W.value, nnz.value, depb.value
+            g = dict(
+                arc_rxn=np.zeros(A, np.int32), arc_dir=np.zeros(A, np.int32), twin=np.zeros(A, np.int32),
+                in_ptr=np.zeros(M + 1, np.int32), in_arc=np.zeros(nnz, np.int32), in_c=np.zeros(nnz, np.int64),
+                out_ptr=np.zeros(M + 1, np.int32), out_arc=np.zeros(nnz, np.int32), out_c=np.zeros(nnz, np.int64),
+                col_ptr=np.zeros(A + 1, np.int32), col_met=np.zeros(nnz, np.int32), col_s=np.zeros(nnz, np.int64),
+                dep_off=np.zeros(M + 1, np.int64), dep=np.zeros(max(depb, 1), np.uint8))
+            order = ["arc_rxn", "arc_dir", "twin", "in_ptr", "in_arc", "in_c", "out_ptr", "out_arc", "out_c",
+                     "col_ptr", "col_met", "col_s", "dep_off", "dep"]
+            lib.oracle_graph_export(handle, *[_ptr(g[k2]) for k2 in order])
+            g["in_arc"] = g["in_arc"][: g["in_ptr"][-1]]
+            g["in_c"] = g["in_c"][: g["in_ptr"][-1]]
+            g["out_arc"] = g["out_arc"][: g["out_ptr"][-1]]
+            g["out_c"] = g["out_c"][: g["out_ptr"][-1]]
+            g["dep"] = g["dep"][:depb]
+            g.update(M=M, A=A, W=W)
+            graph = g
+        n_roots = int(lib.oracle_result_roots(handle))
+    finally:
+        lib.oracle_result_free(handle)
+    res = OracleResult(flux, stats, levels, n_roots, graph)
+    if self_check:
+        from .check import check_outputs
+        check_outputs(S, rev, internal, flux)
+    return res
+
+
+def enumerate_network(net, threads: int = 1, shuffle_seed: int = 0, export_graph: bool = False,
+                      self_check: bool = True, seed_sets="net", **param_overrides) -> OracleResult:
+    """Run the oracle on a ``netgen.Network`` with its own parameters (optionally overridden).
+
+    ``seed_sets="net"`` uses the network's own seed sets (None there = default boundary arcs)."""
+    params = dict(net.params)
+    params.update(param_overrides)
+    seeds = net.seed_sets if isinstance(seed_sets, str) else seed_sets
+    return enumerate_pathways(net.S, net.reversible, net.internal, params, seeds, threads, shuffle_seed,
+                              export_graph, self_check)
+
+
+def state_hash(arcs: Sequence[int], fluxes: Sequence[int], visited: Sequence[Sequence[int]]) -> int:
+    """h of beam B for an explicit state; visited rows are (met, PI, PO, cnt)."""
+    lib = _load()
+    a = np.array(list(arcs), dtype=np.int32)
+    f = np.array(list(fluxes), dtype=np.int64)
+    v = np.array([x for row in visited for x in row], dtype=np.int32)
+    if v.size == 0:
+        v = np.zeros(4, dtype=np.int32)
+    return int(lib.oracle_state_hash(len(a), _ptr(a), _ptr(f), len(visited), _ptr(v)))
+
+
+def mix64(x: int) -> int:
+    return int(_load().oracle_mix64(ctypes.c_uint64(x & ((1 << 64) - 1))))
+
+
+def all_arc_seed_sets(reversible: np.ndarray) -> List[List[int]]:
+    """One seed set per arc (pins P7, P9)."""
+    out: List[List[int]] = []
+    for j, r in enumerate(reversible):
+        out.append([2 * j])
+        if r:
+            out.append([2 * j + 1])
+    return out

@@ -1,0 +1,326 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself: expected values are hand-derived fixtures
+(tests/golden/hand_pins.json), closed forms, textbook enumerations written here independently,
+brute-force subset enumeration, published SplitMix64 test vectors, or invariants.
+"""
+import json
+import os
+from fractions import Fraction
+from math import gcd
+
+import numpy as np
+import pytest
+
+from netgen import SplitMix64, hand_network, make_network, unimolecular_network
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "hand_pins.json")
+
+
+def _cases():
+    with open(GOLDEN) as fh:
+        return json.load(fh)["cases"]
+
+
+@pytest.mark.parametrize("case", _cases(), ids=lambda c: c["name"])
+def test_hand_pins(oracle_mod, case):
+    rx = [(s, p, r) for s, p, r in case["reactions"]]
+    net = hand_network(rx, case["internal"])
+    res = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, case["seeds"])
+    assert res.flux.tolist() == case["flux"]
+    for k in ("expanded", "levels", "discarded_nonpos"):
+        if k in case:
+            assert res.stats[k] == case[k], k
+
+
+def test_linear_chain_closed_form(oracle_mod):
+    """P6 in general: ->A0, c0 A0 -> p0 A1, ..., A_k ->  has the single EFM given by ratio products."""
+    rng = SplitMix64(7)
+    for _trial in range(40):
+        k = rng.between(1, 6)
+        cons = [rng.between(1, 5) for _ in range(k)]
+        prod = [rng.between(1, 5) for _ in range(k)]
+        names = [f"A{t}" for t in range(k + 1)]
+        rx = [({}, {names[0]: 1}, False)]
+        for t in range(k):
+            rx.append(({names[t]: cons[t]}, {names[t + 1]: prod[t]}, False))
+        rx.append(({names[k]: 1}, {}, False))
+        net = hand_network(rx, names)
+        # closed form with rationals: v0 = 1; flux of chain reaction t = (amount of A_t) / cons[t]
+        v = [Fraction(1)]
+        amount = Fraction(1)
+        for t in range(k):
+            v.append(amount / cons[t])
+            amount = v[-1] * prod[t]
+        v.append(amount)
+        den = 1
+        for x in v:
+            den = den * x.denominator // gcd(den, x.denominator)
+        iv = [int(x * den) for x in v]
+        g = 0
+        for x in iv:
+            g = gcd(g, x)
+        expect = [x // g for x in iv]
+        res = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, [[0]])
+        assert res.flux.tolist() == [expect]
+
+
+def _paths_and_cycles(S, rev):
+    """Textbook enumeration on a unimolecular unit network: simple source->sink paths and simple directed
+    cycles over arcs (a reversible reaction contributes two arcs that exclude each other)."""
+    m, n = S.shape
+    arcs = []  # (rxn, dir, tail or None, head or None)
+    for j in range(n):
+        col = S[:, j]
+        tail = [i for i in range(m) if col[i] < 0]
+        head = [i for i in range(m) if col[i] > 0]
+        t = tail[0] if tail else None
+        h = head[0] if head else None
+        arcs.append((j, +1, t, h))
+        if rev[j]:
+            arcs.append((j, -1, h, t))
+    out = set()
+
+    def emit(used):
+        v = [0] * n
+        for a in used:
+            v[arcs[a][0]] += arcs[a][1]
+        out.add(tuple(v))
+
+    by_tail = {}
+    for a, (_j, _d, t, _h) in enumerate(arcs):
+        by_tail.setdefault(t, []).append(a)
+
+    def rxns(used):
+        return {arcs[a][0] for a in used}
+
+    # source -> sink simple paths
+    def dfs(node, used, seen):
+        for a in by_tail.get(node, []):
+            j, _d, _t, h = arcs[a]
+            if j in rxns(used):
+                continue
+            if h is None:
+                emit(used + [a])
+            elif h not in seen:
+                dfs(h, used + [a], seen | {h})
+
+    for a in by_tail.get(None, []):
+        h = arcs[a][3]
+        if h is None:
+            continue
+        dfs(h, [a], {h})
+    # simple directed cycles (rooted at their lowest node)
+    def cyc(start, node, used, seen):
+        for a in by_tail.get(node, []):
+            j, _d, _t, h = arcs[a]
+            if h is None or j in rxns(used):
+                continue
+            if h == start:
+                emit(used + [a])
+            elif h not in seen and h > start:
+                cyc(start, h, used + [a], seen | {h})
+
+    for s in range(m):
+        cyc(s, s, [], {s})
+    return out
+
+
+def test_unimolecular_equals_paths_and_cycles(oracle_mod):
+    """P7 (Lemma 2 type I, Theorem 1): with every arc seeded the output is
+    exactly {simple source->sink paths} U {simple directed cycles}."""
+    total = 0
+    for seed in range(24):
+        net = unimolecular_network(seed, m_int=4 + seed % 4, n_rxn=7 + seed % 6, n_rev=seed % 3)
+        seeds = oracle_mod.all_arc_seed_sets(net.reversible)
+        res = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, seeds)
+        got = set(map(tuple, res.flux.tolist()))
+        expect = _paths_and_cycles(net.S, net.reversible)
+        assert got == expect, f"seed {seed}"
+        total += len(expect)
+    assert total > 50
+
+
+def test_toy_against_brute_force(oracle_mod, capsys):
+    """P9: recall/precision of the (approximate) method against Definition 3 written out."""
+    from oracle.brute_force import brute_force_efms
+    net = make_network("toy", 0)
+    truth = brute_force_efms(net.S, net.reversible, net.internal)
+    assert len(truth) >= 2  # the planted routes
+    for label, seeds in (("boundary", None), ("all-arcs", oracle_mod.all_arc_seed_sets(net.reversible))):
+        res = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, seeds)
+        got = set(map(tuple, res.flux.tolist()))
+        recall = len(got & truth) / len(truth)
+        precision = len(got & truth) / max(1, len(got))
+        with capsys.disabled():
+            print(f"\n[toy/{label}] EFMs {len(truth)}, found {len(got)}, recall {recall:.2f}, precision {precision:.2f}")
+        assert recall >= 0.5 and precision >= 0.5
+    # small brute-forceable random networks: every balanced output must be a true EFM or be reported
+    rng = SplitMix64(3)
+    hits = tot = 0
+    for t in range(12):
+        net = unimolecular_network(100 + t, 4, 8, 1)
+        # make it non-unimolecular: add a hyperarc reaction A+B -> C
+        S = np.concatenate([net.S, np.zeros((net.S.shape[0], 1), np.int32)], axis=1)
+        a, b, c = rng.sample(range(4), 3)
+        S[a, -1], S[b, -1], S[c, -1] = -1, -rng.between(1, 2), rng.between(1, 2)
+        rev = np.concatenate([net.reversible, [0]]).astype(np.uint8)
+        truth = brute_force_efms(S, rev, net.internal)
+        params = dict(max_support=0, max_loop=8, dep_depth=4, max_visited=0, frontier_cap=0)
+        res = oracle_mod.enumerate_pathways(S, rev, net.internal, params, oracle_mod.all_arc_seed_sets(rev))
+        got = set(map(tuple, res.flux.tolist()))
+        hits += len(got & truth)
+        tot += len(truth)
+    assert tot > 0 and hits / tot >= 0.6
+
+
+def test_invariants_and_precision(oracle_mod, capsys):
+    """P8: Def 2 / Def 3 invariants hold on every output; precision by exact rank test is reported."""
+    from oracle.check import check_outputs
+    for name, over in (("toy", {}), ("small", {}), ("core", dict(frontier_cap=2048)),
+                       ("mid", dict(frontier_cap=512)), ("genome", dict(frontier_cap=256))):
+        net = make_network(name, 0)
+        res = oracle_mod.enumerate_network(net, threads=2, self_check=False, **over)
+        rep = check_outputs(net.S, net.reversible, net.internal, res.flux)
+        with capsys.disabled():
+            print(f"\n[{name}] outputs {len(res.flux)}, precision {rep['precision']:.3f}, stats {res.stats}")
+        assert res.stats["output"] == len(res.flux)
+        assert res.stats["unique_supports"] >= res.stats["output"] + res.stats["poisoned"]
+        assert res.stats["children"] + res.n_roots == res.stats["done"] + res.stats["expanded"] + res.stats["truncated_beam"]
+
+
+def test_order_independence(oracle_mod):
+    """P10: shuffling every level and changing the thread count changes nothing, beam active."""
+    for name, cap in (("small", 300), ("core", 1024), ("genome", 128)):
+        net = make_network(name, 0)
+        base = oracle_mod.enumerate_network(net, threads=1, self_check=False, frontier_cap=cap)
+        assert base.stats["truncated_beam"] > 0
+        for threads, shuf in ((1, 12345), (3, 0), (4, 999)):
+            other = oracle_mod.enumerate_network(net, threads=threads, shuffle_seed=shuf, self_check=False,
+                                                 frontier_cap=cap)
+            assert other.stats == base.stats
+            assert np.array_equal(other.flux, base.flux)
+            assert all(np.array_equal(other.levels[k], base.levels[k]) for k in base.levels)
+
+
+def test_beam_is_inactive_above_peak(oracle_mod):
+    """A cap at or above the peak frontier must reproduce the uncapped run exactly."""
+    net = make_network("small", 0)
+    free = oracle_mod.enumerate_network(net, self_check=False)
+    peak = free.stats["peak_frontier"]
+    capped = oracle_mod.enumerate_network(net, self_check=False, frontier_cap=peak)
+    assert capped.stats == free.stats and np.array_equal(capped.flux, free.flux)
+    tight = oracle_mod.enumerate_network(net, self_check=False, frontier_cap=peak - 1)
+    assert tight.stats["truncated_beam"] > 0
+    assert all(a <= peak for a in tight.levels["expanded"])
+    assert all(e <= peak - 1 for e in tight.levels["expanded"])
+
+
+def test_mix64_matches_published_splitmix64_vectors(oracle_mod):
+    """SplitMix64 (Steele, Lea, Flood 2014) seeded with 0 emits 0xE220A8397B1DCDAF, 0x6E789E6AA1B965F4,
+    0x06C45D188009454F; output t is the finaliser applied to t * 0x9E3779B97F4A7C15."""
+    gamma = 0x9E3779B97F4A7C15
+    expect = [0xE220A8397B1DCDAF, 0x6E789E6AA1B965F4, 0x06C45D188009454F]
+    for t, e in enumerate(expect, start=1):
+        assert oracle_mod.mix64((t * gamma) & ((1 << 64) - 1)) == e
+
+
+def test_state_hash_structure(oracle_mod):
+    """h is a function of the complete state and of nothing else (beam B): order-free, field-sensitive,
+    and composed as mix(sum of element terms) - checked through the exported primitive."""
+    h = oracle_mod.state_hash
+    base = h([3, 9, 4], [2, 5, 1], [(1, 3, 9, 0), (7, 4, 9, 2)])
+    assert base == h([4, 3, 9], [1, 2, 5], [(7, 4, 9, 2), (1, 3, 9, 0)])
+    variants = [
+        h([3, 9, 5], [2, 5, 1], [(1, 3, 9, 0), (7, 4, 9, 2)]),
+        h([3, 9, 4], [2, 5, 2], [(1, 3, 9, 0), (7, 4, 9, 2)]),
+        h([3, 9, 4], [2, 5, 1], [(1, 3, 9, 1), (7, 4, 9, 2)]),
+        h([3, 9, 4], [2, 5, 1], [(1, 9, 3, 0), (7, 4, 9, 2)]),
+        h([3, 9, 4], [2, 5, 1], [(2, 3, 9, 0), (7, 4, 9, 2)]),
+        h([3, 9, 4], [2, 5, 1], [(1, 3, 9, 0)]),
+        h([3, 9], [2, 5], [(1, 3, 9, 0), (7, 4, 9, 2)]),
+    ]
+    assert len(set(variants + [base])) == len(variants) + 1
+    m = oracle_mod.mix64
+    mask = (1 << 64) - 1
+    one_arc = m((m((1 << 56) | 11) + 6) & mask)
+    one_vis = m((2 << 56) | (3 << 48) | (5 << 32) | (11 << 16) | 12)
+    assert h([11], [6], []) == m(one_arc)
+    assert h([11], [6], [(5, 11, 12, 3)]) == m((one_arc + one_vis) & mask)
+
+
+def _walk_dep(g, L):
+    """Def 11 / Alg 2 by exhaustive enumeration of arc chains (no breadth-first shortcut)."""
+    M, A = g["M"], g["A"]
+    prods = [[] for _ in range(A)]
+    for a in range(A):
+        for q in range(g["col_ptr"][a], g["col_ptr"][a + 1]):
+            if g["col_s"][q] > 0:
+                prods[a].append(int(g["col_met"][q]))
+    consumers = [[int(x) for x in g["out_arc"][g["out_ptr"][i]:g["out_ptr"][i + 1]]] for i in range(M)]
+    dep = set()
+    for i in range(M):
+        ins = [int(x) for x in g["in_arc"][g["in_ptr"][i]:g["in_ptr"][i + 1]]]
+
+        def walk(o, x, length):
+            if x in ins and x != o:
+                dep.add((i, o, x))
+            if length == L:
+                return
+            for q in prods[x]:
+                if q == i:
+                    continue
+                for y in consumers[q]:
+                    if y != g["twin"][x]:
+                        walk(o, y, length + 1)
+
+        for o in consumers[i]:
+            walk(o, o, 1)
+    return dep
+
+
+def test_graph_and_dep_table(oracle_mod):
+    """O1 against S itself (sign convention PAPER.md:45) and O7 against exhaustive chain enumeration."""
+    for name in ("toy", "small"):
+        net = make_network(name, 0)
+        res = oracle_mod.enumerate_network(net, export_graph=True, self_check=False)
+        g = res.graph
+        Sint = net.S[net.internal.astype(bool)].astype(np.int64)
+        assert g["M"] == Sint.shape[0] and g["A"] == net.n_arcs
+        dense = np.zeros((g["M"], g["A"]), np.int64)
+        for a in range(g["A"]):
+            for q in range(g["col_ptr"][a], g["col_ptr"][a + 1]):
+                dense[g["col_met"][q], a] = g["col_s"][q]
+        for a in range(g["A"]):
+            assert np.array_equal(dense[:, a], Sint[:, g["arc_rxn"][a]] * g["arc_dir"][a])
+            t = g["twin"][a]
+            if t >= 0:
+                assert g["arc_rxn"][t] == g["arc_rxn"][a] and g["arc_dir"][t] == -g["arc_dir"][a]
+                assert net.reversible[g["arc_rxn"][a]]
+        for i in range(g["M"]):
+            ins = g["in_arc"][g["in_ptr"][i]:g["in_ptr"][i + 1]]
+            outs = g["out_arc"][g["out_ptr"][i]:g["out_ptr"][i + 1]]
+            assert list(ins) == [a for a in range(g["A"]) if dense[i, a] > 0]
+            assert list(outs) == [a for a in range(g["A"]) if dense[i, a] < 0]
+            assert list(g["in_c"][g["in_ptr"][i]:g["in_ptr"][i + 1]]) == [dense[i, a] for a in ins]
+            assert list(g["out_c"][g["out_ptr"][i]:g["out_ptr"][i + 1]]) == [-dense[i, a] for a in outs]
+        truth = _walk_dep(g, net.params["dep_depth"])
+        got = set()
+        for i in range(g["M"]):
+            ins = g["in_arc"][g["in_ptr"][i]:g["in_ptr"][i + 1]]
+            outs = g["out_arc"][g["out_ptr"][i]:g["out_ptr"][i + 1]]
+            for lo, o in enumerate(outs):
+                for le, e in enumerate(ins):
+                    if g["dep"][g["dep_off"][i] + lo * len(ins) + le]:
+                        got.add((i, int(o), int(e)))
+        assert got == truth
+        assert len(truth) > 0
+
+
+def test_seed_validation(oracle_mod):
+    net = make_network("toy", 0)
+    j_rev = int(np.nonzero(net.reversible)[0][0])
+    j_irr = int(np.nonzero(net.reversible == 0)[0][0])
+    for bad in ([[2 * j_rev, 2 * j_rev + 1]], [[2 * j_irr + 1]], [[2 * net.n]], [[0, 0]], [[]]):
+        with pytest.raises(ValueError):
+            oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, bad)
