@@ -1,0 +1,161 @@
+/*
+ * efm_b200.h -- C ABI of the B200 (sm_100a) library for the data-parallel hot path of
+ * arXiv 1804.02867 ("A system architecture for parallel analysis of flux-balanced metabolic
+ * pathways"): the AND/OR-graph pathway traversal (Alg 1 + Alg 3 METAx).
+ *
+ * Problem statement the interface follows (Alg 1): "Input: the stoichiometric
+ * matrix of a given metabolic network.  Output: a set of minimal flux-balanced pathways"; the
+ * reversibility flags and the internal/external split are properties of the input network
+ * and the set of initial reactions is a user choice.
+ *
+ * Conventions
+ *   - every function returns EFM_OK (0) or a negative EFM_E_* code; nothing throws;
+ *   - "host" / "device" is stated for every pointer; host inputs are caller-owned and copied;
+ *   - the library never allocates device memory: the caller (PyTorch in this repo) owns one
+ *     workspace allocation and the CUDA stream, both passed to efm_enumerate();
+ *   - results live inside the workspace and are invalidated by the next efm_enumerate() on
+ *     the handle, by freeing the workspace, or by efm_destroy();
+ *   - a handle is not thread-safe;
+ *   - the work is done by CUDA kernels only: there is no CPU fallback.  Without a usable
+ *     CUDA device efm_enumerate() fails with EFM_E_CUDA.
+ */
+#ifndef EFM_B200_H
+#define EFM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EFM_OK 0
+#define EFM_E_INVAL (-1)    /* bad pointer / shape / parameter / seed set                         */
+#define EFM_E_NOMEM (-2)    /* workspace smaller than efm_workspace_bytes() reports               */
+#define EFM_E_CAPACITY (-3) /* a frontier / candidate / key buffer overflowed: results undefined, */
+                            /* never silently truncated                                           */
+#define EFM_E_CUDA (-4)     /* CUDA runtime error (text retained for efm_last_error())            */
+#define EFM_E_STATE (-5)    /* result accessor called before a successful efm_enumerate()         */
+
+/* flags */
+#define EFM_F_TIMING 0x1u       /* record CUDA events around every kernel phase (efm_stats.ms_*)   */
+#define EFM_F_FORCE_TWO_PASS 0x2u /* always run count+select+write, even when the beam cannot bind */
+#define EFM_F_NO_FASTPATH 0x4u  /* evaluate every child with the warp-cooperative general routine  */
+
+typedef struct efm_handle efm_handle; /* opaque: host copy of the graph + pointers INTO the workspace */
+
+/* Traversal parameters.  Alg 1's #defines M, R are taken from S; C (number of
+ * candidate blocks) is replaced by the beam `frontier_cap`; r_max / m_max / #B / #T are thread-index
+ * artefacts of the paper's mapping and do not exist here. */
+typedef struct {
+    int32_t max_support;    /* D: max arcs in a pathway; 0 = number of arcs                          */
+    int32_t max_loop;       /* MAX_LOOP; 0 = 8                          */
+    int32_t dep_depth;      /* L: chain length of the dependent-reaction search; 0 = 4 */
+    int32_t max_visited;    /* V: max visited metabolites per pathway; 0 = 2*D                       */
+    int64_t frontier_cap;   /* beam: entries expanded per level; 0 = unbounded                       */
+    int64_t max_frontier;   /* slots per frontier buffer; 0 = max(frontier_cap, 2^20 when cap == 0)  */
+    int64_t max_candidates; /* capacity of the candidate buffer / support hash; 0 = 2^20             */
+    int64_t max_child_keys; /* capacity of the per-level beam key array; 0 = 64 * frontier_cap       */
+    int32_t device;         /* CUDA device ordinal the workspace lives on                            */
+    uint32_t flags;         /* EFM_F_*                                                               */
+} efm_params;
+
+typedef struct {
+    int64_t levels, expanded, children, done, dead_end, not_efm_maxloop, discarded_nonpos,
+        discarded_overflow, discarded_visited, truncated_beam, unique_supports, poisoned, output;
+    int64_t peak_frontier;  /* largest number of active entries in a level, before the beam          */
+    int64_t algo_bytes;     /* algorithmic bytes of all expansions            */
+    int64_t n_roots;
+    int64_t launches;       /* kernels launched by the last efm_enumerate()                          */
+    int64_t two_pass_levels, direct_levels;
+    /* milliseconds; ms_total is always measured (CUDA events on the caller's stream), the per-phase
+     * figures only with EFM_F_TIMING */
+    double ms_build, ms_total, ms_expand_count, ms_beam, ms_expand_write, ms_direct, ms_hash,
+        ms_filter, ms_output;
+    int64_t n_expand_count, n_expand_write, n_direct; /* launches behind the three expand timers     */
+    int64_t filter_pairs;   /* signature pair tests done by the minimality filter                    */
+} efm_stats;
+
+/* Build the modified AND/OR graph MG (Defs 4-6; "Convert the given matrix to the MG
+ * graph structure") and the static flux-dependency table (Def 11, PAPER.md:130;
+ * Alg 2 DEPTHy).
+ *   S          host, int32, m x n, element (i, j) at S[i*row_stride + j]; > 0 produced, < 0 consumed
+ *
+ *   reversible host, uint8[n]; nonzero = reaction j may run backwards (split into two arcs)
+ *   internal   host, uint8[m]; nonzero = metabolite i is internal (balanced); others are external
+ *   p          host; NULL = all defaults
+ *   out        host; receives the handle (free with efm_destroy)
+ * Errors: EFM_E_INVAL for NULL pointers, m/n <= 0, more than 65535 arcs or internal metabolites,
+ * negative parameters. */
+int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const uint8_t* reversible,
+               const uint8_t* internal, const efm_params* p, efm_handle** out);
+
+/* Sizes of the graph: internal metabolites M, arcs A, 64-bit bitset words W = ceil(A/64), nonzeros of the
+ * internal arc columns, entries of the dependency table (sum over nodes of |O| * |I|).  All host. */
+int efm_graph_info(const efm_handle* h, int32_t* n_internal, int32_t* n_arcs, int32_t* bitset_words,
+                   int64_t* nnz, int64_t* dep_entries);
+
+/* Copy the host-side graph out (builder tests).  Every pointer is host memory sized from
+ * efm_graph_info(): arc_rxn/arc_dir/twin [A]; in_ptr/out_ptr [M+1]; in_arc/in_c and out_arc/out_c
+ * [in_ptr[M]] / [out_ptr[M]]; col_ptr [A+1]; col_met/col_s [nnz]; dep_off [M+1]; dep [dep_entries]
+ * with dep[dep_off[i] + lo*|I_i| + le] = 1 iff (O_i[lo], I_i[le]) are flux-dependent.  NULLs are skipped. */
+int efm_graph_export(const efm_handle* h, int32_t* arc_rxn, int32_t* arc_dir, int32_t* twin, int32_t* in_ptr,
+                     int32_t* in_arc, int64_t* in_c, int32_t* out_ptr, int32_t* out_arc, int64_t* out_c,
+                     int32_t* col_ptr, int32_t* col_met, int64_t* col_s, int64_t* dep_off, uint8_t* dep);
+
+/* Bytes of device workspace efm_enumerate() needs for this handle's parameters (host out). */
+int efm_workspace_bytes(const efm_handle* h, size_t* bytes);
+
+/* Run the traversal (INIT + METAx), the support dedup, the minimality filter
+ * (Def 3) and the canonical output stage, all on the device.
+ *   seed_ptr      host, int32[n_sets+1], CSR offsets into seed_arc_code
+ *   seed_arc_code host, int32: 2*j + (direction < 0) for reaction j; each set becomes one root pathway
+ *                 with those arcs at flux 1
+ *   n_sets        0 = default seeds: one root per boundary arc (Def 8)
+ *   d_workspace   DEVICE memory, >= efm_workspace_bytes(), 256-byte aligned, caller-owned
+ *   cuda_stream   a cudaStream_t (NULL = default stream); all work is enqueued there and the call
+ *                 returns after the stream has been synchronised
+ * Errors: EFM_E_INVAL (bad seed: unknown code, duplicate, both twins, backward arc of an irreversible
+ * reaction, empty or larger than D), EFM_E_NOMEM, EFM_E_CAPACITY, EFM_E_CUDA. */
+int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_arc_code, int32_t n_sets,
+                  void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Number of pathways found (host out). */
+int efm_result_count(const efm_handle* h, int64_t* n_pathways);
+
+/* Dense result: flux is HOST memory, capacity_rows x n int64 row-major; row r = coprime integer flux
+ * vector in reaction space (v_j = f_j+ - f_j-), rows in strict lexicographic order.  Rows are densified
+ * on the device in chunks and copied back.  EFM_E_INVAL if capacity_rows < count. */
+int efm_result_copy(const efm_handle* h, int64_t* flux, int64_t capacity_rows);
+
+/* Sparse result to HOST memory: nnz[count]; rxn and val are count x row_capacity (row_capacity from
+ * efm_result_sparse_stride()), entries beyond nnz[r] are unspecified; rxn ascending within a row. */
+int efm_result_sparse_stride(const efm_handle* h, int32_t* row_capacity);
+int efm_result_copy_sparse(const efm_handle* h, int32_t* nnz, int32_t* rxn, int64_t* val, int64_t capacity_rows);
+
+/* DEVICE pointers to the sparse result inside the workspace (same layout as above). */
+int efm_result_device(const efm_handle* h, const int32_t** d_nnz, const int32_t** d_rxn, const int64_t** d_val);
+
+/* Densify rows [row0, row0+n_rows) into caller-owned DEVICE memory d_out (n_rows x n int64) on `cuda_stream`. */
+int efm_result_densify(const efm_handle* h, int64_t row0, int64_t n_rows, int64_t* d_out, void* cuda_stream);
+
+int efm_get_stats(const efm_handle* h, efm_stats* st);
+
+/* Per-level counters of the last run (host out, each `capacity` long; returns the number of levels through
+ * *n_levels): active entries before the beam, balanced (Done) entries, entries expanded, children generated. */
+int efm_get_level_stats(const efm_handle* h, int64_t* active, int64_t* done, int64_t* expanded, int64_t* children,
+                        int64_t capacity, int64_t* n_levels);
+
+/* Beam key of an explicit state, computed by a one-thread kernel on `device`; test hook
+ * for the device copy of the state hash.  All pointers host. vis4 rows are (met, PI, PO, cnt). */
+int efm_debug_state_hash(int32_t device, int32_t n_supp, const int32_t* arc, const int64_t* flux, int32_t n_vis,
+                         const int32_t* vis4, uint64_t* hash_out);
+
+void efm_destroy(efm_handle* h);
+const char* efm_strerror(int code);
+const char* efm_last_error(const efm_handle* h); /* text of the last CUDA error, "" if none */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EFM_B200_H */

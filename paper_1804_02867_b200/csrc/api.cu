@@ -1,0 +1,622 @@
+// C ABI of the library (include/efm_b200.h) and the host driver of the level loop (Alg 1 main body).
+// The driver only sequences kernels and reads back one small control block per level; every step of the path
+// (roots, classify, beam select, expand, dedup, minimality filter, canonical output) runs in the kernels.
+#include <algorithm>
+#include <cstdio>
+#include <ctime>
+#include <cstddef>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/efm_b200.h"
+#include "device_common.cuh"
+#include "graph.hpp"
+#include "launch.hpp"
+
+using namespace efm;
+
+namespace {
+
+struct Region { size_t off = 0, bytes = 0; };
+
+struct Layout {
+    Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir;
+    Region ctl, buf[2], keys, cand, table, isrep, poison, uniq, size_hist, bucket_start, bucket_fill;
+    Region order, sig, size_sorted, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, dense;
+    size_t total = 0;
+};
+
+size_t pow2_at_least(size_t x) { size_t p = 1; while (p < x) p <<= 1; return p; }
+
+}  // namespace
+
+struct efm_handle {
+    HostGraph G;
+    int32_t D = 0, V = 0, max_loop = 8, L = 4;
+    int64_t cap = 0, max_frontier = 0, max_cand = 0, max_keys = 0;
+    int32_t device = 0;
+    uint32_t flags = 0;
+    uint32_t stride = 0, cand_stride = 0;
+    size_t table_size = 0, dense_bytes = 0;
+    Layout lay;
+    double ms_build = 0;
+    // run state
+    unsigned char* ws = nullptr;
+    bool have_result = false;
+    int64_t n_out = 0;
+    efm_stats stats;
+    std::vector<int64_t> lvl_active, lvl_done, lvl_expanded, lvl_children;
+    std::string last_error;
+    Ctl* h_ctl = nullptr;   // pinned host mirror of the control block
+    int sm_count = 148;
+    std::vector<cudaEvent_t> events;
+};
+
+namespace {
+
+void add_region(Layout& L, Region& r, size_t bytes) {
+    L.total = (L.total + 255) & ~(size_t)255;
+    r.off = L.total;
+    r.bytes = bytes;
+    L.total += bytes;
+}
+
+void make_layout(efm_handle* h) {
+    const HostGraph& G = h->G;
+    Layout L;
+    add_region(L, L.col_ptr, sizeof(int) * (G.A + 1));
+    add_region(L, L.col, sizeof(int2) * (G.col.size() + 1));
+    add_region(L, L.in_ptr, sizeof(int) * (G.M + 1));
+    add_region(L, L.in_e, sizeof(int2) * (G.in.size() + 1));
+    add_region(L, L.out_ptr, sizeof(int) * (G.M + 1));
+    add_region(L, L.out_e, sizeof(int2) * (G.out.size() + 1));
+    add_region(L, L.twin, sizeof(int) * (G.A + 1));
+    add_region(L, L.dep_off, sizeof(i64) * (G.M + 1));
+    add_region(L, L.dep_bits, sizeof(u32) * G.dep_bits.size());
+    add_region(L, L.arc_rxn, sizeof(int) * (G.A + 1));
+    add_region(L, L.arc_dir, sizeof(int) * (G.A + 1));
+    add_region(L, L.ctl, sizeof(Ctl));
+    add_region(L, L.buf[0], (size_t)h->max_frontier * h->stride);
+    add_region(L, L.buf[1], (size_t)h->max_frontier * h->stride);
+    add_region(L, L.keys, (size_t)h->max_keys * 8);
+    const size_t C = (size_t)h->max_cand;
+    add_region(L, L.cand, C * h->cand_stride);
+    add_region(L, L.table, h->table_size * 4);
+    add_region(L, L.isrep, C + 1);
+    add_region(L, L.poison, C + 1);
+    add_region(L, L.uniq, C * 4);
+    const size_t bins = (size_t)h->D + 2;
+    add_region(L, L.size_hist, bins * 4);
+    add_region(L, L.bucket_start, bins * 4);
+    add_region(L, L.bucket_fill, bins * 4);
+    add_region(L, L.order, C * 4);
+    add_region(L, L.sig, C * 16);
+    add_region(L, L.size_sorted, C * 2);
+    add_region(L, L.keep, C);
+    add_region(L, L.u_nnz, C * 4);
+    add_region(L, L.u_rxn, C * h->D * 4);
+    add_region(L, L.u_val, C * h->D * 8);
+    add_region(L, L.sort_idx, pow2_at_least(C) * 4);
+    add_region(L, L.r_nnz, C * 4);
+    add_region(L, L.r_rxn, C * h->D * 4);
+    add_region(L, L.r_val, C * h->D * 8);
+    add_region(L, L.dense, h->dense_bytes);
+    L.total = (L.total + 255) & ~(size_t)255;
+    h->lay = L;
+}
+
+int fail_cuda(efm_handle* h, cudaError_t e, const char* what) {
+    char buf[256];
+    snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+    h->last_error = buf;
+    cudaGetLastError();
+    return EFM_E_CUDA;
+}
+#define CK(call)                                                       \
+    do {                                                               \
+        cudaError_t e__ = (call);                                      \
+        if (e__ != cudaSuccess) return fail_cuda(h, e__, #call);       \
+    } while (0)
+
+DevGraph dev_graph(const efm_handle* h, unsigned char* ws) {
+    const Layout& L = h->lay;
+    DevGraph g;
+    g.M = h->G.M; g.A = h->G.A; g.W32 = (h->G.A + 31) / 32; g.M32 = (h->G.M + 31) / 32;
+    g.col_ptr = (const int*)(ws + L.col_ptr.off);   g.col = (const int2*)(ws + L.col.off);
+    g.in_ptr = (const int*)(ws + L.in_ptr.off);     g.in_e = (const int2*)(ws + L.in_e.off);
+    g.out_ptr = (const int*)(ws + L.out_ptr.off);   g.out_e = (const int2*)(ws + L.out_e.off);
+    g.twin = (const int*)(ws + L.twin.off);
+    g.dep_off = (const i64*)(ws + L.dep_off.off);   g.dep_bits = (const u32*)(ws + L.dep_bits.off);
+    g.arc_rxn = (const int*)(ws + L.arc_rxn.off);   g.arc_dir = (const int*)(ws + L.arc_dir.off);
+    return g;
+}
+
+// Events for the optional per-phase timers.
+struct Timer {
+    efm_handle* h; cudaStream_t s; bool on; size_t used = 0;
+    struct Span { size_t a, b; int phase; };
+    std::vector<Span> spans;
+    cudaEvent_t get() {
+        if (used == h->events.size()) { cudaEvent_t e; cudaEventCreate(&e); h->events.push_back(e); }
+        return h->events[used++];
+    }
+    size_t mark() { if (!on) return 0; cudaEvent_t e = get(); cudaEventRecord(e, s); return used - 1; }
+    void span(size_t a, size_t b, int phase) { if (on) spans.push_back(Span{a, b, phase}); }
+};
+enum { PH_COUNT = 0, PH_BEAM, PH_WRITE, PH_DIRECT, PH_HASH, PH_FILTER, PH_OUTPUT, PH_N };
+
+}  // namespace
+
+extern "C" {
+
+const char* efm_strerror(int code) {
+    switch (code) {
+        case EFM_OK: return "ok";
+        case EFM_E_INVAL: return "invalid argument";
+        case EFM_E_NOMEM: return "workspace too small";
+        case EFM_E_CAPACITY: return "frontier / candidate / key capacity exceeded (results undefined)";
+        case EFM_E_CUDA: return "CUDA error (see efm_last_error)";
+        case EFM_E_STATE: return "no result available";
+        default: return "unknown error";
+    }
+}
+const char* efm_last_error(const efm_handle* h) { return h ? h->last_error.c_str() : ""; }
+
+int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const uint8_t* reversible,
+               const uint8_t* internal, const efm_params* p, efm_handle** out) {
+    if (!out) return EFM_E_INVAL;
+    *out = nullptr;
+    efm_params P;
+    memset(&P, 0, sizeof P);
+    if (p) P = *p;
+    if (P.max_support < 0 || P.max_loop < 0 || P.dep_depth < 0 || P.max_visited < 0 || P.frontier_cap < 0 ||
+        P.max_frontier < 0 || P.max_candidates < 0 || P.max_child_keys < 0 || P.device < 0)
+        return EFM_E_INVAL;
+    efm_handle* h = new (std::nothrow) efm_handle();
+    if (!h) return EFM_E_NOMEM;
+    memset(&h->stats, 0, sizeof h->stats);
+    cudaEvent_t t0 = nullptr;
+    (void)t0;
+    const auto c0 = std::clock();
+    h->L = P.dep_depth ? P.dep_depth : 4;
+    int rc = build_graph(h->G, S, m, n, row_stride, reversible, internal, h->L);
+    if (rc != EFM_OK) { delete h; return rc; }
+    h->ms_build = 1000.0 * (double)(std::clock() - c0) / CLOCKS_PER_SEC;
+    const HostGraph& G = h->G;
+    h->D = P.max_support ? P.max_support : G.A;
+    if (h->D > G.A) h->D = std::max(G.A, 1);
+    h->V = P.max_visited ? P.max_visited : 2 * h->D;
+    h->max_loop = P.max_loop ? P.max_loop : 8;
+    if (h->D > 4096 || h->max_loop > 65535) { delete h; return EFM_E_INVAL; }
+    h->cap = P.frontier_cap;
+    h->device = P.device;
+    h->flags = P.flags;
+    const int Veff = std::min(h->V, std::max(G.M, 1));   // a pathway cannot visit more nodes than exist
+    h->stride = entry_bytes((u32)h->D, (u32)Veff);
+    h->cand_stride = entry_bytes((u32)h->D, 0);
+    h->max_frontier = P.max_frontier ? P.max_frontier : (h->cap ? std::max<int64_t>(h->cap, 4096) : (int64_t)1 << 20);
+    h->max_cand = P.max_candidates ? P.max_candidates : (int64_t)1 << 20;
+    if (h->max_cand > 0xFFFFFFF0LL) { delete h; return EFM_E_INVAL; }
+    h->max_keys = P.max_child_keys ? P.max_child_keys : std::max<int64_t>(h->cap * (int64_t)G.max_fanout, 65536);
+    h->table_size = pow2_at_least((size_t)h->max_cand * 2);
+    h->dense_bytes = std::max<size_t>((size_t)64 << 20, (size_t)n * 8 * 64);
+    make_layout(h);
+    *out = h;
+    return EFM_OK;
+}
+
+int efm_graph_info(const efm_handle* h, int32_t* n_internal, int32_t* n_arcs, int32_t* bitset_words, int64_t* nnz,
+                   int64_t* dep_entries) {
+    if (!h) return EFM_E_INVAL;
+    if (n_internal) *n_internal = h->G.M;
+    if (n_arcs) *n_arcs = h->G.A;
+    if (bitset_words) *bitset_words = (h->G.A + 63) / 64;
+    if (nnz) *nnz = (int64_t)h->G.col.size();
+    if (dep_entries) *dep_entries = h->G.dep_off[h->G.M];
+    return EFM_OK;
+}
+
+int efm_graph_export(const efm_handle* h, int32_t* arc_rxn, int32_t* arc_dir, int32_t* twin, int32_t* in_ptr,
+                     int32_t* in_arc, int64_t* in_c, int32_t* out_ptr, int32_t* out_arc, int64_t* out_c,
+                     int32_t* col_ptr, int32_t* col_met, int64_t* col_s, int64_t* dep_off, uint8_t* dep) {
+    if (!h) return EFM_E_INVAL;
+    const HostGraph& G = h->G;
+    for (int a = 0; a < G.A; ++a) {
+        if (arc_rxn) arc_rxn[a] = G.arc_rxn[a];
+        if (arc_dir) arc_dir[a] = G.arc_dir[a];
+        if (twin) twin[a] = G.twin[a];
+    }
+    for (int i = 0; i <= G.M; ++i) {
+        if (in_ptr) in_ptr[i] = G.in_ptr[i];
+        if (out_ptr) out_ptr[i] = G.out_ptr[i];
+        if (dep_off) dep_off[i] = G.dep_off[i];
+    }
+    for (size_t q = 0; q < G.in.size(); ++q) { if (in_arc) in_arc[q] = G.in[q].arc; if (in_c) in_c[q] = G.in[q].c; }
+    for (size_t q = 0; q < G.out.size(); ++q) { if (out_arc) out_arc[q] = G.out[q].arc; if (out_c) out_c[q] = G.out[q].c; }
+    for (int a = 0; a <= G.A; ++a) if (col_ptr) col_ptr[a] = G.col_ptr[a];
+    for (size_t q = 0; q < G.col.size(); ++q) { if (col_met) col_met[q] = G.col[q].met; if (col_s) col_s[q] = G.col[q].s; }
+    if (dep)
+        for (int64_t b = 0; b < G.dep_off[G.M]; ++b) dep[b] = (uint8_t)((G.dep_bits[b >> 5] >> (b & 31)) & 1u);
+    return EFM_OK;
+}
+
+int efm_workspace_bytes(const efm_handle* h, size_t* bytes) {
+    if (!h || !bytes) return EFM_E_INVAL;
+    *bytes = h->lay.total;
+    return EFM_OK;
+}
+
+int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_arc_code, int32_t n_sets,
+                  void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!h || !d_workspace || n_sets < 0 || (n_sets > 0 && (!seed_ptr || !seed_arc_code))) return EFM_E_INVAL;
+    if (((uintptr_t)d_workspace & 255) != 0) return EFM_E_INVAL;
+    if (workspace_bytes < h->lay.total) return EFM_E_NOMEM;
+    h->have_result = false;
+    h->last_error.clear();
+    const HostGraph& G = h->G;
+    const Layout& L = h->lay;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+
+    // ---- O2 roots (INIT kernel of the paper): host packs the seed sets, the device classifies them
+    std::vector<std::vector<int>> roots;
+    if (n_sets == 0) {
+        // default: one root per boundary arc = non-empty, single-signed internal column (Def 8)
+        for (int a = 0; a < G.A; ++a) {
+            int pos = 0, neg = 0;
+            for (int q = G.col_ptr[a]; q < G.col_ptr[a + 1]; ++q) (G.col[q].s > 0 ? pos : neg)++;
+            if ((pos > 0) != (neg > 0)) roots.push_back(std::vector<int>(1, a));
+        }
+    } else {
+        std::vector<char> mark((size_t)G.A, 0);
+        for (int t = 0; t < n_sets; ++t) {
+            const int cnt = seed_ptr[t + 1] - seed_ptr[t];
+            if (cnt <= 0 || cnt > h->D) return EFM_E_INVAL;
+            std::vector<int> arcs;
+            bool bad = false;
+            for (int k = 0; k < cnt && !bad; ++k) {
+                const int code = seed_arc_code[seed_ptr[t] + k];
+                const int a = (code >= 0 && code < 2 * G.n) ? G.code2arc[code] : -1;
+                if (a < 0 || mark[a] || (G.twin[a] >= 0 && mark[G.twin[a]])) bad = true;
+                else { mark[a] = 1; arcs.push_back(a); }
+            }
+            for (int a : arcs) mark[a] = 0;
+            if (bad) return EFM_E_INVAL;
+            std::sort(arcs.begin(), arcs.end());
+            roots.push_back(arcs);
+        }
+    }
+    const u64 n_roots = roots.size();
+    if ((int64_t)n_roots > h->max_frontier || (int64_t)n_roots > h->max_keys) return EFM_E_CAPACITY;
+    std::vector<unsigned char> root_img((size_t)n_roots * h->stride, 0);
+    for (size_t r = 0; r < roots.size(); ++r) {
+        unsigned char* e = root_img.data() + r * h->stride;
+        const u32 ns = (u32)roots[r].size();
+        *(u32*)e = ns;   // n_vis = 0
+        i64* f = (i64*)(e + 16);
+        u16* arc = (u16*)(e + 16 + 8 * (size_t)ns);
+        for (u32 k = 0; k < ns; ++k) { f[k] = 1; arc[k] = (u16)roots[r][k]; }
+    }
+
+    CK(cudaSetDevice(h->device));
+    if (!h->h_ctl) {
+        CK(cudaMallocHost((void**)&h->h_ctl, sizeof(Ctl)));
+        int smc = 0;
+        CK(cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, h->device));
+        if (smc > 0) h->sm_count = smc;
+    }
+    unsigned char* ws = (unsigned char*)d_workspace;
+    h->ws = ws;
+    Timer tm{h, s, (h->flags & EFM_F_TIMING) != 0};
+    cudaEvent_t ev_start = tm.get(), ev_end = tm.get();
+    CK(cudaEventRecord(ev_start, s));
+
+    // ---- upload the graph (~100 KB) and the roots; clear the control block
+    auto up = [&](const Region& r, const void* src, size_t bytes) -> cudaError_t {
+        if (bytes == 0) return cudaSuccess;
+        return cudaMemcpyAsync(ws + r.off, src, bytes, cudaMemcpyHostToDevice, s);
+    };
+    CK(up(L.col_ptr, G.col_ptr.data(), sizeof(int) * G.col_ptr.size()));
+    CK(up(L.col, G.col.data(), sizeof(ColRef) * G.col.size()));
+    CK(up(L.in_ptr, G.in_ptr.data(), sizeof(int) * G.in_ptr.size()));
+    CK(up(L.in_e, G.in.data(), sizeof(ArcRef) * G.in.size()));
+    CK(up(L.out_ptr, G.out_ptr.data(), sizeof(int) * G.out_ptr.size()));
+    CK(up(L.out_e, G.out.data(), sizeof(ArcRef) * G.out.size()));
+    CK(up(L.twin, G.twin.data(), sizeof(int) * G.twin.size()));
+    CK(up(L.dep_off, G.dep_off.data(), sizeof(i64) * G.dep_off.size()));
+    CK(up(L.dep_bits, G.dep_bits.data(), sizeof(u32) * G.dep_bits.size()));
+    CK(up(L.arc_rxn, G.arc_rxn.data(), sizeof(int) * G.arc_rxn.size()));
+    CK(up(L.arc_dir, G.arc_dir.data(), sizeof(int) * G.arc_dir.size()));
+    CK(up(L.buf[1], root_img.data(), root_img.size()));
+    CK(cudaMemsetAsync(ws + L.ctl.off, 0, sizeof(Ctl), s));
+    CK(cudaStreamSynchronize(s));   // the host staging vectors above go out of scope later; keep it simple
+
+    Ctl* d_ctl = (Ctl*)(ws + L.ctl.off);
+    Ctl* hc = h->h_ctl;
+    const size_t ctl_read = offsetof(Ctl, hist);
+    int launches = 0;
+    ExpandArgs ea;
+    memset(&ea, 0, sizeof ea);
+    ea.g = dev_graph(h, ws);
+    ea.cand = ws + L.cand.off;
+    ea.keys = (u64*)(ws + L.keys.off);
+    ea.ctl = d_ctl;
+    ea.stride = h->stride; ea.cand_stride = h->cand_stride;
+    ea.max_frontier = (u64)h->max_frontier; ea.max_cand = (u64)h->max_cand; ea.max_keys = (u64)h->max_keys;
+    ea.D = h->D; ea.V = h->V; ea.max_loop = h->max_loop;
+    expand_smem_layout(ea);
+
+    auto read_ctl = [&]() -> cudaError_t {
+        cudaError_t e = cudaMemcpyAsync(hc, d_ctl, ctl_read, cudaMemcpyDeviceToHost, s);
+        if (e != cudaSuccess) return e;
+        return cudaStreamSynchronize(s);
+    };
+
+    efm_stats& st = h->stats;
+    memset(&st, 0, sizeof st);
+    st.ms_build = h->ms_build;
+    st.n_roots = (int64_t)n_roots;
+    h->lvl_active.clear(); h->lvl_done.clear(); h->lvl_expanded.clear(); h->lvl_children.clear();
+    int64_t truncated = 0, done_total = 0;
+
+    // ---- level 0: classify the roots, beam-select, keep the survivors
+    int cur = 0;
+    u64 n_cur = 0;
+    if (n_roots > 0) {
+        CK(launch_level_begin(d_ctl, s)); ++launches;
+        ea.cur = ws + L.buf[1].off; ea.nxt = ws + L.buf[0].off; ea.n_cur = n_roots;
+        size_t t0 = tm.mark();
+        CK(launch_expand(0, true, ea, h->sm_count, s)); ++launches;
+        size_t t1 = tm.mark();
+        CK(launch_select(ea.keys, d_ctl, (u64)h->cap, ea.max_keys, n_roots, h->sm_count, s, &launches));
+        size_t t2 = tm.mark();
+        CK(launch_expand(1, true, ea, h->sm_count, s)); ++launches;
+        size_t t3 = tm.mark();
+        tm.span(t0, t1, PH_COUNT); tm.span(t1, t2, PH_BEAM); tm.span(t2, t3, PH_WRITE);
+        CK(read_ctl());
+        if (hc->error) return EFM_E_CAPACITY;
+        h->lvl_active.push_back((int64_t)hc->n_keys);
+        h->lvl_done.push_back((int64_t)hc->lvl_done);
+        h->lvl_expanded.push_back(0);
+        h->lvl_children.push_back(0);
+        done_total += (int64_t)hc->lvl_done;
+        truncated += (int64_t)hc->n_keys - (int64_t)hc->n_next;
+        n_cur = hc->n_next;
+        cur = 0;
+    }
+
+    // ---- level loop (Alg 3 while(true), as level-synchronous frontier expansion)
+    while (n_cur > 0) {
+        const size_t lvl = h->lvl_active.size() - 1;   // level of the parents
+        CK(launch_level_begin(d_ctl, s)); ++launches;
+        ea.cur = ws + L.buf[cur].off; ea.nxt = ws + L.buf[cur ^ 1].off; ea.n_cur = n_cur;
+        const bool beam_possible = h->cap > 0 && ((h->flags & EFM_F_FORCE_TWO_PASS) || n_cur * (u64)G.max_fanout > (u64)h->cap);
+        if (beam_possible) {
+            size_t t0 = tm.mark();
+            CK(launch_expand(0, false, ea, h->sm_count, s)); ++launches;
+            size_t t1 = tm.mark();
+            CK(launch_select(ea.keys, d_ctl, (u64)h->cap, ea.max_keys, std::min<u64>(ea.max_keys, n_cur * (u64)G.max_fanout), h->sm_count, s, &launches));
+            size_t t2 = tm.mark();
+            CK(launch_expand(1, false, ea, h->sm_count, s)); ++launches;
+            size_t t3 = tm.mark();
+            tm.span(t0, t1, PH_COUNT); tm.span(t1, t2, PH_BEAM); tm.span(t2, t3, PH_WRITE);
+            st.two_pass_levels++; st.n_expand_count++; st.n_expand_write++;
+        } else {
+            size_t t0 = tm.mark();
+            CK(launch_expand(2, false, ea, h->sm_count, s)); ++launches;
+            size_t t1 = tm.mark();
+            tm.span(t0, t1, PH_DIRECT);
+            st.direct_levels++; st.n_direct++;
+        }
+        CK(read_ctl());
+        if (hc->error) return EFM_E_CAPACITY;
+        h->lvl_expanded[lvl] = (int64_t)hc->lvl_expanded;
+        h->lvl_children[lvl] = (int64_t)hc->lvl_children;
+        const int64_t active = beam_possible ? (int64_t)hc->n_keys : (int64_t)hc->n_next;
+        const int64_t done = (int64_t)hc->lvl_done;
+        if (active + done > 0) {
+            h->lvl_active.push_back(active);
+            h->lvl_done.push_back(done);
+            h->lvl_expanded.push_back(0);
+            h->lvl_children.push_back(0);
+        }
+        done_total += done;
+        truncated += active - (int64_t)hc->n_next;
+        n_cur = hc->n_next;
+        cur ^= 1;
+    }
+
+    // ---- O8: support dedup + poison (a-6), minimality filter (a-7), canonical output (a-8)
+    const u64 n_cand = n_roots ? hc->n_cand : 0;
+    PostArgs pa;
+    memset(&pa, 0, sizeof pa);
+    pa.g = ea.g; pa.ctl = d_ctl;
+    pa.cand = ws + L.cand.off; pa.cand_stride = h->cand_stride; pa.max_cand = (u64)h->max_cand;
+    pa.table = (u32*)(ws + L.table.off); pa.table_size = h->table_size;
+    pa.isrep = ws + L.isrep.off; pa.poison = ws + L.poison.off; pa.uniq = (u32*)(ws + L.uniq.off);
+    pa.size_hist = (u32*)(ws + L.size_hist.off); pa.bucket_start = (u32*)(ws + L.bucket_start.off);
+    pa.bucket_fill = (u32*)(ws + L.bucket_fill.off); pa.n_size_bins = h->D + 2;
+    pa.order = (u32*)(ws + L.order.off); pa.sig = (ulonglong2*)(ws + L.sig.off);
+    pa.size_sorted = (u16*)(ws + L.size_sorted.off); pa.keep = ws + L.keep.off;
+    pa.D = h->D; pa.n_rxn = G.n;
+    pa.u_nnz = (int*)(ws + L.u_nnz.off); pa.u_rxn = (int*)(ws + L.u_rxn.off); pa.u_val = (i64*)(ws + L.u_val.off);
+    pa.sort_idx = (u32*)(ws + L.sort_idx.off);
+    pa.r_nnz = (int*)(ws + L.r_nnz.off); pa.r_rxn = (int*)(ws + L.r_rxn.off); pa.r_val = (i64*)(ws + L.r_val.off);
+    u64 n_uniq_ok = 0, n_keep = 0;
+    if (n_cand > 0) {
+        size_t t0 = tm.mark();
+        CK(launch_dedup(pa, n_cand, s, &launches));
+        size_t t1 = tm.mark();
+        tm.span(t0, t1, PH_HASH);
+        CK(read_ctl());
+        n_uniq_ok = hc->n_uniq_ok;
+        st.unique_supports = (int64_t)hc->n_unique;
+        st.poisoned = (int64_t)hc->n_poisoned;
+        if (n_uniq_ok > 0) {
+            size_t t2 = tm.mark();
+            CK(launch_filter(pa, n_uniq_ok, h->sm_count, s, &launches));
+            size_t t3 = tm.mark();
+            CK(launch_output_rows(pa, n_uniq_ok, s, &launches));
+            CK(read_ctl());
+            n_keep = hc->n_keep;
+            st.filter_pairs = (int64_t)hc->filter_pairs;
+            pa.n_pad = pow2_at_least((size_t)std::max<u64>(n_keep, 2));
+            CK(launch_output_sort(pa, n_keep, s, &launches));
+            size_t t4 = tm.mark();
+            tm.span(t2, t3, PH_FILTER); tm.span(t3, t4, PH_OUTPUT);
+        }
+    }
+    CK(cudaEventRecord(ev_end, s));
+    CK(cudaStreamSynchronize(s));
+
+    st.levels = (int64_t)h->lvl_active.size();
+    st.expanded = (int64_t)hc->st[ST_EXPANDED];
+    st.children = (int64_t)hc->st[ST_CHILDREN];
+    st.done = done_total;
+    st.dead_end = (int64_t)hc->st[ST_DEAD_END];
+    st.not_efm_maxloop = (int64_t)hc->st[ST_NOT_EFM];
+    st.discarded_nonpos = (int64_t)hc->st[ST_NONPOS];
+    st.discarded_overflow = (int64_t)hc->st[ST_OVERFLOW];
+    st.discarded_visited = (int64_t)hc->st[ST_VISITED];
+    st.truncated_beam = truncated;
+    st.output = (int64_t)n_keep;
+    st.algo_bytes = (int64_t)hc->st[ST_ALGO_BYTES];
+    st.peak_frontier = 0;
+    for (int64_t a : h->lvl_active) st.peak_frontier = std::max(st.peak_frontier, a);
+    st.launches = launches;
+    float ms = 0;
+    CK(cudaEventElapsedTime(&ms, ev_start, ev_end));
+    st.ms_total = ms;
+    if (tm.on) {
+        double acc[PH_N] = {0};
+        for (const Timer::Span& sp : tm.spans) {
+            float t = 0;
+            CK(cudaEventElapsedTime(&t, h->events[sp.a], h->events[sp.b]));
+            acc[sp.phase] += t;
+        }
+        st.ms_expand_count = acc[PH_COUNT]; st.ms_beam = acc[PH_BEAM]; st.ms_expand_write = acc[PH_WRITE];
+        st.ms_direct = acc[PH_DIRECT]; st.ms_hash = acc[PH_HASH]; st.ms_filter = acc[PH_FILTER]; st.ms_output = acc[PH_OUTPUT];
+    }
+    h->n_out = (int64_t)n_keep;
+    h->have_result = true;
+    return EFM_OK;
+}
+
+int efm_result_count(const efm_handle* h, int64_t* n_pathways) {
+    if (!h || !n_pathways) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    *n_pathways = h->n_out;
+    return EFM_OK;
+}
+
+int efm_result_device(const efm_handle* h, const int32_t** d_nnz, const int32_t** d_rxn, const int64_t** d_val) {
+    if (!h) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    if (d_nnz) *d_nnz = (const int32_t*)(h->ws + h->lay.r_nnz.off);
+    if (d_rxn) *d_rxn = (const int32_t*)(h->ws + h->lay.r_rxn.off);
+    if (d_val) *d_val = (const int64_t*)(h->ws + h->lay.r_val.off);
+    return EFM_OK;
+}
+
+int efm_result_sparse_stride(const efm_handle* h, int32_t* row_capacity) {
+    if (!h || !row_capacity) return EFM_E_INVAL;
+    *row_capacity = h->D;
+    return EFM_OK;
+}
+
+int efm_result_densify(const efm_handle* hc, int64_t row0, int64_t n_rows, int64_t* d_out, void* cuda_stream) {
+    efm_handle* h = const_cast<efm_handle*>(hc);
+    if (!h || !d_out || row0 < 0 || n_rows < 0) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    if (row0 + n_rows > h->n_out) return EFM_E_INVAL;
+    CK(cudaSetDevice(h->device));
+    CK(launch_densify((const int*)(h->ws + h->lay.r_nnz.off), (const int*)(h->ws + h->lay.r_rxn.off),
+                      (const i64*)(h->ws + h->lay.r_val.off), h->D, h->G.n, row0, n_rows, (i64*)d_out, (cudaStream_t)cuda_stream));
+    return EFM_OK;
+}
+
+int efm_result_copy(const efm_handle* hc, int64_t* flux, int64_t capacity_rows) {
+    efm_handle* h = const_cast<efm_handle*>(hc);
+    if (!h || (!flux && capacity_rows > 0)) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    if (capacity_rows < h->n_out) return EFM_E_INVAL;
+    if (h->n_out == 0) return EFM_OK;
+    CK(cudaSetDevice(h->device));
+    const int64_t n = h->G.n;
+    const int64_t chunk = std::max<int64_t>(1, (int64_t)(h->lay.dense.bytes / ((size_t)n * 8)));
+    i64* d_dense = (i64*)(h->ws + h->lay.dense.off);
+    for (int64_t r0 = 0; r0 < h->n_out; r0 += chunk) {
+        const int64_t nr = std::min(chunk, h->n_out - r0);
+        CK(launch_densify((const int*)(h->ws + h->lay.r_nnz.off), (const int*)(h->ws + h->lay.r_rxn.off),
+                          (const i64*)(h->ws + h->lay.r_val.off), h->D, (int)n, r0, nr, d_dense, 0));
+        CK(cudaMemcpyAsync(flux + r0 * n, d_dense, (size_t)nr * n * 8, cudaMemcpyDeviceToHost, 0));
+        CK(cudaStreamSynchronize(0));
+    }
+    return EFM_OK;
+}
+
+int efm_result_copy_sparse(const efm_handle* hc, int32_t* nnz, int32_t* rxn, int64_t* val, int64_t capacity_rows) {
+    efm_handle* h = const_cast<efm_handle*>(hc);
+    if (!h) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    if (capacity_rows < h->n_out) return EFM_E_INVAL;
+    if (h->n_out == 0) return EFM_OK;
+    CK(cudaSetDevice(h->device));
+    const size_t K = (size_t)h->n_out;
+    if (nnz) CK(cudaMemcpy(nnz, h->ws + h->lay.r_nnz.off, K * 4, cudaMemcpyDeviceToHost));
+    if (rxn) CK(cudaMemcpy(rxn, h->ws + h->lay.r_rxn.off, K * h->D * 4, cudaMemcpyDeviceToHost));
+    if (val) CK(cudaMemcpy(val, h->ws + h->lay.r_val.off, K * h->D * 8, cudaMemcpyDeviceToHost));
+    return EFM_OK;
+}
+
+int efm_get_stats(const efm_handle* h, efm_stats* st) {
+    if (!h || !st) return EFM_E_INVAL;
+    *st = h->stats;
+    return EFM_OK;
+}
+
+int efm_get_level_stats(const efm_handle* h, int64_t* active, int64_t* done, int64_t* expanded, int64_t* children,
+                        int64_t capacity, int64_t* n_levels) {
+    if (!h || !n_levels) return EFM_E_INVAL;
+    const int64_t nl = (int64_t)h->lvl_active.size();
+    *n_levels = nl;
+    for (int64_t i = 0; i < std::min(nl, capacity); ++i) {
+        if (active) active[i] = h->lvl_active[i];
+        if (done) done[i] = h->lvl_done[i];
+        if (expanded) expanded[i] = h->lvl_expanded[i];
+        if (children) children[i] = h->lvl_children[i];
+    }
+    return EFM_OK;
+}
+
+int efm_debug_state_hash(int32_t device, int32_t n_supp, const int32_t* arc, const int64_t* flux, int32_t n_vis,
+                         const int32_t* vis4, uint64_t* hash_out) {
+    if (n_supp < 0 || n_vis < 0 || !hash_out || (n_supp && (!arc || !flux)) || (n_vis && !vis4)) return EFM_E_INVAL;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return EFM_E_CUDA; }
+    // pinned, device-mapped host staging: the library never allocates device memory
+    const size_t bytes = 16 + (size_t)n_supp * 12 + (size_t)n_vis * 16 + 64;
+    unsigned char* p = nullptr;
+    if (cudaHostAlloc((void**)&p, bytes, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); return EFM_E_CUDA; }
+    u64* out = (u64*)p;
+    i64* f = (i64*)(p + 16);
+    int* a = (int*)(f + n_supp);
+    int* v = a + n_supp;
+    for (int t = 0; t < n_supp; ++t) { f[t] = flux[t]; a[t] = arc[t]; }
+    for (int t = 0; t < 4 * n_vis; ++t) v[t] = vis4[t];
+    cudaError_t e = launch_debug_hash(n_supp, a, f, n_vis, v, out, 0);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+    if (e == cudaSuccess) *hash_out = *out;
+    cudaFreeHost(p);
+    if (e != cudaSuccess) { cudaGetLastError(); return EFM_E_CUDA; }
+    return EFM_OK;
+}
+
+void efm_destroy(efm_handle* h) {
+    if (!h) return;
+    for (cudaEvent_t e : h->events) cudaEventDestroy(e);
+    if (h->h_ctl) cudaFreeHost(h->h_ctl);
+    delete h;
+}
+
+}  // extern "C"

@@ -1,0 +1,102 @@
+// Types shared by the kernels and the host driver.  Notation follows the paper: M internal metabolites (nodes),
+// I / O input / output reaction arrays of a node, c coefficient, f flux, EF extra flux (Eq 2),
+// PI / PO primary input / output (Def 10).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace efm {
+
+typedef unsigned long long u64;
+typedef long long i64;
+typedef unsigned int u32;
+typedef unsigned short u16;
+
+// ---------------------------------------------------------------------------------------------------------------
+// Entry format in HBM.  A frontier slot is `stride` bytes; the entry occupies a prefix:
+//   [ 0,16)  header: u32 n_supp | n_vis << 16, 12 spare bytes
+//   i64  flux[n_supp]   fluxes of the support arcs, > 0, gcd 1
+//   u64  vis[n_vis]     visited records: cnt << 48 | met << 32 | PI << 16 | PO   (unordered)
+//   u16  arc[n_supp]    support arcs, ascending arc id
+// A candidate slot holds the same with n_vis = 0.
+// ---------------------------------------------------------------------------------------------------------------
+__host__ __device__ inline u32 entry_bytes(u32 n_supp, u32 n_vis) {
+    return (16u + 8u * n_supp + 8u * n_vis + 2u * n_supp + 15u) & ~15u;
+}
+// irreducible content of an entry, the unit of the algorithmic-byte count
+__host__ __device__ inline u32 algo_entry_bytes(u32 n_supp, u32 n_vis) { return n_supp * 10u + n_vis * 7u + 16u; }
+
+struct DevGraph {
+    int M, A, W32, M32;
+    const int* col_ptr;   const int2* col;    // {met, s}
+    const int* in_ptr;    const int2* in_e;   // {arc, c}
+    const int* out_ptr;   const int2* out_e;
+    const int* twin;
+    const i64* dep_off;   const u32* dep_bits;
+    const int* arc_rxn;   const int* arc_dir;
+};
+
+// Device-resident control block: per-level counters, beam-select state, cumulative statistics.
+enum { ST_EXPANDED = 0, ST_CHILDREN, ST_DONE, ST_DEAD_END, ST_NOT_EFM, ST_NONPOS, ST_OVERFLOW, ST_VISITED,
+       ST_ALGO_BYTES, ST_COUNT };
+enum { ERR_FRONTIER = 1, ERR_CAND = 2, ERR_KEYS = 4 };
+enum { SEL_BINS = 2048 };
+
+struct Ctl {
+    // per level (reset by k_level_begin)
+    u64 n_next;        // active survivors written to the next frontier buffer
+    u64 n_keys;        // active children generated (= keys written by the count pass)
+    u64 lvl_done;      // balanced children generated
+    u64 lvl_children;  // children generated (active + done)
+    u64 lvl_expanded;  // parents expanded
+    // persistent
+    u64 n_cand;        // candidates emitted so far
+    u32 error;
+    u32 notrunc;       // beam does not bind on this level
+    u64 X;             // beam threshold: keep key < X
+    u64 sel_prefix, sel_rank;
+    u32 sel_ticket, pad0;
+    u64 st[ST_COUNT];
+    // post-processing counters
+    u64 n_unique, n_poisoned, n_uniq_ok, n_keep, filter_pairs;
+    // everything above is read back by the host once per level; the histogram stays on the device
+    u32 hist[SEL_BINS];
+};
+
+struct ExpandArgs {
+    DevGraph g;
+    const unsigned char* cur;   // parents
+    unsigned char* nxt;         // children that stay active
+    unsigned char* cand;        // balanced children
+    u64* keys;                  // beam keys of the active children (count pass)
+    Ctl* ctl;
+    u64 n_cur;
+    u32 stride, cand_stride;
+    u64 max_frontier, max_cand, max_keys;
+    int D, V, max_loop;
+    int count_algo_children;    // 0 for the root level (roots are not written by an expansion)
+    // shared-memory carve-up per group (bytes)
+    u32 sm_group, sm_EF, sm_sbits, sm_mseen;
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// SURVEY.md 8(c)-B state hash: written here from the formula, independently of oracle/.
+//   mix = SplitMix64 finaliser
+//   h = mix( sum_{a in supp} mix( mix(0x01<<56 | a) + f_a ) + sum_{i visited} mix(0x02<<56 | cnt<<48 | i<<32 | PI<<16 | PO) )
+//   key = min(n_unb, 255) << 56 | h >> 8
+// ---------------------------------------------------------------------------------------------------------------
+__host__ __device__ inline u64 mix64(u64 x) {
+    x ^= x >> 30; x *= 0xBF58476D1CE4E5B9ULL;
+    x ^= x >> 27; x *= 0x94D049BB133111EBULL;
+    x ^= x >> 31; return x;
+}
+__host__ __device__ inline u64 arc_term(u32 a, u64 f) { return mix64(mix64(0x0100000000000000ULL | (u64)a) + f); }
+__host__ __device__ inline u64 vis_term(u64 rec) { return mix64(0x0200000000000000ULL | rec); }
+__host__ __device__ inline u64 vis_pack(u32 met, u32 PI, u32 PO, u32 cnt) {
+    return ((u64)cnt << 48) | ((u64)met << 32) | ((u64)PI << 16) | (u64)PO;
+}
+__host__ __device__ inline u64 beam_key(u32 n_unb, u64 h) { return ((u64)(n_unb > 255u ? 255u : n_unb) << 56) | (h >> 8); }
+
+#define EFM_GUARD (1ULL << 62)   // reading G21: any state integer above 2^62 discards the pathway
+
+}  // namespace efm

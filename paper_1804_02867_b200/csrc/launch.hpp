@@ -1,0 +1,38 @@
+// Host-callable launchers of the kernels in expand.cu and post.cu.
+#pragma once
+#include "device_common.cuh"
+
+namespace efm {
+
+// expand.cu
+void expand_smem_layout(ExpandArgs& a);
+cudaError_t launch_expand(int mode /*0 count, 1 write, 2 direct*/, bool roots, const ExpandArgs& a, int sm_count, cudaStream_t s);
+cudaError_t launch_level_begin(Ctl* ctl, cudaStream_t s);
+
+// post.cu
+struct PostArgs {
+    DevGraph g;
+    Ctl* ctl;
+    const unsigned char* cand; u32 cand_stride; u64 max_cand;
+    u32* table; u64 table_size;        // open-addressing support hash (a-6), power of two
+    unsigned char* isrep; unsigned char* poison;
+    u32* uniq;                         // candidate ids of the unique, unpoisoned supports
+    // minimality filter (a-7)
+    u32* size_hist; u32* bucket_start; u32* bucket_fill; int n_size_bins;
+    u32* order; ulonglong2* sig; u16* size_sorted; unsigned char* keep;
+    // canonical output (a-8)
+    int D; int n_rxn;
+    int* u_nnz; int* u_rxn; i64* u_val;   // unsorted reaction-space rows
+    u32* sort_idx; u64 n_pad;
+    int* r_nnz; int* r_rxn; i64* r_val;   // final, lexicographic order
+};
+cudaError_t launch_select(const u64* keys, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches);
+cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_launches);
+cudaError_t launch_filter(const PostArgs& a, u64 n_uniq, int sm_count, cudaStream_t s, int* n_launches);
+cudaError_t launch_output_rows(const PostArgs& a, u64 n_uniq, cudaStream_t s, int* n_launches);
+cudaError_t launch_output_sort(const PostArgs& a, u64 n_keep, cudaStream_t s, int* n_launches);
+cudaError_t launch_densify(const int* r_nnz, const int* r_rxn, const i64* r_val, int D, int n_rxn, i64 row0, i64 n_rows,
+                           i64* d_out, cudaStream_t s);
+cudaError_t launch_debug_hash(int n_supp, const int* arc, const i64* flux, int n_vis, const int* vis4, u64* out, cudaStream_t s);
+
+}  // namespace efm

@@ -1,0 +1,368 @@
+// Beam threshold selection (a-4), candidate support dedup (a-6), minimality filter (a-7) and canonical output (a-8).
+#include "device_common.cuh"
+#include "launch.hpp"
+
+namespace efm {
+
+// =================================================================================================================
+// a-4  Beam select: X = the key at sorted position `cap`; the level keeps exactly {key < X}.
+// MSD radix select over the 64-bit keys, 11/11/11/11/10/10-bit digits, shared-memory histograms; the last block
+// of a round (ticket) scans the global histogram and narrows the prefix.  No host round trip.
+// =================================================================================================================
+__global__ void k_select_init(Ctl* ctl, u64 cap) {
+    const u64 n = ctl->n_keys;
+    ctl->notrunc = (cap == 0 || n <= cap) ? 1u : 0u;
+    ctl->sel_prefix = 0; ctl->sel_rank = cap; ctl->sel_ticket = 0; ctl->X = 0;
+}
+
+__global__ void __launch_bounds__(256) k_select_round(const u64* __restrict__ keys, Ctl* ctl, u64 max_keys, int shift, int bits, int first, int last) {
+    if (ctl->notrunc) return;
+    __shared__ u32 h[SEL_BINS];
+    __shared__ bool is_last;
+    const int nb = 1 << bits;
+    for (int b = threadIdx.x; b < nb; b += blockDim.x) h[b] = 0;
+    __syncthreads();
+    const u64 n = min(ctl->n_keys, max_keys);   // an overflowed key array is reported by the host (ERR_KEYS)
+    const u64 prefix = ctl->sel_prefix;
+    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
+        const u64 key = keys[i];
+        if (first || (key >> (shift + bits)) == prefix) atomicAdd(&h[(key >> shift) & (u64)(nb - 1)], 1u);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nb; b += blockDim.x) if (h[b]) atomicAdd(&ctl->hist[b], h[b]);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) is_last = atomicAdd(&ctl->sel_ticket, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    if (threadIdx.x == 0) {
+        volatile u32* gh = ctl->hist;
+        u64 rank = ctl->sel_rank, cum = 0;
+        int b = 0;
+        for (; b < nb; ++b) { const u64 c = gh[b]; if (rank < cum + c) break; cum += c; }
+        if (b == nb) b = nb - 1;   // unreachable while n_keys > cap
+        ctl->sel_rank = rank - cum;
+        const u64 np = (prefix << bits) | (u64)b;
+        ctl->sel_prefix = np;
+        ctl->sel_ticket = 0;
+        if (last) ctl->X = np;
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nb; b += blockDim.x) ctl->hist[b] = 0;
+}
+
+cudaError_t launch_select(const u64* keys, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches) {
+    k_select_init<<<1, 1, 0, s>>>(ctl, cap);
+    ++*n_launches;
+    if (cap == 0) return cudaGetLastError();
+    static const int bits[6] = {11, 11, 11, 11, 10, 10};
+    int shift = 64;
+    u64 blocks = (n_keys_hint + 256 * 8 - 1) / (256 * 8);
+    if (blocks > (u64)sm_count * 8) blocks = (u64)sm_count * 8;
+    if (blocks < 1) blocks = 1;
+    for (int r = 0; r < 6; ++r) {
+        shift -= bits[r];
+        k_select_round<<<(unsigned)blocks, 256, 0, s>>>(keys, ctl, max_keys, shift, bits[r], r == 0, r == 5);
+        ++*n_launches;
+    }
+    return cudaGetLastError();
+}
+
+// =================================================================================================================
+// a-6  Candidate dedup: open-addressing hash keyed on the arc-space support (the sorted arc list is the bitset in
+// sparse form).  The first candidate to claim a slot represents its support; a later candidate with the same support
+// and a different coprime flux vector poisons it (reading G18) -- order-independent.
+// =================================================================================================================
+__device__ __forceinline__ const i64* cand_flux(const unsigned char* e) { return (const i64*)(e + 16); }
+__device__ __forceinline__ int cand_n(const unsigned char* e) { return (int)(*(const u32*)e & 0xffffu); }
+__device__ __forceinline__ const u16* cand_arc(const unsigned char* e, int n) { return (const u16*)(e + 16 + 8 * (size_t)n); }
+
+__global__ void __launch_bounds__(256) k_dedup_insert(const PostArgs a, u64 n_cand) {
+    const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_cand) return;
+    const unsigned char* e = a.cand + i * a.cand_stride;
+    const int n = cand_n(e);
+    const u16* arc = cand_arc(e, n);
+    const i64* f = cand_flux(e);
+    u64 h = 0;
+    for (int t = 0; t < n; ++t) h += mix64(0x0300000000000000ULL | (u64)arc[t]);
+    u64 slot = mix64(h) & (a.table_size - 1);
+    for (;;) {
+        const u32 prev = atomicCAS(&a.table[slot], 0xFFFFFFFFu, (u32)i);
+        if (prev == 0xFFFFFFFFu) { a.isrep[i] = 1; return; }
+        const unsigned char* o = a.cand + (u64)prev * a.cand_stride;
+        const int no = cand_n(o);
+        if (no == n) {
+            const u16* oarc = cand_arc(o, no);
+            bool same = true;
+            for (int t = 0; t < n && same; ++t) same = arc[t] == oarc[t];
+            if (same) {
+                const i64* of = cand_flux(o);
+                bool eq = true;
+                for (int t = 0; t < n && eq; ++t) eq = f[t] == of[t];
+                if (!eq) a.poison[prev] = 1;
+                return;
+            }
+        }
+        slot = (slot + 1) & (a.table_size - 1);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_dedup_collect(const PostArgs a, u64 n_cand) {
+    const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_cand || !a.isrep[i]) return;
+    atomicAdd(&a.ctl->n_unique, 1ULL);
+    if (a.poison[i]) { atomicAdd(&a.ctl->n_poisoned, 1ULL); return; }
+    const u64 pos = atomicAdd(&a.ctl->n_uniq_ok, 1ULL);
+    a.uniq[pos] = (u32)i;
+}
+
+cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_launches) {
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(a.table, 0xFF, a.table_size * sizeof(u32), s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(a.isrep, 0, n_cand + 1, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(a.poison, 0, n_cand + 1, s)) != cudaSuccess) return e;
+    if (n_cand == 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)((n_cand + 255) / 256);
+    k_dedup_insert<<<blocks, 256, 0, s>>>(a, n_cand);
+    k_dedup_collect<<<blocks, 256, 0, s>>>(a, n_cand);
+    *n_launches += 2;
+    return cudaGetLastError();
+}
+
+// =================================================================================================================
+// a-7  Minimality filter (Def 3; reading G17): drop v if some other unique support w
+// is a strict subset.  Rows are counting-sorted by popcount so that only smaller supports are tested against v;
+// the pair test runs on 128-bit signatures (exact bitsets when A <= 128, a 128-bucket image of the arc set
+// otherwise) staged tile by tile through shared memory; signature hits are verified on the sorted arc lists.
+// =================================================================================================================
+__device__ __forceinline__ u32 sig_bit(int arc, bool exact) { return exact ? (u32)arc : ((u32)arc * 0x9E3779B1u) >> 25; }
+
+__global__ void __launch_bounds__(256) k_filter_sizes(const PostArgs a, u64 K) {
+    const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= K) return;
+    const unsigned char* e = a.cand + (u64)a.uniq[u] * a.cand_stride;
+    atomicAdd(&a.size_hist[cand_n(e)], 1u);
+}
+__global__ void k_filter_scan(const PostArgs a) {   // exclusive scan over the popcount bins (at most D+2 of them)
+    u32 acc = 0;
+    for (int b = 0; b < a.n_size_bins; ++b) { a.bucket_start[b] = acc; a.bucket_fill[b] = acc; acc += a.size_hist[b]; }
+}
+__global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K) {
+    const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= K) return;
+    const u32 id = a.uniq[u];
+    const unsigned char* e = a.cand + (u64)id * a.cand_stride;
+    const int n = cand_n(e);
+    const u16* arc = cand_arc(e, n);
+    const bool exact = a.g.A <= 128;
+    u64 lo = 0, hi = 0;
+    for (int t = 0; t < n; ++t) {
+        const u32 b = sig_bit(arc[t], exact);
+        if (b < 64) lo |= 1ULL << b; else hi |= 1ULL << (b - 64);
+    }
+    const u32 pos = atomicAdd(&a.bucket_fill[n], 1u);
+    a.order[pos] = id;
+    a.sig[pos] = make_ulonglong2(lo, hi);
+    a.size_sorted[pos] = (u16)n;
+}
+__device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   // supp(w) subset of supp(v), sorted lists
+    const int nw = cand_n(w), nv = cand_n(v);
+    const u16* aw = cand_arc(w, nw);
+    const u16* av = cand_arc(v, nv);
+    int j = 0;
+    for (int t = 0; t < nw; ++t) {
+        while (j < nv && av[j] < aw[t]) ++j;
+        if (j == nv || av[j] != aw[t]) return false;
+        ++j;
+    }
+    return true;
+}
+constexpr int kFilterTile = 256;
+__global__ void __launch_bounds__(kFilterTile) k_filter(const PostArgs a, u64 K) {
+    __shared__ ulonglong2 wsig[kFilterTile];
+    __shared__ u32 blimit;
+    const u64 p = (u64)blockIdx.x * kFilterTile + threadIdx.x;
+    const bool valid = p < K;
+    ulonglong2 v = make_ulonglong2(0, 0);
+    u32 limit = 0;
+    if (valid) { v = a.sig[p]; limit = a.bucket_start[a.size_sorted[p]]; }   // rows with a strictly smaller support
+    // sizes ascend with p: the last valid row of the block has the largest limit
+    const u64 lastp = min((u64)blockIdx.x * kFilterTile + kFilterTile - 1, K - 1);
+    if (threadIdx.x == 0) blimit = a.bucket_start[a.size_sorted[lastp]];
+    __syncthreads();
+    const u32 bl = blimit;
+    const bool exact = a.g.A <= 128;
+    bool keep = true;
+    const u64 nvx = ~v.x, nvy = ~v.y;
+    for (u32 base = 0; base < bl; base += kFilterTile) {
+        if (base + threadIdx.x < bl) wsig[threadIdx.x] = a.sig[base + threadIdx.x];
+        __syncthreads();
+        if (keep && base < limit) {
+            const int jn = (int)min((u32)kFilterTile, limit - base);
+#pragma unroll 4
+            for (int j = 0; j < jn; ++j) {
+                const ulonglong2 w = wsig[j];
+                if (((w.x & nvx) | (w.y & nvy)) == 0) {
+                    if (exact || arcs_subset(a.cand + (u64)a.order[base + j] * a.cand_stride, a.cand + (u64)a.order[p] * a.cand_stride)) {
+                        keep = false;
+                        break;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+    if (valid) {
+        a.keep[p] = keep ? 1 : 0;
+        atomicAdd(&a.ctl->filter_pairs, (u64)limit);
+    }
+}
+
+cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s, int* n_launches) {
+    (void)sm_count;
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(a.size_hist, 0, sizeof(u32) * a.n_size_bins, s)) != cudaSuccess) return e;
+    if (K == 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)((K + 255) / 256);
+    k_filter_sizes<<<blocks, 256, 0, s>>>(a, K);
+    k_filter_scan<<<1, 1, 0, s>>>(a);
+    k_filter_scatter<<<blocks, 256, 0, s>>>(a, K);
+    k_filter<<<(unsigned)((K + kFilterTile - 1) / kFilterTile), kFilterTile, 0, s>>>(a, K);
+    *n_launches += 4;
+    return cudaGetLastError();
+}
+
+// =================================================================================================================
+// a-8  Canonical output: arc space -> reaction space (v_j = f_j+ - f_j-), lexicographic order of the dense signed
+// vectors, computed on the sparse rows with a bitonic sort of row indices.
+// =================================================================================================================
+__global__ void __launch_bounds__(256) k_out_rows(const PostArgs a, u64 K) {
+    const u64 p = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= K || !a.keep[p]) return;
+    const u64 r = atomicAdd(&a.ctl->n_keep, 1ULL);
+    const unsigned char* e = a.cand + (u64)a.order[p] * a.cand_stride;
+    const int n = cand_n(e);
+    const u16* arc = cand_arc(e, n);
+    const i64* f = cand_flux(e);
+    a.u_nnz[r] = n;
+    for (int t = 0; t < n; ++t) {   // arcs ascend => reactions ascend (twins never share a support)
+        a.u_rxn[r * a.D + t] = a.g.arc_rxn[arc[t]];
+        a.u_val[r * a.D + t] = a.g.arc_dir[arc[t]] < 0 ? -f[t] : f[t];
+    }
+}
+
+// strict lexicographic "row x < row y" on the dense vectors, evaluated on the sparse rows
+__device__ bool row_less(const PostArgs& a, u32 x, u32 y) {
+    if (x == 0xFFFFFFFFu) return false;   // padding sorts last
+    if (y == 0xFFFFFFFFu) return true;
+    const int nx = a.u_nnz[x], ny = a.u_nnz[y];
+    const int* jx = a.u_rxn + (u64)x * a.D; const int* jy = a.u_rxn + (u64)y * a.D;
+    const i64* vx = a.u_val + (u64)x * a.D; const i64* vy = a.u_val + (u64)y * a.D;
+    int tx = 0, ty = 0;
+    for (;;) {
+        if (tx == nx && ty == ny) return false;
+        const int cx = tx < nx ? jx[tx] : 0x7fffffff, cy = ty < ny ? jy[ty] : 0x7fffffff;
+        if (cx == cy) { if (vx[tx] != vy[ty]) return vx[tx] < vy[ty]; ++tx; ++ty; }
+        else if (cx < cy) return vx[tx] < 0;   // y is 0 at reaction cx
+        else return 0 < vy[ty];                // x is 0 at reaction cy
+    }
+}
+__global__ void __launch_bounds__(256) k_sort_init(const PostArgs a, u64 n_keep) {
+    const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < a.n_pad) a.sort_idx[i] = i < n_keep ? (u32)i : 0xFFFFFFFFu;
+}
+__global__ void __launch_bounds__(256) k_bitonic_global(const PostArgs a, u64 j, u64 k) {
+    const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= a.n_pad) return;
+    const u64 ixj = i ^ j;
+    if (ixj <= i) return;
+    const bool asc = (i & k) == 0;
+    const u32 x = a.sort_idx[i], y = a.sort_idx[ixj];
+    if (asc ? row_less(a, y, x) : row_less(a, x, y)) { a.sort_idx[i] = y; a.sort_idx[ixj] = x; }
+}
+constexpr int kSortChunk = 1024;
+// all compare-exchange steps with j < kSortChunk of the stages k in [k_lo, k_hi] on one shared-memory chunk
+__global__ void __launch_bounds__(kSortChunk / 2) k_bitonic_local(const PostArgs a, u64 k_lo, u64 k_hi) {
+    __shared__ u32 s[kSortChunk];
+    const u64 base = (u64)blockIdx.x * kSortChunk;
+    for (int t = threadIdx.x; t < kSortChunk; t += blockDim.x) s[t] = base + t < a.n_pad ? a.sort_idx[base + t] : 0xFFFFFFFFu;
+    __syncthreads();
+    for (u64 k = k_lo; k <= k_hi; k <<= 1) {
+        for (u64 j = min(k >> 1, (u64)kSortChunk >> 1); j > 0; j >>= 1) {
+            const int t = threadIdx.x;
+            const int i = (int)(((t & ~((int)j - 1)) << 1) | (t & ((int)j - 1)));   // lower index of the pair
+            const int ixj = i | (int)j;
+            const bool asc = ((base + i) & k) == 0;
+            const u32 x = s[i], y = s[ixj];
+            if (asc ? row_less(a, y, x) : row_less(a, x, y)) { s[i] = y; s[ixj] = x; }
+            __syncthreads();
+        }
+    }
+    for (int t = threadIdx.x; t < kSortChunk; t += blockDim.x) if (base + t < a.n_pad) a.sort_idx[base + t] = s[t];
+}
+__global__ void __launch_bounds__(256) k_out_gather(const PostArgs a, u64 n_keep) {
+    const u64 r = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_keep) return;
+    const u32 src = a.sort_idx[r];
+    const int n = a.u_nnz[src];
+    a.r_nnz[r] = n;
+    for (int t = 0; t < n; ++t) { a.r_rxn[r * a.D + t] = a.u_rxn[(u64)src * a.D + t]; a.r_val[r * a.D + t] = a.u_val[(u64)src * a.D + t]; }
+}
+
+cudaError_t launch_output_rows(const PostArgs& a, u64 K, cudaStream_t s, int* n_launches) {
+    if (K == 0) return cudaSuccess;
+    k_out_rows<<<(unsigned)((K + 255) / 256), 256, 0, s>>>(a, K);
+    ++*n_launches;
+    return cudaGetLastError();
+}
+cudaError_t launch_output_sort(const PostArgs& a, u64 n_keep, cudaStream_t s, int* n_launches) {
+    if (n_keep == 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)((a.n_pad + 255) / 256);
+    k_sort_init<<<blocks, 256, 0, s>>>(a, n_keep);
+    ++*n_launches;
+    const unsigned chunks = (unsigned)((a.n_pad + kSortChunk - 1) / kSortChunk);
+    const u64 k_local_hi = a.n_pad < (u64)kSortChunk ? a.n_pad : (u64)kSortChunk;
+    k_bitonic_local<<<chunks, kSortChunk / 2, 0, s>>>(a, 2, k_local_hi);
+    ++*n_launches;
+    for (u64 k = (u64)kSortChunk * 2; k <= a.n_pad; k <<= 1) {
+        for (u64 j = k >> 1; j >= (u64)kSortChunk; j >>= 1) { k_bitonic_global<<<blocks, 256, 0, s>>>(a, j, k); ++*n_launches; }
+        k_bitonic_local<<<chunks, kSortChunk / 2, 0, s>>>(a, k, k);
+        ++*n_launches;
+    }
+    k_out_gather<<<(unsigned)((n_keep + 255) / 256), 256, 0, s>>>(a, n_keep);
+    ++*n_launches;
+    return cudaGetLastError();
+}
+
+__global__ void __launch_bounds__(256) k_densify(const int* r_nnz, const int* r_rxn, const i64* r_val, int D, int n_rxn,
+                                                 i64 row0, i64 n_rows, i64* out) {
+    const i64 r = (i64)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
+    if (r >= n_rows) return;
+    const int lane = threadIdx.x & 31;
+    const i64 src = row0 + r;
+    const int n = r_nnz[src];
+    for (int t = lane; t < n; t += 32) out[r * n_rxn + r_rxn[src * D + t]] = r_val[src * D + t];
+}
+cudaError_t launch_densify(const int* r_nnz, const int* r_rxn, const i64* r_val, int D, int n_rxn, i64 row0, i64 n_rows,
+                           i64* d_out, cudaStream_t s) {
+    if (n_rows <= 0) return cudaSuccess;
+    cudaError_t e = cudaMemsetAsync(d_out, 0, (size_t)n_rows * n_rxn * sizeof(i64), s);
+    if (e != cudaSuccess) return e;
+    k_densify<<<(unsigned)((n_rows + 7) / 8), 256, 0, s>>>(r_nnz, r_rxn, r_val, D, n_rxn, row0, n_rows, d_out);
+    return cudaGetLastError();
+}
+
+__global__ void k_debug_hash(int n_supp, const int* arc, const i64* flux, int n_vis, const int* vis4, u64* out) {
+    u64 s = 0;
+    for (int t = 0; t < n_supp; ++t) s += arc_term((u32)arc[t], (u64)flux[t]);
+    for (int u = 0; u < n_vis; ++u) s += vis_term(vis_pack((u32)vis4[4 * u], (u32)vis4[4 * u + 1], (u32)vis4[4 * u + 2], (u32)vis4[4 * u + 3]));
+    *out = mix64(s);
+}
+cudaError_t launch_debug_hash(int n_supp, const int* arc, const i64* flux, int n_vis, const int* vis4, u64* out, cudaStream_t s) {
+    k_debug_hash<<<1, 1, 0, s>>>(n_supp, arc, flux, n_vis, vis4, out);
+    return cudaGetLastError();
+}
+
+}  // namespace efm

@@ -1,0 +1,194 @@
+"""GPU <-> oracle parity (bit-exact): the CUDA path, called through the C ABI, must return the same set of pathways
+as the CPU oracle -- same coprime integer flux vectors in the same canonical order -- and the same counters
+(every discard reason, per-level frontier sizes, beam truncation, unique supports, algorithmic bytes)."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from netgen import hand_network, make_network, unimolecular_network
+
+pytestmark = pytest.mark.gpu
+
+STAT_KEYS = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxloop", "discarded_nonpos",
+             "discarded_overflow", "discarded_visited", "truncated_beam", "unique_supports", "poisoned", "output",
+             "peak_frontier", "algo_bytes"]
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "hand_pins.json")
+
+
+@pytest.fixture(scope="module")
+def efm():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_1804_02867_b200 import build
+    build.build()
+    import paper_1804_02867_b200 as mod
+    mod.load()
+    return mod
+
+
+def _threads(oracle_mod):
+    return max(1, min(oracle_mod.max_threads(), os.cpu_count() or 1, 64))
+
+
+def assert_parity(efm, oracle_mod, net, seeds="net", flags=0, check_levels=True, **over):
+    got = efm.enumerate_network(net, seed_sets=seeds, flags=flags, **over)
+    okeys = {k: v for k, v in over.items() if k in ("max_support", "max_loop", "dep_depth", "max_visited", "frontier_cap")}
+    ref = oracle_mod.enumerate_network(net, threads=_threads(oracle_mod), seed_sets=seeds, self_check=False, **okeys)
+    for k in STAT_KEYS:
+        assert int(got.stats[k]) == int(ref.stats[k]), (k, got.stats[k], ref.stats[k])
+    if check_levels:
+        for k in ("active", "done", "expanded", "children"):
+            assert np.array_equal(got.levels[k], ref.levels[k]), k
+    assert got.flux.shape == ref.flux.shape
+    assert np.array_equal(got.flux, ref.flux)
+    assert int(got.stats["n_roots"]) == ref.n_roots
+    return got, ref
+
+
+def test_hash_matches_oracle_hash(efm, oracle_mod):
+    cases = [([11], [6], []), ([11], [6], [(5, 11, 12, 3)]), ([3, 9, 4], [2, 5, 1], [(1, 3, 9, 0), (7, 4, 9, 2)]),
+             ([0, 65535], [1 << 61, 1], [(65535, 65535, 0, 8)])]
+    for arcs, flux, vis in cases:
+        assert efm.debug_state_hash(arcs, flux, vis) == oracle_mod.state_hash(arcs, flux, vis)
+
+
+def _golden_cases():
+    with open(GOLDEN) as fh:
+        return json.load(fh)["cases"]
+
+
+@pytest.mark.parametrize("case", _golden_cases(), ids=lambda c: c["name"])
+def test_hand_pins_on_gpu(efm, case):
+    """The hand-derived fixtures of tests/golden pin the CUDA path directly (no oracle involved)."""
+    net = hand_network([(s, p, r) for s, p, r in case["reactions"]], case["internal"])
+    got = efm.enumerate_network(net, seed_sets=case["seeds"])
+    assert got.flux.tolist() == case["flux"]
+    for k in ("expanded", "levels", "discarded_nonpos"):
+        if k in case:
+            assert int(got.stats[k]) == case[k], k
+
+
+@pytest.mark.parametrize("two_pass", [False, True])
+def test_toy(efm, oracle_mod, two_pass):
+    net = make_network("toy", 0)
+    flags = efm.EFM_F_FORCE_TWO_PASS if two_pass else 0
+    over = dict(frontier_cap=1 << 20) if two_pass else {}
+    assert_parity(efm, oracle_mod, net, flags=flags, **over)
+    assert_parity(efm, oracle_mod, net, seeds=oracle_mod.all_arc_seed_sets(net.reversible), flags=flags, **over)
+
+
+def test_small(efm, oracle_mod):
+    net = make_network("small", 0)
+    got, _ = assert_parity(efm, oracle_mod, net)
+    assert got.stats["direct_levels"] > 0 and got.stats["two_pass_levels"] == 0
+    got, _ = assert_parity(efm, oracle_mod, net, flags=efm.EFM_F_FORCE_TWO_PASS, frontier_cap=1 << 20)
+    assert got.stats["two_pass_levels"] > 0 and got.stats["truncated_beam"] == 0
+
+
+@pytest.mark.parametrize("cap", [300, 1000, 3918, 3919])
+def test_small_beam(efm, oracle_mod, cap):
+    """The beam binds (or just does not, at the peak frontier 3919): threshold selection must agree exactly."""
+    net = make_network("small", 0)
+    got, ref = assert_parity(efm, oracle_mod, net, frontier_cap=cap)
+    assert (got.stats["truncated_beam"] > 0) == (cap < 3919)
+
+
+def test_unimolecular_networks(efm, oracle_mod):
+    for seed in range(12):
+        net = unimolecular_network(seed, m_int=4 + seed % 4, n_rxn=7 + seed % 6, n_rev=seed % 3)
+        assert_parity(efm, oracle_mod, net, seeds=oracle_mod.all_arc_seed_sets(net.reversible))
+
+
+def test_core_full(efm, oracle_mod):
+    net = make_network("core", 0)
+    assert_parity(efm, oracle_mod, net)
+
+
+@pytest.mark.parametrize("cap", [2048, 65536])
+def test_core_beam(efm, oracle_mod, cap):
+    net = make_network("core", 0)
+    got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=cap)
+    assert got.stats["truncated_beam"] > 0
+
+
+@pytest.mark.parametrize("cap", [512, 16384])
+def test_mid(efm, oracle_mod, cap):
+    net = make_network("mid", 0)
+    got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=cap)
+    assert got.stats["truncated_beam"] > 0
+
+
+@pytest.mark.parametrize("cap", [256, 4096])
+def test_genome(efm, oracle_mod, cap):
+    net = make_network("genome", 0)
+    got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=cap)
+    assert got.stats["truncated_beam"] > 0 and got.stats["output"] > 1000
+
+
+def test_other_seeds_of_the_generator(efm, oracle_mod):
+    for name, seed, over in (("small", 1, {}), ("small", 2, dict(frontier_cap=500)), ("core", 1, dict(frontier_cap=4096)),
+                             ("mid", 3, dict(frontier_cap=1024))):
+        assert_parity(efm, oracle_mod, make_network(name, seed), **over)
+
+
+def test_parameter_edges(efm, oracle_mod):
+    net = make_network("small", 0)
+    assert_parity(efm, oracle_mod, net, max_loop=1)
+    assert_parity(efm, oracle_mod, net, max_support=6)
+    assert_parity(efm, oracle_mod, net, max_visited=3)
+    assert_parity(efm, oracle_mod, net, dep_depth=1)
+    assert_parity(efm, oracle_mod, net, frontier_cap=1)
+    assert_parity(efm, oracle_mod, net, frontier_cap=2, seeds=oracle_mod.all_arc_seed_sets(net.reversible))
+
+
+def test_overflow_guard(efm, oracle_mod):
+    """Coefficient chains that multiply the scale past 2^62 (reading G21): both sides must discard identically."""
+    names = [f"A{t}" for t in range(48)]
+    rx = [({}, {names[0]: 1}, False)]
+    for t in range(47):
+        rx.append(({names[t]: 3}, {names[t + 1]: 1}, False))
+    rx.append(({names[47]: 1}, {}, False))
+    net = hand_network(rx, names)
+    got, ref = assert_parity(efm, oracle_mod, net, seeds=[[0]])
+    assert ref.stats["discarded_overflow"] > 0
+    rx2 = [({}, {names[0]: 1}, False)]
+    for t in range(30):
+        rx2.append(({names[t]: 3}, {names[t + 1]: 2}, False))
+    rx2.append(({names[30]: 1}, {}, False))
+    got, ref = assert_parity(efm, oracle_mod, hand_network(rx2, names[:31]), seeds=[[0]])
+    assert ref.stats["output"] == 1 and int(abs(ref.flux).max()) == 3 ** 30
+
+
+def test_degenerate_inputs(efm, oracle_mod):
+    # a seed that is balanced at once (all-external reaction) and a network without any internal metabolite
+    net = hand_network([({"X": 1}, {"Y": 1}, False), ({}, {"A": 1}, False), ({"A": 1}, {}, False)], ["A"])
+    assert_parity(efm, oracle_mod, net, seeds=[[0], [2]])
+    net0 = hand_network([({"X": 1}, {"Y": 2}, True)], [])
+    got = efm.enumerate_network(net0)
+    assert got.n_out == 0 and got.stats["levels"] == 0
+    got = efm.enumerate_network(net0, seed_sets=[[0], [1]])
+    assert got.flux.tolist() == [[-1], [1]]
+    # capacity errors are reported, never silently truncated
+    net = make_network("small", 0)
+    with pytest.raises(efm.EfmError) as ei:
+        efm.enumerate_network(net, max_frontier=64)
+    assert ei.value.code == efm.EFM_E_CAPACITY
+    with pytest.raises(efm.EfmError) as ei:
+        efm.enumerate_network(net, max_candidates=4)
+    assert ei.value.code == efm.EFM_E_CAPACITY
+
+
+def test_sparse_and_dense_results_agree(efm):
+    net = make_network("small", 0)
+    en = efm.Enumerator(net.S, net.reversible, net.internal, net.params)
+    res = en.enumerate()
+    nnz, rxn, val = en.result_sparse()
+    dense = np.zeros_like(res.flux)
+    for r in range(res.n_out):
+        dense[r, rxn[r, : nnz[r]]] = val[r, : nnz[r]]
+    assert np.array_equal(dense, res.flux)
+    again = en.enumerate()   # the handle and the workspace are reusable
+    assert np.array_equal(again.flux, res.flux)
+    en.close()
