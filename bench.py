@@ -1,0 +1,297 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the AND/OR-graph pathway traversal (arXiv 1804.02867) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload genome] [--cap 65536]
+
+A *step* is one pass of the whole hot path (roots, classify, beam select, expand, support dedup, minimality filter,
+canonical output: SURVEY.md 8(a) rows a-2..a-8) over one seeded synthetic network that is already resident in HBM
+(the graph builder a-1 ran before; it is inside the `e2e` figure).  Metric = partial pathways expanded per second,
+whole job; EFMs/s and children/s ride along in `extra`.  Prints ONE JSON line on rank 0.
+
+N > 1 (torchrun): the path shards by independent problems -- rank r traverses the network of generator seed r with
+the same parameters, no data-path collective, scaling = weak.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores, on bounded samples of the same
+workload (same network and parameters, smaller beam), as the tier's reference arm.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "partial_pathways_expanded_per_sec"
+UNIT = "expanded/s"
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(index)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for r in self.rows if t0 <= r[0] <= t1 + 0.2] or self.rows
+        for _, line in rows:
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+                for nm, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _workload(name: str, seed: int, cap: int):
+    from netgen import make_network
+    net = make_network(name, seed)
+    params = dict(net.params)
+    if cap:
+        params["frontier_cap"] = cap
+    return net, params
+
+
+def _oracle_threads():
+    import oracle
+    return max(1, min(oracle.max_threads(), os.cpu_count() or 1))
+
+
+def run_oracle_sample(name: str, cap: int):
+    """One oracle run on the bounded sample; returns (expanded, seconds, outputs, threads)."""
+    import oracle
+    oracle.build()
+    net, params = _workload(name, 0, cap)
+    th = _oracle_threads()
+    t = time.time()
+    res = oracle.enumerate_pathways(net.S, net.reversible, net.internal, params, net.seed_sets, threads=th,
+                                    self_check=False)
+    dt = time.time() - t
+    return res.stats["expanded"], dt, res.stats["output"], th
+
+
+def main_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    # bounded sample: same network and parameters, beam small enough that (steps + warmup) runs end in minutes.
+    # The oracle costs ~2 ms per unit of frontier_cap per 8 threads on the genome network (measured).
+    cores = _oracle_threads()
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    per_cap = {"genome": 2.0e-3, "mid": 1.3e-4, "core": 2.5e-6, "small": 1e-7, "toy": 1e-8}.get(args.workload, 2e-3) * 8.0 / cores
+    cap = 256
+    while cap * 2 <= args.cap and cap * 2 * per_cap <= budget:
+        cap *= 2
+    for _ in range(args.warmup):
+        run_oracle_sample(args.workload, cap)
+    t_sum, exp_sum, outs = 0.0, 0, 0
+    for _ in range(args.steps):
+        e, dt, outs, _th = run_oracle_sample(args.workload, cap)
+        t_sum += dt
+        exp_sum += e
+    value = exp_sum / t_sum
+    sample = f"same network/parameters as config.workload, frontier_cap {cap} instead of {args.cap}; whole oracle run per step"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1000.0 * t_sum / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}-seed0 (BASELINE.json configs[4])", "frontier_cap": args.cap,
+                       "reference_sample_cap": cap},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "extra": {"efms_per_s": outs * args.steps / t_sum}}
+    print(json.dumps(line))
+    return 0
+
+
+def main_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_1804_02867_b200 import build
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_1804_02867_b200 as efm
+
+    # rank r owns the independent problem of generator seed r (weak scaling, no collective on the data path)
+    net, params = _workload(args.workload, rank, args.cap)
+    params["max_candidates"] = args.max_candidates
+    en = efm.Enumerator(net.S, net.reversible, net.internal, params, device=local, flags=efm.EFM_F_TIMING)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        en.enumerate(net.seed_sets, dense=False)
+    # ---- device-resident figure: K steps, each timed by the library with CUDA events on the launching stream
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    t0 = time.time()
+    ms = 0.0
+    acc = {}
+    for _ in range(args.steps):
+        flush.fill_(1)   # evict L2 between timed iterations (not timed)
+        torch.cuda.synchronize()
+        st = en.enumerate(net.seed_sets, dense=False).stats
+        ms += st["ms_total"]
+        for k, v in st.items():
+            acc[k] = acc.get(k, 0) + v
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    # ---- end to end through the public API with HOST buffers: graph build from S, upload, traversal, result D2H
+    e2e_s = 0.0
+    h2d = d2h = 0
+    for _ in range(args.steps):
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        t = time.time()
+        en2 = efm.Enumerator(net.S, net.reversible, net.internal, params, device=local)
+        en2._workspace = en._workspace          # device memory is allocated once by torch, outside the step
+        en2._lib.efm_workspace_invalidate(en2._h)
+        r2 = en2.enumerate(net.seed_sets, dense=False)
+        nnz, rxn, val = en2.result_sparse()
+        e2e_s += time.time() - t
+        gi = en2.graph_info()
+        h2d = 8 * (2 * gi["nnz"]) + 4 * (3 * gi["A"] + 2 * gi["M"]) * 2 + gi["dep_entries"] // 8 + int(r2.stats["n_roots"]) * 64
+        d2h = nnz.nbytes + rxn.nbytes + val.nbytes + int(r2.stats["levels"]) * 256
+        en2.close()
+    barrier()
+
+    expanded = acc["expanded"]
+    vals = torch.tensor([ms, e2e_s * 1000.0, float(expanded), float(acc["output"]), float(acc["children"])],
+                        dtype=torch.float64, device="cuda")
+    if world > 1:
+        mx = vals.clone()
+        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = vals.clone()
+        dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        ms_max, e2e_ms_max = mx[0].item(), mx[1].item()
+        expanded_all, outputs_all, children_all = sm[2].item(), sm[3].item(), sm[4].item()
+    else:
+        ms_max, e2e_ms_max = ms, e2e_s * 1000.0
+        expanded_all, outputs_all, children_all = float(expanded), float(acc["output"]), float(acc["children"])
+
+    if rank == 0:
+        peak, peak_src = _peaks()
+        n_exp_launch = acc["n_expand_count"] + acc["n_expand_write"] + acc["n_direct"]
+        ms_expand = acc["ms_expand_count"] + acc["ms_expand_write"] + acc["ms_direct"]
+        achieved = acc["algo_bytes"] / (ms_expand * 1e-3) / 1e9 if ms_expand > 0 else 0.0
+        roofline = {"bound": "hbm", "kernel": "k_expand (count + write + direct launches)", "achieved": achieved,
+                    "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": args.traffic,
+                    "peak_source": peak_src, "launches_per_step": n_exp_launch / args.steps,
+                    "avg_launch_ms": ms_expand / max(1, n_exp_launch),
+                    "algo_bytes_per_launch": acc["algo_bytes"] / max(1, n_exp_launch),
+                    "share_of_step": ms_expand / ms if ms else None}
+        # the oracle as it stands on this box's host cores, bounded sample of the same workload
+        cpu = None
+        if not args.no_cpu_baseline:
+            cap_s = min(args.cap, 4096 if args.workload == "genome" else args.cap)
+            e, dt, outs, th = run_oracle_sample(args.workload, cap_s)
+            cpu = {"value": e / dt, "unit": UNIT, "cores": th, "kind": "oracle",
+                   "sample": f"same network/parameters, frontier_cap {cap_s} instead of {args.cap}; one whole oracle run "
+                             f"({dt:.1f} s, {e} expansions, {outs} outputs)"}
+        line = {"metric": METRIC, "value": expanded_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+                "config": {"workload": f"{args.workload}-seed{{rank}} (BASELINE.json configs[4]: 1000+150 metabolites, 2000 reactions, "
+                                       "30% reversible, depth cap 60, 8 target exchange reactions)",
+                           "frontier_cap": args.cap, "params": {k: int(v) for k, v in params.items()},
+                           "l2": "flushed between timed iterations (256 MiB write)", "parallelism": f"replicas x{world}"},
+                "clocks": clocks,
+                "e2e": {"value": expanded_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                        "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms_max / args.steps,
+                        "what": "efm_create (graph builder from host S) + efm_enumerate (graph upload + traversal) + "
+                                "efm_result_copy_sparse to host, wall clock"},
+                "gpu_launches": int(acc["launches"]),
+                "roofline": roofline,
+                "cpu_baseline": cpu,
+                "extra": {"efms_per_s": outputs_all / (ms_max * 1e-3), "children_per_s": children_all / (ms_max * 1e-3),
+                          "outputs_per_step": outputs_all / args.steps / world, "levels": acc["levels"] / args.steps,
+                          "phase_ms_per_step": {k: acc[k] / args.steps for k in
+                                                ("ms_expand_count", "ms_beam", "ms_expand_write", "ms_direct", "ms_hash",
+                                                 "ms_filter", "ms_output")},
+                          "filter_pairs_per_s": (acc["filter_pairs"] / (acc["ms_filter"] * 1e-3)) if acc["ms_filter"] else None}}
+        print(json.dumps(line))
+    en.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="genome", choices=["toy", "small", "core", "mid", "genome"])
+    ap.add_argument("--cap", type=int, default=65536, help="frontier_cap (beam) of the workload")
+    ap.add_argument("--max-candidates", type=int, default=1 << 20)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="ncu dram bytes per expand launch from profiles/ (null until captured)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return main_reference(args)
+    return main_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

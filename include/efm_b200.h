@@ -120,6 +120,11 @@ int efm_workspace_bytes(const efm_handle* h, size_t* bytes);
 int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_arc_code, int32_t n_sets,
                   void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* The graph arrays are uploaded into the workspace by the first efm_enumerate() that sees a given workspace
+ * pointer and are assumed resident afterwards (the network is an input that stays in HBM across calls).  A caller
+ * that overwrites the workspace, or frees it and gets the same address back, must call this before the next run. */
+int efm_workspace_invalidate(efm_handle* h);
+
 /* Number of pathways found (host out). */
 int efm_result_count(const efm_handle* h, int64_t* n_pathways);
 

@@ -68,6 +68,7 @@ def load() -> ctypes.CDLL:
     lib.efm_graph_export.argtypes = [vp] + [vp] * 14
     lib.efm_workspace_bytes.argtypes = [vp, P(sz)]
     lib.efm_enumerate.argtypes = [vp, vp, vp, i32, vp, sz, vp]
+    lib.efm_workspace_invalidate.argtypes = [vp]
     lib.efm_result_count.argtypes = [vp, P(i64)]
     lib.efm_result_copy.argtypes = [vp, vp, i64]
     lib.efm_result_sparse_stride.argtypes = [vp, P(i32)]
@@ -196,6 +197,7 @@ class Enumerator:
         need = self.workspace_bytes()
         if self._workspace is None or self._workspace.numel() < need:
             self._workspace = torch.empty(need, dtype=torch.uint8, device=f"cuda:{self.device}")
+            self._check(self._lib.efm_workspace_invalidate(self._h))
         with torch.cuda.device(self.device):
             stream = torch.cuda.current_stream().cuda_stream
             self.enumerate_raw(seed_sets, self._workspace.data_ptr(), self._workspace.numel(), stream)

@@ -44,6 +44,7 @@ struct efm_handle {
     double ms_build = 0;
     // run state
     unsigned char* ws = nullptr;
+    unsigned char* graph_ws = nullptr;   // workspace the graph arrays were last uploaded to
     bool have_result = false;
     int64_t n_out = 0;
     efm_stats stats;
@@ -317,17 +318,21 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         if (bytes == 0) return cudaSuccess;
         return cudaMemcpyAsync(ws + r.off, src, bytes, cudaMemcpyHostToDevice, s);
     };
-    CK(up(L.col_ptr, G.col_ptr.data(), sizeof(int) * G.col_ptr.size()));
-    CK(up(L.col, G.col.data(), sizeof(ColRef) * G.col.size()));
-    CK(up(L.in_ptr, G.in_ptr.data(), sizeof(int) * G.in_ptr.size()));
-    CK(up(L.in_e, G.in.data(), sizeof(ArcRef) * G.in.size()));
-    CK(up(L.out_ptr, G.out_ptr.data(), sizeof(int) * G.out_ptr.size()));
-    CK(up(L.out_e, G.out.data(), sizeof(ArcRef) * G.out.size()));
-    CK(up(L.twin, G.twin.data(), sizeof(int) * G.twin.size()));
-    CK(up(L.dep_off, G.dep_off.data(), sizeof(i64) * G.dep_off.size()));
-    CK(up(L.dep_bits, G.dep_bits.data(), sizeof(u32) * G.dep_bits.size()));
-    CK(up(L.arc_rxn, G.arc_rxn.data(), sizeof(int) * G.arc_rxn.size()));
-    CK(up(L.arc_dir, G.arc_dir.data(), sizeof(int) * G.arc_dir.size()));
+    if (h->graph_ws != ws) {   // the network is an input: it stays resident in the workspace across calls
+        h->graph_ws = nullptr;
+        CK(up(L.col_ptr, G.col_ptr.data(), sizeof(int) * G.col_ptr.size()));
+        CK(up(L.col, G.col.data(), sizeof(ColRef) * G.col.size()));
+        CK(up(L.in_ptr, G.in_ptr.data(), sizeof(int) * G.in_ptr.size()));
+        CK(up(L.in_e, G.in.data(), sizeof(ArcRef) * G.in.size()));
+        CK(up(L.out_ptr, G.out_ptr.data(), sizeof(int) * G.out_ptr.size()));
+        CK(up(L.out_e, G.out.data(), sizeof(ArcRef) * G.out.size()));
+        CK(up(L.twin, G.twin.data(), sizeof(int) * G.twin.size()));
+        CK(up(L.dep_off, G.dep_off.data(), sizeof(i64) * G.dep_off.size()));
+        CK(up(L.dep_bits, G.dep_bits.data(), sizeof(u32) * G.dep_bits.size()));
+        CK(up(L.arc_rxn, G.arc_rxn.data(), sizeof(int) * G.arc_rxn.size()));
+        CK(up(L.arc_dir, G.arc_dir.data(), sizeof(int) * G.arc_dir.size()));
+        h->graph_ws = ws;
+    }
     CK(up(L.buf[1], root_img.data(), root_img.size()));
     CK(cudaMemsetAsync(ws + L.ctl.off, 0, sizeof(Ctl), s));
     CK(cudaStreamSynchronize(s));   // the host staging vectors above go out of scope later; keep it simple
@@ -500,6 +505,13 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     }
     h->n_out = (int64_t)n_keep;
     h->have_result = true;
+    return EFM_OK;
+}
+
+int efm_workspace_invalidate(efm_handle* h) {
+    if (!h) return EFM_E_INVAL;
+    h->graph_ws = nullptr;
+    h->have_result = false;
     return EFM_OK;
 }
 
