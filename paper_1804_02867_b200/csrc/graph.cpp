@@ -2,6 +2,7 @@
 #include "graph.hpp"
 
 #include <algorithm>
+#include <thread>
 
 #include "../../include/efm_b200.h"
 
@@ -79,39 +80,62 @@ int build_graph(HostGraph& G, const int32_t* S, int32_t m, int32_t n, int64_t ro
     for (int32_t i = 0; i < G.M; ++i)
         G.dep_off[i + 1] = G.dep_off[i] + (int64_t)(G.out_ptr[i + 1] - G.out_ptr[i]) * (G.in_ptr[i + 1] - G.in_ptr[i]);
     G.dep_bits.assign((size_t)((G.dep_off[G.M] + 31) / 32) + 1, 0u);
-    std::vector<int32_t> stamp((size_t)G.A, -1), frontier, next;
-    int32_t epoch = 0;
-    for (int32_t i = 0; i < G.M; ++i) {
-        const int32_t nI = G.in_ptr[i + 1] - G.in_ptr[i];
-        if (nI == 0) continue;
-        for (int32_t lo = 0; lo < G.out_ptr[i + 1] - G.out_ptr[i]; ++lo) {
-            const int32_t o = G.out[G.out_ptr[i] + lo].arc;
-            ++epoch;
-            frontier.assign(1, o);
-            stamp[o] = epoch;
-            for (int32_t hop = 1; hop < dep_depth && !frontier.empty(); ++hop) {
-                next.clear();
-                for (int32_t x : frontier)
-                    for (int32_t q = G.col_ptr[x]; q < G.col_ptr[x + 1]; ++q) {
-                        if (G.col[q].s <= 0 || G.col[q].met == i) continue;
-                        const int32_t via = G.col[q].met;
-                        for (int32_t r = G.out_ptr[via]; r < G.out_ptr[via + 1]; ++r) {
-                            const int32_t y = G.out[r].arc;
-                            if (y == G.twin[x] || stamp[y] == epoch) continue;
-                            stamp[y] = epoch;
-                            next.push_back(y);
+    // A metabolite's consumer list is swept once per search: the first arc x that reaches q stamps every consumer but
+    // twin(x); a second, different arc reaching q can only add that one twin.  Nodes are independent, so the searches
+    // are spread over host threads (bits of neighbouring nodes can share a word: atomic OR).
+    auto worker = [&G, dep_depth](int32_t tid, int32_t nthreads) {
+        std::vector<int32_t> stamp((size_t)G.A, -1), frontier, next;
+        std::vector<int32_t> q_epoch((size_t)G.M, -1), q_first((size_t)G.M, -1);
+        std::vector<char> q_full((size_t)G.M, 0);
+        int32_t epoch = 0;
+        for (int32_t i = tid; i < G.M; i += nthreads) {
+            const int32_t nI = G.in_ptr[i + 1] - G.in_ptr[i];
+            if (nI == 0) continue;
+            for (int32_t lo = 0; lo < G.out_ptr[i + 1] - G.out_ptr[i]; ++lo) {
+                const int32_t o = G.out[G.out_ptr[i] + lo].arc;
+                ++epoch;
+                frontier.assign(1, o);
+                stamp[o] = epoch;
+                for (int32_t hop = 1; hop < dep_depth && !frontier.empty(); ++hop) {
+                    next.clear();
+                    for (int32_t x : frontier)
+                        for (int32_t q = G.col_ptr[x]; q < G.col_ptr[x + 1]; ++q) {
+                            if (G.col[q].s <= 0 || G.col[q].met == i) continue;
+                            const int32_t via = G.col[q].met;
+                            if (q_epoch[via] != epoch) {
+                                q_epoch[via] = epoch; q_first[via] = x; q_full[via] = 0;
+                                for (int32_t r = G.out_ptr[via]; r < G.out_ptr[via + 1]; ++r) {
+                                    const int32_t y = G.out[r].arc;
+                                    if (y == G.twin[x] || stamp[y] == epoch) continue;
+                                    stamp[y] = epoch;
+                                    next.push_back(y);
+                                }
+                            } else if (!q_full[via] && q_first[via] != x) {
+                                q_full[via] = 1;
+                                const int32_t y = G.twin[q_first[via]];   // consumes `via` because its twin produces it
+                                if (y >= 0 && stamp[y] != epoch) { stamp[y] = epoch; next.push_back(y); }
+                            }
                         }
+                    frontier.swap(next);
+                }
+                for (int32_t le = 0; le < nI; ++le) {
+                    const int32_t e = G.in[G.in_ptr[i] + le].arc;
+                    if (e != o && stamp[e] == epoch) {
+                        const int64_t b = G.dep_off[i] + (int64_t)lo * nI + le;
+                        __atomic_fetch_or(&G.dep_bits[b >> 5], 1u << (b & 31), __ATOMIC_RELAXED);
                     }
-                frontier.swap(next);
-            }
-            for (int32_t le = 0; le < nI; ++le) {
-                const int32_t e = G.in[G.in_ptr[i] + le].arc;
-                if (e != o && stamp[e] == epoch) {
-                    const int64_t b = G.dep_off[i] + (int64_t)lo * nI + le;
-                    G.dep_bits[b >> 5] |= 1u << (b & 31);
                 }
             }
         }
+    };
+    int32_t nthreads = (int32_t)std::thread::hardware_concurrency();
+    nthreads = std::max(1, std::min(nthreads, 32));
+    if (G.dep_off[G.M] < 4096) nthreads = 1;
+    if (nthreads == 1) worker(0, 1);
+    else {
+        std::vector<std::thread> pool;
+        for (int32_t t = 0; t < nthreads; ++t) pool.emplace_back(worker, t, nthreads);
+        for (std::thread& t : pool) t.join();
     }
     return EFM_OK;
 }
