@@ -22,7 +22,7 @@ namespace {
 struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
-    Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir;
+    Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
     Region ctl, buf[2], keys, cand, table, isrep, poison, uniq, size_hist, bucket_start, bucket_fill;
     Region order, sig, size_sorted, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, dense;
     size_t total = 0;
@@ -78,6 +78,7 @@ void make_layout(efm_handle* h) {
     add_region(L, L.dep_bits, sizeof(u32) * G.dep_bits.size());
     add_region(L, L.arc_rxn, sizeof(int) * (G.A + 1));
     add_region(L, L.arc_dir, sizeof(int) * (G.A + 1));
+    add_region(L, L.arc_mix, sizeof(u64) * (G.A + 1));
     add_region(L, L.ctl, sizeof(Ctl));
     add_region(L, L.buf[0], (size_t)h->max_frontier * h->stride);
     add_region(L, L.buf[1], (size_t)h->max_frontier * h->stride);
@@ -131,6 +132,9 @@ DevGraph dev_graph(const efm_handle* h, unsigned char* ws) {
     g.twin = (const int*)(ws + L.twin.off);
     g.dep_off = (const i64*)(ws + L.dep_off.off);   g.dep_bits = (const u32*)(ws + L.dep_bits.off);
     g.arc_rxn = (const int*)(ws + L.arc_rxn.off);   g.arc_dir = (const int*)(ws + L.arc_dir.off);
+    g.arc_mix = (const u64*)(ws + L.arc_mix.off);
+    g.max_coef = 0;
+    for (const ColRef& c : h->G.col) g.max_coef = std::max(g.max_coef, c.s < 0 ? -c.s : c.s);
     return g;
 }
 
@@ -200,7 +204,8 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     h->max_frontier = P.max_frontier ? P.max_frontier : (h->cap ? std::max<int64_t>(h->cap, 4096) : (int64_t)1 << 20);
     h->max_cand = P.max_candidates ? P.max_candidates : (int64_t)1 << 20;
     if (h->max_cand > 0xFFFFFFF0LL) { delete h; return EFM_E_INVAL; }
-    h->max_keys = P.max_child_keys ? P.max_child_keys : std::max<int64_t>(h->cap * (int64_t)G.max_fanout, 65536);
+    h->max_keys = (P.max_child_keys ? P.max_child_keys : std::max<int64_t>(h->cap * (int64_t)G.max_fanout, 65536)) +
+                  (int64_t)expand_key_slack();
     h->table_size = pow2_at_least((size_t)h->max_cand * 2);
     h->dense_bytes = std::max<size_t>((size_t)64 << 20, (size_t)n * 8 * 64);
     make_layout(h);
@@ -294,10 +299,12 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     for (size_t r = 0; r < roots.size(); ++r) {
         unsigned char* e = root_img.data() + r * h->stride;
         const u32 ns = (u32)roots[r].size();
-        *(u32*)e = ns;   // n_vis = 0
-        i64* f = (i64*)(e + 16);
-        u16* arc = (u16*)(e + 16 + 8 * (size_t)ns);
-        for (u32 k = 0; k < ns; ++k) { f[k] = 1; arc[k] = (u16)roots[r][k]; }
+        *(u32*)e = ns;   // n_vis = 0; n_unb is filled in by the classify pass
+        i64* f = (i64*)(e + kHdr);
+        u16* arc = (u16*)(e + kHdr + 8 * (size_t)ns);
+        u64 hs = 0;
+        for (u32 k = 0; k < ns; ++k) { f[k] = 1; arc[k] = (u16)roots[r][k]; hs += arc_term((u32)roots[r][k], 1ULL); }
+        ((u64*)e)[1] = hs;   // hv = 0: nothing visited
     }
 
     CK(cudaSetDevice(h->device));
@@ -318,6 +325,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         if (bytes == 0) return cudaSuccess;
         return cudaMemcpyAsync(ws + r.off, src, bytes, cudaMemcpyHostToDevice, s);
     };
+    std::vector<u64> arc_mix;
     if (h->graph_ws != ws) {   // the network is an input: it stays resident in the workspace across calls
         h->graph_ws = nullptr;
         CK(up(L.col_ptr, G.col_ptr.data(), sizeof(int) * G.col_ptr.size()));
@@ -331,6 +339,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         CK(up(L.dep_bits, G.dep_bits.data(), sizeof(u32) * G.dep_bits.size()));
         CK(up(L.arc_rxn, G.arc_rxn.data(), sizeof(int) * G.arc_rxn.size()));
         CK(up(L.arc_dir, G.arc_dir.data(), sizeof(int) * G.arc_dir.size()));
+        arc_mix.resize((size_t)G.A);
+        for (int a = 0; a < G.A; ++a) arc_mix[a] = mix64(0x0100000000000000ULL | (u64)a);   // inner mix of arc_term
+        CK(up(L.arc_mix, arc_mix.data(), sizeof(u64) * arc_mix.size()));
         h->graph_ws = ws;
     }
     CK(up(L.buf[1], root_img.data(), root_img.size()));
@@ -350,6 +361,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.stride = h->stride; ea.cand_stride = h->cand_stride;
     ea.max_frontier = (u64)h->max_frontier; ea.max_cand = (u64)h->max_cand; ea.max_keys = (u64)h->max_keys;
     ea.D = h->D; ea.V = h->V; ea.max_loop = h->max_loop;
+    ea.no_fast = (h->flags & EFM_F_NO_FASTPATH) ? 1 : 0;
     expand_smem_layout(ea);
 
     auto read_ctl = [&]() -> cudaError_t {

@@ -14,14 +14,18 @@ typedef unsigned short u16;
 
 // ---------------------------------------------------------------------------------------------------------------
 // Entry format in HBM.  A frontier slot is `stride` bytes; the entry occupies a prefix:
-//   [ 0,16)  header: u32 n_supp | n_vis << 16, 12 spare bytes
+//   [ 0,32)  header: u32 n_supp | n_vis << 16; u32 n_unb (unbalanced internal metabolites);
+//            u64 hs = sum of the arc terms of the state hash; u64 hv = sum of its visited terms; 8 spare bytes.
+//            hs / hv / n_unb are derived data the producer has in registers anyway: carrying them (20 B) saves the
+//            consumer one full re-hash of the parent.
 //   i64  flux[n_supp]   fluxes of the support arcs, > 0, gcd 1
 //   u64  vis[n_vis]     visited records: cnt << 48 | met << 32 | PI << 16 | PO   (unordered)
 //   u16  arc[n_supp]    support arcs, ascending arc id
 // A candidate slot holds the same with n_vis = 0.
 // ---------------------------------------------------------------------------------------------------------------
+constexpr u32 kHdr = 32;   // header bytes of a frontier / candidate slot
 __host__ __device__ inline u32 entry_bytes(u32 n_supp, u32 n_vis) {
-    return (16u + 8u * n_supp + 8u * n_vis + 2u * n_supp + 15u) & ~15u;
+    return (kHdr + 8u * n_supp + 8u * n_vis + 2u * n_supp + 15u) & ~15u;
 }
 // irreducible content of an entry, the unit of the algorithmic-byte count
 __host__ __device__ inline u32 algo_entry_bytes(u32 n_supp, u32 n_vis) { return n_supp * 10u + n_vis * 7u + 16u; }
@@ -34,6 +38,8 @@ struct DevGraph {
     const int* twin;
     const i64* dep_off;   const u32* dep_bits;
     const int* arc_rxn;   const int* arc_dir;
+    const u64* arc_mix;   // mix64(0x01 << 56 | a): the inner mix of the arc term of the state hash, per arc
+    int max_coef;         // largest |s_ia| of the network (bounds the lane-parallel fast path)
 };
 
 // Device-resident control block: per-level counters, beam-select state, cumulative statistics.
@@ -45,7 +51,8 @@ enum { SEL_BINS = 2048 };
 struct Ctl {
     // per level (reset by k_level_begin)
     u64 n_next;        // active survivors written to the next frontier buffer
-    u64 n_keys;        // active children generated (= keys written by the count pass)
+    u64 n_keys;        // active children generated (= valid keys written by the count pass)
+    u64 n_slots;       // key slots reserved by the count pass (chunked per warp; unused slots hold kKeySentinel)
     u64 lvl_done;      // balanced children generated
     u64 lvl_children;  // children generated (active + done)
     u64 lvl_expanded;  // parents expanded
@@ -74,7 +81,7 @@ struct ExpandArgs {
     u32 stride, cand_stride;
     u64 max_frontier, max_cand, max_keys;
     int D, V, max_loop;
-    int count_algo_children;    // 0 for the root level (roots are not written by an expansion)
+    int no_fast;                // EFM_F_NO_FASTPATH: every child through the warp-cooperative general routine
     // shared-memory carve-up per group (bytes)
     u32 sm_group, sm_EF, sm_sbits, sm_mseen;
 };
@@ -96,6 +103,9 @@ __host__ __device__ inline u64 vis_pack(u32 met, u32 PI, u32 PO, u32 cnt) {
     return ((u64)cnt << 48) | ((u64)met << 32) | ((u64)PI << 16) | (u64)PO;
 }
 __host__ __device__ inline u64 beam_key(u32 n_unb, u64 h) { return ((u64)(n_unb > 255u ? 255u : n_unb) << 56) | (h >> 8); }
+
+constexpr u64 kKeySentinel = ~0ULL;   // filler of reserved but unused key slots: never < X, skipped by the select
+constexpr u32 kKeyChunk = 64;         // key slots a warp reserves per atomic
 
 #define EFM_GUARD (1ULL << 62)   // reading G21: any state integer above 2^62 discards the pathway
 

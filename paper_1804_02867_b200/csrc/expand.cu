@@ -1,9 +1,13 @@
-// Frontier expansion kernels: one lane group ("group", GW lanes of a warp)
-// owns one partial pathway.  The group stages the parent entry in shared memory, scatters its extra fluxes
-// EF_i (Eq 2) into a dense per-group shared array, picks the lowest unbalanced metabolite i*
-// (reading G12), fans out over the OR-alternatives of i* (first visit, PROC1/1', Eq 3) or applies
-// Eq 4 / Eq 5 (revisit, PROC2-4), rescales to integers with gcd normalisation (reading G10) and
-// classifies every child (balanced -> candidate; otherwise beam key).  Three modes:
+// Frontier expansion kernels: one warp owns one partial pathway at a time.
+// The warp stages the parent entry in shared memory, scatters its extra fluxes EF_i (Eq 2) into a
+// dense per-warp shared array, picks the lowest unbalanced metabolite i* (reading G12) and then
+//   first visit (PROC1/1', Eq 3): fans out over the OR-alternatives of i*, ONE LANE PER
+//       ALTERNATIVE -- a child that adds a new arc to a pathway whose integers are far from the 2^62 guard needs only
+//       lane-local work (scale k = c/gcd(|E|,c), its own column of S for the new unbalanced count, an incremental
+//       state hash); anything else (arc already in the support, large integers) takes the warp-cooperative general
+//       routine eval_child();
+//   revisit (PROC2-4, Eq 4 / Eq 5): exactly one child, general routine.
+// Children are classified where they are generated (balanced -> candidate; otherwise beam key).  Three modes:
 //   COUNT  : count children, write only their 8-byte beam keys           (pass 1 of a level the beam may cut)
 //   WRITE  : regenerate the children and materialise those with key < X  (pass 2)
 //   DIRECT : single pass, every child is materialised                     (beam cannot bind)
@@ -17,37 +21,24 @@ namespace efm {
 enum { MODE_COUNT = 0, MODE_WRITE = 1, MODE_DIRECT = 2 };
 enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
 constexpr int kBlock = 128;
+constexpr int kWarps = kBlock / 32;
+constexpr u32 FULL = 0xffffffffu;
+constexpr u64 kSmall = 1ULL << 40;   // fast path: every flux and extra flux of the parent below this ...
+constexpr int kSmallCoef = 1 << 20;  // ... and every coefficient below this: no product can reach 2^62
 
-// ------------------------------------------------------------------ group collectives (GW lanes of one warp)
-template <int GW> __device__ __forceinline__ u64 g_sum(u64 v, u32 m) {
+// ------------------------------------------------------------------ warp collectives
+__device__ __forceinline__ u64 w_sum(u64 v) {
 #pragma unroll
-    for (int o = GW / 2; o; o >>= 1) v += __shfl_xor_sync(m, v, o, GW);
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
     return v;
 }
-template <int GW> __device__ __forceinline__ int g_sum(int v, u32 m) {
-#pragma unroll
-    for (int o = GW / 2; o; o >>= 1) v += __shfl_xor_sync(m, v, o, GW);
-    return v;
+__device__ __forceinline__ u64 w_max(u64 v) {   // two 32-bit redux instead of five 64-bit shuffle rounds
+    const u32 hi = (u32)(v >> 32);
+    const u32 mh = __reduce_max_sync(FULL, hi);
+    const u32 ml = __reduce_max_sync(FULL, hi == mh ? (u32)v : 0u);
+    return ((u64)mh << 32) | ml;
 }
-template <int GW> __device__ __forceinline__ u64 g_max(u64 v, u32 m) {
-#pragma unroll
-    for (int o = GW / 2; o; o >>= 1) { u64 w = __shfl_xor_sync(m, v, o, GW); v = w > v ? w : v; }
-    return v;
-}
-template <int GW> __device__ __forceinline__ int g_max(int v, u32 m) {
-#pragma unroll
-    for (int o = GW / 2; o; o >>= 1) v = max(v, __shfl_xor_sync(m, v, o, GW));
-    return v;
-}
-template <int GW> __device__ __forceinline__ int g_min(int v, u32 m) {
-#pragma unroll
-    for (int o = GW / 2; o; o >>= 1) v = min(v, __shfl_xor_sync(m, v, o, GW));
-    return v;
-}
-// ballot restricted to the group, bit l = lane l of the group
-template <int GW> __device__ __forceinline__ u32 g_ballot(bool p, u32 m, int shift) {
-    return (__ballot_sync(m, p) & m) >> shift;
-}
+__device__ __forceinline__ u64 w_bcast(u64 v, int src) { return __shfl_sync(FULL, v, src); }
 
 // ------------------------------------------------------------------ integer helpers
 __device__ __forceinline__ u64 gcd64(u64 a, u64 b) {   // binary gcd
@@ -62,9 +53,9 @@ __device__ __forceinline__ u64 gcd64(u64 a, u64 b) {   // binary gcd
     } while (b);
     return a << sh;
 }
-template <int GW> __device__ __forceinline__ u64 g_gcd(u64 v, u32 m) {
+__device__ __forceinline__ u64 w_gcd(u64 v) {
 #pragma unroll
-    for (int o = GW / 2; o; o >>= 1) { u64 w = __shfl_xor_sync(m, v, o, GW); v = gcd64(v, w); }
+    for (int o = 16; o; o >>= 1) { u64 w = __shfl_xor_sync(FULL, v, o); v = gcd64(v, w); }
     return v;
 }
 struct S128 { u64 lo; i64 hi; };
@@ -79,8 +70,10 @@ __device__ __forceinline__ bool abs_gt_guard(S128 x) {   // |x| > 2^62
 __device__ __forceinline__ bool umul_gt_guard(u64 a, u64 b) {  // a*b > 2^62, a, b >= 0
     return __umul64hi(a, b) != 0 || a * b > EFM_GUARD;
 }
+// arc term of the state hash through the per-arc table of inner mixes (device_common.cuh: arc_term)
+__device__ __forceinline__ u64 arc_term_t(const DevGraph& g, u32 a, u64 f) { return mix64(__ldg(&g.arc_mix[a]) + f); }
 
-// ------------------------------------------------------------------ per-parent context (group-uniform)
+// ------------------------------------------------------------------ per-parent context (warp-uniform)
 struct Parent {
     int n_supp, n_vis;
     const i64* flux; const u64* vis; const u16* arc;   // shared-memory staging
@@ -89,31 +82,35 @@ struct Parent {
     int n_unb, istar;
     i64 E;
 };
-struct Child {          // group-uniform description of one child relative to its parent
-    int status; bool done; u64 key;
-    int a; bool in_supp; int ia, ins;
-    u64 k, d, g2, T;    // scale, increment, common divisor, un-normalised new flux of arc a
+struct Child {          // warp-uniform description of one child relative to its parent
+    int status; bool done;
+    int a; bool in_supp; int ia;
+    u64 k, g2, T;       // scale, common divisor, un-normalised new flux of arc a
+    u64 hs, hv;         // hash sums of the child state
     int n_unb;
 };
 
 __device__ __forceinline__ bool sbit(const u32* sbits, int a) { return (sbits[a >> 5] >> (a & 31)) & 1u; }
 
-// Evaluate the child bump(f, a, sign*|E|/c) cooperatively.
-//   first: new visited record (istar, PI, PO, 0); otherwise record index vk is replaced by newrec
-template <int GW, bool NEED_KEY>
-__device__ __forceinline__ void eval_child(const DevGraph& g, const Parent& P, int lane, u32 gmask, int a, int c, int sign,
-                                           bool first, u64 oldrec, u64 newrec, Child& ch) {
+// General routine: evaluate the child bump(f, a, sign*|E|/c) with the whole warp.
+//   first: new visited record newrec; otherwise record oldrec is replaced by newrec
+__device__ __noinline__ void eval_child(const DevGraph& g, const Parent& P, int lane, int a, int c, int sign,
+                                        bool first, u64 oldrec, u64 newrec, Child& ch) {
     const u64 absE = (u64)(P.E < 0 ? -P.E : P.E);
     const u64 gg = gcd64(absE, (u64)c);
     const u64 k = gg == 1 ? (u64)c : (u64)c / gg;
     const u64 d = gg == 1 ? absE : absE / gg;
-    ch.a = a; ch.k = k; ch.d = d; ch.g2 = 1;
+    ch.a = a; ch.k = k; ch.g2 = 1;
     ch.in_supp = sbit(P.sbits, a);
-    // position of a in the sorted support
-    int ia = -1, ins = 0;
-    for (int t = lane; t < P.n_supp; t += GW) { int at = P.arc[t]; ia = at == a ? t : ia; ins += at < a; }
-    ia = g_max<GW>(ia, gmask); ins = g_sum<GW>(ins, gmask);
-    ch.ia = ia; ch.ins = ins;
+    int ia = -1;
+    if (ch.in_supp) {   // position of a in the sorted support
+        for (int base = 0; base < P.n_supp && ia < 0; base += 32) {
+            const int t = base + lane;
+            const u32 hit = __ballot_sync(FULL, t < P.n_supp && P.arc[t] == a);
+            if (hit) ia = base + __ffs(hit) - 1;
+        }
+    }
+    ch.ia = ia;
     // scaled fluxes F_t = k f_t, F_a = k f_a +- d: overflow first, then non-positive (order of the definition, O6)
     bool ovf = false, nonpos = false;
     u64 T = d;
@@ -131,8 +128,8 @@ __device__ __forceinline__ void eval_child(const DevGraph& g, const Parent& P, i
         if (k > 1 && umul_gt_guard(k, P.fmax)) {
             // exact: the largest flux among t != ia
             u64 mx = 0;
-            for (int t = lane; t < P.n_supp; t += GW) if (t != ia) mx = max(mx, (u64)P.flux[t]);
-            mx = g_max<GW>(mx, gmask);
+            for (int t = lane; t < P.n_supp; t += 32) if (t != ia) mx = max(mx, (u64)P.flux[t]);
+            mx = w_max(mx);
             ovf = ovf || umul_gt_guard(k, mx);
         }
     } else {
@@ -146,7 +143,7 @@ __device__ __forceinline__ void eval_child(const DevGraph& g, const Parent& P, i
     if (k > 1 && umul_gt_guard(k, P.maxabsEF)) {
         // exact sweep over every touched metabolite outside col(a)
         const int qa0 = g.col_ptr[a], qa1 = g.col_ptr[a + 1];
-        for (int t = lane; t < P.n_supp; t += GW) {
+        for (int t = lane; t < P.n_supp; t += 32) {
             const int at = P.arc[t];
             for (int q = g.col_ptr[at]; q < g.col_ptr[at + 1]; ++q) {
                 const int i = g.col[q].x;
@@ -157,333 +154,449 @@ __device__ __forceinline__ void eval_child(const DevGraph& g, const Parent& P, i
         }
     }
     int delta = 0;
-    for (int q = g.col_ptr[a] + lane; q < g.col_ptr[a + 1]; q += GW) {
+    for (int q = g.col_ptr[a] + lane; q < g.col_ptr[a + 1]; q += 32) {
         const int2 e = g.col[q];
         const i64 efp = P.EF[e.x];
         S128 x = add_s(mul_s((i64)k, efp), mul_s(sign > 0 ? (i64)d : -(i64)d, (i64)e.y));
         ovf2 = ovf2 || abs_gt_guard(x);
         delta += (int)((x.lo | (u64)x.hi) != 0) - (int)(efp != 0);
     }
-    ovf2 = g_ballot<GW>(ovf2, gmask, 0) != 0;   // any lane of the group (shift irrelevant for a zero test)
-    if (ovf2) { ch.status = CH_OVERFLOW; return; }
-    delta = g_sum<GW>(delta, gmask);
+    if (__any_sync(FULL, ovf2)) { ch.status = CH_OVERFLOW; return; }
+    delta = __reduce_add_sync(FULL, delta);
     ch.status = CH_OK;
     ch.n_unb = P.n_unb + delta;
     ch.done = ch.n_unb == 0;
     // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and gcd(k, d) = 1.
     if (ch.in_supp) {
         u64 G = 0;
-        for (int t = lane; t < P.n_supp; t += GW) if (t != ia) G = gcd64(G, (u64)P.flux[t]);
-        G = g_gcd<GW>(G, gmask);
+        for (int t = lane; t < P.n_supp; t += 32) if (t != ia) G = gcd64(G, (u64)P.flux[t]);
+        G = w_gcd(G);
         ch.g2 = gcd64(k * G, T);   // k G <= k fmax <= 2^62
     }
-    if (NEED_KEY) {
-        u64 hs;
-        if (k == 1 && ch.g2 == 1) {
-            hs = P.hs + arc_term((u32)a, T) - (ch.in_supp ? arc_term((u32)a, (u64)P.flux[ia]) : 0ULL);
-        } else {
-            hs = 0;
-            for (int t = lane; t < P.n_supp; t += GW) {
-                u64 F = t == ia ? T : k * (u64)P.flux[t];
-                if (ch.g2 > 1) F /= ch.g2;
-                hs += arc_term((u32)P.arc[t], F);
-            }
-            hs = g_sum<GW>(hs, gmask);
-            if (!ch.in_supp) hs += arc_term((u32)a, T);
+    u64 hs;
+    if (k == 1 && ch.g2 == 1) {
+        hs = P.hs + arc_term_t(g, (u32)a, T) - (ch.in_supp ? arc_term_t(g, (u32)a, (u64)P.flux[ia]) : 0ULL);
+    } else {
+        hs = 0;
+        for (int t = lane; t < P.n_supp; t += 32) {
+            u64 F = t == ia ? T : k * (u64)P.flux[t];
+            if (ch.g2 > 1) F /= ch.g2;
+            hs += arc_term_t(g, (u32)P.arc[t], F);
         }
-        const u64 hv = P.hv + vis_term(newrec) - (first ? 0ULL : vis_term(oldrec));
-        ch.key = beam_key((u32)ch.n_unb, mix64(hs + hv));
+        hs = w_sum(hs);
+        if (!ch.in_supp) hs += arc_term_t(g, (u32)a, T);
     }
+    ch.hs = hs;
+    ch.hv = P.hv + vis_term(newrec) - (first ? 0ULL : vis_term(oldrec));
 }
 
 // Write the child into a frontier slot (or a candidate slot: no visited records).
-template <int GW>
 __device__ __forceinline__ void write_child(unsigned char* dst, const Parent& P, const Child& ch, int lane, bool first,
                                             int vk, u64 newrec, bool to_cand) {
     const int n2 = P.n_supp + (ch.in_supp ? 0 : 1);
     const int nv2 = to_cand ? 0 : P.n_vis + (first ? 1 : 0);
-    if (lane == 0) *(uint4*)dst = make_uint4((u32)n2 | ((u32)nv2 << 16), 0u, 0u, 0u);
-    i64* flux2 = (i64*)(dst + 16);
+    int ins = 0;   // a new arc goes where the ascending order puts it
+    if (!ch.in_supp)
+        for (int base = 0; base < P.n_supp; base += 32) {
+            const int t = base + lane;
+            ins += __popc(__ballot_sync(FULL, t < P.n_supp && (int)P.arc[t] < ch.a));
+        }
+    if (lane == 0) {
+        uint4* h4 = (uint4*)dst;
+        h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)ch.n_unb, (u32)ch.hs, (u32)(ch.hs >> 32));
+        h4[1] = make_uint4((u32)ch.hv, (u32)(ch.hv >> 32), 0u, 0u);
+    }
+    i64* flux2 = (i64*)(dst + kHdr);
     u64* vis2 = (u64*)(flux2 + n2);
     u16* arc2 = (u16*)(vis2 + nv2);
-    for (int t = lane; t < P.n_supp; t += GW) {
+    for (int t = lane; t < P.n_supp; t += 32) {
         u64 F = t == ch.ia ? ch.T : ch.k * (u64)P.flux[t];
         if (ch.g2 > 1) F /= ch.g2;
-        const int pos = t + ((!ch.in_supp && t >= ch.ins) ? 1 : 0);
+        const int pos = t + ((!ch.in_supp && t >= ins) ? 1 : 0);
         flux2[pos] = (i64)F;
         arc2[pos] = P.arc[t];
     }
-    if (!ch.in_supp && lane == 0) { flux2[ch.ins] = (i64)ch.T; arc2[ch.ins] = (u16)ch.a; }
+    if (!ch.in_supp && lane == 0) { flux2[ins] = (i64)ch.T; arc2[ins] = (u16)ch.a; }
     if (!to_cand) {
-        for (int u = lane; u < P.n_vis; u += GW) vis2[u] = (!first && u == vk) ? newrec : P.vis[u];
+        for (int u = lane; u < P.n_vis; u += 32) vis2[u] = (!first && u == vk) ? newrec : P.vis[u];
         if (first && lane == 0) vis2[P.n_vis] = newrec;
     }
 }
 
-template <int GW, int MODE, bool ROOTS>
+// Per-warp chunked reservation of beam-key slots: one atomic per kKeyChunk keys instead of one per child.
+struct KeyOut {
+    u64 base; u32 left;
+    __device__ __forceinline__ void push(const ExpandArgs& A, int lane, bool want, u64 key) {
+        const u32 m = __ballot_sync(FULL, want);
+        const u32 cnt = (u32)__popc(m);
+        if (cnt == 0) return;
+        if (cnt > left) {
+            for (u32 t = lane; t < left; t += 32) A.keys[base + t] = kKeySentinel;
+            u64 b = 0;
+            if (lane == 0) b = atomicAdd(&A.ctl->n_slots, (u64)kKeyChunk);
+            b = w_bcast(b, 0);
+            if (b + kKeyChunk > A.max_keys) {
+                if (lane == 0) atomicOr(&A.ctl->error, (u32)ERR_KEYS);
+                left = 0;
+                return;
+            }
+            base = b; left = kKeyChunk;
+        }
+        if (want) A.keys[base + __popc(m & ((1u << lane) - 1u))] = key;
+        base += cnt; left -= cnt;
+    }
+    __device__ __forceinline__ void finish(const ExpandArgs& A, int lane) {
+        for (u32 t = lane; t < left; t += 32) A.keys[base + t] = kKeySentinel;
+        left = 0;
+    }
+};
+
+// gcd(E, c), E / gcd and c / gcd for the small coefficients of the fast path (c < 2^20); c = 2, 3 without a division
+__device__ __forceinline__ void scale_small(u64 absE, u32 c, u32& k, u64& d) {
+    if (c == 2) { const bool ev = (absE & 1ULL) == 0; k = ev ? 1u : 2u; d = ev ? absE >> 1 : absE; return; }
+    if (c == 3) { const u64 qd = absE / 3ULL; const bool dv = qd * 3ULL == absE; k = dv ? 1u : 3u; d = dv ? qd : absE; return; }
+    const u32 gg = (u32)gcd64(absE % (u64)c, (u64)c);
+    k = c / gg; d = absE / (u64)gg;
+}
+
+template <int MODE, bool ROOTS>
 __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevGraph& g = A.g;
-    const int lane = threadIdx.x % GW;
-    const int gib = threadIdx.x / GW;
-    constexpr int GPB = kBlock / GW;
-    const int shift = (threadIdx.x & 31) / GW * GW;
-    const u32 gmask = GW == 32 ? 0xffffffffu : (((1u << GW) - 1u) << shift);
-    unsigned char* gs = smem + (size_t)gib * A.sm_group;
+    const int lane = threadIdx.x & 31;
+    const int wib = threadIdx.x >> 5;
+    unsigned char* gs = smem + (size_t)wib * A.sm_group;
     uint4* stage = (uint4*)gs;
     Parent P;
     P.EF = (i64*)(gs + A.sm_EF);
     P.sbits = (u32*)(gs + A.sm_sbits);
     P.mseen = (u32*)(gs + A.sm_mseen);
-    for (int i = lane; i < g.M; i += GW) P.EF[i] = 0;
-    for (int i = lane; i < g.W32; i += GW) P.sbits[i] = 0;
-    for (int i = lane; i < g.M32; i += GW) P.mseen[i] = 0;
-    __syncwarp(gmask);
+    for (int i = lane; i < g.M; i += 32) P.EF[i] = 0;
+    for (int i = lane; i < g.W32; i += 32) P.sbits[i] = 0;
+    for (int i = lane; i < g.M32; i += 32) P.mseen[i] = 0;
+    __syncwarp();
 
     Ctl* ctl = A.ctl;
     const bool notrunc = MODE == MODE_WRITE ? ctl->notrunc != 0 : true;
     const u64 X = MODE == MODE_WRITE ? ctl->X : 0;
+    const bool fast_graph = !A.no_fast && g.max_coef < kSmallCoef;
 
-    u64 st[ST_COUNT];
-#pragma unroll
-    for (int i = 0; i < ST_COUNT; ++i) st[i] = 0;
-    u64 l_done = 0, l_children = 0, l_expanded = 0;
+    // warp-uniform counters, flushed once per warp
+    u64 s_expanded = 0, s_children = 0, s_done = 0, s_active = 0, s_dead = 0, s_notefm = 0, s_nonpos = 0, s_ovf = 0,
+        s_visited = 0, s_bytes = 0;
+    KeyOut ko; ko.base = 0; ko.left = 0;
     const u32 slot_chunks = A.stride / 16;
 
-    for (u64 p = (u64)blockIdx.x * GPB + gib; p < A.n_cur; p += (u64)gridDim.x * GPB) {
-        // ---- stage the parent: the first GW 16-byte chunks speculatively, the rest once the header is known
+    for (u64 p = (u64)blockIdx.x * kWarps + wib; p < A.n_cur; p += (u64)gridDim.x * kWarps) {
+        // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
         const uint4* src = (const uint4*)(A.cur + p * A.stride);
         uint4 first = make_uint4(0, 0, 0, 0);
         if ((u32)lane < slot_chunks) first = __ldg(src + lane);
-        const u32 hdr = __shfl_sync(gmask, first.x, 0, GW);
+        const u32 hdr = __shfl_sync(FULL, first.x, 0);
         P.n_supp = (int)(hdr & 0xffffu);
         P.n_vis = (int)(hdr >> 16);
         const u32 nch = entry_bytes((u32)P.n_supp, (u32)P.n_vis) / 16;
         if ((u32)lane < nch) stage[lane] = first;
-        for (u32 c = lane + GW; c < nch; c += GW) stage[c] = __ldg(src + c);
-        __syncwarp(gmask);
-        P.flux = (const i64*)(stage + 1);
+        for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldg(src + c);
+        __syncwarp();
+        P.hs = ((const u64*)stage)[1];
+        P.hv = ((const u64*)stage)[2];
+        P.flux = (const i64*)(gs + kHdr);
         P.vis = (const u64*)(P.flux + P.n_supp);
         P.arc = (const u16*)(P.vis + P.n_vis);
 
-        // ---- Eq 2: scatter s_ia f_a into the dense EF array; support bitset; hash sums; largest flux
-        u64 hs = 0, hv = 0, fmax = 0;
-        for (int t = lane; t < P.n_supp; t += GW) {
+        // ---- Eq 2: scatter s_ia f_a into the dense EF array; support bitset; touched-metabolite bitset; largest flux
+        u64 fmax = 0;
+        for (int t = lane; t < P.n_supp; t += 32) {
             const u32 a = P.arc[t];
             const i64 f = P.flux[t];
             atomicOr(&P.sbits[a >> 5], 1u << (a & 31));
-            const int q1 = g.col_ptr[a + 1];
-            for (int q = g.col_ptr[a]; q < q1; ++q) {
+            const int q1 = __ldg(&g.col_ptr[a + 1]);
+            for (int q = __ldg(&g.col_ptr[a]); q < q1; ++q) {
                 const int2 e = __ldg(&g.col[q]);
                 atomicAdd((u64*)&P.EF[e.x], (u64)((i64)e.y * f));
+                atomicOr(&P.mseen[e.x >> 5], 1u << (e.x & 31));
             }
-            if (MODE != MODE_DIRECT) hs += arc_term(a, (u64)f);
             fmax = max(fmax, (u64)f);
         }
-        if (MODE != MODE_DIRECT) {
-            for (int u = lane; u < P.n_vis; u += GW) hv += vis_term(P.vis[u]);
-            hs = g_sum<GW>(hs, gmask);
-            hv = g_sum<GW>(hv, gmask);
-        }
-        fmax = g_max<GW>(fmax, gmask);
-        __syncwarp(gmask);
+        fmax = w_max(fmax);
+        __syncwarp();
         // ---- PROC0: lowest unbalanced metabolite i*, number of unbalanced metabolites, largest |EF|
         int imin = INT_MAX, cnt = 0;
         u64 maxabs = 0;
-        for (int t = lane; t < P.n_supp; t += GW) {
-            const u32 a = P.arc[t];
-            const int q1 = g.col_ptr[a + 1];
-            for (int q = g.col_ptr[a]; q < q1; ++q) {
-                const int i = __ldg(&g.col[q]).x;
+        for (int w = lane; w < g.M32; w += 32) {
+            u32 bits = P.mseen[w];
+            while (bits) {
+                const int i = w * 32 + __ffs(bits) - 1;
+                bits &= bits - 1;
                 const i64 v = P.EF[i];
                 if (v != 0) {
                     imin = min(imin, i);
                     maxabs = max(maxabs, (u64)(v < 0 ? -v : v));
-                    const u32 bit = 1u << (i & 31);
-                    const u32 old = atomicOr(&P.mseen[i >> 5], bit);
-                    cnt += (old & bit) ? 0 : 1;
+                    ++cnt;
                 }
             }
         }
-        imin = g_min<GW>(imin, gmask);
-        cnt = g_sum<GW>(cnt, gmask);
-        maxabs = g_max<GW>(maxabs, gmask);
-        P.hs = hs; P.hv = hv; P.fmax = fmax; P.maxabsEF = maxabs; P.n_unb = cnt; P.istar = imin;
+        imin = __reduce_min_sync(FULL, imin);
+        cnt = __reduce_add_sync(FULL, cnt);
+        maxabs = w_max(maxabs);
+        P.fmax = fmax; P.maxabsEF = maxabs; P.n_unb = cnt; P.istar = imin;
 
         if (ROOTS) {
             // level 0: classify the root itself (arbiter "Done")
             const bool done = cnt == 0;
-            const u64 key = beam_key((u32)cnt, mix64(hs + hv));
+            const u64 key = beam_key((u32)cnt, mix64(P.hs + P.hv));
             if (MODE == MODE_COUNT) {
-                if (done) l_done++;
-                else {
-                    u64 ks = 0;
-                    if (lane == 0) ks = atomicAdd(&ctl->n_keys, 1ULL);
-                    ks = __shfl_sync(gmask, ks, 0, GW);
-                    if (ks < A.max_keys) { if (lane == 0) A.keys[ks] = key; }
-                    else if (lane == 0) atomicOr(&ctl->error, (u32)ERR_KEYS);
-                }
+                if (done) s_done++;
+                else { s_active++; ko.push(A, lane, lane == 0, key); }
             } else if (done || notrunc || key < X) {
                 u64 slot = 0;
                 if (lane == 0) slot = atomicAdd(done ? &ctl->n_cand : &ctl->n_next, 1ULL);
-                slot = __shfl_sync(gmask, slot, 0, GW);
+                slot = w_bcast(slot, 0);
                 if (slot >= (done ? A.max_cand : A.max_frontier)) {
                     if (lane == 0) atomicOr(&ctl->error, (u32)(done ? ERR_CAND : ERR_FRONTIER));
                 } else {
                     unsigned char* dst = done ? A.cand + slot * A.cand_stride : A.nxt + slot * A.stride;
-                    if (lane == 0) *(uint4*)dst = make_uint4((u32)P.n_supp | ((u32)(done ? 0 : P.n_vis) << 16), 0u, 0u, 0u);
-                    i64* flux2 = (i64*)(dst + 16);
+                    const int nv2 = done ? 0 : P.n_vis;
+                    if (lane == 0) {
+                        uint4* h4 = (uint4*)dst;
+                        h4[0] = make_uint4((u32)P.n_supp | ((u32)nv2 << 16), (u32)cnt, (u32)P.hs, (u32)(P.hs >> 32));
+                        h4[1] = make_uint4((u32)P.hv, (u32)(P.hv >> 32), 0u, 0u);
+                    }
+                    i64* flux2 = (i64*)(dst + kHdr);
                     u64* vis2 = (u64*)(flux2 + P.n_supp);
-                    u16* arc2 = (u16*)(vis2 + (done ? 0 : P.n_vis));
-                    for (int t = lane; t < P.n_supp; t += GW) { flux2[t] = P.flux[t]; arc2[t] = P.arc[t]; }
-                    if (!done) for (int u = lane; u < P.n_vis; u += GW) vis2[u] = P.vis[u];
+                    u16* arc2 = (u16*)(vis2 + nv2);
+                    for (int t = lane; t < P.n_supp; t += 32) { flux2[t] = P.flux[t]; arc2[t] = P.arc[t]; }
+                    for (int u = lane; u < nv2; u += 32) vis2[u] = P.vis[u];
                 }
             }
         } else {
             P.E = P.EF[imin];
             const int istar = imin;
             const bool fwd = P.E > 0;
-            if (MODE != MODE_WRITE) { l_expanded++; st[ST_EXPANDED]++; st[ST_ALGO_BYTES] += algo_entry_bytes((u32)P.n_supp, (u32)P.n_vis); }
+            const u64 absE = (u64)(fwd ? P.E : -P.E);
+            if (MODE != MODE_WRITE) { s_expanded++; s_bytes += algo_entry_bytes((u32)P.n_supp, (u32)P.n_vis); }
             // visited?
             int vk = -1;
-            for (int u = lane; u < P.n_vis; u += GW) if ((int)((P.vis[u] >> 32) & 0xffffu) == istar) vk = u;
-            vk = g_max<GW>(vk, gmask);
-            const int in0 = g.in_ptr[istar], nI = g.in_ptr[istar + 1] - in0;
-            const int out0 = g.out_ptr[istar], nO = g.out_ptr[istar + 1] - out0;
+            for (int base = 0; base < P.n_vis && vk < 0; base += 32) {
+                const int u = base + lane;
+                const u32 hit = __ballot_sync(FULL, u < P.n_vis && (int)((P.vis[u] >> 32) & 0xffffu) == istar);
+                if (hit) vk = base + __ffs(hit) - 1;
+            }
+            const int in0 = __ldg(&g.in_ptr[istar]), nI = __ldg(&g.in_ptr[istar + 1]) - in0;
+            const int out0 = __ldg(&g.out_ptr[istar]), nO = __ldg(&g.out_ptr[istar + 1]) - out0;
 
-            // shared tail: account for / emit one evaluated child
-            auto emit = [&](const Child& ch, bool first, u64 newrec) {
-                if (ch.status != CH_OK) {
-                    if (MODE != MODE_WRITE) st[ch.status == CH_OVERFLOW ? ST_OVERFLOW : ST_NONPOS]++;
-                    return;
-                }
-                if (MODE != MODE_WRITE) { st[ST_CHILDREN]++; l_children++; st[ST_ALGO_BYTES] += 8; if (ch.done) l_done++; }
-                if (MODE == MODE_COUNT) {
-                    if (!ch.done) {
-                        u64 ks = 0;
-                        if (lane == 0) ks = atomicAdd(&ctl->n_keys, 1ULL);
-                        ks = __shfl_sync(gmask, ks, 0, GW);
-                        if (ks < A.max_keys) { if (lane == 0) A.keys[ks] = ch.key; }
-                        else if (lane == 0) atomicOr(&ctl->error, (u32)ERR_KEYS);
-                    }
-                    return;
-                }
-                const bool keep = ch.done || MODE == MODE_DIRECT || notrunc || ch.key < X;
-                if (!keep) return;
+            // materialise one kept child (warp-uniform description)
+            auto place = [&](const Child& ch, bool first, u64 newrec) {
                 const int n2 = P.n_supp + (ch.in_supp ? 0 : 1), nv2 = P.n_vis + (first ? 1 : 0);
-                st[ST_ALGO_BYTES] += algo_entry_bytes((u32)n2, (u32)nv2);
+                s_bytes += algo_entry_bytes((u32)n2, (u32)nv2);
                 u64 slot = 0;
                 if (lane == 0) slot = atomicAdd(ch.done ? &ctl->n_cand : &ctl->n_next, 1ULL);
-                slot = __shfl_sync(gmask, slot, 0, GW);
+                slot = w_bcast(slot, 0);
                 if (slot >= (ch.done ? A.max_cand : A.max_frontier)) {
                     if (lane == 0) atomicOr(&ctl->error, (u32)(ch.done ? ERR_CAND : ERR_FRONTIER));
                     return;
                 }
                 unsigned char* dst = ch.done ? A.cand + slot * A.cand_stride : A.nxt + slot * A.stride;
-                write_child<GW>(dst, P, ch, lane, first, vk, newrec, ch.done);
+                write_child(dst, P, ch, lane, first, vk, newrec, ch.done);
+            };
+            // account for / emit one child evaluated by the general routine
+            auto emit = [&](const Child& ch, bool first, u64 newrec) {
+                if (ch.status != CH_OK) {
+                    if (MODE != MODE_WRITE) { if (ch.status == CH_OVERFLOW) s_ovf++; else s_nonpos++; }
+                    return;
+                }
+                if (MODE != MODE_WRITE) { s_children++; s_bytes += 8; if (ch.done) s_done++; }
+                const u64 key = beam_key((u32)ch.n_unb, mix64(ch.hs + ch.hv));
+                if (MODE == MODE_COUNT) {
+                    if (!ch.done) { s_active++; ko.push(A, lane, lane == 0, key); }
+                    return;
+                }
+                if (ch.done || MODE == MODE_DIRECT || notrunc || key < X) place(ch, first, newrec);
             };
 
             if (vk < 0) {
                 // ---- first visit: PROC1 / PROC1' (Eq 3; readings G1, G13, G14, G15, G22)
                 if (P.n_vis >= A.V) {
-                    if (MODE != MODE_WRITE) st[ST_VISITED]++;
+                    if (MODE != MODE_WRITE) s_visited++;
                 } else {
                     // primary on the side the flux arrives from: lowest arc of that side in the support (G13)
                     const int2* plist = fwd ? g.in_e + in0 : g.out_e + out0;
                     const int plen = fwd ? nI : nO;
                     int prim = -1;
-                    for (int base = 0; base < plen && prim < 0; base += GW) {
+                    for (int base = 0; base < plen && prim < 0; base += 32) {
                         const int q = base + lane;
                         const int pa = q < plen ? __ldg(&plist[q]).x : -1;
-                        const u32 bal = g_ballot<GW>(pa >= 0 && sbit(P.sbits, pa), gmask, shift);
-                        if (bal) prim = __shfl_sync(gmask, pa, __ffs(bal) - 1, GW);
+                        const u32 bal = __ballot_sync(FULL, pa >= 0 && sbit(P.sbits, pa));
+                        if (bal) prim = __shfl_sync(FULL, pa, __ffs(bal) - 1);
                     }
                     const int2* alist = fwd ? g.out_e + out0 : g.in_e + in0;
                     const int alen = fwd ? nO : nI;
+                    const bool fastP = fast_graph && fmax < kSmall && maxabs < kSmall;
+                    u64 kc_k0 = 0, kc_s0 = 0, kc_k1 = 0, kc_s1 = 0;   // hash sums of the k-scaled support, last two k
                     int n_adm = 0;
-                    for (int base = 0; base < alen; base += GW) {
+                    for (int base = 0; base < alen; base += 32) {
                         const int q = base + lane;
-                        int2 e = make_int2(-1, 0);
-                        bool adm = false;
+                        int a = -1, c = 1;
+                        bool adm = false, insup = false;
                         if (q < alen) {
-                            e = __ldg(&alist[q]);
-                            const int tw = __ldg(&g.twin[e.x]);
-                            adm = !(tw >= 0 && sbit(P.sbits, tw)) && (sbit(P.sbits, e.x) || P.n_supp < A.D);
+                            const int2 e = __ldg(&alist[q]);
+                            a = e.x; c = e.y;
+                            const int tw = __ldg(&g.twin[a]);
+                            insup = sbit(P.sbits, a);
+                            adm = !(tw >= 0 && sbit(P.sbits, tw)) && (insup || P.n_supp < A.D);
                         }
-                        u32 bal = g_ballot<GW>(adm, gmask, shift);
-                        n_adm += __popc(bal);
-                        while (bal) {
-                            const int l = __ffs(bal) - 1;
-                            bal &= bal - 1;
-                            const int a = __shfl_sync(gmask, e.x, l, GW);
-                            const int c = __shfl_sync(gmask, e.y, l, GW);
+                        const u32 adm_m = __ballot_sync(FULL, adm);
+                        if (adm_m == 0) continue;
+                        n_adm += __popc(adm_m);
+                        // ---- lane-parallel evaluation: new arc, small integers => no overflow, no common factor
+                        const bool fast = adm && !insup && fastP;
+                        const u32 fast_m = __ballot_sync(FULL, fast);
+                        u32 k = 1; u64 d = absE;
+                        int nu2 = cnt;
+                        if (fast) {
+                            if (c != 1) scale_small(absE, (u32)c, k, d);
+                            const int q1 = __ldg(&g.col_ptr[a + 1]);
+                            for (int qq = __ldg(&g.col_ptr[a]); qq < q1; ++qq) {
+                                const int2 e = __ldg(&g.col[qq]);
+                                const i64 efp = P.EF[e.x];
+                                const i64 x = (i64)k * efp + (i64)d * (i64)e.y;   // |.| < 2^60 + 2^60
+                                nu2 += (int)(x != 0) - (int)(efp != 0);
+                            }
+                        }
+                        u64 hsb = P.hs;
+                        u32 need = __ballot_sync(FULL, fast && k > 1);
+                        while (need) {
+                            const u32 kk = __shfl_sync(FULL, k, __ffs(need) - 1);
+                            u64 s;
+                            if ((u64)kk == kc_k0) s = kc_s0;
+                            else if ((u64)kk == kc_k1) s = kc_s1;
+                            else {
+                                s = 0;
+                                for (int t = lane; t < P.n_supp; t += 32) s += arc_term_t(g, (u32)P.arc[t], (u64)kk * (u64)P.flux[t]);
+                                s = w_sum(s);
+                                kc_k1 = kc_k0; kc_s1 = kc_s0; kc_k0 = kk; kc_s0 = s;
+                            }
+                            const bool same = fast && k == kk;
+                            if (same) hsb = s;
+                            need &= ~__ballot_sync(FULL, same);
+                        }
+                        u64 hs2 = 0, hv2 = 0, key = 0;
+                        bool done = false;
+                        if (fast) {
                             const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : a), (u32)(fwd ? a : prim), 0u);
+                            hs2 = hsb + arc_term_t(g, (u32)a, d);
+                            hv2 = P.hv + vis_term(newrec);
+                            key = beam_key((u32)nu2, mix64(hs2 + hv2));
+                            done = nu2 == 0;
+                        }
+                        const u32 done_m = __ballot_sync(FULL, done);
+                        if (MODE != MODE_WRITE) {
+                            const int nf = __popc(fast_m);
+                            s_children += nf; s_bytes += 8 * nf; s_done += __popc(done_m);
+                        }
+                        if (MODE == MODE_COUNT) {
+                            s_active += __popc(fast_m & ~done_m);
+                            ko.push(A, lane, fast && !done, key);
+                        } else {
+                            u32 keep_m = __ballot_sync(FULL, fast && (done || MODE == MODE_DIRECT || notrunc || key < X));
+                            while (keep_m) {
+                                const int l = __ffs(keep_m) - 1;
+                                keep_m &= keep_m - 1;
+                                Child ch;
+                                ch.status = CH_OK; ch.in_supp = false; ch.ia = -1; ch.g2 = 1;
+                                ch.a = __shfl_sync(FULL, a, l);
+                                ch.k = __shfl_sync(FULL, k, l);
+                                ch.T = w_bcast(d, l);
+                                ch.hs = w_bcast(hs2, l);
+                                ch.hv = w_bcast(hv2, l);
+                                ch.n_unb = __shfl_sync(FULL, nu2, l);
+                                ch.done = ch.n_unb == 0;
+                                const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : ch.a), (u32)(fwd ? ch.a : prim), 0u);
+                                place(ch, true, newrec);
+                            }
+                        }
+                        // ---- everything else through the general routine
+                        u32 slow_m = adm_m & ~fast_m;
+                        while (slow_m) {
+                            const int l = __ffs(slow_m) - 1;
+                            slow_m &= slow_m - 1;
+                            const int sa = __shfl_sync(FULL, a, l);
+                            const int sc = __shfl_sync(FULL, c, l);
+                            const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : sa), (u32)(fwd ? sa : prim), 0u);
                             Child ch;
-                            eval_child<GW, MODE != MODE_DIRECT>(g, P, lane, gmask, a, c, +1, true, 0ULL, newrec, ch);
+                            eval_child(g, P, lane, sa, sc, +1, true, 0ULL, newrec, ch);
                             emit(ch, true, newrec);
                         }
                     }
-                    if (n_adm == 0 && MODE != MODE_WRITE) st[ST_DEAD_END]++;
+                    if (n_adm == 0 && MODE != MODE_WRITE) s_dead++;
                 }
             } else {
                 // ---- revisit: PROC2-4 (readings G2-G5)
                 const u64 rec = P.vis[vk];
                 const int cntv = (int)(rec >> 48) + 1;
                 if (cntv > A.max_loop) {
-                    if (MODE != MODE_WRITE) st[ST_NOT_EFM]++;
+                    if (MODE != MODE_WRITE) s_notefm++;
                 } else {
                     const int PI = (int)((rec >> 16) & 0xffffu), PO = (int)(rec & 0xffffu);
                     int lPI = -1, lPO = -1, cPI = 0, cPO = 0;
-                    for (int q = lane; q < nI; q += GW) { const int2 e = __ldg(&g.in_e[in0 + q]); if (e.x == PI) { lPI = q; cPI = e.y; } }
-                    for (int q = lane; q < nO; q += GW) { const int2 e = __ldg(&g.out_e[out0 + q]); if (e.x == PO) { lPO = q; cPO = e.y; } }
-                    lPI = g_max<GW>(lPI, gmask); cPI = g_max<GW>(cPI, gmask);
-                    lPO = g_max<GW>(lPO, gmask); cPO = g_max<GW>(cPO, gmask);
+                    for (int q = lane; q < nI; q += 32) { const int2 e = __ldg(&g.in_e[in0 + q]); if (e.x == PI) { lPI = q; cPI = e.y; } }
+                    for (int q = lane; q < nO; q += 32) { const int2 e = __ldg(&g.out_e[out0 + q]); if (e.x == PO) { lPO = q; cPO = e.y; } }
+                    lPI = __reduce_max_sync(FULL, lPI); cPI = __reduce_max_sync(FULL, cPI);
+                    lPO = __reduce_max_sync(FULL, lPO); cPO = __reduce_max_sync(FULL, cPO);
                     // Def 11: forward PO ~ SI, backward PI ~ SO, secondary = any arc of that side in the support (G5)
                     bool dep = false;
-                    const i64 doff = g.dep_off[istar];
+                    const i64 doff = __ldg(&g.dep_off[istar]);
                     if (fwd) {
-                        for (int q = lane; q < nI; q += GW) {
+                        for (int q = lane; q < nI; q += 32) {
                             const i64 b = doff + (i64)lPO * nI + q;
                             dep = dep || (sbit(P.sbits, __ldg(&g.in_e[in0 + q]).x) && ((__ldg(&g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
                         }
                     } else {
-                        for (int q = lane; q < nO; q += GW) {
+                        for (int q = lane; q < nO; q += 32) {
                             const i64 b = doff + (i64)q * nI + lPI;
                             dep = dep || (sbit(P.sbits, __ldg(&g.out_e[out0 + q]).x) && ((__ldg(&g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
                         }
                     }
-                    dep = g_ballot<GW>(dep, gmask, 0) != 0;
+                    dep = __any_sync(FULL, dep);
                     int a, c, sign;
                     if (fwd) { if (!dep) { a = PO; c = cPO; sign = +1; } else { a = PI; c = cPI; sign = -1; } }   // Eq 4 / Eq 5
                     else     { if (!dep) { a = PI; c = cPI; sign = +1; } else { a = PO; c = cPO; sign = -1; } }
                     const u64 newrec = vis_pack((u32)istar, (u32)PI, (u32)PO, (u32)cntv);
                     Child ch;
-                    eval_child<GW, MODE != MODE_DIRECT>(g, P, lane, gmask, a, c, sign, false, rec, newrec, ch);
+                    eval_child(g, P, lane, a, c, sign, false, rec, newrec, ch);
                     emit(ch, false, newrec);
                 }
             }
         }
         // ---- restore the shared scratch to zero for the next parent
-        __syncwarp(gmask);
-        for (int t = lane; t < P.n_supp; t += GW) {
-            const u32 a = P.arc[t];
-            P.sbits[a >> 5] = 0;
-            const int q1 = g.col_ptr[a + 1];
-            for (int q = g.col_ptr[a]; q < q1; ++q) { const int i = __ldg(&g.col[q]).x; P.EF[i] = 0; P.mseen[i >> 5] = 0; }
+        __syncwarp();
+        for (int t = lane; t < P.n_supp; t += 32) P.sbits[P.arc[t] >> 5] = 0;
+        for (int w = lane; w < g.M32; w += 32) {
+            u32 bits = P.mseen[w];
+            while (bits) { P.EF[w * 32 + __ffs(bits) - 1] = 0; bits &= bits - 1; }
+            P.mseen[w] = 0;
         }
-        __syncwarp(gmask);
+        __syncwarp();
     }
+    if (MODE == MODE_COUNT) ko.finish(A, lane);
     if (lane == 0) {
-#pragma unroll
-        for (int i = 0; i < ST_COUNT; ++i) if (st[i]) atomicAdd(&ctl->st[i], st[i]);
-        if (l_done) atomicAdd(&ctl->lvl_done, l_done);
-        if (l_children) atomicAdd(&ctl->lvl_children, l_children);
-        if (l_expanded) atomicAdd(&ctl->lvl_expanded, l_expanded);
+        u64* st = ctl->st;
+        if (s_expanded) { atomicAdd(&st[ST_EXPANDED], s_expanded); atomicAdd(&ctl->lvl_expanded, s_expanded); }
+        if (s_children) { atomicAdd(&st[ST_CHILDREN], s_children); atomicAdd(&ctl->lvl_children, s_children); }
+        if (s_done) atomicAdd(&ctl->lvl_done, s_done);
+        if (s_active) atomicAdd(&ctl->n_keys, s_active);
+        if (s_dead) atomicAdd(&st[ST_DEAD_END], s_dead);
+        if (s_notefm) atomicAdd(&st[ST_NOT_EFM], s_notefm);
+        if (s_nonpos) atomicAdd(&st[ST_NONPOS], s_nonpos);
+        if (s_ovf) atomicAdd(&st[ST_OVERFLOW], s_ovf);
+        if (s_visited) atomicAdd(&st[ST_VISITED], s_visited);
+        if (s_bytes) atomicAdd(&st[ST_ALGO_BYTES], s_bytes);
     }
 }
 
 __global__ void k_level_begin(Ctl* ctl) {
-    ctl->n_next = 0; ctl->n_keys = 0; ctl->lvl_done = 0; ctl->lvl_children = 0; ctl->lvl_expanded = 0;
+    ctl->n_next = 0; ctl->n_keys = 0; ctl->n_slots = 0; ctl->lvl_done = 0; ctl->lvl_children = 0; ctl->lvl_expanded = 0;
 }
 
 // ------------------------------------------------------------------ host launchers
@@ -497,36 +610,40 @@ void expand_smem_layout(ExpandArgs& a) {
     a.sm_group = (u32)off;
 }
 
-template <int GW, int MODE, bool ROOTS>
+// key slots the count pass can leave unused: every warp of the largest grid may strand one chunk
+constexpr u64 kMaxGrid = 16384;
+u64 expand_key_slack() { return kMaxGrid * kWarps * kKeyChunk; }
+
+template <int MODE, bool ROOTS>
 static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
-    const int gpb = kBlock / GW;
-    const size_t smem = (size_t)a.sm_group * gpb;
+    const size_t smem = (size_t)a.sm_group * kWarps;
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_expand<GW, MODE, ROOTS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_expand<MODE, ROOTS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    u64 need = (a.n_cur + gpb - 1) / gpb;
+    u64 need = (a.n_cur + kWarps - 1) / kWarps;
     int bps = (int)((227 * 1024) / (smem + 1024));
     if (bps > 16) bps = 16;
     if (bps < 1) bps = 1;
     u64 cap = (u64)sm_count * bps * 4;
+    if (cap > kMaxGrid) cap = kMaxGrid;
     unsigned grid = (unsigned)(need < cap ? need : cap);
     if (grid == 0) grid = 1;
-    k_expand<GW, MODE, ROOTS><<<grid, kBlock, smem, s>>>(a);
+    k_expand<MODE, ROOTS><<<grid, kBlock, smem, s>>>(a);
     return cudaGetLastError();
 }
 
 cudaError_t launch_expand(int mode, bool roots, const ExpandArgs& a, int sm_count, cudaStream_t s) {
     if (roots) {
-        if (mode == MODE_COUNT) return launch_t<32, MODE_COUNT, true>(a, sm_count, s);
-        return launch_t<32, MODE_WRITE, true>(a, sm_count, s);
+        if (mode == MODE_COUNT) return launch_t<MODE_COUNT, true>(a, sm_count, s);
+        return launch_t<MODE_WRITE, true>(a, sm_count, s);
     }
-    if (mode == MODE_COUNT) return launch_t<32, MODE_COUNT, false>(a, sm_count, s);
-    if (mode == MODE_WRITE) return launch_t<32, MODE_WRITE, false>(a, sm_count, s);
-    return launch_t<32, MODE_DIRECT, false>(a, sm_count, s);
+    if (mode == MODE_COUNT) return launch_t<MODE_COUNT, false>(a, sm_count, s);
+    if (mode == MODE_WRITE) return launch_t<MODE_WRITE, false>(a, sm_count, s);
+    return launch_t<MODE_DIRECT, false>(a, sm_count, s);
 }
 
 cudaError_t launch_level_begin(Ctl* ctl, cudaStream_t s) {

@@ -10,7 +10,7 @@ namespace efm {
 // of a round (ticket) scans the global histogram and narrows the prefix.  No host round trip.
 // =================================================================================================================
 __global__ void k_select_init(Ctl* ctl, u64 cap) {
-    const u64 n = ctl->n_keys;
+    const u64 n = ctl->n_keys;   // valid keys; the slot array may also hold kKeySentinel fillers
     ctl->notrunc = (cap == 0 || n <= cap) ? 1u : 0u;
     ctl->sel_prefix = 0; ctl->sel_rank = cap; ctl->sel_ticket = 0; ctl->X = 0;
 }
@@ -22,10 +22,11 @@ __global__ void __launch_bounds__(256) k_select_round(const u64* __restrict__ ke
     const int nb = 1 << bits;
     for (int b = threadIdx.x; b < nb; b += blockDim.x) h[b] = 0;
     __syncthreads();
-    const u64 n = min(ctl->n_keys, max_keys);   // an overflowed key array is reported by the host (ERR_KEYS)
+    const u64 n = min(ctl->n_slots, max_keys);   // an overflowed key array is reported by the host (ERR_KEYS)
     const u64 prefix = ctl->sel_prefix;
     for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
         const u64 key = keys[i];
+        if (key == kKeySentinel) continue;   // filler of a reserved, unused slot
         if (first || (key >> (shift + bits)) == prefix) atomicAdd(&h[(key >> shift) & (u64)(nb - 1)], 1u);
     }
     __syncthreads();
@@ -74,9 +75,9 @@ cudaError_t launch_select(const u64* keys, Ctl* ctl, u64 cap, u64 max_keys, u64 
 // sparse form).  The first candidate to claim a slot represents its support; a later candidate with the same support
 // and a different coprime flux vector poisons it (reading G18) -- order-independent.
 // =================================================================================================================
-__device__ __forceinline__ const i64* cand_flux(const unsigned char* e) { return (const i64*)(e + 16); }
+__device__ __forceinline__ const i64* cand_flux(const unsigned char* e) { return (const i64*)(e + kHdr); }
 __device__ __forceinline__ int cand_n(const unsigned char* e) { return (int)(*(const u32*)e & 0xffffu); }
-__device__ __forceinline__ const u16* cand_arc(const unsigned char* e, int n) { return (const u16*)(e + 16 + 8 * (size_t)n); }
+__device__ __forceinline__ const u16* cand_arc(const unsigned char* e, int n) { return (const u16*)(e + kHdr + 8 * (size_t)n); }
 
 __global__ void __launch_bounds__(256) k_dedup_insert(const PostArgs a, u64 n_cand) {
     const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;

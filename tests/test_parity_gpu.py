@@ -127,6 +127,15 @@ def test_genome(efm, oracle_mod, cap):
     assert got.stats["truncated_beam"] > 0 and got.stats["output"] > 1000
 
 
+def test_general_routine_only(efm, oracle_mod):
+    """EFM_F_NO_FASTPATH sends every child through the warp-cooperative general routine: both routes must agree
+    with the oracle (and hence with each other)."""
+    for name, over in (("small", {}), ("core", dict(frontier_cap=2048)), ("genome", dict(frontier_cap=256))):
+        assert_parity(efm, oracle_mod, make_network(name, 0), flags=efm.EFM_F_NO_FASTPATH, **over)
+    assert_parity(efm, oracle_mod, make_network("small", 0), flags=efm.EFM_F_NO_FASTPATH | efm.EFM_F_FORCE_TWO_PASS,
+                  frontier_cap=1 << 20)
+
+
 def test_other_seeds_of_the_generator(efm, oracle_mod):
     for name, seed, over in (("small", 1, {}), ("small", 2, dict(frontier_cap=500)), ("core", 1, dict(frontier_cap=4096)),
                              ("mid", 3, dict(frontier_cap=1024))):
