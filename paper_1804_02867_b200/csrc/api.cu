@@ -23,7 +23,7 @@ struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
     Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
-    Region ctl, buf[2], keys, cand, table, isrep, poison, uniq, size_hist, bucket_start, bucket_fill;
+    Region ctl, buf[2], keys, ckeys, cand, table, isrep, poison, uniq, size_hist, bucket_start, bucket_fill;
     Region order, sig, size_sorted, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, dense;
     size_t total = 0;
 };
@@ -83,6 +83,7 @@ void make_layout(efm_handle* h) {
     add_region(L, L.buf[0], (size_t)h->max_frontier * h->stride);
     add_region(L, L.buf[1], (size_t)h->max_frontier * h->stride);
     add_region(L, L.keys, (size_t)h->max_keys * 8);
+    add_region(L, L.ckeys, (size_t)h->max_keys * 8);
     const size_t C = (size_t)h->max_cand;
     add_region(L, L.cand, C * h->cand_stride);
     add_region(L, L.table, h->table_size * 4);
@@ -386,7 +387,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         size_t t0 = tm.mark();
         CK(launch_expand(0, true, ea, h->sm_count, s)); ++launches;
         size_t t1 = tm.mark();
-        CK(launch_select(ea.keys, d_ctl, (u64)h->cap, ea.max_keys, n_roots, h->sm_count, s, &launches));
+        CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), d_ctl, (u64)h->cap, ea.max_keys, n_roots, h->sm_count, s, &launches));
         size_t t2 = tm.mark();
         CK(launch_expand(1, true, ea, h->sm_count, s)); ++launches;
         size_t t3 = tm.mark();
@@ -413,7 +414,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
             size_t t0 = tm.mark();
             CK(launch_expand(0, false, ea, h->sm_count, s)); ++launches;
             size_t t1 = tm.mark();
-            CK(launch_select(ea.keys, d_ctl, (u64)h->cap, ea.max_keys, std::min<u64>(ea.max_keys, n_cur * (u64)G.max_fanout), h->sm_count, s, &launches));
+            CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), d_ctl, (u64)h->cap, ea.max_keys, std::min<u64>(ea.max_keys, n_cur * (u64)G.max_fanout), h->sm_count, s, &launches));
             size_t t2 = tm.mark();
             CK(launch_expand(1, false, ea, h->sm_count, s)); ++launches;
             size_t t3 = tm.mark();

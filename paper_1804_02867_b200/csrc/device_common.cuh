@@ -61,7 +61,7 @@ struct Ctl {
     u32 error;
     u32 notrunc;       // beam does not bind on this level
     u64 X;             // beam threshold: keep key < X
-    u64 sel_prefix, sel_rank;
+    u64 sel_prefix, sel_rank, n_compact;
     u32 sel_ticket, pad0;
     u64 st[ST_COUNT];
     // post-processing counters

@@ -27,7 +27,7 @@ struct PostArgs {
     u32* sort_idx; u64 n_pad;
     int* r_nnz; int* r_rxn; i64* r_val;   // final, lexicographic order
 };
-cudaError_t launch_select(const u64* keys, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches);
+cudaError_t launch_select(const u64* keys, u64* ckeys /*compact buffer, max_keys slots*/, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches);
 cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_launches);
 cudaError_t launch_filter(const PostArgs& a, u64 n_uniq, int sm_count, cudaStream_t s, int* n_launches);
 cudaError_t launch_output_rows(const PostArgs& a, u64 n_uniq, cudaStream_t s, int* n_launches);

@@ -6,67 +6,143 @@ namespace efm {
 
 // =================================================================================================================
 // a-4  Beam select: X = the key at sorted position `cap`; the level keeps exactly {key < X}.
-// MSD radix select over the 64-bit keys, 11/11/11/11/10/10-bit digits, shared-memory histograms; the last block
-// of a round (ticket) scans the global histogram and narrows the prefix.  No host round trip.
+// MSD radix select over the 64-bit keys without a host round trip, three launches:
+//   k_select_hist    histogram of the top 11 bits over all keys; the last block (ticket) finds the bin holding rank cap
+//   k_select_narrow  copies the keys of that bin to a compact buffer; the last block finishes the remaining 53 bits on
+//                    the compact buffer alone (11/11/11/10/10-bit rounds in shared memory)
 // =================================================================================================================
+constexpr int kSelThreads = 256;
+constexpr int kTopBits = 11;
+
 __global__ void k_select_init(Ctl* ctl, u64 cap) {
     const u64 n = ctl->n_keys;   // valid keys; the slot array may also hold kKeySentinel fillers
     ctl->notrunc = (cap == 0 || n <= cap) ? 1u : 0u;
-    ctl->sel_prefix = 0; ctl->sel_rank = cap; ctl->sel_ticket = 0; ctl->X = 0;
+    ctl->sel_prefix = 0; ctl->sel_rank = cap; ctl->sel_ticket = 0; ctl->X = 0; ctl->n_compact = 0;
 }
 
-__global__ void __launch_bounds__(256) k_select_round(const u64* __restrict__ keys, Ctl* ctl, u64 max_keys, int shift, int bits, int first, int last) {
+// Whole block: the bin b with cum(b) <= rank < cum(b) + h[b]; returns through shared memory.
+__device__ void block_find_bin(const u32* h, int nb, u64 rank, u32* s_bin, u64* s_cum, u64* scratch) {
+    const int T = blockDim.x, per = (nb + T - 1) / T, b0 = threadIdx.x * per;
+    u64 sum = 0;
+    for (int j = 0; j < per; ++j) if (b0 + j < nb) sum += h[b0 + j];
+    scratch[threadIdx.x] = sum;
+    if (threadIdx.x == 0) { *s_bin = (u32)(nb - 1); *s_cum = 0; }   // rank beyond the total: unreachable while n_keys > cap
+    __syncthreads();
+    for (int off = 1; off < T; off <<= 1) {
+        const u64 v = threadIdx.x >= off ? scratch[threadIdx.x - off] : 0;
+        __syncthreads();
+        scratch[threadIdx.x] += v;
+        __syncthreads();
+    }
+    const u64 incl = scratch[threadIdx.x];
+    u64 cum = incl - sum;
+    if (cum <= rank && rank < incl)
+        for (int j = 0; j < per; ++j) {
+            const u64 c = h[b0 + j];
+            if (rank < cum + c) { *s_bin = (u32)(b0 + j); *s_cum = cum; break; }
+            cum += c;
+        }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restrict__ keys, Ctl* ctl, u64 max_keys) {
     if (ctl->notrunc) return;
     __shared__ u32 h[SEL_BINS];
-    __shared__ bool is_last;
-    const int nb = 1 << bits;
-    for (int b = threadIdx.x; b < nb; b += blockDim.x) h[b] = 0;
+    __shared__ u64 scratch[kSelThreads];
+    __shared__ u32 s_bin; __shared__ u64 s_cum; __shared__ bool is_last;
+    for (int b = threadIdx.x; b < SEL_BINS; b += kSelThreads) h[b] = 0;
     __syncthreads();
     const u64 n = min(ctl->n_slots, max_keys);   // an overflowed key array is reported by the host (ERR_KEYS)
-    const u64 prefix = ctl->sel_prefix;
-    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
-        const u64 key = keys[i];
-        if (key == kKeySentinel) continue;   // filler of a reserved, unused slot
-        if (first || (key >> (shift + bits)) == prefix) atomicAdd(&h[(key >> shift) & (u64)(nb - 1)], 1u);
+    // keys of one parent are neighbours and share their top bits: aggregate runs of equal bins per thread
+    constexpr int RUN = 4;
+    for (u64 i0 = ((u64)blockIdx.x * kSelThreads + threadIdx.x) * RUN; i0 < n; i0 += (u64)gridDim.x * kSelThreads * RUN) {
+        u32 cur = 0xffffffffu, cnt = 0;
+#pragma unroll
+        for (int j = 0; j < RUN; ++j) {
+            if (i0 + j >= n) break;
+            const u64 key = keys[i0 + j];
+            if (key == kKeySentinel) continue;   // filler of a reserved, unused slot
+            const u32 b = (u32)(key >> (64 - kTopBits));
+            if (b != cur) { if (cnt) atomicAdd(&h[cur], cnt); cur = b; cnt = 0; }
+            ++cnt;
+        }
+        if (cnt) atomicAdd(&h[cur], cnt);
     }
     __syncthreads();
-    for (int b = threadIdx.x; b < nb; b += blockDim.x) if (h[b]) atomicAdd(&ctl->hist[b], h[b]);
+    for (int b = threadIdx.x; b < SEL_BINS; b += kSelThreads) if (h[b]) atomicAdd(&ctl->hist[b], h[b]);
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) is_last = atomicAdd(&ctl->sel_ticket, 1u) == gridDim.x - 1;
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    if (threadIdx.x == 0) {
-        volatile u32* gh = ctl->hist;
-        u64 rank = ctl->sel_rank, cum = 0;
-        int b = 0;
-        for (; b < nb; ++b) { const u64 c = gh[b]; if (rank < cum + c) break; cum += c; }
-        if (b == nb) b = nb - 1;   // unreachable while n_keys > cap
-        ctl->sel_rank = rank - cum;
-        const u64 np = (prefix << bits) | (u64)b;
-        ctl->sel_prefix = np;
-        ctl->sel_ticket = 0;
-        if (last) ctl->X = np;
-    }
+    for (int b = threadIdx.x; b < SEL_BINS; b += kSelThreads) { h[b] = ((volatile u32*)ctl->hist)[b]; ctl->hist[b] = 0; }
     __syncthreads();
-    for (int b = threadIdx.x; b < nb; b += blockDim.x) ctl->hist[b] = 0;
+    block_find_bin(h, SEL_BINS, ctl->sel_rank, &s_bin, &s_cum, scratch);
+    if (threadIdx.x == 0) { ctl->sel_prefix = s_bin; ctl->sel_rank -= s_cum; ctl->sel_ticket = 0; }
 }
 
-cudaError_t launch_select(const u64* keys, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches) {
+__global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __restrict__ keys, u64* __restrict__ ckeys, Ctl* ctl, u64 max_keys) {
+    if (ctl->notrunc) return;
+    __shared__ u32 h[SEL_BINS];
+    __shared__ u64 scratch[kSelThreads];
+    __shared__ u32 s_bin; __shared__ u64 s_cum; __shared__ bool is_last;
+    const u64 n = min(ctl->n_slots, max_keys);
+    const u64 top = ctl->sel_prefix;
+    const int lane = threadIdx.x & 31;
+    const u64 span = (u64)gridDim.x * kSelThreads;
+    for (u64 base = (u64)blockIdx.x * kSelThreads; base < n; base += span) {   // warp-uniform trip count
+        const u64 i = base + threadIdx.x;
+        const u64 key = i < n ? keys[i] : kKeySentinel;
+        const bool hit = key != kKeySentinel && (key >> (64 - kTopBits)) == top;
+        const u32 m = __ballot_sync(0xffffffffu, hit);
+        if (m) {
+            u64 pos = 0;
+            if (lane == 0) pos = atomicAdd(&ctl->n_compact, (u64)__popc(m));
+            pos = __shfl_sync(0xffffffffu, pos, 0);
+            if (hit) ckeys[pos + __popc(m & ((1u << lane) - 1u))] = key;
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) is_last = atomicAdd(&ctl->sel_ticket, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    // the remaining 53 bits on the compact buffer alone
+    const u64 nc = *(volatile u64*)&ctl->n_compact;
+    u64 rank = ctl->sel_rank, prefix = 0;
+    const int bits[5] = {11, 11, 11, 10, 10};
+    int shift = 64 - kTopBits;
+    for (int r = 0; r < 5; ++r) {
+        shift -= bits[r];
+        const int nb = 1 << bits[r];
+        for (int b = threadIdx.x; b < nb; b += kSelThreads) h[b] = 0;
+        __syncthreads();
+        const u64 low = (1ULL << (64 - kTopBits)) - 1ULL;
+        for (u64 i = threadIdx.x; i < nc; i += kSelThreads) {
+            const u64 key = __ldcg(&ckeys[i]) & low;
+            if (r == 0 || (key >> (shift + bits[r])) == prefix) atomicAdd(&h[(key >> shift) & (u64)(nb - 1)], 1u);
+        }
+        __syncthreads();
+        block_find_bin(h, nb, rank, &s_bin, &s_cum, scratch);
+        prefix = (prefix << bits[r]) | (u64)s_bin;
+        rank -= s_cum;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { ctl->X = (top << (64 - kTopBits)) | prefix; ctl->sel_ticket = 0; }
+}
+
+cudaError_t launch_select(const u64* keys, u64* ckeys, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches) {
     k_select_init<<<1, 1, 0, s>>>(ctl, cap);
     ++*n_launches;
     if (cap == 0) return cudaGetLastError();
-    static const int bits[6] = {11, 11, 11, 11, 10, 10};
-    int shift = 64;
-    u64 blocks = (n_keys_hint + 256 * 8 - 1) / (256 * 8);
+    u64 blocks = (n_keys_hint + kSelThreads * 8 - 1) / (kSelThreads * 8);
     if (blocks > (u64)sm_count * 8) blocks = (u64)sm_count * 8;
     if (blocks < 1) blocks = 1;
-    for (int r = 0; r < 6; ++r) {
-        shift -= bits[r];
-        k_select_round<<<(unsigned)blocks, 256, 0, s>>>(keys, ctl, max_keys, shift, bits[r], r == 0, r == 5);
-        ++*n_launches;
-    }
+    k_select_hist<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ctl, max_keys);
+    k_select_narrow<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ckeys, ctl, max_keys);
+    *n_launches += 2;
     return cudaGetLastError();
 }
 
