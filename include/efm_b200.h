@@ -53,11 +53,14 @@ typedef struct {
     int32_t dep_depth;      /* L: chain length of the dependent-reaction search; 0 = 4 */
     int32_t max_visited;    /* V: max visited metabolites per pathway; 0 = 2*D                       */
     int64_t frontier_cap;   /* beam: entries expanded per level; 0 = unbounded                       */
-    int64_t max_frontier;   /* slots per frontier buffer; 0 = max(frontier_cap, 2^20 when cap == 0)  */
+    int64_t max_frontier;   /* entries per frontier buffer; 0 = max(frontier_cap, 4096), 2^20 when cap == 0 */
     int64_t max_candidates; /* capacity of the candidate buffer / support hash; 0 = 2^20             */
     int64_t max_child_keys; /* capacity of the per-level beam key array; 0 = 64 * frontier_cap       */
     int32_t device;         /* CUDA device ordinal the workspace lives on                            */
     uint32_t flags;         /* EFM_F_*                                                               */
+    int64_t max_frontier_bytes; /* bytes of one frontier buffer (entries are packed, variable size);         */
+                            /* 0 = max_frontier * the largest possible entry, which can never overflow;      */
+                            /* a smaller value saves HBM and reports EFM_E_CAPACITY if a level outgrows it   */
 } efm_params;
 
 typedef struct {

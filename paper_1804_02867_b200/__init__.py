@@ -27,7 +27,7 @@ class efm_params(ctypes.Structure):
     _fields_ = [("max_support", ctypes.c_int32), ("max_loop", ctypes.c_int32), ("dep_depth", ctypes.c_int32),
                 ("max_visited", ctypes.c_int32), ("frontier_cap", ctypes.c_int64), ("max_frontier", ctypes.c_int64),
                 ("max_candidates", ctypes.c_int64), ("max_child_keys", ctypes.c_int64), ("device", ctypes.c_int32),
-                ("flags", ctypes.c_uint32)]
+                ("flags", ctypes.c_uint32), ("max_frontier_bytes", ctypes.c_int64)]
 
 
 _STAT_INT = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxloop", "discarded_nonpos",
@@ -118,7 +118,8 @@ class Enumerator:
         p = efm_params(int(params.get("max_support", 0)), int(params.get("max_loop", 0)), int(params.get("dep_depth", 0)),
                        int(params.get("max_visited", 0)), int(params.get("frontier_cap", 0)),
                        int(params.get("max_frontier", 0)), int(params.get("max_candidates", 0)),
-                       int(params.get("max_child_keys", 0)), int(device), int(flags))
+                       int(params.get("max_child_keys", 0)), int(device), int(flags),
+                       int(params.get("max_frontier_bytes", 0)))
         self.device = int(device)
         self._check(self._lib.efm_create(_ptr(S), self.m, self.n, self.n, _ptr(rev), _ptr(internal), ctypes.byref(p),
                                          ctypes.byref(self._h)))

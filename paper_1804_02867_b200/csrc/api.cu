@@ -23,7 +23,7 @@ struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
     Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
-    Region ctl, buf[2], keys, ckeys, cand, table, isrep, poison, uniq, size_hist, bucket_start, bucket_fill;
+    Region ctl, buf[2], off[2], pmin, keys, ckeys, cand, table, isrep, poison, uniq, size_hist, bucket_start, bucket_fill;
     Region order, sig, size_sorted, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, dense;
     size_t total = 0;
 };
@@ -38,7 +38,8 @@ struct efm_handle {
     int64_t cap = 0, max_frontier = 0, max_cand = 0, max_keys = 0;
     int32_t device = 0;
     uint32_t flags = 0;
-    uint32_t stride = 0, cand_stride = 0;
+    uint32_t max_entry = 0, cand_stride = 0;   // largest frontier entry in bytes; candidate slot stride
+    int64_t frontier_bytes = 0;                // bytes of one packed frontier buffer
     size_t table_size = 0, dense_bytes = 0;
     Layout lay;
     double ms_build = 0;
@@ -80,8 +81,11 @@ void make_layout(efm_handle* h) {
     add_region(L, L.arc_dir, sizeof(int) * (G.A + 1));
     add_region(L, L.arc_mix, sizeof(u64) * (G.A + 1));
     add_region(L, L.ctl, sizeof(Ctl));
-    add_region(L, L.buf[0], (size_t)h->max_frontier * h->stride);
-    add_region(L, L.buf[1], (size_t)h->max_frontier * h->stride);
+    add_region(L, L.buf[0], (size_t)h->frontier_bytes + 512);   // 512: the speculative first load of a parent
+    add_region(L, L.buf[1], (size_t)h->frontier_bytes + 512);
+    add_region(L, L.off[0], (size_t)h->max_frontier * 8);
+    add_region(L, L.off[1], (size_t)h->max_frontier * 8);
+    add_region(L, L.pmin, (size_t)(h->max_frontier + 1) * 8);
     add_region(L, L.keys, (size_t)h->max_keys * 8);
     add_region(L, L.ckeys, (size_t)h->max_keys * 8);
     const size_t C = (size_t)h->max_cand;
@@ -178,7 +182,7 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     memset(&P, 0, sizeof P);
     if (p) P = *p;
     if (P.max_support < 0 || P.max_loop < 0 || P.dep_depth < 0 || P.max_visited < 0 || P.frontier_cap < 0 ||
-        P.max_frontier < 0 || P.max_candidates < 0 || P.max_child_keys < 0 || P.device < 0)
+        P.max_frontier < 0 || P.max_candidates < 0 || P.max_child_keys < 0 || P.device < 0 || P.max_frontier_bytes < 0)
         return EFM_E_INVAL;
     efm_handle* h = new (std::nothrow) efm_handle();
     if (!h) return EFM_E_NOMEM;
@@ -200,9 +204,19 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     h->device = P.device;
     h->flags = P.flags;
     const int Veff = std::min(h->V, std::max(G.M, 1));   // a pathway cannot visit more nodes than exist
-    h->stride = entry_bytes((u32)h->D, (u32)Veff);
-    h->cand_stride = entry_bytes((u32)h->D, 0);
+    int max_col = 0;
+    for (int a = 0; a < G.A; ++a) max_col = std::max(max_col, G.col_ptr[a + 1] - G.col_ptr[a]);
+    const int64_t Ueff = std::min<int64_t>(G.M, (int64_t)h->D * max_col);   // unbalanced metabolites a pathway can have
+    h->max_entry = entry_bytes((u32)h->D, (u32)Veff, (u32)Ueff);
+    h->cand_stride = entry_bytes((u32)h->D, 0, 0);
     h->max_frontier = P.max_frontier ? P.max_frontier : (h->cap ? std::max<int64_t>(h->cap, 4096) : (int64_t)1 << 20);
+    if (h->max_frontier >= ((int64_t)1 << (64 - kAllocShift))) { delete h; return EFM_E_INVAL; }
+    h->frontier_bytes = P.max_frontier_bytes ? ((P.max_frontier_bytes + 15) & ~(int64_t)15) : h->max_frontier * (int64_t)h->max_entry;
+    if (h->frontier_bytes < (int64_t)h->max_entry) h->frontier_bytes = h->max_entry;
+    if ((uint64_t)h->frontier_bytes >> 4 > kAllocUnitMask) {
+        if (P.max_frontier_bytes) { delete h; return EFM_E_INVAL; }
+        h->frontier_bytes = (int64_t)(kAllocUnitMask << 4);   // the default never needs more than the allocator can address
+    }
     h->max_cand = P.max_candidates ? P.max_candidates : (int64_t)1 << 20;
     if (h->max_cand > 0xFFFFFFF0LL) { delete h; return EFM_E_INVAL; }
     h->max_keys = (P.max_child_keys ? P.max_child_keys : std::max<int64_t>(h->cap * (int64_t)G.max_fanout, 65536)) +
@@ -296,17 +310,20 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     }
     const u64 n_roots = roots.size();
     if ((int64_t)n_roots > h->max_frontier || (int64_t)n_roots > h->max_keys) return EFM_E_CAPACITY;
-    std::vector<unsigned char> root_img((size_t)n_roots * h->stride, 0);
+    // seed sets as CSR of arc ids + the offset of every root entry in the staging buffer (16-byte units); the
+    // entries themselves are built on the device (k_roots)
+    std::vector<int> h_seed_ptr(n_roots + 1, 0), h_seed_arc;
+    std::vector<u64> stage_off(n_roots, 0);
+    u64 stage_units = 0;
     for (size_t r = 0; r < roots.size(); ++r) {
-        unsigned char* e = root_img.data() + r * h->stride;
-        const u32 ns = (u32)roots[r].size();
-        *(u32*)e = ns;   // n_vis = 0; n_unb is filled in by the classify pass
-        i64* f = (i64*)(e + kHdr);
-        u16* arc = (u16*)(e + kHdr + 8 * (size_t)ns);
-        u64 hs = 0;
-        for (u32 k = 0; k < ns; ++k) { f[k] = 1; arc[k] = (u16)roots[r][k]; hs += arc_term((u32)roots[r][k], 1ULL); }
-        ((u64*)e)[1] = hs;   // hv = 0: nothing visited
+        int64_t touched = 0;
+        for (int a : roots[r]) { h_seed_arc.push_back(a); touched += G.col_ptr[a + 1] - G.col_ptr[a]; }
+        h_seed_ptr[r + 1] = (int)h_seed_arc.size();
+        stage_off[r] = stage_units;
+        stage_units += entry_bytes((u32)roots[r].size(), 0, (u32)std::min<int64_t>(touched, G.M)) >> 4;
     }
+    if ((int64_t)(stage_units << 4) > h->frontier_bytes || h_seed_arc.size() * sizeof(int) > (size_t)h->max_keys * 8)
+        return EFM_E_CAPACITY;
 
     CK(cudaSetDevice(h->device));
     if (!h->h_ctl) {
@@ -345,7 +362,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         CK(up(L.arc_mix, arc_mix.data(), sizeof(u64) * arc_mix.size()));
         h->graph_ws = ws;
     }
-    CK(up(L.buf[1], root_img.data(), root_img.size()));
+    CK(up(L.pmin, h_seed_ptr.data(), sizeof(int) * h_seed_ptr.size()));        // regions unused until level 1
+    CK(up(L.ckeys, h_seed_arc.data(), sizeof(int) * h_seed_arc.size()));
+    CK(up(L.off[1], stage_off.data(), sizeof(u64) * stage_off.size()));
     CK(cudaMemsetAsync(ws + L.ctl.off, 0, sizeof(Ctl), s));
     CK(cudaStreamSynchronize(s));   // the host staging vectors above go out of scope later; keep it simple
 
@@ -359,7 +378,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.cand = ws + L.cand.off;
     ea.keys = (u64*)(ws + L.keys.off);
     ea.ctl = d_ctl;
-    ea.stride = h->stride; ea.cand_stride = h->cand_stride;
+    ea.pmin = (u64*)(ws + L.pmin.off);
+    ea.max_entry = h->max_entry; ea.cand_stride = h->cand_stride;
+    ea.frontier_units = (u64)h->frontier_bytes >> 4;
     ea.max_frontier = (u64)h->max_frontier; ea.max_cand = (u64)h->max_cand; ea.max_keys = (u64)h->max_keys;
     ea.D = h->D; ea.V = h->V; ea.max_loop = h->max_loop;
     ea.no_fast = (h->flags & EFM_F_NO_FASTPATH) ? 1 : 0;
@@ -383,13 +404,21 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     u64 n_cur = 0;
     if (n_roots > 0) {
         CK(launch_level_begin(d_ctl, s)); ++launches;
-        ea.cur = ws + L.buf[1].off; ea.nxt = ws + L.buf[0].off; ea.n_cur = n_roots;
+        RootArgs ra;
+        memset(&ra, 0, sizeof ra);
+        ra.g = ea.g; ra.ctl = d_ctl; ra.n_roots = n_roots;
+        ra.seed_ptr = (const int*)(ws + L.pmin.off); ra.seed_arc = (const int*)(ws + L.ckeys.off);
+        ra.stage_off = (const u64*)(ws + L.off[1].off); ra.stage = ws + L.buf[1].off;
+        ra.nxt = ws + L.buf[0].off; ra.nxt_off = (u64*)(ws + L.off[0].off);
+        ra.cand = ea.cand; ra.cand_stride = h->cand_stride; ra.keys = ea.keys;
+        ra.max_frontier = ea.max_frontier; ra.frontier_units = ea.frontier_units; ra.max_cand = ea.max_cand;
         size_t t0 = tm.mark();
-        CK(launch_expand(0, true, ea, h->sm_count, s)); ++launches;
+        CK(launch_roots(false, ra, s)); ++launches;
         size_t t1 = tm.mark();
+        // the select's compact buffer is the region the seed arcs sit in: they are dead once the roots are built
         CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), d_ctl, (u64)h->cap, ea.max_keys, n_roots, h->sm_count, s, &launches));
         size_t t2 = tm.mark();
-        CK(launch_expand(1, true, ea, h->sm_count, s)); ++launches;
+        CK(launch_roots(true, ra, s)); ++launches;
         size_t t3 = tm.mark();
         tm.span(t0, t1, PH_COUNT); tm.span(t1, t2, PH_BEAM); tm.span(t2, t3, PH_WRITE);
         CK(read_ctl());
@@ -399,8 +428,8 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         h->lvl_expanded.push_back(0);
         h->lvl_children.push_back(0);
         done_total += (int64_t)hc->lvl_done;
-        truncated += (int64_t)hc->n_keys - (int64_t)hc->n_next;
-        n_cur = hc->n_next;
+        truncated += (int64_t)hc->n_keys - (int64_t)(hc->n_next >> kAllocShift);
+        n_cur = hc->n_next >> kAllocShift;
         cur = 0;
     }
 
@@ -409,20 +438,21 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         const size_t lvl = h->lvl_active.size() - 1;   // level of the parents
         CK(launch_level_begin(d_ctl, s)); ++launches;
         ea.cur = ws + L.buf[cur].off; ea.nxt = ws + L.buf[cur ^ 1].off; ea.n_cur = n_cur;
+        ea.cur_off = (const u64*)(ws + L.off[cur].off); ea.nxt_off = (u64*)(ws + L.off[cur ^ 1].off);
         const bool beam_possible = h->cap > 0 && ((h->flags & EFM_F_FORCE_TWO_PASS) || n_cur * (u64)G.max_fanout > (u64)h->cap);
         if (beam_possible) {
             size_t t0 = tm.mark();
-            CK(launch_expand(0, false, ea, h->sm_count, s)); ++launches;
+            CK(launch_expand(0, ea, h->sm_count, s)); ++launches;
             size_t t1 = tm.mark();
             CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), d_ctl, (u64)h->cap, ea.max_keys, std::min<u64>(ea.max_keys, n_cur * (u64)G.max_fanout), h->sm_count, s, &launches));
             size_t t2 = tm.mark();
-            CK(launch_expand(1, false, ea, h->sm_count, s)); ++launches;
+            CK(launch_expand(1, ea, h->sm_count, s)); ++launches;
             size_t t3 = tm.mark();
             tm.span(t0, t1, PH_COUNT); tm.span(t1, t2, PH_BEAM); tm.span(t2, t3, PH_WRITE);
             st.two_pass_levels++; st.n_expand_count++; st.n_expand_write++;
         } else {
             size_t t0 = tm.mark();
-            CK(launch_expand(2, false, ea, h->sm_count, s)); ++launches;
+            CK(launch_expand(2, ea, h->sm_count, s)); ++launches;
             size_t t1 = tm.mark();
             tm.span(t0, t1, PH_DIRECT);
             st.direct_levels++; st.n_direct++;
@@ -431,7 +461,8 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         if (hc->error) return EFM_E_CAPACITY;
         h->lvl_expanded[lvl] = (int64_t)hc->lvl_expanded;
         h->lvl_children[lvl] = (int64_t)hc->lvl_children;
-        const int64_t active = beam_possible ? (int64_t)hc->n_keys : (int64_t)hc->n_next;
+        const int64_t n_next = (int64_t)(hc->n_next >> kAllocShift);
+        const int64_t active = beam_possible ? (int64_t)hc->n_keys : n_next;
         const int64_t done = (int64_t)hc->lvl_done;
         if (active + done > 0) {
             h->lvl_active.push_back(active);
@@ -440,8 +471,8 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
             h->lvl_children.push_back(0);
         }
         done_total += done;
-        truncated += active - (int64_t)hc->n_next;
-        n_cur = hc->n_next;
+        truncated += active - n_next;
+        n_cur = (u64)n_next;
         cur ^= 1;
     }
 

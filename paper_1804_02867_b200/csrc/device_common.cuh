@@ -13,22 +13,29 @@ typedef unsigned int u32;
 typedef unsigned short u16;
 
 // ---------------------------------------------------------------------------------------------------------------
-// Entry format in HBM.  A frontier slot is `stride` bytes; the entry occupies a prefix:
-//   [ 0,32)  header: u32 n_supp | n_vis << 16; u32 n_unb (unbalanced internal metabolites);
-//            u64 hs = sum of the arc terms of the state hash; u64 hv = sum of its visited terms; 8 spare bytes.
-//            hs / hv / n_unb are derived data the producer has in registers anyway: carrying them (20 B) saves the
-//            consumer one full re-hash of the parent.
+// Entry format in HBM.  Frontier entries are PACKED back to back (16-byte aligned); a
+// per-level offset array (u64, in 16-byte units) locates entry p.  An entry is
+//   [ 0,32)  header: u32 n_supp | n_vis << 16; u32 n_unb; u64 hs = sum of the arc terms of the state hash;
+//            u64 hv = sum of its visited terms; u64 big = max(largest flux, largest |EF|)
 //   i64  flux[n_supp]   fluxes of the support arcs, > 0, gcd 1
 //   u64  vis[n_vis]     visited records: cnt << 48 | met << 32 | PI << 16 | PO   (unordered)
+//   i64  ef[n_unb]      the non-zero extra fluxes EF_i (Eq 2) of the state   (unordered)
 //   u16  arc[n_supp]    support arcs, ascending arc id
-// A candidate slot holds the same with n_vis = 0.
+//   u16  efmet[n_unb]   metabolite of each ef[] element
+// hs / hv / big / ef[] are derived data the producer has in registers anyway: carrying them saves the consumer the
+// re-hash of the parent and the whole Eq 2 scatter over the support (children update the list incrementally:
+// EF' = (k EF + sign d s_.a) / g).  A candidate slot (fixed stride) holds the same with n_vis = n_unb = 0.
 // ---------------------------------------------------------------------------------------------------------------
-constexpr u32 kHdr = 32;   // header bytes of a frontier / candidate slot
-__host__ __device__ inline u32 entry_bytes(u32 n_supp, u32 n_vis) {
-    return (kHdr + 8u * n_supp + 8u * n_vis + 2u * n_supp + 15u) & ~15u;
+constexpr u32 kHdr = 32;   // header bytes of a frontier / candidate entry
+__host__ __device__ inline u32 entry_bytes(u32 n_supp, u32 n_vis, u32 n_unb) {
+    return (kHdr + 10u * n_supp + 8u * n_vis + 10u * n_unb + 15u) & ~15u;
 }
 // irreducible content of an entry, the unit of the algorithmic-byte count
 __host__ __device__ inline u32 algo_entry_bytes(u32 n_supp, u32 n_vis) { return n_supp * 10u + n_vis * 7u + 16u; }
+// packed allocation counter of the next frontier: entry count in the high 30 bits, 16-byte units in the low 34
+// (2^34 units = 256 GB, more than a B200 holds)
+constexpr int kAllocShift = 34;
+constexpr u64 kAllocUnitMask = (1ULL << kAllocShift) - 1ULL;
 
 struct DevGraph {
     int M, A, W32, M32;
@@ -50,7 +57,7 @@ enum { SEL_BINS = 2048 };
 
 struct Ctl {
     // per level (reset by k_level_begin)
-    u64 n_next;        // active survivors written to the next frontier buffer
+    u64 n_next;        // packed allocator of the next frontier: count << 34 | 16-byte units (kAllocShift)
     u64 n_keys;        // active children generated (= valid keys written by the count pass)
     u64 n_slots;       // key slots reserved by the count pass (chunked per warp; unused slots hold kKeySentinel)
     u64 lvl_done;      // balanced children generated
@@ -72,18 +79,36 @@ struct Ctl {
 
 struct ExpandArgs {
     DevGraph g;
-    const unsigned char* cur;   // parents
-    unsigned char* nxt;         // children that stay active
-    unsigned char* cand;        // balanced children
+    const unsigned char* cur;   // parents (packed)
+    const u64* cur_off;         // 16-byte-unit offset of parent p
+    unsigned char* nxt;         // children that stay active (packed)
+    u64* nxt_off;
+    unsigned char* cand;        // balanced children (fixed stride)
     u64* keys;                  // beam keys of the active children (count pass)
+    u64* pmin;                  // per parent: smallest key among its active children (count pass -> write pass)
     Ctl* ctl;
     u64 n_cur;
-    u32 stride, cand_stride;
-    u64 max_frontier, max_cand, max_keys;
+    u32 max_entry, cand_stride; // largest entry in bytes (shared-memory staging), candidate slot stride
+    u64 max_frontier, frontier_units, max_cand, max_keys;
     int D, V, max_loop;
     int no_fast;                // EFM_F_NO_FASTPATH: every child through the warp-cooperative general routine
-    // shared-memory carve-up per group (bytes)
-    u32 sm_group, sm_EF, sm_sbits, sm_mseen;
+    // shared-memory carve-up per warp (bytes)
+    u32 sm_group, sm_sbits, sm_ubits;
+};
+
+// roots (INIT): seed sets uploaded by the host, entries built and classified on the device
+struct RootArgs {
+    DevGraph g;
+    const int* seed_ptr; const int* seed_arc;   // CSR of arc ids, ascending inside a set
+    const u64* stage_off;                       // 16-byte-unit offset of root r in the staging buffer
+    unsigned char* stage;                       // root entries (packed), built by the count pass
+    unsigned char* nxt; u64* nxt_off;           // surviving active roots
+    unsigned char* cand;
+    u64* keys;                                  // one key per root (kKeySentinel for balanced roots)
+    Ctl* ctl;
+    u64 n_roots;
+    u32 cand_stride;
+    u64 max_frontier, frontier_units, max_cand;
 };
 
 // ---------------------------------------------------------------------------------------------------------------

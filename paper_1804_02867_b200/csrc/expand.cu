@@ -1,6 +1,7 @@
 // Frontier expansion kernels: one warp owns one partial pathway at a time.
-// The warp stages the parent entry in shared memory, scatters its extra fluxes EF_i (Eq 2) into a
-// dense per-warp shared array, picks the lowest unbalanced metabolite i* (reading G12) and then
+// The warp stages the packed parent entry in shared memory.  The entry carries its non-zero extra fluxes EF_i
+// (Eq 2) as a short list, so the lowest unbalanced metabolite i* (reading G12) is a warp min and no
+// scatter over the support is needed; children update the list incrementally, EF' = (k EF + sign d s_.a) / g.
 //   first visit (PROC1/1', Eq 3): fans out over the OR-alternatives of i*, ONE LANE PER
 //       ALTERNATIVE -- a child that adds a new arc to a pathway whose integers are far from the 2^62 guard needs only
 //       lane-local work (scale k = c/gcd(|E|,c), its own column of S for the new unbalanced count, an incremental
@@ -8,8 +9,8 @@
 //       routine eval_child();
 //   revisit (PROC2-4, Eq 4 / Eq 5): exactly one child, general routine.
 // Children are classified where they are generated (balanced -> candidate; otherwise beam key).  Three modes:
-//   COUNT  : count children, write only their 8-byte beam keys           (pass 1 of a level the beam may cut)
-//   WRITE  : regenerate the children and materialise those with key < X  (pass 2)
+//   COUNT  : count children, write their 8-byte beam keys and the balanced children (pass 1 of a level the beam may cut)
+//   WRITE  : regenerate the children of parents that have a survivor and materialise those with key < X  (pass 2)
 //   DIRECT : single pass, every child is materialised                     (beam cannot bind)
 #include <climits>
 
@@ -38,6 +39,7 @@ __device__ __forceinline__ u64 w_max(u64 v) {   // two 32-bit redux instead of f
     const u32 ml = __reduce_max_sync(FULL, hi == mh ? (u32)v : 0u);
     return ((u64)mh << 32) | ml;
 }
+__device__ __forceinline__ u64 w_min(u64 v) { return ~w_max(~v); }
 __device__ __forceinline__ u64 w_bcast(u64 v, int src) { return __shfl_sync(FULL, v, src); }
 
 // ------------------------------------------------------------------ integer helpers
@@ -53,9 +55,27 @@ __device__ __forceinline__ u64 gcd64(u64 a, u64 b) {   // binary gcd
     } while (b);
     return a << sh;
 }
-__device__ __forceinline__ u64 w_gcd(u64 v) {
+__device__ __forceinline__ u32 gcd32(u32 a, u32 b) {
+    if (a == 0) return b;
+    if (b == 0) return a;
+    const int sh = __ffs((int)(a | b)) - 1;
+    a >>= (__ffs((int)a) - 1);
+    do {
+        b >>= (__ffs((int)b) - 1);
+        if (a > b) { u32 t = a; a = b; b = t; }
+        b -= a;
+    } while (b);
+    return a << sh;
+}
+__device__ __forceinline__ u64 w_gcd(u64 v, bool narrow) {
+    if (narrow) {   // every value below 2^32
+        u32 x = (u32)v;
 #pragma unroll
-    for (int o = 16; o; o >>= 1) { u64 w = __shfl_xor_sync(FULL, v, o); v = gcd64(v, w); }
+        for (int o = 16; o; o >>= 1) { const u32 w = __shfl_xor_sync(FULL, x, o); x = gcd32(x, w); }
+        return x;
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) { const u64 w = __shfl_xor_sync(FULL, v, o); v = gcd64(v, w); }
     return v;
 }
 struct S128 { u64 lo; i64 hi; };
@@ -70,37 +90,47 @@ __device__ __forceinline__ bool abs_gt_guard(S128 x) {   // |x| > 2^62
 __device__ __forceinline__ bool umul_gt_guard(u64 a, u64 b) {  // a*b > 2^62, a, b >= 0
     return __umul64hi(a, b) != 0 || a * b > EFM_GUARD;
 }
+__device__ __forceinline__ u64 abs64(i64 v) { return (u64)(v < 0 ? -v : v); }
 // arc term of the state hash through the per-arc table of inner mixes (device_common.cuh: arc_term)
 __device__ __forceinline__ u64 arc_term_t(const DevGraph& g, u32 a, u64 f) { return mix64(__ldg(&g.arc_mix[a]) + f); }
 
 // ------------------------------------------------------------------ per-parent context (warp-uniform)
 struct Parent {
-    int n_supp, n_vis;
-    const i64* flux; const u64* vis; const u16* arc;   // shared-memory staging
-    i64* EF; u32* sbits; u32* mseen;
-    u64 hs, hv, fmax, maxabsEF;
-    int n_unb, istar;
+    int n_supp, n_vis, n_unb;
+    const i64* flux; const u64* vis; const i64* ef; const u16* arc; const u16* efmet;   // shared-memory staging
+    u32* sbits;   // support bitset over arcs
+    u32* ubits;   // bitset over metabolites: member of the EF list
+    u64 hs, hv, big;
+    int istar;
     i64 E;
 };
 struct Child {          // warp-uniform description of one child relative to its parent
     int status; bool done;
-    int a; bool in_supp; int ia;
-    u64 k, g2, T;       // scale, common divisor, un-normalised new flux of arc a
+    int a; bool in_supp; int ia; int sign;
+    u64 k, g2, T, d;    // scale, common divisor, un-normalised new flux of arc a, |E| / gcd(|E|, c)
     u64 hs, hv;         // hash sums of the child state
     int n_unb;
 };
 
-__device__ __forceinline__ bool sbit(const u32* sbits, int a) { return (sbits[a >> 5] >> (a & 31)) & 1u; }
+__device__ __forceinline__ bool sbit(const u32* bits, int a) { return (bits[a >> 5] >> (a & 31)) & 1u; }
+
+// EF_met of the parent: zero unless met is in the list
+__device__ __forceinline__ i64 ef_lookup(const Parent& P, int met) {
+    if (met == P.istar) return P.E;
+    if (!sbit(P.ubits, met)) return 0;
+    for (int t = 0; t < P.n_unb; ++t) if ((int)P.efmet[t] == met) return P.ef[t];
+    return 0;
+}
 
 // General routine: evaluate the child bump(f, a, sign*|E|/c) with the whole warp.
 //   first: new visited record newrec; otherwise record oldrec is replaced by newrec
 __device__ __noinline__ void eval_child(const DevGraph& g, const Parent& P, int lane, int a, int c, int sign,
                                         bool first, u64 oldrec, u64 newrec, Child& ch) {
-    const u64 absE = (u64)(P.E < 0 ? -P.E : P.E);
-    const u64 gg = gcd64(absE, (u64)c);
+    const u64 absE = abs64(P.E);
+    const u64 gg = c == 1 ? 1ULL : gcd64(absE, (u64)c);
     const u64 k = gg == 1 ? (u64)c : (u64)c / gg;
     const u64 d = gg == 1 ? absE : absE / gg;
-    ch.a = a; ch.k = k; ch.g2 = 1;
+    ch.a = a; ch.k = k; ch.g2 = 1; ch.d = d; ch.sign = sign;
     ch.in_supp = sbit(P.sbits, a);
     int ia = -1;
     if (ch.in_supp) {   // position of a in the sorted support
@@ -111,7 +141,9 @@ __device__ __noinline__ void eval_child(const DevGraph& g, const Parent& P, int 
         }
     }
     ch.ia = ia;
-    // scaled fluxes F_t = k f_t, F_a = k f_a +- d: overflow first, then non-positive (order of the definition, O6)
+    // scaled fluxes F_t = k f_t, F_a = k f_a +- d: overflow first, then non-positive (order of the definition, O6).
+    // P.big >= every flux and every |EF| of the parent: products below the guard with it need no exact sweep.
+    const bool bigk = k > 1 && umul_gt_guard(k, P.big);
     bool ovf = false, nonpos = false;
     u64 T = d;
     if (ch.in_supp) {
@@ -125,38 +157,31 @@ __device__ __noinline__ void eval_child(const DevGraph& g, const Parent& P, int 
             if (hi == 0 && lo <= d) { nonpos = true; T = 0; }           // k f_a - d <= 0
             else { T = lo - d; const u64 hi2 = hi - (lo < d); ovf = hi2 != 0 || T > EFM_GUARD; }
         }
-        if (k > 1 && umul_gt_guard(k, P.fmax)) {
-            // exact: the largest flux among t != ia
-            u64 mx = 0;
-            for (int t = lane; t < P.n_supp; t += 32) if (t != ia) mx = max(mx, (u64)P.flux[t]);
-            mx = w_max(mx);
-            ovf = ovf || umul_gt_guard(k, mx);
-        }
-    } else {
-        ovf = k > 1 && umul_gt_guard(k, P.fmax);   // the new arc carries d <= |E| <= 2^62
+    }
+    if (bigk) {   // exact: the largest flux among t != ia (the new arc carries d <= |E| <= 2^62)
+        u64 mx = 0;
+        for (int t = lane; t < P.n_supp; t += 32) if (t != ia) mx = max(mx, (u64)P.flux[t]);
+        mx = w_max(mx);
+        ovf = ovf || umul_gt_guard(k, mx);
     }
     ch.T = T;
     if (ovf) { ch.status = CH_OVERFLOW; return; }
     if (nonpos) { ch.status = CH_NONPOS; return; }   // Prop 3, reading G11
     // extra fluxes of the un-normalised child: EF'_i = k EF_i + sign d s_ia  (Eq 2 on the scaled fluxes)
+    const int qa0 = __ldg(&g.col_ptr[a]), qa1 = __ldg(&g.col_ptr[a + 1]);
     bool ovf2 = false;
-    if (k > 1 && umul_gt_guard(k, P.maxabsEF)) {
-        // exact sweep over every touched metabolite outside col(a)
-        const int qa0 = g.col_ptr[a], qa1 = g.col_ptr[a + 1];
-        for (int t = lane; t < P.n_supp; t += 32) {
-            const int at = P.arc[t];
-            for (int q = g.col_ptr[at]; q < g.col_ptr[at + 1]; ++q) {
-                const int i = g.col[q].x;
-                bool in_a = false;
-                for (int r = qa0; r < qa1; ++r) in_a = in_a || g.col[r].x == i;
-                if (!in_a) ovf2 = ovf2 || abs_gt_guard(mul_s((i64)k, P.EF[i]));
-            }
+    if (bigk) {   // exact sweep over the unbalanced metabolites outside col(a)
+        for (int t = lane; t < P.n_unb; t += 32) {
+            const int i = P.efmet[t];
+            bool in_a = false;
+            for (int r = qa0; r < qa1; ++r) in_a = in_a || __ldg(&g.col[r]).x == i;
+            if (!in_a) ovf2 = ovf2 || abs_gt_guard(mul_s((i64)k, P.ef[t]));
         }
     }
     int delta = 0;
-    for (int q = g.col_ptr[a] + lane; q < g.col_ptr[a + 1]; q += 32) {
-        const int2 e = g.col[q];
-        const i64 efp = P.EF[e.x];
+    for (int q = qa0 + lane; q < qa1; q += 32) {
+        const int2 e = __ldg(&g.col[q]);
+        const i64 efp = ef_lookup(P, e.x);
         S128 x = add_s(mul_s((i64)k, efp), mul_s(sign > 0 ? (i64)d : -(i64)d, (i64)e.y));
         ovf2 = ovf2 || abs_gt_guard(x);
         delta += (int)((x.lo | (u64)x.hi) != 0) - (int)(efp != 0);
@@ -167,11 +192,19 @@ __device__ __noinline__ void eval_child(const DevGraph& g, const Parent& P, int 
     ch.n_unb = P.n_unb + delta;
     ch.done = ch.n_unb == 0;
     // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and gcd(k, d) = 1.
-    if (ch.in_supp) {
-        u64 G = 0;
-        for (int t = lane; t < P.n_supp; t += 32) if (t != ia) G = gcd64(G, (u64)P.flux[t]);
-        G = w_gcd(G);
-        ch.g2 = gcd64(k * G, T);   // k G <= k fmax <= 2^62
+    // An arc of the support: g = gcd(k G, T) with G the gcd of the other fluxes; another flux equal to 1 gives G = 1
+    // and g = gcd(k, k f_a +- d) = gcd(k, d) = 1 without any gcd.
+    if (ch.in_supp && T != 1) {
+        bool one = false;
+        for (int t = lane; t < P.n_supp; t += 32) one = one || (t != ia && P.flux[t] == 1);
+        if (!__any_sync(FULL, one)) {
+            const bool narrow = P.big < (1ULL << 32);
+            u64 G = 0;
+            for (int t = lane; t < P.n_supp; t += 32)
+                if (t != ia) G = narrow ? (u64)gcd32((u32)G, (u32)P.flux[t]) : gcd64(G, (u64)P.flux[t]);
+            G = w_gcd(G, narrow);
+            ch.g2 = gcd64(k * G, T);   // k G <= k fmax <= 2^62
+        }
     }
     u64 hs;
     if (k == 1 && ch.g2 == 1) {
@@ -190,36 +223,84 @@ __device__ __noinline__ void eval_child(const DevGraph& g, const Parent& P, int 
     ch.hv = P.hv + vis_term(newrec) - (first ? 0ULL : vis_term(oldrec));
 }
 
-// Write the child into a frontier slot (or a candidate slot: no visited records).
-__device__ __forceinline__ void write_child(unsigned char* dst, const Parent& P, const Child& ch, int lane, bool first,
-                                            int vk, u64 newrec, bool to_cand) {
+// Write the child into a packed frontier entry (or a candidate slot: no visited records, no EF list).
+__device__ __forceinline__ void write_child(const DevGraph& g, unsigned char* dst, const Parent& P, const Child& ch,
+                                            int lane, bool first, int vk, u64 newrec, bool to_cand) {
     const int n2 = P.n_supp + (ch.in_supp ? 0 : 1);
     const int nv2 = to_cand ? 0 : P.n_vis + (first ? 1 : 0);
+    const int nu2 = to_cand ? 0 : ch.n_unb;
+    const u32 lt = (1u << lane) - 1u;
     int ins = 0;   // a new arc goes where the ascending order puts it
     if (!ch.in_supp)
         for (int base = 0; base < P.n_supp; base += 32) {
             const int t = base + lane;
             ins += __popc(__ballot_sync(FULL, t < P.n_supp && (int)P.arc[t] < ch.a));
         }
-    if (lane == 0) {
-        uint4* h4 = (uint4*)dst;
-        h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)ch.n_unb, (u32)ch.hs, (u32)(ch.hs >> 32));
-        h4[1] = make_uint4((u32)ch.hv, (u32)(ch.hv >> 32), 0u, 0u);
-    }
     i64* flux2 = (i64*)(dst + kHdr);
     u64* vis2 = (u64*)(flux2 + n2);
-    u16* arc2 = (u16*)(vis2 + nv2);
+    i64* ef2 = (i64*)(vis2 + nv2);
+    u16* arc2 = (u16*)(ef2 + nu2);
+    u16* efmet2 = arc2 + n2;
+    u64 mx = ch.in_supp ? 0ULL : (ch.g2 > 1 ? ch.T / ch.g2 : ch.T);
     for (int t = lane; t < P.n_supp; t += 32) {
         u64 F = t == ch.ia ? ch.T : ch.k * (u64)P.flux[t];
         if (ch.g2 > 1) F /= ch.g2;
         const int pos = t + ((!ch.in_supp && t >= ins) ? 1 : 0);
         flux2[pos] = (i64)F;
         arc2[pos] = P.arc[t];
+        mx = max(mx, F);
     }
     if (!ch.in_supp && lane == 0) { flux2[ins] = (i64)ch.T; arc2[ins] = (u16)ch.a; }
     if (!to_cand) {
         for (int u = lane; u < P.n_vis; u += 32) vis2[u] = (!first && u == vk) ? newrec : P.vis[u];
         if (first && lane == 0) vis2[P.n_vis] = newrec;
+        // EF list of the child: EF' = (k EF + sign d s_.a) / g over the parent's list, then the metabolites of col(a)
+        // that were balanced in the parent.  eval_child / the fast path established that nothing exceeds 2^62, so
+        // the wrapping 64-bit arithmetic below is exact.
+        const int qa0 = __ldg(&g.col_ptr[ch.a]), qa1 = __ldg(&g.col_ptr[ch.a + 1]);
+        const u64 sd = ch.sign > 0 ? ch.d : (u64)0 - ch.d;
+        int base = 0;
+        for (int t0 = 0; t0 < P.n_unb; t0 += 32) {
+            const int t = t0 + lane;
+            const bool valid = t < P.n_unb;
+            i64 x = 0;
+            int met = 0;
+            if (valid) {
+                met = P.efmet[t];
+                i64 s = 0;
+                for (int q = qa0; q < qa1; ++q) { const int2 e = __ldg(&g.col[q]); if (e.x == met) s = e.y; }
+                x = (i64)(ch.k * (u64)P.ef[t] + sd * (u64)s);
+                if (ch.g2 > 1) x /= (i64)ch.g2;
+            }
+            const u32 nz = __ballot_sync(FULL, valid && x != 0);
+            if (valid && x != 0) {
+                const int pos = base + __popc(nz & lt);
+                ef2[pos] = x; efmet2[pos] = (u16)met;
+                mx = max(mx, abs64(x));
+            }
+            base += __popc(nz);
+        }
+        for (int q0 = qa0; q0 < qa1; q0 += 32) {
+            const int q = q0 + lane;
+            int2 e = make_int2(0, 0);
+            bool only = false;
+            if (q < qa1) { e = __ldg(&g.col[q]); only = !sbit(P.ubits, e.x); }
+            const u32 m = __ballot_sync(FULL, only);
+            if (only) {
+                i64 x = (i64)(sd * (u64)(i64)e.y);
+                if (ch.g2 > 1) x /= (i64)ch.g2;
+                const int pos = base + __popc(m & lt);
+                ef2[pos] = x; efmet2[pos] = (u16)e.x;
+                mx = max(mx, abs64(x));
+            }
+            base += __popc(m);
+        }
+        mx = w_max(mx);
+    }
+    if (lane == 0) {
+        uint4* h4 = (uint4*)dst;
+        h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2, (u32)ch.hs, (u32)(ch.hs >> 32));
+        h4[1] = make_uint4((u32)ch.hv, (u32)(ch.hv >> 32), (u32)mx, (u32)(mx >> 32));
     }
 }
 
@@ -259,21 +340,20 @@ __device__ __forceinline__ void scale_small(u64 absE, u32 c, u32& k, u64& d) {
     k = c / gg; d = absE / (u64)gg;
 }
 
-template <int MODE, bool ROOTS>
+template <int MODE>
 __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevGraph& g = A.g;
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
+    const u32 lt = (1u << lane) - 1u;
     unsigned char* gs = smem + (size_t)wib * A.sm_group;
     uint4* stage = (uint4*)gs;
     Parent P;
-    P.EF = (i64*)(gs + A.sm_EF);
     P.sbits = (u32*)(gs + A.sm_sbits);
-    P.mseen = (u32*)(gs + A.sm_mseen);
-    for (int i = lane; i < g.M; i += 32) P.EF[i] = 0;
+    P.ubits = (u32*)(gs + A.sm_ubits);
     for (int i = lane; i < g.W32; i += 32) P.sbits[i] = 0;
-    for (int i = lane; i < g.M32; i += 32) P.mseen[i] = 0;
+    for (int i = lane; i < g.M32; i += 32) P.ubits[i] = 0;
     __syncwarp();
 
     Ctl* ctl = A.ctl;
@@ -285,97 +365,48 @@ __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
     u64 s_expanded = 0, s_children = 0, s_done = 0, s_active = 0, s_dead = 0, s_notefm = 0, s_nonpos = 0, s_ovf = 0,
         s_visited = 0, s_bytes = 0;
     KeyOut ko; ko.base = 0; ko.left = 0;
-    const u32 slot_chunks = A.stride / 16;
 
     for (u64 p = (u64)blockIdx.x * kWarps + wib; p < A.n_cur; p += (u64)gridDim.x * kWarps) {
+        if (MODE == MODE_WRITE && !notrunc && __ldg(&A.pmin[p]) >= X) continue;   // no child of p survives the beam
         // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
-        const uint4* src = (const uint4*)(A.cur + p * A.stride);
-        uint4 first = make_uint4(0, 0, 0, 0);
-        if ((u32)lane < slot_chunks) first = __ldg(src + lane);
+        const uint4* src = (const uint4*)(A.cur + (__ldg(&A.cur_off[p]) << 4));
+        const uint4 first = __ldg(src + lane);   // the buffers end in 512 spare bytes
         const u32 hdr = __shfl_sync(FULL, first.x, 0);
         P.n_supp = (int)(hdr & 0xffffu);
         P.n_vis = (int)(hdr >> 16);
-        const u32 nch = entry_bytes((u32)P.n_supp, (u32)P.n_vis) / 16;
+        P.n_unb = (int)__shfl_sync(FULL, first.y, 0);
+        const u32 nch = entry_bytes((u32)P.n_supp, (u32)P.n_vis, (u32)P.n_unb) / 16;
         if ((u32)lane < nch) stage[lane] = first;
         for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldg(src + c);
         __syncwarp();
         P.hs = ((const u64*)stage)[1];
         P.hv = ((const u64*)stage)[2];
+        P.big = ((const u64*)stage)[3];
         P.flux = (const i64*)(gs + kHdr);
         P.vis = (const u64*)(P.flux + P.n_supp);
-        P.arc = (const u16*)(P.vis + P.n_vis);
+        P.ef = (const i64*)(P.vis + P.n_vis);
+        P.arc = (const u16*)(P.ef + P.n_unb);
+        P.efmet = P.arc + P.n_supp;
 
-        // ---- Eq 2: scatter s_ia f_a into the dense EF array; support bitset; touched-metabolite bitset; largest flux
-        u64 fmax = 0;
-        for (int t = lane; t < P.n_supp; t += 32) {
-            const u32 a = P.arc[t];
-            const i64 f = P.flux[t];
-            atomicOr(&P.sbits[a >> 5], 1u << (a & 31));
-            const int q1 = __ldg(&g.col_ptr[a + 1]);
-            for (int q = __ldg(&g.col_ptr[a]); q < q1; ++q) {
-                const int2 e = __ldg(&g.col[q]);
-                atomicAdd((u64*)&P.EF[e.x], (u64)((i64)e.y * f));
-                atomicOr(&P.mseen[e.x >> 5], 1u << (e.x & 31));
-            }
-            fmax = max(fmax, (u64)f);
+        // ---- support bitset, unbalanced-metabolite bitset, PROC0: lowest unbalanced metabolite i* (reading G12)
+        for (int t = lane; t < P.n_supp; t += 32) { const u32 a = P.arc[t]; atomicOr(&P.sbits[a >> 5], 1u << (a & 31)); }
+        u32 best = 0xffffffffu;
+        for (int t = lane; t < P.n_unb; t += 32) {
+            const u32 i = P.efmet[t];
+            atomicOr(&P.ubits[i >> 5], 1u << (i & 31));
+            best = min(best, (i << 16) | (u32)t);
         }
-        fmax = w_max(fmax);
+        best = __reduce_min_sync(FULL, best);
         __syncwarp();
-        // ---- PROC0: lowest unbalanced metabolite i*, number of unbalanced metabolites, largest |EF|
-        int imin = INT_MAX, cnt = 0;
-        u64 maxabs = 0;
-        for (int w = lane; w < g.M32; w += 32) {
-            u32 bits = P.mseen[w];
-            while (bits) {
-                const int i = w * 32 + __ffs(bits) - 1;
-                bits &= bits - 1;
-                const i64 v = P.EF[i];
-                if (v != 0) {
-                    imin = min(imin, i);
-                    maxabs = max(maxabs, (u64)(v < 0 ? -v : v));
-                    ++cnt;
-                }
-            }
-        }
-        imin = __reduce_min_sync(FULL, imin);
-        cnt = __reduce_add_sync(FULL, cnt);
-        maxabs = w_max(maxabs);
-        P.fmax = fmax; P.maxabsEF = maxabs; P.n_unb = cnt; P.istar = imin;
-
-        if (ROOTS) {
-            // level 0: classify the root itself (arbiter "Done")
-            const bool done = cnt == 0;
-            const u64 key = beam_key((u32)cnt, mix64(P.hs + P.hv));
-            if (MODE == MODE_COUNT) {
-                if (done) s_done++;
-                else { s_active++; ko.push(A, lane, lane == 0, key); }
-            } else if (done || notrunc || key < X) {
-                u64 slot = 0;
-                if (lane == 0) slot = atomicAdd(done ? &ctl->n_cand : &ctl->n_next, 1ULL);
-                slot = w_bcast(slot, 0);
-                if (slot >= (done ? A.max_cand : A.max_frontier)) {
-                    if (lane == 0) atomicOr(&ctl->error, (u32)(done ? ERR_CAND : ERR_FRONTIER));
-                } else {
-                    unsigned char* dst = done ? A.cand + slot * A.cand_stride : A.nxt + slot * A.stride;
-                    const int nv2 = done ? 0 : P.n_vis;
-                    if (lane == 0) {
-                        uint4* h4 = (uint4*)dst;
-                        h4[0] = make_uint4((u32)P.n_supp | ((u32)nv2 << 16), (u32)cnt, (u32)P.hs, (u32)(P.hs >> 32));
-                        h4[1] = make_uint4((u32)P.hv, (u32)(P.hv >> 32), 0u, 0u);
-                    }
-                    i64* flux2 = (i64*)(dst + kHdr);
-                    u64* vis2 = (u64*)(flux2 + P.n_supp);
-                    u16* arc2 = (u16*)(vis2 + nv2);
-                    for (int t = lane; t < P.n_supp; t += 32) { flux2[t] = P.flux[t]; arc2[t] = P.arc[t]; }
-                    for (int u = lane; u < nv2; u += 32) vis2[u] = P.vis[u];
-                }
-            }
-        } else {
-            P.E = P.EF[imin];
-            const int istar = imin;
+        const int cnt = P.n_unb;
+        const int istar = (int)(best >> 16);
+        P.istar = istar;
+        P.E = P.ef[best & 0xffffu];
+        {
             const bool fwd = P.E > 0;
-            const u64 absE = (u64)(fwd ? P.E : -P.E);
+            const u64 absE = abs64(P.E);
             if (MODE != MODE_WRITE) { s_expanded++; s_bytes += algo_entry_bytes((u32)P.n_supp, (u32)P.n_vis); }
+            u64 kmin = ~0ULL;   // smallest key among the active children of p (count pass)
             // visited?
             int vk = -1;
             for (int base = 0; base < P.n_vis && vk < 0; base += 32) {
@@ -390,15 +421,27 @@ __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
             auto place = [&](const Child& ch, bool first, u64 newrec) {
                 const int n2 = P.n_supp + (ch.in_supp ? 0 : 1), nv2 = P.n_vis + (first ? 1 : 0);
                 s_bytes += algo_entry_bytes((u32)n2, (u32)nv2);
-                u64 slot = 0;
-                if (lane == 0) slot = atomicAdd(ch.done ? &ctl->n_cand : &ctl->n_next, 1ULL);
-                slot = w_bcast(slot, 0);
-                if (slot >= (ch.done ? A.max_cand : A.max_frontier)) {
-                    if (lane == 0) atomicOr(&ctl->error, (u32)(ch.done ? ERR_CAND : ERR_FRONTIER));
-                    return;
+                unsigned char* dst;
+                if (ch.done) {
+                    u64 slot = 0;
+                    if (lane == 0) slot = atomicAdd(&ctl->n_cand, 1ULL);
+                    slot = w_bcast(slot, 0);
+                    if (slot >= A.max_cand) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_CAND); return; }
+                    dst = A.cand + slot * A.cand_stride;
+                } else {
+                    const u64 units = entry_bytes((u32)n2, (u32)nv2, (u32)ch.n_unb) >> 4;
+                    u64 old = 0;
+                    if (lane == 0) old = atomicAdd(&ctl->n_next, (1ULL << kAllocShift) | units);
+                    old = w_bcast(old, 0);
+                    const u64 slot = old >> kAllocShift, off = old & kAllocUnitMask;
+                    if (slot >= A.max_frontier || off + units > A.frontier_units) {
+                        if (lane == 0) atomicOr(&ctl->error, (u32)ERR_FRONTIER);
+                        return;
+                    }
+                    if (lane == 0) A.nxt_off[slot] = off;
+                    dst = A.nxt + (off << 4);
                 }
-                unsigned char* dst = ch.done ? A.cand + slot * A.cand_stride : A.nxt + slot * A.stride;
-                write_child(dst, P, ch, lane, first, vk, newrec, ch.done);
+                write_child(g, dst, P, ch, lane, first, vk, newrec, ch.done);
             };
             // account for / emit one child evaluated by the general routine
             auto emit = [&](const Child& ch, bool first, u64 newrec) {
@@ -407,12 +450,16 @@ __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
                     return;
                 }
                 if (MODE != MODE_WRITE) { s_children++; s_bytes += 8; if (ch.done) s_done++; }
-                const u64 key = beam_key((u32)ch.n_unb, mix64(ch.hs + ch.hv));
-                if (MODE == MODE_COUNT) {
-                    if (!ch.done) { s_active++; ko.push(A, lane, lane == 0, key); }
+                if (ch.done) {   // balanced children are written where they are first seen
+                    if (MODE != MODE_WRITE) place(ch, first, newrec);
                     return;
                 }
-                if (ch.done || MODE == MODE_DIRECT || notrunc || key < X) place(ch, first, newrec);
+                const u64 key = beam_key((u32)ch.n_unb, mix64(ch.hs + ch.hv));
+                if (MODE == MODE_COUNT) {
+                    s_active++; ko.push(A, lane, lane == 0, key); kmin = min(kmin, key);
+                    return;
+                }
+                if (MODE == MODE_DIRECT || notrunc || key < X) place(ch, first, newrec);
             };
 
             if (vk < 0) {
@@ -432,7 +479,7 @@ __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
                     }
                     const int2* alist = fwd ? g.out_e + out0 : g.in_e + in0;
                     const int alen = fwd ? nO : nI;
-                    const bool fastP = fast_graph && fmax < kSmall && maxabs < kSmall;
+                    const bool fastP = fast_graph && P.big < kSmall;
                     u64 kc_k0 = 0, kc_s0 = 0, kc_k1 = 0, kc_s1 = 0;   // hash sums of the k-scaled support, last two k
                     int n_adm = 0;
                     for (int base = 0; base < alen; base += 32) {
@@ -459,7 +506,7 @@ __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
                             const int q1 = __ldg(&g.col_ptr[a + 1]);
                             for (int qq = __ldg(&g.col_ptr[a]); qq < q1; ++qq) {
                                 const int2 e = __ldg(&g.col[qq]);
-                                const i64 efp = P.EF[e.x];
+                                const i64 efp = ef_lookup(P, e.x);
                                 const i64 x = (i64)k * efp + (i64)d * (i64)e.y;   // |.| < 2^60 + 2^60
                                 nu2 += (int)(x != 0) - (int)(efp != 0);
                             }
@@ -495,26 +542,32 @@ __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
                             const int nf = __popc(fast_m);
                             s_children += nf; s_bytes += 8 * nf; s_done += __popc(done_m);
                         }
+                        u32 keep_m;
                         if (MODE == MODE_COUNT) {
                             s_active += __popc(fast_m & ~done_m);
                             ko.push(A, lane, fast && !done, key);
+                            if (fast && !done) kmin = min(kmin, key);
+                            keep_m = done_m;
+                        } else if (MODE == MODE_WRITE) {
+                            keep_m = __ballot_sync(FULL, fast && !done && (notrunc || key < X));
                         } else {
-                            u32 keep_m = __ballot_sync(FULL, fast && (done || MODE == MODE_DIRECT || notrunc || key < X));
-                            while (keep_m) {
-                                const int l = __ffs(keep_m) - 1;
-                                keep_m &= keep_m - 1;
-                                Child ch;
-                                ch.status = CH_OK; ch.in_supp = false; ch.ia = -1; ch.g2 = 1;
-                                ch.a = __shfl_sync(FULL, a, l);
-                                ch.k = __shfl_sync(FULL, k, l);
-                                ch.T = w_bcast(d, l);
-                                ch.hs = w_bcast(hs2, l);
-                                ch.hv = w_bcast(hv2, l);
-                                ch.n_unb = __shfl_sync(FULL, nu2, l);
-                                ch.done = ch.n_unb == 0;
-                                const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : ch.a), (u32)(fwd ? ch.a : prim), 0u);
-                                place(ch, true, newrec);
-                            }
+                            keep_m = fast_m;
+                        }
+                        while (keep_m) {
+                            const int l = __ffs(keep_m) - 1;
+                            keep_m &= keep_m - 1;
+                            Child ch;
+                            ch.status = CH_OK; ch.in_supp = false; ch.ia = -1; ch.g2 = 1; ch.sign = +1;
+                            ch.a = __shfl_sync(FULL, a, l);
+                            ch.k = __shfl_sync(FULL, k, l);
+                            ch.T = w_bcast(d, l);
+                            ch.d = ch.T;
+                            ch.hs = w_bcast(hs2, l);
+                            ch.hv = w_bcast(hv2, l);
+                            ch.n_unb = __shfl_sync(FULL, nu2, l);
+                            ch.done = ch.n_unb == 0;
+                            const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : ch.a), (u32)(fwd ? ch.a : prim), 0u);
+                            place(ch, true, newrec);
                         }
                         // ---- everything else through the general routine
                         u32 slow_m = adm_m & ~fast_m;
@@ -568,15 +621,15 @@ __global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
                     emit(ch, false, newrec);
                 }
             }
+            if (MODE == MODE_COUNT) {
+                kmin = w_min(kmin);
+                if (lane == 0) A.pmin[p] = kmin;
+            }
         }
-        // ---- restore the shared scratch to zero for the next parent
+        // ---- restore the shared bitsets to zero for the next parent
         __syncwarp();
         for (int t = lane; t < P.n_supp; t += 32) P.sbits[P.arc[t] >> 5] = 0;
-        for (int w = lane; w < g.M32; w += 32) {
-            u32 bits = P.mseen[w];
-            while (bits) { P.EF[w * 32 + __ffs(bits) - 1] = 0; bits &= bits - 1; }
-            P.mseen[w] = 0;
-        }
+        for (int t = lane; t < P.n_unb; t += 32) P.ubits[P.efmet[t] >> 5] = 0;
         __syncwarp();
     }
     if (MODE == MODE_COUNT) ko.finish(A, lane);
@@ -599,14 +652,83 @@ __global__ void k_level_begin(Ctl* ctl) {
     ctl->n_next = 0; ctl->n_keys = 0; ctl->n_slots = 0; ctl->lvl_done = 0; ctl->lvl_children = 0; ctl->lvl_expanded = 0;
 }
 
+// ------------------------------------------------------------------ roots (INIT kernel of the paper)
+// One thread per seed set.  BUILD: every seed arc gets flux 1, the extra fluxes follow from Eq 2; the
+// root is classified like any other entry (balanced -> candidate, otherwise its beam key).  Seed sets are tiny, so
+// the quadratic duplicate scan below is cheaper than any scatter.  WRITE: the roots the beam keeps become level 0.
+template <bool WRITE>
+__global__ void __launch_bounds__(128) k_roots(const RootArgs R) {
+    const u64 r = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R.n_roots) return;
+    const DevGraph& g = R.g;
+    Ctl* ctl = R.ctl;
+    unsigned char* e = R.stage + (R.stage_off[r] << 4);
+    if (WRITE) {
+        const u64 key = R.keys[r];
+        if (key == kKeySentinel || !(ctl->notrunc || key < ctl->X)) return;
+        const u32 w0 = *(const u32*)e, nu = ((const u32*)e)[1];
+        const u64 units = entry_bytes(w0 & 0xffffu, w0 >> 16, nu) >> 4;
+        const u64 old = atomicAdd(&ctl->n_next, (1ULL << kAllocShift) | units);
+        const u64 slot = old >> kAllocShift, off = old & kAllocUnitMask;
+        if (slot >= R.max_frontier || off + units > R.frontier_units) { atomicOr(&ctl->error, (u32)ERR_FRONTIER); return; }
+        R.nxt_off[slot] = off;
+        uint4* dst = (uint4*)(R.nxt + (off << 4));
+        for (u64 c = 0; c < units; ++c) dst[c] = ((const uint4*)e)[c];
+        return;
+    }
+    if (r == 0) ctl->n_slots = R.n_roots;
+    const int s0 = R.seed_ptr[r], ns = R.seed_ptr[r + 1] - s0;
+    const int* arcs = R.seed_arc + s0;
+    // Eq 2 with every flux = 1: EF_i = sum of s_ia over the seed arcs; (t, q) is the first occurrence of its metabolite
+    auto ef_at = [&](int t, int q, i64& sum) -> bool {
+        const int met = g.col[q].x;
+        sum = 0;
+        for (int t2 = 0; t2 < ns; ++t2)
+            for (int q2 = g.col_ptr[arcs[t2]]; q2 < g.col_ptr[arcs[t2] + 1]; ++q2)
+                if (g.col[q2].x == met) {
+                    if (t2 < t || (t2 == t && q2 < q)) return false;
+                    sum += g.col[q2].y;
+                }
+        return sum != 0;
+    };
+    int nu = 0;
+    for (int t = 0; t < ns; ++t)
+        for (int q = g.col_ptr[arcs[t]]; q < g.col_ptr[arcs[t] + 1]; ++q) { i64 s; if (ef_at(t, q, s)) ++nu; }
+    i64* flux = (i64*)(e + kHdr);
+    i64* ef = flux + ns;          // n_vis = 0
+    u16* arc = (u16*)(ef + nu);
+    u16* efmet = arc + ns;
+    u64 hs = 0, big = 1;
+    for (int t = 0; t < ns; ++t) { flux[t] = 1; arc[t] = (u16)arcs[t]; hs += arc_term((u32)arcs[t], 1ULL); }
+    int w = 0;
+    for (int t = 0; t < ns; ++t)
+        for (int q = g.col_ptr[arcs[t]]; q < g.col_ptr[arcs[t] + 1]; ++q) {
+            i64 s;
+            if (ef_at(t, q, s)) { ef[w] = s; efmet[w] = (u16)g.col[q].x; big = max(big, abs64(s)); ++w; }
+        }
+    ((u32*)e)[0] = (u32)ns; ((u32*)e)[1] = (u32)nu;
+    ((u64*)e)[1] = hs; ((u64*)e)[2] = 0; ((u64*)e)[3] = big;
+    if (nu == 0) {   // balanced at once (arbiter "Done")
+        R.keys[r] = kKeySentinel;
+        atomicAdd(&ctl->lvl_done, 1ULL);
+        const u64 slot = atomicAdd(&ctl->n_cand, 1ULL);
+        if (slot >= R.max_cand) { atomicOr(&ctl->error, (u32)ERR_CAND); return; }
+        unsigned char* dst = R.cand + slot * R.cand_stride;
+        const u32 bytes = entry_bytes((u32)ns, 0, 0);
+        for (u32 c = 0; c < bytes / 16; ++c) ((uint4*)dst)[c] = ((const uint4*)e)[c];
+    } else {
+        R.keys[r] = beam_key((u32)nu, mix64(hs));
+        atomicAdd(&ctl->n_keys, 1ULL);
+    }
+}
+
 // ------------------------------------------------------------------ host launchers
 static size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 
 void expand_smem_layout(ExpandArgs& a) {
-    size_t off = align16(a.stride);   // staging holds the largest entry
-    a.sm_EF = (u32)off;    off = align16(off + (size_t)a.g.M * 8);
+    size_t off = align16(a.max_entry);   // staging holds the largest entry
     a.sm_sbits = (u32)off; off = align16(off + (size_t)a.g.W32 * 4);
-    a.sm_mseen = (u32)off; off = align16(off + (size_t)a.g.M32 * 4);
+    a.sm_ubits = (u32)off; off = align16(off + (size_t)a.g.M32 * 4);
     a.sm_group = (u32)off;
 }
 
@@ -614,12 +736,12 @@ void expand_smem_layout(ExpandArgs& a) {
 constexpr u64 kMaxGrid = 16384;
 u64 expand_key_slack() { return kMaxGrid * kWarps * kKeyChunk; }
 
-template <int MODE, bool ROOTS>
+template <int MODE>
 static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
     const size_t smem = (size_t)a.sm_group * kWarps;
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_expand<MODE, ROOTS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_expand<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
@@ -632,18 +754,21 @@ static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
     if (cap > kMaxGrid) cap = kMaxGrid;
     unsigned grid = (unsigned)(need < cap ? need : cap);
     if (grid == 0) grid = 1;
-    k_expand<MODE, ROOTS><<<grid, kBlock, smem, s>>>(a);
+    k_expand<MODE><<<grid, kBlock, smem, s>>>(a);
     return cudaGetLastError();
 }
 
-cudaError_t launch_expand(int mode, bool roots, const ExpandArgs& a, int sm_count, cudaStream_t s) {
-    if (roots) {
-        if (mode == MODE_COUNT) return launch_t<MODE_COUNT, true>(a, sm_count, s);
-        return launch_t<MODE_WRITE, true>(a, sm_count, s);
-    }
-    if (mode == MODE_COUNT) return launch_t<MODE_COUNT, false>(a, sm_count, s);
-    if (mode == MODE_WRITE) return launch_t<MODE_WRITE, false>(a, sm_count, s);
-    return launch_t<MODE_DIRECT, false>(a, sm_count, s);
+cudaError_t launch_expand(int mode, const ExpandArgs& a, int sm_count, cudaStream_t s) {
+    if (mode == MODE_COUNT) return launch_t<MODE_COUNT>(a, sm_count, s);
+    if (mode == MODE_WRITE) return launch_t<MODE_WRITE>(a, sm_count, s);
+    return launch_t<MODE_DIRECT>(a, sm_count, s);
+}
+
+cudaError_t launch_roots(bool write, const RootArgs& r, cudaStream_t s) {
+    const unsigned blocks = (unsigned)((r.n_roots + 127) / 128);
+    if (write) k_roots<true><<<blocks, 128, 0, s>>>(r);
+    else k_roots<false><<<blocks, 128, 0, s>>>(r);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_level_begin(Ctl* ctl, cudaStream_t s) {

@@ -7,7 +7,8 @@ namespace efm {
 // expand.cu
 void expand_smem_layout(ExpandArgs& a);
 u64 expand_key_slack();   // key slots the chunked reservation of the count pass can strand
-cudaError_t launch_expand(int mode /*0 count, 1 write, 2 direct*/, bool roots, const ExpandArgs& a, int sm_count, cudaStream_t s);
+cudaError_t launch_expand(int mode /*0 count, 1 write, 2 direct*/, const ExpandArgs& a, int sm_count, cudaStream_t s);
+cudaError_t launch_roots(bool write /*false: build + classify, true: keep the survivors*/, const RootArgs& r, cudaStream_t s);
 cudaError_t launch_level_begin(Ctl* ctl, cudaStream_t s);
 
 // post.cu
