@@ -93,7 +93,7 @@ struct ExpandArgs {
     int D, V, max_loop;
     int no_fast;                // EFM_F_NO_FASTPATH: every child through the warp-cooperative general routine
     // shared-memory carve-up per warp (bytes)
-    u32 sm_group, sm_sbits, sm_ubits;
+    u32 sm_group, sm_sbits, sm_upos, sm_misc;
 };
 
 // roots (INIT): seed sets uploaded by the host, entries built and classified on the device

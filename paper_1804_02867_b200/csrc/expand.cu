@@ -94,216 +94,6 @@ __device__ __forceinline__ u64 abs64(i64 v) { return (u64)(v < 0 ? -v : v); }
 // arc term of the state hash through the per-arc table of inner mixes (device_common.cuh: arc_term)
 __device__ __forceinline__ u64 arc_term_t(const DevGraph& g, u32 a, u64 f) { return mix64(__ldg(&g.arc_mix[a]) + f); }
 
-// ------------------------------------------------------------------ per-parent context (warp-uniform)
-struct Parent {
-    int n_supp, n_vis, n_unb;
-    const i64* flux; const u64* vis; const i64* ef; const u16* arc; const u16* efmet;   // shared-memory staging
-    u32* sbits;   // support bitset over arcs
-    u32* ubits;   // bitset over metabolites: member of the EF list
-    u64 hs, hv, big;
-    int istar;
-    i64 E;
-};
-struct Child {          // warp-uniform description of one child relative to its parent
-    int status; bool done;
-    int a; bool in_supp; int ia; int sign;
-    u64 k, g2, T, d;    // scale, common divisor, un-normalised new flux of arc a, |E| / gcd(|E|, c)
-    u64 hs, hv;         // hash sums of the child state
-    int n_unb;
-};
-
-__device__ __forceinline__ bool sbit(const u32* bits, int a) { return (bits[a >> 5] >> (a & 31)) & 1u; }
-
-// EF_met of the parent: zero unless met is in the list
-__device__ __forceinline__ i64 ef_lookup(const Parent& P, int met) {
-    if (met == P.istar) return P.E;
-    if (!sbit(P.ubits, met)) return 0;
-    for (int t = 0; t < P.n_unb; ++t) if ((int)P.efmet[t] == met) return P.ef[t];
-    return 0;
-}
-
-// General routine: evaluate the child bump(f, a, sign*|E|/c) with the whole warp.
-//   first: new visited record newrec; otherwise record oldrec is replaced by newrec
-__device__ __noinline__ void eval_child(const DevGraph& g, const Parent& P, int lane, int a, int c, int sign,
-                                        bool first, u64 oldrec, u64 newrec, Child& ch) {
-    const u64 absE = abs64(P.E);
-    const u64 gg = c == 1 ? 1ULL : gcd64(absE, (u64)c);
-    const u64 k = gg == 1 ? (u64)c : (u64)c / gg;
-    const u64 d = gg == 1 ? absE : absE / gg;
-    ch.a = a; ch.k = k; ch.g2 = 1; ch.d = d; ch.sign = sign;
-    ch.in_supp = sbit(P.sbits, a);
-    int ia = -1;
-    if (ch.in_supp) {   // position of a in the sorted support
-        for (int base = 0; base < P.n_supp && ia < 0; base += 32) {
-            const int t = base + lane;
-            const u32 hit = __ballot_sync(FULL, t < P.n_supp && P.arc[t] == a);
-            if (hit) ia = base + __ffs(hit) - 1;
-        }
-    }
-    ch.ia = ia;
-    // scaled fluxes F_t = k f_t, F_a = k f_a +- d: overflow first, then non-positive (order of the definition, O6).
-    // P.big >= every flux and every |EF| of the parent: products below the guard with it need no exact sweep.
-    const bool bigk = k > 1 && umul_gt_guard(k, P.big);
-    bool ovf = false, nonpos = false;
-    u64 T = d;
-    if (ch.in_supp) {
-        const u64 fa = (u64)P.flux[ia];
-        const u64 lo = k * fa, hi = __umul64hi(k, fa);
-        if (sign > 0) {
-            T = lo + d;
-            const u64 hi2 = hi + (T < lo);
-            ovf = hi2 != 0 || T > EFM_GUARD;
-        } else {
-            if (hi == 0 && lo <= d) { nonpos = true; T = 0; }           // k f_a - d <= 0
-            else { T = lo - d; const u64 hi2 = hi - (lo < d); ovf = hi2 != 0 || T > EFM_GUARD; }
-        }
-    }
-    if (bigk) {   // exact: the largest flux among t != ia (the new arc carries d <= |E| <= 2^62)
-        u64 mx = 0;
-        for (int t = lane; t < P.n_supp; t += 32) if (t != ia) mx = max(mx, (u64)P.flux[t]);
-        mx = w_max(mx);
-        ovf = ovf || umul_gt_guard(k, mx);
-    }
-    ch.T = T;
-    if (ovf) { ch.status = CH_OVERFLOW; return; }
-    if (nonpos) { ch.status = CH_NONPOS; return; }   // Prop 3, reading G11
-    // extra fluxes of the un-normalised child: EF'_i = k EF_i + sign d s_ia  (Eq 2 on the scaled fluxes)
-    const int qa0 = __ldg(&g.col_ptr[a]), qa1 = __ldg(&g.col_ptr[a + 1]);
-    bool ovf2 = false;
-    if (bigk) {   // exact sweep over the unbalanced metabolites outside col(a)
-        for (int t = lane; t < P.n_unb; t += 32) {
-            const int i = P.efmet[t];
-            bool in_a = false;
-            for (int r = qa0; r < qa1; ++r) in_a = in_a || __ldg(&g.col[r]).x == i;
-            if (!in_a) ovf2 = ovf2 || abs_gt_guard(mul_s((i64)k, P.ef[t]));
-        }
-    }
-    int delta = 0;
-    for (int q = qa0 + lane; q < qa1; q += 32) {
-        const int2 e = __ldg(&g.col[q]);
-        const i64 efp = ef_lookup(P, e.x);
-        S128 x = add_s(mul_s((i64)k, efp), mul_s(sign > 0 ? (i64)d : -(i64)d, (i64)e.y));
-        ovf2 = ovf2 || abs_gt_guard(x);
-        delta += (int)((x.lo | (u64)x.hi) != 0) - (int)(efp != 0);
-    }
-    if (__any_sync(FULL, ovf2)) { ch.status = CH_OVERFLOW; return; }
-    delta = __reduce_add_sync(FULL, delta);
-    ch.status = CH_OK;
-    ch.n_unb = P.n_unb + delta;
-    ch.done = ch.n_unb == 0;
-    // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and gcd(k, d) = 1.
-    // An arc of the support: g = gcd(k G, T) with G the gcd of the other fluxes; another flux equal to 1 gives G = 1
-    // and g = gcd(k, k f_a +- d) = gcd(k, d) = 1 without any gcd.
-    if (ch.in_supp && T != 1) {
-        bool one = false;
-        for (int t = lane; t < P.n_supp; t += 32) one = one || (t != ia && P.flux[t] == 1);
-        if (!__any_sync(FULL, one)) {
-            const bool narrow = P.big < (1ULL << 32);
-            u64 G = 0;
-            for (int t = lane; t < P.n_supp; t += 32)
-                if (t != ia) G = narrow ? (u64)gcd32((u32)G, (u32)P.flux[t]) : gcd64(G, (u64)P.flux[t]);
-            G = w_gcd(G, narrow);
-            ch.g2 = gcd64(k * G, T);   // k G <= k fmax <= 2^62
-        }
-    }
-    u64 hs;
-    if (k == 1 && ch.g2 == 1) {
-        hs = P.hs + arc_term_t(g, (u32)a, T) - (ch.in_supp ? arc_term_t(g, (u32)a, (u64)P.flux[ia]) : 0ULL);
-    } else {
-        hs = 0;
-        for (int t = lane; t < P.n_supp; t += 32) {
-            u64 F = t == ia ? T : k * (u64)P.flux[t];
-            if (ch.g2 > 1) F /= ch.g2;
-            hs += arc_term_t(g, (u32)P.arc[t], F);
-        }
-        hs = w_sum(hs);
-        if (!ch.in_supp) hs += arc_term_t(g, (u32)a, T);
-    }
-    ch.hs = hs;
-    ch.hv = P.hv + vis_term(newrec) - (first ? 0ULL : vis_term(oldrec));
-}
-
-// Write the child into a packed frontier entry (or a candidate slot: no visited records, no EF list).
-__device__ __forceinline__ void write_child(const DevGraph& g, unsigned char* dst, const Parent& P, const Child& ch,
-                                            int lane, bool first, int vk, u64 newrec, bool to_cand) {
-    const int n2 = P.n_supp + (ch.in_supp ? 0 : 1);
-    const int nv2 = to_cand ? 0 : P.n_vis + (first ? 1 : 0);
-    const int nu2 = to_cand ? 0 : ch.n_unb;
-    const u32 lt = (1u << lane) - 1u;
-    int ins = 0;   // a new arc goes where the ascending order puts it
-    if (!ch.in_supp)
-        for (int base = 0; base < P.n_supp; base += 32) {
-            const int t = base + lane;
-            ins += __popc(__ballot_sync(FULL, t < P.n_supp && (int)P.arc[t] < ch.a));
-        }
-    i64* flux2 = (i64*)(dst + kHdr);
-    u64* vis2 = (u64*)(flux2 + n2);
-    i64* ef2 = (i64*)(vis2 + nv2);
-    u16* arc2 = (u16*)(ef2 + nu2);
-    u16* efmet2 = arc2 + n2;
-    u64 mx = ch.in_supp ? 0ULL : (ch.g2 > 1 ? ch.T / ch.g2 : ch.T);
-    for (int t = lane; t < P.n_supp; t += 32) {
-        u64 F = t == ch.ia ? ch.T : ch.k * (u64)P.flux[t];
-        if (ch.g2 > 1) F /= ch.g2;
-        const int pos = t + ((!ch.in_supp && t >= ins) ? 1 : 0);
-        flux2[pos] = (i64)F;
-        arc2[pos] = P.arc[t];
-        mx = max(mx, F);
-    }
-    if (!ch.in_supp && lane == 0) { flux2[ins] = (i64)ch.T; arc2[ins] = (u16)ch.a; }
-    if (!to_cand) {
-        for (int u = lane; u < P.n_vis; u += 32) vis2[u] = (!first && u == vk) ? newrec : P.vis[u];
-        if (first && lane == 0) vis2[P.n_vis] = newrec;
-        // EF list of the child: EF' = (k EF + sign d s_.a) / g over the parent's list, then the metabolites of col(a)
-        // that were balanced in the parent.  eval_child / the fast path established that nothing exceeds 2^62, so
-        // the wrapping 64-bit arithmetic below is exact.
-        const int qa0 = __ldg(&g.col_ptr[ch.a]), qa1 = __ldg(&g.col_ptr[ch.a + 1]);
-        const u64 sd = ch.sign > 0 ? ch.d : (u64)0 - ch.d;
-        int base = 0;
-        for (int t0 = 0; t0 < P.n_unb; t0 += 32) {
-            const int t = t0 + lane;
-            const bool valid = t < P.n_unb;
-            i64 x = 0;
-            int met = 0;
-            if (valid) {
-                met = P.efmet[t];
-                i64 s = 0;
-                for (int q = qa0; q < qa1; ++q) { const int2 e = __ldg(&g.col[q]); if (e.x == met) s = e.y; }
-                x = (i64)(ch.k * (u64)P.ef[t] + sd * (u64)s);
-                if (ch.g2 > 1) x /= (i64)ch.g2;
-            }
-            const u32 nz = __ballot_sync(FULL, valid && x != 0);
-            if (valid && x != 0) {
-                const int pos = base + __popc(nz & lt);
-                ef2[pos] = x; efmet2[pos] = (u16)met;
-                mx = max(mx, abs64(x));
-            }
-            base += __popc(nz);
-        }
-        for (int q0 = qa0; q0 < qa1; q0 += 32) {
-            const int q = q0 + lane;
-            int2 e = make_int2(0, 0);
-            bool only = false;
-            if (q < qa1) { e = __ldg(&g.col[q]); only = !sbit(P.ubits, e.x); }
-            const u32 m = __ballot_sync(FULL, only);
-            if (only) {
-                i64 x = (i64)(sd * (u64)(i64)e.y);
-                if (ch.g2 > 1) x /= (i64)ch.g2;
-                const int pos = base + __popc(m & lt);
-                ef2[pos] = x; efmet2[pos] = (u16)e.x;
-                mx = max(mx, abs64(x));
-            }
-            base += __popc(m);
-        }
-        mx = w_max(mx);
-    }
-    if (lane == 0) {
-        uint4* h4 = (uint4*)dst;
-        h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2, (u32)ch.hs, (u32)(ch.hs >> 32));
-        h4[1] = make_uint4((u32)ch.hv, (u32)(ch.hv >> 32), (u32)mx, (u32)(mx >> 32));
-    }
-}
-
 // Per-warp chunked reservation of beam-key slots: one atomic per kKeyChunk keys instead of one per child.
 struct KeyOut {
     u64 base; u32 left;
@@ -340,311 +130,475 @@ __device__ __forceinline__ void scale_small(u64 absE, u32 c, u32& k, u64& d) {
     k = c / gg; d = absE / (u64)gg;
 }
 
+__device__ __forceinline__ bool sbit(const u32* bits, int a) { return (bits[a >> 5] >> (a & 31)) & 1u; }
+
+// per-warp statistics live in shared memory (one u64 each), flushed to the control block once per warp
+enum { SS_EXPANDED = 0, SS_CHILDREN, SS_DONE, SS_ACTIVE, SS_DEAD, SS_NOTEFM, SS_NONPOS, SS_OVF, SS_VISITED, SS_BYTES,
+       SS_KC,   // 4 words: the hash sums of the k-scaled support for the last two scales k (k0, s0, k1, s1)
+       SS_WORDS = SS_KC + 4 };
+
+// One kernel body, every routine inlined once: the staged parent is addressed through shared-memory pointers the
+// compiler can track, and both kinds of children (lane-parallel "fast" ones and warp-cooperative "general" ones) funnel
+// into a single evaluate / place / write sequence.
 template <int MODE>
-__global__ void __launch_bounds__(kBlock) k_expand(const ExpandArgs A) {
-    extern __shared__ __align__(16) unsigned char smem[];
-    const DevGraph& g = A.g;
+__global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ ExpandArgs A) {
+    extern __shared__ uint4 smem4[];
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
     const u32 lt = (1u << lane) - 1u;
-    unsigned char* gs = smem + (size_t)wib * A.sm_group;
+    unsigned char* gs = (unsigned char*)smem4 + (size_t)wib * A.sm_group;
     uint4* stage = (uint4*)gs;
-    Parent P;
-    P.sbits = (u32*)(gs + A.sm_sbits);
-    P.ubits = (u32*)(gs + A.sm_ubits);
-    for (int i = lane; i < g.W32; i += 32) P.sbits[i] = 0;
-    for (int i = lane; i < g.M32; i += 32) P.ubits[i] = 0;
+    u32* sbits = (u32*)(gs + A.sm_sbits);   // support bitset over arcs
+    u16* upos = (u16*)(gs + A.sm_upos);     // metabolite -> 1 + index in the EF list of the parent, 0 = balanced
+    u64* sst = (u64*)(gs + A.sm_misc);
+    for (int i = lane; i < A.g.W32; i += 32) sbits[i] = 0;
+    for (int i = lane; i < (A.g.M + 1) / 2; i += 32) ((u32*)upos)[i] = 0;
+    if (lane < SS_WORDS) sst[lane] = 0;
     __syncwarp();
 
     Ctl* ctl = A.ctl;
     const bool notrunc = MODE == MODE_WRITE ? ctl->notrunc != 0 : true;
     const u64 X = MODE == MODE_WRITE ? ctl->X : 0;
-    const bool fast_graph = !A.no_fast && g.max_coef < kSmallCoef;
-
-    // warp-uniform counters, flushed once per warp
-    u64 s_expanded = 0, s_children = 0, s_done = 0, s_active = 0, s_dead = 0, s_notefm = 0, s_nonpos = 0, s_ovf = 0,
-        s_visited = 0, s_bytes = 0;
+    const bool fast_graph = !A.no_fast && A.g.max_coef < kSmallCoef;
     KeyOut ko; ko.base = 0; ko.left = 0;
+    const u64 wstride = (u64)gridDim.x * (blockDim.x >> 5);
 
-    for (u64 p = (u64)blockIdx.x * kWarps + wib; p < A.n_cur; p += (u64)gridDim.x * kWarps) {
+    for (u64 p = (u64)blockIdx.x * (blockDim.x >> 5) + wib; p < A.n_cur; p += wstride) {
         if (MODE == MODE_WRITE && !notrunc && __ldg(&A.pmin[p]) >= X) continue;   // no child of p survives the beam
         // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
         const uint4* src = (const uint4*)(A.cur + (__ldg(&A.cur_off[p]) << 4));
-        const uint4 first = __ldg(src + lane);   // the buffers end in 512 spare bytes
-        const u32 hdr = __shfl_sync(FULL, first.x, 0);
-        P.n_supp = (int)(hdr & 0xffffu);
-        P.n_vis = (int)(hdr >> 16);
-        P.n_unb = (int)__shfl_sync(FULL, first.y, 0);
-        const u32 nch = entry_bytes((u32)P.n_supp, (u32)P.n_vis, (u32)P.n_unb) / 16;
-        if ((u32)lane < nch) stage[lane] = first;
+        const uint4 first16 = __ldg(src + lane);   // the buffers end in 512 spare bytes
+        const u32 hdr = __shfl_sync(FULL, first16.x, 0);
+        const int ns = (int)(hdr & 0xffffu), nv = (int)(hdr >> 16);
+        const int nu = (int)__shfl_sync(FULL, first16.y, 0);
+        const u32 nch = entry_bytes((u32)ns, (u32)nv, (u32)nu) / 16;
+        if ((u32)lane < nch) stage[lane] = first16;
         for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldg(src + c);
         __syncwarp();
-        P.hs = ((const u64*)stage)[1];
-        P.hv = ((const u64*)stage)[2];
-        P.big = ((const u64*)stage)[3];
-        P.flux = (const i64*)(gs + kHdr);
-        P.vis = (const u64*)(P.flux + P.n_supp);
-        P.ef = (const i64*)(P.vis + P.n_vis);
-        P.arc = (const u16*)(P.ef + P.n_unb);
-        P.efmet = P.arc + P.n_supp;
+        const u64 Phs = ((const u64*)stage)[1], Phv = ((const u64*)stage)[2], Pbig = ((const u64*)stage)[3];
+        const i64* flux = (const i64*)(gs + kHdr);
+        const u64* vis = (const u64*)(flux + ns);
+        const i64* ef = (const i64*)(vis + nv);
+        const u16* arc = (const u16*)(ef + nu);
+        const u16* efmet = arc + ns;
 
-        // ---- support bitset, unbalanced-metabolite bitset, PROC0: lowest unbalanced metabolite i* (reading G12)
-        for (int t = lane; t < P.n_supp; t += 32) { const u32 a = P.arc[t]; atomicOr(&P.sbits[a >> 5], 1u << (a & 31)); }
+        // ---- support bitset, EF index table, PROC0: lowest unbalanced metabolite i* (reading G12)
+        for (int t = lane; t < ns; t += 32) { const u32 a = arc[t]; atomicOr(&sbits[a >> 5], 1u << (a & 31)); }
         u32 best = 0xffffffffu;
-        for (int t = lane; t < P.n_unb; t += 32) {
-            const u32 i = P.efmet[t];
-            atomicOr(&P.ubits[i >> 5], 1u << (i & 31));
+        for (int t = lane; t < nu; t += 32) {
+            const u32 i = efmet[t];
+            upos[i] = (u16)(t + 1);
             best = min(best, (i << 16) | (u32)t);
         }
         best = __reduce_min_sync(FULL, best);
+        if (lane == 0) { sst[SS_KC] = 0; sst[SS_KC + 2] = 0; }
         __syncwarp();
-        const int cnt = P.n_unb;
         const int istar = (int)(best >> 16);
-        P.istar = istar;
-        P.E = P.ef[best & 0xffffu];
-        {
-            const bool fwd = P.E > 0;
-            const u64 absE = abs64(P.E);
-            if (MODE != MODE_WRITE) { s_expanded++; s_bytes += algo_entry_bytes((u32)P.n_supp, (u32)P.n_vis); }
-            u64 kmin = ~0ULL;   // smallest key among the active children of p (count pass)
-            // visited?
-            int vk = -1;
-            for (int base = 0; base < P.n_vis && vk < 0; base += 32) {
-                const int u = base + lane;
-                const u32 hit = __ballot_sync(FULL, u < P.n_vis && (int)((P.vis[u] >> 32) & 0xffffu) == istar);
-                if (hit) vk = base + __ffs(hit) - 1;
-            }
-            const int in0 = __ldg(&g.in_ptr[istar]), nI = __ldg(&g.in_ptr[istar + 1]) - in0;
-            const int out0 = __ldg(&g.out_ptr[istar]), nO = __ldg(&g.out_ptr[istar + 1]) - out0;
+        const i64 E = ef[best & 0xffffu];
+        const bool fwd = E > 0;
+        const u64 absE = abs64(E);
+        auto ef_of = [&](int met) -> i64 { const u32 u = upos[met]; return u ? ef[u - 1] : 0; };
+        if (MODE != MODE_WRITE && lane == 0) { sst[SS_EXPANDED]++; sst[SS_BYTES] += algo_entry_bytes((u32)ns, (u32)nv); }
+        u64 kmin = ~0ULL;   // smallest key among the active children of p (count pass)
+        // visited?
+        int vk = -1;
+        for (int base = 0; base < nv && vk < 0; base += 32) {
+            const int u = base + lane;
+            const u32 hit = __ballot_sync(FULL, u < nv && (int)((vis[u] >> 32) & 0xffffu) == istar);
+            if (hit) vk = base + __ffs(hit) - 1;
+        }
+        const bool firstv = vk < 0;
+        const int in0 = __ldg(&A.g.in_ptr[istar]), nI = __ldg(&A.g.in_ptr[istar + 1]) - in0;
+        const int out0 = __ldg(&A.g.out_ptr[istar]), nO = __ldg(&A.g.out_ptr[istar + 1]) - out0;
 
-            // materialise one kept child (warp-uniform description)
-            auto place = [&](const Child& ch, bool first, u64 newrec) {
-                const int n2 = P.n_supp + (ch.in_supp ? 0 : 1), nv2 = P.n_vis + (first ? 1 : 0);
-                s_bytes += algo_entry_bytes((u32)n2, (u32)nv2);
+        // ---- what to branch over: the OR-alternatives of i* (first visit) or the single Eq 4 / Eq 5 bump (revisit)
+        const int2* alist = nullptr;
+        int alen = 0, prim = -1;
+        int r_a = 0, r_c = 1, r_sign = +1;
+        u64 rec = 0, r_newrec = 0;
+        if (firstv) {
+            // PROC1 / PROC1' (Eq 3; readings G1, G13, G14, G15, G22)
+            if (nv >= A.V) {
+                if (MODE != MODE_WRITE && lane == 0) sst[SS_VISITED]++;
+            } else {
+                // primary on the side the flux arrives from: lowest arc of that side in the support (G13)
+                const int2* plist = fwd ? A.g.in_e + in0 : A.g.out_e + out0;
+                const int plen = fwd ? nI : nO;
+                for (int base = 0; base < plen && prim < 0; base += 32) {
+                    const int q = base + lane;
+                    const int pa = q < plen ? __ldg(&plist[q]).x : -1;
+                    const u32 bal = __ballot_sync(FULL, pa >= 0 && sbit(sbits, pa));
+                    if (bal) prim = __shfl_sync(FULL, pa, __ffs(bal) - 1);
+                }
+                alist = fwd ? A.g.out_e + out0 : A.g.in_e + in0;
+                alen = fwd ? nO : nI;
+            }
+        } else {
+            // PROC2-4 (readings G2-G5)
+            rec = vis[vk];
+            const int cntv = (int)(rec >> 48) + 1;
+            if (cntv > A.max_loop) {
+                if (MODE != MODE_WRITE && lane == 0) sst[SS_NOTEFM]++;
+            } else {
+                const int PI = (int)((rec >> 16) & 0xffffu), PO = (int)(rec & 0xffffu);
+                int lPI = -1, lPO = -1, cPI = 0, cPO = 0;
+                for (int q = lane; q < nI; q += 32) { const int2 e = __ldg(&A.g.in_e[in0 + q]); if (e.x == PI) { lPI = q; cPI = e.y; } }
+                for (int q = lane; q < nO; q += 32) { const int2 e = __ldg(&A.g.out_e[out0 + q]); if (e.x == PO) { lPO = q; cPO = e.y; } }
+                lPI = __reduce_max_sync(FULL, lPI); cPI = __reduce_max_sync(FULL, cPI);
+                lPO = __reduce_max_sync(FULL, lPO); cPO = __reduce_max_sync(FULL, cPO);
+                // Def 11: forward PO ~ SI, backward PI ~ SO, secondary = any arc of that side in the support (G5)
+                bool dep = false;
+                const i64 doff = __ldg(&A.g.dep_off[istar]);
+                if (fwd) {
+                    for (int q = lane; q < nI; q += 32) {
+                        const i64 b = doff + (i64)lPO * nI + q;
+                        dep = dep || (sbit(sbits, __ldg(&A.g.in_e[in0 + q]).x) && ((__ldg(&A.g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
+                    }
+                } else {
+                    for (int q = lane; q < nO; q += 32) {
+                        const i64 b = doff + (i64)q * nI + lPI;
+                        dep = dep || (sbit(sbits, __ldg(&A.g.out_e[out0 + q]).x) && ((__ldg(&A.g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
+                    }
+                }
+                dep = __any_sync(FULL, dep);
+                if (fwd) { if (!dep) { r_a = PO; r_c = cPO; r_sign = +1; } else { r_a = PI; r_c = cPI; r_sign = -1; } }   // Eq 4 / Eq 5
+                else     { if (!dep) { r_a = PI; r_c = cPI; r_sign = +1; } else { r_a = PO; r_c = cPO; r_sign = -1; } }
+                r_newrec = vis_pack((u32)istar, (u32)PI, (u32)PO, (u32)cntv);
+                alen = 1;
+            }
+        }
+        const bool fastP = firstv && fast_graph && Pbig < kSmall;
+        int n_adm = 0;
+        for (int base = 0; base < alen; base += 32) {
+            const int q = base + lane;
+            int a = -1, c = 1;
+            bool adm = false, insup = false;
+            if (firstv) {
+                if (q < alen) {
+                    const int2 e = __ldg(&alist[q]);
+                    a = e.x; c = e.y;
+                    const int tw = __ldg(&A.g.twin[a]);
+                    insup = sbit(sbits, a);
+                    adm = !(tw >= 0 && sbit(sbits, tw)) && (insup || ns < A.D);
+                }
+            } else if (lane == 0) {
+                a = r_a; c = r_c; adm = true; insup = true;   // PI / PO are arcs of the support
+            }
+            const u32 adm_m = __ballot_sync(FULL, adm);
+            if (adm_m == 0) continue;
+            n_adm += __popc(adm_m);
+            // ---- lane-parallel evaluation: new arc, small integers => no overflow, no common factor
+            const bool fast = adm && !insup && fastP;
+            const u32 fast_m = __ballot_sync(FULL, fast);
+            u32 k = 1; u64 d = absE;
+            int nu2 = nu;
+            u64 hs2 = 0, hv2 = 0, key = 0;
+            if (fast_m) {
+                if (fast) {
+                    if (c != 1) scale_small(absE, (u32)c, k, d);
+                    const int q1 = __ldg(&A.g.col_ptr[a + 1]);
+                    for (int qq = __ldg(&A.g.col_ptr[a]); qq < q1; ++qq) {
+                        const int2 e = __ldg(&A.g.col[qq]);
+                        const i64 efp = ef_of(e.x);
+                        const i64 x = (i64)k * efp + (i64)d * (i64)e.y;   // |.| < 2^60 + 2^60
+                        nu2 += (int)(x != 0) - (int)(efp != 0);
+                    }
+                }
+                u64 hsb = Phs;
+                u32 need = __ballot_sync(FULL, fast && k > 1);
+                while (need) {
+                    const u32 kk = __shfl_sync(FULL, k, __ffs(need) - 1);
+                    u64 s;
+                    if ((u64)kk == sst[SS_KC]) s = sst[SS_KC + 1];
+                    else if ((u64)kk == sst[SS_KC + 2]) s = sst[SS_KC + 3];
+                    else {
+                        s = 0;
+                        for (int t = lane; t < ns; t += 32) s += arc_term_t(A.g, (u32)arc[t], (u64)kk * (u64)flux[t]);
+                        s = w_sum(s);
+                        __syncwarp();
+                        if (lane == 0) { sst[SS_KC + 2] = sst[SS_KC]; sst[SS_KC + 3] = sst[SS_KC + 1]; sst[SS_KC] = kk; sst[SS_KC + 1] = s; }
+                        __syncwarp();
+                    }
+                    const bool same = fast && k == kk;
+                    if (same) hsb = s;
+                    need &= ~__ballot_sync(FULL, same);
+                }
+                if (fast) {
+                    const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : a), (u32)(fwd ? a : prim), 0u);
+                    hs2 = hsb + arc_term_t(A.g, (u32)a, d);
+                    hv2 = Phv + vis_term(newrec);
+                    key = beam_key((u32)nu2, mix64(hs2 + hv2));
+                }
+            }
+            const u32 done_m = __ballot_sync(FULL, fast && nu2 == 0);
+            if (MODE != MODE_WRITE && lane == 0) {
+                const int nf = __popc(fast_m);
+                sst[SS_CHILDREN] += nf; sst[SS_BYTES] += 8 * nf; sst[SS_DONE] += __popc(done_m);
+            }
+            u32 keep_m;
+            if (MODE == MODE_COUNT) {
+                const bool act = fast && nu2 != 0;
+                if (lane == 0) sst[SS_ACTIVE] += __popc(fast_m & ~done_m);
+                ko.push(A, lane, act, key);
+                if (act) kmin = min(kmin, key);
+                keep_m = done_m;
+            } else if (MODE == MODE_WRITE) {
+                keep_m = __ballot_sync(FULL, fast && nu2 != 0 && (notrunc || key < X));
+            } else {
+                keep_m = fast_m;
+            }
+            // ---- one child at a time: general evaluation (arc of the support, large integers) and / or materialisation
+            const u32 slow_m = adm_m & ~fast_m;
+            u32 work_m = keep_m | slow_m;
+            while (work_m) {
+                const int l = __ffs(work_m) - 1;
+                work_m &= work_m - 1;
+                const bool general = (slow_m >> l) & 1u;
+                // warp-uniform description of the child relative to its parent
+                const int ca = __shfl_sync(FULL, a, l);
+                u64 ck = __shfl_sync(FULL, k, l);        // scale
+                u64 cd = w_bcast(d, l);                  // |E| / gcd(|E|, c)
+                u64 cT = cd;                             // un-normalised new flux of arc ca
+                u64 cg = 1;                              // common divisor of the un-normalised child
+                u64 chs = w_bcast(hs2, l), chv = w_bcast(hv2, l);
+                int cnu = __shfl_sync(FULL, nu2, l);
+                int csign = +1, cia = -1;
+                bool cin = false, keep = true;
+                u64 newrec = firstv ? vis_pack((u32)istar, (u32)(fwd ? prim : ca), (u32)(fwd ? ca : prim), 0u) : r_newrec;
+                const int qa0 = __ldg(&A.g.col_ptr[ca]), qa1 = __ldg(&A.g.col_ptr[ca + 1]);
+                if (general) {
+                    // bump(f, a, sign*|E|/c) of SURVEY.md 8(c) O6 with the whole warp
+                    const int cc = __shfl_sync(FULL, c, l);
+                    csign = firstv ? +1 : r_sign;
+                    const u64 gg = cc == 1 ? 1ULL : gcd64(absE, (u64)cc);
+                    ck = gg == 1 ? (u64)cc : (u64)cc / gg;
+                    cd = gg == 1 ? absE : absE / gg;
+                    cin = sbit(sbits, ca);
+                    if (cin) {   // position of the arc in the sorted support
+                        for (int b2 = 0; b2 < ns && cia < 0; b2 += 32) {
+                            const int t = b2 + lane;
+                            const u32 hit = __ballot_sync(FULL, t < ns && arc[t] == ca);
+                            if (hit) cia = b2 + __ffs(hit) - 1;
+                        }
+                    }
+                    // scaled fluxes F_t = k f_t, F_a = k f_a +- d: overflow first, then non-positive (order of O6).
+                    // Pbig >= every flux and |EF| of the parent: products below the guard with it need no exact sweep.
+                    const bool bigk = ck > 1 && umul_gt_guard(ck, Pbig);
+                    bool ovf = false, nonpos = false;
+                    cT = cd;
+                    if (cin) {
+                        const u64 fa = (u64)flux[cia];
+                        const u64 lo = ck * fa, hi = __umul64hi(ck, fa);
+                        if (csign > 0) {
+                            cT = lo + cd;
+                            const u64 hi2 = hi + (cT < lo);
+                            ovf = hi2 != 0 || cT > EFM_GUARD;
+                        } else {
+                            if (hi == 0 && lo <= cd) { nonpos = true; cT = 0; }           // k f_a - d <= 0
+                            else { cT = lo - cd; const u64 hi2 = hi - (lo < cd); ovf = hi2 != 0 || cT > EFM_GUARD; }
+                        }
+                    }
+                    if (bigk) {   // exact: the largest flux among t != ia (a new arc carries d <= |E| <= 2^62)
+                        u64 mx = 0;
+                        for (int t = lane; t < ns; t += 32) if (t != cia) mx = max(mx, (u64)flux[t]);
+                        mx = w_max(mx);
+                        ovf = ovf || umul_gt_guard(ck, mx);
+                    }
+                    int status = ovf ? CH_OVERFLOW : (nonpos ? CH_NONPOS : CH_OK);   // Prop 3, G11
+                    if (status == CH_OK) {
+                        // extra fluxes of the un-normalised child: EF'_i = k EF_i + sign d s_ia (Eq 2 on the scaled fluxes)
+                        bool ovf2 = false;
+                        if (bigk) {   // exact sweep over the unbalanced metabolites outside col(a)
+                            for (int t = lane; t < nu; t += 32) {
+                                const int i = efmet[t];
+                                bool in_a = false;
+                                for (int r = qa0; r < qa1; ++r) in_a = in_a || __ldg(&A.g.col[r]).x == i;
+                                if (!in_a) ovf2 = ovf2 || abs_gt_guard(mul_s((i64)ck, ef[t]));
+                            }
+                        }
+                        int delta = 0;
+                        for (int qq = qa0 + lane; qq < qa1; qq += 32) {
+                            const int2 e = __ldg(&A.g.col[qq]);
+                            const i64 efp = ef_of(e.x);
+                            const S128 x = add_s(mul_s((i64)ck, efp), mul_s(csign > 0 ? (i64)cd : -(i64)cd, (i64)e.y));
+                            ovf2 = ovf2 || abs_gt_guard(x);
+                            delta += (int)((x.lo | (u64)x.hi) != 0) - (int)(efp != 0);
+                        }
+                        if (__any_sync(FULL, ovf2)) status = CH_OVERFLOW;
+                        else cnu = nu + __reduce_add_sync(FULL, delta);
+                    }
+                    if (status != CH_OK) {
+                        if (MODE != MODE_WRITE && lane == 0) sst[status == CH_OVERFLOW ? SS_OVF : SS_NONPOS]++;
+                        continue;
+                    }
+                    // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and
+                    // gcd(k, d) = 1.  An arc of the support: g = gcd(k G, T) with G the gcd of the other fluxes; another
+                    // flux equal to 1 gives G = 1 and g = gcd(k, k f_a +- d) = gcd(k, d) = 1 without any gcd.
+                    if (cin && cT != 1) {
+                        bool one = false;
+                        for (int t = lane; t < ns; t += 32) one = one || (t != cia && flux[t] == 1);
+                        if (!__any_sync(FULL, one)) {
+                            const bool narrow = Pbig < (1ULL << 32);
+                            u64 G = 0;
+                            for (int t = lane; t < ns; t += 32)
+                                if (t != cia) G = narrow ? (u64)gcd32((u32)G, (u32)flux[t]) : gcd64(G, (u64)flux[t]);
+                            G = w_gcd(G, narrow);
+                            cg = gcd64(ck * G, cT);   // k G <= k fmax <= 2^62
+                        }
+                    }
+                    if (ck == 1 && cg == 1) {
+                        chs = Phs + arc_term_t(A.g, (u32)ca, cT) - (cin ? arc_term_t(A.g, (u32)ca, (u64)flux[cia]) : 0ULL);
+                    } else {
+                        chs = 0;
+                        for (int t = lane; t < ns; t += 32) {
+                            u64 F = t == cia ? cT : ck * (u64)flux[t];
+                            if (cg > 1) F /= cg;
+                            chs += arc_term_t(A.g, (u32)arc[t], F);
+                        }
+                        chs = w_sum(chs);
+                        if (!cin) chs += arc_term_t(A.g, (u32)ca, cT);
+                    }
+                    chv = Phv + vis_term(newrec) - (firstv ? 0ULL : vis_term(rec));
+                    // account for the child, classify it, decide whether it is materialised in this pass
+                    const bool cdone = cnu == 0;
+                    if (MODE != MODE_WRITE && lane == 0) { sst[SS_CHILDREN]++; sst[SS_BYTES] += 8; if (cdone) sst[SS_DONE]++; }
+                    if (cdone) keep = MODE != MODE_WRITE;   // balanced children are written where they are first seen
+                    else {
+                        const u64 ckey = beam_key((u32)cnu, mix64(chs + chv));
+                        if (MODE == MODE_COUNT) {
+                            if (lane == 0) sst[SS_ACTIVE]++;
+                            ko.push(A, lane, lane == 0, ckey);
+                            kmin = min(kmin, ckey);
+                            keep = false;
+                        } else keep = MODE == MODE_DIRECT || notrunc || ckey < X;
+                    }
+                }
+                if (!keep) continue;
+                // ---- place: a candidate slot (balanced) or a packed entry of the next frontier
+                const bool to_cand = cnu == 0;
+                const int n2 = ns + (cin ? 0 : 1);
+                const int nv2 = to_cand ? 0 : nv + (firstv ? 1 : 0);
+                const int nu2c = to_cand ? 0 : cnu;
+                if (lane == 0) sst[SS_BYTES] += algo_entry_bytes((u32)n2, (u32)(nv + (firstv ? 1 : 0)));
                 unsigned char* dst;
-                if (ch.done) {
+                if (to_cand) {
                     u64 slot = 0;
                     if (lane == 0) slot = atomicAdd(&ctl->n_cand, 1ULL);
                     slot = w_bcast(slot, 0);
-                    if (slot >= A.max_cand) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_CAND); return; }
+                    if (slot >= A.max_cand) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_CAND); continue; }
                     dst = A.cand + slot * A.cand_stride;
                 } else {
-                    const u64 units = entry_bytes((u32)n2, (u32)nv2, (u32)ch.n_unb) >> 4;
+                    const u64 units = entry_bytes((u32)n2, (u32)nv2, (u32)nu2c) >> 4;
                     u64 old = 0;
                     if (lane == 0) old = atomicAdd(&ctl->n_next, (1ULL << kAllocShift) | units);
                     old = w_bcast(old, 0);
                     const u64 slot = old >> kAllocShift, off = old & kAllocUnitMask;
                     if (slot >= A.max_frontier || off + units > A.frontier_units) {
                         if (lane == 0) atomicOr(&ctl->error, (u32)ERR_FRONTIER);
-                        return;
+                        continue;
                     }
                     if (lane == 0) A.nxt_off[slot] = off;
                     dst = A.nxt + (off << 4);
                 }
-                write_child(g, dst, P, ch, lane, first, vk, newrec, ch.done);
-            };
-            // account for / emit one child evaluated by the general routine
-            auto emit = [&](const Child& ch, bool first, u64 newrec) {
-                if (ch.status != CH_OK) {
-                    if (MODE != MODE_WRITE) { if (ch.status == CH_OVERFLOW) s_ovf++; else s_nonpos++; }
-                    return;
-                }
-                if (MODE != MODE_WRITE) { s_children++; s_bytes += 8; if (ch.done) s_done++; }
-                if (ch.done) {   // balanced children are written where they are first seen
-                    if (MODE != MODE_WRITE) place(ch, first, newrec);
-                    return;
-                }
-                const u64 key = beam_key((u32)ch.n_unb, mix64(ch.hs + ch.hv));
-                if (MODE == MODE_COUNT) {
-                    s_active++; ko.push(A, lane, lane == 0, key); kmin = min(kmin, key);
-                    return;
-                }
-                if (MODE == MODE_DIRECT || notrunc || key < X) place(ch, first, newrec);
-            };
-
-            if (vk < 0) {
-                // ---- first visit: PROC1 / PROC1' (Eq 3; readings G1, G13, G14, G15, G22)
-                if (P.n_vis >= A.V) {
-                    if (MODE != MODE_WRITE) s_visited++;
-                } else {
-                    // primary on the side the flux arrives from: lowest arc of that side in the support (G13)
-                    const int2* plist = fwd ? g.in_e + in0 : g.out_e + out0;
-                    const int plen = fwd ? nI : nO;
-                    int prim = -1;
-                    for (int base = 0; base < plen && prim < 0; base += 32) {
-                        const int q = base + lane;
-                        const int pa = q < plen ? __ldg(&plist[q]).x : -1;
-                        const u32 bal = __ballot_sync(FULL, pa >= 0 && sbit(P.sbits, pa));
-                        if (bal) prim = __shfl_sync(FULL, pa, __ffs(bal) - 1);
+                // ---- write
+                int ins = 0;   // a new arc goes where the ascending order puts it
+                if (!cin)
+                    for (int b2 = 0; b2 < ns; b2 += 32) {
+                        const int t = b2 + lane;
+                        ins += __popc(__ballot_sync(FULL, t < ns && (int)arc[t] < ca));
                     }
-                    const int2* alist = fwd ? g.out_e + out0 : g.in_e + in0;
-                    const int alen = fwd ? nO : nI;
-                    const bool fastP = fast_graph && P.big < kSmall;
-                    u64 kc_k0 = 0, kc_s0 = 0, kc_k1 = 0, kc_s1 = 0;   // hash sums of the k-scaled support, last two k
-                    int n_adm = 0;
-                    for (int base = 0; base < alen; base += 32) {
-                        const int q = base + lane;
-                        int a = -1, c = 1;
-                        bool adm = false, insup = false;
-                        if (q < alen) {
-                            const int2 e = __ldg(&alist[q]);
-                            a = e.x; c = e.y;
-                            const int tw = __ldg(&g.twin[a]);
-                            insup = sbit(P.sbits, a);
-                            adm = !(tw >= 0 && sbit(P.sbits, tw)) && (insup || P.n_supp < A.D);
-                        }
-                        const u32 adm_m = __ballot_sync(FULL, adm);
-                        if (adm_m == 0) continue;
-                        n_adm += __popc(adm_m);
-                        // ---- lane-parallel evaluation: new arc, small integers => no overflow, no common factor
-                        const bool fast = adm && !insup && fastP;
-                        const u32 fast_m = __ballot_sync(FULL, fast);
-                        u32 k = 1; u64 d = absE;
-                        int nu2 = cnt;
-                        if (fast) {
-                            if (c != 1) scale_small(absE, (u32)c, k, d);
-                            const int q1 = __ldg(&g.col_ptr[a + 1]);
-                            for (int qq = __ldg(&g.col_ptr[a]); qq < q1; ++qq) {
-                                const int2 e = __ldg(&g.col[qq]);
-                                const i64 efp = ef_lookup(P, e.x);
-                                const i64 x = (i64)k * efp + (i64)d * (i64)e.y;   // |.| < 2^60 + 2^60
-                                nu2 += (int)(x != 0) - (int)(efp != 0);
-                            }
-                        }
-                        u64 hsb = P.hs;
-                        u32 need = __ballot_sync(FULL, fast && k > 1);
-                        while (need) {
-                            const u32 kk = __shfl_sync(FULL, k, __ffs(need) - 1);
-                            u64 s;
-                            if ((u64)kk == kc_k0) s = kc_s0;
-                            else if ((u64)kk == kc_k1) s = kc_s1;
-                            else {
-                                s = 0;
-                                for (int t = lane; t < P.n_supp; t += 32) s += arc_term_t(g, (u32)P.arc[t], (u64)kk * (u64)P.flux[t]);
-                                s = w_sum(s);
-                                kc_k1 = kc_k0; kc_s1 = kc_s0; kc_k0 = kk; kc_s0 = s;
-                            }
-                            const bool same = fast && k == kk;
-                            if (same) hsb = s;
-                            need &= ~__ballot_sync(FULL, same);
-                        }
-                        u64 hs2 = 0, hv2 = 0, key = 0;
-                        bool done = false;
-                        if (fast) {
-                            const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : a), (u32)(fwd ? a : prim), 0u);
-                            hs2 = hsb + arc_term_t(g, (u32)a, d);
-                            hv2 = P.hv + vis_term(newrec);
-                            key = beam_key((u32)nu2, mix64(hs2 + hv2));
-                            done = nu2 == 0;
-                        }
-                        const u32 done_m = __ballot_sync(FULL, done);
-                        if (MODE != MODE_WRITE) {
-                            const int nf = __popc(fast_m);
-                            s_children += nf; s_bytes += 8 * nf; s_done += __popc(done_m);
-                        }
-                        u32 keep_m;
-                        if (MODE == MODE_COUNT) {
-                            s_active += __popc(fast_m & ~done_m);
-                            ko.push(A, lane, fast && !done, key);
-                            if (fast && !done) kmin = min(kmin, key);
-                            keep_m = done_m;
-                        } else if (MODE == MODE_WRITE) {
-                            keep_m = __ballot_sync(FULL, fast && !done && (notrunc || key < X));
-                        } else {
-                            keep_m = fast_m;
-                        }
-                        while (keep_m) {
-                            const int l = __ffs(keep_m) - 1;
-                            keep_m &= keep_m - 1;
-                            Child ch;
-                            ch.status = CH_OK; ch.in_supp = false; ch.ia = -1; ch.g2 = 1; ch.sign = +1;
-                            ch.a = __shfl_sync(FULL, a, l);
-                            ch.k = __shfl_sync(FULL, k, l);
-                            ch.T = w_bcast(d, l);
-                            ch.d = ch.T;
-                            ch.hs = w_bcast(hs2, l);
-                            ch.hv = w_bcast(hv2, l);
-                            ch.n_unb = __shfl_sync(FULL, nu2, l);
-                            ch.done = ch.n_unb == 0;
-                            const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : ch.a), (u32)(fwd ? ch.a : prim), 0u);
-                            place(ch, true, newrec);
-                        }
-                        // ---- everything else through the general routine
-                        u32 slow_m = adm_m & ~fast_m;
-                        while (slow_m) {
-                            const int l = __ffs(slow_m) - 1;
-                            slow_m &= slow_m - 1;
-                            const int sa = __shfl_sync(FULL, a, l);
-                            const int sc = __shfl_sync(FULL, c, l);
-                            const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : sa), (u32)(fwd ? sa : prim), 0u);
-                            Child ch;
-                            eval_child(g, P, lane, sa, sc, +1, true, 0ULL, newrec, ch);
-                            emit(ch, true, newrec);
-                        }
-                    }
-                    if (n_adm == 0 && MODE != MODE_WRITE) s_dead++;
+                i64* flux2 = (i64*)(dst + kHdr);
+                u64* vis2 = (u64*)(flux2 + n2);
+                i64* ef2 = (i64*)(vis2 + nv2);
+                u16* arc2 = (u16*)(ef2 + nu2c);
+                u16* efmet2 = arc2 + n2;
+                u64 mx = cin ? 0ULL : cT;   // a new arc never comes with a common divisor
+                for (int t = lane; t < ns; t += 32) {
+                    u64 F = t == cia ? cT : ck * (u64)flux[t];
+                    if (cg > 1) F /= cg;
+                    const int pos = t + ((!cin && t >= ins) ? 1 : 0);
+                    flux2[pos] = (i64)F;
+                    arc2[pos] = arc[t];
+                    mx = max(mx, F);
                 }
-            } else {
-                // ---- revisit: PROC2-4 (readings G2-G5)
-                const u64 rec = P.vis[vk];
-                const int cntv = (int)(rec >> 48) + 1;
-                if (cntv > A.max_loop) {
-                    if (MODE != MODE_WRITE) s_notefm++;
-                } else {
-                    const int PI = (int)((rec >> 16) & 0xffffu), PO = (int)(rec & 0xffffu);
-                    int lPI = -1, lPO = -1, cPI = 0, cPO = 0;
-                    for (int q = lane; q < nI; q += 32) { const int2 e = __ldg(&g.in_e[in0 + q]); if (e.x == PI) { lPI = q; cPI = e.y; } }
-                    for (int q = lane; q < nO; q += 32) { const int2 e = __ldg(&g.out_e[out0 + q]); if (e.x == PO) { lPO = q; cPO = e.y; } }
-                    lPI = __reduce_max_sync(FULL, lPI); cPI = __reduce_max_sync(FULL, cPI);
-                    lPO = __reduce_max_sync(FULL, lPO); cPO = __reduce_max_sync(FULL, cPO);
-                    // Def 11: forward PO ~ SI, backward PI ~ SO, secondary = any arc of that side in the support (G5)
-                    bool dep = false;
-                    const i64 doff = __ldg(&g.dep_off[istar]);
-                    if (fwd) {
-                        for (int q = lane; q < nI; q += 32) {
-                            const i64 b = doff + (i64)lPO * nI + q;
-                            dep = dep || (sbit(P.sbits, __ldg(&g.in_e[in0 + q]).x) && ((__ldg(&g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
+                if (!cin && lane == 0) { flux2[ins] = (i64)cT; arc2[ins] = (u16)ca; }
+                if (!to_cand) {
+                    for (int u = lane; u < nv; u += 32) vis2[u] = (!firstv && u == vk) ? newrec : vis[u];
+                    if (firstv && lane == 0) vis2[nv] = newrec;
+                    // EF list of the child: EF' = (k EF + sign d s_.a) / g over the parent's list, then the metabolites
+                    // of col(a) that were balanced in the parent.  The evaluation above (or the bounds of the fast path)
+                    // established that nothing exceeds 2^62, so the wrapping 64-bit arithmetic is exact.
+                    const u64 sd = csign > 0 ? cd : (u64)0 - cd;
+                    int wbase = 0;
+                    for (int t0 = 0; t0 < nu; t0 += 32) {
+                        const int t = t0 + lane;
+                        const bool valid = t < nu;
+                        i64 x = 0;
+                        int met = 0;
+                        if (valid) {
+                            met = efmet[t];
+                            i64 s = 0;
+                            for (int qq = qa0; qq < qa1; ++qq) { const int2 e = __ldg(&A.g.col[qq]); if (e.x == met) s = e.y; }
+                            x = (i64)(ck * (u64)ef[t] + sd * (u64)s);
+                            if (cg > 1) x /= (i64)cg;
                         }
-                    } else {
-                        for (int q = lane; q < nO; q += 32) {
-                            const i64 b = doff + (i64)q * nI + lPI;
-                            dep = dep || (sbit(P.sbits, __ldg(&g.out_e[out0 + q]).x) && ((__ldg(&g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
+                        const u32 nz = __ballot_sync(FULL, valid && x != 0);
+                        if (valid && x != 0) {
+                            const int pos = wbase + __popc(nz & lt);
+                            ef2[pos] = x; efmet2[pos] = (u16)met;
+                            mx = max(mx, abs64(x));
                         }
+                        wbase += __popc(nz);
                     }
-                    dep = __any_sync(FULL, dep);
-                    int a, c, sign;
-                    if (fwd) { if (!dep) { a = PO; c = cPO; sign = +1; } else { a = PI; c = cPI; sign = -1; } }   // Eq 4 / Eq 5
-                    else     { if (!dep) { a = PI; c = cPI; sign = +1; } else { a = PO; c = cPO; sign = -1; } }
-                    const u64 newrec = vis_pack((u32)istar, (u32)PI, (u32)PO, (u32)cntv);
-                    Child ch;
-                    eval_child(g, P, lane, a, c, sign, false, rec, newrec, ch);
-                    emit(ch, false, newrec);
+                    for (int q0 = qa0; q0 < qa1; q0 += 32) {
+                        const int qq = q0 + lane;
+                        int2 e = make_int2(0, 0);
+                        bool only = false;
+                        if (qq < qa1) { e = __ldg(&A.g.col[qq]); only = upos[e.x] == 0; }
+                        const u32 m = __ballot_sync(FULL, only);
+                        if (only) {
+                            i64 x = (i64)(sd * (u64)(i64)e.y);
+                            if (cg > 1) x /= (i64)cg;
+                            const int pos = wbase + __popc(m & lt);
+                            ef2[pos] = x; efmet2[pos] = (u16)e.x;
+                            mx = max(mx, abs64(x));
+                        }
+                        wbase += __popc(m);
+                    }
+                    mx = w_max(mx);
                 }
-            }
-            if (MODE == MODE_COUNT) {
-                kmin = w_min(kmin);
-                if (lane == 0) A.pmin[p] = kmin;
+                if (lane == 0) {
+                    uint4* h4 = (uint4*)dst;
+                    h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2c, (u32)chs, (u32)(chs >> 32));
+                    h4[1] = make_uint4((u32)chv, (u32)(chv >> 32), (u32)mx, (u32)(mx >> 32));
+                }
             }
         }
-        // ---- restore the shared bitsets to zero for the next parent
+        if (MODE != MODE_WRITE && firstv && nv < A.V && n_adm == 0 && lane == 0) sst[SS_DEAD]++;   // no admissible alternative
+        if (MODE == MODE_COUNT) {
+            kmin = w_min(kmin);
+            if (lane == 0) A.pmin[p] = kmin;
+        }
+        // ---- restore the shared tables to zero for the next parent
         __syncwarp();
-        for (int t = lane; t < P.n_supp; t += 32) P.sbits[P.arc[t] >> 5] = 0;
-        for (int t = lane; t < P.n_unb; t += 32) P.ubits[P.efmet[t] >> 5] = 0;
+        for (int t = lane; t < ns; t += 32) sbits[arc[t] >> 5] = 0;
+        for (int t = lane; t < nu; t += 32) upos[efmet[t]] = 0;
         __syncwarp();
     }
     if (MODE == MODE_COUNT) ko.finish(A, lane);
+    __syncwarp();
     if (lane == 0) {
         u64* st = ctl->st;
-        if (s_expanded) { atomicAdd(&st[ST_EXPANDED], s_expanded); atomicAdd(&ctl->lvl_expanded, s_expanded); }
-        if (s_children) { atomicAdd(&st[ST_CHILDREN], s_children); atomicAdd(&ctl->lvl_children, s_children); }
-        if (s_done) atomicAdd(&ctl->lvl_done, s_done);
-        if (s_active) atomicAdd(&ctl->n_keys, s_active);
-        if (s_dead) atomicAdd(&st[ST_DEAD_END], s_dead);
-        if (s_notefm) atomicAdd(&st[ST_NOT_EFM], s_notefm);
-        if (s_nonpos) atomicAdd(&st[ST_NONPOS], s_nonpos);
-        if (s_ovf) atomicAdd(&st[ST_OVERFLOW], s_ovf);
-        if (s_visited) atomicAdd(&st[ST_VISITED], s_visited);
-        if (s_bytes) atomicAdd(&st[ST_ALGO_BYTES], s_bytes);
+        if (sst[SS_EXPANDED]) { atomicAdd(&st[ST_EXPANDED], sst[SS_EXPANDED]); atomicAdd(&ctl->lvl_expanded, sst[SS_EXPANDED]); }
+        if (sst[SS_CHILDREN]) { atomicAdd(&st[ST_CHILDREN], sst[SS_CHILDREN]); atomicAdd(&ctl->lvl_children, sst[SS_CHILDREN]); }
+        if (sst[SS_DONE]) atomicAdd(&ctl->lvl_done, sst[SS_DONE]);
+        if (sst[SS_ACTIVE]) atomicAdd(&ctl->n_keys, sst[SS_ACTIVE]);
+        if (sst[SS_DEAD]) atomicAdd(&st[ST_DEAD_END], sst[SS_DEAD]);
+        if (sst[SS_NOTEFM]) atomicAdd(&st[ST_NOT_EFM], sst[SS_NOTEFM]);
+        if (sst[SS_NONPOS]) atomicAdd(&st[ST_NONPOS], sst[SS_NONPOS]);
+        if (sst[SS_OVF]) atomicAdd(&st[ST_OVERFLOW], sst[SS_OVF]);
+        if (sst[SS_VISITED]) atomicAdd(&st[ST_VISITED], sst[SS_VISITED]);
+        if (sst[SS_BYTES]) atomicAdd(&st[ST_ALGO_BYTES], sst[SS_BYTES]);
     }
 }
 
@@ -728,7 +682,8 @@ static size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 void expand_smem_layout(ExpandArgs& a) {
     size_t off = align16(a.max_entry);   // staging holds the largest entry
     a.sm_sbits = (u32)off; off = align16(off + (size_t)a.g.W32 * 4);
-    a.sm_ubits = (u32)off; off = align16(off + (size_t)a.g.M32 * 4);
+    a.sm_upos = (u32)off;  off = align16(off + (size_t)a.g.M * 2 + 2);
+    a.sm_misc = (u32)off;  off = align16(off + (size_t)SS_WORDS * 8);
     a.sm_group = (u32)off;
 }
 
@@ -738,23 +693,29 @@ u64 expand_key_slack() { return kMaxGrid * kWarps * kKeyChunk; }
 
 template <int MODE>
 static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
-    const size_t smem = (size_t)a.sm_group * kWarps;
-    static bool attr_done = false;
-    if (!attr_done) {
+    // warps per block: as many as fit beside the per-warp staging (huge networks fall back to fewer warps)
+    int warps = kWarps;
+    while (warps > 1 && (size_t)a.sm_group * warps > 200 * 1024) warps >>= 1;
+    const size_t smem = (size_t)a.sm_group * warps;
+    if (smem > 227 * 1024) return cudaErrorInvalidValue;
+    static int bps_cache[kWarps + 1] = {0};
+    static size_t smem_cache[kWarps + 1] = {0};
+    if (bps_cache[warps] == 0 || smem_cache[warps] != smem) {
         cudaError_t e = cudaFuncSetAttribute(k_expand<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        int bps = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_expand<MODE>, warps * 32, smem);
+        if (e != cudaSuccess) return e;
+        bps_cache[warps] = bps < 1 ? 1 : bps;
+        smem_cache[warps] = smem;
     }
-    if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    u64 need = (a.n_cur + kWarps - 1) / kWarps;
-    int bps = (int)((227 * 1024) / (smem + 1024));
-    if (bps > 16) bps = 16;
-    if (bps < 1) bps = 1;
-    u64 cap = (u64)sm_count * bps * 4;
+    // persistent grid: every resident warp walks the parents with a grid stride (per-warp set-up is paid once)
+    const u64 need = (a.n_cur + warps - 1) / warps;
+    u64 cap = (u64)sm_count * bps_cache[warps];
     if (cap > kMaxGrid) cap = kMaxGrid;
     unsigned grid = (unsigned)(need < cap ? need : cap);
     if (grid == 0) grid = 1;
-    k_expand<MODE><<<grid, kBlock, smem, s>>>(a);
+    k_expand<MODE><<<grid, warps * 32, smem, s>>>(a);
     return cudaGetLastError();
 }
 
