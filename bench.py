@@ -267,6 +267,9 @@ def main_ours(args):
                           "phase_ms_per_step": {k: acc[k] / args.steps for k in
                                                 ("ms_expand_count", "ms_beam", "ms_expand_write", "ms_direct", "ms_hash",
                                                  "ms_filter", "ms_output")},
+                          "work_profile_per_step": {k: acc[k] / args.steps for k in
+                                                    ("expanded", "alt_rounds", "first_visits", "general_children",
+                                                     "saturated_parents", "write_pass_parents")},
                           "filter_pairs_per_s": (acc["filter_pairs"] / (acc["ms_filter"] * 1e-3)) if acc["ms_filter"] else None}}
         print(json.dumps(line))
     en.close()

@@ -77,6 +77,9 @@ typedef struct {
         ms_filter, ms_output;
     int64_t n_expand_count, n_expand_write, n_direct; /* launches behind the three expand timers     */
     int64_t filter_pairs;   /* signature pair tests done by the minimality filter                    */
+    /* work profile of the expand kernels: rounds of 32 OR-alternatives, first-visit parents, children through
+     * the general routine, parents whose support is at the cap D, parents the write pass re-expanded        */
+    int64_t alt_rounds, first_visits, general_children, saturated_parents, write_pass_parents;
 } efm_stats;
 
 /* Build the modified AND/OR graph MG (Defs 4-6; "Convert the given matrix to the MG

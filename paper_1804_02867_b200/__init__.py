@@ -35,7 +35,8 @@ _STAT_INT = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxl
              "peak_frontier", "algo_bytes", "n_roots", "launches", "two_pass_levels", "direct_levels"]
 _STAT_MS = ["ms_build", "ms_total", "ms_expand_count", "ms_beam", "ms_expand_write", "ms_direct", "ms_hash",
             "ms_filter", "ms_output"]
-_STAT_INT2 = ["n_expand_count", "n_expand_write", "n_direct", "filter_pairs"]
+_STAT_INT2 = ["n_expand_count", "n_expand_write", "n_direct", "filter_pairs", "alt_rounds", "first_visits",
+              "general_children", "saturated_parents", "write_pass_parents"]
 
 
 class efm_stats(ctypes.Structure):

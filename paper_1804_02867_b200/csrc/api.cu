@@ -531,6 +531,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     st.truncated_beam = truncated;
     st.output = (int64_t)n_keep;
     st.algo_bytes = (int64_t)hc->st[ST_ALGO_BYTES];
+    st.alt_rounds = (int64_t)hc->st[ST_ROUNDS]; st.first_visits = (int64_t)hc->st[ST_FIRST];
+    st.general_children = (int64_t)hc->st[ST_GENERAL]; st.saturated_parents = (int64_t)hc->st[ST_SATURATED];
+    st.write_pass_parents = (int64_t)hc->st[ST_WRITE_PARENTS];
     st.peak_frontier = 0;
     for (int64_t a : h->lvl_active) st.peak_frontier = std::max(st.peak_frontier, a);
     st.launches = launches;

@@ -21,6 +21,9 @@ namespace efm {
 
 enum { MODE_COUNT = 0, MODE_WRITE = 1, MODE_DIRECT = 2 };
 enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
+#ifndef EFM_MIN_BLOCKS
+#define EFM_MIN_BLOCKS 4   // resident blocks per SM the register allocation aims at
+#endif
 constexpr int kBlock = 128;
 constexpr int kWarps = kBlock / 32;
 constexpr u32 FULL = 0xffffffffu;
@@ -102,6 +105,7 @@ struct KeyOut {
         const u32 cnt = (u32)__popc(m);
         if (cnt == 0) return;
         if (cnt > left) {
+#pragma unroll 1
             for (u32 t = lane; t < left; t += 32) A.keys[base + t] = kKeySentinel;
             u64 b = 0;
             if (lane == 0) b = atomicAdd(&A.ctl->n_slots, (u64)kKeyChunk);
@@ -134,6 +138,7 @@ __device__ __forceinline__ bool sbit(const u32* bits, int a) { return (bits[a >>
 
 // per-warp statistics live in shared memory (one u64 each), flushed to the control block once per warp
 enum { SS_EXPANDED = 0, SS_CHILDREN, SS_DONE, SS_ACTIVE, SS_DEAD, SS_NOTEFM, SS_NONPOS, SS_OVF, SS_VISITED, SS_BYTES,
+       SS_ROUNDS, SS_FIRST, SS_GENERAL, SS_SATURATED, SS_WRITE_PARENTS,
        SS_KC,   // 4 words: the hash sums of the k-scaled support for the last two scales k (k0, s0, k1, s1)
        SS_WORDS = SS_KC + 4 };
 
@@ -141,7 +146,7 @@ enum { SS_EXPANDED = 0, SS_CHILDREN, SS_DONE, SS_ACTIVE, SS_DEAD, SS_NOTEFM, SS_
 // compiler can track, and both kinds of children (lane-parallel "fast" ones and warp-cooperative "general" ones) funnel
 // into a single evaluate / place / write sequence.
 template <int MODE>
-__global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ ExpandArgs A) {
+__global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_constant__ ExpandArgs A) {
     extern __shared__ uint4 smem4[];
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
@@ -151,7 +156,9 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
     u32* sbits = (u32*)(gs + A.sm_sbits);   // support bitset over arcs
     u16* upos = (u16*)(gs + A.sm_upos);     // metabolite -> 1 + index in the EF list of the parent, 0 = balanced
     u64* sst = (u64*)(gs + A.sm_misc);
+    #pragma unroll 1
     for (int i = lane; i < A.g.W32; i += 32) sbits[i] = 0;
+    #pragma unroll 1
     for (int i = lane; i < (A.g.M + 1) / 2; i += 32) ((u32*)upos)[i] = 0;
     if (lane < SS_WORDS) sst[lane] = 0;
     __syncwarp();
@@ -163,6 +170,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
     KeyOut ko; ko.base = 0; ko.left = 0;
     const u64 wstride = (u64)gridDim.x * (blockDim.x >> 5);
 
+    #pragma unroll 1
     for (u64 p = (u64)blockIdx.x * (blockDim.x >> 5) + wib; p < A.n_cur; p += wstride) {
         if (MODE == MODE_WRITE && !notrunc && __ldg(&A.pmin[p]) >= X) continue;   // no child of p survives the beam
         // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
@@ -173,6 +181,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
         const int nu = (int)__shfl_sync(FULL, first16.y, 0);
         const u32 nch = entry_bytes((u32)ns, (u32)nv, (u32)nu) / 16;
         if ((u32)lane < nch) stage[lane] = first16;
+        #pragma unroll 1
         for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldg(src + c);
         __syncwarp();
         const u64 Phs = ((const u64*)stage)[1], Phv = ((const u64*)stage)[2], Pbig = ((const u64*)stage)[3];
@@ -183,8 +192,10 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
         const u16* efmet = arc + ns;
 
         // ---- support bitset, EF index table, PROC0: lowest unbalanced metabolite i* (reading G12)
+        #pragma unroll 1
         for (int t = lane; t < ns; t += 32) { const u32 a = arc[t]; atomicOr(&sbits[a >> 5], 1u << (a & 31)); }
         u32 best = 0xffffffffu;
+        #pragma unroll 1
         for (int t = lane; t < nu; t += 32) {
             const u32 i = efmet[t];
             upos[i] = (u16)(t + 1);
@@ -199,15 +210,18 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
         const u64 absE = abs64(E);
         auto ef_of = [&](int met) -> i64 { const u32 u = upos[met]; return u ? ef[u - 1] : 0; };
         if (MODE != MODE_WRITE && lane == 0) { sst[SS_EXPANDED]++; sst[SS_BYTES] += algo_entry_bytes((u32)ns, (u32)nv); }
+        if (MODE == MODE_WRITE && lane == 0) sst[SS_WRITE_PARENTS]++;
         u64 kmin = ~0ULL;   // smallest key among the active children of p (count pass)
         // visited?
         int vk = -1;
+        #pragma unroll 1
         for (int base = 0; base < nv && vk < 0; base += 32) {
             const int u = base + lane;
             const u32 hit = __ballot_sync(FULL, u < nv && (int)((vis[u] >> 32) & 0xffffu) == istar);
             if (hit) vk = base + __ffs(hit) - 1;
         }
         const bool firstv = vk < 0;
+        if (MODE != MODE_WRITE && lane == 0) { sst[SS_FIRST] += firstv; sst[SS_SATURATED] += ns >= A.D; }
         const int in0 = __ldg(&A.g.in_ptr[istar]), nI = __ldg(&A.g.in_ptr[istar + 1]) - in0;
         const int out0 = __ldg(&A.g.out_ptr[istar]), nO = __ldg(&A.g.out_ptr[istar + 1]) - out0;
 
@@ -224,6 +238,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                 // primary on the side the flux arrives from: lowest arc of that side in the support (G13)
                 const int2* plist = fwd ? A.g.in_e + in0 : A.g.out_e + out0;
                 const int plen = fwd ? nI : nO;
+                #pragma unroll 1
                 for (int base = 0; base < plen && prim < 0; base += 32) {
                     const int q = base + lane;
                     const int pa = q < plen ? __ldg(&plist[q]).x : -1;
@@ -242,7 +257,9 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
             } else {
                 const int PI = (int)((rec >> 16) & 0xffffu), PO = (int)(rec & 0xffffu);
                 int lPI = -1, lPO = -1, cPI = 0, cPO = 0;
+                #pragma unroll 1
                 for (int q = lane; q < nI; q += 32) { const int2 e = __ldg(&A.g.in_e[in0 + q]); if (e.x == PI) { lPI = q; cPI = e.y; } }
+                #pragma unroll 1
                 for (int q = lane; q < nO; q += 32) { const int2 e = __ldg(&A.g.out_e[out0 + q]); if (e.x == PO) { lPO = q; cPO = e.y; } }
                 lPI = __reduce_max_sync(FULL, lPI); cPI = __reduce_max_sync(FULL, cPI);
                 lPO = __reduce_max_sync(FULL, lPO); cPO = __reduce_max_sync(FULL, cPO);
@@ -250,11 +267,13 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                 bool dep = false;
                 const i64 doff = __ldg(&A.g.dep_off[istar]);
                 if (fwd) {
+                    #pragma unroll 1
                     for (int q = lane; q < nI; q += 32) {
                         const i64 b = doff + (i64)lPO * nI + q;
                         dep = dep || (sbit(sbits, __ldg(&A.g.in_e[in0 + q]).x) && ((__ldg(&A.g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
                     }
                 } else {
+                    #pragma unroll 1
                     for (int q = lane; q < nO; q += 32) {
                         const i64 b = doff + (i64)q * nI + lPI;
                         dep = dep || (sbit(sbits, __ldg(&A.g.out_e[out0 + q]).x) && ((__ldg(&A.g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
@@ -269,6 +288,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
         }
         const bool fastP = firstv && fast_graph && Pbig < kSmall;
         int n_adm = 0;
+        #pragma unroll 1
         for (int base = 0; base < alen; base += 32) {
             const int q = base + lane;
             int a = -1, c = 1;
@@ -284,6 +304,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
             } else if (lane == 0) {
                 a = r_a; c = r_c; adm = true; insup = true;   // PI / PO are arcs of the support
             }
+            if (MODE != MODE_WRITE && lane == 0) sst[SS_ROUNDS]++;
             const u32 adm_m = __ballot_sync(FULL, adm);
             if (adm_m == 0) continue;
             n_adm += __popc(adm_m);
@@ -297,6 +318,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                 if (fast) {
                     if (c != 1) scale_small(absE, (u32)c, k, d);
                     const int q1 = __ldg(&A.g.col_ptr[a + 1]);
+                    #pragma unroll 1
                     for (int qq = __ldg(&A.g.col_ptr[a]); qq < q1; ++qq) {
                         const int2 e = __ldg(&A.g.col[qq]);
                         const i64 efp = ef_of(e.x);
@@ -306,6 +328,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                 }
                 u64 hsb = Phs;
                 u32 need = __ballot_sync(FULL, fast && k > 1);
+                #pragma unroll 1
                 while (need) {
                     const u32 kk = __shfl_sync(FULL, k, __ffs(need) - 1);
                     u64 s;
@@ -313,6 +336,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                     else if ((u64)kk == sst[SS_KC + 2]) s = sst[SS_KC + 3];
                     else {
                         s = 0;
+                        #pragma unroll 1
                         for (int t = lane; t < ns; t += 32) s += arc_term_t(A.g, (u32)arc[t], (u64)kk * (u64)flux[t]);
                         s = w_sum(s);
                         __syncwarp();
@@ -350,6 +374,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
             // ---- one child at a time: general evaluation (arc of the support, large integers) and / or materialisation
             const u32 slow_m = adm_m & ~fast_m;
             u32 work_m = keep_m | slow_m;
+            #pragma unroll 1
             while (work_m) {
                 const int l = __ffs(work_m) - 1;
                 work_m &= work_m - 1;
@@ -375,6 +400,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                     cd = gg == 1 ? absE : absE / gg;
                     cin = sbit(sbits, ca);
                     if (cin) {   // position of the arc in the sorted support
+                        #pragma unroll 1
                         for (int b2 = 0; b2 < ns && cia < 0; b2 += 32) {
                             const int t = b2 + lane;
                             const u32 hit = __ballot_sync(FULL, t < ns && arc[t] == ca);
@@ -400,6 +426,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                     }
                     if (bigk) {   // exact: the largest flux among t != ia (a new arc carries d <= |E| <= 2^62)
                         u64 mx = 0;
+                        #pragma unroll 1
                         for (int t = lane; t < ns; t += 32) if (t != cia) mx = max(mx, (u64)flux[t]);
                         mx = w_max(mx);
                         ovf = ovf || umul_gt_guard(ck, mx);
@@ -409,14 +436,17 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                         // extra fluxes of the un-normalised child: EF'_i = k EF_i + sign d s_ia (Eq 2 on the scaled fluxes)
                         bool ovf2 = false;
                         if (bigk) {   // exact sweep over the unbalanced metabolites outside col(a)
+                            #pragma unroll 1
                             for (int t = lane; t < nu; t += 32) {
                                 const int i = efmet[t];
                                 bool in_a = false;
+                                #pragma unroll 1
                                 for (int r = qa0; r < qa1; ++r) in_a = in_a || __ldg(&A.g.col[r]).x == i;
                                 if (!in_a) ovf2 = ovf2 || abs_gt_guard(mul_s((i64)ck, ef[t]));
                             }
                         }
                         int delta = 0;
+                        #pragma unroll 1
                         for (int qq = qa0 + lane; qq < qa1; qq += 32) {
                             const int2 e = __ldg(&A.g.col[qq]);
                             const i64 efp = ef_of(e.x);
@@ -436,10 +466,12 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                     // flux equal to 1 gives G = 1 and g = gcd(k, k f_a +- d) = gcd(k, d) = 1 without any gcd.
                     if (cin && cT != 1) {
                         bool one = false;
+                        #pragma unroll 1
                         for (int t = lane; t < ns; t += 32) one = one || (t != cia && flux[t] == 1);
                         if (!__any_sync(FULL, one)) {
                             const bool narrow = Pbig < (1ULL << 32);
                             u64 G = 0;
+                            #pragma unroll 1
                             for (int t = lane; t < ns; t += 32)
                                 if (t != cia) G = narrow ? (u64)gcd32((u32)G, (u32)flux[t]) : gcd64(G, (u64)flux[t]);
                             G = w_gcd(G, narrow);
@@ -450,6 +482,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                         chs = Phs + arc_term_t(A.g, (u32)ca, cT) - (cin ? arc_term_t(A.g, (u32)ca, (u64)flux[cia]) : 0ULL);
                     } else {
                         chs = 0;
+                        #pragma unroll 1
                         for (int t = lane; t < ns; t += 32) {
                             u64 F = t == cia ? cT : ck * (u64)flux[t];
                             if (cg > 1) F /= cg;
@@ -461,7 +494,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                     chv = Phv + vis_term(newrec) - (firstv ? 0ULL : vis_term(rec));
                     // account for the child, classify it, decide whether it is materialised in this pass
                     const bool cdone = cnu == 0;
-                    if (MODE != MODE_WRITE && lane == 0) { sst[SS_CHILDREN]++; sst[SS_BYTES] += 8; if (cdone) sst[SS_DONE]++; }
+                    if (MODE != MODE_WRITE && lane == 0) { sst[SS_CHILDREN]++; sst[SS_GENERAL]++; sst[SS_BYTES] += 8; if (cdone) sst[SS_DONE]++; }
                     if (cdone) keep = MODE != MODE_WRITE;   // balanced children are written where they are first seen
                     else {
                         const u64 ckey = beam_key((u32)cnu, mix64(chs + chv));
@@ -503,6 +536,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                 // ---- write
                 int ins = 0;   // a new arc goes where the ascending order puts it
                 if (!cin)
+                    #pragma unroll 1
                     for (int b2 = 0; b2 < ns; b2 += 32) {
                         const int t = b2 + lane;
                         ins += __popc(__ballot_sync(FULL, t < ns && (int)arc[t] < ca));
@@ -513,6 +547,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                 u16* arc2 = (u16*)(ef2 + nu2c);
                 u16* efmet2 = arc2 + n2;
                 u64 mx = cin ? 0ULL : cT;   // a new arc never comes with a common divisor
+                #pragma unroll 1
                 for (int t = lane; t < ns; t += 32) {
                     u64 F = t == cia ? cT : ck * (u64)flux[t];
                     if (cg > 1) F /= cg;
@@ -523,6 +558,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                 }
                 if (!cin && lane == 0) { flux2[ins] = (i64)cT; arc2[ins] = (u16)ca; }
                 if (!to_cand) {
+                    #pragma unroll 1
                     for (int u = lane; u < nv; u += 32) vis2[u] = (!firstv && u == vk) ? newrec : vis[u];
                     if (firstv && lane == 0) vis2[nv] = newrec;
                     // EF list of the child: EF' = (k EF + sign d s_.a) / g over the parent's list, then the metabolites
@@ -530,6 +566,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                     // established that nothing exceeds 2^62, so the wrapping 64-bit arithmetic is exact.
                     const u64 sd = csign > 0 ? cd : (u64)0 - cd;
                     int wbase = 0;
+                    #pragma unroll 1
                     for (int t0 = 0; t0 < nu; t0 += 32) {
                         const int t = t0 + lane;
                         const bool valid = t < nu;
@@ -538,6 +575,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                         if (valid) {
                             met = efmet[t];
                             i64 s = 0;
+                            #pragma unroll 1
                             for (int qq = qa0; qq < qa1; ++qq) { const int2 e = __ldg(&A.g.col[qq]); if (e.x == met) s = e.y; }
                             x = (i64)(ck * (u64)ef[t] + sd * (u64)s);
                             if (cg > 1) x /= (i64)cg;
@@ -550,6 +588,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
                         }
                         wbase += __popc(nz);
                     }
+                    #pragma unroll 1
                     for (int q0 = qa0; q0 < qa1; q0 += 32) {
                         const int qq = q0 + lane;
                         int2 e = make_int2(0, 0);
@@ -581,7 +620,9 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
         }
         // ---- restore the shared tables to zero for the next parent
         __syncwarp();
+        #pragma unroll 1
         for (int t = lane; t < ns; t += 32) sbits[arc[t] >> 5] = 0;
+        #pragma unroll 1
         for (int t = lane; t < nu; t += 32) upos[efmet[t]] = 0;
         __syncwarp();
     }
@@ -599,6 +640,11 @@ __global__ void __launch_bounds__(kBlock, 4) k_expand(const __grid_constant__ Ex
         if (sst[SS_OVF]) atomicAdd(&st[ST_OVERFLOW], sst[SS_OVF]);
         if (sst[SS_VISITED]) atomicAdd(&st[ST_VISITED], sst[SS_VISITED]);
         if (sst[SS_BYTES]) atomicAdd(&st[ST_ALGO_BYTES], sst[SS_BYTES]);
+        if (sst[SS_ROUNDS]) atomicAdd(&st[ST_ROUNDS], sst[SS_ROUNDS]);
+        if (sst[SS_FIRST]) atomicAdd(&st[ST_FIRST], sst[SS_FIRST]);
+        if (sst[SS_GENERAL]) atomicAdd(&st[ST_GENERAL], sst[SS_GENERAL]);
+        if (sst[SS_SATURATED]) atomicAdd(&st[ST_SATURATED], sst[SS_SATURATED]);
+        if (sst[SS_WRITE_PARENTS]) atomicAdd(&st[ST_WRITE_PARENTS], sst[SS_WRITE_PARENTS]);
     }
 }
 
