@@ -23,8 +23,8 @@ struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
     Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
-    Region ctl, buf[2], off[2], pmin, keys, ckeys, cand, table, isrep, poison, uniq, size_hist, bucket_start, bucket_fill;
-    Region order, sig, size_sorted, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, dense;
+    Region ctl, buf[2], off[2], pmin, keys, ckeys, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill;
+    Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, dense;
     size_t total = 0;
 };
 
@@ -94,13 +94,14 @@ void make_layout(efm_handle* h) {
     add_region(L, L.isrep, C + 1);
     add_region(L, L.poison, C + 1);
     add_region(L, L.uniq, C * 4);
-    const size_t bins = (size_t)h->D + 2;
-    add_region(L, L.size_hist, bins * 4);
-    add_region(L, L.bucket_start, bins * 4);
-    add_region(L, L.bucket_fill, bins * 4);
-    add_region(L, L.order, C * 4);
-    add_region(L, L.sig, C * 16);
-    add_region(L, L.size_sorted, C * 2);
+    const size_t bins = (size_t)h->G.A + 2;   // per-arc tables of the minimality filter
+    add_region(L, L.freq, bins * 4);
+    add_region(L, L.gcount, bins * 4);
+    add_region(L, L.gstart, bins * 4);
+    add_region(L, L.gfill, bins * 4);
+    add_region(L, L.g_row, C * 4);
+    add_region(L, L.g_sig, C * 16);
+    add_region(L, L.g_size, C * 2);
     add_region(L, L.keep, C);
     add_region(L, L.u_nnz, C * 4);
     add_region(L, L.u_rxn, C * h->D * 4);
@@ -220,7 +221,7 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     h->max_cand = P.max_candidates ? P.max_candidates : (int64_t)1 << 20;
     if (h->max_cand > 0xFFFFFFF0LL) { delete h; return EFM_E_INVAL; }
     h->max_keys = (P.max_child_keys ? P.max_child_keys : std::max<int64_t>(h->cap * (int64_t)G.max_fanout, 65536)) +
-                  (int64_t)expand_key_slack();
+                  (int64_t)expand_key_slack((u64)h->max_frontier);
     h->table_size = pow2_at_least((size_t)h->max_cand * 2);
     h->dense_bytes = std::max<size_t>((size_t)64 << 20, (size_t)n * 8 * 64);
     make_layout(h);
@@ -484,10 +485,10 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     pa.cand = ws + L.cand.off; pa.cand_stride = h->cand_stride; pa.max_cand = (u64)h->max_cand;
     pa.table = (u32*)(ws + L.table.off); pa.table_size = h->table_size;
     pa.isrep = ws + L.isrep.off; pa.poison = ws + L.poison.off; pa.uniq = (u32*)(ws + L.uniq.off);
-    pa.size_hist = (u32*)(ws + L.size_hist.off); pa.bucket_start = (u32*)(ws + L.bucket_start.off);
-    pa.bucket_fill = (u32*)(ws + L.bucket_fill.off); pa.n_size_bins = h->D + 2;
-    pa.order = (u32*)(ws + L.order.off); pa.sig = (ulonglong2*)(ws + L.sig.off);
-    pa.size_sorted = (u16*)(ws + L.size_sorted.off); pa.keep = ws + L.keep.off;
+    pa.freq = (u32*)(ws + L.freq.off); pa.gcount = (u32*)(ws + L.gcount.off);
+    pa.gstart = (u32*)(ws + L.gstart.off); pa.gfill = (u32*)(ws + L.gfill.off);
+    pa.g_row = (u32*)(ws + L.g_row.off); pa.g_sig = (ulonglong2*)(ws + L.g_sig.off);
+    pa.g_size = (u16*)(ws + L.g_size.off); pa.keep = ws + L.keep.off;
     pa.D = h->D; pa.n_rxn = G.n;
     pa.u_nnz = (int*)(ws + L.u_nnz.off); pa.u_rxn = (int*)(ws + L.u_rxn.off); pa.u_val = (i64*)(ws + L.u_val.off);
     pa.sort_idx = (u32*)(ws + L.sort_idx.off);

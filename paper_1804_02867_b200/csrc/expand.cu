@@ -22,10 +22,11 @@ namespace efm {
 enum { MODE_COUNT = 0, MODE_WRITE = 1, MODE_DIRECT = 2 };
 enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
 #ifndef EFM_MIN_BLOCKS
-#define EFM_MIN_BLOCKS 4   // resident blocks per SM the register allocation aims at
+#define EFM_MIN_BLOCKS 16   // resident one-warp blocks per SM the register allocation aims at (128 registers)
 #endif
-constexpr int kBlock = 128;
+constexpr int kBlock = 32;    // one warp per block: a finished warp frees its slot at once (parents differ a lot in cost)
 constexpr int kWarps = kBlock / 32;
+constexpr int kParentsPerWarp = 8;
 constexpr u32 FULL = 0xffffffffu;
 constexpr u64 kSmall = 1ULL << 40;   // fast path: every flux and extra flux of the parent below this ...
 constexpr int kSmallCoef = 1 << 20;  // ... and every coefficient below this: no product can reach 2^62
@@ -168,10 +169,13 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
     const u64 X = MODE == MODE_WRITE ? ctl->X : 0;
     const bool fast_graph = !A.no_fast && A.g.max_coef < kSmallCoef;
     KeyOut ko; ko.base = 0; ko.left = 0;
-    const u64 wstride = (u64)gridDim.x * (blockDim.x >> 5);
+    // a warp owns kParentsPerWarp consecutive parents; the grid covers the level and the block scheduler evens out the
+    // very different costs of parents (skipped / first visit over a hub / revisit)
+    const u64 p0 = ((u64)blockIdx.x * (blockDim.x >> 5) + wib) * kParentsPerWarp;
+    const u64 p1 = min(p0 + kParentsPerWarp, A.n_cur);
 
-    #pragma unroll 1
-    for (u64 p = (u64)blockIdx.x * (blockDim.x >> 5) + wib; p < A.n_cur; p += wstride) {
+#pragma unroll 1
+    for (u64 p = p0; p < p1; ++p) {
         if (MODE == MODE_WRITE && !notrunc && __ldg(&A.pmin[p]) >= X) continue;   // no child of p survives the beam
         // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
         const uint4* src = (const uint4*)(A.cur + (__ldg(&A.cur_off[p]) << 4));
@@ -734,8 +738,8 @@ void expand_smem_layout(ExpandArgs& a) {
 }
 
 // key slots the count pass can leave unused: every warp of the largest grid may strand one chunk
-constexpr u64 kMaxGrid = 16384;
-u64 expand_key_slack() { return kMaxGrid * kWarps * kKeyChunk; }
+// every warp may strand one chunk of key slots; a warp covers kParentsPerWarp parents
+u64 expand_key_slack(u64 max_parents) { return (max_parents / kParentsPerWarp + kWarps + 1) * kKeyChunk; }
 
 template <int MODE>
 static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
@@ -755,12 +759,11 @@ static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
         bps_cache[warps] = bps < 1 ? 1 : bps;
         smem_cache[warps] = smem;
     }
-    // persistent grid: every resident warp walks the parents with a grid stride (per-warp set-up is paid once)
-    const u64 need = (a.n_cur + warps - 1) / warps;
-    u64 cap = (u64)sm_count * bps_cache[warps];
-    if (cap > kMaxGrid) cap = kMaxGrid;
-    unsigned grid = (unsigned)(need < cap ? need : cap);
-    if (grid == 0) grid = 1;
+    const u64 per_block = (u64)warps * kParentsPerWarp;
+    const u64 need = (a.n_cur + per_block - 1) / per_block;
+    if (need > 0x7fffffffULL) return cudaErrorInvalidValue;
+    unsigned grid = (unsigned)(need ? need : 1);
+    (void)sm_count;
     k_expand<MODE><<<grid, warps * 32, smem, s>>>(a);
     return cudaGetLastError();
 }

@@ -6,7 +6,7 @@ namespace efm {
 
 // expand.cu
 void expand_smem_layout(ExpandArgs& a);
-u64 expand_key_slack();   // key slots the chunked reservation of the count pass can strand
+u64 expand_key_slack(u64 max_parents);   // key slots the chunked reservation of the count pass can strand
 cudaError_t launch_expand(int mode /*0 count, 1 write, 2 direct*/, const ExpandArgs& a, int sm_count, cudaStream_t s);
 cudaError_t launch_roots(bool write /*false: build + classify, true: keep the survivors*/, const RootArgs& r, cudaStream_t s);
 cudaError_t launch_level_begin(Ctl* ctl, cudaStream_t s);
@@ -20,8 +20,9 @@ struct PostArgs {
     unsigned char* isrep; unsigned char* poison;
     u32* uniq;                         // candidate ids of the unique, unpoisoned supports
     // minimality filter (a-7)
-    u32* size_hist; u32* bucket_start; u32* bucket_fill; int n_size_bins;
-    u32* order; ulonglong2* sig; u16* size_sorted; unsigned char* keep;
+    u32* freq; u32* gcount; u32* gstart; u32* gfill;      // per arc: candidates using it, group size / start / fill
+    u32* g_row; ulonglong2* g_sig; u16* g_size;           // rows grouped by their rarest arc: candidate id, signature, |supp|
+    unsigned char* keep;                                  // per unique support (uniq order)
     // canonical output (a-8)
     int D; int n_rxn;
     int* u_nnz; int* u_rxn; i64* u_val;   // unsorted reaction-space rows

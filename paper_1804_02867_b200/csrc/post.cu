@@ -210,21 +210,52 @@ cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_l
 
 // =================================================================================================================
 // a-7  Minimality filter (Def 3; reading G17): drop v if some other unique support w
-// is a strict subset.  Rows are counting-sorted by popcount so that only smaller supports are tested against v;
-// the pair test runs on 128-bit signatures (exact bitsets when A <= 128, a 128-bucket image of the arc set
-// otherwise) staged tile by tile through shared memory; signature hits are verified on the sorted arc lists.
+// is a strict subset.  supp(w) inside supp(v) needs EVERY arc of w in v, in particular the arc of w that is rarest
+// among all candidates.  So rows are grouped by their rarest arc (counting sort over arcs) and a row v is tested
+// only against the groups of its own arcs: sum over a in supp(v) of |group(a)| pair tests instead of K.  A pair test
+// is the 128-bit signature test (exact bitsets when A <= 128, a 128-bucket image of the arc set otherwise; coalesced
+// 16-byte loads, one lane per w), signature hits are verified on the sorted arc lists.
 // =================================================================================================================
 __device__ __forceinline__ u32 sig_bit(int arc, bool exact) { return exact ? (u32)arc : ((u32)arc * 0x9E3779B1u) >> 25; }
 
-__global__ void __launch_bounds__(256) k_filter_sizes(const PostArgs a, u64 K) {
+__global__ void __launch_bounds__(256) k_filter_freq(const PostArgs a, u64 K) {   // how many candidates use each arc
     const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= K) return;
     const unsigned char* e = a.cand + (u64)a.uniq[u] * a.cand_stride;
-    atomicAdd(&a.size_hist[cand_n(e)], 1u);
+    const int n = cand_n(e);
+    const u16* arc = cand_arc(e, n);
+    for (int t = 0; t < n; ++t) atomicAdd(&a.freq[arc[t]], 1u);
 }
-__global__ void k_filter_scan(const PostArgs a) {   // exclusive scan over the popcount bins (at most D+2 of them)
-    u32 acc = 0;
-    for (int b = 0; b < a.n_size_bins; ++b) { a.bucket_start[b] = acc; a.bucket_fill[b] = acc; acc += a.size_hist[b]; }
+__device__ __forceinline__ int rarest_arc(const PostArgs& a, const u16* arc, int n) {   // ties: lowest arc id
+    u32 best = 0xffffffffu; int key = 0;
+    for (int t = 0; t < n; ++t) { const u32 f = a.freq[arc[t]]; if (f < best) { best = f; key = arc[t]; } }
+    return key;
+}
+__global__ void __launch_bounds__(256) k_filter_count(const PostArgs a, u64 K) {
+    const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= K) return;
+    const unsigned char* e = a.cand + (u64)a.uniq[u] * a.cand_stride;
+    const int n = cand_n(e);
+    if (n == 0) return;   // the empty support belongs to no group (it has no strict subset and nothing tests against it)
+    atomicAdd(&a.gcount[rarest_arc(a, cand_arc(e, n), n)], 1u);
+}
+__global__ void __launch_bounds__(1024) k_filter_scan(const PostArgs a) {   // exclusive scan of the group sizes over arcs
+    __shared__ u32 part[1024];
+    const int A = a.g.A, T = blockDim.x, per = (A + T - 1) / T, b0 = threadIdx.x * per;
+    u32 sum = 0;
+    for (int j = 0; j < per; ++j) if (b0 + j < A) sum += a.gcount[b0 + j];
+    part[threadIdx.x] = sum;
+    __syncthreads();
+    for (int off = 1; off < T; off <<= 1) {
+        const u32 v = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
+        __syncthreads();
+        part[threadIdx.x] += v;
+        __syncthreads();
+    }
+    u32 acc = part[threadIdx.x] - sum;
+    for (int j = 0; j < per; ++j)
+        if (b0 + j < A) { const u32 c = a.gcount[b0 + j]; a.gstart[b0 + j] = acc; a.gfill[b0 + j] = acc; acc += c; }
+    if (threadIdx.x == T - 1) a.gstart[A] = part[T - 1];
 }
 __global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K) {
     const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
@@ -232,6 +263,7 @@ __global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K)
     const u32 id = a.uniq[u];
     const unsigned char* e = a.cand + (u64)id * a.cand_stride;
     const int n = cand_n(e);
+    if (n == 0) return;
     const u16* arc = cand_arc(e, n);
     const bool exact = a.g.A <= 128;
     u64 lo = 0, hi = 0;
@@ -239,10 +271,10 @@ __global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K)
         const u32 b = sig_bit(arc[t], exact);
         if (b < 64) lo |= 1ULL << b; else hi |= 1ULL << (b - 64);
     }
-    const u32 pos = atomicAdd(&a.bucket_fill[n], 1u);
-    a.order[pos] = id;
-    a.sig[pos] = make_ulonglong2(lo, hi);
-    a.size_sorted[pos] = (u16)n;
+    const u32 pos = atomicAdd(&a.gfill[rarest_arc(a, arc, n)], 1u);
+    a.g_row[pos] = id;
+    a.g_sig[pos] = make_ulonglong2(lo, hi);
+    a.g_size[pos] = (u16)n;
 }
 __device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   // supp(w) subset of supp(v), sorted lists
     const int nw = cand_n(w), nv = cand_n(v);
@@ -256,58 +288,62 @@ __device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   
     }
     return true;
 }
-constexpr int kFilterTile = 256;
-__global__ void __launch_bounds__(kFilterTile) k_filter(const PostArgs a, u64 K) {
-    __shared__ ulonglong2 wsig[kFilterTile];
-    __shared__ u32 blimit;
-    const u64 p = (u64)blockIdx.x * kFilterTile + threadIdx.x;
-    const bool valid = p < K;
-    ulonglong2 v = make_ulonglong2(0, 0);
-    u32 limit = 0;
-    if (valid) { v = a.sig[p]; limit = a.bucket_start[a.size_sorted[p]]; }   // rows with a strictly smaller support
-    // sizes ascend with p: the last valid row of the block has the largest limit
-    const u64 lastp = min((u64)blockIdx.x * kFilterTile + kFilterTile - 1, K - 1);
-    if (threadIdx.x == 0) blimit = a.bucket_start[a.size_sorted[lastp]];
-    __syncthreads();
-    const u32 bl = blimit;
+constexpr int kFilterWarps = 8;
+// one warp per row v; lanes walk the group of every arc of v
+__global__ void __launch_bounds__(kFilterWarps * 32) k_filter(const PostArgs a, u64 K) {
+    const u64 u = (u64)blockIdx.x * kFilterWarps + (threadIdx.x >> 5);
+    if (u >= K) return;
+    const int lane = threadIdx.x & 31;
+    const unsigned char* ev = a.cand + (u64)a.uniq[u] * a.cand_stride;
+    const int n = cand_n(ev);
+    const u16* arc = cand_arc(ev, n);
     const bool exact = a.g.A <= 128;
-    bool keep = true;
-    const u64 nvx = ~v.x, nvy = ~v.y;
-    for (u32 base = 0; base < bl; base += kFilterTile) {
-        if (base + threadIdx.x < bl) wsig[threadIdx.x] = a.sig[base + threadIdx.x];
-        __syncthreads();
-        if (keep && base < limit) {
-            const int jn = (int)min((u32)kFilterTile, limit - base);
-#pragma unroll 4
-            for (int j = 0; j < jn; ++j) {
-                const ulonglong2 w = wsig[j];
-                if (((w.x & nvx) | (w.y & nvy)) == 0) {
-                    if (exact || arcs_subset(a.cand + (u64)a.order[base + j] * a.cand_stride, a.cand + (u64)a.order[p] * a.cand_stride)) {
-                        keep = false;
-                        break;
-                    }
-                }
-            }
-        }
-        __syncthreads();
+    u64 lo = 0, hi = 0;
+    for (int t = lane; t < n; t += 32) {
+        const u32 b = sig_bit(arc[t], exact);
+        if (b < 64) lo |= 1ULL << b; else hi |= 1ULL << (b - 64);
     }
-    if (valid) {
-        a.keep[p] = keep ? 1 : 0;
-        atomicAdd(&a.ctl->filter_pairs, (u64)limit);
+#pragma unroll
+    for (int o = 16; o; o >>= 1) { lo |= __shfl_xor_sync(0xffffffffu, lo, o); hi |= __shfl_xor_sync(0xffffffffu, hi, o); }
+    const u64 nlo = ~lo, nhi = ~hi;
+    bool found = false;
+    u64 pairs = 0;
+    for (int t = 0; t < n && !found; ++t) {
+        const int ga = arc[t];
+        const u32 g0 = a.gstart[ga], g1 = a.gstart[ga + 1];
+        for (u32 base = g0; base < g1 && !found; base += 32) {
+            const u32 w = base + lane;
+            bool hit = false;
+            if (w < g1 && (int)a.g_size[w] < n) {   // a strict subset is strictly smaller (equal supports were merged by a-6)
+                const ulonglong2 sw = a.g_sig[w];
+                ++pairs;
+                if (((sw.x & nlo) | (sw.y & nhi)) == 0)
+                    hit = exact || arcs_subset(a.cand + (u64)a.g_row[w] * a.cand_stride, ev);
+            }
+            found = __any_sync(0xffffffffu, hit);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) pairs += __shfl_xor_sync(0xffffffffu, pairs, o);
+    if (lane == 0) {
+        a.keep[u] = found ? 0 : 1;
+        atomicAdd(&a.ctl->filter_pairs, pairs);
     }
 }
 
 cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s, int* n_launches) {
     (void)sm_count;
     cudaError_t e;
-    if ((e = cudaMemsetAsync(a.size_hist, 0, sizeof(u32) * a.n_size_bins, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(a.freq, 0, sizeof(u32) * (a.g.A + 2), s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(a.gcount, 0, sizeof(u32) * (a.g.A + 2), s)) != cudaSuccess) return e;
     if (K == 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((K + 255) / 256);
-    k_filter_sizes<<<blocks, 256, 0, s>>>(a, K);
-    k_filter_scan<<<1, 1, 0, s>>>(a);
+    k_filter_freq<<<blocks, 256, 0, s>>>(a, K);
+    k_filter_count<<<blocks, 256, 0, s>>>(a, K);
+    k_filter_scan<<<1, 1024, 0, s>>>(a);
     k_filter_scatter<<<blocks, 256, 0, s>>>(a, K);
-    k_filter<<<(unsigned)((K + kFilterTile - 1) / kFilterTile), kFilterTile, 0, s>>>(a, K);
-    *n_launches += 4;
+    k_filter<<<(unsigned)((K + kFilterWarps - 1) / kFilterWarps), kFilterWarps * 32, 0, s>>>(a, K);
+    *n_launches += 5;
     return cudaGetLastError();
 }
 
@@ -319,7 +355,7 @@ __global__ void __launch_bounds__(256) k_out_rows(const PostArgs a, u64 K) {
     const u64 p = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= K || !a.keep[p]) return;
     const u64 r = atomicAdd(&a.ctl->n_keep, 1ULL);
-    const unsigned char* e = a.cand + (u64)a.order[p] * a.cand_stride;
+    const unsigned char* e = a.cand + (u64)a.uniq[p] * a.cand_stride;
     const int n = cand_n(e);
     const u16* arc = cand_arc(e, n);
     const i64* f = cand_flux(e);
