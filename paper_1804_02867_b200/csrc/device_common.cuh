@@ -94,9 +94,10 @@ struct ExpandArgs {
     u32 max_entry, cand_stride; // largest entry in bytes (shared-memory staging), candidate slot stride
     u64 max_frontier, frontier_units, max_cand, max_keys;
     int D, V, max_loop;
+    u32 ppw;                    // consecutive parents a warp owns (set by the launcher)
     int no_fast;                // EFM_F_NO_FASTPATH: every child through the warp-cooperative general routine
     // shared-memory carve-up per warp (bytes)
-    u32 sm_group, sm_sbits, sm_upos, sm_misc;
+    u32 sm_group, sm_sbits, sm_upos, sm_misc, sm_out, sm_out_bytes;
 };
 
 // roots (INIT): seed sets uploaded by the host, entries built and classified on the device

@@ -26,7 +26,10 @@ enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
 #endif
 constexpr int kBlock = 32;    // one warp per block: a finished warp frees its slot at once (parents differ a lot in cost)
 constexpr int kWarps = kBlock / 32;
-constexpr int kParentsPerWarp = 8;
+#ifndef EFM_PPW
+#define EFM_PPW 8
+#endif
+constexpr int kParentsPerWarp = EFM_PPW;
 constexpr u32 FULL = 0xffffffffu;
 constexpr u64 kSmall = 1ULL << 40;   // fast path: every flux and extra flux of the parent below this ...
 constexpr int kSmallCoef = 1 << 20;  // ... and every coefficient below this: no product can reach 2^62
@@ -118,7 +121,7 @@ struct KeyOut {
             }
             base = b; left = kKeyChunk;
         }
-        if (want) A.keys[base + __popc(m & ((1u << lane) - 1u))] = key;
+        if (want) __stcs(&A.keys[base + __popc(m & ((1u << lane) - 1u))], key);
         base += cnt; left -= cnt;
     }
     __device__ __forceinline__ void finish(const ExpandArgs& A, int lane) {
@@ -160,7 +163,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
     #pragma unroll 1
     for (int i = lane; i < A.g.W32; i += 32) sbits[i] = 0;
     #pragma unroll 1
-    for (int i = lane; i < (A.g.M + 1) / 2; i += 32) ((u32*)upos)[i] = 0;
+    for (int i = lane; i < (A.g.M + 8) / 8; i += 32) ((uint4*)upos)[i] = make_uint4(0, 0, 0, 0);
     if (lane < SS_WORDS) sst[lane] = 0;
     __syncwarp();
 
@@ -169,24 +172,24 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
     const u64 X = MODE == MODE_WRITE ? ctl->X : 0;
     const bool fast_graph = !A.no_fast && A.g.max_coef < kSmallCoef;
     KeyOut ko; ko.base = 0; ko.left = 0;
-    // a warp owns kParentsPerWarp consecutive parents; the grid covers the level and the block scheduler evens out the
+    // a warp owns A.ppw (<= kParentsPerWarp) consecutive parents; the grid covers the level and the block scheduler evens out the
     // very different costs of parents (skipped / first visit over a hub / revisit)
-    const u64 p0 = ((u64)blockIdx.x * (blockDim.x >> 5) + wib) * kParentsPerWarp;
-    const u64 p1 = min(p0 + kParentsPerWarp, A.n_cur);
+    const u64 p0 = ((u64)blockIdx.x * (blockDim.x >> 5) + wib) * A.ppw;
+    const u64 p1 = min(p0 + A.ppw, A.n_cur);
 
 #pragma unroll 1
     for (u64 p = p0; p < p1; ++p) {
-        if (MODE == MODE_WRITE && !notrunc && __ldg(&A.pmin[p]) >= X) continue;   // no child of p survives the beam
+        if (MODE == MODE_WRITE && !notrunc && __ldcs(&A.pmin[p]) >= X) continue;   // no child of p survives the beam
         // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
-        const uint4* src = (const uint4*)(A.cur + (__ldg(&A.cur_off[p]) << 4));
-        const uint4 first16 = __ldg(src + lane);   // the buffers end in 512 spare bytes
+        const uint4* src = (const uint4*)(A.cur + (__ldcs(&A.cur_off[p]) << 4));
+        const uint4 first16 = __ldcs(src + lane);   // the buffers end in 512 spare bytes
         const u32 hdr = __shfl_sync(FULL, first16.x, 0);
         const int ns = (int)(hdr & 0xffffu), nv = (int)(hdr >> 16);
         const int nu = (int)__shfl_sync(FULL, first16.y, 0);
         const u32 nch = entry_bytes((u32)ns, (u32)nv, (u32)nu) / 16;
         if ((u32)lane < nch) stage[lane] = first16;
         #pragma unroll 1
-        for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldg(src + c);
+        for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldcs(src + c);   // streaming: the frontier must not evict the graph from L1
         __syncwarp();
         const u64 Phs = ((const u64*)stage)[1], Phv = ((const u64*)stage)[2], Pbig = ((const u64*)stage)[3];
         const i64* flux = (const i64*)(gs + kHdr);
@@ -466,21 +469,22 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                         continue;
                     }
                     // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and
-                    // gcd(k, d) = 1.  An arc of the support: g = gcd(k G, T) with G the gcd of the other fluxes; another
-                    // flux equal to 1 gives G = 1 and g = gcd(k, k f_a +- d) = gcd(k, d) = 1 without any gcd.
+                    // gcd(k, d) = 1.  An arc of the support: g = gcd(T, k f_t for t != a).
                     if (cin && cT != 1) {
-                        bool one = false;
+                        // every lane folds its scaled fluxes into r = gcd(T, k f_t, ...); r divides T, and one lane with
+                        // r = 1 settles g = 1 (the usual case: T is small and some flux is coprime to it)
+                        const bool narrow = cT < (1ULL << 32);
+                        u64 r = cT;
                         #pragma unroll 1
-                        for (int t = lane; t < ns; t += 32) one = one || (t != cia && flux[t] == 1);
-                        if (!__any_sync(FULL, one)) {
-                            const bool narrow = Pbig < (1ULL << 32);
-                            u64 G = 0;
-                            #pragma unroll 1
-                            for (int t = lane; t < ns; t += 32)
-                                if (t != cia) G = narrow ? (u64)gcd32((u32)G, (u32)flux[t]) : gcd64(G, (u64)flux[t]);
-                            G = w_gcd(G, narrow);
-                            cg = gcd64(ck * G, cT);   // k G <= k fmax <= 2^62
+                        for (int t = lane; t < ns; t += 32) {
+                            if (t == cia) continue;
+                            const u64 x = ck * (u64)flux[t];   // <= 2^62 (no overflow was found above)
+                            if (narrow) {
+                                const u32 r32 = (u32)r;
+                                r = gcd32(r32, (x >> 32) == 0 ? (u32)x % r32 : (u32)(x % (u64)r32));
+                            } else r = gcd64(r, x);
                         }
+                        if (!__any_sync(FULL, r == 1)) cg = w_gcd(r, narrow);
                     }
                     if (ck == 1 && cg == 1) {
                         chs = Phs + arc_term_t(A.g, (u32)ca, cT) - (cin ? arc_term_t(A.g, (u32)ca, (u64)flux[cia]) : 0ULL);
@@ -545,7 +549,13 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                         const int t = b2 + lane;
                         ins += __popc(__ballot_sync(FULL, t < ns && (int)arc[t] < ca));
                     }
-                i64* flux2 = (i64*)(dst + kHdr);
+                // The child is assembled in shared memory and leaves the SM as whole 16-byte chunks, so HBM sees full
+                // sectors (element-wise stores into fresh lines make the L2 fill every sector from DRAM first).  An
+                // entry larger than the assembly buffer is written in place.
+                const u32 cbytes = entry_bytes((u32)n2, (u32)nv2, (u32)nu2c);
+                const bool via_smem = cbytes <= A.sm_out_bytes;
+                unsigned char* wb = via_smem ? gs + A.sm_out : dst;
+                i64* flux2 = (i64*)(wb + kHdr);
                 u64* vis2 = (u64*)(flux2 + n2);
                 i64* ef2 = (i64*)(vis2 + nv2);
                 u16* arc2 = (u16*)(ef2 + nu2c);
@@ -611,9 +621,16 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     mx = w_max(mx);
                 }
                 if (lane == 0) {
-                    uint4* h4 = (uint4*)dst;
+                    uint4* h4 = (uint4*)wb;
                     h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2c, (u32)chs, (u32)(chs >> 32));
                     h4[1] = make_uint4((u32)chv, (u32)(chv >> 32), (u32)mx, (u32)(mx >> 32));
+                }
+                if (via_smem) {
+                    __syncwarp();
+                    const uint4* o4 = (const uint4*)(gs + A.sm_out);
+                    #pragma unroll 1
+                    for (u32 c = lane; c < cbytes / 16; c += 32) __stcs((uint4*)dst + c, o4[c]);
+                    __syncwarp();
                 }
             }
         }
@@ -732,14 +749,16 @@ static size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 void expand_smem_layout(ExpandArgs& a) {
     size_t off = align16(a.max_entry);   // staging holds the largest entry
     a.sm_sbits = (u32)off; off = align16(off + (size_t)a.g.W32 * 4);
-    a.sm_upos = (u32)off;  off = align16(off + (size_t)a.g.M * 2 + 2);
+    a.sm_upos = (u32)off;  off = align16(off + (size_t)a.g.M * 2 + 16);   // zeroed in 16-byte chunks
     a.sm_misc = (u32)off;  off = align16(off + (size_t)SS_WORDS * 8);
+    a.sm_out_bytes = a.max_entry < 2048u ? a.max_entry : 2048u;   // child assembly buffer (larger children: in place)
+    a.sm_out = (u32)off;   off = align16(off + a.sm_out_bytes);
     a.sm_group = (u32)off;
 }
 
 // key slots the count pass can leave unused: every warp of the largest grid may strand one chunk
 // every warp may strand one chunk of key slots; a warp covers kParentsPerWarp parents
-u64 expand_key_slack(u64 max_parents) { return (max_parents / kParentsPerWarp + kWarps + 1) * kKeyChunk; }
+u64 expand_key_slack(u64 max_parents) { return (max_parents / kParentsPerWarp + 16384) * kKeyChunk; }
 
 template <int MODE>
 static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
@@ -759,12 +778,16 @@ static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
         bps_cache[warps] = bps < 1 ? 1 : bps;
         smem_cache[warps] = smem;
     }
-    const u64 per_block = (u64)warps * kParentsPerWarp;
+    // small levels: fewer parents per warp so that every SM still gets its share of warps
+    u64 ppw = a.n_cur / ((u64)sm_count * 32);
+    ppw = ppw < 1 ? 1 : (ppw > (u64)kParentsPerWarp ? (u64)kParentsPerWarp : ppw);
+    ExpandArgs a2 = a;
+    a2.ppw = (u32)ppw;
+    const u64 per_block = (u64)warps * ppw;
     const u64 need = (a.n_cur + per_block - 1) / per_block;
     if (need > 0x7fffffffULL) return cudaErrorInvalidValue;
     unsigned grid = (unsigned)(need ? need : 1);
-    (void)sm_count;
-    k_expand<MODE><<<grid, warps * 32, smem, s>>>(a);
+    k_expand<MODE><<<grid, warps * 32, smem, s>>>(a2);
     return cudaGetLastError();
 }
 
