@@ -55,7 +55,8 @@ typedef struct {
     int64_t frontier_cap;   /* beam: entries expanded per level; 0 = unbounded                       */
     int64_t max_frontier;   /* entries per frontier buffer; 0 = max(frontier_cap, 4096), 2^20 when cap == 0 */
     int64_t max_candidates; /* capacity of the candidate buffer / support hash; 0 = 2^20             */
-    int64_t max_child_keys; /* capacity of the per-level beam key array; 0 = 64 * frontier_cap       */
+    int64_t max_child_keys; /* child slots per level (8-byte beam key + 64-byte task each, < 2^32);  */
+                            /* 0 = frontier_cap * the largest fan-out of a node                      */
     int32_t device;         /* CUDA device ordinal the workspace lives on                            */
     uint32_t flags;         /* EFM_F_*                                                               */
     int64_t max_frontier_bytes; /* bytes of one frontier buffer (entries are packed, variable size);         */

@@ -23,7 +23,7 @@ struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
     Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
-    Region ctl, buf[2], off[2], pmin, keys, ckeys, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill;
+    Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill;
     Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, dense;
     size_t total = 0;
 };
@@ -88,6 +88,8 @@ void make_layout(efm_handle* h) {
     add_region(L, L.pmin, (size_t)(h->max_frontier + 1) * 8);
     add_region(L, L.keys, (size_t)h->max_keys * 8);
     add_region(L, L.ckeys, (size_t)h->max_keys * 8);
+    for (int t = 0; t < 4; ++t) add_region(L, L.task[t], (size_t)h->max_keys * 16);
+    add_region(L, L.surv, (size_t)h->max_keys * 4);
     const size_t C = (size_t)h->max_cand;
     add_region(L, L.cand, C * h->cand_stride);
     add_region(L, L.table, h->table_size * 4);
@@ -222,6 +224,11 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     if (h->max_cand > 0xFFFFFFF0LL) { delete h; return EFM_E_INVAL; }
     h->max_keys = (P.max_child_keys ? P.max_child_keys : std::max<int64_t>(h->cap * (int64_t)G.max_fanout, 65536)) +
                   (int64_t)expand_key_slack((u64)h->max_frontier);
+    // child slots are addressed with 32 bits (survivor list); the default is clamped, an explicit request is refused
+    if (h->max_keys > 0xFFFFFFF0LL) {
+        if (P.max_child_keys) { delete h; return EFM_E_INVAL; }
+        h->max_keys = 0xFFFFFFF0LL;
+    }
     h->table_size = pow2_at_least((size_t)h->max_cand * 2);
     h->dense_bytes = std::max<size_t>((size_t)64 << 20, (size_t)n * 8 * 64);
     make_layout(h);
@@ -379,7 +386,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.cand = ws + L.cand.off;
     ea.keys = (u64*)(ws + L.keys.off);
     ea.ctl = d_ctl;
-    ea.pmin = (u64*)(ws + L.pmin.off);
+    ea.t0 = (uint4*)(ws + L.task[0].off); ea.t1 = (uint4*)(ws + L.task[1].off);
+    ea.t2 = (uint4*)(ws + L.task[2].off); ea.t3 = (uint4*)(ws + L.task[3].off);
+    ea.surv = (u32*)(ws + L.surv.off);
     ea.max_entry = h->max_entry; ea.cand_stride = h->cand_stride;
     ea.frontier_units = (u64)h->frontier_bytes >> 4;
     ea.max_frontier = (u64)h->max_frontier; ea.max_cand = (u64)h->max_cand; ea.max_keys = (u64)h->max_keys;
@@ -441,29 +450,25 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         ea.cur = ws + L.buf[cur].off; ea.nxt = ws + L.buf[cur ^ 1].off; ea.n_cur = n_cur;
         ea.cur_off = (const u64*)(ws + L.off[cur].off); ea.nxt_off = (u64*)(ws + L.off[cur ^ 1].off);
         const bool beam_possible = h->cap > 0 && ((h->flags & EFM_F_FORCE_TWO_PASS) || n_cur * (u64)G.max_fanout > (u64)h->cap);
-        if (beam_possible) {
-            size_t t0 = tm.mark();
-            CK(launch_expand(0, ea, h->sm_count, s)); ++launches;
-            size_t t1 = tm.mark();
-            CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), d_ctl, (u64)h->cap, ea.max_keys, std::min<u64>(ea.max_keys, n_cur * (u64)G.max_fanout), h->sm_count, s, &launches));
-            size_t t2 = tm.mark();
-            CK(launch_expand(1, ea, h->sm_count, s)); ++launches;
-            size_t t3 = tm.mark();
-            tm.span(t0, t1, PH_COUNT); tm.span(t1, t2, PH_BEAM); tm.span(t2, t3, PH_WRITE);
-            st.two_pass_levels++; st.n_expand_count++; st.n_expand_write++;
-        } else {
-            size_t t0 = tm.mark();
-            CK(launch_expand(2, ea, h->sm_count, s)); ++launches;
-            size_t t1 = tm.mark();
-            tm.span(t0, t1, PH_DIRECT);
-            st.direct_levels++; st.n_direct++;
-        }
+        // evaluate every child (keys + tasks) -> beam threshold -> list of survivors -> materialise them
+        size_t t0 = tm.mark();
+        CK(launch_expand(ea, h->sm_count, s)); ++launches;
+        size_t t1 = tm.mark();
+        CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), d_ctl, beam_possible ? (u64)h->cap : 0ULL, ea.max_keys,
+                         std::min<u64>(ea.max_keys, n_cur * (u64)G.max_fanout), h->sm_count, s, &launches));
+        size_t t2 = tm.mark();
+        CK(launch_materialise(ea, std::min<u64>(ea.max_keys, n_cur * 16), 0, h->sm_count, s, 0)); ++launches;
+        CK(launch_materialise(ea, 0, 0, h->sm_count, s, 1)); ++launches;
+        size_t t3 = tm.mark();
+        tm.span(t0, t1, PH_COUNT); tm.span(t1, t2, PH_BEAM); tm.span(t2, t3, PH_WRITE);
+        st.n_expand_count++; st.n_expand_write++;
+        if (beam_possible) st.two_pass_levels++; else st.direct_levels++;
         CK(read_ctl());
         if (hc->error) return EFM_E_CAPACITY;
         h->lvl_expanded[lvl] = (int64_t)hc->lvl_expanded;
         h->lvl_children[lvl] = (int64_t)hc->lvl_children;
         const int64_t n_next = (int64_t)(hc->n_next >> kAllocShift);
-        const int64_t active = beam_possible ? (int64_t)hc->n_keys : n_next;
+        const int64_t active = (int64_t)hc->n_keys;
         const int64_t done = (int64_t)hc->lvl_done;
         if (active + done > 0) {
             h->lvl_active.push_back(active);

@@ -62,6 +62,7 @@ struct Ctl {
     // per level (reset by k_level_begin)
     u64 n_next;        // packed allocator of the next frontier: count << 34 | 16-byte units (kAllocShift)
     u64 n_keys;        // active children generated (= valid keys written by the count pass)
+    u64 n_surv;        // children of the level that are materialised (k_compact)
     u64 n_slots;       // key slots reserved by the count pass (chunked per warp; unused slots hold kKeySentinel)
     u64 lvl_done;      // balanced children generated
     u64 lvl_children;  // children generated (active + done)
@@ -87,8 +88,9 @@ struct ExpandArgs {
     unsigned char* nxt;         // children that stay active (packed)
     u64* nxt_off;
     unsigned char* cand;        // balanced children (fixed stride)
-    u64* keys;                  // beam keys of the active children (count pass)
-    u64* pmin;                  // per parent: smallest key among its active children (count pass -> write pass)
+    u64* keys;                  // per child slot: beam key (kKeyDone: balanced child; kKeySentinel: unused slot)
+    uint4* t0; uint4* t1; uint4* t2; uint4* t3;   // per child slot: the task (see k_expand / k_materialise)
+    u32* surv;                  // slots of the children that are materialised
     Ctl* ctl;
     u64 n_cur;
     u32 max_entry, cand_stride; // largest entry in bytes (shared-memory staging), candidate slot stride
@@ -133,6 +135,8 @@ __host__ __device__ inline u64 vis_pack(u32 met, u32 PI, u32 PO, u32 cnt) {
 }
 __host__ __device__ inline u64 beam_key(u32 n_unb, u64 h) { return ((u64)(n_unb > 255u ? 255u : n_unb) << 56) | (h >> 8); }
 
+constexpr u64 kKeyDone = ~0ULL - 1ULL;   // key slot of a balanced child: always materialised, outside the beam ranking
+enum { TF_NEG = 1, TF_FIRST = 2, TF_INSUPP = 4 };   // task flags: bump subtracts (Eq 5); first visit; arc already in the support
 constexpr u64 kKeySentinel = ~0ULL;   // filler of reserved but unused key slots: never < X, skipped by the select
 constexpr u32 kKeyChunk = 64;         // key slots a warp reserves per atomic
 

@@ -19,7 +19,6 @@
 
 namespace efm {
 
-enum { MODE_COUNT = 0, MODE_WRITE = 1, MODE_DIRECT = 2 };
 enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
 #ifndef EFM_MIN_BLOCKS
 #define EFM_MIN_BLOCKS 16   // resident one-warp blocks per SM the register allocation aims at (128 registers)
@@ -102,12 +101,14 @@ __device__ __forceinline__ u64 abs64(i64 v) { return (u64)(v < 0 ? -v : v); }
 __device__ __forceinline__ u64 arc_term_t(const DevGraph& g, u32 a, u64 f) { return mix64(__ldg(&g.arc_mix[a]) + f); }
 
 // Per-warp chunked reservation of beam-key slots: one atomic per kKeyChunk keys instead of one per child.
+constexpr u64 kNoSlot = ~0ULL;
 struct KeyOut {
     u64 base; u32 left;
-    __device__ __forceinline__ void push(const ExpandArgs& A, int lane, bool want, u64 key) {
+    // one slot for every lane with want = true (others, and everyone after an overflow, get kNoSlot)
+    __device__ __forceinline__ u64 reserve(const ExpandArgs& A, int lane, bool want) {
         const u32 m = __ballot_sync(FULL, want);
         const u32 cnt = (u32)__popc(m);
-        if (cnt == 0) return;
+        if (cnt == 0) return kNoSlot;
         if (cnt > left) {
 #pragma unroll 1
             for (u32 t = lane; t < left; t += 32) A.keys[base + t] = kKeySentinel;
@@ -117,12 +118,13 @@ struct KeyOut {
             if (b + kKeyChunk > A.max_keys) {
                 if (lane == 0) atomicOr(&A.ctl->error, (u32)ERR_KEYS);
                 left = 0;
-                return;
+                return kNoSlot;
             }
             base = b; left = kKeyChunk;
         }
-        if (want) __stcs(&A.keys[base + __popc(m & ((1u << lane) - 1u))], key);
+        const u64 slot = want ? base + __popc(m & ((1u << lane) - 1u)) : kNoSlot;
         base += cnt; left -= cnt;
+        return slot;
     }
     __device__ __forceinline__ void finish(const ExpandArgs& A, int lane) {
         for (u32 t = lane; t < left; t += 32) A.keys[base + t] = kKeySentinel;
@@ -147,9 +149,9 @@ enum { SS_EXPANDED = 0, SS_CHILDREN, SS_DONE, SS_ACTIVE, SS_DEAD, SS_NOTEFM, SS_
        SS_WORDS = SS_KC + 4 };
 
 // One kernel body, every routine inlined once: the staged parent is addressed through shared-memory pointers the
-// compiler can track, and both kinds of children (lane-parallel "fast" ones and warp-cooperative "general" ones) funnel
-// into a single evaluate / place / write sequence.
-template <int MODE>
+// compiler can track.  The kernel only EVALUATES: every child that passes the discard tests gets a slot holding its
+// beam key and a 64-byte task (what k_materialise needs to build it from its parent); nothing is written to the next
+// frontier here, so a parent with hundreds of surviving children costs this warp no more than one without any.
 __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_constant__ ExpandArgs A) {
     extern __shared__ uint4 smem4[];
     const int lane = threadIdx.x & 31;
@@ -168,8 +170,6 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
     __syncwarp();
 
     Ctl* ctl = A.ctl;
-    const bool notrunc = MODE == MODE_WRITE ? ctl->notrunc != 0 : true;
-    const u64 X = MODE == MODE_WRITE ? ctl->X : 0;
     const bool fast_graph = !A.no_fast && A.g.max_coef < kSmallCoef;
     KeyOut ko; ko.base = 0; ko.left = 0;
     // a warp owns A.ppw (<= kParentsPerWarp) consecutive parents; the grid covers the level and the block scheduler evens out the
@@ -179,7 +179,6 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
 
 #pragma unroll 1
     for (u64 p = p0; p < p1; ++p) {
-        if (MODE == MODE_WRITE && !notrunc && __ldcs(&A.pmin[p]) >= X) continue;   // no child of p survives the beam
         // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
         const uint4* src = (const uint4*)(A.cur + (__ldcs(&A.cur_off[p]) << 4));
         const uint4 first16 = __ldcs(src + lane);   // the buffers end in 512 spare bytes
@@ -216,9 +215,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         const bool fwd = E > 0;
         const u64 absE = abs64(E);
         auto ef_of = [&](int met) -> i64 { const u32 u = upos[met]; return u ? ef[u - 1] : 0; };
-        if (MODE != MODE_WRITE && lane == 0) { sst[SS_EXPANDED]++; sst[SS_BYTES] += algo_entry_bytes((u32)ns, (u32)nv); }
-        if (MODE == MODE_WRITE && lane == 0) sst[SS_WRITE_PARENTS]++;
-        u64 kmin = ~0ULL;   // smallest key among the active children of p (count pass)
+        if (lane == 0) { sst[SS_EXPANDED]++; sst[SS_BYTES] += algo_entry_bytes((u32)ns, (u32)nv); }
         // visited?
         int vk = -1;
         #pragma unroll 1
@@ -228,7 +225,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
             if (hit) vk = base + __ffs(hit) - 1;
         }
         const bool firstv = vk < 0;
-        if (MODE != MODE_WRITE && lane == 0) { sst[SS_FIRST] += firstv; sst[SS_SATURATED] += ns >= A.D; }
+        if (lane == 0) { sst[SS_FIRST] += firstv; sst[SS_SATURATED] += ns >= A.D; }
         const int in0 = __ldg(&A.g.in_ptr[istar]), nI = __ldg(&A.g.in_ptr[istar + 1]) - in0;
         const int out0 = __ldg(&A.g.out_ptr[istar]), nO = __ldg(&A.g.out_ptr[istar + 1]) - out0;
 
@@ -240,7 +237,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         if (firstv) {
             // PROC1 / PROC1' (Eq 3; readings G1, G13, G14, G15, G22)
             if (nv >= A.V) {
-                if (MODE != MODE_WRITE && lane == 0) sst[SS_VISITED]++;
+                if (lane == 0) sst[SS_VISITED]++;
             } else {
                 // primary on the side the flux arrives from: lowest arc of that side in the support (G13)
                 const int2* plist = fwd ? A.g.in_e + in0 : A.g.out_e + out0;
@@ -260,7 +257,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
             rec = vis[vk];
             const int cntv = (int)(rec >> 48) + 1;
             if (cntv > A.max_loop) {
-                if (MODE != MODE_WRITE && lane == 0) sst[SS_NOTEFM]++;
+                if (lane == 0) sst[SS_NOTEFM]++;
             } else {
                 const int PI = (int)((rec >> 16) & 0xffffu), PO = (int)(rec & 0xffffu);
                 int lPI = -1, lPO = -1, cPI = 0, cPO = 0;
@@ -311,7 +308,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
             } else if (lane == 0) {
                 a = r_a; c = r_c; adm = true; insup = true;   // PI / PO are arcs of the support
             }
-            if (MODE != MODE_WRITE && lane == 0) sst[SS_ROUNDS]++;
+            if (lane == 0) sst[SS_ROUNDS]++;
             const u32 adm_m = __ballot_sync(FULL, adm);
             if (adm_m == 0) continue;
             n_adm += __popc(adm_m);
@@ -362,283 +359,153 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 }
             }
             const u32 done_m = __ballot_sync(FULL, fast && nu2 == 0);
-            if (MODE != MODE_WRITE && lane == 0) {
+            if (lane == 0) {
                 const int nf = __popc(fast_m);
-                sst[SS_CHILDREN] += nf; sst[SS_BYTES] += 8 * nf; sst[SS_DONE] += __popc(done_m);
+                sst[SS_CHILDREN] += nf; sst[SS_BYTES] += 8 * nf; sst[SS_DONE] += __popc(done_m); sst[SS_ACTIVE] += __popc(fast_m & ~done_m);
             }
-            u32 keep_m;
-            if (MODE == MODE_COUNT) {
-                const bool act = fast && nu2 != 0;
-                if (lane == 0) sst[SS_ACTIVE] += __popc(fast_m & ~done_m);
-                ko.push(A, lane, act, key);
-                if (act) kmin = min(kmin, key);
-                keep_m = done_m;
-            } else if (MODE == MODE_WRITE) {
-                keep_m = __ballot_sync(FULL, fast && nu2 != 0 && (notrunc || key < X));
-            } else {
-                keep_m = fast_m;
+            // ---- emit the lane-parallel children: one slot each (beam key + task)
+            if (fast_m) {
+                const u64 slot = ko.reserve(A, lane, fast);
+                if (fast && slot != kNoSlot) {
+                    const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : a), (u32)(fwd ? a : prim), 0u);
+                    __stcs(&A.keys[slot], nu2 == 0 ? kKeyDone : key);
+                    __stcs(&A.t0[slot], make_uint4((u32)p, (u32)a | 0xffff0000u, (u32)nu2 | ((u32)TF_FIRST << 16), k));
+                    __stcs(&A.t1[slot], make_uint4((u32)d, (u32)(d >> 32), (u32)d, (u32)(d >> 32)));
+                    __stcs(&A.t2[slot], make_uint4(1u, 0u, (u32)hs2, (u32)(hs2 >> 32)));
+                    __stcs(&A.t3[slot], make_uint4((u32)hv2, (u32)(hv2 >> 32), (u32)newrec, (u32)(newrec >> 32)));
+                }
             }
-            // ---- one child at a time: general evaluation (arc of the support, large integers) and / or materialisation
-            const u32 slow_m = adm_m & ~fast_m;
-            u32 work_m = keep_m | slow_m;
+            // ---- one child at a time: general evaluation (arc of the support, large integers)
+            u32 slow_m = adm_m & ~fast_m;
             #pragma unroll 1
-            while (work_m) {
-                const int l = __ffs(work_m) - 1;
-                work_m &= work_m - 1;
-                const bool general = (slow_m >> l) & 1u;
+            while (slow_m) {
+                const int l = __ffs(slow_m) - 1;
+                slow_m &= slow_m - 1;
                 // warp-uniform description of the child relative to its parent
                 const int ca = __shfl_sync(FULL, a, l);
-                u64 ck = __shfl_sync(FULL, k, l);        // scale
-                u64 cd = w_bcast(d, l);                  // |E| / gcd(|E|, c)
-                u64 cT = cd;                             // un-normalised new flux of arc ca
-                u64 cg = 1;                              // common divisor of the un-normalised child
-                u64 chs = w_bcast(hs2, l), chv = w_bcast(hv2, l);
-                int cnu = __shfl_sync(FULL, nu2, l);
-                int csign = +1, cia = -1;
-                bool cin = false, keep = true;
-                u64 newrec = firstv ? vis_pack((u32)istar, (u32)(fwd ? prim : ca), (u32)(fwd ? ca : prim), 0u) : r_newrec;
+                u64 ck, cd, cT, cg = 1, chs, chv;   // scale, |E| / gcd(|E|, c), un-normalised new flux of ca, common divisor, hash sums
+                int cnu = nu, csign = +1, cia = -1;
+                bool cin = false;
+                const u64 newrec = firstv ? vis_pack((u32)istar, (u32)(fwd ? prim : ca), (u32)(fwd ? ca : prim), 0u) : r_newrec;
                 const int qa0 = __ldg(&A.g.col_ptr[ca]), qa1 = __ldg(&A.g.col_ptr[ca + 1]);
-                if (general) {
-                    // bump(f, a, sign*|E|/c) of SURVEY.md 8(c) O6 with the whole warp
-                    const int cc = __shfl_sync(FULL, c, l);
-                    csign = firstv ? +1 : r_sign;
-                    const u64 gg = cc == 1 ? 1ULL : gcd64(absE, (u64)cc);
-                    ck = gg == 1 ? (u64)cc : (u64)cc / gg;
-                    cd = gg == 1 ? absE : absE / gg;
-                    cin = sbit(sbits, ca);
-                    if (cin) {   // position of the arc in the sorted support
-                        #pragma unroll 1
-                        for (int b2 = 0; b2 < ns && cia < 0; b2 += 32) {
-                            const int t = b2 + lane;
-                            const u32 hit = __ballot_sync(FULL, t < ns && arc[t] == ca);
-                            if (hit) cia = b2 + __ffs(hit) - 1;
-                        }
-                    }
-                    // scaled fluxes F_t = k f_t, F_a = k f_a +- d: overflow first, then non-positive (order of O6).
-                    // Pbig >= every flux and |EF| of the parent: products below the guard with it need no exact sweep.
-                    const bool bigk = ck > 1 && umul_gt_guard(ck, Pbig);
-                    bool ovf = false, nonpos = false;
-                    cT = cd;
-                    if (cin) {
-                        const u64 fa = (u64)flux[cia];
-                        const u64 lo = ck * fa, hi = __umul64hi(ck, fa);
-                        if (csign > 0) {
-                            cT = lo + cd;
-                            const u64 hi2 = hi + (cT < lo);
-                            ovf = hi2 != 0 || cT > EFM_GUARD;
-                        } else {
-                            if (hi == 0 && lo <= cd) { nonpos = true; cT = 0; }           // k f_a - d <= 0
-                            else { cT = lo - cd; const u64 hi2 = hi - (lo < cd); ovf = hi2 != 0 || cT > EFM_GUARD; }
-                        }
-                    }
-                    if (bigk) {   // exact: the largest flux among t != ia (a new arc carries d <= |E| <= 2^62)
-                        u64 mx = 0;
-                        #pragma unroll 1
-                        for (int t = lane; t < ns; t += 32) if (t != cia) mx = max(mx, (u64)flux[t]);
-                        mx = w_max(mx);
-                        ovf = ovf || umul_gt_guard(ck, mx);
-                    }
-                    int status = ovf ? CH_OVERFLOW : (nonpos ? CH_NONPOS : CH_OK);   // Prop 3, G11
-                    if (status == CH_OK) {
-                        // extra fluxes of the un-normalised child: EF'_i = k EF_i + sign d s_ia (Eq 2 on the scaled fluxes)
-                        bool ovf2 = false;
-                        if (bigk) {   // exact sweep over the unbalanced metabolites outside col(a)
-                            #pragma unroll 1
-                            for (int t = lane; t < nu; t += 32) {
-                                const int i = efmet[t];
-                                bool in_a = false;
-                                #pragma unroll 1
-                                for (int r = qa0; r < qa1; ++r) in_a = in_a || __ldg(&A.g.col[r]).x == i;
-                                if (!in_a) ovf2 = ovf2 || abs_gt_guard(mul_s((i64)ck, ef[t]));
-                            }
-                        }
-                        int delta = 0;
-                        #pragma unroll 1
-                        for (int qq = qa0 + lane; qq < qa1; qq += 32) {
-                            const int2 e = __ldg(&A.g.col[qq]);
-                            const i64 efp = ef_of(e.x);
-                            const S128 x = add_s(mul_s((i64)ck, efp), mul_s(csign > 0 ? (i64)cd : -(i64)cd, (i64)e.y));
-                            ovf2 = ovf2 || abs_gt_guard(x);
-                            delta += (int)((x.lo | (u64)x.hi) != 0) - (int)(efp != 0);
-                        }
-                        if (__any_sync(FULL, ovf2)) status = CH_OVERFLOW;
-                        else cnu = nu + __reduce_add_sync(FULL, delta);
-                    }
-                    if (status != CH_OK) {
-                        if (MODE != MODE_WRITE && lane == 0) sst[status == CH_OVERFLOW ? SS_OVF : SS_NONPOS]++;
-                        continue;
-                    }
-                    // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and
-                    // gcd(k, d) = 1.  An arc of the support: g = gcd(T, k f_t for t != a).
-                    if (cin && cT != 1) {
-                        // every lane folds its scaled fluxes into r = gcd(T, k f_t, ...); r divides T, and one lane with
-                        // r = 1 settles g = 1 (the usual case: T is small and some flux is coprime to it)
-                        const bool narrow = cT < (1ULL << 32);
-                        u64 r = cT;
-                        #pragma unroll 1
-                        for (int t = lane; t < ns; t += 32) {
-                            if (t == cia) continue;
-                            const u64 x = ck * (u64)flux[t];   // <= 2^62 (no overflow was found above)
-                            if (narrow) {
-                                const u32 r32 = (u32)r;
-                                r = gcd32(r32, (x >> 32) == 0 ? (u32)x % r32 : (u32)(x % (u64)r32));
-                            } else r = gcd64(r, x);
-                        }
-                        if (!__any_sync(FULL, r == 1)) cg = w_gcd(r, narrow);
-                    }
-                    if (ck == 1 && cg == 1) {
-                        chs = Phs + arc_term_t(A.g, (u32)ca, cT) - (cin ? arc_term_t(A.g, (u32)ca, (u64)flux[cia]) : 0ULL);
-                    } else {
-                        chs = 0;
-                        #pragma unroll 1
-                        for (int t = lane; t < ns; t += 32) {
-                            u64 F = t == cia ? cT : ck * (u64)flux[t];
-                            if (cg > 1) F /= cg;
-                            chs += arc_term_t(A.g, (u32)arc[t], F);
-                        }
-                        chs = w_sum(chs);
-                        if (!cin) chs += arc_term_t(A.g, (u32)ca, cT);
-                    }
-                    chv = Phv + vis_term(newrec) - (firstv ? 0ULL : vis_term(rec));
-                    // account for the child, classify it, decide whether it is materialised in this pass
-                    const bool cdone = cnu == 0;
-                    if (MODE != MODE_WRITE && lane == 0) { sst[SS_CHILDREN]++; sst[SS_GENERAL]++; sst[SS_BYTES] += 8; if (cdone) sst[SS_DONE]++; }
-                    if (cdone) keep = MODE != MODE_WRITE;   // balanced children are written where they are first seen
-                    else {
-                        const u64 ckey = beam_key((u32)cnu, mix64(chs + chv));
-                        if (MODE == MODE_COUNT) {
-                            if (lane == 0) sst[SS_ACTIVE]++;
-                            ko.push(A, lane, lane == 0, ckey);
-                            kmin = min(kmin, ckey);
-                            keep = false;
-                        } else keep = MODE == MODE_DIRECT || notrunc || ckey < X;
-                    }
-                }
-                if (!keep) continue;
-                // ---- place: a candidate slot (balanced) or a packed entry of the next frontier
-                const bool to_cand = cnu == 0;
-                const int n2 = ns + (cin ? 0 : 1);
-                const int nv2 = to_cand ? 0 : nv + (firstv ? 1 : 0);
-                const int nu2c = to_cand ? 0 : cnu;
-                if (lane == 0) sst[SS_BYTES] += algo_entry_bytes((u32)n2, (u32)(nv + (firstv ? 1 : 0)));
-                unsigned char* dst;
-                if (to_cand) {
-                    u64 slot = 0;
-                    if (lane == 0) slot = atomicAdd(&ctl->n_cand, 1ULL);
-                    slot = w_bcast(slot, 0);
-                    if (slot >= A.max_cand) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_CAND); continue; }
-                    dst = A.cand + slot * A.cand_stride;
-                } else {
-                    const u64 units = entry_bytes((u32)n2, (u32)nv2, (u32)nu2c) >> 4;
-                    u64 old = 0;
-                    if (lane == 0) old = atomicAdd(&ctl->n_next, (1ULL << kAllocShift) | units);
-                    old = w_bcast(old, 0);
-                    const u64 slot = old >> kAllocShift, off = old & kAllocUnitMask;
-                    if (slot >= A.max_frontier || off + units > A.frontier_units) {
-                        if (lane == 0) atomicOr(&ctl->error, (u32)ERR_FRONTIER);
-                        continue;
-                    }
-                    if (lane == 0) A.nxt_off[slot] = off;
-                    dst = A.nxt + (off << 4);
-                }
-                // ---- write
-                int ins = 0;   // a new arc goes where the ascending order puts it
-                if (!cin)
+                {
+                // bump(f, a, sign*|E|/c) of SURVEY.md 8(c) O6 with the whole warp
+                const int cc = __shfl_sync(FULL, c, l);
+                csign = firstv ? +1 : r_sign;
+                const u64 gg = cc == 1 ? 1ULL : gcd64(absE, (u64)cc);
+                ck = gg == 1 ? (u64)cc : (u64)cc / gg;
+                cd = gg == 1 ? absE : absE / gg;
+                cin = sbit(sbits, ca);
+                if (cin) {   // position of the arc in the sorted support
                     #pragma unroll 1
-                    for (int b2 = 0; b2 < ns; b2 += 32) {
+                    for (int b2 = 0; b2 < ns && cia < 0; b2 += 32) {
                         const int t = b2 + lane;
-                        ins += __popc(__ballot_sync(FULL, t < ns && (int)arc[t] < ca));
+                        const u32 hit = __ballot_sync(FULL, t < ns && arc[t] == ca);
+                        if (hit) cia = b2 + __ffs(hit) - 1;
                     }
-                // The child is assembled in shared memory and leaves the SM as whole 16-byte chunks, so HBM sees full
-                // sectors (element-wise stores into fresh lines make the L2 fill every sector from DRAM first).  An
-                // entry larger than the assembly buffer is written in place.
-                const u32 cbytes = entry_bytes((u32)n2, (u32)nv2, (u32)nu2c);
-                const bool via_smem = cbytes <= A.sm_out_bytes;
-                unsigned char* wb = via_smem ? gs + A.sm_out : dst;
-                i64* flux2 = (i64*)(wb + kHdr);
-                u64* vis2 = (u64*)(flux2 + n2);
-                i64* ef2 = (i64*)(vis2 + nv2);
-                u16* arc2 = (u16*)(ef2 + nu2c);
-                u16* efmet2 = arc2 + n2;
-                u64 mx = cin ? 0ULL : cT;   // a new arc never comes with a common divisor
-                #pragma unroll 1
-                for (int t = lane; t < ns; t += 32) {
-                    u64 F = t == cia ? cT : ck * (u64)flux[t];
-                    if (cg > 1) F /= cg;
-                    const int pos = t + ((!cin && t >= ins) ? 1 : 0);
-                    flux2[pos] = (i64)F;
-                    arc2[pos] = arc[t];
-                    mx = max(mx, F);
                 }
-                if (!cin && lane == 0) { flux2[ins] = (i64)cT; arc2[ins] = (u16)ca; }
-                if (!to_cand) {
-                    #pragma unroll 1
-                    for (int u = lane; u < nv; u += 32) vis2[u] = (!firstv && u == vk) ? newrec : vis[u];
-                    if (firstv && lane == 0) vis2[nv] = newrec;
-                    // EF list of the child: EF' = (k EF + sign d s_.a) / g over the parent's list, then the metabolites
-                    // of col(a) that were balanced in the parent.  The evaluation above (or the bounds of the fast path)
-                    // established that nothing exceeds 2^62, so the wrapping 64-bit arithmetic is exact.
-                    const u64 sd = csign > 0 ? cd : (u64)0 - cd;
-                    int wbase = 0;
-                    #pragma unroll 1
-                    for (int t0 = 0; t0 < nu; t0 += 32) {
-                        const int t = t0 + lane;
-                        const bool valid = t < nu;
-                        i64 x = 0;
-                        int met = 0;
-                        if (valid) {
-                            met = efmet[t];
-                            i64 s = 0;
-                            #pragma unroll 1
-                            for (int qq = qa0; qq < qa1; ++qq) { const int2 e = __ldg(&A.g.col[qq]); if (e.x == met) s = e.y; }
-                            x = (i64)(ck * (u64)ef[t] + sd * (u64)s);
-                            if (cg > 1) x /= (i64)cg;
-                        }
-                        const u32 nz = __ballot_sync(FULL, valid && x != 0);
-                        if (valid && x != 0) {
-                            const int pos = wbase + __popc(nz & lt);
-                            ef2[pos] = x; efmet2[pos] = (u16)met;
-                            mx = max(mx, abs64(x));
-                        }
-                        wbase += __popc(nz);
+                // scaled fluxes F_t = k f_t, F_a = k f_a +- d: overflow first, then non-positive (order of O6).
+                // Pbig >= every flux and |EF| of the parent: products below the guard with it need no exact sweep.
+                const bool bigk = ck > 1 && umul_gt_guard(ck, Pbig);
+                bool ovf = false, nonpos = false;
+                cT = cd;
+                if (cin) {
+                    const u64 fa = (u64)flux[cia];
+                    const u64 lo = ck * fa, hi = __umul64hi(ck, fa);
+                    if (csign > 0) {
+                        cT = lo + cd;
+                        const u64 hi2 = hi + (cT < lo);
+                        ovf = hi2 != 0 || cT > EFM_GUARD;
+                    } else {
+                        if (hi == 0 && lo <= cd) { nonpos = true; cT = 0; }           // k f_a - d <= 0
+                        else { cT = lo - cd; const u64 hi2 = hi - (lo < cd); ovf = hi2 != 0 || cT > EFM_GUARD; }
                     }
+                }
+                if (bigk) {   // exact: the largest flux among t != ia (a new arc carries d <= |E| <= 2^62)
+                    u64 mx = 0;
                     #pragma unroll 1
-                    for (int q0 = qa0; q0 < qa1; q0 += 32) {
-                        const int qq = q0 + lane;
-                        int2 e = make_int2(0, 0);
-                        bool only = false;
-                        if (qq < qa1) { e = __ldg(&A.g.col[qq]); only = upos[e.x] == 0; }
-                        const u32 m = __ballot_sync(FULL, only);
-                        if (only) {
-                            i64 x = (i64)(sd * (u64)(i64)e.y);
-                            if (cg > 1) x /= (i64)cg;
-                            const int pos = wbase + __popc(m & lt);
-                            ef2[pos] = x; efmet2[pos] = (u16)e.x;
-                            mx = max(mx, abs64(x));
-                        }
-                        wbase += __popc(m);
-                    }
+                    for (int t = lane; t < ns; t += 32) if (t != cia) mx = max(mx, (u64)flux[t]);
                     mx = w_max(mx);
+                    ovf = ovf || umul_gt_guard(ck, mx);
                 }
-                if (lane == 0) {
-                    uint4* h4 = (uint4*)wb;
-                    h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2c, (u32)chs, (u32)(chs >> 32));
-                    h4[1] = make_uint4((u32)chv, (u32)(chv >> 32), (u32)mx, (u32)(mx >> 32));
-                }
-                if (via_smem) {
-                    __syncwarp();
-                    const uint4* o4 = (const uint4*)(gs + A.sm_out);
+                int status = ovf ? CH_OVERFLOW : (nonpos ? CH_NONPOS : CH_OK);   // Prop 3, G11
+                if (status == CH_OK) {
+                    // extra fluxes of the un-normalised child: EF'_i = k EF_i + sign d s_ia (Eq 2 on the scaled fluxes)
+                    bool ovf2 = false;
+                    if (bigk) {   // exact sweep over the unbalanced metabolites outside col(a)
+                        #pragma unroll 1
+                        for (int t = lane; t < nu; t += 32) {
+                            const int i = efmet[t];
+                            bool in_a = false;
+                            #pragma unroll 1
+                            for (int r = qa0; r < qa1; ++r) in_a = in_a || __ldg(&A.g.col[r]).x == i;
+                            if (!in_a) ovf2 = ovf2 || abs_gt_guard(mul_s((i64)ck, ef[t]));
+                        }
+                    }
+                    int delta = 0;
                     #pragma unroll 1
-                    for (u32 c = lane; c < cbytes / 16; c += 32) __stcs((uint4*)dst + c, o4[c]);
-                    __syncwarp();
+                    for (int qq = qa0 + lane; qq < qa1; qq += 32) {
+                        const int2 e = __ldg(&A.g.col[qq]);
+                        const i64 efp = ef_of(e.x);
+                        const S128 x = add_s(mul_s((i64)ck, efp), mul_s(csign > 0 ? (i64)cd : -(i64)cd, (i64)e.y));
+                        ovf2 = ovf2 || abs_gt_guard(x);
+                        delta += (int)((x.lo | (u64)x.hi) != 0) - (int)(efp != 0);
+                    }
+                    if (__any_sync(FULL, ovf2)) status = CH_OVERFLOW;
+                    else cnu = nu + __reduce_add_sync(FULL, delta);
+                }
+                if (status != CH_OK) {
+                    if (lane == 0) sst[status == CH_OVERFLOW ? SS_OVF : SS_NONPOS]++;
+                    continue;
+                }
+                // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and
+                // gcd(k, d) = 1.  An arc of the support: g = gcd(T, k f_t for t != a).
+                if (cin && cT != 1) {
+                    // every lane folds its scaled fluxes into r = gcd(T, k f_t, ...); r divides T, and one lane with
+                    // r = 1 settles g = 1 (the usual case: T is small and some flux is coprime to it)
+                    const bool narrow = cT < (1ULL << 32);
+                    u64 r = cT;
+                    #pragma unroll 1
+                    for (int t = lane; t < ns; t += 32) {
+                        if (t == cia) continue;
+                        const u64 x = ck * (u64)flux[t];   // <= 2^62 (no overflow was found above)
+                        if (narrow) {
+                            const u32 r32 = (u32)r;
+                            r = gcd32(r32, (x >> 32) == 0 ? (u32)x % r32 : (u32)(x % (u64)r32));
+                        } else r = gcd64(r, x);
+                    }
+                    if (!__any_sync(FULL, r == 1)) cg = w_gcd(r, narrow);
+                }
+                if (ck == 1 && cg == 1) {
+                    chs = Phs + arc_term_t(A.g, (u32)ca, cT) - (cin ? arc_term_t(A.g, (u32)ca, (u64)flux[cia]) : 0ULL);
+                } else {
+                    chs = 0;
+                    #pragma unroll 1
+                    for (int t = lane; t < ns; t += 32) {
+                        u64 F = t == cia ? cT : ck * (u64)flux[t];
+                        if (cg > 1) F /= cg;
+                        chs += arc_term_t(A.g, (u32)arc[t], F);
+                    }
+                    chs = w_sum(chs);
+                    if (!cin) chs += arc_term_t(A.g, (u32)ca, cT);
+                }
+                chv = Phv + vis_term(newrec) - (firstv ? 0ULL : vis_term(rec));
+                }
+                // account for the child and emit it
+                const bool cdone = cnu == 0;
+                if (lane == 0) { sst[SS_CHILDREN]++; sst[SS_GENERAL]++; sst[SS_BYTES] += 8; sst[cdone ? SS_DONE : SS_ACTIVE]++; }
+                const u64 slot = ko.reserve(A, lane, lane == 0);
+                if (lane == 0 && slot != kNoSlot) {
+                    const u32 flags = (csign < 0 ? TF_NEG : 0u) | (firstv ? TF_FIRST : 0u) | (cin ? TF_INSUPP : 0u);
+                    __stcs(&A.keys[slot], cdone ? kKeyDone : beam_key((u32)cnu, mix64(chs + chv)));
+                    __stcs(&A.t0[slot], make_uint4((u32)p, (u32)ca | ((u32)(cia & 0xffff) << 16), (u32)cnu | (flags << 16), (u32)ck));
+                    __stcs(&A.t1[slot], make_uint4((u32)cd, (u32)(cd >> 32), (u32)cT, (u32)(cT >> 32)));
+                    __stcs(&A.t2[slot], make_uint4((u32)cg, (u32)(cg >> 32), (u32)chs, (u32)(chs >> 32)));
+                    __stcs(&A.t3[slot], make_uint4((u32)chv, (u32)(chv >> 32), (u32)newrec, (u32)(newrec >> 32)));
                 }
             }
         }
-        if (MODE != MODE_WRITE && firstv && nv < A.V && n_adm == 0 && lane == 0) sst[SS_DEAD]++;   // no admissible alternative
-        if (MODE == MODE_COUNT) {
-            kmin = w_min(kmin);
-            if (lane == 0) A.pmin[p] = kmin;
-        }
+        if (firstv && nv < A.V && n_adm == 0 && lane == 0) sst[SS_DEAD]++;   // no admissible alternative
         // ---- restore the shared tables to zero for the next parent
         __syncwarp();
         #pragma unroll 1
@@ -647,7 +514,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         for (int t = lane; t < nu; t += 32) upos[efmet[t]] = 0;
         __syncwarp();
     }
-    if (MODE == MODE_COUNT) ko.finish(A, lane);
+    ko.finish(A, lane);
     __syncwarp();
     if (lane == 0) {
         u64* st = ctl->st;
@@ -665,12 +532,201 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         if (sst[SS_FIRST]) atomicAdd(&st[ST_FIRST], sst[SS_FIRST]);
         if (sst[SS_GENERAL]) atomicAdd(&st[ST_GENERAL], sst[SS_GENERAL]);
         if (sst[SS_SATURATED]) atomicAdd(&st[ST_SATURATED], sst[SS_SATURATED]);
-        if (sst[SS_WRITE_PARENTS]) atomicAdd(&st[ST_WRITE_PARENTS], sst[SS_WRITE_PARENTS]);
+    }
+}
+
+// ------------------------------------------------------------------ survivors of the beam -> list of slots
+// One thread per key slot: balanced children (kKeyDone) and active children with key < X (all of them when the beam
+// does not bind).  Warp-aggregated append; the order of the list does not matter.
+__global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, u32* __restrict__ surv, Ctl* ctl, u64 max_keys) {
+    const u64 n = min(ctl->n_slots, max_keys);
+    const bool notrunc = ctl->notrunc != 0;
+    const u64 X = ctl->X;
+    const int lane = threadIdx.x & 31;
+    for (u64 base = ((u64)blockIdx.x * blockDim.x + threadIdx.x) & ~31ULL; base < n; base += (u64)gridDim.x * blockDim.x) {
+        const u64 i = base + lane;
+        const u64 key = i < n ? __ldcs(&keys[i]) : kKeySentinel;
+        const bool take = key == kKeyDone || (key != kKeySentinel && (notrunc || key < X));
+        const u32 m = __ballot_sync(0xffffffffu, take);
+        if (m) {
+            u64 pos = 0;
+            if (lane == 0) pos = atomicAdd(&ctl->n_surv, (u64)__popc(m));
+            pos = __shfl_sync(0xffffffffu, pos, 0);
+            if (take) surv[pos + __popc(m & ((1u << lane) - 1u))] = (u32)i;
+        }
+    }
+}
+
+// ------------------------------------------------------------------ materialise: one warp per surviving child
+// Reads the task, reads the parent entry straight from HBM / L2 (every element is needed once) and writes the child:
+// a candidate slot if it is balanced, otherwise a packed entry of the next frontier.  A block of kMatWarps children
+// reserves its output with one atomic per kind.
+constexpr int kMatWarps = 8;
+__global__ void __launch_bounds__(kMatWarps * 32) k_materialise(const __grid_constant__ ExpandArgs A) {
+    __shared__ u32 s_units[kMatWarps];
+    __shared__ u64 s_base[kMatWarps];
+    __shared__ u64 s_slot[kMatWarps];
+    __shared__ u32 s_bytes[kMatWarps];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const u32 lt = (1u << lane) - 1u;
+    Ctl* ctl = A.ctl;
+    const u64 n_surv = ctl->n_surv;
+    for (u64 blk = blockIdx.x; blk * kMatWarps < n_surv; blk += gridDim.x) {   // block-uniform trip count
+    const u64 sidx = blk * kMatWarps + wib;
+    const bool live = sidx < n_surv;
+    // ---- the task
+    uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0, q2 = q0, q3 = q0;
+    if (live) {
+        const u32 slot = A.surv[sidx];
+        q0 = __ldcs(&A.t0[slot]); q1 = __ldcs(&A.t1[slot]); q2 = __ldcs(&A.t2[slot]); q3 = __ldcs(&A.t3[slot]);
+    }
+    const u64 p = q0.x;
+    const int ca = (int)(q0.y & 0xffffu);
+    const int cia = (q0.y >> 16) == 0xffffu ? -1 : (int)(q0.y >> 16);
+    const int cnu = (int)(q0.z & 0xffffu);
+    const u32 flags = q0.z >> 16;
+    const bool cin = (flags & TF_INSUPP) != 0, firstv = (flags & TF_FIRST) != 0;
+    const u64 ck = q0.w;
+    const u64 cd = (u64)q1.x | ((u64)q1.y << 32), cT = (u64)q1.z | ((u64)q1.w << 32);
+    const u64 cg = (u64)q2.x | ((u64)q2.y << 32), chs = (u64)q2.z | ((u64)q2.w << 32);
+    const u64 chv = (u64)q3.x | ((u64)q3.y << 32), newrec = (u64)q3.z | ((u64)q3.w << 32);
+    const u64 sd = (flags & TF_NEG) ? (u64)0 - cd : cd;
+    // ---- the parent
+    const unsigned char* pe = A.cur + ((live ? __ldg(&A.cur_off[p]) : 0ULL) << 4);
+    const uint4 h0 = live ? __ldg((const uint4*)pe) : make_uint4(0, 0, 0, 0);
+    const int ns = (int)(h0.x & 0xffffu), nv = (int)(h0.x >> 16), nu = (int)h0.y;
+    const i64* flux = (const i64*)(pe + kHdr);
+    const u64* vis = (const u64*)(flux + ns);
+    const i64* ef = (const i64*)(vis + nv);
+    const u16* arc = (const u16*)(ef + nu);
+    const u16* efmet = arc + ns;
+    const bool to_cand = cnu == 0;
+    const int n2 = ns + (cin ? 0 : 1);
+    const int nv2 = to_cand ? 0 : nv + (firstv ? 1 : 0);
+    const int nu2 = to_cand ? 0 : cnu;
+    const u32 units = live ? (to_cand ? 0u : entry_bytes((u32)n2, (u32)nv2, (u32)nu2) >> 4) : 0u;
+    // ---- reserve the output of the whole block: one atomic for the frontier entries, one for the candidates
+    if (lane == 0) {
+        s_units[wib] = units; s_slot[wib] = (live && to_cand) ? 1 : 0;
+        s_bytes[wib] = live ? algo_entry_bytes((u32)n2, (u32)(nv + (firstv ? 1 : 0))) : 0u;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        u64 tot_units = 0, n_front = 0, n_cand = 0, bytes = 0;
+        for (int w = 0; w < kMatWarps; ++w) { tot_units += s_units[w]; n_front += s_units[w] != 0; n_cand += s_slot[w]; bytes += s_bytes[w]; }
+        if (bytes) atomicAdd(&ctl->st[ST_ALGO_BYTES], bytes);
+        u64 fbase = 0, cbase = 0;
+        if (n_front) fbase = atomicAdd(&ctl->n_next, (n_front << kAllocShift) | tot_units);
+        if (n_cand) cbase = atomicAdd(&ctl->n_cand, n_cand);
+        u64 fs = fbase >> kAllocShift, fo = fbase & kAllocUnitMask;
+        for (int w = 0; w < kMatWarps; ++w) {
+            if (s_units[w]) { const u32 un = s_units[w]; s_base[w] = fo; s_slot[w] = fs++; fo += un; }
+            else if (s_slot[w]) { s_slot[w] = cbase++; }
+        }
+    }
+    __syncthreads();
+    bool ok = live;
+    unsigned char* dst = nullptr;
+    if (live && to_cand) {
+        const u64 slot = s_slot[wib];
+        if (slot >= A.max_cand) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_CAND); ok = false; }
+        dst = A.cand + slot * A.cand_stride;
+    } else if (live) {
+        const u64 slot = s_slot[wib], off = s_base[wib];
+        if (slot >= A.max_frontier || off + units > A.frontier_units) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_FRONTIER); ok = false; }
+        else if (lane == 0) A.nxt_off[slot] = off;
+        dst = A.nxt + (off << 4);
+    }
+    if (ok) {
+    // ---- write
+    int ins = 0;   // a new arc goes where the ascending order puts it
+    if (!cin)
+        for (int b2 = 0; b2 < ns; b2 += 32) {
+            const int t = b2 + lane;
+            ins += __popc(__ballot_sync(0xffffffffu, t < ns && (int)arc[t] < ca));
+        }
+    i64* flux2 = (i64*)(dst + kHdr);
+    u64* vis2 = (u64*)(flux2 + n2);
+    i64* ef2 = (i64*)(vis2 + nv2);
+    u16* arc2 = (u16*)(ef2 + nu2);
+    u16* efmet2 = arc2 + n2;
+    u64 mx = cin ? 0ULL : cT;   // a new arc never comes with a common divisor
+    for (int t = lane; t < ns; t += 32) {
+        u64 F = t == cia ? cT : ck * (u64)flux[t];
+        if (cg > 1) F /= cg;
+        const int pos = t + ((!cin && t >= ins) ? 1 : 0);
+        flux2[pos] = (i64)F;
+        arc2[pos] = arc[t];
+        mx = max(mx, F);
+    }
+    if (!cin && lane == 0) { flux2[ins] = (i64)cT; arc2[ins] = (u16)ca; }
+    if (!to_cand) {
+        // the visited record of i* is appended (first visit) or replaced (revisit)
+        const u32 met_star = (u32)((newrec >> 32) & 0xffffu);
+        for (int u = lane; u < nv; u += 32) {
+            const u64 r = vis[u];
+            vis2[u] = (!firstv && (u32)((r >> 32) & 0xffffu) == met_star) ? newrec : r;
+        }
+        if (firstv && lane == 0) vis2[nv] = newrec;
+        // EF list of the child: EF' = (k EF + sign d s_.a) / g over the parent's list, then the metabolites of col(a)
+        // that were balanced in the parent.  k_expand established that nothing exceeds 2^62, so the wrapping 64-bit
+        // arithmetic is exact.
+        const int qa0 = __ldg(&A.g.col_ptr[ca]), qa1 = __ldg(&A.g.col_ptr[ca + 1]);
+        int wbase = 0;
+        u32 seen = 0;   // bit q - qa0: metabolite of col(a)[q] is in the parent's list (columns longer than 32: see below)
+        for (int t0 = 0; t0 < nu; t0 += 32) {
+            const int t = t0 + lane;
+            const bool valid = t < nu;
+            i64 x = 0;
+            int met = -1;
+            if (valid) {
+                met = efmet[t];
+                i64 s = 0;
+                for (int qq = qa0; qq < qa1; ++qq) { const int2 e = __ldg(&A.g.col[qq]); if (e.x == met) s = e.y; }
+                x = (i64)(ck * (u64)ef[t] + sd * (u64)s);
+                if (cg > 1) x /= (i64)cg;
+            }
+            for (int qq = qa0; qq < qa1 && qq < qa0 + 32; ++qq)
+                if (__any_sync(0xffffffffu, valid && __ldg(&A.g.col[qq]).x == met)) seen |= 1u << (qq - qa0);
+            const u32 nz = __ballot_sync(0xffffffffu, valid && x != 0);
+            if (valid && x != 0) {
+                const int pos = wbase + __popc(nz & lt);
+                ef2[pos] = x; efmet2[pos] = (u16)met;
+                mx = max(mx, abs64(x));
+            }
+            wbase += __popc(nz);
+        }
+        for (int qq = qa0; qq < qa1; ++qq) {   // warp-uniform, a handful of entries
+            const int2 e = __ldg(&A.g.col[qq]);
+            bool in_parent;
+            if (qq < qa0 + 32) in_parent = (seen >> (qq - qa0)) & 1u;
+            else {   // columns longer than 32 entries: scan the parent's list again
+                bool f = false;
+                for (int t = lane; t < nu; t += 32) f = f || (int)efmet[t] == e.x;
+                in_parent = __any_sync(0xffffffffu, f);
+            }
+            if (!in_parent) {
+                i64 x = (i64)(sd * (u64)(i64)e.y);
+                if (cg > 1) x /= (i64)cg;
+                if (lane == 0) { ef2[wbase] = x; efmet2[wbase] = (u16)e.x; }
+                mx = max(mx, abs64(x));
+                ++wbase;
+            }
+        }
+        mx = w_max(mx);
+    }
+    if (lane == 0) {
+        uint4* h4 = (uint4*)dst;
+        h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2, (u32)chs, (u32)(chs >> 32));
+        h4[1] = make_uint4((u32)chv, (u32)(chv >> 32), (u32)mx, (u32)(mx >> 32));
+    }
+    }   // ok
+    __syncthreads();   // the reservation arrays are reused by the next round of the block
     }
 }
 
 __global__ void k_level_begin(Ctl* ctl) {
-    ctl->n_next = 0; ctl->n_keys = 0; ctl->n_slots = 0; ctl->lvl_done = 0; ctl->lvl_children = 0; ctl->lvl_expanded = 0;
+    ctl->n_next = 0; ctl->n_keys = 0; ctl->n_slots = 0; ctl->n_surv = 0; ctl->lvl_done = 0; ctl->lvl_children = 0; ctl->lvl_expanded = 0;
 }
 
 // ------------------------------------------------------------------ roots (INIT kernel of the paper)
@@ -760,23 +816,17 @@ void expand_smem_layout(ExpandArgs& a) {
 // every warp may strand one chunk of key slots; a warp covers kParentsPerWarp parents
 u64 expand_key_slack(u64 max_parents) { return (max_parents / kParentsPerWarp + 16384) * kKeyChunk; }
 
-template <int MODE>
-static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
+cudaError_t launch_expand(const ExpandArgs& a, int sm_count, cudaStream_t s) {
     // warps per block: as many as fit beside the per-warp staging (huge networks fall back to fewer warps)
     int warps = kWarps;
     while (warps > 1 && (size_t)a.sm_group * warps > 200 * 1024) warps >>= 1;
     const size_t smem = (size_t)a.sm_group * warps;
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    static int bps_cache[kWarps + 1] = {0};
-    static size_t smem_cache[kWarps + 1] = {0};
-    if (bps_cache[warps] == 0 || smem_cache[warps] != smem) {
-        cudaError_t e = cudaFuncSetAttribute(k_expand<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_expand, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
-        int bps = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_expand<MODE>, warps * 32, smem);
-        if (e != cudaSuccess) return e;
-        bps_cache[warps] = bps < 1 ? 1 : bps;
-        smem_cache[warps] = smem;
+        attr_done = true;
     }
     // small levels: fewer parents per warp so that every SM still gets its share of warps
     u64 ppw = a.n_cur / ((u64)sm_count * 32);
@@ -786,15 +836,22 @@ static cudaError_t launch_t(const ExpandArgs& a, int sm_count, cudaStream_t s) {
     const u64 per_block = (u64)warps * ppw;
     const u64 need = (a.n_cur + per_block - 1) / per_block;
     if (need > 0x7fffffffULL) return cudaErrorInvalidValue;
-    unsigned grid = (unsigned)(need ? need : 1);
-    k_expand<MODE><<<grid, warps * 32, smem, s>>>(a2);
+    k_expand<<<(unsigned)(need ? need : 1), warps * 32, smem, s>>>(a2);
     return cudaGetLastError();
 }
 
-cudaError_t launch_expand(int mode, const ExpandArgs& a, int sm_count, cudaStream_t s) {
-    if (mode == MODE_COUNT) return launch_t<MODE_COUNT>(a, sm_count, s);
-    if (mode == MODE_WRITE) return launch_t<MODE_WRITE>(a, sm_count, s);
-    return launch_t<MODE_DIRECT>(a, sm_count, s);
+// survivors of the level -> next frontier / candidates.  n_hint bounds the key slots in use (host side estimate).
+cudaError_t launch_materialise(const ExpandArgs& a, u64 n_slots_hint, u64 n_surv, int sm_count, cudaStream_t s, int phase) {
+    if (phase == 0) {   // compact
+        u64 blocks = (n_slots_hint + 2047) / 2048;
+        if (blocks > (u64)sm_count * 16) blocks = (u64)sm_count * 16;
+        if (blocks < 1) blocks = 1;
+        k_compact<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.surv, a.ctl, a.max_keys);
+        return cudaGetLastError();
+    }
+    (void)n_surv;   // read on the device (ctl->n_surv): no host round trip between the two kernels
+    k_materialise<<<(unsigned)(sm_count * 32), kMatWarps * 32, 0, s>>>(a);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_roots(bool write, const RootArgs& r, cudaStream_t s) {

@@ -7,7 +7,8 @@ namespace efm {
 // expand.cu
 void expand_smem_layout(ExpandArgs& a);
 u64 expand_key_slack(u64 max_parents);   // key slots the chunked reservation of the count pass can strand
-cudaError_t launch_expand(int mode /*0 count, 1 write, 2 direct*/, const ExpandArgs& a, int sm_count, cudaStream_t s);
+cudaError_t launch_expand(const ExpandArgs& a, int sm_count, cudaStream_t s);
+cudaError_t launch_materialise(const ExpandArgs& a, u64 n_slots_hint, u64 n_surv, int sm_count, cudaStream_t s, int phase /*0 compact, 1 write*/);
 cudaError_t launch_roots(bool write /*false: build + classify, true: keep the survivors*/, const RootArgs& r, cudaStream_t s);
 cudaError_t launch_level_begin(Ctl* ctl, cudaStream_t s);
 

@@ -61,7 +61,7 @@ __global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restri
         for (int j = 0; j < RUN; ++j) {
             if (i0 + j >= n) break;
             const u64 key = keys[i0 + j];
-            if (key == kKeySentinel) continue;   // filler of a reserved, unused slot
+            if (key >= kKeyDone) continue;   // filler of a reserved, unused slot / balanced child
             const u32 b = (u32)(key >> (64 - kTopBits));
             if (b != cur) { if (cnt) atomicAdd(&h[cur], cnt); cur = b; cnt = 0; }
             ++cnt;
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __rest
     for (u64 base = (u64)blockIdx.x * kSelThreads; base < n; base += span) {   // warp-uniform trip count
         const u64 i = base + threadIdx.x;
         const u64 key = i < n ? keys[i] : kKeySentinel;
-        const bool hit = key != kKeySentinel && (key >> (64 - kTopBits)) == top;
+        const bool hit = key < kKeyDone && (key >> (64 - kTopBits)) == top;
         const u32 m = __ballot_sync(0xffffffffu, hit);
         if (m) {
             u64 pos = 0;
