@@ -146,6 +146,24 @@ def main_reference(args):
     return 0
 
 
+def reduce_over_ranks(times_ms, counts, dist, device):
+    """Whole-job figures of a replica run: every time is the MAX over ranks, every count the SUM over ranks
+    (rank r works on its own independent problem).  `dist` is torch.distributed or None."""
+    import torch
+    if dist is None:
+        return list(times_ms) + list(counts)
+    t = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    c = torch.tensor(list(counts), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return t.tolist() + c.tolist()
+
+
+def rank_problem(workload: str, rank: int, cap: int):
+    """The independent problem rank `rank` owns: the synthetic network of generator seed `rank`."""
+    return _workload(workload, rank, cap)
+
+
 def main_ours(args):
     import numpy as np
     import torch
@@ -167,7 +185,7 @@ def main_ours(args):
     import paper_1804_02867_b200 as efm
 
     # rank r owns the independent problem of generator seed r (weak scaling, no collective on the data path)
-    net, params = _workload(args.workload, rank, args.cap)
+    net, params = rank_problem(args.workload, rank, args.cap)
     params["max_candidates"] = args.max_candidates
     en = efm.Enumerator(net.S, net.reversible, net.internal, params, device=local, flags=efm.EFM_F_TIMING)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
@@ -214,26 +232,17 @@ def main_ours(args):
         en2.close()
     barrier()
 
-    expanded = acc["expanded"]
-    vals = torch.tensor([ms, e2e_s * 1000.0, float(expanded), float(acc["output"]), float(acc["children"])],
-                        dtype=torch.float64, device="cuda")
-    if world > 1:
-        mx = vals.clone()
-        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = vals.clone()
-        dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        ms_max, e2e_ms_max = mx[0].item(), mx[1].item()
-        expanded_all, outputs_all, children_all = sm[2].item(), sm[3].item(), sm[4].item()
-    else:
-        ms_max, e2e_ms_max = ms, e2e_s * 1000.0
-        expanded_all, outputs_all, children_all = float(expanded), float(acc["output"]), float(acc["children"])
+    ms_max, e2e_ms_max, expanded_all, outputs_all, children_all = reduce_over_ranks(
+        [ms, e2e_s * 1000.0], [float(acc["expanded"]), float(acc["output"]), float(acc["children"])],
+        dist if world > 1 else None, torch.device("cuda", local))
 
     if rank == 0:
         peak, peak_src = _peaks()
-        n_exp_launch = acc["n_expand_count"] + acc["n_expand_write"] + acc["n_direct"]
-        ms_expand = acc["ms_expand_count"] + acc["ms_expand_write"] + acc["ms_direct"]
+        # one "launch" of the expansion = k_expand (evaluate) + k_compact + k_materialise of one level
+        n_exp_launch = acc["n_expand_count"]
+        ms_expand = acc["ms_expand_count"] + acc["ms_expand_write"]
         achieved = acc["algo_bytes"] / (ms_expand * 1e-3) / 1e9 if ms_expand > 0 else 0.0
-        roofline = {"bound": "hbm", "kernel": "k_expand (count + write + direct launches)", "achieved": achieved,
+        roofline = {"bound": "hbm", "kernel": "expansion of one level: k_expand (evaluate) + k_compact + k_materialise", "achieved": achieved,
                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": args.traffic,
                     "peak_source": peak_src, "launches_per_step": n_exp_launch / args.steps,
                     "avg_launch_ms": ms_expand / max(1, n_exp_launch),
@@ -265,11 +274,14 @@ def main_ours(args):
                 "extra": {"efms_per_s": outputs_all / (ms_max * 1e-3), "children_per_s": children_all / (ms_max * 1e-3),
                           "outputs_per_step": outputs_all / args.steps / world, "levels": acc["levels"] / args.steps,
                           "phase_ms_per_step": {k: acc[k] / args.steps for k in
-                                                ("ms_expand_count", "ms_beam", "ms_expand_write", "ms_direct", "ms_hash",
+                                                ("ms_expand_count", "ms_beam", "ms_expand_write", "ms_hash",
                                                  "ms_filter", "ms_output")},
+                          "phase_names": {"ms_expand_count": "k_expand", "ms_beam": "k_select_*", "ms_expand_write":
+                                          "k_compact + k_materialise", "ms_hash": "k_dedup_*", "ms_filter": "k_filter_*",
+                                          "ms_output": "k_out_* + k_bitonic_*"},
                           "work_profile_per_step": {k: acc[k] / args.steps for k in
                                                     ("expanded", "alt_rounds", "first_visits", "general_children",
-                                                     "saturated_parents", "write_pass_parents")},
+                                                     "saturated_parents")},
                           "filter_pairs_per_s": (acc["filter_pairs"] / (acc["ms_filter"] * 1e-3)) if acc["ms_filter"] else None}}
         print(json.dumps(line))
     en.close()

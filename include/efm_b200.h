@@ -39,7 +39,7 @@ extern "C" {
 
 /* flags */
 #define EFM_F_TIMING 0x1u       /* record CUDA events around every kernel phase (efm_stats.ms_*)   */
-#define EFM_F_FORCE_TWO_PASS 0x2u /* always run count+select+write, even when the beam cannot bind */
+#define EFM_F_FORCE_TWO_PASS 0x2u /* always run the threshold selection, even when the beam cannot bind */
 #define EFM_F_NO_FASTPATH 0x4u  /* evaluate every child with the warp-cooperative general routine  */
 
 typedef struct efm_handle efm_handle; /* opaque: host copy of the graph + pointers INTO the workspace */
@@ -71,16 +71,18 @@ typedef struct {
     int64_t algo_bytes;     /* algorithmic bytes of all expansions            */
     int64_t n_roots;
     int64_t launches;       /* kernels launched by the last efm_enumerate()                          */
-    int64_t two_pass_levels, direct_levels;
+    int64_t two_pass_levels, direct_levels; /* levels on which the beam threshold was / was not computed      */
     /* milliseconds; ms_total is always measured (CUDA events on the caller's stream), the per-phase
      * figures only with EFM_F_TIMING */
     double ms_build, ms_total, ms_expand_count, ms_beam, ms_expand_write, ms_direct, ms_hash,
         ms_filter, ms_output;
-    int64_t n_expand_count, n_expand_write, n_direct; /* launches behind the three expand timers     */
+    /* ms_expand_count: k_expand (evaluates every child: beam key + task); ms_beam: threshold selection;
+     * ms_expand_write: k_compact + k_materialise (survivors -> next frontier / candidates); ms_direct: unused (0) */
+    int64_t n_expand_count, n_expand_write, n_direct; /* launches behind the expand timers (n_direct: 0)     */
     int64_t filter_pairs;   /* signature pair tests done by the minimality filter                    */
-    /* work profile of the expand kernels: rounds of 32 OR-alternatives, first-visit parents, children through
-     * the general routine, parents whose support is at the cap D, parents the write pass re-expanded        */
-    int64_t alt_rounds, first_visits, general_children, saturated_parents, write_pass_parents;
+    /* work profile of the expansion: rounds of 32 OR-alternatives, first-visit parents, children through the
+     * general routine, parents whose support is at the cap D, children materialised (survivors + balanced) */
+    int64_t alt_rounds, first_visits, general_children, saturated_parents, materialised;
 } efm_stats;
 
 /* Build the modified AND/OR graph MG (Defs 4-6; "Convert the given matrix to the MG

@@ -36,7 +36,7 @@ _STAT_INT = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxl
 _STAT_MS = ["ms_build", "ms_total", "ms_expand_count", "ms_beam", "ms_expand_write", "ms_direct", "ms_hash",
             "ms_filter", "ms_output"]
 _STAT_INT2 = ["n_expand_count", "n_expand_write", "n_direct", "filter_pairs", "alt_rounds", "first_visits",
-              "general_children", "saturated_parents", "write_pass_parents"]
+              "general_children", "saturated_parents", "materialised"]
 
 
 class efm_stats(ctypes.Structure):

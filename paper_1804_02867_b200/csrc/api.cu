@@ -407,7 +407,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     st.ms_build = h->ms_build;
     st.n_roots = (int64_t)n_roots;
     h->lvl_active.clear(); h->lvl_done.clear(); h->lvl_expanded.clear(); h->lvl_children.clear();
-    int64_t truncated = 0, done_total = 0;
+    int64_t truncated = 0, done_total = 0, materialised = 0;
 
     // ---- level 0: classify the roots, beam-select, keep the survivors
     int cur = 0;
@@ -465,6 +465,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         if (beam_possible) st.two_pass_levels++; else st.direct_levels++;
         CK(read_ctl());
         if (hc->error) return EFM_E_CAPACITY;
+        materialised += (int64_t)hc->n_surv;
         h->lvl_expanded[lvl] = (int64_t)hc->lvl_expanded;
         h->lvl_children[lvl] = (int64_t)hc->lvl_children;
         const int64_t n_next = (int64_t)(hc->n_next >> kAllocShift);
@@ -539,7 +540,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     st.algo_bytes = (int64_t)hc->st[ST_ALGO_BYTES];
     st.alt_rounds = (int64_t)hc->st[ST_ROUNDS]; st.first_visits = (int64_t)hc->st[ST_FIRST];
     st.general_children = (int64_t)hc->st[ST_GENERAL]; st.saturated_parents = (int64_t)hc->st[ST_SATURATED];
-    st.write_pass_parents = (int64_t)hc->st[ST_WRITE_PARENTS];
+    st.materialised = materialised;
     st.peak_frontier = 0;
     for (int64_t a : h->lvl_active) st.peak_frontier = std::max(st.peak_frontier, a);
     st.launches = launches;

@@ -53,8 +53,8 @@ struct DevGraph {
 enum { ST_EXPANDED = 0, ST_CHILDREN, ST_DONE, ST_DEAD_END, ST_NOT_EFM, ST_NONPOS, ST_OVERFLOW, ST_VISITED,
        ST_ALGO_BYTES,
        // work profile of the expand kernels (not part of the oracle parity): alternative rounds of 32 lanes, first-visit
-       // parents, children through the general routine, parents at the support cap D, parents the write pass re-expanded
-       ST_ROUNDS, ST_FIRST, ST_GENERAL, ST_SATURATED, ST_WRITE_PARENTS, ST_COUNT };
+       // parents, children through the general routine, parents at the support cap D
+       ST_ROUNDS, ST_FIRST, ST_GENERAL, ST_SATURATED, ST_COUNT };
 enum { ERR_FRONTIER = 1, ERR_CAND = 2, ERR_KEYS = 4 };
 enum { SEL_BINS = 2048 };
 

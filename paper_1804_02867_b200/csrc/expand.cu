@@ -144,7 +144,7 @@ __device__ __forceinline__ bool sbit(const u32* bits, int a) { return (bits[a >>
 
 // per-warp statistics live in shared memory (one u64 each), flushed to the control block once per warp
 enum { SS_EXPANDED = 0, SS_CHILDREN, SS_DONE, SS_ACTIVE, SS_DEAD, SS_NOTEFM, SS_NONPOS, SS_OVF, SS_VISITED, SS_BYTES,
-       SS_ROUNDS, SS_FIRST, SS_GENERAL, SS_SATURATED, SS_WRITE_PARENTS,
+       SS_ROUNDS, SS_FIRST, SS_GENERAL, SS_SATURATED,
        SS_KC,   // 4 words: the hash sums of the k-scaled support for the last two scales k (k0, s0, k1, s1)
        SS_WORDS = SS_KC + 4 };
 

@@ -201,3 +201,57 @@ def test_sparse_and_dense_results_agree(efm):
     again = en.enumerate()   # the handle and the workspace are reusable
     assert np.array_equal(again.flux, res.flux)
     en.close()
+
+
+def test_bench_configuration_properties(efm):
+    """The configuration bench.py times (genome seed 0, frontier_cap 65536) is too large for the oracle (about
+    2 ms per unit of cap), so it is held by what is true at any size: Def 2 on every output, canonical form,
+    support-minimality and lexicographic order on samples, counter identities, and run-to-run determinism (the
+    kernels allocate with atomics, the result must not depend on their order)."""
+    import scipy.sparse as sp
+    net = make_network("genome", 0)
+    params = dict(net.params, frontier_cap=65536, max_candidates=1 << 20)
+    en = efm.Enumerator(net.S, net.reversible, net.internal, params)
+    res = en.enumerate(net.seed_sets, dense=False)
+    nnz, rxn, val = en.result_sparse()
+    st, lv = res.stats, res.levels
+    K, n = res.n_out, net.S.shape[1]
+    assert K == int(st["output"]) > 100000 and st["truncated_beam"] > 0
+    mask = np.arange(rxn.shape[1])[None, :] < nnz[:, None]
+    rows = np.repeat(np.arange(K), nnz)
+    V = sp.csr_matrix((val[mask], (rows, rxn[mask])), shape=(K, n), dtype=np.int64)
+    # Def 2 (PAPER.md:49-52): S_int . v = 0, v >= 0 on irreversible reactions; gcd 1 (reading G10)
+    Sint = sp.csr_matrix(net.S[net.internal.astype(bool)].astype(np.int64))
+    assert (Sint @ V.T).count_nonzero() == 0
+    assert np.all(val[mask][~net.reversible.astype(bool)[rxn[mask]]] > 0)
+    assert np.all(val[mask] != 0) and np.all(np.diff(np.where(mask, rxn, n + np.arange(rxn.shape[1])[None, :]), axis=1) > 0)
+    assert np.all(np.gcd.reduce(np.where(mask, np.abs(val), 0), axis=1) == 1)
+    # strict lexicographic order on sampled neighbours
+    rng = np.random.default_rng(0)
+    for r in rng.choice(K - 1, 3000, replace=False):
+        a, b = V[r].toarray()[0], V[r + 1].toarray()[0]
+        d = np.nonzero(a != b)[0]
+        assert d.size and a[d[0]] < b[d[0]], r
+    # Def 3 (PAPER.md:57) on sampled outputs: no other output support strictly inside (arc space: sign matters)
+    arcs = np.where(val[mask] > 0, rxn[mask], rxn[mask] + n)
+    B = sp.csr_matrix((np.ones(arcs.size, np.int32), (rows, arcs)), shape=(K, 2 * n))
+    size = np.asarray(B.sum(axis=1)).ravel()
+    for r in rng.choice(K, 400, replace=False):
+        shared = np.asarray((B @ B[r].T).todense()).ravel()
+        inside = (shared == size) & (size < size[r])
+        assert not inside.any(), (r, int(np.nonzero(inside)[0][0]))
+    # counters
+    assert int(st["expanded"]) == int(lv["expanded"].sum()) and int(st["children"]) == int(lv["children"].sum())
+    assert int(st["done"]) == int(lv["done"].sum()) >= int(st["unique_supports"])
+    assert int(st["unique_supports"]) - int(st["poisoned"]) >= K
+    assert int(st["peak_frontier"]) == int(lv["active"].max()) and int(st["levels"]) == len(lv["active"])
+    assert np.all(lv["expanded"] <= 65536) and int(lv["expanded"].max()) > 60000
+    assert int(st["truncated_beam"]) == int(lv["active"].sum() - lv["expanded"].sum())
+    # determinism
+    again = en.enumerate(net.seed_sets, dense=False)
+    nnz2, rxn2, val2 = en.result_sparse()
+    assert again.n_out == K and np.array_equal(nnz, nnz2)
+    assert np.array_equal(np.where(mask, rxn, 0), np.where(mask, rxn2, 0)) and np.array_equal(np.where(mask, val, 0), np.where(mask, val2, 0))
+    for k in STAT_KEYS:
+        assert int(again.stats[k]) == int(st[k]), k
+    en.close()
