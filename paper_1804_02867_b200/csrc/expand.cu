@@ -21,7 +21,7 @@ namespace efm {
 
 enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
 #ifndef EFM_MIN_BLOCKS
-#define EFM_MIN_BLOCKS 16   // resident one-warp blocks per SM the register allocation aims at (128 registers)
+#define EFM_MIN_BLOCKS 24   // resident one-warp blocks per SM the register allocation aims at (80 registers)
 #endif
 constexpr int kBlock = 32;    // one warp per block: a finished warp frees its slot at once (parents differ a lot in cost)
 constexpr int kWarps = kBlock / 32;
@@ -807,8 +807,6 @@ void expand_smem_layout(ExpandArgs& a) {
     a.sm_sbits = (u32)off; off = align16(off + (size_t)a.g.W32 * 4);
     a.sm_upos = (u32)off;  off = align16(off + (size_t)a.g.M * 2 + 16);   // zeroed in 16-byte chunks
     a.sm_misc = (u32)off;  off = align16(off + (size_t)SS_WORDS * 8);
-    a.sm_out_bytes = a.max_entry < 2048u ? a.max_entry : 2048u;   // child assembly buffer (larger children: in place)
-    a.sm_out = (u32)off;   off = align16(off + a.sm_out_bytes);
     a.sm_group = (u32)off;
 }
 
