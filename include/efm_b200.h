@@ -41,6 +41,8 @@ extern "C" {
 #define EFM_F_TIMING 0x1u       /* record CUDA events around every kernel phase (efm_stats.ms_*)   */
 #define EFM_F_FORCE_TWO_PASS 0x2u /* always run the threshold selection, even when the beam cannot bind */
 #define EFM_F_NO_FASTPATH 0x4u  /* evaluate every child with the warp-cooperative general routine  */
+#define EFM_F_NO_STAGING 0x8u   /* read every parent in place (the route of entries larger than the   */
+                                /* shared-memory staging buffer)                                      */
 
 typedef struct efm_handle efm_handle; /* opaque: host copy of the graph + pointers INTO the workspace */
 

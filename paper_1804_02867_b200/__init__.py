@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libefm_b200.so")
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "efm_b200.h")
 
 EFM_OK, EFM_E_INVAL, EFM_E_NOMEM, EFM_E_CAPACITY, EFM_E_CUDA, EFM_E_STATE = 0, -1, -2, -3, -4, -5
-EFM_F_TIMING, EFM_F_FORCE_TWO_PASS, EFM_F_NO_FASTPATH = 0x1, 0x2, 0x4
+EFM_F_TIMING, EFM_F_FORCE_TWO_PASS, EFM_F_NO_FASTPATH, EFM_F_NO_STAGING = 0x1, 0x2, 0x4, 0x8
 
 
 class efm_params(ctypes.Structure):

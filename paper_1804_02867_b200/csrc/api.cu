@@ -395,6 +395,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.D = h->D; ea.V = h->V; ea.max_loop = h->max_loop;
     ea.no_fast = (h->flags & EFM_F_NO_FASTPATH) ? 1 : 0;
     expand_smem_layout(ea);
+    if (h->flags & EFM_F_NO_STAGING) ea.sm_stage_bytes = 0;
 
     auto read_ctl = [&]() -> cudaError_t {
         cudaError_t e = cudaMemcpyAsync(hc, d_ctl, ctl_read, cudaMemcpyDeviceToHost, s);

@@ -99,7 +99,7 @@ struct ExpandArgs {
     u32 ppw;                    // consecutive parents a warp owns (set by the launcher)
     int no_fast;                // EFM_F_NO_FASTPATH: every child through the warp-cooperative general routine
     // shared-memory carve-up per warp (bytes)
-    u32 sm_group, sm_sbits, sm_upos, sm_misc;
+    u32 sm_group, sm_stage_bytes, sm_sbits, sm_upos, sm_misc;
 };
 
 // roots (INIT): seed sets uploaded by the host, entries built and classified on the device

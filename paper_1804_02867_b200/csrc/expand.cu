@@ -186,12 +186,19 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         const int ns = (int)(hdr & 0xffffu), nv = (int)(hdr >> 16);
         const int nu = (int)__shfl_sync(FULL, first16.y, 0);
         const u32 nch = entry_bytes((u32)ns, (u32)nv, (u32)nu) / 16;
-        if ((u32)lane < nch) stage[lane] = first16;
-        #pragma unroll 1
-        for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldcs(src + c);   // streaming: the frontier must not evict the graph from L1
+        // entries that fit the staging buffer are copied to shared memory; the rare larger ones are read in place
+        const bool staged = nch * 16 <= A.sm_stage_bytes;
+        if (staged) {
+            if ((u32)lane < nch) stage[lane] = first16;
+            #pragma unroll 1
+            for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldcs(src + c);   // streaming: the frontier must not evict the graph from L1
+        }
         __syncwarp();
-        const u64 Phs = ((const u64*)stage)[1], Phv = ((const u64*)stage)[2], Pbig = ((const u64*)stage)[3];
-        const i64* flux = (const i64*)(gs + kHdr);
+        const u64 Phs = (u64)__shfl_sync(FULL, first16.z, 0) | ((u64)__shfl_sync(FULL, first16.w, 0) << 32);
+        const u64 Phv = (u64)__shfl_sync(FULL, first16.x, 1) | ((u64)__shfl_sync(FULL, first16.y, 1) << 32);
+        const u64 Pbig = (u64)__shfl_sync(FULL, first16.z, 1) | ((u64)__shfl_sync(FULL, first16.w, 1) << 32);
+        const unsigned char* eb = staged ? (const unsigned char*)gs : (const unsigned char*)src;
+        const i64* flux = (const i64*)(eb + kHdr);
         const u64* vis = (const u64*)(flux + ns);
         const i64* ef = (const i64*)(vis + nv);
         const u16* arc = (const u16*)(ef + nu);
@@ -803,7 +810,10 @@ __global__ void __launch_bounds__(128) k_roots(const RootArgs R) {
 static size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 
 void expand_smem_layout(ExpandArgs& a) {
-    size_t off = align16(a.max_entry);   // staging holds the largest entry
+    // staging: the largest entry if it is small, otherwise 1.5 KB (larger entries are rare and read in place);
+    // the smaller the per-warp footprint, the more of the graph stays in L1
+    a.sm_stage_bytes = a.max_entry < 1536u ? a.max_entry : 1536u;
+    size_t off = align16(a.sm_stage_bytes);
     a.sm_sbits = (u32)off; off = align16(off + (size_t)a.g.W32 * 4);
     a.sm_upos = (u32)off;  off = align16(off + (size_t)a.g.M * 2 + 16);   // zeroed in 16-byte chunks
     a.sm_misc = (u32)off;  off = align16(off + (size_t)SS_WORDS * 8);

@@ -136,6 +136,13 @@ def test_general_routine_only(efm, oracle_mod):
                   frontier_cap=1 << 20)
 
 
+def test_parents_read_in_place(efm, oracle_mod):
+    """EFM_F_NO_STAGING: every parent takes the route of entries larger than the staging buffer (read from HBM in
+    place instead of from shared memory)."""
+    for name, over in (("small", {}), ("core", dict(frontier_cap=2048)), ("genome", dict(frontier_cap=256))):
+        assert_parity(efm, oracle_mod, make_network(name, 0), flags=efm.EFM_F_NO_STAGING, **over)
+
+
 def test_other_seeds_of_the_generator(efm, oracle_mod):
     for name, seed, over in (("small", 1, {}), ("small", 2, dict(frontier_cap=500)), ("core", 1, dict(frontier_cap=4096)),
                              ("mid", 3, dict(frontier_cap=1024))):
