@@ -89,7 +89,7 @@ void make_layout(efm_handle* h) {
     add_region(L, L.keys, (size_t)h->max_keys * 8);
     add_region(L, L.ckeys, (size_t)h->max_keys * 8);
     for (int t = 0; t < 4; ++t) add_region(L, L.task[t], (size_t)h->max_keys * 16);
-    add_region(L, L.surv, (size_t)h->max_keys * 4);
+    add_region(L, L.surv, (size_t)h->max_keys * 16);
     const size_t C = (size_t)h->max_cand;
     add_region(L, L.cand, C * h->cand_stride);
     add_region(L, L.table, h->table_size * 4);
@@ -388,7 +388,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.ctl = d_ctl;
     ea.t0 = (uint4*)(ws + L.task[0].off); ea.t1 = (uint4*)(ws + L.task[1].off);
     ea.t2 = (uint4*)(ws + L.task[2].off); ea.t3 = (uint4*)(ws + L.task[3].off);
-    ea.surv = (u32*)(ws + L.surv.off);
+    ea.surv = (ulonglong2*)(ws + L.surv.off);
     ea.max_entry = h->max_entry; ea.cand_stride = h->cand_stride;
     ea.frontier_units = (u64)h->frontier_bytes >> 4;
     ea.max_frontier = (u64)h->max_frontier; ea.max_cand = (u64)h->max_cand; ea.max_keys = (u64)h->max_keys;

@@ -90,7 +90,7 @@ struct ExpandArgs {
     unsigned char* cand;        // balanced children (fixed stride)
     u64* keys;                  // per child slot: beam key (kKeyDone: balanced child; kKeySentinel: unused slot)
     uint4* t0; uint4* t1; uint4* t2; uint4* t3;   // per child slot: the task (see k_expand / k_materialise)
-    u32* surv;                  // slots of the children that are materialised
+    ulonglong2* surv;           // children that are materialised: {slot, offset of the parent entry in 16-byte units}
     Ctl* ctl;
     u64 n_cur;
     u32 max_entry, cand_stride; // largest entry in bytes (shared-memory staging), candidate slot stride

@@ -23,7 +23,10 @@ enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
 #ifndef EFM_MIN_BLOCKS
 #define EFM_MIN_BLOCKS 24   // resident one-warp blocks per SM the register allocation aims at (80 registers)
 #endif
-constexpr int kBlock = 32;    // one warp per block: a finished warp frees its slot at once (parents differ a lot in cost)
+#ifndef EFM_KBLOCK
+#define EFM_KBLOCK 32
+#endif
+constexpr int kBlock = EFM_KBLOCK;    // one warp per block: a finished warp frees its slot at once (parents differ a lot in cost)
 constexpr int kWarps = kBlock / 32;
 #ifndef EFM_PPW
 #define EFM_PPW 8
@@ -545,7 +548,8 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
 // ------------------------------------------------------------------ survivors of the beam -> list of slots
 // One thread per key slot: balanced children (kKeyDone) and active children with key < X (all of them when the beam
 // does not bind).  Warp-aggregated append; the order of the list does not matter.
-__global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, u32* __restrict__ surv, Ctl* ctl, u64 max_keys) {
+__global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, const uint4* __restrict__ t0, const u64* __restrict__ cur_off,
+                                                 ulonglong2* __restrict__ surv, Ctl* ctl, u64 max_keys) {
     const u64 n = min(ctl->n_slots, max_keys);
     const bool notrunc = ctl->notrunc != 0;
     const u64 X = ctl->X;
@@ -559,7 +563,8 @@ __global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, u
             u64 pos = 0;
             if (lane == 0) pos = atomicAdd(&ctl->n_surv, (u64)__popc(m));
             pos = __shfl_sync(0xffffffffu, pos, 0);
-            if (take) surv[pos + __popc(m & ((1u << lane) - 1u))] = (u32)i;
+            // the survivor record carries the offset of its parent: one dependent load less in k_materialise
+            if (take) surv[pos + __popc(m & ((1u << lane) - 1u))] = make_ulonglong2(i, __ldg(&cur_off[__ldcs(&t0[i]).x]));
         }
     }
 }
@@ -569,7 +574,7 @@ __global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, u
 // a candidate slot if it is balanced, otherwise a packed entry of the next frontier.  A block of kMatWarps children
 // reserves its output with one atomic per kind.
 constexpr int kMatWarps = 8;
-__global__ void __launch_bounds__(kMatWarps * 32) k_materialise(const __grid_constant__ ExpandArgs A) {
+__global__ void __launch_bounds__(kMatWarps * 32, 4) k_materialise(const __grid_constant__ ExpandArgs A) {
     __shared__ u32 s_units[kMatWarps];
     __shared__ u64 s_base[kMatWarps];
     __shared__ u64 s_slot[kMatWarps];
@@ -582,12 +587,15 @@ __global__ void __launch_bounds__(kMatWarps * 32) k_materialise(const __grid_con
     const u64 sidx = blk * kMatWarps + wib;
     const bool live = sidx < n_surv;
     // ---- the task
-    uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0, q2 = q0, q3 = q0;
+    uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0, q2 = q0, q3 = q0, h0 = q0;
+    const unsigned char* pe = A.cur;
     if (live) {
-        const u32 slot = A.surv[sidx];
+        const ulonglong2 sv = __ldcs(&A.surv[sidx]);
+        const u64 slot = sv.x;
+        pe = A.cur + (sv.y << 4);
         q0 = __ldcs(&A.t0[slot]); q1 = __ldcs(&A.t1[slot]); q2 = __ldcs(&A.t2[slot]); q3 = __ldcs(&A.t3[slot]);
+        h0 = __ldg((const uint4*)pe);
     }
-    const u64 p = q0.x;
     const int ca = (int)(q0.y & 0xffffu);
     const int cia = (q0.y >> 16) == 0xffffu ? -1 : (int)(q0.y >> 16);
     const int cnu = (int)(q0.z & 0xffffu);
@@ -599,8 +607,6 @@ __global__ void __launch_bounds__(kMatWarps * 32) k_materialise(const __grid_con
     const u64 chv = (u64)q3.x | ((u64)q3.y << 32), newrec = (u64)q3.z | ((u64)q3.w << 32);
     const u64 sd = (flags & TF_NEG) ? (u64)0 - cd : cd;
     // ---- the parent
-    const unsigned char* pe = A.cur + ((live ? __ldg(&A.cur_off[p]) : 0ULL) << 4);
-    const uint4 h0 = live ? __ldg((const uint4*)pe) : make_uint4(0, 0, 0, 0);
     const int ns = (int)(h0.x & 0xffffu), nv = (int)(h0.x >> 16), nu = (int)h0.y;
     const i64* flux = (const i64*)(pe + kHdr);
     const u64* vis = (const u64*)(flux + ns);
@@ -854,7 +860,7 @@ cudaError_t launch_materialise(const ExpandArgs& a, u64 n_slots_hint, u64 n_surv
         u64 blocks = (n_slots_hint + 2047) / 2048;
         if (blocks > (u64)sm_count * 16) blocks = (u64)sm_count * 16;
         if (blocks < 1) blocks = 1;
-        k_compact<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.surv, a.ctl, a.max_keys);
+        k_compact<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.t0, a.cur_off, a.surv, a.ctl, a.max_keys);
         return cudaGetLastError();
     }
     (void)n_surv;   // read on the device (ctl->n_surv): no host round trip between the two kernels
