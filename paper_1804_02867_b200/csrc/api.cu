@@ -494,8 +494,8 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     pa.isrep = ws + L.isrep.off; pa.poison = ws + L.poison.off; pa.uniq = (u32*)(ws + L.uniq.off);
     pa.freq = (u32*)(ws + L.freq.off); pa.gcount = (u32*)(ws + L.gcount.off);
     pa.gstart = (u32*)(ws + L.gstart.off); pa.gfill = (u32*)(ws + L.gfill.off);
-    pa.g_row = (u32*)(ws + L.g_row.off); pa.g_sig = (ulonglong2*)(ws + L.g_sig.off);
-    pa.g_size = (u16*)(ws + L.g_size.off); pa.keep = ws + L.keep.off;
+    pa.g_row = (u32*)(ws + L.g_row.off); pa.g_sig = (uint4*)(ws + L.g_sig.off);
+    pa.keep = ws + L.keep.off;
     pa.D = h->D; pa.n_rxn = G.n;
     pa.u_nnz = (int*)(ws + L.u_nnz.off); pa.u_rxn = (int*)(ws + L.u_rxn.off); pa.u_val = (i64*)(ws + L.u_val.off);
     pa.sort_idx = (u32*)(ws + L.sort_idx.off);

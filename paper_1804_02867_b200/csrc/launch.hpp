@@ -22,7 +22,7 @@ struct PostArgs {
     u32* uniq;                         // candidate ids of the unique, unpoisoned supports
     // minimality filter (a-7)
     u32* freq; u32* gcount; u32* gstart; u32* gfill;      // per arc: candidates using it, group size / start / fill
-    u32* g_row; ulonglong2* g_sig; u16* g_size;           // rows grouped by their rarest arc: candidate id, signature, |supp|
+    u32* g_row; uint4* g_sig;                             // rows grouped by their rarest arc: candidate id, 112-bit signature + |supp|
     unsigned char* keep;                                  // per unique support (uniq order)
     // canonical output (a-8)
     int D; int n_rxn;

@@ -216,15 +216,33 @@ cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_l
 // is the 128-bit signature test (exact bitsets when A <= 128, a 128-bucket image of the arc set otherwise; coalesced
 // 16-byte loads, one lane per w), signature hits are verified on the sorted arc lists.
 // =================================================================================================================
-__device__ __forceinline__ u32 sig_bit(int arc, bool exact) { return exact ? (u32)arc : ((u32)arc * 0x9E3779B1u) >> 25; }
+// 112-bit signature of a support (exact bitset when A <= 112, otherwise arc -> one of 112 buckets); the remaining 16
+// bits of the 128-bit record hold |supp| so that one 16-byte load serves the whole pair test
+constexpr int kSigBits = 112;
+__device__ __forceinline__ u32 sig_bit(int arc, bool exact) { return exact ? (u32)arc : (((u32)arc * 0x9E3779B1u) >> 16) % (u32)kSigBits; }
+__device__ __forceinline__ uint4 sig_of(const u16* arc, int n, bool exact) {   // whole signature by one thread
+    u32 w[4] = {0, 0, 0, 0};
+    for (int t = 0; t < n; ++t) { const u32 b = sig_bit(arc[t], exact); w[b >> 5] |= 1u << (b & 31); }
+    return make_uint4(w[0], w[1], w[2], w[3] | ((u32)n << 16));
+}
 
-__global__ void __launch_bounds__(256) k_filter_freq(const PostArgs a, u64 K) {   // how many candidates use each arc
-    const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (u >= K) return;
-    const unsigned char* e = a.cand + (u64)a.uniq[u] * a.cand_stride;
-    const int n = cand_n(e);
-    const u16* arc = cand_arc(e, n);
-    for (int t = 0; t < n; ++t) atomicAdd(&a.freq[arc[t]], 1u);
+__global__ void __launch_bounds__(256) k_filter_freq(const PostArgs a, u64 K, int use_smem) {
+    // per-block histogram in shared memory when the arcs fit (popular arcs would otherwise serialise in L2)
+    extern __shared__ u32 hist[];
+    if (use_smem) {
+        for (int i = threadIdx.x; i < a.g.A; i += blockDim.x) hist[i] = 0;
+        __syncthreads();
+    }
+    for (u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x; u < K; u += (u64)gridDim.x * blockDim.x) {
+        const unsigned char* e = a.cand + (u64)a.uniq[u] * a.cand_stride;
+        const int n = cand_n(e);
+        const u16* arc = cand_arc(e, n);
+        for (int t = 0; t < n; ++t) atomicAdd(use_smem ? &hist[arc[t]] : &a.freq[arc[t]], 1u);
+    }
+    if (use_smem) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < a.g.A; i += blockDim.x) if (hist[i]) atomicAdd(&a.freq[i], hist[i]);
+    }
 }
 __device__ __forceinline__ int rarest_arc(const PostArgs& a, const u16* arc, int n) {   // ties: lowest arc id
     u32 best = 0xffffffffu; int key = 0;
@@ -265,16 +283,9 @@ __global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K)
     const int n = cand_n(e);
     if (n == 0) return;
     const u16* arc = cand_arc(e, n);
-    const bool exact = a.g.A <= 128;
-    u64 lo = 0, hi = 0;
-    for (int t = 0; t < n; ++t) {
-        const u32 b = sig_bit(arc[t], exact);
-        if (b < 64) lo |= 1ULL << b; else hi |= 1ULL << (b - 64);
-    }
     const u32 pos = atomicAdd(&a.gfill[rarest_arc(a, arc, n)], 1u);
     a.g_row[pos] = id;
-    a.g_sig[pos] = make_ulonglong2(lo, hi);
-    a.g_size[pos] = (u16)n;
+    a.g_sig[pos] = sig_of(arc, n, a.g.A <= kSigBits);
 }
 __device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   // supp(w) subset of supp(v), sorted lists
     const int nw = cand_n(w), nv = cand_n(v);
@@ -289,7 +300,7 @@ __device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   
     return true;
 }
 constexpr int kFilterWarps = 8;
-// one warp per row v; lanes walk the group of every arc of v
+// one warp per row v; lanes walk the group of every arc of v, four 16-byte records in flight per lane
 __global__ void __launch_bounds__(kFilterWarps * 32) k_filter(const PostArgs a, u64 K) {
     const u64 u = (u64)blockIdx.x * kFilterWarps + (threadIdx.x >> 5);
     if (u >= K) return;
@@ -297,30 +308,44 @@ __global__ void __launch_bounds__(kFilterWarps * 32) k_filter(const PostArgs a, 
     const unsigned char* ev = a.cand + (u64)a.uniq[u] * a.cand_stride;
     const int n = cand_n(ev);
     const u16* arc = cand_arc(ev, n);
-    const bool exact = a.g.A <= 128;
-    u64 lo = 0, hi = 0;
+    const bool exact = a.g.A <= kSigBits;
+    u32 w0 = 0, w1 = 0, w2 = 0, w3 = 0;
     for (int t = lane; t < n; t += 32) {
         const u32 b = sig_bit(arc[t], exact);
-        if (b < 64) lo |= 1ULL << b; else hi |= 1ULL << (b - 64);
+        const u32 m = 1u << (b & 31);
+        if (b < 32) w0 |= m; else if (b < 64) w1 |= m; else if (b < 96) w2 |= m; else w3 |= m;
     }
-#pragma unroll
-    for (int o = 16; o; o >>= 1) { lo |= __shfl_xor_sync(0xffffffffu, lo, o); hi |= __shfl_xor_sync(0xffffffffu, hi, o); }
-    const u64 nlo = ~lo, nhi = ~hi;
+    w0 = __reduce_or_sync(0xffffffffu, w0); w1 = __reduce_or_sync(0xffffffffu, w1);
+    w2 = __reduce_or_sync(0xffffffffu, w2); w3 = __reduce_or_sync(0xffffffffu, w3);
+    const u32 n0 = ~w0, n1 = ~w1, n2 = ~w2, n3 = ~w3 & 0xffffu;
     bool found = false;
     u64 pairs = 0;
-    for (int t = 0; t < n && !found; ++t) {
-        const int ga = arc[t];
-        const u32 g0 = a.gstart[ga], g1 = a.gstart[ga + 1];
-        for (u32 base = g0; base < g1 && !found; base += 32) {
-            const u32 w = base + lane;
-            bool hit = false;
-            if (w < g1 && (int)a.g_size[w] < n) {   // a strict subset is strictly smaller (equal supports were merged by a-6)
-                const ulonglong2 sw = a.g_sig[w];
-                ++pairs;
-                if (((sw.x & nlo) | (sw.y & nhi)) == 0)
-                    hit = exact || arcs_subset(a.cand + (u64)a.g_row[w] * a.cand_stride, ev);
+    for (int t0 = 0; t0 < n && !found; t0 += 32) {
+        // group ranges of 32 arcs of v at a time (one per lane), then the groups one after the other
+        const int tt = t0 + lane;
+        u32 myg0 = 0, myg1 = 0;
+        if (tt < n) { const int ga = arc[tt]; myg0 = a.gstart[ga]; myg1 = a.gstart[ga + 1]; }
+        const int cnt = min(32, n - t0);
+        for (int j = 0; j < cnt && !found; ++j) {
+            const u32 g0 = __shfl_sync(0xffffffffu, myg0, j), g1 = __shfl_sync(0xffffffffu, myg1, j);
+            for (u32 base = g0; base < g1 && !found; base += 128) {
+                uint4 r[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const u32 w = base + 32 * q + lane;
+                    r[q] = w < g1 ? __ldg(&a.g_sig[w]) : make_uint4(0xffffffffu, 0, 0, 0xffffffffu);   // never a subset
+                }
+                bool hit = false;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const u32 w = base + 32 * q + lane;
+                    pairs += w < g1;
+                    // a strict subset is strictly smaller (equal supports were merged by a-6)
+                    if (((r[q].x & n0) | (r[q].y & n1) | (r[q].z & n2) | (r[q].w & n3)) == 0 && (int)(r[q].w >> 16) < n)
+                        hit = hit || exact || arcs_subset(a.cand + (u64)a.g_row[w] * a.cand_stride, ev);
+                }
+                found = __any_sync(0xffffffffu, hit);
             }
-            found = __any_sync(0xffffffffu, hit);
         }
     }
 #pragma unroll
@@ -332,13 +357,16 @@ __global__ void __launch_bounds__(kFilterWarps * 32) k_filter(const PostArgs a, 
 }
 
 cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s, int* n_launches) {
-    (void)sm_count;
     cudaError_t e;
     if ((e = cudaMemsetAsync(a.freq, 0, sizeof(u32) * (a.g.A + 2), s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(a.gcount, 0, sizeof(u32) * (a.g.A + 2), s)) != cudaSuccess) return e;
     if (K == 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((K + 255) / 256);
-    k_filter_freq<<<blocks, 256, 0, s>>>(a, K);
+    {
+        const int use_smem = (size_t)a.g.A * 4 <= 40 * 1024;
+        unsigned fb = blocks < (unsigned)sm_count * 8 ? blocks : (unsigned)sm_count * 8;
+        k_filter_freq<<<fb, 256, use_smem ? (size_t)a.g.A * 4 : 0, s>>>(a, K, use_smem);
+    }
     k_filter_count<<<blocks, 256, 0, s>>>(a, K);
     k_filter_scan<<<1, 1024, 0, s>>>(a);
     k_filter_scatter<<<blocks, 256, 0, s>>>(a, K);
