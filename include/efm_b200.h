@@ -149,6 +149,12 @@ int efm_result_copy(const efm_handle* h, int64_t* flux, int64_t capacity_rows);
 int efm_result_sparse_stride(const efm_handle* h, int32_t* row_capacity);
 int efm_result_copy_sparse(const efm_handle* h, int32_t* nnz, int32_t* rxn, int64_t* val, int64_t capacity_rows);
 
+/* Compressed sparse rows to HOST memory (pinned memory makes the copies fast): row_ptr[count+1], then rxn / val with
+ * efm_result_nnz() entries; row r occupies [row_ptr[r], row_ptr[r+1]), reactions ascending.  The copies are enqueued
+ * on `cuda_stream` and the call returns after they completed. */
+int efm_result_nnz(const efm_handle* h, int64_t* total_nnz);
+int efm_result_copy_csr(const efm_handle* h, int64_t* row_ptr, int32_t* rxn, int64_t* val, void* cuda_stream);
+
 /* DEVICE pointers to the sparse result inside the workspace (same layout as above). */
 int efm_result_device(const efm_handle* h, const int32_t** d_nnz, const int32_t** d_rxn, const int64_t** d_val);
 

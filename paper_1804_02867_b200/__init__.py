@@ -74,6 +74,8 @@ def load() -> ctypes.CDLL:
     lib.efm_result_copy.argtypes = [vp, vp, i64]
     lib.efm_result_sparse_stride.argtypes = [vp, P(i32)]
     lib.efm_result_copy_sparse.argtypes = [vp, vp, vp, vp, i64]
+    lib.efm_result_nnz.argtypes = [vp, P(i64)]
+    lib.efm_result_copy_csr.argtypes = [vp, vp, vp, vp, vp]
     lib.efm_result_device.argtypes = [vp, P(vp), P(vp), P(vp)]
     lib.efm_result_densify.argtypes = [vp, i64, i64, vp, vp]
     lib.efm_get_stats.argtypes = [vp, P(efm_stats)]
@@ -224,6 +226,23 @@ class Enumerator:
         val = np.zeros((k.value, cap.value), np.int64)
         self._check(self._lib.efm_result_copy_sparse(self._h, _ptr(nnz), _ptr(rxn), _ptr(val), k.value))
         return nnz, rxn, val
+
+    def result_csr(self, pinned: bool = True):
+        """Compressed rows (row_ptr int64[K+1], rxn int32[nnz], val int64[nnz]) as torch CPU tensors; pinned host
+        memory by default so that the device-to-host copies run at link speed."""
+        import torch
+        k, z = ctypes.c_int64(), ctypes.c_int64()
+        self._check(self._lib.efm_result_count(self._h, ctypes.byref(k)))
+        self._check(self._lib.efm_result_nnz(self._h, ctypes.byref(z)))
+        pin = bool(pinned) and torch.cuda.is_available()
+        row_ptr = torch.empty(k.value + 1, dtype=torch.int64, pin_memory=pin)
+        rxn = torch.empty(max(z.value, 1), dtype=torch.int32, pin_memory=pin)
+        val = torch.empty(max(z.value, 1), dtype=torch.int64, pin_memory=pin)
+        with torch.cuda.device(self.device):
+            stream = torch.cuda.current_stream().cuda_stream
+            self._check(self._lib.efm_result_copy_csr(self._h, ctypes.c_void_p(row_ptr.data_ptr()), ctypes.c_void_p(rxn.data_ptr()),
+                                                      ctypes.c_void_p(val.data_ptr()), ctypes.c_void_p(stream)))
+        return row_ptr, rxn[: z.value], val[: z.value]
 
     def stats(self) -> Dict[str, float]:
         st = efm_stats()

@@ -24,7 +24,7 @@ struct Region { size_t off = 0, bytes = 0; };
 struct Layout {
     Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
     Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill;
-    Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, dense;
+    Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
 };
 
@@ -47,7 +47,7 @@ struct efm_handle {
     unsigned char* ws = nullptr;
     unsigned char* graph_ws = nullptr;   // workspace the graph arrays were last uploaded to
     bool have_result = false;
-    int64_t n_out = 0;
+    int64_t n_out = 0, csr_nnz = 0;
     efm_stats stats;
     std::vector<int64_t> lvl_active, lvl_done, lvl_expanded, lvl_children;
     std::string last_error;
@@ -112,6 +112,7 @@ void make_layout(efm_handle* h) {
     add_region(L, L.r_nnz, C * 4);
     add_region(L, L.r_rxn, C * h->D * 4);
     add_region(L, L.r_val, C * h->D * 8);
+    add_region(L, L.csr_ptr, (C + 1) * 8);
     add_region(L, L.dense, h->dense_bytes);
     L.total = (L.total + 255) & ~(size_t)255;
     h->lay = L;
@@ -520,6 +521,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
             st.filter_pairs = (int64_t)hc->filter_pairs;
             pa.n_pad = pow2_at_least((size_t)std::max<u64>(n_keep, 2));
             CK(launch_output_sort(pa, n_keep, s, &launches));
+            // compressed rows for efm_result_copy_csr (the unsorted row arrays are dead by now and hold the packed rows)
+            CK(launch_output_csr(pa, n_keep, (i64*)(ws + L.csr_ptr.off), pa.u_rxn, pa.u_val, s, &launches));
+            CK(read_ctl());
             size_t t4 = tm.mark();
             tm.span(t2, t3, PH_FILTER); tm.span(t3, t4, PH_OUTPUT);
         }
@@ -559,6 +563,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         st.ms_direct = acc[PH_DIRECT]; st.ms_hash = acc[PH_HASH]; st.ms_filter = acc[PH_FILTER]; st.ms_output = acc[PH_OUTPUT];
     }
     h->n_out = (int64_t)n_keep;
+    h->csr_nnz = n_keep ? (int64_t)hc->csr_nnz : 0;
     h->have_result = true;
     return EFM_OK;
 }
@@ -620,6 +625,29 @@ int efm_result_copy(const efm_handle* hc, int64_t* flux, int64_t capacity_rows) 
         CK(cudaMemcpyAsync(flux + r0 * n, d_dense, (size_t)nr * n * 8, cudaMemcpyDeviceToHost, 0));
         CK(cudaStreamSynchronize(0));
     }
+    return EFM_OK;
+}
+
+int efm_result_nnz(const efm_handle* h, int64_t* total_nnz) {
+    if (!h || !total_nnz) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    *total_nnz = h->csr_nnz;
+    return EFM_OK;
+}
+
+int efm_result_copy_csr(const efm_handle* hc, int64_t* row_ptr, int32_t* rxn, int64_t* val, void* cuda_stream) {
+    efm_handle* h = const_cast<efm_handle*>(hc);
+    if (!h || !row_ptr) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    if (h->n_out == 0) { row_ptr[0] = 0; return EFM_OK; }
+    if (!rxn || !val) return EFM_E_INVAL;
+    CK(cudaSetDevice(h->device));
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t K = (size_t)h->n_out, Z = (size_t)h->csr_nnz;
+    CK(cudaMemcpyAsync(row_ptr, h->ws + h->lay.csr_ptr.off, (K + 1) * 8, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(rxn, h->ws + h->lay.u_rxn.off, Z * 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(val, h->ws + h->lay.u_val.off, Z * 8, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
     return EFM_OK;
 }
 

@@ -76,7 +76,7 @@ struct Ctl {
     u32 sel_ticket, pad0;
     u64 st[ST_COUNT];
     // post-processing counters
-    u64 n_unique, n_poisoned, n_uniq_ok, n_keep, filter_pairs;
+    u64 n_unique, n_poisoned, n_uniq_ok, n_keep, filter_pairs, csr_nnz;
     // everything above is read back by the host once per level; the histogram stays on the device
     u32 hist[SEL_BINS];
 };

@@ -80,57 +80,57 @@ int build_graph(HostGraph& G, const int32_t* S, int32_t m, int32_t n, int64_t ro
     for (int32_t i = 0; i < G.M; ++i)
         G.dep_off[i + 1] = G.dep_off[i] + (int64_t)(G.out_ptr[i + 1] - G.out_ptr[i]) * (G.in_ptr[i + 1] - G.in_ptr[i]);
     G.dep_bits.assign((size_t)((G.dep_off[G.M] + 31) / 32) + 1, 0u);
-    // A metabolite's consumer list is swept once per search: the first arc x that reaches q stamps every consumer but
-    // twin(x); a second, different arc reaching q can only add that one twin.  Nodes are independent, so the searches
-    // are spread over host threads (bits of neighbouring nodes can share a word: atomic OR).
-    auto worker = [&G, dep_depth](int32_t tid, int32_t nthreads) {
-        std::vector<int32_t> stamp((size_t)G.A, -1), frontier, next;
-        std::vector<int32_t> q_epoch((size_t)G.M, -1), q_first((size_t)G.M, -1);
-        std::vector<char> q_full((size_t)G.M, 0);
-        int32_t epoch = 0;
-        for (int32_t i = tid; i < G.M; i += nthreads) {
-            const int32_t nI = G.in_ptr[i + 1] - G.in_ptr[i];
-            if (nI == 0) continue;
-            for (int32_t lo = 0; lo < G.out_ptr[i + 1] - G.out_ptr[i]; ++lo) {
-                const int32_t o = G.out[G.out_ptr[i] + lo].arc;
-                ++epoch;
-                frontier.assign(1, o);
-                stamp[o] = epoch;
-                for (int32_t hop = 1; hop < dep_depth && !frontier.empty(); ++hop) {
-                    next.clear();
-                    for (int32_t x : frontier)
-                        for (int32_t q = G.col_ptr[x]; q < G.col_ptr[x + 1]; ++q) {
-                            if (G.col[q].s <= 0 || G.col[q].met == i) continue;
-                            const int32_t via = G.col[q].met;
-                            if (q_epoch[via] != epoch) {
-                                q_epoch[via] = epoch; q_first[via] = x; q_full[via] = 0;
-                                for (int32_t r = G.out_ptr[via]; r < G.out_ptr[via + 1]; ++r) {
-                                    const int32_t y = G.out[r].arc;
-                                    if (y == G.twin[x] || stamp[y] == epoch) continue;
-                                    stamp[y] = epoch;
-                                    next.push_back(y);
-                                }
-                            } else if (!q_full[via] && q_first[via] != x) {
-                                q_full[via] = 1;
-                                const int32_t y = G.twin[q_first[via]];   // consumes `via` because its twin produces it
-                                if (y >= 0 && stamp[y] != epoch) { stamp[y] = epoch; next.push_back(y); }
-                            }
-                        }
-                    frontier.swap(next);
+    // 64 searches run at once, one bit each (bit s of R[y]: arc y is reachable from the start arc of search s).  A hop
+    // goes through the metabolites: ANY[q] = OR of R over the producers of q, MULTI[q] = bits set in at least two of
+    // them, both without the searches whose own node is q (the chain must not pass through N_i).  A consumer y of q
+    // whose twin also produces q must not be entered from that twin: it takes MULTI[q] | (ANY[q] & ~R[twin(y)]),
+    // every other consumer takes ANY[q].  The relation x -> y is a property of the pair, so reachability within
+    // L-1 hops is R_{h+1} = R_h | step(R_h).
+    struct Src { int32_t node, lo, arc; };
+    std::vector<Src> srcs;
+    for (int32_t i = 0; i < G.M; ++i) {
+        if (G.in_ptr[i + 1] == G.in_ptr[i]) continue;
+        for (int32_t lo = 0; lo < G.out_ptr[i + 1] - G.out_ptr[i]; ++lo) srcs.push_back(Src{i, lo, G.out[G.out_ptr[i] + lo].arc});
+    }
+    const int64_t n_batches = ((int64_t)srcs.size() + 63) / 64;
+    auto worker = [&G, &srcs, n_batches, dep_depth](int32_t tid, int32_t nthreads) {
+        std::vector<uint64_t> R((size_t)G.A), Rn((size_t)G.A), any((size_t)G.M), multi((size_t)G.M), ex((size_t)G.M, 0);
+        for (int64_t b = tid; b < n_batches; b += nthreads) {
+            const size_t s0 = (size_t)b * 64, s1 = std::min(srcs.size(), s0 + 64);
+            std::fill(R.begin(), R.end(), 0ULL);
+            for (size_t s = s0; s < s1; ++s) { R[srcs[s].arc] |= 1ULL << (s - s0); ex[srcs[s].node] |= 1ULL << (s - s0); }
+            for (int32_t hop = 1; hop < dep_depth; ++hop) {
+                for (int32_t q = 0; q < G.M; ++q) {
+                    uint64_t an = 0, mu = 0;
+                    for (int32_t r = G.in_ptr[q]; r < G.in_ptr[q + 1]; ++r) { const uint64_t v = R[G.in[r].arc]; mu |= an & v; an |= v; }
+                    any[q] = an & ~ex[q]; multi[q] = mu & ~ex[q];
                 }
+                for (int32_t y = 0; y < G.A; ++y) {
+                    uint64_t acc = 0;
+                    const int32_t t = G.twin[y];
+                    const uint64_t not_t = t >= 0 ? ~R[t] : ~0ULL;   // twin(y) produces exactly what y consumes
+                    for (int32_t q = G.col_ptr[y]; q < G.col_ptr[y + 1]; ++q)
+                        if (G.col[q].s < 0) acc |= multi[G.col[q].met] | (any[G.col[q].met] & not_t);
+                    Rn[y] = R[y] | acc;
+                }
+                R.swap(Rn);
+            }
+            for (size_t s = s0; s < s1; ++s) {
+                const int32_t i = srcs[s].node, nI = G.in_ptr[i + 1] - G.in_ptr[i];
                 for (int32_t le = 0; le < nI; ++le) {
                     const int32_t e = G.in[G.in_ptr[i] + le].arc;
-                    if (e != o && stamp[e] == epoch) {
-                        const int64_t b = G.dep_off[i] + (int64_t)lo * nI + le;
-                        __atomic_fetch_or(&G.dep_bits[b >> 5], 1u << (b & 31), __ATOMIC_RELAXED);
+                    if (e != srcs[s].arc && ((R[e] >> (s - s0)) & 1ULL)) {
+                        const int64_t bit = G.dep_off[i] + (int64_t)srcs[s].lo * nI + le;
+                        __atomic_fetch_or(&G.dep_bits[bit >> 5], 1u << (bit & 31), __ATOMIC_RELAXED);
                     }
                 }
+                ex[srcs[s].node] = 0;
             }
         }
     };
     int32_t nthreads = (int32_t)std::thread::hardware_concurrency();
     nthreads = std::max(1, std::min(nthreads, 32));
-    if (G.dep_off[G.M] < 4096) nthreads = 1;
+    nthreads = (int32_t)std::max<int64_t>(1, std::min<int64_t>(nthreads, n_batches));
     if (nthreads == 1) worker(0, 1);
     else {
         std::vector<std::thread> pool;

@@ -35,6 +35,7 @@ cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_l
 cudaError_t launch_filter(const PostArgs& a, u64 n_uniq, int sm_count, cudaStream_t s, int* n_launches);
 cudaError_t launch_output_rows(const PostArgs& a, u64 n_uniq, cudaStream_t s, int* n_launches);
 cudaError_t launch_output_sort(const PostArgs& a, u64 n_keep, cudaStream_t s, int* n_launches);
+cudaError_t launch_output_csr(const PostArgs& a, u64 n_keep, i64* row_ptr, int* c_rxn, i64* c_val, cudaStream_t s, int* n_launches);
 cudaError_t launch_densify(const int* r_nnz, const int* r_rxn, const i64* r_val, int D, int n_rxn, i64 row0, i64 n_rows,
                            i64* d_out, cudaStream_t s);
 cudaError_t launch_debug_hash(int n_supp, const int* arc, const i64* flux, int n_vis, const int* vis4, u64* out, cudaStream_t s);

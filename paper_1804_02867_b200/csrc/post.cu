@@ -452,6 +452,44 @@ __global__ void __launch_bounds__(256) k_out_gather(const PostArgs a, u64 n_keep
     for (int t = 0; t < n; ++t) { a.r_rxn[r * a.D + t] = a.u_rxn[(u64)src * a.D + t]; a.r_val[r * a.D + t] = a.u_val[(u64)src * a.D + t]; }
 }
 
+// Compressed rows (CSR) of the final result: row pointer by a one-block chunked scan, then one warp per row.
+__global__ void __launch_bounds__(1024) k_csr_scan(const int* __restrict__ r_nnz, u64 K, i64* __restrict__ row_ptr, Ctl* ctl) {
+    __shared__ i64 part[1024];
+    __shared__ i64 carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (u64 base = 0; base < K; base += 1024) {
+        const u64 r = base + threadIdx.x;
+        const i64 v = r < K ? r_nnz[r] : 0;
+        part[threadIdx.x] = v;
+        __syncthreads();
+        for (int off = 1; off < 1024; off <<= 1) {
+            const i64 x = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
+            __syncthreads();
+            part[threadIdx.x] += x;
+            __syncthreads();
+        }
+        if (r < K) row_ptr[r] = carry + part[threadIdx.x] - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry += part[1023];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { row_ptr[K] = carry; ctl->csr_nnz = (u64)carry; }
+}
+__global__ void __launch_bounds__(256) k_csr_pack(const PostArgs a, u64 K, const i64* __restrict__ row_ptr, int* __restrict__ c_rxn, i64* __restrict__ c_val) {
+    const u64 r = (u64)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (r >= K) return;
+    const int lane = threadIdx.x & 31, n = a.r_nnz[r];
+    const i64 o = row_ptr[r];
+    for (int t = lane; t < n; t += 32) { c_rxn[o + t] = a.r_rxn[r * a.D + t]; c_val[o + t] = a.r_val[r * a.D + t]; }
+}
+cudaError_t launch_output_csr(const PostArgs& a, u64 K, i64* row_ptr, int* c_rxn, i64* c_val, cudaStream_t s, int* n_launches) {
+    k_csr_scan<<<1, 1024, 0, s>>>(a.r_nnz, K, row_ptr, a.ctl);
+    ++*n_launches;
+    if (K) { k_csr_pack<<<(unsigned)((K + 7) / 8), 256, 0, s>>>(a, K, row_ptr, c_rxn, c_val); ++*n_launches; }
+    return cudaGetLastError();
+}
+
 cudaError_t launch_output_rows(const PostArgs& a, u64 K, cudaStream_t s, int* n_launches) {
     if (K == 0) return cudaSuccess;
     k_out_rows<<<(unsigned)((K + 255) / 256), 256, 0, s>>>(a, K);

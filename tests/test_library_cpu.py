@@ -36,7 +36,7 @@ def test_struct_sizes_match_header(lib_mod):
 
 @pytest.mark.parametrize("name", ["toy", "small", "core", "mid", "genome"])
 def test_graph_builder_matches_oracle_graph(lib_mod, oracle_mod, name):
-    """Two independent builders (library: counting sort + stamped BFS; oracle: dense scans + seen array) must
+    """Two independent builders (library: counting sort + 64-way bit-parallel reachability; oracle: dense scans + seen array) must
     produce the same MG graph and the same dependency table."""
     net = make_network(name, 0)
     en = lib_mod.Enumerator(net.S, net.reversible, net.internal, net.params)

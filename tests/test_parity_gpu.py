@@ -205,6 +205,11 @@ def test_sparse_and_dense_results_agree(efm):
     for r in range(res.n_out):
         dense[r, rxn[r, : nnz[r]]] = val[r, : nnz[r]]
     assert np.array_equal(dense, res.flux)
+    row_ptr, crxn, cval = (t.numpy() for t in en.result_csr())
+    assert row_ptr[0] == 0 and np.array_equal(np.diff(row_ptr), nnz)
+    for r in range(res.n_out):
+        assert np.array_equal(crxn[row_ptr[r]: row_ptr[r + 1]], rxn[r, : nnz[r]])
+        assert np.array_equal(cval[row_ptr[r]: row_ptr[r + 1]], val[r, : nnz[r]])
     again = en.enumerate()   # the handle and the workspace are reusable
     assert np.array_equal(again.flux, res.flux)
     en.close()
