@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the AND/OR-graph pathway traversal (arXiv 1804.02867) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload genome] [--cap 65536]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload genome] [--cap 262144]
 
 A *step* is one pass of the whole hot path (roots, classify, beam select, expand, support dedup, minimality filter,
 canonical output: SURVEY.md 8(a) rows a-2..a-8) over one seeded synthetic network that is already resident in HBM
@@ -28,6 +28,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+DEFAULT_CAP = 262144          # frontier_cap of the timed workload
+DEFAULT_MAX_CANDIDATES = 1 << 22
 METRIC = "partial_pathways_expanded_per_sec"
 UNIT = "expanded/s"
 
@@ -254,7 +256,7 @@ def main_ours(args):
         # the oracle as it stands on this box's host cores, bounded sample of the same workload
         cpu = None
         if not args.no_cpu_baseline:
-            cap_s = min(args.cap, 4096 if args.workload == "genome" else args.cap)
+            cap_s = min(args.cap, 16384 if args.workload == "genome" else args.cap)   # about 10 s on 16 cores
             e, dt, outs, th = run_oracle_sample(args.workload, cap_s)
             cpu = {"value": e / dt, "unit": UNIT, "cores": th, "kind": "oracle",
                    "sample": f"same network/parameters, frontier_cap {cap_s} instead of {args.cap}; one whole oracle run "
@@ -302,8 +304,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="genome", choices=["toy", "small", "core", "mid", "genome"])
-    ap.add_argument("--cap", type=int, default=65536, help="frontier_cap (beam) of the workload")
-    ap.add_argument("--max-candidates", type=int, default=1 << 20)
+    ap.add_argument("--cap", type=int, default=DEFAULT_CAP, help="frontier_cap (beam) of the workload")
+    ap.add_argument("--max-candidates", type=int, default=DEFAULT_MAX_CANDIDATES)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram bytes per expand launch from profiles/ (null until captured)")

@@ -216,13 +216,15 @@ def test_sparse_and_dense_results_agree(efm):
 
 
 def test_bench_configuration_properties(efm):
-    """The configuration bench.py times (genome seed 0, frontier_cap 65536) is too large for the oracle (about
+    """The configuration bench.py times (genome seed 0, frontier_cap bench.DEFAULT_CAP) is too large for the oracle (about
     2 ms per unit of cap), so it is held by what is true at any size: Def 2 on every output, canonical form,
     support-minimality and lexicographic order on samples, counter identities, and run-to-run determinism (the
     kernels allocate with atomics, the result must not depend on their order)."""
     import scipy.sparse as sp
+    import bench
+    cap = bench.DEFAULT_CAP
     net = make_network("genome", 0)
-    params = dict(net.params, frontier_cap=65536, max_candidates=1 << 20)
+    params = dict(net.params, frontier_cap=cap, max_candidates=bench.DEFAULT_MAX_CANDIDATES)
     en = efm.Enumerator(net.S, net.reversible, net.internal, params)
     res = en.enumerate(net.seed_sets, dense=False)
     nnz, rxn, val = en.result_sparse()
@@ -257,7 +259,7 @@ def test_bench_configuration_properties(efm):
     assert int(st["done"]) == int(lv["done"].sum()) >= int(st["unique_supports"])
     assert int(st["unique_supports"]) - int(st["poisoned"]) >= K
     assert int(st["peak_frontier"]) == int(lv["active"].max()) and int(st["levels"]) == len(lv["active"])
-    assert np.all(lv["expanded"] <= 65536) and int(lv["expanded"].max()) > 60000
+    assert np.all(lv["expanded"] <= cap) and int(lv["expanded"].max()) > 0.9 * cap
     assert int(st["truncated_beam"]) == int(lv["active"].sum() - lv["expanded"].sum())
     # determinism
     again = en.enumerate(net.seed_sets, dense=False)
