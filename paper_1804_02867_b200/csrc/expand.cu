@@ -573,8 +573,11 @@ __global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, c
 // Reads the task, reads the parent entry straight from HBM / L2 (every element is needed once) and writes the child:
 // a candidate slot if it is balanced, otherwise a packed entry of the next frontier.  A block of kMatWarps children
 // reserves its output with one atomic per kind.
+#ifndef EFM_MAT_BLOCKS
+#define EFM_MAT_BLOCKS 4
+#endif
 constexpr int kMatWarps = 8;
-__global__ void __launch_bounds__(kMatWarps * 32, 4) k_materialise(const __grid_constant__ ExpandArgs A) {
+__global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(const __grid_constant__ ExpandArgs A) {
     __shared__ u32 s_units[kMatWarps];
     __shared__ u64 s_base[kMatWarps];
     __shared__ u64 s_slot[kMatWarps];
@@ -618,6 +621,22 @@ __global__ void __launch_bounds__(kMatWarps * 32, 4) k_materialise(const __grid_
     const int nv2 = to_cand ? 0 : nv + (firstv ? 1 : 0);
     const int nu2 = to_cand ? 0 : cnu;
     const u32 units = live ? (to_cand ? 0u : entry_bytes((u32)n2, (u32)nv2, (u32)nu2) >> 4) : 0u;
+    // ---- every element of the parent this lane will need, requested before anything waits: the loads overlap each
+    // other and the block-wide reservation below (entries beyond 64 arcs / records are loaded where they are used)
+    u32 pa0 = 0xffffffffu, pa1 = 0xffffffffu, pm0 = 0xffffffffu;
+    i64 pf0 = 0, pf1 = 0, pe0 = 0;
+    u64 pv0 = 0, pv1 = 0;
+    int pcol0 = 0, pcol1 = 0;
+    if (live) {
+        if (lane < ns) { pa0 = arc[lane]; pf0 = flux[lane]; }
+        if (lane + 32 < ns) { pa1 = arc[lane + 32]; pf1 = flux[lane + 32]; }
+        if (!to_cand) {
+            if (lane < nv) pv0 = vis[lane];
+            if (lane + 32 < nv) pv1 = vis[lane + 32];
+            if (lane < nu) { pm0 = efmet[lane]; pe0 = ef[lane]; }
+            pcol0 = __ldg(&A.g.col_ptr[ca]); pcol1 = __ldg(&A.g.col_ptr[ca + 1]);
+        }
+    }
     // ---- reserve the output of the whole block: one atomic for the frontier entries, one for the candidates
     if (lane == 0) {
         s_units[wib] = units; s_slot[wib] = (live && to_cand) ? 1 : 0;
@@ -656,7 +675,8 @@ __global__ void __launch_bounds__(kMatWarps * 32, 4) k_materialise(const __grid_
     if (!cin)
         for (int b2 = 0; b2 < ns; b2 += 32) {
             const int t = b2 + lane;
-            ins += __popc(__ballot_sync(0xffffffffu, t < ns && (int)arc[t] < ca));
+            const u32 at = b2 == 0 ? pa0 : (b2 == 32 ? pa1 : (t < ns ? (u32)arc[t] : 0xffffffffu));
+            ins += __popc(__ballot_sync(0xffffffffu, at < (u32)ca));
         }
     i64* flux2 = (i64*)(dst + kHdr);
     u64* vis2 = (u64*)(flux2 + n2);
@@ -665,11 +685,12 @@ __global__ void __launch_bounds__(kMatWarps * 32, 4) k_materialise(const __grid_
     u16* efmet2 = arc2 + n2;
     u64 mx = cin ? 0ULL : cT;   // a new arc never comes with a common divisor
     for (int t = lane; t < ns; t += 32) {
-        u64 F = t == cia ? cT : ck * (u64)flux[t];
+        const u64 ft = t < 32 ? (u64)pf0 : (t < 64 ? (u64)pf1 : (u64)flux[t]);
+        u64 F = t == cia ? cT : ck * ft;
         if (cg > 1) F /= cg;
         const int pos = t + ((!cin && t >= ins) ? 1 : 0);
         flux2[pos] = (i64)F;
-        arc2[pos] = arc[t];
+        arc2[pos] = (u16)(t < 32 ? pa0 : (t < 64 ? pa1 : (u32)arc[t]));
         mx = max(mx, F);
     }
     if (!cin && lane == 0) { flux2[ins] = (i64)cT; arc2[ins] = (u16)ca; }
@@ -677,14 +698,14 @@ __global__ void __launch_bounds__(kMatWarps * 32, 4) k_materialise(const __grid_
         // the visited record of i* is appended (first visit) or replaced (revisit)
         const u32 met_star = (u32)((newrec >> 32) & 0xffffu);
         for (int u = lane; u < nv; u += 32) {
-            const u64 r = vis[u];
+            const u64 r = u < 32 ? pv0 : (u < 64 ? pv1 : vis[u]);
             vis2[u] = (!firstv && (u32)((r >> 32) & 0xffffu) == met_star) ? newrec : r;
         }
         if (firstv && lane == 0) vis2[nv] = newrec;
         // EF list of the child: EF' = (k EF + sign d s_.a) / g over the parent's list, then the metabolites of col(a)
         // that were balanced in the parent.  k_expand established that nothing exceeds 2^62, so the wrapping 64-bit
         // arithmetic is exact.
-        const int qa0 = __ldg(&A.g.col_ptr[ca]), qa1 = __ldg(&A.g.col_ptr[ca + 1]);
+        const int qa0 = pcol0, qa1 = pcol1;
         int wbase = 0;
         u32 seen = 0;   // bit q - qa0: metabolite of col(a)[q] is in the parent's list (columns longer than 32: see below)
         for (int t0 = 0; t0 < nu; t0 += 32) {
@@ -693,10 +714,10 @@ __global__ void __launch_bounds__(kMatWarps * 32, 4) k_materialise(const __grid_
             i64 x = 0;
             int met = -1;
             if (valid) {
-                met = efmet[t];
+                met = t0 == 0 ? (int)pm0 : (int)efmet[t];
                 i64 s = 0;
                 for (int qq = qa0; qq < qa1; ++qq) { const int2 e = __ldg(&A.g.col[qq]); if (e.x == met) s = e.y; }
-                x = (i64)(ck * (u64)ef[t] + sd * (u64)s);
+                x = (i64)(ck * (u64)(t0 == 0 ? pe0 : ef[t]) + sd * (u64)s);
                 if (cg > 1) x /= (i64)cg;
             }
             for (int qq = qa0; qq < qa1 && qq < qa0 + 32; ++qq)
@@ -857,8 +878,8 @@ cudaError_t launch_expand(const ExpandArgs& a, int sm_count, cudaStream_t s) {
 // survivors of the level -> next frontier / candidates.  n_hint bounds the key slots in use (host side estimate).
 cudaError_t launch_materialise(const ExpandArgs& a, u64 n_slots_hint, u64 n_surv, int sm_count, cudaStream_t s, int phase) {
     if (phase == 0) {   // compact
-        u64 blocks = (n_slots_hint + 2047) / 2048;
-        if (blocks > (u64)sm_count * 16) blocks = (u64)sm_count * 16;
+        u64 blocks = (n_slots_hint + 511) / 512;   // about two keys per thread: the kernel is one dependent-load chain per key
+        if (blocks > (u64)sm_count * 128) blocks = (u64)sm_count * 128;
         if (blocks < 1) blocks = 1;
         k_compact<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.t0, a.cur_off, a.surv, a.ctl, a.max_keys);
         return cudaGetLastError();
