@@ -96,11 +96,12 @@ void make_layout(efm_handle* h) {
     add_region(L, L.isrep, C + 1);
     add_region(L, L.poison, C + 1);
     add_region(L, L.uniq, C * 4);
-    const size_t bins = (size_t)h->G.A + 2;   // per-arc tables of the minimality filter
+    const size_t bins = (size_t)h->G.A + 2;   // per-arc and per-(arc, size) tables of the minimality filter
+    const size_t gbins = (size_t)h->G.A * ((size_t)h->D + 1) + 2;
     add_region(L, L.freq, bins * 4);
-    add_region(L, L.gcount, bins * 4);
-    add_region(L, L.gstart, bins * 4);
-    add_region(L, L.gfill, bins * 4);
+    add_region(L, L.gcount, gbins * 4);
+    add_region(L, L.gstart, gbins * 4);
+    add_region(L, L.gfill, gbins * 4);
     add_region(L, L.g_row, C * 4);
     add_region(L, L.g_sig, C * 16);
     add_region(L, L.g_size, C * 2);
@@ -497,7 +498,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     pa.gstart = (u32*)(ws + L.gstart.off); pa.gfill = (u32*)(ws + L.gfill.off);
     pa.g_row = (u32*)(ws + L.g_row.off); pa.g_sig = (uint4*)(ws + L.g_sig.off);
     pa.keep = ws + L.keep.off;
-    pa.D = h->D; pa.n_rxn = G.n;
+    pa.D = h->D; pa.n_rxn = G.n; pa.n_sizes = h->D + 1;
     pa.u_nnz = (int*)(ws + L.u_nnz.off); pa.u_rxn = (int*)(ws + L.u_rxn.off); pa.u_val = (i64*)(ws + L.u_val.off);
     pa.sort_idx = (u32*)(ws + L.sort_idx.off);
     pa.r_nnz = (int*)(ws + L.r_nnz.off); pa.r_rxn = (int*)(ws + L.r_rxn.off); pa.r_val = (i64*)(ws + L.r_val.off);

@@ -23,6 +23,7 @@ struct PostArgs {
     // minimality filter (a-7)
     u32* freq; u32* gcount; u32* gstart; u32* gfill;      // per arc: candidates using it, group size / start / fill
     u32* g_row; uint4* g_sig;                             // rows grouped by their rarest arc: candidate id, 112-bit signature + |supp|
+    int n_sizes;                                          // D + 1: the (arc, |supp|) bins of gcount / gstart / gfill
     unsigned char* keep;                                  // per unique support (uniq order)
     // canonical output (a-8)
     int D; int n_rxn;

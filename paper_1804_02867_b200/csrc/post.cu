@@ -255,11 +255,11 @@ __global__ void __launch_bounds__(256) k_filter_count(const PostArgs a, u64 K) {
     const unsigned char* e = a.cand + (u64)a.uniq[u] * a.cand_stride;
     const int n = cand_n(e);
     if (n == 0) return;   // the empty support belongs to no group (it has no strict subset and nothing tests against it)
-    atomicAdd(&a.gcount[rarest_arc(a, cand_arc(e, n), n)], 1u);
+    atomicAdd(&a.gcount[(size_t)rarest_arc(a, cand_arc(e, n), n) * a.n_sizes + n], 1u);   // group key: (rarest arc, |supp|)
 }
 __global__ void __launch_bounds__(1024) k_filter_scan(const PostArgs a) {   // exclusive scan of the group sizes over arcs
     __shared__ u32 part[1024];
-    const int A = a.g.A, T = blockDim.x, per = (A + T - 1) / T, b0 = threadIdx.x * per;
+    const int A = a.g.A * a.n_sizes, T = blockDim.x, per = (A + T - 1) / T, b0 = threadIdx.x * per;   // (arc, size) bins
     u32 sum = 0;
     for (int j = 0; j < per; ++j) if (b0 + j < A) sum += a.gcount[b0 + j];
     part[threadIdx.x] = sum;
@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K)
     const int n = cand_n(e);
     if (n == 0) return;
     const u16* arc = cand_arc(e, n);
-    const u32 pos = atomicAdd(&a.gfill[rarest_arc(a, arc, n)], 1u);
+    const u32 pos = atomicAdd(&a.gfill[(size_t)rarest_arc(a, arc, n) * a.n_sizes + n], 1u);
     a.g_row[pos] = id;
     a.g_sig[pos] = sig_of(arc, n, a.g.A <= kSigBits);
 }
@@ -324,7 +324,8 @@ __global__ void __launch_bounds__(kFilterWarps * 32) k_filter(const PostArgs a, 
         // group ranges of 32 arcs of v at a time (one per lane), then the groups one after the other
         const int tt = t0 + lane;
         u32 myg0 = 0, myg1 = 0;
-        if (tt < n) { const int ga = arc[tt]; myg0 = a.gstart[ga]; myg1 = a.gstart[ga + 1]; }
+        // within the group of an arc the rows are ordered by |supp|: only the strictly smaller ones can be subsets
+        if (tt < n) { const size_t gb = (size_t)arc[tt] * a.n_sizes; myg0 = a.gstart[gb]; myg1 = a.gstart[gb + n]; }
         const int cnt = min(32, n - t0);
         for (int j = 0; j < cnt && !found; ++j) {
             const u32 g0 = __shfl_sync(0xffffffffu, myg0, j), g1 = __shfl_sync(0xffffffffu, myg1, j);
@@ -359,7 +360,7 @@ __global__ void __launch_bounds__(kFilterWarps * 32) k_filter(const PostArgs a, 
 cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s, int* n_launches) {
     cudaError_t e;
     if ((e = cudaMemsetAsync(a.freq, 0, sizeof(u32) * (a.g.A + 2), s)) != cudaSuccess) return e;
-    if ((e = cudaMemsetAsync(a.gcount, 0, sizeof(u32) * (a.g.A + 2), s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(a.gcount, 0, sizeof(u32) * ((size_t)a.g.A * a.n_sizes + 2), s)) != cudaSuccess) return e;
     if (K == 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((K + 255) / 256);
     {
