@@ -24,7 +24,7 @@ struct Region { size_t off = 0, bytes = 0; };
 struct Layout {
     Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
     Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill;
-    Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
+    Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, u_key, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
 };
 
@@ -109,6 +109,7 @@ void make_layout(efm_handle* h) {
     add_region(L, L.u_nnz, C * 4);
     add_region(L, L.u_rxn, C * h->D * 4);
     add_region(L, L.u_val, C * h->D * 8);
+    add_region(L, L.u_key, C * 16);
     add_region(L, L.sort_idx, pow2_at_least(C) * 4);
     add_region(L, L.r_nnz, C * 4);
     add_region(L, L.r_rxn, C * h->D * 4);
@@ -500,6 +501,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     pa.keep = ws + L.keep.off;
     pa.D = h->D; pa.n_rxn = G.n; pa.n_sizes = h->D + 1;
     pa.u_nnz = (int*)(ws + L.u_nnz.off); pa.u_rxn = (int*)(ws + L.u_rxn.off); pa.u_val = (i64*)(ws + L.u_val.off);
+    pa.u_key = (ulonglong2*)(ws + L.u_key.off);
     pa.sort_idx = (u32*)(ws + L.sort_idx.off);
     pa.r_nnz = (int*)(ws + L.r_nnz.off); pa.r_rxn = (int*)(ws + L.r_rxn.off); pa.r_val = (i64*)(ws + L.r_val.off);
     u64 n_uniq_ok = 0, n_keep = 0;

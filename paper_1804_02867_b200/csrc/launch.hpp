@@ -28,6 +28,7 @@ struct PostArgs {
     // canonical output (a-8)
     int D; int n_rxn;
     int* u_nnz; int* u_rxn; i64* u_val;   // unsorted reaction-space rows
+    ulonglong2* u_key;                     // order codes of the first two entries of every unsorted row
     u32* sort_idx; u64 n_pad;
     int* r_nnz; int* r_rxn; i64* r_val;   // final, lexicographic order
 };

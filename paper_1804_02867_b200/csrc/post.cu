@@ -380,6 +380,24 @@ cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s
 // a-8  Canonical output: arc space -> reaction space (v_j = f_j+ - f_j-), lexicographic order of the dense signed
 // vectors, computed on the sparse rows with a bitonic sort of row indices.
 // =================================================================================================================
+// Order-preserving 64-bit code of "the next non-zero entry is value v at reaction j" (all earlier reactions equal):
+// a negative entry at a smaller reaction makes the row smaller, a positive one makes it larger, and a row without
+// further entries sits between the two classes.  Values are clamped to 32 bits; codes at the clamp (and the "no entry"
+// code) decide nothing on a tie.  Two such codes (first and second entry) settle almost every comparison of the sort
+// without touching the rows.
+__device__ __forceinline__ u64 order_code(bool has, int j, i64 v) {
+    if (!has) return 1ULL << 63;
+    const i64 L = (1LL << 31) - 1;
+    const u32 c = (u32)((v < -L ? -L : (v > L ? L : v)) + (1LL << 31));   // [1, 2^32 - 1]
+    return v < 0 ? ((u64)(u32)j << 32) | c : (1ULL << 63) | ((u64)(0x7fffffffu - (u32)j) << 32) | c;
+}
+__device__ __forceinline__ int key_cmp(const ulonglong2 kx, const ulonglong2 ky) {   // -1: x < y, +1: x > y, 0: look at the rows
+    if (kx.x != ky.x) return kx.x < ky.x ? -1 : 1;
+    const u32 low = (u32)kx.x;
+    if (low <= 1u || low == 0xffffffffu) return 0;
+    if (kx.y != ky.y) return kx.y < ky.y ? -1 : 1;
+    return 0;
+}
 __global__ void __launch_bounds__(256) k_out_rows(const PostArgs a, u64 K) {
     const u64 p = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= K || !a.keep[p]) return;
@@ -393,6 +411,8 @@ __global__ void __launch_bounds__(256) k_out_rows(const PostArgs a, u64 K) {
         a.u_rxn[r * a.D + t] = a.g.arc_rxn[arc[t]];
         a.u_val[r * a.D + t] = a.g.arc_dir[arc[t]] < 0 ? -f[t] : f[t];
     }
+    a.u_key[r] = make_ulonglong2(order_code(n > 0, n > 0 ? a.u_rxn[r * a.D] : 0, n > 0 ? a.u_val[r * a.D] : 0),
+                                 order_code(n > 1, n > 1 ? a.u_rxn[r * a.D + 1] : 0, n > 1 ? a.u_val[r * a.D + 1] : 0));
 }
 
 // strict lexicographic "row x < row y" on the dense vectors, evaluated on the sparse rows
@@ -422,14 +442,24 @@ __global__ void __launch_bounds__(256) k_bitonic_global(const PostArgs a, u64 j,
     if (ixj <= i) return;
     const bool asc = (i & k) == 0;
     const u32 x = a.sort_idx[i], y = a.sort_idx[ixj];
-    if (asc ? row_less(a, y, x) : row_less(a, x, y)) { a.sort_idx[i] = y; a.sort_idx[ixj] = x; }
+    bool swap;
+    if (x == 0xFFFFFFFFu || y == 0xFFFFFFFFu) swap = asc ? row_less(a, y, x) : row_less(a, x, y);
+    else {
+        const int c = key_cmp(a.u_key[x], a.u_key[y]);   // sign of x - y when the keys decide
+        swap = c ? (asc ? c > 0 : c < 0) : (asc ? row_less(a, y, x) : row_less(a, x, y));
+    }
+    if (swap) { a.sort_idx[i] = y; a.sort_idx[ixj] = x; }
 }
 constexpr int kSortChunk = 1024;
 // all compare-exchange steps with j < kSortChunk of the stages k in [k_lo, k_hi] on one shared-memory chunk
 __global__ void __launch_bounds__(kSortChunk / 2) k_bitonic_local(const PostArgs a, u64 k_lo, u64 k_hi) {
     __shared__ u32 s[kSortChunk];
+    __shared__ ulonglong2 sk[kSortChunk];   // the order keys travel with the indices
     const u64 base = (u64)blockIdx.x * kSortChunk;
-    for (int t = threadIdx.x; t < kSortChunk; t += blockDim.x) s[t] = base + t < a.n_pad ? a.sort_idx[base + t] : 0xFFFFFFFFu;
+    for (int t = threadIdx.x; t < kSortChunk; t += blockDim.x) {
+        s[t] = base + t < a.n_pad ? a.sort_idx[base + t] : 0xFFFFFFFFu;
+        sk[t] = s[t] == 0xFFFFFFFFu ? make_ulonglong2(~0ULL, ~0ULL) : a.u_key[s[t]];
+    }
     __syncthreads();
     for (u64 k = k_lo; k <= k_hi; k <<= 1) {
         for (u64 j = min(k >> 1, (u64)kSortChunk >> 1); j > 0; j >>= 1) {
@@ -438,7 +468,14 @@ __global__ void __launch_bounds__(kSortChunk / 2) k_bitonic_local(const PostArgs
             const int ixj = i | (int)j;
             const bool asc = ((base + i) & k) == 0;
             const u32 x = s[i], y = s[ixj];
-            if (asc ? row_less(a, y, x) : row_less(a, x, y)) { s[i] = y; s[ixj] = x; }
+            const ulonglong2 kx = sk[i], ky = sk[ixj];
+            bool swap;
+            if (x == 0xFFFFFFFFu || y == 0xFFFFFFFFu) swap = asc ? row_less(a, y, x) : row_less(a, x, y);
+            else {
+                const int c = key_cmp(kx, ky);
+                swap = c ? (asc ? c > 0 : c < 0) : (asc ? row_less(a, y, x) : row_less(a, x, y));
+            }
+            if (swap) { s[i] = y; s[ixj] = x; sk[i] = ky; sk[ixj] = kx; }
             __syncthreads();
         }
     }
