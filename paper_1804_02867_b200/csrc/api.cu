@@ -22,7 +22,7 @@ namespace {
 struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
-    Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
+    Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
     Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill;
     Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, u_key, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
@@ -74,6 +74,8 @@ void make_layout(efm_handle* h) {
     add_region(L, L.in_e, sizeof(int2) * (G.in.size() + 1));
     add_region(L, L.out_ptr, sizeof(int) * (G.M + 1));
     add_region(L, L.out_e, sizeof(int2) * (G.out.size() + 1));
+    add_region(L, L.in_alt, 32 * (G.in.size() + 1));
+    add_region(L, L.out_alt, 32 * (G.out.size() + 1));
     add_region(L, L.twin, sizeof(int) * (G.A + 1));
     add_region(L, L.dep_off, sizeof(i64) * (G.M + 1));
     add_region(L, L.dep_bits, sizeof(u32) * G.dep_bits.size());
@@ -140,6 +142,7 @@ DevGraph dev_graph(const efm_handle* h, unsigned char* ws) {
     g.col_ptr = (const int*)(ws + L.col_ptr.off);   g.col = (const int2*)(ws + L.col.off);
     g.in_ptr = (const int*)(ws + L.in_ptr.off);     g.in_e = (const int2*)(ws + L.in_e.off);
     g.out_ptr = (const int*)(ws + L.out_ptr.off);   g.out_e = (const int2*)(ws + L.out_e.off);
+    g.in_alt = (const uint4*)(ws + L.in_alt.off);   g.out_alt = (const uint4*)(ws + L.out_alt.off);
     g.twin = (const int*)(ws + L.twin.off);
     g.dep_off = (const i64*)(ws + L.dep_off.off);   g.dep_bits = (const u32*)(ws + L.dep_bits.off);
     g.arc_rxn = (const int*)(ws + L.arc_rxn.off);   g.arc_dir = (const int*)(ws + L.arc_dir.off);
@@ -147,6 +150,25 @@ DevGraph dev_graph(const efm_handle* h, unsigned char* ws) {
     g.max_coef = 0;
     for (const ColRef& c : h->G.col) g.max_coef = std::max(g.max_coef, c.s < 0 ? -c.s : c.s);
     return g;
+}
+
+// 32-byte records of the OR-alternatives (DevGraph::in_alt / out_alt): 8 words per entry of `list`.
+std::vector<uint32_t> alt_records(const HostGraph& G, const std::vector<ArcRef>& list) {
+    std::vector<uint32_t> out(list.size() * 8, 0u);
+    for (size_t q = 0; q < list.size(); ++q) {
+        const int a = list[q].arc, c = list[q].c;
+        const int n = G.col_ptr[a + 1] - G.col_ptr[a];
+        bool generic = n > 6 || c > 0xffff;
+        uint32_t* w = &out[q * 8];
+        for (int t = 0; t < n && t < 6; ++t) {
+            const ColRef& e = G.col[G.col_ptr[a] + t];
+            if (e.s > 32767 || e.s < -32767) generic = true;
+            w[2 + t] = (uint32_t)e.met | ((uint32_t)(uint16_t)(int16_t)e.s << 16);
+        }
+        w[0] = (uint32_t)a | ((uint32_t)(c & 0xffff) << 16);
+        w[1] = (uint32_t)(G.twin[a] < 0 ? 0xffff : G.twin[a]) | ((uint32_t)(n > 6 ? 0 : n) << 16) | ((generic ? 1u : 0u) << 24);
+    }
+    return out;
 }
 
 // Events for the optional per-phase timers.
@@ -355,6 +377,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         return cudaMemcpyAsync(ws + r.off, src, bytes, cudaMemcpyHostToDevice, s);
     };
     std::vector<u64> arc_mix;
+    std::vector<uint32_t> alt_in, alt_out;
     if (h->graph_ws != ws) {   // the network is an input: it stays resident in the workspace across calls
         h->graph_ws = nullptr;
         CK(up(L.col_ptr, G.col_ptr.data(), sizeof(int) * G.col_ptr.size()));
@@ -363,6 +386,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         CK(up(L.in_e, G.in.data(), sizeof(ArcRef) * G.in.size()));
         CK(up(L.out_ptr, G.out_ptr.data(), sizeof(int) * G.out_ptr.size()));
         CK(up(L.out_e, G.out.data(), sizeof(ArcRef) * G.out.size()));
+        alt_in = alt_records(G, G.in); alt_out = alt_records(G, G.out);
+        CK(up(L.in_alt, alt_in.data(), sizeof(uint32_t) * alt_in.size()));
+        CK(up(L.out_alt, alt_out.data(), sizeof(uint32_t) * alt_out.size()));
         CK(up(L.twin, G.twin.data(), sizeof(int) * G.twin.size()));
         CK(up(L.dep_off, G.dep_off.data(), sizeof(i64) * G.dep_off.size()));
         CK(up(L.dep_bits, G.dep_bits.data(), sizeof(u32) * G.dep_bits.size()));

@@ -42,6 +42,10 @@ struct DevGraph {
     const int* col_ptr;   const int2* col;    // {met, s}
     const int* in_ptr;    const int2* in_e;   // {arc, c}
     const int* out_ptr;   const int2* out_e;
+    // per entry of in_e / out_e one 32-byte record with everything the lane-parallel evaluation of that OR-alternative
+    // needs: {arc | c << 16, twin | ncol << 16 | generic << 24, 6 x (met | s << 16)}; generic = 1: the column has more
+    // than 6 entries or a number does not fit 16 bits, take the general routine
+    const uint4* in_alt;  const uint4* out_alt;
     const int* twin;
     const i64* dep_off;   const u32* dep_bits;
     const int* arc_rxn;   const int* arc_dir;

@@ -241,6 +241,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
 
         // ---- what to branch over: the OR-alternatives of i* (first visit) or the single Eq 4 / Eq 5 bump (revisit)
         const int2* alist = nullptr;
+        const uint4* altl = nullptr;
         int alen = 0, prim = -1;
         int r_a = 0, r_c = 1, r_sign = +1;
         u64 rec = 0, r_newrec = 0;
@@ -260,6 +261,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     if (bal) prim = __shfl_sync(FULL, pa, __ffs(bal) - 1);
                 }
                 alist = fwd ? A.g.out_e + out0 : A.g.in_e + in0;
+                altl = fwd ? A.g.out_alt + 2 * (size_t)out0 : A.g.in_alt + 2 * (size_t)in0;
                 alen = fwd ? nO : nI;
             }
         } else {
@@ -306,14 +308,17 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         for (int base = 0; base < alen; base += 32) {
             const int q = base + lane;
             int a = -1, c = 1;
-            bool adm = false, insup = false;
+            bool adm = false, insup = false, generic = false;
+            uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
             if (firstv) {
-                if (q < alen) {
-                    const int2 e = __ldg(&alist[q]);
-                    a = e.x; c = e.y;
-                    const int tw = __ldg(&A.g.twin[a]);
+                if (q < alen) {   // one 32-byte record per OR-alternative: arc, c, twin and the column of the arc
+                    r0 = __ldg(&altl[2 * q]); r1 = __ldg(&altl[2 * q + 1]);
+                    a = (int)(r0.x & 0xffffu); c = (int)(r0.x >> 16);
+                    const u32 tw = r0.y & 0xffffu;
+                    generic = (r0.y >> 24) & 1u;
+                    if (generic) c = __ldg(&alist[q]).y;   // the coefficient may not fit the record
                     insup = sbit(sbits, a);
-                    adm = !(tw >= 0 && sbit(sbits, tw)) && (insup || ns < A.D);
+                    adm = !(tw != 0xffffu && sbit(sbits, (int)tw)) && (insup || ns < A.D);
                 }
             } else if (lane == 0) {
                 a = r_a; c = r_c; adm = true; insup = true;   // PI / PO are arcs of the support
@@ -323,7 +328,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
             if (adm_m == 0) continue;
             n_adm += __popc(adm_m);
             // ---- lane-parallel evaluation: new arc, small integers => no overflow, no common factor
-            const bool fast = adm && !insup && fastP;
+            const bool fast = adm && !insup && fastP && !generic;
             const u32 fast_m = __ballot_sync(FULL, fast);
             u32 k = 1; u64 d = absE;
             int nu2 = nu;
@@ -331,13 +336,15 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
             if (fast_m) {
                 if (fast) {
                     if (c != 1) scale_small(absE, (u32)c, k, d);
-                    const int q1 = __ldg(&A.g.col_ptr[a + 1]);
-                    #pragma unroll 1
-                    for (int qq = __ldg(&A.g.col_ptr[a]); qq < q1; ++qq) {
-                        const int2 e = __ldg(&A.g.col[qq]);
-                        const i64 efp = ef_of(e.x);
-                        const i64 x = (i64)k * efp + (i64)d * (i64)e.y;   // |.| < 2^60 + 2^60
-                        nu2 += (int)(x != 0) - (int)(efp != 0);
+                    const int ncol = (int)((r0.y >> 16) & 0xffu);
+                    const u32 cw[6] = {r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+#pragma unroll
+                    for (int e = 0; e < 6; ++e) {
+                        if (e < ncol) {
+                            const i64 efp = ef_of((int)(cw[e] & 0xffffu));
+                            const i64 x = (i64)k * efp + (i64)d * (i64)(short)(cw[e] >> 16);   // |.| < 2^60 + 2^60
+                            nu2 += (int)(x != 0) - (int)(efp != 0);
+                        }
                     }
                 }
                 u64 hsb = Phs;

@@ -159,6 +159,19 @@ def test_parameter_edges(efm, oracle_mod):
     assert_parity(efm, oracle_mod, net, frontier_cap=2, seeds=oracle_mod.all_arc_seed_sets(net.reversible))
 
 
+def test_wide_columns_and_large_coefficients(efm, oracle_mod):
+    """Reactions whose column has more than 6 internal metabolites, or a coefficient beyond 16 bits, do not fit the
+    32-byte record of an OR-alternative: they are evaluated by the general routine."""
+    prods = {f"P{t}": 1 + t % 3 for t in range(8)}
+    rx = [({}, {"A": 1}, False), ({"A": 1}, prods, False), ({"A": 70000}, {"B": 3}, False), ({"B": 1}, {}, False),
+          ({"A": 2}, {"B": 70001}, True)]
+    rx += [({f"P{t}": 1}, {}, False) for t in range(8)]
+    net = hand_network(rx, ["A", "B"] + [f"P{t}" for t in range(8)])
+    got, ref = assert_parity(efm, oracle_mod, net, seeds=[[0]])
+    assert ref.stats["output"] >= 2
+    assert_parity(efm, oracle_mod, net, seeds=oracle_mod.all_arc_seed_sets(net.reversible))
+
+
 def test_overflow_guard(efm, oracle_mod):
     """Coefficient chains that multiply the scale past 2^62 (reading G21): both sides must discard identically."""
     names = [f"A{t}" for t in range(48)]
