@@ -6,10 +6,12 @@ namespace efm {
 
 // =================================================================================================================
 // a-4  Beam select: X = the key at sorted position `cap`; the level keeps exactly {key < X}.
-// MSD radix select over the 64-bit keys without a host round trip, three launches:
-//   k_select_hist    histogram of the top 11 bits over all keys; the last block (ticket) finds the bin holding rank cap
-//   k_select_narrow  copies the keys of that bin to a compact buffer; the last block finishes the remaining 53 bits on
-//                    the compact buffer alone (11/11/11/10/10-bit rounds in shared memory)
+// MSD radix select over the 64-bit keys without a host round trip:
+//   k_select_hist x2  histograms of the top 11 bits, then of the next 11 bits inside the selected bin (the top byte of a
+//                     key is n_unb, so the first level alone leaves an eighth of an n_unb class); the last block
+//                     (ticket) finds the bin holding rank cap
+//   k_select_narrow   copies the keys with the selected 22-bit prefix to a compact buffer; the last block finishes the
+//                     remaining 42 bits on the compact buffer alone (11/11/10/10-bit rounds in shared memory)
 // =================================================================================================================
 constexpr int kSelThreads = 256;
 constexpr int kTopBits = 11;
@@ -45,7 +47,9 @@ __device__ void block_find_bin(const u32* h, int nb, u64 rank, u32* s_bin, u64* 
     __syncthreads();
 }
 
-__global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restrict__ keys, Ctl* ctl, u64 max_keys) {
+// level 0: histogram of the top 11 bits of every key; level 1: of the next 11 bits of the keys inside the bin level 0
+// selected.  The last block (ticket) finds the bin that holds the wanted rank and extends the selected prefix.
+__global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restrict__ keys, Ctl* ctl, u64 max_keys, int level) {
     if (ctl->notrunc) return;
     __shared__ u32 h[SEL_BINS];
     __shared__ u64 scratch[kSelThreads];
@@ -53,6 +57,8 @@ __global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restri
     for (int b = threadIdx.x; b < SEL_BINS; b += kSelThreads) h[b] = 0;
     __syncthreads();
     const u64 n = min(ctl->n_slots, max_keys);   // an overflowed key array is reported by the host (ERR_KEYS)
+    const u64 top = ctl->sel_prefix;
+    const int shift = 64 - kTopBits * (level + 1);
     // keys of one parent are neighbours and share their top bits: aggregate runs of equal bins per thread
     constexpr int RUN = 4;
     for (u64 i0 = ((u64)blockIdx.x * kSelThreads + threadIdx.x) * RUN; i0 < n; i0 += (u64)gridDim.x * kSelThreads * RUN) {
@@ -62,7 +68,8 @@ __global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restri
             if (i0 + j >= n) break;
             const u64 key = keys[i0 + j];
             if (key >= kKeyDone) continue;   // filler of a reserved, unused slot / balanced child
-            const u32 b = (u32)(key >> (64 - kTopBits));
+            if (level == 1 && (key >> (64 - kTopBits)) != top) continue;
+            const u32 b = (u32)(key >> shift) & (u32)(SEL_BINS - 1);
             if (b != cur) { if (cnt) atomicAdd(&h[cur], cnt); cur = b; cnt = 0; }
             ++cnt;
         }
@@ -79,9 +86,11 @@ __global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restri
     for (int b = threadIdx.x; b < SEL_BINS; b += kSelThreads) { h[b] = ((volatile u32*)ctl->hist)[b]; ctl->hist[b] = 0; }
     __syncthreads();
     block_find_bin(h, SEL_BINS, ctl->sel_rank, &s_bin, &s_cum, scratch);
-    if (threadIdx.x == 0) { ctl->sel_prefix = s_bin; ctl->sel_rank -= s_cum; ctl->sel_ticket = 0; }
+    if (threadIdx.x == 0) { ctl->sel_prefix = (level == 0 ? 0ULL : top << kTopBits) | s_bin; ctl->sel_rank -= s_cum; ctl->sel_ticket = 0; }
 }
 
+// copies the keys that carry the selected 22-bit prefix to a compact buffer; the last block finishes the remaining
+// 42 bits on that buffer alone
 __global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __restrict__ keys, u64* __restrict__ ckeys, Ctl* ctl, u64 max_keys) {
     if (ctl->notrunc) return;
     __shared__ u32 h[SEL_BINS];
@@ -89,12 +98,13 @@ __global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __rest
     __shared__ u32 s_bin; __shared__ u64 s_cum; __shared__ bool is_last;
     const u64 n = min(ctl->n_slots, max_keys);
     const u64 top = ctl->sel_prefix;
+    constexpr int kLow = 64 - 2 * kTopBits;   // bits still open
     const int lane = threadIdx.x & 31;
     const u64 span = (u64)gridDim.x * kSelThreads;
     for (u64 base = (u64)blockIdx.x * kSelThreads; base < n; base += span) {   // warp-uniform trip count
         const u64 i = base + threadIdx.x;
         const u64 key = i < n ? keys[i] : kKeySentinel;
-        const bool hit = key < kKeyDone && (key >> (64 - kTopBits)) == top;
+        const bool hit = key < kKeyDone && (key >> kLow) == top;
         const u32 m = __ballot_sync(0xffffffffu, hit);
         if (m) {
             u64 pos = 0;
@@ -109,17 +119,16 @@ __global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __rest
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    // the remaining 53 bits on the compact buffer alone
     const u64 nc = *(volatile u64*)&ctl->n_compact;
     u64 rank = ctl->sel_rank, prefix = 0;
-    const int bits[5] = {11, 11, 11, 10, 10};
-    int shift = 64 - kTopBits;
-    for (int r = 0; r < 5; ++r) {
+    const int bits[4] = {11, 11, 10, 10};
+    int shift = kLow;
+    for (int r = 0; r < 4; ++r) {
         shift -= bits[r];
         const int nb = 1 << bits[r];
         for (int b = threadIdx.x; b < nb; b += kSelThreads) h[b] = 0;
         __syncthreads();
-        const u64 low = (1ULL << (64 - kTopBits)) - 1ULL;
+        const u64 low = (1ULL << kLow) - 1ULL;
         for (u64 i = threadIdx.x; i < nc; i += kSelThreads) {
             const u64 key = __ldcg(&ckeys[i]) & low;
             if (r == 0 || (key >> (shift + bits[r])) == prefix) atomicAdd(&h[(key >> shift) & (u64)(nb - 1)], 1u);
@@ -130,7 +139,7 @@ __global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __rest
         rank -= s_cum;
         __syncthreads();
     }
-    if (threadIdx.x == 0) { ctl->X = (top << (64 - kTopBits)) | prefix; ctl->sel_ticket = 0; }
+    if (threadIdx.x == 0) { ctl->X = (top << kLow) | prefix; ctl->sel_ticket = 0; }
 }
 
 cudaError_t launch_select(const u64* keys, u64* ckeys, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches) {
@@ -140,9 +149,10 @@ cudaError_t launch_select(const u64* keys, u64* ckeys, Ctl* ctl, u64 cap, u64 ma
     u64 blocks = (n_keys_hint + kSelThreads * 8 - 1) / (kSelThreads * 8);
     if (blocks > (u64)sm_count * 8) blocks = (u64)sm_count * 8;
     if (blocks < 1) blocks = 1;
-    k_select_hist<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ctl, max_keys);
+    k_select_hist<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ctl, max_keys, 0);
+    k_select_hist<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ctl, max_keys, 1);
     k_select_narrow<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ckeys, ctl, max_keys);
-    *n_launches += 2;
+    *n_launches += 3;
     return cudaGetLastError();
 }
 
