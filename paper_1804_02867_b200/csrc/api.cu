@@ -116,7 +116,7 @@ void make_layout(efm_handle* h) {
     add_region(L, L.r_nnz, C * 4);
     add_region(L, L.r_rxn, C * h->D * 4);
     add_region(L, L.r_val, C * h->D * 8);
-    add_region(L, L.csr_ptr, (C + 1) * 8);
+    add_region(L, L.csr_ptr, (C + 1 + C / 1024 + 2) * 8);   // row pointer + totals of its 1024-row scan blocks
     add_region(L, L.dense, h->dense_bytes);
     L.total = (L.total + 255) & ~(size_t)255;
     h->lay = L;

@@ -408,21 +408,29 @@ __device__ __forceinline__ int key_cmp(const ulonglong2 kx, const ulonglong2 ky)
     if (kx.y != ky.y) return kx.y < ky.y ? -1 : 1;
     return 0;
 }
-__global__ void __launch_bounds__(256) k_out_rows(const PostArgs a, u64 K) {
-    const u64 p = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+__global__ void __launch_bounds__(256) k_out_rows(const PostArgs a, u64 K) {   // one warp per kept row
+    const u64 p = (u64)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (p >= K || !a.keep[p]) return;
-    const u64 r = atomicAdd(&a.ctl->n_keep, 1ULL);
+    const int lane = threadIdx.x & 31;
+    u64 r = 0;
+    if (lane == 0) r = atomicAdd(&a.ctl->n_keep, 1ULL);
+    r = __shfl_sync(0xffffffffu, r, 0);
     const unsigned char* e = a.cand + (u64)a.uniq[p] * a.cand_stride;
     const int n = cand_n(e);
     const u16* arc = cand_arc(e, n);
     const i64* f = cand_flux(e);
-    a.u_nnz[r] = n;
-    for (int t = 0; t < n; ++t) {   // arcs ascend => reactions ascend (twins never share a support)
-        a.u_rxn[r * a.D + t] = a.g.arc_rxn[arc[t]];
-        a.u_val[r * a.D + t] = a.g.arc_dir[arc[t]] < 0 ? -f[t] : f[t];
+    if (lane == 0) a.u_nnz[r] = n;
+    int j01 = 0; i64 v01 = 0;   // lanes 0 and 1 keep the first two entries for the order codes
+    for (int t = lane; t < n; t += 32) {   // arcs ascend => reactions ascend (twins never share a support)
+        const int j = a.g.arc_rxn[arc[t]];
+        const i64 v = a.g.arc_dir[arc[t]] < 0 ? -f[t] : f[t];
+        a.u_rxn[r * a.D + t] = j;
+        a.u_val[r * a.D + t] = v;
+        if (t < 2) { j01 = j; v01 = v; }
     }
-    a.u_key[r] = make_ulonglong2(order_code(n > 0, n > 0 ? a.u_rxn[r * a.D] : 0, n > 0 ? a.u_val[r * a.D] : 0),
-                                 order_code(n > 1, n > 1 ? a.u_rxn[r * a.D + 1] : 0, n > 1 ? a.u_val[r * a.D + 1] : 0));
+    const int j1 = __shfl_sync(0xffffffffu, j01, 1);
+    const i64 v1 = __shfl_sync(0xffffffffu, v01, 1);
+    if (lane == 0) a.u_key[r] = make_ulonglong2(order_code(n > 0, j01, v01), order_code(n > 1, j1, v1));
 }
 
 // strict lexicographic "row x < row y" on the dense vectors, evaluated on the sparse rows
@@ -491,24 +499,41 @@ __global__ void __launch_bounds__(kSortChunk / 2) k_bitonic_local(const PostArgs
     }
     for (int t = threadIdx.x; t < kSortChunk; t += blockDim.x) if (base + t < a.n_pad) a.sort_idx[base + t] = s[t];
 }
-__global__ void __launch_bounds__(256) k_out_gather(const PostArgs a, u64 n_keep) {
-    const u64 r = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+__global__ void __launch_bounds__(256) k_out_gather(const PostArgs a, u64 n_keep) {   // one warp per row
+    const u64 r = (u64)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (r >= n_keep) return;
+    const int lane = threadIdx.x & 31;
     const u32 src = a.sort_idx[r];
     const int n = a.u_nnz[src];
-    a.r_nnz[r] = n;
-    for (int t = 0; t < n; ++t) { a.r_rxn[r * a.D + t] = a.u_rxn[(u64)src * a.D + t]; a.r_val[r * a.D + t] = a.u_val[(u64)src * a.D + t]; }
+    if (lane == 0) a.r_nnz[r] = n;
+    for (int t = lane; t < n; t += 32) { a.r_rxn[r * a.D + t] = a.u_rxn[(u64)src * a.D + t]; a.r_val[r * a.D + t] = a.u_val[(u64)src * a.D + t]; }
 }
 
-// Compressed rows (CSR) of the final result: row pointer by a one-block chunked scan, then one warp per row.
-__global__ void __launch_bounds__(1024) k_csr_scan(const int* __restrict__ r_nnz, u64 K, i64* __restrict__ row_ptr, Ctl* ctl) {
+// Compressed rows (CSR) of the final result: row pointer by a three-step scan (1024-row blocks, their totals, the sum),
+// then one warp per row.
+__global__ void __launch_bounds__(1024) k_csr_scan_blocks(const int* __restrict__ r_nnz, u64 K, i64* __restrict__ row_ptr, i64* __restrict__ totals) {
+    __shared__ i64 part[1024];
+    const u64 r = (u64)blockIdx.x * 1024 + threadIdx.x;
+    const i64 v = r < K ? r_nnz[r] : 0;
+    part[threadIdx.x] = v;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {
+        const i64 x = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
+        __syncthreads();
+        part[threadIdx.x] += x;
+        __syncthreads();
+    }
+    if (r < K) row_ptr[r] = part[threadIdx.x] - v;   // exclusive, block-local
+    if (threadIdx.x == 1023) totals[blockIdx.x] = part[1023];
+}
+__global__ void __launch_bounds__(1024) k_csr_scan_totals(i64* __restrict__ totals, u64 n_blocks, u64 K, i64* __restrict__ row_ptr, Ctl* ctl) {
     __shared__ i64 part[1024];
     __shared__ i64 carry;
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
-    for (u64 base = 0; base < K; base += 1024) {
-        const u64 r = base + threadIdx.x;
-        const i64 v = r < K ? r_nnz[r] : 0;
+    for (u64 base = 0; base < n_blocks; base += 1024) {
+        const u64 b = base + threadIdx.x;
+        const i64 v = b < n_blocks ? totals[b] : 0;
         part[threadIdx.x] = v;
         __syncthreads();
         for (int off = 1; off < 1024; off <<= 1) {
@@ -517,30 +542,37 @@ __global__ void __launch_bounds__(1024) k_csr_scan(const int* __restrict__ r_nnz
             part[threadIdx.x] += x;
             __syncthreads();
         }
-        if (r < K) row_ptr[r] = carry + part[threadIdx.x] - v;
+        if (b < n_blocks) totals[b] = carry + part[threadIdx.x] - v;   // exclusive offset of block b
         __syncthreads();
         if (threadIdx.x == 1023) carry += part[1023];
         __syncthreads();
     }
     if (threadIdx.x == 0) { row_ptr[K] = carry; ctl->csr_nnz = (u64)carry; }
 }
-__global__ void __launch_bounds__(256) k_csr_pack(const PostArgs a, u64 K, const i64* __restrict__ row_ptr, int* __restrict__ c_rxn, i64* __restrict__ c_val) {
+__global__ void __launch_bounds__(256) k_csr_pack(const PostArgs a, u64 K, i64* __restrict__ row_ptr, const i64* __restrict__ totals,
+                                                  int* __restrict__ c_rxn, i64* __restrict__ c_val) {
     const u64 r = (u64)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (r >= K) return;
     const int lane = threadIdx.x & 31, n = a.r_nnz[r];
-    const i64 o = row_ptr[r];
+    const i64 o = row_ptr[r] + totals[r >> 10];
+    __syncwarp();
+    if (lane == 0) row_ptr[r] = o;
     for (int t = lane; t < n; t += 32) { c_rxn[o + t] = a.r_rxn[r * a.D + t]; c_val[o + t] = a.r_val[r * a.D + t]; }
 }
 cudaError_t launch_output_csr(const PostArgs& a, u64 K, i64* row_ptr, int* c_rxn, i64* c_val, cudaStream_t s, int* n_launches) {
-    k_csr_scan<<<1, 1024, 0, s>>>(a.r_nnz, K, row_ptr, a.ctl);
+    // block totals live behind the row pointer (the region holds capacity + 1 + capacity / 1024 + 2 entries)
+    i64* totals = row_ptr + a.max_cand + 1;
+    const u64 nb = (K + 1023) / 1024;
+    if (nb) { k_csr_scan_blocks<<<(unsigned)nb, 1024, 0, s>>>(a.r_nnz, K, row_ptr, totals); ++*n_launches; }
+    k_csr_scan_totals<<<1, 1024, 0, s>>>(totals, nb, K, row_ptr, a.ctl);
     ++*n_launches;
-    if (K) { k_csr_pack<<<(unsigned)((K + 7) / 8), 256, 0, s>>>(a, K, row_ptr, c_rxn, c_val); ++*n_launches; }
+    if (K) { k_csr_pack<<<(unsigned)((K + 7) / 8), 256, 0, s>>>(a, K, row_ptr, totals, c_rxn, c_val); ++*n_launches; }
     return cudaGetLastError();
 }
 
 cudaError_t launch_output_rows(const PostArgs& a, u64 K, cudaStream_t s, int* n_launches) {
     if (K == 0) return cudaSuccess;
-    k_out_rows<<<(unsigned)((K + 255) / 256), 256, 0, s>>>(a, K);
+    k_out_rows<<<(unsigned)((K + 7) / 8), 256, 0, s>>>(a, K);
     ++*n_launches;
     return cudaGetLastError();
 }
@@ -558,7 +590,7 @@ cudaError_t launch_output_sort(const PostArgs& a, u64 n_keep, cudaStream_t s, in
         k_bitonic_local<<<chunks, kSortChunk / 2, 0, s>>>(a, k, k);
         ++*n_launches;
     }
-    k_out_gather<<<(unsigned)((n_keep + 255) / 256), 256, 0, s>>>(a, n_keep);
+    k_out_gather<<<(unsigned)((n_keep + 7) / 8), 256, 0, s>>>(a, n_keep);
     ++*n_launches;
     return cudaGetLastError();
 }
