@@ -576,20 +576,31 @@ __global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, c
     }
 }
 
-// ------------------------------------------------------------------ materialise: one warp per surviving child
+// ------------------------------------------------------------------ materialise: G lanes per surviving child
 // Reads the task, reads the parent entry straight from HBM / L2 (every element is needed once) and writes the child:
-// a candidate slot if it is balanced, otherwise a packed entry of the next frontier.  A block of kMatWarps children
-// reserves its output with one atomic per kind.
+// a candidate slot if it is balanced, otherwise a packed entry of the next frontier.  A block of 256 / G children
+// reserves its output with one atomic per kind.  G = 16 (two children per warp) suits entries of a few dozen arcs:
+// the per-child control flow and address arithmetic is shared by half as many instructions.
 #ifndef EFM_MAT_BLOCKS
 #define EFM_MAT_BLOCKS 4
 #endif
-constexpr int kMatWarps = 8;
-__global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(const __grid_constant__ ExpandArgs A) {
+#ifndef EFM_MAT_GROUP
+#define EFM_MAT_GROUP 16
+#endif
+constexpr int kMatThreads = 256;
+template <int G>
+__global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(const __grid_constant__ ExpandArgs A) {
+    constexpr int kMatWarps = kMatThreads / G;   // children per block
+    const u32 gbits = G == 32 ? 0xffffffffu : ((1u << (G & 31)) - 1u);
+    const u32 gmask = gbits << (threadIdx.x & 31 & ~(G - 1));   // lanes of this child
+    const int gshift = threadIdx.x & 31 & ~(G - 1);
+    auto gballot = [&](bool pred) -> u32 { return (__ballot_sync(gmask, pred) >> gshift) & gbits; };
+    auto gany = [&](bool pred) -> bool { return __any_sync(gmask, pred) != 0; };
     __shared__ u32 s_units[kMatWarps];
     __shared__ u64 s_base[kMatWarps];
     __shared__ u64 s_slot[kMatWarps];
     __shared__ u32 s_bytes[kMatWarps];
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int lane = threadIdx.x & (G - 1), wib = threadIdx.x / G;   // lane within the child's group, group within the block
     const u32 lt = (1u << lane) - 1u;
     Ctl* ctl = A.ctl;
     const u64 n_surv = ctl->n_surv;
@@ -629,17 +640,17 @@ __global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(
     const int nu2 = to_cand ? 0 : cnu;
     const u32 units = live ? (to_cand ? 0u : entry_bytes((u32)n2, (u32)nv2, (u32)nu2) >> 4) : 0u;
     // ---- every element of the parent this lane will need, requested before anything waits: the loads overlap each
-    // other and the block-wide reservation below (entries beyond 64 arcs / records are loaded where they are used)
+    // other and the block-wide reservation below (entries beyond 2 G arcs / records are loaded where they are used)
     u32 pa0 = 0xffffffffu, pa1 = 0xffffffffu, pm0 = 0xffffffffu;
     i64 pf0 = 0, pf1 = 0, pe0 = 0;
     u64 pv0 = 0, pv1 = 0;
     int pcol0 = 0, pcol1 = 0;
     if (live) {
         if (lane < ns) { pa0 = arc[lane]; pf0 = flux[lane]; }
-        if (lane + 32 < ns) { pa1 = arc[lane + 32]; pf1 = flux[lane + 32]; }
+        if (lane + G < ns) { pa1 = arc[lane + G]; pf1 = flux[lane + G]; }
         if (!to_cand) {
             if (lane < nv) pv0 = vis[lane];
-            if (lane + 32 < nv) pv1 = vis[lane + 32];
+            if (lane + G < nv) pv1 = vis[lane + G];
             if (lane < nu) { pm0 = efmet[lane]; pe0 = ef[lane]; }
             pcol0 = __ldg(&A.g.col_ptr[ca]); pcol1 = __ldg(&A.g.col_ptr[ca + 1]);
         }
@@ -680,10 +691,10 @@ __global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(
     // ---- write
     int ins = 0;   // a new arc goes where the ascending order puts it
     if (!cin)
-        for (int b2 = 0; b2 < ns; b2 += 32) {
+        for (int b2 = 0; b2 < ns; b2 += G) {
             const int t = b2 + lane;
-            const u32 at = b2 == 0 ? pa0 : (b2 == 32 ? pa1 : (t < ns ? (u32)arc[t] : 0xffffffffu));
-            ins += __popc(__ballot_sync(0xffffffffu, at < (u32)ca));
+            const u32 at = b2 == 0 ? pa0 : (b2 == G ? pa1 : (t < ns ? (u32)arc[t] : 0xffffffffu));
+            ins += __popc(gballot(at < (u32)ca));
         }
     i64* flux2 = (i64*)(dst + kHdr);
     u64* vis2 = (u64*)(flux2 + n2);
@@ -691,21 +702,21 @@ __global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(
     u16* arc2 = (u16*)(ef2 + nu2);
     u16* efmet2 = arc2 + n2;
     u64 mx = cin ? 0ULL : cT;   // a new arc never comes with a common divisor
-    for (int t = lane; t < ns; t += 32) {
-        const u64 ft = t < 32 ? (u64)pf0 : (t < 64 ? (u64)pf1 : (u64)flux[t]);
+    for (int t = lane; t < ns; t += G) {
+        const u64 ft = t < G ? (u64)pf0 : (t < 2 * G ? (u64)pf1 : (u64)flux[t]);
         u64 F = t == cia ? cT : ck * ft;
         if (cg > 1) F /= cg;
         const int pos = t + ((!cin && t >= ins) ? 1 : 0);
         flux2[pos] = (i64)F;
-        arc2[pos] = (u16)(t < 32 ? pa0 : (t < 64 ? pa1 : (u32)arc[t]));
+        arc2[pos] = (u16)(t < G ? pa0 : (t < 2 * G ? pa1 : (u32)arc[t]));
         mx = max(mx, F);
     }
     if (!cin && lane == 0) { flux2[ins] = (i64)cT; arc2[ins] = (u16)ca; }
     if (!to_cand) {
         // the visited record of i* is appended (first visit) or replaced (revisit)
         const u32 met_star = (u32)((newrec >> 32) & 0xffffu);
-        for (int u = lane; u < nv; u += 32) {
-            const u64 r = u < 32 ? pv0 : (u < 64 ? pv1 : vis[u]);
+        for (int u = lane; u < nv; u += G) {
+            const u64 r = u < G ? pv0 : (u < 2 * G ? pv1 : vis[u]);
             vis2[u] = (!firstv && (u32)((r >> 32) & 0xffffu) == met_star) ? newrec : r;
         }
         if (firstv && lane == 0) vis2[nv] = newrec;
@@ -715,7 +726,7 @@ __global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(
         const int qa0 = pcol0, qa1 = pcol1;
         int wbase = 0;
         u32 seen = 0;   // bit q - qa0: metabolite of col(a)[q] is in the parent's list (columns longer than 32: see below)
-        for (int t0 = 0; t0 < nu; t0 += 32) {
+        for (int t0 = 0; t0 < nu; t0 += G) {
             const int t = t0 + lane;
             const bool valid = t < nu;
             i64 x = 0;
@@ -728,8 +739,8 @@ __global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(
                 if (cg > 1) x /= (i64)cg;
             }
             for (int qq = qa0; qq < qa1 && qq < qa0 + 32; ++qq)
-                if (__any_sync(0xffffffffu, valid && __ldg(&A.g.col[qq]).x == met)) seen |= 1u << (qq - qa0);
-            const u32 nz = __ballot_sync(0xffffffffu, valid && x != 0);
+                if (gany(valid && __ldg(&A.g.col[qq]).x == met)) seen |= 1u << (qq - qa0);
+            const u32 nz = gballot(valid && x != 0);
             if (valid && x != 0) {
                 const int pos = wbase + __popc(nz & lt);
                 ef2[pos] = x; efmet2[pos] = (u16)met;
@@ -743,8 +754,8 @@ __global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(
             if (qq < qa0 + 32) in_parent = (seen >> (qq - qa0)) & 1u;
             else {   // columns longer than 32 entries: scan the parent's list again
                 bool f = false;
-                for (int t = lane; t < nu; t += 32) f = f || (int)efmet[t] == e.x;
-                in_parent = __any_sync(0xffffffffu, f);
+                for (int t = lane; t < nu; t += G) f = f || (int)efmet[t] == e.x;
+                in_parent = gany(f);
             }
             if (!in_parent) {
                 i64 x = (i64)(sd * (u64)(i64)e.y);
@@ -754,7 +765,12 @@ __global__ void __launch_bounds__(kMatWarps * 32, EFM_MAT_BLOCKS) k_materialise(
                 ++wbase;
             }
         }
-        mx = w_max(mx);
+        {   // maximum over the lanes of the child
+            const u32 hi = (u32)(mx >> 32);
+            const u32 mh = __reduce_max_sync(gmask, hi);
+            const u32 ml = __reduce_max_sync(gmask, hi == mh ? (u32)mx : 0u);
+            mx = ((u64)mh << 32) | ml;
+        }
     }
     if (lane == 0) {
         uint4* h4 = (uint4*)dst;
@@ -892,7 +908,7 @@ cudaError_t launch_materialise(const ExpandArgs& a, u64 n_slots_hint, u64 n_surv
         return cudaGetLastError();
     }
     (void)n_surv;   // read on the device (ctl->n_surv): no host round trip between the two kernels
-    k_materialise<<<(unsigned)(sm_count * 32), kMatWarps * 32, 0, s>>>(a);
+    k_materialise<EFM_MAT_GROUP><<<(unsigned)(sm_count * 32), kMatThreads, 0, s>>>(a);
     return cudaGetLastError();
 }
 
