@@ -37,10 +37,18 @@ constexpr u64 kSmall = 1ULL << 40;   // fast path: every flux and extra flux of 
 constexpr int kSmallCoef = 1 << 20;  // ... and every coefficient below this: no product can reach 2^62
 
 // ------------------------------------------------------------------ warp collectives
-__device__ __forceinline__ u64 w_sum(u64 v) {
+// Collectives over a group of G consecutive lanes (G = 32: the warp); `m` is the lane mask of the group.
+template <int G>
+__device__ __forceinline__ u64 g_sum(u32 m, u64 v) {
 #pragma unroll
-    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+    for (int o = G / 2; o; o >>= 1) v += __shfl_xor_sync(m, v, o);
     return v;
+}
+__device__ __forceinline__ u64 g_max(u32 m, u64 v) {   // two 32-bit redux instead of 64-bit shuffle rounds
+    const u32 hi = (u32)(v >> 32);
+    const u32 mh = __reduce_max_sync(m, hi);
+    const u32 ml = __reduce_max_sync(m, hi == mh ? (u32)v : 0u);
+    return ((u64)mh << 32) | ml;
 }
 __device__ __forceinline__ u64 w_max(u64 v) {   // two 32-bit redux instead of five 64-bit shuffle rounds
     const u32 hi = (u32)(v >> 32);
@@ -76,15 +84,16 @@ __device__ __forceinline__ u32 gcd32(u32 a, u32 b) {
     } while (b);
     return a << sh;
 }
-__device__ __forceinline__ u64 w_gcd(u64 v, bool narrow) {
+template <int G>
+__device__ __forceinline__ u64 g_gcd(u32 m, u64 v, bool narrow) {
     if (narrow) {   // every value below 2^32
         u32 x = (u32)v;
 #pragma unroll
-        for (int o = 16; o; o >>= 1) { const u32 w = __shfl_xor_sync(FULL, x, o); x = gcd32(x, w); }
+        for (int o = G / 2; o; o >>= 1) { const u32 w = __shfl_xor_sync(m, x, o); x = gcd32(x, w); }
         return x;
     }
 #pragma unroll
-    for (int o = 16; o; o >>= 1) { const u64 w = __shfl_xor_sync(FULL, v, o); v = gcd64(v, w); }
+    for (int o = G / 2; o; o >>= 1) { const u64 w = __shfl_xor_sync(m, v, o); v = gcd64(v, w); }
     return v;
 }
 struct S128 { u64 lo; i64 hi; };
@@ -105,19 +114,21 @@ __device__ __forceinline__ u64 arc_term_t(const DevGraph& g, u32 a, u64 f) { ret
 
 // Per-warp chunked reservation of beam-key slots: one atomic per kKeyChunk keys instead of one per child.
 constexpr u64 kNoSlot = ~0ULL;
+template <int G>
 struct KeyOut {
     u64 base; u32 left;
+    u32 gmask; int gshift;   // lanes of the group that owns the chunk
     // one slot for every lane with want = true (others, and everyone after an overflow, get kNoSlot)
     __device__ __forceinline__ u64 reserve(const ExpandArgs& A, int lane, bool want) {
-        const u32 m = __ballot_sync(FULL, want);
+        const u32 m = (__ballot_sync(gmask, want) >> gshift) & (G == 32 ? 0xffffffffu : ((1u << (G & 31)) - 1u));
         const u32 cnt = (u32)__popc(m);
         if (cnt == 0) return kNoSlot;
         if (cnt > left) {
 #pragma unroll 1
-            for (u32 t = lane; t < left; t += 32) A.keys[base + t] = kKeySentinel;
+            for (u32 t = lane; t < left; t += G) A.keys[base + t] = kKeySentinel;
             u64 b = 0;
             if (lane == 0) b = atomicAdd(&A.ctl->n_slots, (u64)kKeyChunk);
-            b = w_bcast(b, 0);
+            b = __shfl_sync(gmask, b, 0, G);
             if (b + kKeyChunk > A.max_keys) {
                 if (lane == 0) atomicOr(&A.ctl->error, (u32)ERR_KEYS);
                 left = 0;
@@ -130,7 +141,7 @@ struct KeyOut {
         return slot;
     }
     __device__ __forceinline__ void finish(const ExpandArgs& A, int lane) {
-        for (u32 t = lane; t < left; t += 32) A.keys[base + t] = kKeySentinel;
+        for (u32 t = lane; t < left; t += G) A.keys[base + t] = kKeySentinel;
         left = 0;
     }
 };
@@ -155,10 +166,17 @@ enum { SS_EXPANDED = 0, SS_CHILDREN, SS_DONE, SS_ACTIVE, SS_DEAD, SS_NOTEFM, SS_
 // compiler can track.  The kernel only EVALUATES: every child that passes the discard tests gets a slot holding its
 // beam key and a 64-byte task (what k_materialise needs to build it from its parent); nothing is written to the next
 // frontier here, so a parent with hundreds of surviving children costs this warp no more than one without any.
+template <int G>
 __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_constant__ ExpandArgs A) {
     extern __shared__ uint4 smem4[];
-    const int lane = threadIdx.x & 31;
-    const int wib = threadIdx.x >> 5;
+    // a group of G consecutive lanes owns a parent (G = 32: the warp; G = 16: two parents per warp share the issue slots
+    // of the control flow they have in common)
+    const int lane = threadIdx.x & (G - 1);
+    const int wib = threadIdx.x / G;
+    const u32 gbits = G == 32 ? 0xffffffffu : ((1u << (G & 31)) - 1u);
+    const int gshift = threadIdx.x & 31 & ~(G - 1);
+    const u32 gmask = gbits << gshift;
+    auto gballot = [&](bool pred) -> u32 { return (__ballot_sync(gmask, pred) >> gshift) & gbits; };
     const u32 lt = (1u << lane) - 1u;
     unsigned char* gs = (unsigned char*)smem4 + (size_t)wib * A.sm_group;
     uint4* stage = (uint4*)gs;
@@ -166,18 +184,18 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
     u16* upos = (u16*)(gs + A.sm_upos);     // metabolite -> 1 + index in the EF list of the parent, 0 = balanced
     u64* sst = (u64*)(gs + A.sm_misc);
     #pragma unroll 1
-    for (int i = lane; i < A.g.W32; i += 32) sbits[i] = 0;
+    for (int i = lane; i < A.g.W32; i += G) sbits[i] = 0;
     #pragma unroll 1
-    for (int i = lane; i < (A.g.M + 8) / 8; i += 32) ((uint4*)upos)[i] = make_uint4(0, 0, 0, 0);
-    if (lane < SS_WORDS) sst[lane] = 0;
-    __syncwarp();
+    for (int i = lane; i < (A.g.M + 8) / 8; i += G) ((uint4*)upos)[i] = make_uint4(0, 0, 0, 0);
+    for (int i = lane; i < SS_WORDS; i += G) sst[i] = 0;
+    __syncwarp(gmask);
 
     Ctl* ctl = A.ctl;
     const bool fast_graph = !A.no_fast && A.g.max_coef < kSmallCoef;
-    KeyOut ko; ko.base = 0; ko.left = 0;
+    KeyOut<G> ko; ko.base = 0; ko.left = 0; ko.gmask = gmask; ko.gshift = gshift;
     // a warp owns A.ppw (<= kParentsPerWarp) consecutive parents; the grid covers the level and the block scheduler evens out the
     // very different costs of parents (skipped / first visit over a hub / revisit)
-    const u64 p0 = ((u64)blockIdx.x * (blockDim.x >> 5) + wib) * A.ppw;
+    const u64 p0 = ((u64)blockIdx.x * (blockDim.x / G) + wib) * A.ppw;
     const u64 p1 = min(p0 + A.ppw, A.n_cur);
 
 #pragma unroll 1
@@ -185,21 +203,21 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
         const uint4* src = (const uint4*)(A.cur + (__ldcs(&A.cur_off[p]) << 4));
         const uint4 first16 = __ldcs(src + lane);   // the buffers end in 512 spare bytes
-        const u32 hdr = __shfl_sync(FULL, first16.x, 0);
+        const u32 hdr = __shfl_sync(gmask, first16.x, 0, G);
         const int ns = (int)(hdr & 0xffffu), nv = (int)(hdr >> 16);
-        const int nu = (int)__shfl_sync(FULL, first16.y, 0);
+        const int nu = (int)__shfl_sync(gmask, first16.y, 0, G);
         const u32 nch = entry_bytes((u32)ns, (u32)nv, (u32)nu) / 16;
         // entries that fit the staging buffer are copied to shared memory; the rare larger ones are read in place
         const bool staged = nch * 16 <= A.sm_stage_bytes;
         if (staged) {
             if ((u32)lane < nch) stage[lane] = first16;
             #pragma unroll 1
-            for (u32 c = lane + 32; c < nch; c += 32) stage[c] = __ldcs(src + c);   // streaming: the frontier must not evict the graph from L1
+            for (u32 c = lane + G; c < nch; c += G) stage[c] = __ldcs(src + c);   // streaming: the frontier must not evict the graph from L1
         }
-        __syncwarp();
-        const u64 Phs = (u64)__shfl_sync(FULL, first16.z, 0) | ((u64)__shfl_sync(FULL, first16.w, 0) << 32);
-        const u64 Phv = (u64)__shfl_sync(FULL, first16.x, 1) | ((u64)__shfl_sync(FULL, first16.y, 1) << 32);
-        const u64 Pbig = (u64)__shfl_sync(FULL, first16.z, 1) | ((u64)__shfl_sync(FULL, first16.w, 1) << 32);
+        __syncwarp(gmask);
+        const u64 Phs = (u64)__shfl_sync(gmask, first16.z, 0, G) | ((u64)__shfl_sync(gmask, first16.w, 0, G) << 32);
+        const u64 Phv = (u64)__shfl_sync(gmask, first16.x, 1, G) | ((u64)__shfl_sync(gmask, first16.y, 1, G) << 32);
+        const u64 Pbig = (u64)__shfl_sync(gmask, first16.z, 1, G) | ((u64)__shfl_sync(gmask, first16.w, 1, G) << 32);
         const unsigned char* eb = staged ? (const unsigned char*)gs : (const unsigned char*)src;
         const i64* flux = (const i64*)(eb + kHdr);
         const u64* vis = (const u64*)(flux + ns);
@@ -209,17 +227,17 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
 
         // ---- support bitset, EF index table, PROC0: lowest unbalanced metabolite i* (reading G12)
         #pragma unroll 1
-        for (int t = lane; t < ns; t += 32) { const u32 a = arc[t]; atomicOr(&sbits[a >> 5], 1u << (a & 31)); }
+        for (int t = lane; t < ns; t += G) { const u32 a = arc[t]; atomicOr(&sbits[a >> 5], 1u << (a & 31)); }
         u32 best = 0xffffffffu;
         #pragma unroll 1
-        for (int t = lane; t < nu; t += 32) {
+        for (int t = lane; t < nu; t += G) {
             const u32 i = efmet[t];
             upos[i] = (u16)(t + 1);
             best = min(best, (i << 16) | (u32)t);
         }
-        best = __reduce_min_sync(FULL, best);
+        best = __reduce_min_sync(gmask, best);
         if (lane == 0) { sst[SS_KC] = 0; sst[SS_KC + 2] = 0; }
-        __syncwarp();
+        __syncwarp(gmask);
         const int istar = (int)(best >> 16);
         const i64 E = ef[best & 0xffffu];
         const bool fwd = E > 0;
@@ -229,9 +247,9 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         // visited?
         int vk = -1;
         #pragma unroll 1
-        for (int base = 0; base < nv && vk < 0; base += 32) {
+        for (int base = 0; base < nv && vk < 0; base += G) {
             const int u = base + lane;
-            const u32 hit = __ballot_sync(FULL, u < nv && (int)((vis[u] >> 32) & 0xffffu) == istar);
+            const u32 hit = gballot(u < nv && (int)((vis[u] >> 32) & 0xffffu) == istar);
             if (hit) vk = base + __ffs(hit) - 1;
         }
         const bool firstv = vk < 0;
@@ -254,11 +272,11 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 const int2* plist = fwd ? A.g.in_e + in0 : A.g.out_e + out0;
                 const int plen = fwd ? nI : nO;
                 #pragma unroll 1
-                for (int base = 0; base < plen && prim < 0; base += 32) {
+                for (int base = 0; base < plen && prim < 0; base += G) {
                     const int q = base + lane;
                     const int pa = q < plen ? __ldg(&plist[q]).x : -1;
-                    const u32 bal = __ballot_sync(FULL, pa >= 0 && sbit(sbits, pa));
-                    if (bal) prim = __shfl_sync(FULL, pa, __ffs(bal) - 1);
+                    const u32 bal = gballot(pa >= 0 && sbit(sbits, pa));
+                    if (bal) prim = __shfl_sync(gmask, pa, __ffs(bal) - 1, G);
                 }
                 alist = fwd ? A.g.out_e + out0 : A.g.in_e + in0;
                 altl = fwd ? A.g.out_alt + 2 * (size_t)out0 : A.g.in_alt + 2 * (size_t)in0;
@@ -274,28 +292,28 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 const int PI = (int)((rec >> 16) & 0xffffu), PO = (int)(rec & 0xffffu);
                 int lPI = -1, lPO = -1, cPI = 0, cPO = 0;
                 #pragma unroll 1
-                for (int q = lane; q < nI; q += 32) { const int2 e = __ldg(&A.g.in_e[in0 + q]); if (e.x == PI) { lPI = q; cPI = e.y; } }
+                for (int q = lane; q < nI; q += G) { const int2 e = __ldg(&A.g.in_e[in0 + q]); if (e.x == PI) { lPI = q; cPI = e.y; } }
                 #pragma unroll 1
-                for (int q = lane; q < nO; q += 32) { const int2 e = __ldg(&A.g.out_e[out0 + q]); if (e.x == PO) { lPO = q; cPO = e.y; } }
-                lPI = __reduce_max_sync(FULL, lPI); cPI = __reduce_max_sync(FULL, cPI);
-                lPO = __reduce_max_sync(FULL, lPO); cPO = __reduce_max_sync(FULL, cPO);
+                for (int q = lane; q < nO; q += G) { const int2 e = __ldg(&A.g.out_e[out0 + q]); if (e.x == PO) { lPO = q; cPO = e.y; } }
+                lPI = __reduce_max_sync(gmask, lPI); cPI = __reduce_max_sync(gmask, cPI);
+                lPO = __reduce_max_sync(gmask, lPO); cPO = __reduce_max_sync(gmask, cPO);
                 // Def 11: forward PO ~ SI, backward PI ~ SO, secondary = any arc of that side in the support (G5)
                 bool dep = false;
                 const i64 doff = __ldg(&A.g.dep_off[istar]);
                 if (fwd) {
                     #pragma unroll 1
-                    for (int q = lane; q < nI; q += 32) {
+                    for (int q = lane; q < nI; q += G) {
                         const i64 b = doff + (i64)lPO * nI + q;
                         dep = dep || (sbit(sbits, __ldg(&A.g.in_e[in0 + q]).x) && ((__ldg(&A.g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
                     }
                 } else {
                     #pragma unroll 1
-                    for (int q = lane; q < nO; q += 32) {
+                    for (int q = lane; q < nO; q += G) {
                         const i64 b = doff + (i64)q * nI + lPI;
                         dep = dep || (sbit(sbits, __ldg(&A.g.out_e[out0 + q]).x) && ((__ldg(&A.g.dep_bits[b >> 5]) >> (b & 31)) & 1u));
                     }
                 }
-                dep = __any_sync(FULL, dep);
+                dep = __any_sync(gmask, dep);
                 if (fwd) { if (!dep) { r_a = PO; r_c = cPO; r_sign = +1; } else { r_a = PI; r_c = cPI; r_sign = -1; } }   // Eq 4 / Eq 5
                 else     { if (!dep) { r_a = PI; r_c = cPI; r_sign = +1; } else { r_a = PO; r_c = cPO; r_sign = -1; } }
                 r_newrec = vis_pack((u32)istar, (u32)PI, (u32)PO, (u32)cntv);
@@ -305,7 +323,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         const bool fastP = firstv && fast_graph && Pbig < kSmall;
         int n_adm = 0;
         #pragma unroll 1
-        for (int base = 0; base < alen; base += 32) {
+        for (int base = 0; base < alen; base += G) {
             const int q = base + lane;
             int a = -1, c = 1;
             bool adm = false, insup = false, generic = false;
@@ -324,12 +342,12 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 a = r_a; c = r_c; adm = true; insup = true;   // PI / PO are arcs of the support
             }
             if (lane == 0) sst[SS_ROUNDS]++;
-            const u32 adm_m = __ballot_sync(FULL, adm);
+            const u32 adm_m = gballot(adm);
             if (adm_m == 0) continue;
             n_adm += __popc(adm_m);
             // ---- lane-parallel evaluation: new arc, small integers => no overflow, no common factor
             const bool fast = adm && !insup && fastP && !generic;
-            const u32 fast_m = __ballot_sync(FULL, fast);
+            const u32 fast_m = gballot(fast);
             u32 k = 1; u64 d = absE;
             int nu2 = nu;
             u64 hs2 = 0, hv2 = 0, key = 0;
@@ -348,25 +366,25 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     }
                 }
                 u64 hsb = Phs;
-                u32 need = __ballot_sync(FULL, fast && k > 1);
+                u32 need = gballot(fast && k > 1);
                 #pragma unroll 1
                 while (need) {
-                    const u32 kk = __shfl_sync(FULL, k, __ffs(need) - 1);
+                    const u32 kk = __shfl_sync(gmask, k, __ffs(need) - 1, G);
                     u64 s;
                     if ((u64)kk == sst[SS_KC]) s = sst[SS_KC + 1];
                     else if ((u64)kk == sst[SS_KC + 2]) s = sst[SS_KC + 3];
                     else {
                         s = 0;
                         #pragma unroll 1
-                        for (int t = lane; t < ns; t += 32) s += arc_term_t(A.g, (u32)arc[t], (u64)kk * (u64)flux[t]);
-                        s = w_sum(s);
-                        __syncwarp();
+                        for (int t = lane; t < ns; t += G) s += arc_term_t(A.g, (u32)arc[t], (u64)kk * (u64)flux[t]);
+                        s = g_sum<G>(gmask, s);
+                        __syncwarp(gmask);
                         if (lane == 0) { sst[SS_KC + 2] = sst[SS_KC]; sst[SS_KC + 3] = sst[SS_KC + 1]; sst[SS_KC] = kk; sst[SS_KC + 1] = s; }
-                        __syncwarp();
+                        __syncwarp(gmask);
                     }
                     const bool same = fast && k == kk;
                     if (same) hsb = s;
-                    need &= ~__ballot_sync(FULL, same);
+                    need &= ~gballot(same);
                 }
                 if (fast) {
                     const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : a), (u32)(fwd ? a : prim), 0u);
@@ -375,7 +393,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     key = beam_key((u32)nu2, mix64(hs2 + hv2));
                 }
             }
-            const u32 done_m = __ballot_sync(FULL, fast && nu2 == 0);
+            const u32 done_m = gballot(fast && nu2 == 0);
             if (lane == 0) {
                 const int nf = __popc(fast_m);
                 sst[SS_CHILDREN] += nf; sst[SS_BYTES] += 8 * nf; sst[SS_DONE] += __popc(done_m); sst[SS_ACTIVE] += __popc(fast_m & ~done_m);
@@ -399,7 +417,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 const int l = __ffs(slow_m) - 1;
                 slow_m &= slow_m - 1;
                 // warp-uniform description of the child relative to its parent
-                const int ca = __shfl_sync(FULL, a, l);
+                const int ca = __shfl_sync(gmask, a, l, G);
                 u64 ck, cd, cT, cg = 1, chs, chv;   // scale, |E| / gcd(|E|, c), un-normalised new flux of ca, common divisor, hash sums
                 int cnu = nu, csign = +1, cia = -1;
                 bool cin = false;
@@ -407,7 +425,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 const int qa0 = __ldg(&A.g.col_ptr[ca]), qa1 = __ldg(&A.g.col_ptr[ca + 1]);
                 {
                 // bump(f, a, sign*|E|/c) of SURVEY.md 8(c) O6 with the whole warp
-                const int cc = __shfl_sync(FULL, c, l);
+                const int cc = __shfl_sync(gmask, c, l, G);
                 csign = firstv ? +1 : r_sign;
                 const u64 gg = cc == 1 ? 1ULL : gcd64(absE, (u64)cc);
                 ck = gg == 1 ? (u64)cc : (u64)cc / gg;
@@ -415,9 +433,9 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 cin = sbit(sbits, ca);
                 if (cin) {   // position of the arc in the sorted support
                     #pragma unroll 1
-                    for (int b2 = 0; b2 < ns && cia < 0; b2 += 32) {
+                    for (int b2 = 0; b2 < ns && cia < 0; b2 += G) {
                         const int t = b2 + lane;
-                        const u32 hit = __ballot_sync(FULL, t < ns && arc[t] == ca);
+                        const u32 hit = gballot(t < ns && arc[t] == ca);
                         if (hit) cia = b2 + __ffs(hit) - 1;
                     }
                 }
@@ -441,8 +459,8 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 if (bigk) {   // exact: the largest flux among t != ia (a new arc carries d <= |E| <= 2^62)
                     u64 mx = 0;
                     #pragma unroll 1
-                    for (int t = lane; t < ns; t += 32) if (t != cia) mx = max(mx, (u64)flux[t]);
-                    mx = w_max(mx);
+                    for (int t = lane; t < ns; t += G) if (t != cia) mx = max(mx, (u64)flux[t]);
+                    mx = g_max(gmask, mx);
                     ovf = ovf || umul_gt_guard(ck, mx);
                 }
                 int status = ovf ? CH_OVERFLOW : (nonpos ? CH_NONPOS : CH_OK);   // Prop 3, G11
@@ -451,7 +469,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     bool ovf2 = false;
                     if (bigk) {   // exact sweep over the unbalanced metabolites outside col(a)
                         #pragma unroll 1
-                        for (int t = lane; t < nu; t += 32) {
+                        for (int t = lane; t < nu; t += G) {
                             const int i = efmet[t];
                             bool in_a = false;
                             #pragma unroll 1
@@ -461,15 +479,15 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     }
                     int delta = 0;
                     #pragma unroll 1
-                    for (int qq = qa0 + lane; qq < qa1; qq += 32) {
+                    for (int qq = qa0 + lane; qq < qa1; qq += G) {
                         const int2 e = __ldg(&A.g.col[qq]);
                         const i64 efp = ef_of(e.x);
                         const S128 x = add_s(mul_s((i64)ck, efp), mul_s(csign > 0 ? (i64)cd : -(i64)cd, (i64)e.y));
                         ovf2 = ovf2 || abs_gt_guard(x);
                         delta += (int)((x.lo | (u64)x.hi) != 0) - (int)(efp != 0);
                     }
-                    if (__any_sync(FULL, ovf2)) status = CH_OVERFLOW;
-                    else cnu = nu + __reduce_add_sync(FULL, delta);
+                    if (__any_sync(gmask, ovf2)) status = CH_OVERFLOW;
+                    else cnu = nu + __reduce_add_sync(gmask, delta);
                 }
                 if (status != CH_OK) {
                     if (lane == 0) sst[status == CH_OVERFLOW ? SS_OVF : SS_NONPOS]++;
@@ -483,7 +501,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     const bool narrow = cT < (1ULL << 32);
                     u64 r = cT;
                     #pragma unroll 1
-                    for (int t = lane; t < ns; t += 32) {
+                    for (int t = lane; t < ns; t += G) {
                         if (t == cia) continue;
                         const u64 x = ck * (u64)flux[t];   // <= 2^62 (no overflow was found above)
                         if (narrow) {
@@ -491,19 +509,19 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                             r = gcd32(r32, (x >> 32) == 0 ? (u32)x % r32 : (u32)(x % (u64)r32));
                         } else r = gcd64(r, x);
                     }
-                    if (!__any_sync(FULL, r == 1)) cg = w_gcd(r, narrow);
+                    if (!__any_sync(gmask, r == 1)) cg = g_gcd<G>(gmask, r, narrow);
                 }
                 if (ck == 1 && cg == 1) {
                     chs = Phs + arc_term_t(A.g, (u32)ca, cT) - (cin ? arc_term_t(A.g, (u32)ca, (u64)flux[cia]) : 0ULL);
                 } else {
                     chs = 0;
                     #pragma unroll 1
-                    for (int t = lane; t < ns; t += 32) {
+                    for (int t = lane; t < ns; t += G) {
                         u64 F = t == cia ? cT : ck * (u64)flux[t];
                         if (cg > 1) F /= cg;
                         chs += arc_term_t(A.g, (u32)arc[t], F);
                     }
-                    chs = w_sum(chs);
+                    chs = g_sum<G>(gmask, chs);
                     if (!cin) chs += arc_term_t(A.g, (u32)ca, cT);
                 }
                 chv = Phv + vis_term(newrec) - (firstv ? 0ULL : vis_term(rec));
@@ -524,15 +542,15 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         }
         if (firstv && nv < A.V && n_adm == 0 && lane == 0) sst[SS_DEAD]++;   // no admissible alternative
         // ---- restore the shared tables to zero for the next parent
-        __syncwarp();
+        __syncwarp(gmask);
         #pragma unroll 1
-        for (int t = lane; t < ns; t += 32) sbits[arc[t] >> 5] = 0;
+        for (int t = lane; t < ns; t += G) sbits[arc[t] >> 5] = 0;
         #pragma unroll 1
-        for (int t = lane; t < nu; t += 32) upos[efmet[t]] = 0;
-        __syncwarp();
+        for (int t = lane; t < nu; t += G) upos[efmet[t]] = 0;
+        __syncwarp(gmask);
     }
     ko.finish(A, lane);
-    __syncwarp();
+    __syncwarp(gmask);
     if (lane == 0) {
         u64* st = ctl->st;
         if (sst[SS_EXPANDED]) { atomicAdd(&st[ST_EXPANDED], sst[SS_EXPANDED]); atomicAdd(&ctl->lvl_expanded, sst[SS_EXPANDED]); }
@@ -872,29 +890,35 @@ void expand_smem_layout(ExpandArgs& a) {
 
 // key slots the count pass can leave unused: every warp of the largest grid may strand one chunk
 // every warp may strand one chunk of key slots; a warp covers kParentsPerWarp parents
-u64 expand_key_slack(u64 max_parents) { return (max_parents / kParentsPerWarp + 16384) * kKeyChunk; }
+u64 expand_key_slack(u64 max_parents) { return (max_parents / kParentsPerWarp + 32768) * kKeyChunk; }
 
+#ifndef EFM_EXP_GROUP
+#define EFM_EXP_GROUP 32   // lanes per parent in k_expand (measured on genome / cap 262144: 32 -> 44 ms, 16 -> 64 ms, 8 -> 119 ms:
+                           // the parents of a warp diverge too much to share issue slots, unlike k_materialise)
+#endif
 cudaError_t launch_expand(const ExpandArgs& a, int sm_count, cudaStream_t s) {
-    // warps per block: as many as fit beside the per-warp staging (huge networks fall back to fewer warps)
+    constexpr int G = EFM_EXP_GROUP;
+    // groups per block: as many as fit beside the per-group staging (huge networks fall back to fewer warps)
     int warps = kWarps;
-    while (warps > 1 && (size_t)a.sm_group * warps > 200 * 1024) warps >>= 1;
-    const size_t smem = (size_t)a.sm_group * warps;
+    while (warps > 1 && (size_t)a.sm_group * warps * (32 / G) > 200 * 1024) warps >>= 1;
+    const int groups = warps * (32 / G);
+    const size_t smem = (size_t)a.sm_group * groups;
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_expand, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_expand<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    // small levels: fewer parents per warp so that every SM still gets its share of warps
-    u64 ppw = a.n_cur / ((u64)sm_count * 32);
+    // small levels: fewer parents per group so that every SM still gets its share of warps
+    u64 ppw = a.n_cur / ((u64)sm_count * 32 * (32 / G));
     ppw = ppw < 1 ? 1 : (ppw > (u64)kParentsPerWarp ? (u64)kParentsPerWarp : ppw);
     ExpandArgs a2 = a;
     a2.ppw = (u32)ppw;
-    const u64 per_block = (u64)warps * ppw;
+    const u64 per_block = (u64)groups * ppw;
     const u64 need = (a.n_cur + per_block - 1) / per_block;
     if (need > 0x7fffffffULL) return cudaErrorInvalidValue;
-    k_expand<<<(unsigned)(need ? need : 1), warps * 32, smem, s>>>(a2);
+    k_expand<G><<<(unsigned)(need ? need : 1), warps * 32, smem, s>>>(a2);
     return cudaGetLastError();
 }
 
