@@ -234,6 +234,7 @@ def main_ours(args):
         gi = en2.graph_info()
         h2d = 8 * (2 * gi["nnz"]) + 4 * (3 * gi["A"] + 2 * gi["M"]) * 2 + gi["dep_entries"] // 8 + int(r2.stats["n_roots"]) * 64
         d2h = (row_ptr.numel() * 8 + rxn.numel() * 4 + val.numel() * 8 + int(r2.stats["levels"]) * 256)
+        del row_ptr, rxn, val   # back to torch's pinned-memory cache: the next step reuses the buffers
         en2.close()
     barrier()
 
