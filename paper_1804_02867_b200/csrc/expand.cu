@@ -60,7 +60,12 @@ __device__ __forceinline__ u64 w_min(u64 v) { return ~w_max(~v); }
 __device__ __forceinline__ u64 w_bcast(u64 v, int src) { return __shfl_sync(FULL, v, src); }
 
 // ------------------------------------------------------------------ integer helpers
-__device__ __forceinline__ u64 gcd64(u64 a, u64 b) {   // binary gcd
+// The rarely taken arithmetic (64-bit division, gcd) stays out of line: inlined at every site it was almost half of the
+// kernel's instructions and the hot path paid for it in instruction-cache misses.
+__device__ __noinline__ u64 udiv64(u64 a, u64 b) { return a / b; }
+__device__ __noinline__ u64 umod64(u64 a, u64 b) { return a % b; }
+__device__ __noinline__ i64 sdiv64(i64 a, i64 b) { return a / b; }
+__device__ __noinline__ u64 gcd64(u64 a, u64 b) {   // binary gcd
     if (a == 0) return b;
     if (b == 0) return a;
     const int sh = __ffsll((i64)(a | b)) - 1;
@@ -72,7 +77,7 @@ __device__ __forceinline__ u64 gcd64(u64 a, u64 b) {   // binary gcd
     } while (b);
     return a << sh;
 }
-__device__ __forceinline__ u32 gcd32(u32 a, u32 b) {
+__device__ __noinline__ u32 gcd32(u32 a, u32 b) {
     if (a == 0) return b;
     if (b == 0) return a;
     const int sh = __ffs((int)(a | b)) - 1;
@@ -150,8 +155,8 @@ struct KeyOut {
 __device__ __forceinline__ void scale_small(u64 absE, u32 c, u32& k, u64& d) {
     if (c == 2) { const bool ev = (absE & 1ULL) == 0; k = ev ? 1u : 2u; d = ev ? absE >> 1 : absE; return; }
     if (c == 3) { const u64 qd = absE / 3ULL; const bool dv = qd * 3ULL == absE; k = dv ? 1u : 3u; d = dv ? qd : absE; return; }
-    const u32 gg = (u32)gcd64(absE % (u64)c, (u64)c);
-    k = c / gg; d = absE / (u64)gg;
+    const u32 gg = (u32)gcd64(umod64(absE, (u64)c), (u64)c);
+    k = c / gg; d = udiv64(absE, (u64)gg);
 }
 
 __device__ __forceinline__ bool sbit(const u32* bits, int a) { return (bits[a >> 5] >> (a & 31)) & 1u; }
@@ -428,8 +433,8 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 const int cc = __shfl_sync(gmask, c, l, G);
                 csign = firstv ? +1 : r_sign;
                 const u64 gg = cc == 1 ? 1ULL : gcd64(absE, (u64)cc);
-                ck = gg == 1 ? (u64)cc : (u64)cc / gg;
-                cd = gg == 1 ? absE : absE / gg;
+                ck = gg == 1 ? (u64)cc : (u64)((u32)cc / (u32)gg);
+                cd = gg == 1 ? absE : udiv64(absE, gg);
                 cin = sbit(sbits, ca);
                 if (cin) {   // position of the arc in the sorted support
                     #pragma unroll 1
@@ -506,7 +511,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                         const u64 x = ck * (u64)flux[t];   // <= 2^62 (no overflow was found above)
                         if (narrow) {
                             const u32 r32 = (u32)r;
-                            r = gcd32(r32, (x >> 32) == 0 ? (u32)x % r32 : (u32)(x % (u64)r32));
+                            r = gcd32(r32, (x >> 32) == 0 ? (u32)x % r32 : (u32)umod64(x, (u64)r32));
                         } else r = gcd64(r, x);
                     }
                     if (!__any_sync(gmask, r == 1)) cg = g_gcd<G>(gmask, r, narrow);
@@ -518,7 +523,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     #pragma unroll 1
                     for (int t = lane; t < ns; t += G) {
                         u64 F = t == cia ? cT : ck * (u64)flux[t];
-                        if (cg > 1) F /= cg;
+                        if (cg > 1) F = udiv64(F, cg);
                         chs += arc_term_t(A.g, (u32)arc[t], F);
                     }
                     chs = g_sum<G>(gmask, chs);
@@ -723,7 +728,7 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
     for (int t = lane; t < ns; t += G) {
         const u64 ft = t < G ? (u64)pf0 : (t < 2 * G ? (u64)pf1 : (u64)flux[t]);
         u64 F = t == cia ? cT : ck * ft;
-        if (cg > 1) F /= cg;
+        if (cg > 1) F = udiv64(F, cg);
         const int pos = t + ((!cin && t >= ins) ? 1 : 0);
         flux2[pos] = (i64)F;
         arc2[pos] = (u16)(t < G ? pa0 : (t < 2 * G ? pa1 : (u32)arc[t]));
@@ -754,7 +759,7 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
                 i64 s = 0;
                 for (int qq = qa0; qq < qa1; ++qq) { const int2 e = __ldg(&A.g.col[qq]); if (e.x == met) s = e.y; }
                 x = (i64)(ck * (u64)(t0 == 0 ? pe0 : ef[t]) + sd * (u64)s);
-                if (cg > 1) x /= (i64)cg;
+                if (cg > 1) x = sdiv64(x, (i64)cg);
             }
             for (int qq = qa0; qq < qa1 && qq < qa0 + 32; ++qq)
                 if (gany(valid && __ldg(&A.g.col[qq]).x == met)) seen |= 1u << (qq - qa0);
@@ -777,7 +782,7 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
             }
             if (!in_parent) {
                 i64 x = (i64)(sd * (u64)(i64)e.y);
-                if (cg > 1) x /= (i64)cg;
+                if (cg > 1) x = sdiv64(x, (i64)cg);
                 if (lane == 0) { ef2[wbase] = x; efmet2[wbase] = (u16)e.x; }
                 mx = max(mx, abs64(x));
                 ++wbase;
