@@ -248,8 +248,15 @@ def main_ours(args):
         n_exp_launch = acc["n_expand_count"]
         ms_expand = acc["ms_expand_count"] + acc["ms_expand_write"]
         achieved = acc["algo_bytes"] / (ms_expand * 1e-3) / 1e9 if ms_expand > 0 else 0.0
+        # dram__bytes_read + write per full level from the ncu --set full capture (profiles/r1_v10_expand_full.md); it was
+        # taken on the default workload only
+        traffic, traffic_src = args.traffic, "--traffic"
+        if traffic is None and args.workload == "genome" and args.cap == DEFAULT_CAP:
+            traffic, traffic_src = 7.12e8, "profiles/r1_v10_expand_full.md: k_expand 253 MB + k_materialise 459 MB per full level (algorithmic 216 MB)"
+        elif traffic is None:
+            traffic_src = None
         roofline = {"bound": "hbm", "kernel": "expansion of one level: k_expand (evaluate) + k_compact + k_materialise", "achieved": achieved,
-                    "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": args.traffic,
+                    "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                     "peak_source": peak_src, "launches_per_step": n_exp_launch / args.steps,
                     "avg_launch_ms": ms_expand / max(1, n_exp_launch),
                     "algo_bytes_per_launch": acc["algo_bytes"] / max(1, n_exp_launch),
@@ -309,7 +316,7 @@ def main():
     ap.add_argument("--max-candidates", type=int, default=DEFAULT_MAX_CANDIDATES)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None,
-                    help="ncu dram bytes per expand launch from profiles/ (null until captured)")
+                    help="ncu dram bytes per expansion of a level (default: the profiles/ capture of the default workload)")
     args = ap.parse_args()
     if args.impl == "reference":
         return main_reference(args)
