@@ -576,26 +576,53 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
 }
 
 // ------------------------------------------------------------------ survivors of the beam -> list of slots
-// One thread per key slot: balanced children (kKeyDone) and active children with key < X (all of them when the beam
-// does not bind).  Warp-aggregated append; the order of the list does not matter.
+// Balanced children (kKeyDone) and active children with key < X (all of them when the beam does not bind).  A block
+// appends the survivors of a tile with ONE atomic (a warp-level atomic per 32 keys serialised on the counter); the order
+// of the list does not matter.
+constexpr int kCompactItems = 4;   // keys per thread: a block appends the survivors of 1024 keys with one atomic
 __global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, const uint4* __restrict__ t0, const u64* __restrict__ cur_off,
                                                  ulonglong2* __restrict__ surv, Ctl* ctl, u64 max_keys) {
+    __shared__ u32 s_warp[8];
+    __shared__ u64 s_base;
     const u64 n = min(ctl->n_slots, max_keys);
     const bool notrunc = ctl->notrunc != 0;
     const u64 X = ctl->X;
-    const int lane = threadIdx.x & 31;
-    for (u64 base = ((u64)blockIdx.x * blockDim.x + threadIdx.x) & ~31ULL; base < n; base += (u64)gridDim.x * blockDim.x) {
-        const u64 i = base + lane;
-        const u64 key = i < n ? __ldcs(&keys[i]) : kKeySentinel;
-        const bool take = key == kKeyDone || (key != kKeySentinel && (notrunc || key < X));
-        const u32 m = __ballot_sync(0xffffffffu, take);
-        if (m) {
-            u64 pos = 0;
-            if (lane == 0) pos = atomicAdd(&ctl->n_surv, (u64)__popc(m));
-            pos = __shfl_sync(0xffffffffu, pos, 0);
-            // the survivor record carries the offset of its parent: one dependent load less in k_materialise
-            if (take) surv[pos + __popc(m & ((1u << lane) - 1u))] = make_ulonglong2(i, __ldg(&cur_off[__ldcs(&t0[i]).x]));
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    constexpr u64 kTile = 256 * kCompactItems;
+    for (u64 tile = (u64)blockIdx.x * kTile; tile < n; tile += (u64)gridDim.x * kTile) {   // block-uniform trip count
+        // item j of a thread is key tile + j * 256 + threadIdx.x (coalesced); survivors are numbered warp by warp
+        u32 takes = 0;
+        u32 wm[kCompactItems];
+#pragma unroll
+        for (int j = 0; j < kCompactItems; ++j) {
+            const u64 i = tile + (u64)j * 256 + threadIdx.x;
+            const u64 key = i < n ? __ldcs(&keys[i]) : kKeySentinel;
+            const bool take = key == kKeyDone || (key != kKeySentinel && (notrunc || key < X));
+            wm[j] = __ballot_sync(0xffffffffu, take);
+            if (take) takes |= 1u << j;
         }
+        u32 wtot = 0;
+#pragma unroll
+        for (int j = 0; j < kCompactItems; ++j) wtot += __popc(wm[j]);
+        if (lane == 0) s_warp[wib] = wtot;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            u32 tot = 0;
+            for (int w = 0; w < 8; ++w) { const u32 c = s_warp[w]; s_warp[w] = tot; tot += c; }
+            s_base = tot ? atomicAdd(&ctl->n_surv, (u64)tot) : 0ULL;
+        }
+        __syncthreads();
+        u64 pos = s_base + s_warp[wib];
+#pragma unroll
+        for (int j = 0; j < kCompactItems; ++j) {
+            if ((takes >> j) & 1u) {
+                const u64 i = tile + (u64)j * 256 + threadIdx.x;
+                // the survivor record carries the offset of its parent: one dependent load less in k_materialise
+                surv[pos + __popc(wm[j] & ((1u << lane) - 1u))] = make_ulonglong2(i, __ldg(&cur_off[__ldcs(&t0[i]).x]));
+            }
+            pos += __popc(wm[j]);
+        }
+        __syncthreads();   // s_warp / s_base are reused by the next tile
     }
 }
 
@@ -930,8 +957,8 @@ cudaError_t launch_expand(const ExpandArgs& a, int sm_count, cudaStream_t s) {
 // survivors of the level -> next frontier / candidates.  n_hint bounds the key slots in use (host side estimate).
 cudaError_t launch_materialise(const ExpandArgs& a, u64 n_slots_hint, u64 n_surv, int sm_count, cudaStream_t s, int phase) {
     if (phase == 0) {   // compact
-        u64 blocks = (n_slots_hint + 511) / 512;   // about two keys per thread: the kernel is one dependent-load chain per key
-        if (blocks > (u64)sm_count * 128) blocks = (u64)sm_count * 128;
+        u64 blocks = (n_slots_hint + 1023) / 1024;   // one tile of 256 x kCompactItems keys per block and round
+        if (blocks > (u64)sm_count * 64) blocks = (u64)sm_count * 64;
         if (blocks < 1) blocks = 1;
         k_compact<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.t0, a.cur_off, a.surv, a.ctl, a.max_keys);
         return cudaGetLastError();
