@@ -23,7 +23,7 @@ struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
     Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
-    Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill;
+    Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill, vcount, vstart, vfill, tstart;
     Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, u_key, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
 };
@@ -104,6 +104,10 @@ void make_layout(efm_handle* h) {
     add_region(L, L.gcount, gbins * 4);
     add_region(L, L.gstart, gbins * 4);
     add_region(L, L.gfill, gbins * 4);
+    add_region(L, L.vcount, gbins * 4);
+    add_region(L, L.vstart, gbins * 4);
+    add_region(L, L.vfill, gbins * 4);
+    add_region(L, L.tstart, bins * 4);
     add_region(L, L.g_row, C * 4);
     add_region(L, L.g_sig, C * 16);
     add_region(L, L.g_size, C * 2);
@@ -523,6 +527,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     pa.isrep = ws + L.isrep.off; pa.poison = ws + L.poison.off; pa.uniq = (u32*)(ws + L.uniq.off);
     pa.freq = (u32*)(ws + L.freq.off); pa.gcount = (u32*)(ws + L.gcount.off);
     pa.gstart = (u32*)(ws + L.gstart.off); pa.gfill = (u32*)(ws + L.gfill.off);
+    // the join's row lists and row-order signatures live in regions the output stage fills only afterwards
+    pa.v_row = (u32*)(ws + L.u_rxn.off); pa.r_sig = (uint4*)(ws + L.u_key.off);
+    pa.vcount = (u32*)(ws + L.vcount.off); pa.vstart = (u32*)(ws + L.vstart.off); pa.vfill = (u32*)(ws + L.vfill.off); pa.tstart = (u32*)(ws + L.tstart.off);
     pa.g_row = (u32*)(ws + L.g_row.off); pa.g_sig = (uint4*)(ws + L.g_sig.off);
     pa.keep = ws + L.keep.off;
     pa.D = h->D; pa.n_rxn = G.n; pa.n_sizes = h->D + 1;

@@ -267,11 +267,12 @@ __global__ void __launch_bounds__(256) k_filter_count(const PostArgs a, u64 K) {
     if (n == 0) return;   // the empty support belongs to no group (it has no strict subset and nothing tests against it)
     atomicAdd(&a.gcount[(size_t)rarest_arc(a, cand_arc(e, n), n) * a.n_sizes + n], 1u);   // group key: (rarest arc, |supp|)
 }
-__global__ void __launch_bounds__(1024) k_filter_scan(const PostArgs a) {   // exclusive scan of the group sizes over arcs
+// exclusive scan of `len` counters by one block: start[i] and fill[i] get the prefix, start[len] the total
+__global__ void __launch_bounds__(1024) k_filter_scan(const u32* __restrict__ count, u32* __restrict__ start, u32* __restrict__ fill, int len) {
     __shared__ u32 part[1024];
-    const int A = a.g.A * a.n_sizes, T = blockDim.x, per = (A + T - 1) / T, b0 = threadIdx.x * per;   // (arc, size) bins
+    const int T = blockDim.x, per = (len + T - 1) / T, b0 = threadIdx.x * per;
     u32 sum = 0;
-    for (int j = 0; j < per; ++j) if (b0 + j < A) sum += a.gcount[b0 + j];
+    for (int j = 0; j < per; ++j) if (b0 + j < len) sum += count[b0 + j];
     part[threadIdx.x] = sum;
     __syncthreads();
     for (int off = 1; off < T; off <<= 1) {
@@ -282,8 +283,8 @@ __global__ void __launch_bounds__(1024) k_filter_scan(const PostArgs a) {   // e
     }
     u32 acc = part[threadIdx.x] - sum;
     for (int j = 0; j < per; ++j)
-        if (b0 + j < A) { const u32 c = a.gcount[b0 + j]; a.gstart[b0 + j] = acc; a.gfill[b0 + j] = acc; acc += c; }
-    if (threadIdx.x == T - 1) a.gstart[A] = part[T - 1];
+        if (b0 + j < len) { const u32 c = count[b0 + j]; start[b0 + j] = acc; fill[b0 + j] = acc; acc += c; }
+    if (threadIdx.x == T - 1) start[len] = part[T - 1];
 }
 __global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K) {
     const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
@@ -294,8 +295,10 @@ __global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K)
     if (n == 0) return;
     const u16* arc = cand_arc(e, n);
     const u32 pos = atomicAdd(&a.gfill[(size_t)rarest_arc(a, arc, n) * a.n_sizes + n], 1u);
+    const uint4 sg = sig_of(arc, n, a.g.A <= kSigBits);
     a.g_row[pos] = id;
-    a.g_sig[pos] = sig_of(arc, n, a.g.A <= kSigBits);
+    a.g_sig[pos] = sg;
+    a.r_sig[u] = sg;   // the same record in row order, for the v side of the join
 }
 __device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   // supp(w) subset of supp(v), sorted lists
     const int nw = cand_n(w), nv = cand_n(v);
@@ -309,61 +312,119 @@ __device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   
     }
     return true;
 }
-constexpr int kFilterWarps = 8;
-// one warp per row v; lanes walk the group of every arc of v, four 16-byte records in flight per lane
-__global__ void __launch_bounds__(kFilterWarps * 32) k_filter(const PostArgs a, u64 K) {
-    const u64 u = (u64)blockIdx.x * kFilterWarps + (threadIdx.x >> 5);
+// ---- the join, tiled.  For every arc a: V(a) = the rows that contain a, W(a) = the group of a (rows whose rarest arc
+// is a, ordered by size).  A block takes 256 rows of V(a) -- one per thread, signature in registers -- and streams
+// W(a) through shared memory in tiles of 256 records: every 16-byte record is read from L2 / HBM once per block instead
+// of once per row.  k_filter_vprep sizes V(a) (only for arcs with a non-empty group) and numbers the tiles,
+// k_filter_vscatter fills the lists, k_filter_join maps a block to (arc, tile) by binary search over the tile prefix.
+#ifndef EFM_JOIN_THREADS
+#define EFM_JOIN_THREADS 32   // rows of V(a) per block (measured: 256 -> 10.6 ms, 128 -> 9.1, 64 -> 7.8, 32 -> 6.8: most arcs list few rows)
+#endif
+constexpr int kJoinThreads = EFM_JOIN_THREADS;
+// V lists are ordered by (arc, size) too: the 256 rows of a tile have about the same size, hence the same range of W
+__global__ void __launch_bounds__(256) k_filter_vcount(const PostArgs a, u64 K, int fill) {
+    const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= K) return;
-    const int lane = threadIdx.x & 31;
-    const unsigned char* ev = a.cand + (u64)a.uniq[u] * a.cand_stride;
-    const int n = cand_n(ev);
-    const u16* arc = cand_arc(ev, n);
-    const bool exact = a.g.A <= kSigBits;
-    u32 w0 = 0, w1 = 0, w2 = 0, w3 = 0;
-    for (int t = lane; t < n; t += 32) {
-        const u32 b = sig_bit(arc[t], exact);
-        const u32 m = 1u << (b & 31);
-        if (b < 32) w0 |= m; else if (b < 64) w1 |= m; else if (b < 96) w2 |= m; else w3 |= m;
-    }
-    w0 = __reduce_or_sync(0xffffffffu, w0); w1 = __reduce_or_sync(0xffffffffu, w1);
-    w2 = __reduce_or_sync(0xffffffffu, w2); w3 = __reduce_or_sync(0xffffffffu, w3);
-    const u32 n0 = ~w0, n1 = ~w1, n2 = ~w2, n3 = ~w3 & 0xffffu;
-    bool found = false;
-    u64 pairs = 0;
-    for (int t0 = 0; t0 < n && !found; t0 += 32) {
-        // group ranges of 32 arcs of v at a time (one per lane), then the groups one after the other
-        const int tt = t0 + lane;
-        u32 myg0 = 0, myg1 = 0;
-        // within the group of an arc the rows are ordered by |supp|: only the strictly smaller ones can be subsets
-        if (tt < n) { const size_t gb = (size_t)arc[tt] * a.n_sizes; myg0 = a.gstart[gb]; myg1 = a.gstart[gb + n]; }
-        const int cnt = min(32, n - t0);
-        for (int j = 0; j < cnt && !found; ++j) {
-            const u32 g0 = __shfl_sync(0xffffffffu, myg0, j), g1 = __shfl_sync(0xffffffffu, myg1, j);
-            for (u32 base = g0; base < g1 && !found; base += 128) {
-                uint4 r[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const u32 w = base + 32 * q + lane;
-                    r[q] = w < g1 ? __ldg(&a.g_sig[w]) : make_uint4(0xffffffffu, 0, 0, 0xffffffffu);   // never a subset
-                }
-                bool hit = false;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const u32 w = base + 32 * q + lane;
-                    pairs += w < g1;
-                    // a strict subset is strictly smaller (equal supports were merged by a-6)
-                    if (((r[q].x & n0) | (r[q].y & n1) | (r[q].z & n2) | (r[q].w & n3)) == 0 && (int)(r[q].w >> 16) < n)
-                        hit = hit || exact || arcs_subset(a.cand + (u64)a.g_row[w] * a.cand_stride, ev);
-                }
-                found = __any_sync(0xffffffffu, hit);
-            }
+    if (fill) a.keep[u] = 1;
+    const unsigned char* e = a.cand + (u64)a.uniq[u] * a.cand_stride;
+    const int n = cand_n(e);
+    const u16* arc = cand_arc(e, n);
+    for (int t = 0; t < n; ++t) {
+        const size_t gb = (size_t)arc[t] * a.n_sizes;
+        if (a.gstart[gb + n] > a.gstart[gb]) {   // the group of this arc has rows strictly smaller than this one
+            if (fill) a.v_row[atomicAdd(&a.vfill[gb + n], 1u)] = (u32)u;
+            else atomicAdd(&a.vcount[gb + n], 1u);
         }
     }
-#pragma unroll
-    for (int o = 16; o; o >>= 1) pairs += __shfl_xor_sync(0xffffffffu, pairs, o);
-    if (lane == 0) {
-        a.keep[u] = found ? 0 : 1;
-        atomicAdd(&a.ctl->filter_pairs, pairs);
+}
+__global__ void __launch_bounds__(1024) k_filter_tiles(const PostArgs a) {   // tiles of 256 rows per arc, prefix over the arcs
+    __shared__ u32 part[1024];
+    const int A = a.g.A, T = blockDim.x, per = (A + T - 1) / T, b0 = threadIdx.x * per;
+    u32 st = 0;
+    for (int j = 0; j < per; ++j) {
+        const int x = b0 + j;
+        if (x < A) st += (a.vstart[(size_t)(x + 1) * a.n_sizes] - a.vstart[(size_t)x * a.n_sizes] + kJoinThreads - 1) / kJoinThreads;
+    }
+    part[threadIdx.x] = st;
+    __syncthreads();
+    for (int off = 1; off < T; off <<= 1) {
+        const u32 v = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
+        __syncthreads();
+        part[threadIdx.x] += v;
+        __syncthreads();
+    }
+    u32 at = part[threadIdx.x] - st;
+    for (int j = 0; j < per; ++j) {
+        const int x = b0 + j;
+        if (x >= A) break;
+        a.tstart[x] = at;
+        at += (a.vstart[(size_t)(x + 1) * a.n_sizes] - a.vstart[(size_t)x * a.n_sizes] + kJoinThreads - 1) / kJoinThreads;
+    }
+    if (threadIdx.x == T - 1) a.tstart[A] = part[T - 1];
+}
+__global__ void __launch_bounds__(kJoinThreads) k_filter_join(const PostArgs a) {
+    __shared__ uint4 wtile[kJoinThreads];
+    __shared__ u32 s_gend;
+    __shared__ unsigned long long s_pairs;
+    const int A = a.g.A;
+    const u32 n_tiles = a.tstart[A];
+    const bool exact = A <= kSigBits;
+    for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {   // block-uniform
+        // arc of this tile: the last x with tstart[x] <= tile
+        int lo = 0, hi = A;
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (a.tstart[mid] <= tile) lo = mid; else hi = mid; }
+        const int x = lo;
+        const size_t gb = (size_t)x * a.n_sizes;
+        const u32 vi = a.vstart[gb] + (tile - a.tstart[x]) * kJoinThreads + threadIdx.x;
+        const bool live = vi < a.vstart[gb + a.n_sizes];
+        u32 u = 0, gend = 0;
+        uint4 sv = make_uint4(0, 0, 0, 0);
+        const u32 g0 = a.gstart[gb];
+        if (live) {
+            u = a.v_row[vi];
+            sv = a.r_sig[u];
+            gend = a.gstart[gb + (sv.w >> 16)];   // group rows of size < |supp(v)|
+        }
+        if (threadIdx.x == 0) { s_gend = 0; s_pairs = 0; }
+        __syncthreads();
+        if (live) atomicMax(&s_gend, gend);
+        __syncthreads();
+        const u32 bend = s_gend;
+        const u32 n0 = ~sv.x, n1 = ~sv.y, n2 = ~sv.z, n3 = ~sv.w & 0xffffu;
+        bool found = false;
+        u32 pairs = 0;
+        for (u32 base = g0; base < bend; base += kJoinThreads) {
+            const u32 w = base + threadIdx.x;
+            if (w < bend) wtile[threadIdx.x] = a.g_sig[w];
+            __syncthreads();
+            if (live && !found && base < gend) {
+                const int jn = (int)min((u32)kJoinThreads, gend - base);
+                pairs += (u32)jn;
+                u32 hits = 0;   // signature hits are rare: collect them four records at a time, verify afterwards
+                int j = 0;
+                for (; j + 4 <= jn; j += 4) {
+                    const uint4 r0 = wtile[j], r1 = wtile[j + 1], r2 = wtile[j + 2], r3 = wtile[j + 3];
+                    const u32 m0 = (r0.x & n0) | (r0.y & n1) | (r0.z & n2) | (r0.w & n3);
+                    const u32 m1 = (r1.x & n0) | (r1.y & n1) | (r1.z & n2) | (r1.w & n3);
+                    const u32 m2 = (r2.x & n0) | (r2.y & n1) | (r2.z & n2) | (r2.w & n3);
+                    const u32 m3 = (r3.x & n0) | (r3.y & n1) | (r3.z & n2) | (r3.w & n3);
+                    if (m0 == 0 || m1 == 0 || m2 == 0 || m3 == 0) { hits = 1; break; }
+                }
+                if (hits || j < jn) {   // verify from the first unexamined / hit group of four
+                    for (; j < jn && !found; ++j) {
+                        const uint4 r = wtile[j];
+                        if (((r.x & n0) | (r.y & n1) | (r.z & n2) | (r.w & n3)) == 0)
+                            found = exact || arcs_subset(a.cand + (u64)a.g_row[base + j] * a.cand_stride, a.cand + (u64)a.uniq[u] * a.cand_stride);
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        if (found) a.keep[u] = 0;
+        if (pairs) atomicAdd(&s_pairs, (unsigned long long)pairs);
+        __syncthreads();
+        if (threadIdx.x == 0 && s_pairs) atomicAdd(&a.ctl->filter_pairs, (u64)s_pairs);
+        __syncthreads();
     }
 }
 
@@ -371,6 +432,7 @@ cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s
     cudaError_t e;
     if ((e = cudaMemsetAsync(a.freq, 0, sizeof(u32) * (a.g.A + 2), s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(a.gcount, 0, sizeof(u32) * ((size_t)a.g.A * a.n_sizes + 2), s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(a.vcount, 0, sizeof(u32) * ((size_t)a.g.A * a.n_sizes + 2), s)) != cudaSuccess) return e;
     if (K == 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((K + 255) / 256);
     {
@@ -379,10 +441,14 @@ cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s
         k_filter_freq<<<fb, 256, use_smem ? (size_t)a.g.A * 4 : 0, s>>>(a, K, use_smem);
     }
     k_filter_count<<<blocks, 256, 0, s>>>(a, K);
-    k_filter_scan<<<1, 1024, 0, s>>>(a);
+    k_filter_scan<<<1, 1024, 0, s>>>(a.gcount, a.gstart, a.gfill, a.g.A * a.n_sizes);
     k_filter_scatter<<<blocks, 256, 0, s>>>(a, K);
-    k_filter<<<(unsigned)((K + kFilterWarps - 1) / kFilterWarps), kFilterWarps * 32, 0, s>>>(a, K);
-    *n_launches += 5;
+    k_filter_vcount<<<blocks, 256, 0, s>>>(a, K, 0);
+    k_filter_scan<<<1, 1024, 0, s>>>(a.vcount, a.vstart, a.vfill, a.g.A * a.n_sizes);
+    k_filter_tiles<<<1, 1024, 0, s>>>(a);
+    k_filter_vcount<<<blocks, 256, 0, s>>>(a, K, 1);
+    k_filter_join<<<(unsigned)(sm_count * 16 * (256 / kJoinThreads)), kJoinThreads, 0, s>>>(a);
+    *n_launches += 9;
     return cudaGetLastError();
 }
 
