@@ -120,7 +120,7 @@ def test_mid(efm, oracle_mod, cap):
     assert got.stats["truncated_beam"] > 0
 
 
-@pytest.mark.parametrize("cap", [256, 4096])
+@pytest.mark.parametrize("cap", [256, 4096, 16384])
 def test_genome(efm, oracle_mod, cap):
     net = make_network("genome", 0)
     got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=cap)
