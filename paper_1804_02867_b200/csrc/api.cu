@@ -83,8 +83,8 @@ void make_layout(efm_handle* h) {
     add_region(L, L.arc_dir, sizeof(int) * (G.A + 1));
     add_region(L, L.arc_mix, sizeof(u64) * (G.A + 1));
     add_region(L, L.ctl, sizeof(Ctl));
-    add_region(L, L.buf[0], (size_t)h->frontier_bytes + 512);   // 512: the speculative first load of a parent
-    add_region(L, L.buf[1], (size_t)h->frontier_bytes + 512);
+    add_region(L, L.buf[0], (size_t)h->frontier_bytes + 2048);   // spare bytes: the fixed-size prefetch of a parent
+    add_region(L, L.buf[1], (size_t)h->frontier_bytes + 2048);
     add_region(L, L.off[0], (size_t)h->max_frontier * 8);
     add_region(L, L.off[1], (size_t)h->max_frontier * 8);
     add_region(L, L.pmin, (size_t)(h->max_frontier + 1) * 8);
@@ -428,7 +428,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.D = h->D; ea.V = h->V; ea.max_loop = h->max_loop;
     ea.no_fast = (h->flags & EFM_F_NO_FASTPATH) ? 1 : 0;
     expand_smem_layout(ea);
-    if (h->flags & EFM_F_NO_STAGING) ea.sm_stage_bytes = 0;
+    ea.force_inplace = (h->flags & EFM_F_NO_STAGING) ? 1 : 0;
 
     auto read_ctl = [&]() -> cudaError_t {
         cudaError_t e = cudaMemcpyAsync(hc, d_ctl, ctl_read, cudaMemcpyDeviceToHost, s);

@@ -101,6 +101,7 @@ struct ExpandArgs {
     u64 max_frontier, frontier_units, max_cand, max_keys;
     int D, V, max_loop;
     u32 ppw;                    // consecutive parents a warp owns (set by the launcher)
+    int force_inplace;          // EFM_F_NO_STAGING: read every parent in place
     int no_fast;                // EFM_F_NO_FASTPATH: every child through the warp-cooperative general routine
     // shared-memory carve-up per warp (bytes)
     u32 sm_group, sm_stage_bytes, sm_sbits, sm_upos, sm_misc;

@@ -32,6 +32,8 @@ constexpr int kWarps = kBlock / 32;
 #define EFM_PPW 8
 #endif
 constexpr int kParentsPerWarp = EFM_PPW;
+static_assert(kParentsPerWarp <= 8, "SS_OFF holds 8 parent offsets");
+constexpr int kPrefetch = 1024;   // bytes of the next parent requested ahead (a typical entry; longer ones load the rest later)
 constexpr u32 FULL = 0xffffffffu;
 constexpr u64 kSmall = 1ULL << 40;   // fast path: every flux and extra flux of the parent below this ...
 constexpr int kSmallCoef = 1 << 20;  // ... and every coefficient below this: no product can reach 2^62
@@ -159,13 +161,22 @@ __device__ __forceinline__ void scale_small(u64 absE, u32 c, u32& k, u64& d) {
     k = c / gg; d = udiv64(absE, (u64)gg);
 }
 
+// 16-byte asynchronous copy global -> shared (LDGSTS): no register staging, completion awaited with cp_async_wait()
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem_src));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+
 __device__ __forceinline__ bool sbit(const u32* bits, int a) { return (bits[a >> 5] >> (a & 31)) & 1u; }
 
 // per-warp statistics live in shared memory (one u64 each), flushed to the control block once per warp
 enum { SS_EXPANDED = 0, SS_CHILDREN, SS_DONE, SS_ACTIVE, SS_DEAD, SS_NOTEFM, SS_NONPOS, SS_OVF, SS_VISITED, SS_BYTES,
        SS_ROUNDS, SS_FIRST, SS_GENERAL, SS_SATURATED,
        SS_KC,   // 4 words: the hash sums of the k-scaled support for the last two scales k (k0, s0, k1, s1)
-       SS_WORDS = SS_KC + 4 };
+       SS_OFF = SS_KC + 4,   // kParentsPerWarp words: offsets of the parents of this group
+       SS_WORDS = SS_OFF + 8 };
 
 // One kernel body, every routine inlined once: the staged parent is addressed through shared-memory pointers the
 // compiler can track.  The kernel only EVALUATES: every child that passes the discard tests gets a slot holding its
@@ -203,27 +214,45 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
     const u64 p0 = ((u64)blockIdx.x * (blockDim.x / G) + wib) * A.ppw;
     const u64 p1 = min(p0 + A.ppw, A.n_cur);
 
+    // Double-buffered staging: while parent p is processed, the first kPrefetch bytes of parent p + 1 travel to the other
+    // staging buffer with asynchronous copies (no registers, no waiting); the frontier buffers end in spare bytes so that
+    // the fixed-size copy may run past the end of a short entry.
+    u64* soff = sst + SS_OFF;
+    if (lane < kParentsPerWarp) soff[lane] = p0 + lane < p1 ? __ldcs(&A.cur_off[p0 + lane]) : 0ULL;
+    __syncwarp(gmask);
+    const u32 pre_chunks = min(A.sm_stage_bytes, (u32)kPrefetch) / 16;
+    auto prefetch = [&](u64 p, int b) {
+        const unsigned char* gsrc = A.cur + (soff[p - p0] << 4);
+        unsigned char* sdst = gs + (size_t)b * A.sm_stage_bytes;
+        #pragma unroll 1
+        for (u32 c = lane; c < pre_chunks; c += G) cp_async16(sdst + 16 * c, gsrc + 16 * c);
+        cp_async_commit();
+    };
+    if (p0 < p1) prefetch(p0, 0);
 #pragma unroll 1
     for (u64 p = p0; p < p1; ++p) {
-        // ---- stage the parent: the first 32 16-byte chunks speculatively, the rest once the header is known
-        const uint4* src = (const uint4*)(A.cur + (__ldcs(&A.cur_off[p]) << 4));
-        const uint4 first16 = __ldcs(src + lane);   // the buffers end in 512 spare bytes
-        const u32 hdr = __shfl_sync(gmask, first16.x, 0, G);
-        const int ns = (int)(hdr & 0xffffu), nv = (int)(hdr >> 16);
-        const int nu = (int)__shfl_sync(gmask, first16.y, 0, G);
+        // ---- the parent: its first kPrefetch bytes are on their way already, the rest follows once the header is known
+        const int sb = (int)(p - p0) & 1;
+        const uint4* src = (const uint4*)(A.cur + (soff[p - p0] << 4));
+        cp_async_wait();
+        __syncwarp(gmask);
+        if (p + 1 < p1) prefetch(p + 1, sb ^ 1);
+        stage = (uint4*)(gs + (size_t)sb * A.sm_stage_bytes);
+        const uint4 h0 = stage[0], h1 = stage[1];
+        const int ns = (int)(h0.x & 0xffffu), nv = (int)(h0.x >> 16);
+        const int nu = (int)h0.y;
         const u32 nch = entry_bytes((u32)ns, (u32)nv, (u32)nu) / 16;
-        // entries that fit the staging buffer are copied to shared memory; the rare larger ones are read in place
-        const bool staged = nch * 16 <= A.sm_stage_bytes;
+        // entries that fit the staging buffer are read from shared memory; the rare larger ones are read in place
+        const bool staged = !A.force_inplace && nch * 16 <= A.sm_stage_bytes;
         if (staged) {
-            if ((u32)lane < nch) stage[lane] = first16;
             #pragma unroll 1
-            for (u32 c = lane + G; c < nch; c += G) stage[c] = __ldcs(src + c);   // streaming: the frontier must not evict the graph from L1
+            for (u32 c = pre_chunks + lane; c < nch; c += G) stage[c] = __ldcs(src + c);   // streaming: the frontier must not evict the graph from L1
         }
         __syncwarp(gmask);
-        const u64 Phs = (u64)__shfl_sync(gmask, first16.z, 0, G) | ((u64)__shfl_sync(gmask, first16.w, 0, G) << 32);
-        const u64 Phv = (u64)__shfl_sync(gmask, first16.x, 1, G) | ((u64)__shfl_sync(gmask, first16.y, 1, G) << 32);
-        const u64 Pbig = (u64)__shfl_sync(gmask, first16.z, 1, G) | ((u64)__shfl_sync(gmask, first16.w, 1, G) << 32);
-        const unsigned char* eb = staged ? (const unsigned char*)gs : (const unsigned char*)src;
+        const u64 Phs = (u64)h0.z | ((u64)h0.w << 32);
+        const u64 Phv = (u64)h1.x | ((u64)h1.y << 32);
+        const u64 Pbig = (u64)h1.z | ((u64)h1.w << 32);
+        const unsigned char* eb = staged ? (const unsigned char*)stage : (const unsigned char*)src;
         const i64* flux = (const i64*)(eb + kHdr);
         const u64* vis = (const u64*)(flux + ns);
         const i64* ef = (const i64*)(vis + nv);
@@ -912,8 +941,8 @@ static size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 void expand_smem_layout(ExpandArgs& a) {
     // staging: the largest entry if it is small, otherwise 1.5 KB (larger entries are rare and read in place);
     // the smaller the per-warp footprint, the more of the graph stays in L1
-    a.sm_stage_bytes = a.max_entry < 1536u ? a.max_entry : 1536u;
-    size_t off = align16(a.sm_stage_bytes);
+    a.sm_stage_bytes = (u32)align16(a.max_entry < 1536u ? (a.max_entry < 32u ? 32u : a.max_entry) : 1536u);
+    size_t off = 2 * (size_t)a.sm_stage_bytes;   // two staging buffers
     a.sm_sbits = (u32)off; off = align16(off + (size_t)a.g.W32 * 4);
     a.sm_upos = (u32)off;  off = align16(off + (size_t)a.g.M * 2 + 16);   // zeroed in 16-byte chunks
     a.sm_misc = (u32)off;  off = align16(off + (size_t)SS_WORDS * 8);
