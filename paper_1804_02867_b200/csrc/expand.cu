@@ -33,7 +33,10 @@ constexpr int kWarps = kBlock / 32;
 #endif
 constexpr int kParentsPerWarp = EFM_PPW;
 static_assert(kParentsPerWarp <= 8, "SS_OFF holds 8 parent offsets");
-constexpr int kPrefetch = 1024;   // bytes of the next parent requested ahead (a typical entry; longer ones load the rest later)
+#ifndef EFM_PREFETCH
+#define EFM_PREFETCH 1536
+#endif
+constexpr int kPrefetch = EFM_PREFETCH;   // bytes of the next parent requested ahead (1536 = the whole staging buffer: 41.7 ms, 1024: 42.2 ms)
 constexpr u32 FULL = 0xffffffffu;
 constexpr u64 kSmall = 1ULL << 40;   // fast path: every flux and extra flux of the parent below this ...
 constexpr int kSmallCoef = 1 << 20;  // ... and every coefficient below this: no product can reach 2^62
