@@ -139,7 +139,7 @@ struct KeyOut {
             u64 b = 0;
             if (lane == 0) b = atomicAdd(&A.ctl->n_slots, (u64)kKeyChunk);
             b = __shfl_sync(gmask, b, 0, G);
-            if (b + kKeyChunk > A.max_keys) {
+            if (__builtin_expect(b + kKeyChunk > A.max_keys, 0)) {
                 if (lane == 0) atomicOr(&A.ctl->error, (u32)ERR_KEYS);
                 left = 0;
                 return kNoSlot;
@@ -371,7 +371,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     a = (int)(r0.x & 0xffffu); c = (int)(r0.x >> 16);
                     const u32 tw = r0.y & 0xffffu;
                     generic = (r0.y >> 24) & 1u;
-                    if (generic) c = __ldg(&alist[q]).y;   // the coefficient may not fit the record
+                    if (__builtin_expect(generic, 0)) c = __ldg(&alist[q]).y;   // the coefficient may not fit the record
                     insup = sbit(sbits, a);
                     adm = !(tw != 0xffffu && sbit(sbits, (int)tw)) && (insup || ns < A.D);
                 }
@@ -493,7 +493,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                         else { cT = lo - cd; const u64 hi2 = hi - (lo < cd); ovf = hi2 != 0 || cT > EFM_GUARD; }
                     }
                 }
-                if (bigk) {   // exact: the largest flux among t != ia (a new arc carries d <= |E| <= 2^62)
+                if (__builtin_expect(bigk, 0)) {   // exact: the largest flux among t != ia (a new arc carries d <= |E| <= 2^62)
                     u64 mx = 0;
                     #pragma unroll 1
                     for (int t = lane; t < ns; t += G) if (t != cia) mx = max(mx, (u64)flux[t]);
@@ -504,7 +504,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                 if (status == CH_OK) {
                     // extra fluxes of the un-normalised child: EF'_i = k EF_i + sign d s_ia (Eq 2 on the scaled fluxes)
                     bool ovf2 = false;
-                    if (bigk) {   // exact sweep over the unbalanced metabolites outside col(a)
+                    if (__builtin_expect(bigk, 0)) {   // exact sweep over the unbalanced metabolites outside col(a)
                         #pragma unroll 1
                         for (int t = lane; t < nu; t += G) {
                             const int i = efmet[t];
@@ -546,7 +546,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                             r = gcd32(r32, (x >> 32) == 0 ? (u32)x % r32 : (u32)umod64(x, (u64)r32));
                         } else r = gcd64(r, x);
                     }
-                    if (!__any_sync(gmask, r == 1)) cg = g_gcd<G>(gmask, r, narrow);
+                    if (__builtin_expect(!__any_sync(gmask, r == 1), 0)) cg = g_gcd<G>(gmask, r, narrow);
                 }
                 if (ck == 1 && cg == 1) {
                     chs = Phs + arc_term_t(A.g, (u32)ca, cT) - (cin ? arc_term_t(A.g, (u32)ca, (u64)flux[cia]) : 0ULL);
