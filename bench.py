@@ -248,11 +248,11 @@ def main_ours(args):
         n_exp_launch = acc["n_expand_count"]
         ms_expand = acc["ms_expand_count"] + acc["ms_expand_write"]
         achieved = acc["algo_bytes"] / (ms_expand * 1e-3) / 1e9 if ms_expand > 0 else 0.0
-        # dram__bytes_read + write per full level from the ncu --set full capture (profiles/r1_v10_expand_full.md); it was
+        # dram__bytes_read + write per full level from the ncu --set full capture (profiles/r1_v12_expand_full.md); it was
         # taken on the default workload only
         traffic, traffic_src = args.traffic, "--traffic"
         if traffic is None and args.workload == "genome" and args.cap == DEFAULT_CAP:
-            traffic, traffic_src = 7.12e8, "profiles/r1_v10_expand_full.md: k_expand 253 MB + k_materialise 459 MB per full level (algorithmic 216 MB)"
+            traffic, traffic_src = 7.36e8, "profiles/r1_v12_expand_full.md: k_expand 277 MB + k_materialise 459 MB per full level (algorithmic 216 MB)"
         elif traffic is None:
             traffic_src = None
         roofline = {"bound": "hbm", "kernel": "expansion of one level: k_expand (evaluate) + k_compact + k_materialise", "achieved": achieved,
