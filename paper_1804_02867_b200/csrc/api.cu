@@ -23,7 +23,7 @@ struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
     Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
-    Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill, vcount, vstart, vfill, tstart;
+    Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, surv_dst, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill, vcount, vstart, vfill, tstart;
     Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, u_key, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
 };
@@ -92,6 +92,7 @@ void make_layout(efm_handle* h) {
     add_region(L, L.ckeys, (size_t)h->max_keys * 8);
     for (int t = 0; t < 4; ++t) add_region(L, L.task[t], (size_t)h->max_keys * 16);
     add_region(L, L.surv, (size_t)h->max_keys * 16);
+    add_region(L, L.surv_dst, (size_t)h->max_keys * 8);
     const size_t C = (size_t)h->max_cand;
     add_region(L, L.cand, C * h->cand_stride);
     add_region(L, L.table, h->table_size * 4);
@@ -421,7 +422,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.ctl = d_ctl;
     ea.t0 = (uint4*)(ws + L.task[0].off); ea.t1 = (uint4*)(ws + L.task[1].off);
     ea.t2 = (uint4*)(ws + L.task[2].off); ea.t3 = (uint4*)(ws + L.task[3].off);
-    ea.surv = (ulonglong2*)(ws + L.surv.off);
+    ea.surv = (ulonglong2*)(ws + L.surv.off); ea.surv_dst = (u64*)(ws + L.surv_dst.off);
     ea.max_entry = h->max_entry; ea.cand_stride = h->cand_stride;
     ea.frontier_units = (u64)h->frontier_bytes >> 4;
     ea.max_frontier = (u64)h->max_frontier; ea.max_cand = (u64)h->max_cand; ea.max_keys = (u64)h->max_keys;

@@ -95,6 +95,8 @@ struct ExpandArgs {
     u64* keys;                  // per child slot: beam key (kKeyDone: balanced child; kKeySentinel: unused slot)
     uint4* t0; uint4* t1; uint4* t2; uint4* t3;   // per child slot: the task (see k_expand / k_materialise)
     ulonglong2* surv;           // children that are materialised: {slot, offset of the parent entry in 16-byte units}
+    u64* surv_dst;              // ... and where they go: bit 63 set: candidate slot, else 16-byte unit offset in the next
+                                // frontier (its entry index was written to nxt_off by k_compact); ~0: capacity exceeded
     Ctl* ctl;
     u64 n_cur;
     u32 max_entry, cand_stride; // largest entry in bytes (shared-memory staging), candidate slot stride

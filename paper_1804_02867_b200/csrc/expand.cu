@@ -611,50 +611,94 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
 // Balanced children (kKeyDone) and active children with key < X (all of them when the beam does not bind).  A block
 // appends the survivors of a tile with ONE atomic (a warp-level atomic per 32 keys serialised on the counter); the order
 // of the list does not matter.
-constexpr int kCompactItems = 4;   // keys per thread: a block appends the survivors of 1024 keys with one atomic
-__global__ void __launch_bounds__(256) k_compact(const u64* __restrict__ keys, const uint4* __restrict__ t0, const u64* __restrict__ cur_off,
-                                                 ulonglong2* __restrict__ surv, Ctl* ctl, u64 max_keys) {
-    __shared__ u32 s_warp[8];
-    __shared__ u64 s_base;
-    const u64 n = min(ctl->n_slots, max_keys);
+constexpr int kCompactItems = 4;   // keys per thread: a block handles the survivors of 1024 keys with one atomic per counter
+// Besides listing the survivors, the kernel sizes every child (task + parent header) and reserves its place: an entry
+// index and 16-byte units in the next frontier, or a candidate slot.  k_materialise then needs no coordination at all.
+__global__ void __launch_bounds__(256) k_compact(const __grid_constant__ ExpandArgs A) {
+    __shared__ u32 s_w[4][8];      // per warp totals: survivors, frontier children, frontier units, candidates
+    __shared__ u64 s_base[4];
+    Ctl* ctl = A.ctl;
+    const u64 n = min(ctl->n_slots, A.max_keys);
     const bool notrunc = ctl->notrunc != 0;
     const u64 X = ctl->X;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     constexpr u64 kTile = 256 * kCompactItems;
     for (u64 tile = (u64)blockIdx.x * kTile; tile < n; tile += (u64)gridDim.x * kTile) {   // block-uniform trip count
-        // item j of a thread is key tile + j * 256 + threadIdx.x (coalesced); survivors are numbered warp by warp
-        u32 takes = 0;
-        u32 wm[kCompactItems];
+        // item j of a thread is key tile + j * 256 + threadIdx.x (coalesced loads)
+        u32 takes = 0, my_front = 0, my_units = 0, my_cand = 0, my_bytes = 0;
+        u32 units[kCompactItems];
+        u64 poff[kCompactItems];
 #pragma unroll
         for (int j = 0; j < kCompactItems; ++j) {
             const u64 i = tile + (u64)j * 256 + threadIdx.x;
-            const u64 key = i < n ? __ldcs(&keys[i]) : kKeySentinel;
+            const u64 key = i < n ? __ldcs(&A.keys[i]) : kKeySentinel;
             const bool take = key == kKeyDone || (key != kKeySentinel && (notrunc || key < X));
-            wm[j] = __ballot_sync(0xffffffffu, take);
-            if (take) takes |= 1u << j;
+            units[j] = 0; poff[j] = 0;
+            if (take) {
+                takes |= 1u << j;
+                const uint4 q0 = __ldcs(&A.t0[i]);
+                poff[j] = __ldg(&A.cur_off[q0.x]);
+                const u32 w0 = __ldg((const u32*)(A.cur + (poff[j] << 4)));
+                const u32 ns = w0 & 0xffffu, nv = w0 >> 16, cnu = q0.z & 0xffffu, fl = q0.z >> 16;
+                const u32 n2 = ns + ((fl & TF_INSUPP) ? 0u : 1u), nv2 = nv + ((fl & TF_FIRST) ? 1u : 0u);
+                my_bytes += algo_entry_bytes(n2, nv2);
+                if (cnu == 0) my_cand++;
+                else { units[j] = entry_bytes(n2, nv2, cnu) >> 4; my_front++; my_units += units[j]; }
+            }
         }
-        u32 wtot = 0;
+        // exclusive prefix over the threads of the block for the four counters (warp scan + warp totals)
+        u32 v[4] = {(u32)__popc(takes), my_front, my_units, my_cand};
+        u32 ex[4];
 #pragma unroll
-        for (int j = 0; j < kCompactItems; ++j) wtot += __popc(wm[j]);
-        if (lane == 0) s_warp[wib] = wtot;
+        for (int c = 0; c < 4; ++c) {
+            u32 x = v[c];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const u32 y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+            ex[c] = x - v[c];
+            if (lane == 31) s_w[c][wib] = x;
+        }
+        my_bytes = __reduce_add_sync(0xffffffffu, my_bytes);
+        __syncthreads();
+        if (threadIdx.x < 4) {
+            const int c = threadIdx.x;
+            u32 tot = 0;
+            for (int w = 0; w < 8; ++w) { const u32 t = s_w[c][w]; s_w[c][w] = tot; tot += t; }
+            if (c == 0) s_base[0] = tot ? atomicAdd(&ctl->n_surv, (u64)tot) : 0ULL;
+            if (c == 1) s_base[1] = tot;                      // frontier children of the block (combined with c == 2 below)
+            if (c == 2) s_base[2] = tot;
+            if (c == 3) s_base[3] = tot ? atomicAdd(&ctl->n_cand, (u64)tot) : 0ULL;
+        }
+        if (lane == 0 && my_bytes) atomicAdd(&ctl->st[ST_ALGO_BYTES], (u64)my_bytes);
         __syncthreads();
         if (threadIdx.x == 0) {
-            u32 tot = 0;
-            for (int w = 0; w < 8; ++w) { const u32 c = s_warp[w]; s_warp[w] = tot; tot += c; }
-            s_base = tot ? atomicAdd(&ctl->n_surv, (u64)tot) : 0ULL;
+            const u64 nf = s_base[1], nu = s_base[2];
+            const u64 old = nf ? atomicAdd(&ctl->n_next, (nf << kAllocShift) | nu) : 0ULL;
+            s_base[1] = old >> kAllocShift; s_base[2] = old & kAllocUnitMask;
         }
         __syncthreads();
-        u64 pos = s_base + s_warp[wib];
+        u64 pos = s_base[0] + s_w[0][wib] + ex[0];
+        u64 fidx = s_base[1] + s_w[1][wib] + ex[1], foff = s_base[2] + s_w[2][wib] + ex[2];
+        u64 cidx = s_base[3] + s_w[3][wib] + ex[3];
 #pragma unroll
         for (int j = 0; j < kCompactItems; ++j) {
             if ((takes >> j) & 1u) {
                 const u64 i = tile + (u64)j * 256 + threadIdx.x;
-                // the survivor record carries the offset of its parent: one dependent load less in k_materialise
-                surv[pos + __popc(wm[j] & ((1u << lane) - 1u))] = make_ulonglong2(i, __ldg(&cur_off[__ldcs(&t0[i]).x]));
+                u64 dst;
+                if (units[j] == 0) {   // candidate
+                    if (cidx >= A.max_cand) { atomicOr(&ctl->error, (u32)ERR_CAND); dst = ~0ULL; }
+                    else dst = (1ULL << 63) | cidx;
+                    ++cidx;
+                } else {
+                    if (fidx >= A.max_frontier || foff + units[j] > A.frontier_units) { atomicOr(&ctl->error, (u32)ERR_FRONTIER); dst = ~0ULL; }
+                    else { dst = foff; A.nxt_off[fidx] = foff; }
+                    ++fidx; foff += units[j];
+                }
+                A.surv[pos] = make_ulonglong2(i, poff[j]);
+                A.surv_dst[pos] = dst;
+                ++pos;
             }
-            pos += __popc(wm[j]);
         }
-        __syncthreads();   // s_warp / s_base are reused by the next tile
+        __syncthreads();   // the shared arrays are reused by the next tile
     }
 }
 
@@ -678,22 +722,20 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
     const int gshift = threadIdx.x & 31 & ~(G - 1);
     auto gballot = [&](bool pred) -> u32 { return (__ballot_sync(gmask, pred) >> gshift) & gbits; };
     auto gany = [&](bool pred) -> bool { return __any_sync(gmask, pred) != 0; };
-    __shared__ u32 s_units[kMatWarps];
-    __shared__ u64 s_base[kMatWarps];
-    __shared__ u64 s_slot[kMatWarps];
-    __shared__ u32 s_bytes[kMatWarps];
     const int lane = threadIdx.x & (G - 1), wib = threadIdx.x / G;   // lane within the child's group, group within the block
     const u32 lt = (1u << lane) - 1u;
     Ctl* ctl = A.ctl;
     const u64 n_surv = ctl->n_surv;
-    for (u64 blk = blockIdx.x; blk * kMatWarps < n_surv; blk += gridDim.x) {   // block-uniform trip count
-    const u64 sidx = blk * kMatWarps + wib;
-    const bool live = sidx < n_surv;
+    // k_compact reserved the place of every child: the groups work on their own, no block-wide step is left
+    for (u64 sidx = (u64)blockIdx.x * kMatWarps + wib; sidx < n_surv; sidx += (u64)gridDim.x * kMatWarps) {
+    const bool live = true;
     // ---- the task
     uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0, q2 = q0, q3 = q0, h0 = q0;
+    u64 dstrec = ~0ULL;
     const unsigned char* pe = A.cur;
     if (live) {
         const ulonglong2 sv = __ldcs(&A.surv[sidx]);
+        dstrec = __ldcs(&A.surv_dst[sidx]);
         const u64 slot = sv.x;
         pe = A.cur + (sv.y << 4);
         q0 = __ldcs(&A.t0[slot]); q1 = __ldcs(&A.t1[slot]); q2 = __ldcs(&A.t2[slot]); q3 = __ldcs(&A.t3[slot]);
@@ -737,38 +779,8 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
             pcol0 = __ldg(&A.g.col_ptr[ca]); pcol1 = __ldg(&A.g.col_ptr[ca + 1]);
         }
     }
-    // ---- reserve the output of the whole block: one atomic for the frontier entries, one for the candidates
-    if (lane == 0) {
-        s_units[wib] = units; s_slot[wib] = (live && to_cand) ? 1 : 0;
-        s_bytes[wib] = live ? algo_entry_bytes((u32)n2, (u32)(nv + (firstv ? 1 : 0))) : 0u;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        u64 tot_units = 0, n_front = 0, n_cand = 0, bytes = 0;
-        for (int w = 0; w < kMatWarps; ++w) { tot_units += s_units[w]; n_front += s_units[w] != 0; n_cand += s_slot[w]; bytes += s_bytes[w]; }
-        if (bytes) atomicAdd(&ctl->st[ST_ALGO_BYTES], bytes);
-        u64 fbase = 0, cbase = 0;
-        if (n_front) fbase = atomicAdd(&ctl->n_next, (n_front << kAllocShift) | tot_units);
-        if (n_cand) cbase = atomicAdd(&ctl->n_cand, n_cand);
-        u64 fs = fbase >> kAllocShift, fo = fbase & kAllocUnitMask;
-        for (int w = 0; w < kMatWarps; ++w) {
-            if (s_units[w]) { const u32 un = s_units[w]; s_base[w] = fo; s_slot[w] = fs++; fo += un; }
-            else if (s_slot[w]) { s_slot[w] = cbase++; }
-        }
-    }
-    __syncthreads();
-    bool ok = live;
-    unsigned char* dst = nullptr;
-    if (live && to_cand) {
-        const u64 slot = s_slot[wib];
-        if (slot >= A.max_cand) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_CAND); ok = false; }
-        dst = A.cand + slot * A.cand_stride;
-    } else if (live) {
-        const u64 slot = s_slot[wib], off = s_base[wib];
-        if (slot >= A.max_frontier || off + units > A.frontier_units) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_FRONTIER); ok = false; }
-        else if (lane == 0) A.nxt_off[slot] = off;
-        dst = A.nxt + (off << 4);
-    }
+    const bool ok = dstrec != ~0ULL;   // ~0: a capacity error was flagged by k_compact
+    unsigned char* dst = (dstrec >> 63) ? A.cand + (dstrec & ~(1ULL << 63)) * A.cand_stride : A.nxt + (dstrec << 4);
     if (ok) {
     // ---- write
     int ins = 0;   // a new arc goes where the ascending order puts it
@@ -860,7 +872,6 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
         h4[1] = make_uint4((u32)chv, (u32)(chv >> 32), (u32)mx, (u32)(mx >> 32));
     }
     }   // ok
-    __syncthreads();   // the reservation arrays are reused by the next round of the block
     }
 }
 
@@ -992,7 +1003,7 @@ cudaError_t launch_materialise(const ExpandArgs& a, u64 n_slots_hint, u64 n_surv
         u64 blocks = (n_slots_hint + 1023) / 1024;   // one tile of 256 x kCompactItems keys per block and round
         if (blocks > (u64)sm_count * 64) blocks = (u64)sm_count * 64;
         if (blocks < 1) blocks = 1;
-        k_compact<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.t0, a.cur_off, a.surv, a.ctl, a.max_keys);
+        k_compact<<<(unsigned)blocks, 256, 0, s>>>(a);
         return cudaGetLastError();
     }
     (void)n_surv;   // read on the device (ctl->n_surv): no host round trip between the two kernels
