@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
         const u32 nch = entry_bytes((u32)ns, (u32)nv, (u32)nu) / 16;
         // entries that fit the staging buffer are read from shared memory; the rare larger ones are read in place
         const bool staged = !A.force_inplace && nch * 16 <= A.sm_stage_bytes;
-        if (staged) {
+        if (__builtin_expect(staged, 1)) {
             #pragma unroll 1
             for (u32 c = pre_chunks + lane; c < nch; c += G) stage[c] = __ldcs(src + c);   // streaming: the frontier must not evict the graph from L1
         }
@@ -380,7 +380,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
             }
             if (lane == 0) sst[SS_ROUNDS]++;
             const u32 adm_m = gballot(adm);
-            if (adm_m == 0) continue;
+            if (__builtin_expect(adm_m == 0, 0)) continue;
             n_adm += __popc(adm_m);
             // ---- lane-parallel evaluation: new arc, small integers => no overflow, no common factor
             const bool fast = adm && !insup && fastP && !generic;
@@ -526,7 +526,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     if (__any_sync(gmask, ovf2)) status = CH_OVERFLOW;
                     else cnu = nu + __reduce_add_sync(gmask, delta);
                 }
-                if (status != CH_OK) {
+                if (__builtin_expect(status != CH_OK, 0)) {
                     if (lane == 0) sst[status == CH_OVERFLOW ? SS_OVF : SS_NONPOS]++;
                     continue;
                 }
