@@ -220,8 +220,6 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     efm_handle* h = new (std::nothrow) efm_handle();
     if (!h) return EFM_E_NOMEM;
     memset(&h->stats, 0, sizeof h->stats);
-    cudaEvent_t t0 = nullptr;
-    (void)t0;
     const auto c0 = std::clock();
     h->L = P.dep_depth ? P.dep_depth : 4;
     int rc = build_graph(h->G, S, m, n, row_stride, reversible, internal, h->L);

@@ -196,7 +196,6 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
     const int gshift = threadIdx.x & 31 & ~(G - 1);
     const u32 gmask = gbits << gshift;
     auto gballot = [&](bool pred) -> u32 { return (__ballot_sync(gmask, pred) >> gshift) & gbits; };
-    const u32 lt = (1u << lane) - 1u;
     unsigned char* gs = (unsigned char*)smem4 + (size_t)wib * A.sm_group;
     uint4* stage = (uint4*)gs;
     u32* sbits = (u32*)(gs + A.sm_sbits);   // support bitset over arcs
@@ -724,23 +723,16 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
     auto gany = [&](bool pred) -> bool { return __any_sync(gmask, pred) != 0; };
     const int lane = threadIdx.x & (G - 1), wib = threadIdx.x / G;   // lane within the child's group, group within the block
     const u32 lt = (1u << lane) - 1u;
-    Ctl* ctl = A.ctl;
-    const u64 n_surv = ctl->n_surv;
+    const u64 n_surv = A.ctl->n_surv;
     // k_compact reserved the place of every child: the groups work on their own, no block-wide step is left
     for (u64 sidx = (u64)blockIdx.x * kMatWarps + wib; sidx < n_surv; sidx += (u64)gridDim.x * kMatWarps) {
-    const bool live = true;
-    // ---- the task
-    uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0, q2 = q0, q3 = q0, h0 = q0;
-    u64 dstrec = ~0ULL;
-    const unsigned char* pe = A.cur;
-    if (live) {
-        const ulonglong2 sv = __ldcs(&A.surv[sidx]);
-        dstrec = __ldcs(&A.surv_dst[sidx]);
-        const u64 slot = sv.x;
-        pe = A.cur + (sv.y << 4);
-        q0 = __ldcs(&A.t0[slot]); q1 = __ldcs(&A.t1[slot]); q2 = __ldcs(&A.t2[slot]); q3 = __ldcs(&A.t3[slot]);
-        h0 = __ldg((const uint4*)pe);
-    }
+    // ---- the task, the reserved place, the header of the parent
+    const ulonglong2 sv = __ldcs(&A.surv[sidx]);
+    const u64 dstrec = __ldcs(&A.surv_dst[sidx]);
+    const u64 slot = sv.x;
+    const unsigned char* pe = A.cur + (sv.y << 4);
+    const uint4 q0 = __ldcs(&A.t0[slot]), q1 = __ldcs(&A.t1[slot]), q2 = __ldcs(&A.t2[slot]), q3 = __ldcs(&A.t3[slot]);
+    const uint4 h0 = __ldg((const uint4*)pe);
     const int ca = (int)(q0.y & 0xffffu);
     const int cia = (q0.y >> 16) == 0xffffu ? -1 : (int)(q0.y >> 16);
     const int cnu = (int)(q0.z & 0xffffu);
@@ -762,14 +754,13 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
     const int n2 = ns + (cin ? 0 : 1);
     const int nv2 = to_cand ? 0 : nv + (firstv ? 1 : 0);
     const int nu2 = to_cand ? 0 : cnu;
-    const u32 units = live ? (to_cand ? 0u : entry_bytes((u32)n2, (u32)nv2, (u32)nu2) >> 4) : 0u;
     // ---- every element of the parent this lane will need, requested before anything waits: the loads overlap each
-    // other and the block-wide reservation below (entries beyond 2 G arcs / records are loaded where they are used)
+    // other (entries beyond 2 G arcs / records are loaded where they are used)
     u32 pa0 = 0xffffffffu, pa1 = 0xffffffffu, pm0 = 0xffffffffu;
     i64 pf0 = 0, pf1 = 0, pe0 = 0;
     u64 pv0 = 0, pv1 = 0;
     int pcol0 = 0, pcol1 = 0;
-    if (live) {
+    {
         if (lane < ns) { pa0 = arc[lane]; pf0 = flux[lane]; }
         if (lane + G < ns) { pa1 = arc[lane + G]; pf1 = flux[lane + G]; }
         if (!to_cand) {
