@@ -627,18 +627,29 @@ __global__ void __launch_bounds__(256) k_compact(const __grid_constant__ ExpandA
         u32 takes = 0, my_front = 0, my_units = 0, my_cand = 0, my_bytes = 0;
         u32 units[kCompactItems];
         u64 poff[kCompactItems];
+        // the four items of a thread advance together through the chain key -> task word -> parent offset -> parent header,
+        // so that a thread waits for three memory latencies, not twelve
 #pragma unroll
         for (int j = 0; j < kCompactItems; ++j) {
             const u64 i = tile + (u64)j * 256 + threadIdx.x;
             const u64 key = i < n ? __ldcs(&A.keys[i]) : kKeySentinel;
-            const bool take = key == kKeyDone || (key != kKeySentinel && (notrunc || key < X));
-            units[j] = 0; poff[j] = 0;
-            if (take) {
-                takes |= 1u << j;
-                const uint4 q0 = __ldcs(&A.t0[i]);
-                poff[j] = __ldg(&A.cur_off[q0.x]);
-                const u32 w0 = __ldg((const u32*)(A.cur + (poff[j] << 4)));
-                const u32 ns = w0 & 0xffffu, nv = w0 >> 16, cnu = q0.z & 0xffffu, fl = q0.z >> 16;
+            if (key == kKeyDone || (key != kKeySentinel && (notrunc || key < X))) takes |= 1u << j;
+        }
+        u32 qx[kCompactItems], qz[kCompactItems], w0[kCompactItems];
+#pragma unroll
+        for (int j = 0; j < kCompactItems; ++j) {
+            qx[j] = 0; qz[j] = 0;
+            if ((takes >> j) & 1u) { const uint4 q0 = __ldcs(&A.t0[tile + (u64)j * 256 + threadIdx.x]); qx[j] = q0.x; qz[j] = q0.z; }
+        }
+#pragma unroll
+        for (int j = 0; j < kCompactItems; ++j) poff[j] = ((takes >> j) & 1u) ? __ldg(&A.cur_off[qx[j]]) : 0ULL;
+#pragma unroll
+        for (int j = 0; j < kCompactItems; ++j) w0[j] = ((takes >> j) & 1u) ? __ldg((const u32*)(A.cur + (poff[j] << 4))) : 0u;
+#pragma unroll
+        for (int j = 0; j < kCompactItems; ++j) {
+            units[j] = 0;
+            if ((takes >> j) & 1u) {
+                const u32 ns = w0[j] & 0xffffu, nv = w0[j] >> 16, cnu = qz[j] & 0xffffu, fl = qz[j] >> 16;
                 const u32 n2 = ns + ((fl & TF_INSUPP) ? 0u : 1u), nv2 = nv + ((fl & TF_FIRST) ? 1u : 0u);
                 my_bytes += algo_entry_bytes(n2, nv2);
                 if (cnu == 0) my_cand++;
