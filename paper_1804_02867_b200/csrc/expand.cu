@@ -32,9 +32,13 @@ constexpr int kWarps = kBlock / 32;
 #define EFM_PPW 8
 #endif
 constexpr int kParentsPerWarp = EFM_PPW;
+#ifndef EFM_STAGE_BYTES
+#define EFM_STAGE_BYTES 1536
+#endif
+constexpr int kStageBytes = EFM_STAGE_BYTES;   // staging buffer per parent (larger entries are read in place)
 static_assert(kParentsPerWarp <= 8, "SS_OFF holds 8 parent offsets");
 #ifndef EFM_PREFETCH
-#define EFM_PREFETCH 1536
+#define EFM_PREFETCH EFM_STAGE_BYTES
 #endif
 constexpr int kPrefetch = EFM_PREFETCH;   // bytes of the next parent requested ahead (1536 = the whole staging buffer: 41.7 ms, 1024: 42.2 ms)
 constexpr u32 FULL = 0xffffffffu;
@@ -957,7 +961,7 @@ static size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 void expand_smem_layout(ExpandArgs& a) {
     // staging: the largest entry if it is small, otherwise 1.5 KB (larger entries are rare and read in place);
     // the smaller the per-warp footprint, the more of the graph stays in L1
-    a.sm_stage_bytes = (u32)align16(a.max_entry < 1536u ? (a.max_entry < 32u ? 32u : a.max_entry) : 1536u);
+    a.sm_stage_bytes = (u32)align16(a.max_entry < (u32)kStageBytes ? (a.max_entry < 32u ? 32u : a.max_entry) : (u32)kStageBytes);
     size_t off = 2 * (size_t)a.sm_stage_bytes;   // two staging buffers
     a.sm_sbits = (u32)off; off = align16(off + (size_t)a.g.W32 * 4);
     a.sm_upos = (u32)off;  off = align16(off + (size_t)a.g.M * 2 + 16);   // zeroed in 16-byte chunks
