@@ -113,7 +113,7 @@ def test_core_beam(efm, oracle_mod, cap):
     assert got.stats["truncated_beam"] > 0
 
 
-@pytest.mark.parametrize("cap", [512, 16384])
+@pytest.mark.parametrize("cap", [512, 16384, 65536])
 def test_mid(efm, oracle_mod, cap):
     net = make_network("mid", 0)
     got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=cap)
@@ -207,6 +207,14 @@ def test_degenerate_inputs(efm, oracle_mod):
     with pytest.raises(efm.EfmError) as ei:
         efm.enumerate_network(net, max_candidates=4)
     assert ei.value.code == efm.EFM_E_CAPACITY
+    # the packed frontier buffer can be sized in bytes: too few bytes for the peak level is a capacity error as well,
+    # enough bytes (far below entries x worst case) gives the same result
+    with pytest.raises(efm.EfmError) as ei:
+        efm.enumerate_network(net, max_frontier_bytes=64 * 1024)
+    assert ei.value.code == efm.EFM_E_CAPACITY
+    ref = efm.enumerate_network(net)
+    got = efm.enumerate_network(net, max_frontier_bytes=4 << 20)
+    assert np.array_equal(got.flux, ref.flux)
 
 
 def test_sparse_and_dense_results_agree(efm):
