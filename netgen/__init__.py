@@ -12,5 +12,7 @@ from .networks import (  # noqa: F401
     config_names,
     hand_network,
     make_network,
+    mirrored,
+    random_seed_sets,
     unimolecular_network,
 )

@@ -563,3 +563,28 @@ def unimolecular_network(seed: int, m_int: int, n_rxn: int, n_rev: int = 0) -> N
     A = j + int(rev.sum())
     p = dict(max_support=A, max_loop=8, dep_depth=4, max_visited=2 * A, frontier_cap=0)
     return Network(f"unimolecular-{seed}", seed, S, rev, np.ones(m_int, dtype=np.uint8), p, None, {})
+
+
+def random_seed_sets(net: Network, count: int, size: int, seed: int = 0) -> List[List[int]]:
+    """``count`` seeded random seed sets of ``size`` distinct arcs each (arc codes 2*j + (dir < 0)), never both
+    directions of one reaction.  Multi-arc seed sets reach one support along several routes, which is what exercises
+    the poison rule and the minimality filter."""
+    rng = SplitMix64((seed * 0x9E3779B97F4A7C15 + 0x73656564) & MASK64)
+    codes = []
+    for j in range(net.n):
+        codes.append(2 * j)
+        if net.reversible[j]:
+            codes.append(2 * j + 1)
+    out: List[List[int]] = []
+    while len(out) < count:
+        pick = rng.sample(codes, size)
+        if len({c // 2 for c in pick}) == size:
+            out.append(sorted(pick))
+    return out
+
+
+def mirrored(net: Network) -> Network:
+    """The same network with every reaction reversed (S -> -S); reversibility, masks, parameters and seed sets kept."""
+    return Network(net.name + "-mirrored", net.seed, np.ascontiguousarray(-net.S), net.reversible.copy(),
+                   net.internal.copy(), dict(net.params), None if net.seed_sets is None else [list(s) for s in net.seed_sets],
+                   dict(net.info))

@@ -32,7 +32,7 @@ def build(force: bool = False) -> str:
 class _Params(ctypes.Structure):
     _fields_ = [("max_support", ctypes.c_int32), ("max_loop", ctypes.c_int32), ("dep_depth", ctypes.c_int32),
                 ("max_visited", ctypes.c_int32), ("frontier_cap", ctypes.c_int64), ("threads", ctypes.c_int32),
-                ("reserved", ctypes.c_int32), ("shuffle_seed", ctypes.c_uint64)]
+                ("trace", ctypes.c_int32), ("shuffle_seed", ctypes.c_uint64)]
 
 
 STAT_FIELDS = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxloop", "discarded_nonpos",
@@ -66,6 +66,8 @@ def _load():
         lib.oracle_graph_info.argtypes = [ctypes.c_void_p] + [ctypes.c_void_p] * 5
         lib.oracle_graph_export.argtypes = [ctypes.c_void_p] + [ctypes.c_void_p] * 14
         lib.oracle_result_free.argtypes = [ctypes.c_void_p]
+        lib.oracle_result_trace.restype = ctypes.c_int64
+        lib.oracle_result_trace.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64]
         lib.oracle_state_hash.restype = ctypes.c_uint64
         lib.oracle_state_hash.argtypes = [ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
                                           ctypes.c_void_p]
@@ -87,6 +89,9 @@ class OracleResult:
     levels: Dict[str, np.ndarray]  # per level: active, done, expanded, children
     n_roots: int
     graph: Optional[Dict[str, np.ndarray]] = None
+    # test hook (trace=True): per level the list of entries as dicts
+    # {flux: {arc: f}, visited: {met: (PI, PO, cnt)}, n_unb, istar, key, kept}
+    trace: Optional[List[List[dict]]] = None
 
 
 def _ptr(a: np.ndarray):
@@ -96,7 +101,7 @@ def _ptr(a: np.ndarray):
 def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarray, params: Dict[str, int],
                        seed_sets: Optional[Sequence[Sequence[int]]] = None, threads: int = 1,
                        shuffle_seed: int = 0, export_graph: bool = False,
-                       self_check: bool = True) -> OracleResult:
+                       self_check: bool = True, trace: bool = False) -> OracleResult:
     """Run the oracle.  ``seed_sets`` holds arc codes 2*j + (dir < 0); None = default boundary arcs (O2)."""
     lib = _load()
     S = np.ascontiguousarray(S, dtype=np.int32)
@@ -104,7 +109,7 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
     internal = np.ascontiguousarray(internal, dtype=np.uint8)
     m, n = S.shape
     p = _Params(int(params.get("max_support", 0)), int(params.get("max_loop", 8)), int(params.get("dep_depth", 4)),
-                int(params.get("max_visited", 0)), int(params.get("frontier_cap", 0)), int(threads), 0,
+                int(params.get("max_visited", 0)), int(params.get("frontier_cap", 0)), int(threads), int(trace),
                 int(shuffle_seed))
     if seed_sets:
         ptr = np.zeros(len(seed_sets) + 1, dtype=np.int32)
@@ -156,9 +161,24 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
             g.update(M=M, A=A, W=W)
             graph = g
         n_roots = int(lib.oracle_result_roots(handle))
+        tr = None
+        if trace:
+            nt = int(lib.oracle_result_trace(handle, None, 0))
+            buf = np.zeros(max(nt, 1), dtype=np.int64)
+            lib.oracle_result_trace(handle, _ptr(buf), nt)
+            tr = [[] for _ in range(nl)]
+            x = 0
+            while x < nt:
+                lvl, ns, nv, nu, istar, key, kept = (int(v) for v in buf[x:x + 7])
+                x += 7
+                fl = {int(buf[x + 2 * k]): int(buf[x + 2 * k + 1]) for k in range(ns)}
+                x += 2 * ns
+                vis = {int(buf[x + 4 * k]): tuple(int(v) for v in buf[x + 4 * k + 1:x + 4 * k + 4]) for k in range(nv)}
+                x += 4 * nv
+                tr[lvl].append(dict(flux=fl, visited=vis, n_unb=nu, istar=istar, key=key & ((1 << 64) - 1), kept=bool(kept)))
     finally:
         lib.oracle_result_free(handle)
-    res = OracleResult(flux, stats, levels, n_roots, graph)
+    res = OracleResult(flux, stats, levels, n_roots, graph, tr)
     if self_check:
         from .check import check_outputs
         check_outputs(S, rev, internal, flux)
@@ -166,7 +186,7 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
 
 
 def enumerate_network(net, threads: int = 1, shuffle_seed: int = 0, export_graph: bool = False,
-                      self_check: bool = True, seed_sets="net", **param_overrides) -> OracleResult:
+                      self_check: bool = True, seed_sets="net", trace: bool = False, **param_overrides) -> OracleResult:
     """Run the oracle on a ``netgen.Network`` with its own parameters (optionally overridden).
 
     ``seed_sets="net"`` uses the network's own seed sets (None there = default boundary arcs)."""
@@ -174,7 +194,7 @@ def enumerate_network(net, threads: int = 1, shuffle_seed: int = 0, export_graph
     params.update(param_overrides)
     seeds = net.seed_sets if isinstance(seed_sets, str) else seed_sets
     return enumerate_pathways(net.S, net.reversible, net.internal, params, seeds, threads, shuffle_seed,
-                              export_graph, self_check)
+                              export_graph, self_check, trace)
 
 
 def state_hash(arcs: Sequence[int], fluxes: Sequence[int], visited: Sequence[Sequence[int]]) -> int:

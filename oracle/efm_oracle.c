@@ -5,13 +5,22 @@
  * ("Readings").  It shares NO code with the CUDA library: only tests/, __graft_entry__.smoke()
  * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
  *
- * What is pinned (tests/test_oracle_pins.py, -m "not gpu"): hand-derived mini networks P1-P6,
- * the unimolecular special case P7 (textbook path/cycle enumeration), invariants P8, brute-force
- * EFM enumeration on the toy config P9, order-independence P10, the beam threshold against a
- * sort-based definition, the state hash against values computed by hand from the formula, the
- * DEP table against exhaustive walk enumeration.  Parity unpinned: the exact output sets of the
- * configs "small".."genome" (no external truth exists; they are held by P8, P10 and by
- * GPU<->oracle parity only).
+ * What is pinned (tests/test_oracle_pins.py, -m "not gpu"; every rule below dies under a one-line mutation):
+ *   - hand-derived mini networks P1-P6 and H1-H8 (tests/golden/hand_pins.json) with the state of every partial pathway
+ *     on every level: Eq 3 scaling, Eq 4 / Eq 5 forward and backward, the Def 11 lookup per (output, input) pair,
+ *     PI / PO = lowest arc (G13), lowest metabolite first (G12), first visit over arcs of the support (G22), gcd
+ *     normalisation (G10), MAX_LOOP / V / D exactly reached and exceeded, the poison rule and the minimality filter;
+ *   - closed forms: linear chains (P6), the 2^62 guard on coefficient chains (3^39 < 2^62 < 3^40, 2^62 vs 2^63, the
+ *     extra-flux guard);
+ *   - the mirror symmetry S -> -S (forward and backward halves of the procedure must agree);
+ *   - unimolecular networks = textbook path / cycle enumeration (P7), brute-force EFM enumeration on toy (P9),
+ *     invariants (P8), order independence (P10), default seeds = boundary arcs;
+ *   - beam B against its sort-based definition restated on the level contents (test hook `trace`), ties;
+ *   - O8(ii)/(iii) restated on the oracle's own balanced entries with multi-arc seed sets (poison and drops occur);
+ *   - the state hash against published SplitMix64 vectors and its written composition; the DEP table against
+ *     exhaustive chain enumeration.
+ * Parity unpinned: the exact output sets of the configs "small".."genome" as a whole (no external truth exists; they
+ * are held by the pins above, which cover every rule that produces them, and by GPU<->oracle parity).
  *
  * Arithmetic: fluxes and extra fluxes are exact integers (reading G10); every product is formed
  * in __int128 so the 2^62 guard (reading G21) can never itself overflow.
@@ -39,7 +48,7 @@ typedef struct {
     int32_t max_visited;   /* V  : max visited metabolites per pathway                     */
     int64_t frontier_cap;  /* beam B: entries expanded per level, 0 = unbounded            */
     int32_t threads;       /* OpenMP threads used over the entries of a level              */
-    int32_t reserved;
+    int32_t trace;         /* 1: record every entry of every level, 2: only the balanced ones (test hook) */
     uint64_t shuffle_seed; /* != 0: permute every level before processing (pin P10)        */
 } oracle_params;
 
@@ -232,11 +241,15 @@ static uint64_t mix64(uint64_t x) { /* splitmix64 finaliser */
     x ^= x >> 27; x *= 0x94D049BB133111EBULL;
     x ^= x >> 31; return x;
 }
-/* h = mix( sum_{a in supp} mix( mix(0x01<<56 | a) + f_a ) + sum_{i visited} mix(0x02<<56 | cnt<<48 | i<<32 | PI<<16 | PO) ) */
+/* State hash h of beam B ("a 64-bit hash of the complete state ... The builder may change h,
+ * but it must be written down once and implemented twice, independently"; reading G16 writes it down):
+ *   h = mix( sum_{a in supp} mix(0x01<<56 | a) * f_a  +  sum_{i visited} mix(0x02<<56 | cnt<<48 | i<<32 | PI<<16 | PO) )
+ * all sums and products modulo 2^64.  The arc part is a multiply-add (universal) hash with one fixed
+ * pseudo-random multiplier per arc, so it is linear in the flux vector. */
 static uint64_t state_hash(const entry *e) {
     uint64_t s = 0;
     for (int k = 0; k < e->n_supp; k++)
-        s += mix64(mix64(0x0100000000000000ULL | (uint64_t)e->arc[k]) + (uint64_t)e->f[k]);
+        s += mix64(0x0100000000000000ULL | (uint64_t)e->arc[k]) * (uint64_t)e->f[k];
     for (int k = 0; k < e->n_vis; k++) {
         const visit *v = &e->vis[k];
         s += mix64(0x0200000000000000ULL | ((uint64_t)v->cnt << 48) | ((uint64_t)v->met << 32) |
@@ -407,7 +420,16 @@ typedef struct {
     graph G;
     int n_roots;
     int have_graph;
+    /* test hook: one record per entry of every level, in the order the level was processed:
+     * level, n_supp, n_vis, n_unb, i* (-1 = balanced), beam key (bit pattern), kept (1 = expanded or balanced),
+     * then n_supp x (arc, flux), then n_vis x (met, PI, PO, cnt) */
+    int64_t *trace; int64_t trace_n, trace_cap;
 } oracle_result;
+
+static void trace_push(oracle_result *R, int64_t v) {
+    if (R->trace_n == R->trace_cap) { R->trace_cap = R->trace_cap ? R->trace_cap * 2 : 1024; R->trace = realloc(R->trace, sizeof(int64_t) * R->trace_cap); }
+    R->trace[R->trace_n++] = v;
+}
 
 static int g_sort_n;
 static int cmp_rows(const void *a, const void *b) {
@@ -554,6 +576,15 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
             for (int64_t x = 0; x < N; x++) if (istar[x] >= 0 && !(keys[x] < X)) { keep[x] = 0; st->truncated_beam++; }
             free(keys); free(sorted);
         }
+        if (P.trace)
+            for (int64_t x = 0; x < N; x++) {
+                const entry *e = level.v[x];
+                if (P.trace == 2 && istar[x] >= 0) continue;   /* 2: balanced entries only */
+                trace_push(R, st->levels - 1); trace_push(R, e->n_supp); trace_push(R, e->n_vis); trace_push(R, nunb[x]);
+                trace_push(R, istar[x]); trace_push(R, (int64_t)beam_key(e, nunb[x])); trace_push(R, keep[x] || istar[x] < 0);
+                for (int k = 0; k < e->n_supp; k++) { trace_push(R, e->arc[k]); trace_push(R, e->f[k]); }
+                for (int k = 0; k < e->n_vis; k++) { trace_push(R, e->vis[k].met); trace_push(R, e->vis[k].PI); trace_push(R, e->vis[k].PO); trace_push(R, e->vis[k].cnt); }
+            }
         /* an expansion reads its parent, writes one 8-byte key per generated child and
          * writes the children that survive (balanced ones and those the beam keeps); roots are not written
          * by an expansion */
@@ -691,9 +722,14 @@ void oracle_graph_export(const oracle_result *R, int32_t *arc_rxn, int32_t *arc_
     for (int q = 0; q < G->col_ptr[G->A]; q++) { col_met[q] = G->col_met[q]; col_s[q] = G->col_s[q]; }
     memcpy(dep, G->dep, G->dep_off[G->M]);
 }
+int64_t oracle_result_trace(const oracle_result *R, int64_t *dst, int64_t cap) {
+    for (int64_t x = 0; x < R->trace_n && x < cap; x++) dst[x] = R->trace[x];
+    return R->trace_n;
+}
 void oracle_result_free(oracle_result *R) {
     if (!R) return;
     if (R->have_graph) graph_free(&R->G);
+    free(R->trace);
     free(R->flux); free(R->lvl_active); free(R->lvl_done); free(R->lvl_expanded); free(R->lvl_children);
     free(R);
 }

@@ -12,7 +12,7 @@ from math import gcd
 import numpy as np
 import pytest
 
-from netgen import SplitMix64, hand_network, make_network, unimolecular_network
+from netgen import SplitMix64, hand_network, make_network, mirrored, random_seed_sets, unimolecular_network
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "hand_pins.json")
 
@@ -22,15 +22,29 @@ def _cases():
         return json.load(fh)["cases"]
 
 
+def _norm_trace_level(states):
+    return sorted((tuple(st["f"]), tuple(sorted(tuple(v) for v in st["vis"]))) for st in states)
+
+
 @pytest.mark.parametrize("case", _cases(), ids=lambda c: c["name"])
 def test_hand_pins(oracle_mod, case):
     rx = [(s, p, r) for s, p, r in case["reactions"]]
-    net = hand_network(rx, case["internal"])
-    res = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, case["seeds"])
+    net = hand_network(rx, case["internal"], **case.get("params", {}))
+    res = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, case["seeds"],
+                                        trace="trace" in case)
     assert res.flux.tolist() == case["flux"]
     for k in ("expanded", "levels", "discarded_nonpos"):
         if k in case:
             assert res.stats[k] == case[k], k
+    for k, v in case.get("stats", {}).items():
+        assert res.stats[k] == v, (k, res.stats[k], v)
+    if "trace" in case:
+        A = net.n_arcs
+        assert len(res.trace) == len(case["trace"])
+        for lvl, (got, want) in enumerate(zip(res.trace, case["trace"])):
+            got_n = sorted((tuple(e["flux"].get(a, 0) for a in range(A)),
+                            tuple(sorted((m,) + v for m, v in e["visited"].items()))) for e in got)
+            assert got_n == _norm_trace_level(want), f"level {lvl}"
 
 
 def test_linear_chain_closed_form(oracle_mod):
@@ -243,7 +257,7 @@ def test_state_hash_structure(oracle_mod):
     assert len(set(variants + [base])) == len(variants) + 1
     m = oracle_mod.mix64
     mask = (1 << 64) - 1
-    one_arc = m((m((1 << 56) | 11) + 6) & mask)
+    one_arc = (m((1 << 56) | 11) * 6) & mask   # multiply-add arc term (reading G16)
     one_vis = m((2 << 56) | (3 << 48) | (5 << 32) | (11 << 16) | 12)
     assert h([11], [6], []) == m(one_arc)
     assert h([11], [6], [(5, 11, 12, 3)]) == m((one_arc + one_vis) & mask)
@@ -324,3 +338,190 @@ def test_seed_validation(oracle_mod):
     for bad in ([[2 * j_rev, 2 * j_rev + 1]], [[2 * j_irr + 1]], [[2 * net.n]], [[0, 0]], [[]]):
         with pytest.raises(ValueError):
             oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, bad)
+
+
+def _chain(coef_cons, length, tail=None):
+    """->A0, c A_t -> A_{t+1} (t < length), A_length ->; optional extra product (name, coefficient) of the source."""
+    names = [f"A{t}" for t in range(length + 1)]
+    src = {names[0]: 1}
+    internal = list(names)
+    if tail:
+        src[tail[0]] = tail[1]
+        internal.append(tail[0])   # highest node index: it is visited last (reading G12)
+    rx = [({}, src, False)]
+    for t in range(length):
+        rx.append(({names[t]: coef_cons}, {names[t + 1]: 1}, False))
+    rx.append(({names[length]: 1}, {}, False))
+    if tail:
+        rx.append(({tail[0]: 1}, {}, False))
+    return hand_network(rx, internal)
+
+
+def test_overflow_guard_closed_form(oracle_mod):
+    """Reading G21 (any state integer above 2^62 discards the pathway) on chains whose fluxes are known in closed form:
+    c A_t -> A_{t+1} multiplies the scale by c per step (Eq 3 with the integer rescaling of reading G10), so the source
+    flux is c^length.  3^39 < 2^62 < 3^40; 2^62 itself is allowed, 2^63 is not; and the guard also covers extra fluxes:
+    a source that makes 3 Z per unit has EF_Z = 3 * 2^k, above 2^62 from k = 61 on while every flux is still below."""
+    def run(net):
+        return oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, [[0]])
+    r = run(_chain(3, 30))
+    assert r.stats["output"] == 1 and int(r.flux.max()) == 3 ** 30 and r.stats["discarded_overflow"] == 0
+    r = run(_chain(3, 39))
+    assert r.stats["output"] == 1 and int(r.flux.max()) == 3 ** 39 and r.stats["discarded_overflow"] == 0
+    assert r.flux.tolist()[0] == [3 ** 39] + [3 ** (38 - t) for t in range(39)] + [1]
+    r = run(_chain(3, 40))
+    assert r.stats["output"] == 0 and r.stats["discarded_overflow"] == 1 and r.stats["expanded"] == 40
+    r = run(_chain(2, 62))
+    assert r.stats["output"] == 1 and int(r.flux.max()) == 2 ** 62 and r.stats["discarded_overflow"] == 0
+    r = run(_chain(2, 63))
+    assert r.stats["output"] == 0 and r.stats["discarded_overflow"] == 1
+    r = run(_chain(2, 60, tail=("Z", 3)))
+    assert r.stats["output"] == 1 and int(r.flux.max()) == 3 * 2 ** 60 and r.stats["discarded_overflow"] == 0
+    r = run(_chain(2, 61, tail=("Z", 3)))
+    assert r.stats["output"] == 0 and r.stats["discarded_overflow"] == 1
+
+
+def test_mirror_symmetry(oracle_mod):
+    """Def 9 treats surplus and deficit symmetrically: forward flow pushes through O, backward flow pulls
+    through I; PROC1/PROC1' and Eq 3-5 come in mirrored pairs (Table 1) and Def 11 reads PO~SI one way
+    and PI~SO the other.  Reversing every reaction (S -> -S) therefore swaps the two halves of the procedure and must
+    reproduce the same flux vectors and the same counters.  With the forward half pinned by the hand cases this pins
+    the backward half (Eq 4 / Eq 5 backward, the PI~SO lookup, PO = lowest consumer)."""
+    cases = [(make_network("toy", 0), None, {}), (make_network("small", 0), None, {}), (make_network("small", 3), None, {}),
+             (make_network("core", 0), None, dict(max_support=12))]
+    net = make_network("toy", 0)
+    cases.append((net, oracle_mod.all_arc_seed_sets(net.reversible), {}))
+    net = make_network("small", 0)
+    cases.append((net, random_seed_sets(net, 60, 2, 5), {}))
+    for seed in range(6):
+        net = unimolecular_network(seed, 5, 9, 2)
+        cases.append((net, oracle_mod.all_arc_seed_sets(net.reversible), {}))
+    n_rev = 0
+    for net, seeds, over in cases:
+        kw = dict(seed_sets=seeds) if seeds is not None else {}
+        a = oracle_mod.enumerate_network(net, self_check=False, **kw, **over)
+        b = oracle_mod.enumerate_network(mirrored(net), self_check=False, **kw, **over)
+        assert np.array_equal(a.flux, b.flux), net.name
+        assert a.stats == b.stats, net.name
+        n_rev += a.stats["expanded"] - a.stats["children"] > 0
+    assert n_rev > 0
+
+
+def _python_state_hash(oracle_mod, e):
+    arcs = sorted(e["flux"])
+    return oracle_mod.state_hash(arcs, [e["flux"][a] for a in arcs], [(m,) + v for m, v in sorted(e["visited"].items())])
+
+
+@pytest.mark.parametrize("name,cap", [("small", 300), ("small", 37), ("core", 512)])
+def test_beam_against_sorted_definition(oracle_mod, name, cap):
+    """Beam B restated on the oracle's own level contents (test hook): key = min(n_unb, 255) << 56 |
+    h >> 8 with n_unb counted here from S_int . v; the level keeps exactly the entries with key <= T*, T* the largest
+    value such that #{key <= T*} <= cap (sort-based, ties stand or fall together)."""
+    net = make_network(name, 0)
+    res = oracle_mod.enumerate_network(net, self_check=False, trace=True, frontier_cap=cap)
+    assert res.stats["truncated_beam"] > 0
+    Sint = net.S[net.internal.astype(bool)].astype(object)
+    arc_col = []
+    for j in range(net.n):
+        arc_col.append((j, 1))
+        if net.reversible[j]:
+            arc_col.append((j, -1))
+    cut_levels = 0
+    truncated = 0
+    for lvl in res.trace:
+        keys = []
+        for e in lvl:
+            v = np.zeros(net.n, dtype=object)
+            for a, f in e["flux"].items():
+                v[arc_col[a][0]] += arc_col[a][1] * f
+            n_unb = int(np.count_nonzero(Sint.dot(v)))
+            assert n_unb == e["n_unb"]
+            if n_unb == 0:
+                assert e["kept"] and e["istar"] < 0
+                continue
+            key = (min(n_unb, 255) << 56) | (_python_state_hash(oracle_mod, e) >> 8)
+            assert key == e["key"]
+            keys.append((key, e["kept"]))
+        if len(keys) <= cap:
+            assert all(k for _, k in keys)
+            continue
+        cut_levels += 1
+        srt = sorted(k for k, _ in keys)
+        # T* = largest value with #{key <= T*} <= cap: walk the distinct keys
+        tstar = -1
+        count = 0
+        i = 0
+        while i < len(srt):
+            j = i
+            while j < len(srt) and srt[j] == srt[i]:
+                j += 1
+            if j > cap:
+                break
+            tstar, count, i = srt[i], j, j
+        assert [kept for _, kept in keys] == [k <= tstar for k, _ in keys]
+        assert count <= cap
+        truncated += len(keys) - count
+    assert cut_levels > 0 and truncated == res.stats["truncated_beam"]
+
+
+def test_beam_ties_stand_or_fall_together(oracle_mod):
+    """Two identical seed sets give identical states, hence equal keys: with cap = 1 neither may be kept (SURVEY.md
+    8(c)-B: 'entries with equal keys stand or fall together ... if even the smallest key bucket exceeds cap, the level
+    empties')."""
+    rx = [({}, {"A": 1}, False), ({"A": 1}, {}, False)]
+    net = hand_network(rx, ["A"], frontier_cap=1)
+    res = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, [[0], [0]])
+    assert res.stats["truncated_beam"] == 2 and res.stats["output"] == 0 and res.stats["expanded"] == 0
+    net2 = hand_network(rx, ["A"], frontier_cap=2)
+    res = oracle_mod.enumerate_pathways(net2.S, net2.reversible, net2.internal, net2.params, [[0], [0]])
+    assert res.stats["truncated_beam"] == 0 and res.flux.tolist() == [[1, 1]]
+
+
+@pytest.mark.parametrize("name,over,count,size", [("small", {}, 200, 2), ("core", dict(frontier_cap=4096), 200, 2),
+                                                  ("small", {}, 120, 3)])
+def test_poison_and_minimality_at_scale(oracle_mod, name, over, count, size):
+    """O8(ii)/(iii) restated on the oracle's own balanced entries (test hook): group the Done states by support; a support
+    with two different vectors is poisoned; among the rest, drop every support that strictly contains another
+    (Def 3).  Multi-arc seed sets make both rules fire."""
+    net = make_network(name, 0)
+    seeds = random_seed_sets(net, count, size, 11)
+    res = oracle_mod.enumerate_network(net, self_check=True, seed_sets=seeds, trace=2, threads=2, **over)
+    groups = {}
+    n_done = 0
+    for lvl in res.trace:
+        for e in lvl:
+            if e["n_unb"] == 0:
+                n_done += 1
+                groups.setdefault(frozenset(e["flux"]), set()).add(tuple(sorted(e["flux"].items())))
+    assert n_done == res.stats["done"]
+    ok = {s: next(iter(v)) for s, v in groups.items() if len(v) == 1}
+    poisoned = len(groups) - len(ok)
+    minimal = [s for s in ok if not any(o < s for o in ok)]
+    arc_col = []
+    for j in range(net.n):
+        arc_col.append((j, 1))
+        if net.reversible[j]:
+            arc_col.append((j, -1))
+    rows = []
+    for s in minimal:
+        v = [0] * net.n
+        for a, f in ok[s]:
+            v[arc_col[a][0]] += arc_col[a][1] * f
+        rows.append(v)
+    rows.sort()
+    assert res.stats["unique_supports"] == len(groups) and res.stats["poisoned"] == poisoned
+    assert res.flux.tolist() == rows
+    assert poisoned > 0 and len(ok) - len(minimal) > 0   # both rules did something
+
+
+def test_default_seeds_are_the_boundary_arcs(oracle_mod):
+    """O2 / Def 8 'starting from a boundary reaction': without explicit seeds there is one root per arc whose
+    internal column is non-empty and single-signed.  P5 network: r0 ->A, r1 A<=>B, r2 B->, r3 ->B, r4 A->: the boundary
+    arcs are r0, r2, r3, r4 (codes 0, 4, 6, 8); neither direction of r1 is one; an all-external reaction is none either."""
+    rx = [({}, {"A": 1}, False), ({"A": 1}, {"B": 1}, True), ({"B": 1}, {}, False), ({}, {"B": 1}, False), ({"A": 1}, {}, False),
+          ({"X": 1}, {"Y": 1}, False)]
+    net = hand_network(rx, ["A", "B"])
+    dflt = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, None)
+    expl = oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, [[0], [4], [6], [8]])
+    assert dflt.n_roots == 4 and dflt.stats == expl.stats and np.array_equal(dflt.flux, expl.flux)
+    assert dflt.flux.tolist() == [[0, -1, 0, 1, 1, 0], [0, 0, 1, 1, 0, 0], [1, 0, 0, 0, 1, 0], [1, 1, 1, 0, 0, 0]]
