@@ -3,7 +3,7 @@
 // (roots, classify, beam select, expand, dedup, minimality filter, canonical output) runs in the kernels.
 #include <algorithm>
 #include <cstdio>
-#include <ctime>
+#include <chrono>
 #include <cstddef>
 #include <cstring>
 #include <new>
@@ -53,6 +53,7 @@ struct efm_handle {
     std::string last_error;
     Ctl* h_ctl = nullptr;   // pinned host mirror of the control block
     int sm_count = 148;
+    cudaStream_t stream = nullptr;   // stream of the last efm_enumerate(): the result accessors without a stream argument use it
     std::vector<cudaEvent_t> events;
 };
 
@@ -176,6 +177,17 @@ std::vector<uint32_t> alt_records(const HostGraph& G, const std::vector<ArcRef>&
     return out;
 }
 
+// The API calls run on the handle's device and leave the caller's current device as they found it.
+struct DeviceGuard {
+    int prev = -1; bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; cudaGetLastError(); }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) { ok = false; }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define ON_DEVICE(h) DeviceGuard dg__((h)->device); if (!dg__.ok) return fail_cuda((h), cudaGetLastError(), "cudaSetDevice")
+
 // Events for the optional per-phase timers.
 struct Timer {
     efm_handle* h; cudaStream_t s; bool on; size_t used = 0;
@@ -220,11 +232,11 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     efm_handle* h = new (std::nothrow) efm_handle();
     if (!h) return EFM_E_NOMEM;
     memset(&h->stats, 0, sizeof h->stats);
-    const auto c0 = std::clock();
+    const auto c0 = std::chrono::steady_clock::now();
     h->L = P.dep_depth ? P.dep_depth : 4;
     int rc = build_graph(h->G, S, m, n, row_stride, reversible, internal, h->L);
     if (rc != EFM_OK) { delete h; return rc; }
-    h->ms_build = 1000.0 * (double)(std::clock() - c0) / CLOCKS_PER_SEC;
+    h->ms_build = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - c0).count();   // wall time
     const HostGraph& G = h->G;
     h->D = P.max_support ? P.max_support : G.A;
     if (h->D > G.A) h->D = std::max(G.A, 1);
@@ -361,13 +373,15 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     if ((int64_t)(stage_units << 4) > h->frontier_bytes || h_seed_arc.size() * sizeof(int) > (size_t)h->max_keys * 8)
         return EFM_E_CAPACITY;
 
-    CK(cudaSetDevice(h->device));
+    ON_DEVICE(h);
     if (!h->h_ctl) {
         CK(cudaMallocHost((void**)&h->h_ctl, sizeof(Ctl)));
         int smc = 0;
         CK(cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, h->device));
         if (smc > 0) h->sm_count = smc;
     }
+    memset(h->h_ctl, 0, sizeof(Ctl));   // a run without roots reads no control block: its counters are zero, not stale
+    h->stream = (cudaStream_t)cuda_stream;
     unsigned char* ws = (unsigned char*)d_workspace;
     h->ws = ws;
     Timer tm{h, s, (h->flags & EFM_F_TIMING) != 0};
@@ -637,7 +651,7 @@ int efm_result_densify(const efm_handle* hc, int64_t row0, int64_t n_rows, int64
     if (!h || !d_out || row0 < 0 || n_rows < 0) return EFM_E_INVAL;
     if (!h->have_result) return EFM_E_STATE;
     if (row0 + n_rows > h->n_out) return EFM_E_INVAL;
-    CK(cudaSetDevice(h->device));
+    ON_DEVICE(h);
     CK(launch_densify((const int*)(h->ws + h->lay.r_nnz.off), (const int*)(h->ws + h->lay.r_rxn.off),
                       (const i64*)(h->ws + h->lay.r_val.off), h->D, h->G.n, row0, n_rows, (i64*)d_out, (cudaStream_t)cuda_stream));
     return EFM_OK;
@@ -649,16 +663,16 @@ int efm_result_copy(const efm_handle* hc, int64_t* flux, int64_t capacity_rows) 
     if (!h->have_result) return EFM_E_STATE;
     if (capacity_rows < h->n_out) return EFM_E_INVAL;
     if (h->n_out == 0) return EFM_OK;
-    CK(cudaSetDevice(h->device));
+    ON_DEVICE(h);
     const int64_t n = h->G.n;
     const int64_t chunk = std::max<int64_t>(1, (int64_t)(h->lay.dense.bytes / ((size_t)n * 8)));
     i64* d_dense = (i64*)(h->ws + h->lay.dense.off);
     for (int64_t r0 = 0; r0 < h->n_out; r0 += chunk) {
         const int64_t nr = std::min(chunk, h->n_out - r0);
         CK(launch_densify((const int*)(h->ws + h->lay.r_nnz.off), (const int*)(h->ws + h->lay.r_rxn.off),
-                          (const i64*)(h->ws + h->lay.r_val.off), h->D, (int)n, r0, nr, d_dense, 0));
-        CK(cudaMemcpyAsync(flux + r0 * n, d_dense, (size_t)nr * n * 8, cudaMemcpyDeviceToHost, 0));
-        CK(cudaStreamSynchronize(0));
+                          (const i64*)(h->ws + h->lay.r_val.off), h->D, (int)n, r0, nr, d_dense, h->stream));
+        CK(cudaMemcpyAsync(flux + r0 * n, d_dense, (size_t)nr * n * 8, cudaMemcpyDeviceToHost, h->stream));
+        CK(cudaStreamSynchronize(h->stream));
     }
     return EFM_OK;
 }
@@ -676,7 +690,7 @@ int efm_result_copy_csr(const efm_handle* hc, int64_t* row_ptr, int32_t* rxn, in
     if (!h->have_result) return EFM_E_STATE;
     if (h->n_out == 0) { row_ptr[0] = 0; return EFM_OK; }
     if (!rxn || !val) return EFM_E_INVAL;
-    CK(cudaSetDevice(h->device));
+    ON_DEVICE(h);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const size_t K = (size_t)h->n_out, Z = (size_t)h->csr_nnz;
     CK(cudaMemcpyAsync(row_ptr, h->ws + h->lay.csr_ptr.off, (K + 1) * 8, cudaMemcpyDeviceToHost, s));
@@ -692,11 +706,12 @@ int efm_result_copy_sparse(const efm_handle* hc, int32_t* nnz, int32_t* rxn, int
     if (!h->have_result) return EFM_E_STATE;
     if (capacity_rows < h->n_out) return EFM_E_INVAL;
     if (h->n_out == 0) return EFM_OK;
-    CK(cudaSetDevice(h->device));
+    ON_DEVICE(h);
     const size_t K = (size_t)h->n_out;
-    if (nnz) CK(cudaMemcpy(nnz, h->ws + h->lay.r_nnz.off, K * 4, cudaMemcpyDeviceToHost));
-    if (rxn) CK(cudaMemcpy(rxn, h->ws + h->lay.r_rxn.off, K * h->D * 4, cudaMemcpyDeviceToHost));
-    if (val) CK(cudaMemcpy(val, h->ws + h->lay.r_val.off, K * h->D * 8, cudaMemcpyDeviceToHost));
+    if (nnz) CK(cudaMemcpyAsync(nnz, h->ws + h->lay.r_nnz.off, K * 4, cudaMemcpyDeviceToHost, h->stream));
+    if (rxn) CK(cudaMemcpyAsync(rxn, h->ws + h->lay.r_rxn.off, K * h->D * 4, cudaMemcpyDeviceToHost, h->stream));
+    if (val) CK(cudaMemcpyAsync(val, h->ws + h->lay.r_val.off, K * h->D * 8, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
     return EFM_OK;
 }
 

@@ -49,7 +49,7 @@ struct DevGraph {
     const int* twin;
     const i64* dep_off;   const u32* dep_bits;
     const int* arc_rxn;   const int* arc_dir;
-    const u64* arc_mix;   // mix64(0x01 << 56 | a): the inner mix of the arc term of the state hash, per arc
+    const u64* arc_mix;   // m_a = mix64(0x01 << 56 | a): the multiplier of arc a in the state hash
     int max_coef;         // largest |s_ia| of the network (bounds the lane-parallel fast path)
 };
 
@@ -127,15 +127,17 @@ struct RootArgs {
 // ---------------------------------------------------------------------------------------------------------------
 // SURVEY.md 8(c)-B state hash: written here from the formula, independently of oracle/.
 //   mix = SplitMix64 finaliser
-//   h = mix( sum_{a in supp} mix( mix(0x01<<56 | a) + f_a ) + sum_{i visited} mix(0x02<<56 | cnt<<48 | i<<32 | PI<<16 | PO) )
+//   h = mix( sum_{a in supp} mix(0x01<<56 | a) * f_a + sum_{i visited} mix(0x02<<56 | cnt<<48 | i<<32 | PI<<16 | PO) )
 //   key = min(n_unb, 255) << 56 | h >> 8
+// (sums and products modulo 2^64).  The arc part is linear in the flux vector: the sum of a child whose fluxes are
+// k f + d e_a is k hs + m_a d, no pass over the support (only a common divisor g > 1 needs one).
 // ---------------------------------------------------------------------------------------------------------------
 __host__ __device__ inline u64 mix64(u64 x) {
     x ^= x >> 30; x *= 0xBF58476D1CE4E5B9ULL;
     x ^= x >> 27; x *= 0x94D049BB133111EBULL;
     x ^= x >> 31; return x;
 }
-__host__ __device__ inline u64 arc_term(u32 a, u64 f) { return mix64(mix64(0x0100000000000000ULL | (u64)a) + f); }
+__host__ __device__ inline u64 arc_term(u32 a, u64 f) { return mix64(0x0100000000000000ULL | (u64)a) * f; }
 __host__ __device__ inline u64 vis_term(u64 rec) { return mix64(0x0200000000000000ULL | rec); }
 __host__ __device__ inline u64 vis_pack(u32 met, u32 PI, u32 PO, u32 cnt) {
     return ((u64)cnt << 48) | ((u64)met << 32) | ((u64)PI << 16) | (u64)PO;

@@ -123,8 +123,8 @@ __device__ __forceinline__ bool umul_gt_guard(u64 a, u64 b) {  // a*b > 2^62, a,
     return __umul64hi(a, b) != 0 || a * b > EFM_GUARD;
 }
 __device__ __forceinline__ u64 abs64(i64 v) { return (u64)(v < 0 ? -v : v); }
-// arc term of the state hash through the per-arc table of inner mixes (device_common.cuh: arc_term)
-__device__ __forceinline__ u64 arc_term_t(const DevGraph& g, u32 a, u64 f) { return mix64(__ldg(&g.arc_mix[a]) + f); }
+// arc term of the state hash through the per-arc table of multipliers (device_common.cuh: arc_term)
+__device__ __forceinline__ u64 arc_term_t(const DevGraph& g, u32 a, u64 f) { return __ldg(&g.arc_mix[a]) * f; }
 
 // Per-warp chunked reservation of beam-key slots: one atomic per kKeyChunk keys instead of one per child.
 constexpr u64 kNoSlot = ~0ULL;
@@ -181,8 +181,7 @@ __device__ __forceinline__ bool sbit(const u32* bits, int a) { return (bits[a >>
 // per-warp statistics live in shared memory (one u64 each), flushed to the control block once per warp
 enum { SS_EXPANDED = 0, SS_CHILDREN, SS_DONE, SS_ACTIVE, SS_DEAD, SS_NOTEFM, SS_NONPOS, SS_OVF, SS_VISITED, SS_BYTES,
        SS_ROUNDS, SS_FIRST, SS_GENERAL, SS_SATURATED,
-       SS_KC,   // 4 words: the hash sums of the k-scaled support for the last two scales k (k0, s0, k1, s1)
-       SS_OFF = SS_KC + 4,   // kParentsPerWarp words: offsets of the parents of this group
+       SS_OFF,   // kParentsPerWarp words: offsets of the parents of this group
        SS_WORDS = SS_OFF + 8 };
 
 // One kernel body, every routine inlined once: the staged parent is addressed through shared-memory pointers the
@@ -276,7 +275,6 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
             best = min(best, (i << 16) | (u32)t);
         }
         best = __reduce_min_sync(gmask, best);
-        if (lane == 0) { sst[SS_KC] = 0; sst[SS_KC + 2] = 0; }
         __syncwarp(gmask);
         const int istar = (int)(best >> 16);
         const i64 E = ef[best & 0xffffu];
@@ -405,27 +403,7 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                         }
                     }
                 }
-                u64 hsb = Phs;
-                u32 need = gballot(fast && k > 1);
-                #pragma unroll 1
-                while (need) {
-                    const u32 kk = __shfl_sync(gmask, k, __ffs(need) - 1, G);
-                    u64 s;
-                    if ((u64)kk == sst[SS_KC]) s = sst[SS_KC + 1];
-                    else if ((u64)kk == sst[SS_KC + 2]) s = sst[SS_KC + 3];
-                    else {
-                        s = 0;
-                        #pragma unroll 1
-                        for (int t = lane; t < ns; t += G) s += arc_term_t(A.g, (u32)arc[t], (u64)kk * (u64)flux[t]);
-                        s = g_sum<G>(gmask, s);
-                        __syncwarp(gmask);
-                        if (lane == 0) { sst[SS_KC + 2] = sst[SS_KC]; sst[SS_KC + 3] = sst[SS_KC + 1]; sst[SS_KC] = kk; sst[SS_KC + 1] = s; }
-                        __syncwarp(gmask);
-                    }
-                    const bool same = fast && k == kk;
-                    if (same) hsb = s;
-                    need &= ~gballot(same);
-                }
+                const u64 hsb = (u64)k * Phs;   // the arc part of the state hash is linear in the fluxes
                 if (fast) {
                     const u64 newrec = vis_pack((u32)istar, (u32)(fwd ? prim : a), (u32)(fwd ? a : prim), 0u);
                     hs2 = hsb + arc_term_t(A.g, (u32)a, d);
@@ -551,8 +529,8 @@ __global__ void __launch_bounds__(kBlock, EFM_MIN_BLOCKS) k_expand(const __grid_
                     }
                     if (__builtin_expect(!__any_sync(gmask, r == 1), 0)) cg = g_gcd<G>(gmask, r, narrow);
                 }
-                if (ck == 1 && cg == 1) {
-                    chs = Phs + arc_term_t(A.g, (u32)ca, cT) - (cin ? arc_term_t(A.g, (u32)ca, (u64)flux[cia]) : 0ULL);
+                if (cg == 1) {   // linear: sum of m_t (k f_t) with the term of arc a replaced by m_a T
+                    chs = ck * Phs + arc_term_t(A.g, (u32)ca, cT - (cin ? ck * (u64)flux[cia] : 0ULL));
                 } else {
                     chs = 0;
                     #pragma unroll 1

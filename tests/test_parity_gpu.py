@@ -7,7 +7,7 @@ import os
 import numpy as np
 import pytest
 
-from netgen import hand_network, make_network, unimolecular_network
+from netgen import hand_network, make_network, random_seed_sets, unimolecular_network
 
 pytestmark = pytest.mark.gpu
 
@@ -62,12 +62,59 @@ def _golden_cases():
 @pytest.mark.parametrize("case", _golden_cases(), ids=lambda c: c["name"])
 def test_hand_pins_on_gpu(efm, case):
     """The hand-derived fixtures of tests/golden pin the CUDA path directly (no oracle involved)."""
-    net = hand_network([(s, p, r) for s, p, r in case["reactions"]], case["internal"])
+    net = hand_network([(s, p, r) for s, p, r in case["reactions"]], case["internal"], **case.get("params", {}))
     got = efm.enumerate_network(net, seed_sets=case["seeds"])
     assert got.flux.tolist() == case["flux"]
     for k in ("expanded", "levels", "discarded_nonpos"):
         if k in case:
             assert int(got.stats[k]) == case[k], k
+    for k, v in case.get("stats", {}).items():
+        assert int(got.stats[k]) == v, (k, got.stats[k], v)
+
+
+def _h7_shifted(n_pad):
+    """The H7 network of tests/golden (r0: ->A, r1: A->, r2: ->B, r3: 2B->) behind n_pad reversible reactions between
+    external metabolites: the arc ids move past 2 * n_pad, so with n_pad >= 56 the supports no longer fit the exact
+    112-bit signature of the minimality filter and the hashed signature + sorted-list verification decides."""
+    rx = [({"X%d" % t: 1}, {"Y%d" % t: 1}, True) for t in range(n_pad)]
+    rx += [({}, {"A": 1}, False), ({"A": 1}, {}, False), ({}, {"B": 1}, False), ({"B": 2}, {}, False)]
+    return hand_network(rx, ["A", "B"]), 2 * n_pad
+
+
+@pytest.mark.parametrize("n_pad", [0, 60, 700])
+def test_filter_drop_and_poison_by_hand(efm, n_pad):
+    """Def 3 / PAPER.md:456 and SURVEY.md 8(c) O8(ii), derived by hand (tests/golden H7): seeds {r0, r2} and
+    {r0} balance to supports {r0,r1,r2,r3} and {r0,r1}: the superset is dropped.  Seeds {r0, r2} and {r0, r3} reach the
+    support {r0,r1,r2,r3} with fluxes (2,2,2,1) and (1,1,2,1): poisoned, nothing is left.  No oracle involved."""
+    net, c0 = _h7_shifted(n_pad)
+    z = [0] * n_pad
+    got = efm.enumerate_network(net, seed_sets=[[c0, c0 + 4], [c0]])
+    assert got.flux.tolist() == [z + [1, 1, 0, 0]]
+    assert (got.stats["unique_supports"], got.stats["poisoned"], got.stats["output"]) == (2, 0, 1)
+    got = efm.enumerate_network(net, seed_sets=[[c0, c0 + 4], [c0, c0 + 6]])
+    assert got.flux.tolist() == []
+    assert (got.stats["done"], got.stats["unique_supports"], got.stats["poisoned"], got.stats["output"]) == (2, 1, 1, 0)
+    # three nested supports plus an unrelated one: only the minimal ones stay, in canonical order
+    got = efm.enumerate_network(net, seed_sets=[[c0, c0 + 4], [c0], [c0 + 4]])
+    assert got.flux.tolist() == [z + [0, 0, 2, 1], z + [1, 1, 0, 0]]
+    assert (got.stats["unique_supports"], got.stats["poisoned"], got.stats["output"]) == (3, 0, 2)
+
+
+@pytest.mark.parametrize("name,over,count,size", [("small", {}, 200, 2), ("small", {}, 120, 3),
+                                                  ("core", dict(frontier_cap=4096), 200, 2),
+                                                  ("mid", dict(frontier_cap=4096), 300, 2),
+                                                  ("genome", dict(frontier_cap=4096), 300, 2)])
+def test_poison_and_minimality_at_scale(efm, oracle_mod, name, over, count, size):
+    """Multi-arc seed sets reach one support along several routes: the poison rule (a-6) and the drop branch of the
+    minimality filter (a-7) both fire, on both sides, and the results stay bit-exact.  core / mid / genome have more
+    than 112 arcs: the hashed-signature route with its sorted-list verification runs with true positives."""
+    net = make_network(name, 0)
+    seeds = random_seed_sets(net, count, size, 11)
+    got, ref = assert_parity(efm, oracle_mod, net, seeds=seeds, **over)
+    for st in (got.stats, ref.stats):
+        assert int(st["poisoned"]) > 0
+        if name != "mid":
+            assert int(st["unique_supports"]) - int(st["poisoned"]) - int(st["output"]) > 0
 
 
 @pytest.mark.parametrize("two_pass", [False, True])
