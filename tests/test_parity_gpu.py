@@ -160,7 +160,7 @@ def test_core_beam(efm, oracle_mod, cap):
     assert got.stats["truncated_beam"] > 0
 
 
-@pytest.mark.parametrize("cap", [512, 16384, 65536])
+@pytest.mark.parametrize("cap", [512, 16384, 65536, 262144])
 def test_mid(efm, oracle_mod, cap):
     net = make_network("mid", 0)
     got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=cap)
@@ -172,6 +172,15 @@ def test_genome(efm, oracle_mod, cap):
     net = make_network("genome", 0)
     got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=cap)
     assert got.stats["truncated_beam"] > 0 and got.stats["output"] > 1000
+
+
+def test_genome_at_the_bench_configuration(efm, oracle_mod):
+    """Element-by-element parity of the configuration bench.py times (genome seed 0, frontier_cap bench.DEFAULT_CAP, the
+    bench's candidate capacity): the oracle needs a few minutes on the box's host cores."""
+    import bench
+    net = make_network("genome", 0)
+    got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=bench.DEFAULT_CAP, max_candidates=bench.DEFAULT_MAX_CANDIDATES)
+    assert got.stats["truncated_beam"] > 0 and got.stats["output"] > 100000
 
 
 def test_general_routine_only(efm, oracle_mod):
@@ -217,6 +226,27 @@ def test_wide_columns_and_large_coefficients(efm, oracle_mod):
     got, ref = assert_parity(efm, oracle_mod, net, seeds=[[0]])
     assert ref.stats["output"] >= 2
     assert_parity(efm, oracle_mod, net, seeds=oracle_mod.all_arc_seed_sets(net.reversible))
+
+
+def test_columns_longer_than_a_warp(efm, oracle_mod):
+    """A reaction with 40 internal products: the column of its arc is longer than 32 entries (the route of
+    k_materialise that scans the parent's list again) and every product becomes unbalanced at once."""
+    names = ["A"] + [f"P{t}" for t in range(40)]
+    rx = [({}, {"A": 1}, False), ({"A": 2}, {f"P{t}": 1 + t % 3 for t in range(40)}, False)]
+    rx += [({f"P{t}": 1}, {}, False) for t in range(40)]
+    rx += [({f"P{t}": 2, f"P{t + 1}": 1}, {"A": 1}, False) for t in range(0, 40, 8)]
+    net = hand_network(rx, names)
+    got, ref = assert_parity(efm, oracle_mod, net, seeds=[[0]])
+    assert ref.stats["output"] >= 1 and ref.stats["expanded"] > 40
+    assert_parity(efm, oracle_mod, net, seeds=[[0], [2], [2 * 41 + 2]])
+
+
+def test_key_capacity_error(efm):
+    """max_child_keys too small for a level: EFM_E_CAPACITY, never a silently truncated result."""
+    net = make_network("core", 0)
+    with pytest.raises(efm.EfmError) as ei:
+        efm.enumerate_network(net, frontier_cap=4096, max_child_keys=64, max_frontier=4096)
+    assert ei.value.code == efm.EFM_E_CAPACITY
 
 
 def test_overflow_guard(efm, oracle_mod):
