@@ -39,7 +39,6 @@ extern "C" {
 
 /* flags */
 #define EFM_F_TIMING 0x1u       /* record CUDA events around every kernel phase (efm_stats.ms_*)   */
-#define EFM_F_FORCE_TWO_PASS 0x2u /* always run the threshold selection, even when the beam cannot bind */
 #define EFM_F_NO_FASTPATH 0x4u  /* evaluate every child with the warp-cooperative general routine  */
 #define EFM_F_NO_STAGING 0x8u   /* read every parent in place (the route of entries larger than the   */
                                 /* shared-memory staging buffer)                                      */
@@ -57,13 +56,17 @@ typedef struct {
     int64_t frontier_cap;   /* beam: entries expanded per level; 0 = unbounded                       */
     int64_t max_frontier;   /* entries per frontier buffer; 0 = max(frontier_cap, 4096), 2^20 when cap == 0 */
     int64_t max_candidates; /* capacity of the candidate buffer / support hash; 0 = 2^20             */
-    int64_t max_child_keys; /* child slots per level (8-byte beam key + 64-byte task each, < 2^32);  */
-                            /* 0 = frontier_cap * the largest fan-out of a node                      */
+    int64_t max_child_keys; /* child slots per level (8-byte beam key + 8-byte tag each, < 2^32);    */
+                            /* 0 = frontier_cap * the largest fan-out of a node (never overflows);   */
+                            /* a smaller value saves HBM and reports EFM_E_CAPACITY when exceeded    */
     int32_t device;         /* CUDA device ordinal the workspace lives on                            */
     uint32_t flags;         /* EFM_F_*                                                               */
     int64_t max_frontier_bytes; /* bytes of one frontier buffer (entries are packed, variable size);         */
                             /* 0 = max_frontier * the largest possible entry, which can never overflow;      */
                             /* a smaller value saves HBM and reports EFM_E_CAPACITY if a level outgrows it   */
+    int64_t max_child_tasks; /* 64-byte tasks per level (children on arcs of the support: every revisit, some     */
+                            /* alternatives of a first visit); 0 = 4 * max_frontier + 65536 (max_child_keys with     */
+                            /* EFM_F_NO_FASTPATH); EFM_E_CAPACITY when exceeded                                      */
 } efm_params;
 
 typedef struct {
@@ -73,18 +76,18 @@ typedef struct {
     int64_t algo_bytes;     /* algorithmic bytes of all expansions            */
     int64_t n_roots;
     int64_t launches;       /* kernels launched by the last efm_enumerate()                          */
-    int64_t two_pass_levels, direct_levels; /* levels on which the beam threshold was / was not computed      */
+    int64_t two_pass_levels, direct_levels; /* levels enqueued with / without the threshold selection (frontier_cap > 0 / = 0) */
+    int64_t h2d_bytes;      /* bytes efm_enumerate() copied host -> device (graph on first use, seed sets)          */
+    int64_t host_syncs;     /* stream synchronisations inside efm_enumerate(): one per batch of levels + post stages */
     /* milliseconds; ms_total is always measured (CUDA events on the caller's stream), the per-phase
      * figures only with EFM_F_TIMING */
-    double ms_build, ms_total, ms_expand_count, ms_beam, ms_expand_write, ms_direct, ms_hash,
-        ms_filter, ms_output;
-    /* ms_expand_count: k_expand (evaluates every child: beam key + task); ms_beam: threshold selection;
-     * ms_expand_write: k_compact + k_materialise (survivors -> next frontier / candidates); ms_direct: unused (0) */
-    int64_t n_expand_count, n_expand_write, n_direct; /* launches behind the expand timers (n_direct: 0)     */
+    double ms_build, ms_total, ms_order, ms_expand_count, ms_beam, ms_expand_write, ms_hash, ms_filter, ms_output;
+    /* ms_order: k_order (parents by kind); ms_expand_count: k_expand (evaluates every child: beam key + tag);
+     * ms_beam: threshold selection; ms_expand_write: k_compact + k_materialise (survivors -> next frontier / candidates) */
+    int64_t n_expand_count; /* levels enqueued (levels behind the end of the traversal return at once)                 */
     int64_t filter_pairs;   /* signature pair tests done by the minimality filter                    */
-    /* work profile of the expansion: rounds of 32 OR-alternatives, first-visit parents, children through the
-     * general routine, parents whose support is at the cap D, children materialised (survivors + balanced) */
-    int64_t alt_rounds, first_visits, general_children, saturated_parents, materialised;
+    /* work profile of the expansion: first-visit parents, children through the general routine, children materialised */
+    int64_t first_visits, general_children, materialised;
 } efm_stats;
 
 /* Build the modified AND/OR graph MG (Defs 4-6; "Convert the given matrix to the MG

@@ -20,23 +20,23 @@ LIB_PATH = os.path.join(_HERE, "libefm_b200.so")
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "efm_b200.h")
 
 EFM_OK, EFM_E_INVAL, EFM_E_NOMEM, EFM_E_CAPACITY, EFM_E_CUDA, EFM_E_STATE = 0, -1, -2, -3, -4, -5
-EFM_F_TIMING, EFM_F_FORCE_TWO_PASS, EFM_F_NO_FASTPATH, EFM_F_NO_STAGING = 0x1, 0x2, 0x4, 0x8
+EFM_F_TIMING, EFM_F_NO_FASTPATH, EFM_F_NO_STAGING = 0x1, 0x4, 0x8
 
 
 class efm_params(ctypes.Structure):
     _fields_ = [("max_support", ctypes.c_int32), ("max_loop", ctypes.c_int32), ("dep_depth", ctypes.c_int32),
                 ("max_visited", ctypes.c_int32), ("frontier_cap", ctypes.c_int64), ("max_frontier", ctypes.c_int64),
                 ("max_candidates", ctypes.c_int64), ("max_child_keys", ctypes.c_int64), ("device", ctypes.c_int32),
-                ("flags", ctypes.c_uint32), ("max_frontier_bytes", ctypes.c_int64)]
+                ("flags", ctypes.c_uint32), ("max_frontier_bytes", ctypes.c_int64), ("max_child_tasks", ctypes.c_int64)]
 
 
 _STAT_INT = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxloop", "discarded_nonpos",
              "discarded_overflow", "discarded_visited", "truncated_beam", "unique_supports", "poisoned", "output",
-             "peak_frontier", "algo_bytes", "n_roots", "launches", "two_pass_levels", "direct_levels"]
-_STAT_MS = ["ms_build", "ms_total", "ms_expand_count", "ms_beam", "ms_expand_write", "ms_direct", "ms_hash",
+             "peak_frontier", "algo_bytes", "n_roots", "launches", "two_pass_levels", "direct_levels", "h2d_bytes",
+             "host_syncs"]
+_STAT_MS = ["ms_build", "ms_total", "ms_order", "ms_expand_count", "ms_beam", "ms_expand_write", "ms_hash",
             "ms_filter", "ms_output"]
-_STAT_INT2 = ["n_expand_count", "n_expand_write", "n_direct", "filter_pairs", "alt_rounds", "first_visits",
-              "general_children", "saturated_parents", "materialised"]
+_STAT_INT2 = ["n_expand_count", "filter_pairs", "first_visits", "general_children", "materialised"]
 
 
 class efm_stats(ctypes.Structure):
@@ -122,7 +122,7 @@ class Enumerator:
                        int(params.get("max_visited", 0)), int(params.get("frontier_cap", 0)),
                        int(params.get("max_frontier", 0)), int(params.get("max_candidates", 0)),
                        int(params.get("max_child_keys", 0)), int(device), int(flags),
-                       int(params.get("max_frontier_bytes", 0)))
+                       int(params.get("max_frontier_bytes", 0)), int(params.get("max_child_tasks", 0)))
         self.device = int(device)
         self._check(self._lib.efm_create(_ptr(S), self.m, self.n, self.n, _ptr(rev), _ptr(internal), ctypes.byref(p),
                                          ctypes.byref(self._h)))

@@ -22,8 +22,8 @@ namespace {
 struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
-    Region col_ptr, col, in_ptr, in_e, out_ptr, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
-    Region ctl, buf[2], off[2], pmin, keys, ckeys, task[4], surv, surv_dst, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill, vcount, vstart, vfill, tstart;
+    Region col_ptr, col, node, in_e, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
+    Region ctl, lvl, buf[2], off[2], plist, pprim, keys, tags, ckeys, tasks, surv, surv_dst, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill, vcount, vstart, vfill, tstart;
     Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, u_key, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
 };
@@ -35,7 +35,7 @@ size_t pow2_at_least(size_t x) { size_t p = 1; while (p < x) p <<= 1; return p; 
 struct efm_handle {
     HostGraph G;
     int32_t D = 0, V = 0, max_loop = 8, L = 4;
-    int64_t cap = 0, max_frontier = 0, max_cand = 0, max_keys = 0;
+    int64_t cap = 0, max_frontier = 0, max_cand = 0, max_keys = 0, max_tasks = 0, max_ckeys = 0, max_surv = 0, max_levels = 0;
     int32_t device = 0;
     uint32_t flags = 0;
     uint32_t max_entry = 0, cand_stride = 0;   // largest frontier entry in bytes; candidate slot stride
@@ -71,9 +71,8 @@ void make_layout(efm_handle* h) {
     Layout L;
     add_region(L, L.col_ptr, sizeof(int) * (G.A + 1));
     add_region(L, L.col, sizeof(int2) * (G.col.size() + 1));
-    add_region(L, L.in_ptr, sizeof(int) * (G.M + 1));
+    add_region(L, L.node, sizeof(int4) * (G.M + 1));
     add_region(L, L.in_e, sizeof(int2) * (G.in.size() + 1));
-    add_region(L, L.out_ptr, sizeof(int) * (G.M + 1));
     add_region(L, L.out_e, sizeof(int2) * (G.out.size() + 1));
     add_region(L, L.in_alt, 32 * (G.in.size() + 1));
     add_region(L, L.out_alt, 32 * (G.out.size() + 1));
@@ -84,16 +83,19 @@ void make_layout(efm_handle* h) {
     add_region(L, L.arc_dir, sizeof(int) * (G.A + 1));
     add_region(L, L.arc_mix, sizeof(u64) * (G.A + 1));
     add_region(L, L.ctl, sizeof(Ctl));
-    add_region(L, L.buf[0], (size_t)h->frontier_bytes + 2048);   // spare bytes: the fixed-size prefetch of a parent
-    add_region(L, L.buf[1], (size_t)h->frontier_bytes + 2048);
-    add_region(L, L.off[0], (size_t)h->max_frontier * 8);
-    add_region(L, L.off[1], (size_t)h->max_frontier * 8);
-    add_region(L, L.pmin, (size_t)(h->max_frontier + 1) * 8);
+    add_region(L, L.lvl, sizeof(LevelStats) * (size_t)(h->max_levels + 2));
+    add_region(L, L.buf[0], (size_t)h->frontier_bytes + 256);
+    add_region(L, L.buf[1], (size_t)h->frontier_bytes + 256);
+    add_region(L, L.off[0], (size_t)(h->max_frontier + 1) * 8);
+    add_region(L, L.off[1], (size_t)(h->max_frontier + 1) * 8);
+    add_region(L, L.plist, (size_t)(h->max_frontier + 1) * 8);
+    add_region(L, L.pprim, (size_t)(h->max_frontier + 1) * 4);
     add_region(L, L.keys, (size_t)h->max_keys * 8);
-    add_region(L, L.ckeys, (size_t)h->max_keys * 8);
-    for (int t = 0; t < 4; ++t) add_region(L, L.task[t], (size_t)h->max_keys * 16);
-    add_region(L, L.surv, (size_t)h->max_keys * 16);
-    add_region(L, L.surv_dst, (size_t)h->max_keys * 8);
+    add_region(L, L.tags, (size_t)h->max_keys * 8);
+    add_region(L, L.ckeys, (size_t)h->max_ckeys * 8);
+    add_region(L, L.tasks, (size_t)h->max_tasks * 64);
+    add_region(L, L.surv, (size_t)h->max_surv * 16);
+    add_region(L, L.surv_dst, (size_t)h->max_surv * 8);
     const size_t C = (size_t)h->max_cand;
     add_region(L, L.cand, C * h->cand_stride);
     add_region(L, L.table, h->table_size * 4);
@@ -146,8 +148,8 @@ DevGraph dev_graph(const efm_handle* h, unsigned char* ws) {
     DevGraph g;
     g.M = h->G.M; g.A = h->G.A; g.W32 = (h->G.A + 31) / 32; g.M32 = (h->G.M + 31) / 32;
     g.col_ptr = (const int*)(ws + L.col_ptr.off);   g.col = (const int2*)(ws + L.col.off);
-    g.in_ptr = (const int*)(ws + L.in_ptr.off);     g.in_e = (const int2*)(ws + L.in_e.off);
-    g.out_ptr = (const int*)(ws + L.out_ptr.off);   g.out_e = (const int2*)(ws + L.out_e.off);
+    g.node = (const int4*)(ws + L.node.off);
+    g.in_e = (const int2*)(ws + L.in_e.off);        g.out_e = (const int2*)(ws + L.out_e.off);
     g.in_alt = (const uint4*)(ws + L.in_alt.off);   g.out_alt = (const uint4*)(ws + L.out_alt.off);
     g.twin = (const int*)(ws + L.twin.off);
     g.dep_off = (const i64*)(ws + L.dep_off.off);   g.dep_bits = (const u32*)(ws + L.dep_bits.off);
@@ -200,7 +202,7 @@ struct Timer {
     size_t mark() { if (!on) return 0; cudaEvent_t e = get(); cudaEventRecord(e, s); return used - 1; }
     void span(size_t a, size_t b, int phase) { if (on) spans.push_back(Span{a, b, phase}); }
 };
-enum { PH_COUNT = 0, PH_BEAM, PH_WRITE, PH_DIRECT, PH_HASH, PH_FILTER, PH_OUTPUT, PH_N };
+enum { PH_ORDER = 0, PH_COUNT, PH_BEAM, PH_WRITE, PH_HASH, PH_FILTER, PH_OUTPUT, PH_N };
 
 }  // namespace
 
@@ -227,7 +229,8 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     memset(&P, 0, sizeof P);
     if (p) P = *p;
     if (P.max_support < 0 || P.max_loop < 0 || P.dep_depth < 0 || P.max_visited < 0 || P.frontier_cap < 0 ||
-        P.max_frontier < 0 || P.max_candidates < 0 || P.max_child_keys < 0 || P.device < 0 || P.max_frontier_bytes < 0)
+        P.max_frontier < 0 || P.max_candidates < 0 || P.max_child_keys < 0 || P.device < 0 || P.max_frontier_bytes < 0 ||
+        P.max_child_tasks < 0)
         return EFM_E_INVAL;
     efm_handle* h = new (std::nothrow) efm_handle();
     if (!h) return EFM_E_NOMEM;
@@ -262,13 +265,30 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     }
     h->max_cand = P.max_candidates ? P.max_candidates : (int64_t)1 << 20;
     if (h->max_cand > 0xFFFFFFF0LL) { delete h; return EFM_E_INVAL; }
+    // child slots of a level (8-byte key + 8-byte tag each).  The evaluation strands at most one chunk per resident warp
+    // (kSlackSMs bounds the SM count of the device the handle will run on).
+    int kSlackSMs = 256;
+    {
+        int smc = 0;
+        if (cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, P.device) == cudaSuccess && smc > 0) kSlackSMs = smc;
+        else cudaGetLastError();
+    }
     h->max_keys = (P.max_child_keys ? P.max_child_keys : std::max<int64_t>(h->cap * (int64_t)G.max_fanout, 65536)) +
-                  (int64_t)expand_key_slack((u64)h->max_frontier);
-    // child slots are addressed with 32 bits (survivor list); the default is clamped, an explicit request is refused
-    if (h->max_keys > 0xFFFFFFF0LL) {
+                  (int64_t)expand_key_slack(kSlackSMs);
+    if (h->max_keys > 0xFFFFFFF0LL) {   // slots are addressed with 32 bits; the default is clamped, an explicit request is refused
         if (P.max_child_keys) { delete h; return EFM_E_INVAL; }
         h->max_keys = 0xFFFFFFF0LL;
     }
+    // 64-byte tasks of the children of the general routine: one per revisit parent plus the alternatives of a first visit
+    // that are arcs of the support; every child when EFM_F_NO_FASTPATH sends all of them there
+    h->max_tasks = P.max_child_tasks ? P.max_child_tasks
+                   : ((P.flags & EFM_F_NO_FASTPATH) ? h->max_keys : std::min<int64_t>(h->max_keys, 4 * h->max_frontier + 65536));
+    h->max_tasks += (int64_t)expand_task_slack(kSlackSMs);
+    // keys sharing the selected 22-bit prefix (8 bits of n_unb + 14 bits of the state hash): 1 / 16384 of a class on average
+    h->max_ckeys = std::max<int64_t>(h->max_keys / 64, std::min<int64_t>(h->max_keys, (int64_t)1 << 20));
+    h->max_surv = h->max_frontier + h->max_cand + 1024;
+    // a pathway gains a visited node or a revisit count with every level
+    h->max_levels = std::min<int64_t>((int64_t)std::min(h->V, std::max(G.M, 1)) * ((int64_t)h->max_loop + 1) + 2, (int64_t)1 << 20);
     h->table_size = pow2_at_least((size_t)h->max_cand * 2);
     h->dense_bytes = std::max<size_t>((size_t)64 << 20, (size_t)n * 8 * 64);
     make_layout(h);
@@ -388,39 +408,61 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     cudaEvent_t ev_start = tm.get(), ev_end = tm.get();
     CK(cudaEventRecord(ev_start, s));
 
-    // ---- upload the graph (~100 KB) and the roots; clear the control block
-    auto up = [&](const Region& r, const void* src, size_t bytes) -> cudaError_t {
+    // ---- upload the graph (~0.5 MB) and the roots; clear the control block
+    int64_t h2d = 0;
+    auto up = [&](unsigned char* dst, const void* src, size_t bytes) -> cudaError_t {
         if (bytes == 0) return cudaSuccess;
-        return cudaMemcpyAsync(ws + r.off, src, bytes, cudaMemcpyHostToDevice, s);
+        h2d += (int64_t)bytes;
+        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s);
     };
     std::vector<u64> arc_mix;
     std::vector<uint32_t> alt_in, alt_out;
+    std::vector<int> node, colp;
     if (h->graph_ws != ws) {   // the network is an input: it stays resident in the workspace across calls
         h->graph_ws = nullptr;
-        CK(up(L.col_ptr, G.col_ptr.data(), sizeof(int) * G.col_ptr.size()));
-        CK(up(L.col, G.col.data(), sizeof(ColRef) * G.col.size()));
-        CK(up(L.in_ptr, G.in_ptr.data(), sizeof(int) * G.in_ptr.size()));
-        CK(up(L.in_e, G.in.data(), sizeof(ArcRef) * G.in.size()));
-        CK(up(L.out_ptr, G.out_ptr.data(), sizeof(int) * G.out_ptr.size()));
-        CK(up(L.out_e, G.out.data(), sizeof(ArcRef) * G.out.size()));
+        // columns with the position of the arc in I[met] / O[met] next to the metabolite: {met | pos << 16, s}
+        colp.resize(2 * G.col.size());
+        {
+            std::vector<int> fin(G.in_ptr.begin(), G.in_ptr.end() - 1), fout(G.out_ptr.begin(), G.out_ptr.end() - 1);
+            for (int a = 0; a < G.A; ++a)
+                for (int q = G.col_ptr[a]; q < G.col_ptr[a + 1]; ++q) {
+                    const ColRef& e = G.col[q];
+                    const int pos = e.s > 0 ? fin[e.met]++ - G.in_ptr[e.met] : fout[e.met]++ - G.out_ptr[e.met];
+                    colp[2 * (size_t)q] = (int)((uint32_t)e.met | ((uint32_t)pos << 16));
+                    colp[2 * (size_t)q + 1] = e.s;
+                }
+        }
+        node.resize(4 * (size_t)G.M);
+        for (int i = 0; i < G.M; ++i) {
+            node[4 * (size_t)i] = G.in_ptr[i]; node[4 * (size_t)i + 1] = G.in_ptr[i + 1] - G.in_ptr[i];
+            node[4 * (size_t)i + 2] = G.out_ptr[i]; node[4 * (size_t)i + 3] = G.out_ptr[i + 1] - G.out_ptr[i];
+        }
+        CK(up(ws + L.col_ptr.off, G.col_ptr.data(), sizeof(int) * G.col_ptr.size()));
+        CK(up(ws + L.col.off, colp.data(), sizeof(int) * colp.size()));
+        CK(up(ws + L.node.off, node.data(), sizeof(int) * node.size()));
+        CK(up(ws + L.in_e.off, G.in.data(), sizeof(ArcRef) * G.in.size()));
+        CK(up(ws + L.out_e.off, G.out.data(), sizeof(ArcRef) * G.out.size()));
         alt_in = alt_records(G, G.in); alt_out = alt_records(G, G.out);
-        CK(up(L.in_alt, alt_in.data(), sizeof(uint32_t) * alt_in.size()));
-        CK(up(L.out_alt, alt_out.data(), sizeof(uint32_t) * alt_out.size()));
-        CK(up(L.twin, G.twin.data(), sizeof(int) * G.twin.size()));
-        CK(up(L.dep_off, G.dep_off.data(), sizeof(i64) * G.dep_off.size()));
-        CK(up(L.dep_bits, G.dep_bits.data(), sizeof(u32) * G.dep_bits.size()));
-        CK(up(L.arc_rxn, G.arc_rxn.data(), sizeof(int) * G.arc_rxn.size()));
-        CK(up(L.arc_dir, G.arc_dir.data(), sizeof(int) * G.arc_dir.size()));
+        CK(up(ws + L.in_alt.off, alt_in.data(), sizeof(uint32_t) * alt_in.size()));
+        CK(up(ws + L.out_alt.off, alt_out.data(), sizeof(uint32_t) * alt_out.size()));
+        CK(up(ws + L.twin.off, G.twin.data(), sizeof(int) * G.twin.size()));
+        CK(up(ws + L.dep_off.off, G.dep_off.data(), sizeof(i64) * G.dep_off.size()));
+        CK(up(ws + L.dep_bits.off, G.dep_bits.data(), sizeof(u32) * G.dep_bits.size()));
+        CK(up(ws + L.arc_rxn.off, G.arc_rxn.data(), sizeof(int) * G.arc_rxn.size()));
+        CK(up(ws + L.arc_dir.off, G.arc_dir.data(), sizeof(int) * G.arc_dir.size()));
         arc_mix.resize((size_t)G.A);
-        for (int a = 0; a < G.A; ++a) arc_mix[a] = mix64(0x0100000000000000ULL | (u64)a);   // inner mix of arc_term
-        CK(up(L.arc_mix, arc_mix.data(), sizeof(u64) * arc_mix.size()));
+        for (int a = 0; a < G.A; ++a) arc_mix[a] = mix64(0x0100000000000000ULL | (u64)a);   // multiplier of arc a in the state hash
+        CK(up(ws + L.arc_mix.off, arc_mix.data(), sizeof(u64) * arc_mix.size()));
         h->graph_ws = ws;
     }
-    CK(up(L.pmin, h_seed_ptr.data(), sizeof(int) * h_seed_ptr.size()));        // regions unused until level 1
-    CK(up(L.ckeys, h_seed_arc.data(), sizeof(int) * h_seed_arc.size()));
-    CK(up(L.off[1], stage_off.data(), sizeof(u64) * stage_off.size()));
+    // the seed sets travel in regions that are unused until the first level is ordered / expanded
+    CK(up(ws + L.plist.off, h_seed_ptr.data(), sizeof(int) * h_seed_ptr.size()));
+    CK(up(ws + L.tags.off, h_seed_arc.data(), sizeof(int) * h_seed_arc.size()));
+    CK(up(ws + L.off[1].off, stage_off.data(), sizeof(u64) * stage_off.size()));
     CK(cudaMemsetAsync(ws + L.ctl.off, 0, sizeof(Ctl), s));
+    CK(cudaMemsetAsync(ws + L.lvl.off, 0, sizeof(LevelStats) * 2, s));
     CK(cudaStreamSynchronize(s));   // the host staging vectors above go out of scope later; keep it simple
+    int host_syncs = 1;
 
     Ctl* d_ctl = (Ctl*)(ws + L.ctl.off);
     Ctl* hc = h->h_ctl;
@@ -431,13 +473,18 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.g = dev_graph(h, ws);
     ea.cand = ws + L.cand.off;
     ea.keys = (u64*)(ws + L.keys.off);
+    ea.tags = (u64*)(ws + L.tags.off);
+    ea.tasks = (uint4*)(ws + L.tasks.off);
+    ea.plist = (u64*)(ws + L.plist.off);
+    ea.pprim = (u32*)(ws + L.pprim.off);
+    ea.lvl = (LevelStats*)(ws + L.lvl.off);
     ea.ctl = d_ctl;
-    ea.t0 = (uint4*)(ws + L.task[0].off); ea.t1 = (uint4*)(ws + L.task[1].off);
-    ea.t2 = (uint4*)(ws + L.task[2].off); ea.t3 = (uint4*)(ws + L.task[3].off);
     ea.surv = (ulonglong2*)(ws + L.surv.off); ea.surv_dst = (u64*)(ws + L.surv_dst.off);
     ea.max_entry = h->max_entry; ea.cand_stride = h->cand_stride;
     ea.frontier_units = (u64)h->frontier_bytes >> 4;
     ea.max_frontier = (u64)h->max_frontier; ea.max_cand = (u64)h->max_cand; ea.max_keys = (u64)h->max_keys;
+    ea.max_tasks = (u64)h->max_tasks; ea.max_surv = (u64)h->max_surv; ea.max_levels = (u64)h->max_levels;
+    ea.cap = (u64)h->cap;
     ea.D = h->D; ea.V = h->V; ea.max_loop = h->max_loop;
     ea.no_fast = (h->flags & EFM_F_NO_FASTPATH) ? 1 : 0;
     expand_smem_layout(ea);
@@ -446,6 +493,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     auto read_ctl = [&]() -> cudaError_t {
         cudaError_t e = cudaMemcpyAsync(hc, d_ctl, ctl_read, cudaMemcpyDeviceToHost, s);
         if (e != cudaSuccess) return e;
+        ++host_syncs;
         return cudaStreamSynchronize(s);
     };
 
@@ -456,78 +504,76 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     h->lvl_active.clear(); h->lvl_done.clear(); h->lvl_expanded.clear(); h->lvl_children.clear();
     int64_t truncated = 0, done_total = 0, materialised = 0;
 
-    // ---- level 0: classify the roots, beam-select, keep the survivors
-    int cur = 0;
-    u64 n_cur = 0;
     if (n_roots > 0) {
-        CK(launch_level_begin(d_ctl, s)); ++launches;
+        // ---- level 0: classify the roots, beam-select, keep the survivors
         RootArgs ra;
         memset(&ra, 0, sizeof ra);
-        ra.g = ea.g; ra.ctl = d_ctl; ra.n_roots = n_roots;
-        ra.seed_ptr = (const int*)(ws + L.pmin.off); ra.seed_arc = (const int*)(ws + L.ckeys.off);
+        ra.g = ea.g; ra.ctl = d_ctl; ra.lvl = ea.lvl; ra.n_roots = n_roots;
+        ra.seed_ptr = (const int*)(ws + L.plist.off); ra.seed_arc = (const int*)(ws + L.tags.off);
         ra.stage_off = (const u64*)(ws + L.off[1].off); ra.stage = ws + L.buf[1].off;
         ra.nxt = ws + L.buf[0].off; ra.nxt_off = (u64*)(ws + L.off[0].off);
         ra.cand = ea.cand; ra.cand_stride = h->cand_stride; ra.keys = ea.keys;
-        ra.max_frontier = ea.max_frontier; ra.frontier_units = ea.frontier_units; ra.max_cand = ea.max_cand;
+        ra.max_frontier = ea.max_frontier; ra.frontier_units = ea.frontier_units; ra.max_cand = ea.max_cand; ra.cap = ea.cap;
         size_t t0 = tm.mark();
         CK(launch_roots(false, ra, s)); ++launches;
         size_t t1 = tm.mark();
-        // the select's compact buffer is the region the seed arcs sit in: they are dead once the roots are built
-        CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), d_ctl, (u64)h->cap, ea.max_keys, n_roots, h->sm_count, s, &launches));
+        CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), (u64)h->max_ckeys, d_ctl, 1, (u64)h->cap, ea.max_keys, h->sm_count, s, &launches));
         size_t t2 = tm.mark();
         CK(launch_roots(true, ra, s)); ++launches;
         size_t t3 = tm.mark();
         tm.span(t0, t1, PH_COUNT); tm.span(t1, t2, PH_BEAM); tm.span(t2, t3, PH_WRITE);
-        CK(read_ctl());
-        if (hc->error) return EFM_E_CAPACITY;
-        h->lvl_active.push_back((int64_t)hc->n_keys);
-        h->lvl_done.push_back((int64_t)hc->lvl_done);
-        h->lvl_expanded.push_back(0);
-        h->lvl_children.push_back(0);
-        done_total += (int64_t)hc->lvl_done;
-        truncated += (int64_t)hc->n_keys - (int64_t)(hc->n_next >> kAllocShift);
-        n_cur = hc->n_next >> kAllocShift;
-        cur = 0;
-    }
 
-    // ---- level loop (Alg 3 while(true), as level-synchronous frontier expansion)
-    while (n_cur > 0) {
-        const size_t lvl = h->lvl_active.size() - 1;   // level of the parents
-        CK(launch_level_begin(d_ctl, s)); ++launches;
-        ea.cur = ws + L.buf[cur].off; ea.nxt = ws + L.buf[cur ^ 1].off; ea.n_cur = n_cur;
-        ea.cur_off = (const u64*)(ws + L.off[cur].off); ea.nxt_off = (u64*)(ws + L.off[cur ^ 1].off);
-        const bool beam_possible = h->cap > 0 && ((h->flags & EFM_F_FORCE_TWO_PASS) || n_cur * (u64)G.max_fanout > (u64)h->cap);
-        // evaluate every child (keys + tasks) -> beam threshold -> list of survivors -> materialise them
-        size_t t0 = tm.mark();
-        CK(launch_expand(ea, h->sm_count, s)); ++launches;
-        size_t t1 = tm.mark();
-        CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), d_ctl, beam_possible ? (u64)h->cap : 0ULL, ea.max_keys,
-                         std::min<u64>(ea.max_keys, n_cur * (u64)G.max_fanout), h->sm_count, s, &launches));
-        size_t t2 = tm.mark();
-        CK(launch_materialise(ea, std::min<u64>(ea.max_keys, n_cur * 16), 0, h->sm_count, s, 0)); ++launches;
-        CK(launch_materialise(ea, 0, 0, h->sm_count, s, 1)); ++launches;
-        size_t t3 = tm.mark();
-        tm.span(t0, t1, PH_COUNT); tm.span(t1, t2, PH_BEAM); tm.span(t2, t3, PH_WRITE);
-        st.n_expand_count++; st.n_expand_write++;
-        if (beam_possible) st.two_pass_levels++; else st.direct_levels++;
-        CK(read_ctl());
-        if (hc->error) return EFM_E_CAPACITY;
-        materialised += (int64_t)hc->n_surv;
-        h->lvl_expanded[lvl] = (int64_t)hc->lvl_expanded;
-        h->lvl_children[lvl] = (int64_t)hc->lvl_children;
-        const int64_t n_next = (int64_t)(hc->n_next >> kAllocShift);
-        const int64_t active = (int64_t)hc->n_keys;
-        const int64_t done = (int64_t)hc->lvl_done;
-        if (active + done > 0) {
+        // ---- level loop (Alg 3 while(true), as level-synchronous frontier expansion).  The kernels find
+        // their work through the control block, so a whole batch of levels is enqueued before the host looks again; the
+        // levels behind the end of the traversal see an empty frontier and return at once.
+        std::vector<LevelStats> recs;
+        const int kBatch = 8;
+        u64 level = 0;
+        bool more = true;
+        while (more) {
+            const u64 l0 = level;
+            for (int bi = 0; bi < kBatch && level < (u64)h->max_levels; ++bi, ++level) {
+                const int par = (int)(level & 1);
+                ea.level = (u32)level; ea.par = (u32)par;
+                ea.cur = ws + L.buf[par].off; ea.nxt = ws + L.buf[par ^ 1].off;
+                ea.cur_off = (const u64*)(ws + L.off[par].off); ea.nxt_off = (u64*)(ws + L.off[par ^ 1].off);
+                // order the parents -> evaluate every child (keys + tags) -> beam threshold -> survivors -> materialise them
+                size_t a0 = tm.mark();
+                CK(launch_order(ea, h->sm_count, s)); ++launches;
+                size_t a1 = tm.mark();
+                CK(launch_expand(ea, h->sm_count, s)); ++launches;
+                size_t a2 = tm.mark();
+                CK(launch_select(ea.keys, (u64*)(ws + L.ckeys.off), (u64)h->max_ckeys, d_ctl, par, (u64)h->cap, ea.max_keys, h->sm_count, s, &launches));
+                size_t a3 = tm.mark();
+                CK(launch_compact(ea, h->sm_count, s)); ++launches;
+                CK(launch_materialise(ea, h->sm_count, s)); ++launches;
+                size_t a4 = tm.mark();
+                tm.span(a0, a1, PH_ORDER); tm.span(a1, a2, PH_COUNT); tm.span(a2, a3, PH_BEAM); tm.span(a3, a4, PH_WRITE);
+                st.n_expand_count++;
+                if (h->cap > 0) st.two_pass_levels++; else st.direct_levels++;
+            }
+            // records 0 .. level (record 0: the roots; record L + 1: the children of level L)
+            recs.resize((size_t)level + 1);
+            CK(cudaMemcpyAsync(recs.data() + l0, ws + L.lvl.off + sizeof(LevelStats) * l0, sizeof(LevelStats) * (size_t)(level + 1 - l0),
+                               cudaMemcpyDeviceToHost, s));
+            CK(read_ctl());
+            if (hc->error) return EFM_E_CAPACITY;
+            more = (hc->lv[level & 1].alloc >> kAllocShift) != 0;
+            if (more && level >= (u64)h->max_levels) return EFM_E_CAPACITY;
+        }
+        // per-level figures: record r holds the children of level r - 1 = the entries of level r
+        for (size_t r = 0; r < recs.size(); ++r) {
+            const int64_t active = (int64_t)recs[r].active_children, done = (int64_t)recs[r].done_children;
+            if (active + done == 0) break;
+            const bool have_next = r + 1 < recs.size();
             h->lvl_active.push_back(active);
             h->lvl_done.push_back(done);
-            h->lvl_expanded.push_back(0);
-            h->lvl_children.push_back(0);
+            h->lvl_expanded.push_back(have_next ? (int64_t)recs[r + 1].parents : 0);
+            h->lvl_children.push_back(have_next ? (int64_t)(recs[r + 1].active_children + recs[r + 1].done_children) : 0);
+            done_total += done;
+            truncated += active - (have_next ? (int64_t)recs[r + 1].parents : 0);
+            materialised += (int64_t)recs[r].surv;
         }
-        done_total += done;
-        truncated += active - n_next;
-        n_cur = (u64)n_next;
-        cur ^= 1;
     }
 
     // ---- O8: support dedup + poison (a-6), minimality filter (a-7), canonical output (a-8)
@@ -592,9 +638,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     st.truncated_beam = truncated;
     st.output = (int64_t)n_keep;
     st.algo_bytes = (int64_t)hc->st[ST_ALGO_BYTES];
-    st.alt_rounds = (int64_t)hc->st[ST_ROUNDS]; st.first_visits = (int64_t)hc->st[ST_FIRST];
-    st.general_children = (int64_t)hc->st[ST_GENERAL]; st.saturated_parents = (int64_t)hc->st[ST_SATURATED];
+    st.general_children = (int64_t)hc->st[ST_GENERAL]; st.first_visits = (int64_t)hc->st[ST_FIRST];
     st.materialised = materialised;
+    st.h2d_bytes = h2d; st.host_syncs = host_syncs;
     st.peak_frontier = 0;
     for (int64_t a : h->lvl_active) st.peak_frontier = std::max(st.peak_frontier, a);
     st.launches = launches;
@@ -608,8 +654,8 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
             CK(cudaEventElapsedTime(&t, h->events[sp.a], h->events[sp.b]));
             acc[sp.phase] += t;
         }
-        st.ms_expand_count = acc[PH_COUNT]; st.ms_beam = acc[PH_BEAM]; st.ms_expand_write = acc[PH_WRITE];
-        st.ms_direct = acc[PH_DIRECT]; st.ms_hash = acc[PH_HASH]; st.ms_filter = acc[PH_FILTER]; st.ms_output = acc[PH_OUTPUT];
+        st.ms_order = acc[PH_ORDER]; st.ms_expand_count = acc[PH_COUNT]; st.ms_beam = acc[PH_BEAM]; st.ms_expand_write = acc[PH_WRITE];
+        st.ms_hash = acc[PH_HASH]; st.ms_filter = acc[PH_FILTER]; st.ms_output = acc[PH_OUTPUT];
     }
     h->n_out = (int64_t)n_keep;
     h->csr_nnz = n_keep ? (int64_t)hc->csr_nnz : 0;

@@ -138,6 +138,7 @@ struct RootArgs {
     unsigned char* nxt; u64* nxt_off;           // surviving active roots
     unsigned char* cand;
     u64* keys;                                  // one key per root (kKeySentinel for balanced roots)
+    LevelStats* lvl;                            // record 0: the roots as children of a level "-1"
     Ctl* ctl;
     u64 n_roots;
     u32 cand_stride;

@@ -6,11 +6,13 @@ namespace efm {
 
 // expand.cu
 void expand_smem_layout(ExpandArgs& a);
-u64 expand_key_slack(u64 max_parents);   // key slots the chunked reservation of the count pass can strand
+u64 expand_key_slack(int sm_count);    // key slots the evaluation can strand (one chunk per resident warp)
+u64 expand_task_slack(int sm_count);
+cudaError_t launch_order(const ExpandArgs& a, int sm_count, cudaStream_t s);
 cudaError_t launch_expand(const ExpandArgs& a, int sm_count, cudaStream_t s);
-cudaError_t launch_materialise(const ExpandArgs& a, u64 n_slots_hint, u64 n_surv, int sm_count, cudaStream_t s, int phase /*0 compact, 1 write*/);
+cudaError_t launch_compact(const ExpandArgs& a, int sm_count, cudaStream_t s);
+cudaError_t launch_materialise(const ExpandArgs& a, int sm_count, cudaStream_t s);
 cudaError_t launch_roots(bool write /*false: build + classify, true: keep the survivors*/, const RootArgs& r, cudaStream_t s);
-cudaError_t launch_level_begin(Ctl* ctl, cudaStream_t s);
 
 // post.cu
 struct PostArgs {
@@ -33,7 +35,7 @@ struct PostArgs {
     u32* sort_idx; u64 n_pad;
     int* r_nnz; int* r_rxn; i64* r_val;   // final, lexicographic order
 };
-cudaError_t launch_select(const u64* keys, u64* ckeys /*compact buffer, max_keys slots*/, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches);
+cudaError_t launch_select(const u64* keys, u64* ckeys /*compact buffer*/, u64 max_ckeys, Ctl* ctl, int par /*level set holding n_keys / n_slots*/, u64 cap, u64 max_keys, int sm_count, cudaStream_t s, int* n_launches);
 cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_launches);
 cudaError_t launch_filter(const PostArgs& a, u64 n_uniq, int sm_count, cudaStream_t s, int* n_launches);
 cudaError_t launch_output_rows(const PostArgs& a, u64 n_uniq, cudaStream_t s, int* n_launches);

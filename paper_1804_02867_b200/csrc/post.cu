@@ -16,12 +16,6 @@ namespace efm {
 constexpr int kSelThreads = 256;
 constexpr int kTopBits = 11;
 
-__global__ void k_select_init(Ctl* ctl, u64 cap) {
-    const u64 n = ctl->n_keys;   // valid keys; the slot array may also hold kKeySentinel fillers
-    ctl->notrunc = (cap == 0 || n <= cap) ? 1u : 0u;
-    ctl->sel_prefix = 0; ctl->sel_rank = cap; ctl->sel_ticket = 0; ctl->X = 0; ctl->n_compact = 0;
-}
-
 // Whole block: the bin b with cum(b) <= rank < cum(b) + h[b]; returns through shared memory.
 __device__ void block_find_bin(const u32* h, int nb, u64 rank, u32* s_bin, u64* s_cum, u64* scratch) {
     const int T = blockDim.x, per = (nb + T - 1) / T, b0 = threadIdx.x * per;
@@ -49,15 +43,16 @@ __device__ void block_find_bin(const u32* h, int nb, u64 rank, u32* s_bin, u64* 
 
 // level 0: histogram of the top 11 bits of every key; level 1: of the next 11 bits of the keys inside the bin level 0
 // selected.  The last block (ticket) finds the bin that holds the wanted rank and extends the selected prefix.
-__global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restrict__ keys, Ctl* ctl, u64 max_keys, int level) {
-    if (ctl->notrunc) return;
+__global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restrict__ keys, Ctl* ctl, int par, u64 cap, u64 max_keys, int level) {
+    const LevelCtl* lv = &ctl->lv[par];
+    if (cap == 0 || lv->n_keys <= cap) return;   // the beam does not bind on this level
     __shared__ u32 h[SEL_BINS];
     __shared__ u64 scratch[kSelThreads];
     __shared__ u32 s_bin; __shared__ u64 s_cum; __shared__ bool is_last;
     for (int b = threadIdx.x; b < SEL_BINS; b += kSelThreads) h[b] = 0;
     __syncthreads();
-    const u64 n = min(ctl->n_slots, max_keys);   // an overflowed key array is reported by the host (ERR_KEYS)
-    const u64 top = ctl->sel_prefix;
+    const u64 n = min(lv->n_slots, max_keys);   // an overflowed key array is reported by the host (ERR_KEYS)
+    const u64 top = level == 0 ? 0ULL : ctl->sel_prefix;
     const int shift = 64 - kTopBits * (level + 1);
     // keys of one parent are neighbours and share their top bits: aggregate runs of equal bins per thread
     constexpr int RUN = 4;
@@ -85,18 +80,24 @@ __global__ void __launch_bounds__(kSelThreads) k_select_hist(const u64* __restri
     __threadfence();
     for (int b = threadIdx.x; b < SEL_BINS; b += kSelThreads) { h[b] = ((volatile u32*)ctl->hist)[b]; ctl->hist[b] = 0; }
     __syncthreads();
-    block_find_bin(h, SEL_BINS, ctl->sel_rank, &s_bin, &s_cum, scratch);
-    if (threadIdx.x == 0) { ctl->sel_prefix = (level == 0 ? 0ULL : top << kTopBits) | s_bin; ctl->sel_rank -= s_cum; ctl->sel_ticket = 0; }
+    const u64 rank = level == 0 ? cap : ctl->sel_rank;   // level 0 starts the selection: X = the key at sorted position cap
+    block_find_bin(h, SEL_BINS, rank, &s_bin, &s_cum, scratch);
+    if (threadIdx.x == 0) {
+        ctl->sel_prefix = (level == 0 ? 0ULL : top << kTopBits) | s_bin; ctl->sel_rank = rank - s_cum; ctl->sel_ticket = 0;
+        ctl->n_compact = 0;
+    }
 }
 
 // copies the keys that carry the selected 22-bit prefix to a compact buffer; the last block finishes the remaining
 // 42 bits on that buffer alone
-__global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __restrict__ keys, u64* __restrict__ ckeys, Ctl* ctl, u64 max_keys) {
-    if (ctl->notrunc) return;
+__global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __restrict__ keys, u64* __restrict__ ckeys, u64 max_ckeys, Ctl* ctl,
+                                                               int par, u64 cap, u64 max_keys) {
+    const LevelCtl* lv = &ctl->lv[par];
+    if (cap == 0 || lv->n_keys <= cap) return;
     __shared__ u32 h[SEL_BINS];
     __shared__ u64 scratch[kSelThreads];
     __shared__ u32 s_bin; __shared__ u64 s_cum; __shared__ bool is_last;
-    const u64 n = min(ctl->n_slots, max_keys);
+    const u64 n = min(lv->n_slots, max_keys);
     const u64 top = ctl->sel_prefix;
     constexpr int kLow = 64 - 2 * kTopBits;   // bits still open
     const int lane = threadIdx.x & 31;
@@ -110,7 +111,8 @@ __global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __rest
             u64 pos = 0;
             if (lane == 0) pos = atomicAdd(&ctl->n_compact, (u64)__popc(m));
             pos = __shfl_sync(0xffffffffu, pos, 0);
-            if (hit) ckeys[pos + __popc(m & ((1u << lane) - 1u))] = key;
+            if (pos + __popc(m) > max_ckeys) { if (lane == 0) atomicOr(&ctl->error, (u32)ERR_KEYS); }   // loud, never a wrong threshold
+            else if (hit) ckeys[pos + __popc(m & ((1u << lane) - 1u))] = key;
         }
     }
     __threadfence();
@@ -119,7 +121,7 @@ __global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __rest
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    const u64 nc = *(volatile u64*)&ctl->n_compact;
+    const u64 nc = min(*(volatile u64*)&ctl->n_compact, max_ckeys);
     u64 rank = ctl->sel_rank, prefix = 0;
     const int bits[4] = {11, 11, 10, 10};
     int shift = kLow;
@@ -142,16 +144,15 @@ __global__ void __launch_bounds__(kSelThreads) k_select_narrow(const u64* __rest
     if (threadIdx.x == 0) { ctl->X = (top << kLow) | prefix; ctl->sel_ticket = 0; }
 }
 
-cudaError_t launch_select(const u64* keys, u64* ckeys, Ctl* ctl, u64 cap, u64 max_keys, u64 n_keys_hint, int sm_count, cudaStream_t s, int* n_launches) {
-    k_select_init<<<1, 1, 0, s>>>(ctl, cap);
-    ++*n_launches;
-    if (cap == 0) return cudaGetLastError();
-    u64 blocks = (n_keys_hint + kSelThreads * 8 - 1) / (kSelThreads * 8);
+cudaError_t launch_select(const u64* keys, u64* ckeys, u64 max_ckeys, Ctl* ctl, int par, u64 cap, u64 max_keys, int sm_count, cudaStream_t s,
+                          int* n_launches) {
+    if (cap == 0) return cudaSuccess;
+    u64 blocks = (max_keys + kSelThreads * 8 - 1) / (kSelThreads * 8);
     if (blocks > (u64)sm_count * 8) blocks = (u64)sm_count * 8;
     if (blocks < 1) blocks = 1;
-    k_select_hist<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ctl, max_keys, 0);
-    k_select_hist<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ctl, max_keys, 1);
-    k_select_narrow<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ckeys, ctl, max_keys);
+    k_select_hist<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ctl, par, cap, max_keys, 0);
+    k_select_hist<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ctl, par, cap, max_keys, 1);
+    k_select_narrow<<<(unsigned)blocks, kSelThreads, 0, s>>>(keys, ckeys, max_ckeys, ctl, par, cap, max_keys);
     *n_launches += 3;
     return cudaGetLastError();
 }

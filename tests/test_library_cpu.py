@@ -1,3 +1,4 @@
+import os
 """CPU-side checks of the CUDA library: it builds, loads, exports the C ABI of include/efm_b200.h, its host-side
 graph builder (SURVEY.md 8(a) a-1) agrees with the oracle's graph, seeds are validated, and without a GPU the
 product path fails loudly instead of falling back to anything."""
@@ -28,10 +29,16 @@ def test_exports_every_declared_symbol(lib_mod):
     assert b"capacity" in lib.efm_strerror(lib_mod.EFM_E_CAPACITY)
 
 
-def test_struct_sizes_match_header(lib_mod):
-    # 4 x int32 + 4 x int64 + int32 + uint32 + int64; 23 x int64 + 9 x double
-    assert ctypes.sizeof(lib_mod.efm_params) == 64
-    assert ctypes.sizeof(lib_mod.efm_stats) == 8 * (19 + 9 + 9)
+def test_struct_sizes_match_header(lib_mod, tmp_path):
+    """The ctypes mirrors of efm_params / efm_stats have the sizes a C compiler gives the header's structs."""
+    import subprocess
+    src = tmp_path / "sz.c"
+    src.write_text('#include <stdio.h>\n#include "efm_b200.h"\nint main(void) { printf("%zu %zu\\n", sizeof(efm_params), sizeof(efm_stats)); return 0; }\n')
+    exe = tmp_path / "sz"
+    subprocess.run(["gcc", "-I", os.path.dirname(lib_mod.HEADER_PATH), str(src), "-o", str(exe)], check=True)
+    c_params, c_stats = (int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split())
+    assert ctypes.sizeof(lib_mod.efm_params) == c_params == 72
+    assert ctypes.sizeof(lib_mod.efm_stats) == c_stats
 
 
 @pytest.mark.parametrize("name", ["toy", "small", "core", "mid", "genome"])

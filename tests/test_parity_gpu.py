@@ -120,17 +120,16 @@ def test_poison_and_minimality_at_scale(efm, oracle_mod, name, over, count, size
 @pytest.mark.parametrize("two_pass", [False, True])
 def test_toy(efm, oracle_mod, two_pass):
     net = make_network("toy", 0)
-    flags = efm.EFM_F_FORCE_TWO_PASS if two_pass else 0
-    over = dict(frontier_cap=1 << 20) if two_pass else {}
-    assert_parity(efm, oracle_mod, net, flags=flags, **over)
-    assert_parity(efm, oracle_mod, net, seeds=oracle_mod.all_arc_seed_sets(net.reversible), flags=flags, **over)
+    over = dict(frontier_cap=1 << 20) if two_pass else {}   # with a cap the threshold selection is enqueued on every level
+    assert_parity(efm, oracle_mod, net, **over)
+    assert_parity(efm, oracle_mod, net, seeds=oracle_mod.all_arc_seed_sets(net.reversible), **over)
 
 
 def test_small(efm, oracle_mod):
     net = make_network("small", 0)
     got, _ = assert_parity(efm, oracle_mod, net)
     assert got.stats["direct_levels"] > 0 and got.stats["two_pass_levels"] == 0
-    got, _ = assert_parity(efm, oracle_mod, net, flags=efm.EFM_F_FORCE_TWO_PASS, frontier_cap=1 << 20)
+    got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=1 << 20)
     assert got.stats["two_pass_levels"] > 0 and got.stats["truncated_beam"] == 0
 
 
@@ -188,8 +187,7 @@ def test_general_routine_only(efm, oracle_mod):
     with the oracle (and hence with each other)."""
     for name, over in (("small", {}), ("core", dict(frontier_cap=2048)), ("genome", dict(frontier_cap=256))):
         assert_parity(efm, oracle_mod, make_network(name, 0), flags=efm.EFM_F_NO_FASTPATH, **over)
-    assert_parity(efm, oracle_mod, make_network("small", 0), flags=efm.EFM_F_NO_FASTPATH | efm.EFM_F_FORCE_TWO_PASS,
-                  frontier_cap=1 << 20)
+    assert_parity(efm, oracle_mod, make_network("small", 0), flags=efm.EFM_F_NO_FASTPATH, frontier_cap=1 << 20)
 
 
 def test_parents_read_in_place(efm, oracle_mod):
@@ -243,9 +241,12 @@ def test_columns_longer_than_a_warp(efm, oracle_mod):
 
 def test_key_capacity_error(efm):
     """max_child_keys too small for a level: EFM_E_CAPACITY, never a silently truncated result."""
-    net = make_network("core", 0)
-    with pytest.raises(efm.EfmError) as ei:
-        efm.enumerate_network(net, frontier_cap=4096, max_child_keys=64, max_frontier=4096)
+    net = make_network("genome", 0)
+    with pytest.raises(efm.EfmError) as ei:   # a level of 32768 parents evaluates about half a million children
+        efm.enumerate_network(net, frontier_cap=32768, max_child_keys=64)
+    assert ei.value.code == efm.EFM_E_CAPACITY
+    with pytest.raises(efm.EfmError) as ei:   # ... and sends thousands of them through the general routine
+        efm.enumerate_network(net, frontier_cap=32768, max_child_tasks=16, flags=efm.EFM_F_NO_FASTPATH)
     assert ei.value.code == efm.EFM_E_CAPACITY
 
 
