@@ -22,7 +22,7 @@ namespace {
 struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
-    Region col_ptr, col, node, in_e, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
+    Region col_ptr, col, colsig, node, in_e, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
     Region ctl, lvl, buf[2], off[2], plist, pprim, keys, tags, ckeys, tasks, surv, surv_dst, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill, vcount, vstart, vfill, tstart;
     Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, u_key, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
@@ -71,6 +71,7 @@ void make_layout(efm_handle* h) {
     Layout L;
     add_region(L, L.col_ptr, sizeof(int) * (G.A + 1));
     add_region(L, L.col, sizeof(int2) * (G.col.size() + 1));
+    add_region(L, L.colsig, sizeof(u64) * 2 * (G.A + 1));
     add_region(L, L.node, sizeof(int4) * (G.M + 1));
     add_region(L, L.in_e, sizeof(int2) * (G.in.size() + 1));
     add_region(L, L.out_e, sizeof(int2) * (G.out.size() + 1));
@@ -148,7 +149,7 @@ DevGraph dev_graph(const efm_handle* h, unsigned char* ws) {
     DevGraph g;
     g.M = h->G.M; g.A = h->G.A; g.W32 = (h->G.A + 31) / 32; g.M32 = (h->G.M + 31) / 32;
     g.col_ptr = (const int*)(ws + L.col_ptr.off);   g.col = (const int2*)(ws + L.col.off);
-    g.node = (const int4*)(ws + L.node.off);
+    g.node = (const int4*)(ws + L.node.off);        g.colsig = (const u64*)(ws + L.colsig.off);
     g.in_e = (const int2*)(ws + L.in_e.off);        g.out_e = (const int2*)(ws + L.out_e.off);
     g.in_alt = (const uint4*)(ws + L.in_alt.off);   g.out_alt = (const uint4*)(ws + L.out_alt.off);
     g.twin = (const int*)(ws + L.twin.off);
@@ -415,13 +416,14 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         h2d += (int64_t)bytes;
         return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s);
     };
-    std::vector<u64> arc_mix;
+    std::vector<u64> arc_mix, colsig;
     std::vector<uint32_t> alt_in, alt_out;
     std::vector<int> node, colp;
     if (h->graph_ws != ws) {   // the network is an input: it stays resident in the workspace across calls
         h->graph_ws = nullptr;
         // columns with the position of the arc in I[met] / O[met] next to the metabolite: {met | pos << 16, s}
         colp.resize(2 * G.col.size());
+        colsig.assign(2 * (size_t)G.A, 0ULL);
         {
             std::vector<int> fin(G.in_ptr.begin(), G.in_ptr.end() - 1), fout(G.out_ptr.begin(), G.out_ptr.end() - 1);
             for (int a = 0; a < G.A; ++a)
@@ -430,6 +432,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
                     const int pos = e.s > 0 ? fin[e.met]++ - G.in_ptr[e.met] : fout[e.met]++ - G.out_ptr[e.met];
                     colp[2 * (size_t)q] = (int)((uint32_t)e.met | ((uint32_t)pos << 16));
                     colp[2 * (size_t)q + 1] = e.s;
+                    colsig[2 * (size_t)a + (e.s > 0 ? 0 : 1)] |= 1ULL << (e.met & 63);
                 }
         }
         node.resize(4 * (size_t)G.M);
@@ -439,6 +442,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         }
         CK(up(ws + L.col_ptr.off, G.col_ptr.data(), sizeof(int) * G.col_ptr.size()));
         CK(up(ws + L.col.off, colp.data(), sizeof(int) * colp.size()));
+        CK(up(ws + L.colsig.off, colsig.data(), sizeof(u64) * colsig.size()));
         CK(up(ws + L.node.off, node.data(), sizeof(int) * node.size()));
         CK(up(ws + L.in_e.off, G.in.data(), sizeof(ArcRef) * G.in.size()));
         CK(up(ws + L.out_e.off, G.out.data(), sizeof(ArcRef) * G.out.size()));

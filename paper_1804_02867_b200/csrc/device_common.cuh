@@ -19,7 +19,7 @@ typedef unsigned short u16;
 //   [ 0,48)  header: u32 n_supp | n_vis << 16; u32 n_unb; u64 hs = sum of the arc terms of the state hash;
 //            u64 hv = sum of its visited terms; u64 big = max(largest flux, largest |EF|);
 //            i64 E = EF of i*; u32 i* | (vk + 1) << 16 (i* = lowest unbalanced metabolite, reading G12; vk = index of
-//            its visited record, vk + 1 = 0: first visit); u32 spare
+//            its visited record, vk + 1 = 0: first visit); u32 number of fluxes equal to 1
 //   i64  flux[n_supp]   fluxes of the support arcs, > 0, gcd 1
 //   u64  vis[n_vis]     visited records: cnt << 48 | met << 32 | PI << 16 | PO   (unordered)
 //   i64  ef[n_unb]      the non-zero extra fluxes EF_i (Eq 2) of the state   (unordered)
@@ -54,6 +54,7 @@ struct DevGraph {
     // needs: {arc | c << 16, twin | ncol << 16 | generic << 24, 6 x (met | s << 16)}; generic = 1: the column has more
     // than 6 entries or a number does not fit 16 bits, take the general routine
     const uint4* in_alt;  const uint4* out_alt;
+    const u64* colsig;    // per arc two words: bit (met & 63) set for every metabolite the arc produces / consumes (filter of the column scans)
     const int* twin;
     const i64* dep_off;   const u32* dep_bits;
     const int* arc_rxn;   const int* arc_dir;

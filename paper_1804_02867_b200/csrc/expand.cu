@@ -26,8 +26,14 @@ enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
 #ifndef EFM_MIN_BLOCKS
 #define EFM_MIN_BLOCKS 24   // resident one-warp blocks per SM the register allocation aims at (80 registers)
 #endif
-constexpr int kParentsPerItem = 8;     // first-visit parents a warp takes per work item
-constexpr int kRevisitPerItem = 32;    // revisit parents a warp takes per work item (four at a time)
+#ifndef EFM_RPI
+#define EFM_RPI 4
+#endif
+#ifndef EFM_PPI
+#define EFM_PPI 4
+#endif
+constexpr int kParentsPerItem = EFM_PPI;     // first-visit parents a warp takes per work item
+constexpr int kRevisitPerItem = EFM_RPI;    // revisit parents a warp takes per work item (four at a time)
 #ifndef EFM_STAGE_BYTES
 #define EFM_STAGE_BYTES 1536
 #endif
@@ -109,9 +115,11 @@ __device__ __forceinline__ u64 common_divisor(u32 gmask, int gl, const i64* flux
     for (;;) {
         u64 mn = ~0ULL;
 #pragma unroll 1
-        for (int t = gl; t < ns; t += G) {
-            if (t == ia) continue;
-            const u64 m = mod_any(k * (u64)flux[t], r);   // k f_t <= 2^62 (no overflow was found before)
+        for (int t0 = 0; t0 < ns; t0 += G) {   // group-uniform trip count
+            const int t = t0 + gl;
+            u64 m = 0;
+            if (t < ns && t != ia) m = mod_any(k * (u64)flux[t], r);   // k f_t <= 2^62 (no overflow was found before)
+            if (__any_sync(gmask, m == 1)) return 1;
             if (m) mn = min(mn, m);
         }
         mn = g_min(gmask, mn);
@@ -280,7 +288,7 @@ struct WarpAcc { u32 children, done, general; };   // warp-uniform counters kept
 
 // Header of an entry (three 16-byte words) decoded into registers.
 struct Hdr {
-    int ns, nv, nu, istar, vk;
+    int ns, nv, nu, istar, vk, ones;
     u64 hs, hv, big;
     i64 E;
 };
@@ -292,6 +300,7 @@ __device__ __forceinline__ Hdr decode_hdr(const uint4 h0, const uint4 h1, const 
     H.big = (u64)h1.z | ((u64)h1.w << 32);
     H.E = (i64)((u64)h2.x | ((u64)h2.y << 32));
     H.istar = (int)(h2.z & 0xffffu); H.vk = (int)(h2.z >> 16) - 1;
+    H.ones = (int)h2.w;
     return H;
 }
 __device__ __forceinline__ void write_task(const ExpandArgs& A, u64 ti, int ca, int cia, int cnu, u32 flags, u64 ck, u64 cd, u64 cT, u64 cg,
@@ -311,13 +320,25 @@ __device__ __forceinline__ void expand_revisits(const ExpandArgs& A, LevelCtl* l
     const u32 gmask = 0xffu << (grp * 8);
     Ctl* ctl = A.ctl;
     const bool small_graph = A.g.max_coef < kSmallCoef;
+    // list words of the item's parents: lane l holds parent l.  The entries are read in place; while four parents are
+    // processed, the lines of the next four are requested into L1 (one 128-byte line per lane and step).
+    const u64 mylw = first + (u64)lane < nR ? __ldg(&A.plist[A.max_frontier - 1 - (first + (u64)lane)]) : 0ULL;
+    auto request = [&](int r) {
+        const u64 w = __shfl_sync(FULL, mylw, (4 * r + grp) & 31);
+        const unsigned char* e = A.cur + ((w & kListOffMask) << 4);
+        const u32 bytes = (u32)((w >> kListShift) << 4);
+#pragma unroll 1
+        for (u32 o = (u32)gl * 128u; o < bytes; o += 1024u) asm volatile("prefetch.global.L1 [%0];\n" ::"l"(e + o));
+    };
+    request(0);
 #pragma unroll 1
     for (int r = 0; r < kRevisitPerItem / 4; ++r) {
         const u64 idx = first + (u64)(4 * r + grp);
         const bool live = idx < nR;
         if (!__any_sync(FULL, live)) break;
+        if (r + 1 < kRevisitPerItem / 4) request(r + 1);
         const u64 pid = A.max_frontier - 1 - (live ? idx : first);
-        const u64 lw = __ldg(&A.plist[pid]);
+        const u64 lw = __shfl_sync(FULL, mylw, live ? 4 * r + grp : 0);
         const unsigned char* eb = A.cur + ((lw & kListOffMask) << 4);
         const Hdr H = decode_hdr(__ldg((const uint4*)eb), __ldg((const uint4*)eb + 1), __ldg((const uint4*)eb + 2));
         const int ns = H.ns, nv = H.nv, nu = H.nu, istar = H.istar;
@@ -354,13 +375,18 @@ __device__ __forceinline__ void expand_revisits(const ExpandArgs& A, LevelCtl* l
         // and the positions of PI and PO in the support come along.
         const int nI = __ldg(&A.g.node[istar]).y;
         const i64 doff = __ldg(&A.g.dep_off[istar]);
-        bool dep = false;
+        // the pair (PO, PI) itself is one of the candidates in either direction: its bit often settles the test
+        const i64 b0 = doff + (i64)lPO * nI + lPI;
+        const bool dep0 = ((__ldg(&A.g.dep_bits[b0 >> 5]) >> (b0 & 31)) & 1u) != 0;
+        bool dep = dep0;
         int iaPI = -1, iaPO = -1;
+        const u64* sig = A.g.colsig + (fwd ? 0 : 1);   // metabolites an arc produces / consumes
 #pragma unroll 1
         for (int t = gl; t < ns; t += G) {
             const int a = arc[t];
-            if (a == PI) iaPI = t;
-            if (a == PO) iaPO = t;
+            if (a == PI) { iaPI = t; continue; }
+            if (a == PO) { iaPO = t; continue; }
+            if (dep0 || !((__ldg(&sig[2 * a]) >> (istar & 63)) & 1ULL)) continue;   // the column of a does not hold i* on that side
             const int q0 = __ldg(&A.g.col_ptr[a]), q1 = __ldg(&A.g.col_ptr[a + 1]);
 #pragma unroll 1
             for (int q = q0; q < q1; ++q) {
@@ -439,8 +465,9 @@ __device__ __forceinline__ void expand_revisits(const ExpandArgs& A, LevelCtl* l
             act = false;
         }
         // gcd normalisation (reading G10): g = gcd(T, k f_t for t != a)
+        // A flux of 1 on another arc settles it: g divides k then, and gcd(T, k) = gcd(d, k) = 1.
         u64 cg = 1;
-        if (act) cg = common_divisor<G>(gmask, gl, flux, ns, cia, ck, cT);
+        if (act && H.ones - (int)(fa == 1) <= 0) cg = common_divisor<G>(gmask, gl, flux, ns, cia, ck, cT);
         u64 chs;
         if (cg == 1) chs = ck * H.hs + arc_mult(A.g, (u32)ca) * (cT - ck * fa);   // linear arc part of the state hash
         else {
@@ -522,13 +549,23 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
         const bool fwd = E > 0;
         const u64 absE = abs64(E);
         u32* sbits = S.sbits; u16* upos = S.upos;
+        // the graph data of i* is requested before the tables are built: slices of I / O, the first 32 OR-alternative
+        // records and the first 32 arcs of the primary search
+        const int4 nd = __ldg(&A.g.node[istar]);
+        const int in0 = nd.x, nI = nd.y, out0 = nd.z, nO = nd.w;
+        const int2* alist = fwd ? A.g.out_e + out0 : A.g.in_e + in0;
+        const uint4* altl = fwd ? A.g.out_alt + 2 * (size_t)out0 : A.g.in_alt + 2 * (size_t)in0;
+        const int alen = fwd ? nO : nI;
+        const int2* plist = fwd ? A.g.in_e + in0 : A.g.out_e + out0;
+        const int plen = fwd ? nI : nO;
+        uint4 r0n = make_uint4(0, 0, 0, 0), r1n = r0n;
+        if (lane < alen) { r0n = __ldg(&altl[2 * lane]); r1n = __ldg(&altl[2 * lane + 1]); }
+        int pan = lane < plen ? __ldg(&plist[lane]).x : -1;
         // ---- support bitset, EF index table
 #pragma unroll 1
         for (int t = lane; t < ns; t += 32) { const u32 a = arc[t]; atomicOr(&sbits[a >> 5], 1u << (a & 31)); }
 #pragma unroll 1
         for (int t = lane; t < nu; t += 32) upos[efmet[t]] = (u16)(t + 1);
-        const int4 nd = __ldg(&A.g.node[istar]);
-        const int in0 = nd.x, nI = nd.y, out0 = nd.z, nO = nd.w;
         __syncwarp();
         auto ef_of = [&](int met) -> i64 { const u32 u = upos[met]; return u ? ef[u - 1] : 0; };
         int n_adm = 0;
@@ -537,21 +574,15 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
         } else {
             // primary on the side the flux arrives from: lowest arc of that side in the support (G13)
             int prim = -1;
-            {
-                const int2* plist = fwd ? A.g.in_e + in0 : A.g.out_e + out0;
-                const int plen = fwd ? nI : nO;
 #pragma unroll 1
-                for (int base = 0; base < plen && prim < 0; base += 32) {
-                    const int q = base + lane;
-                    const int pa = q < plen ? __ldg(&plist[q]).x : -1;
-                    const u32 bal = __ballot_sync(FULL, pa >= 0 && sbit(sbits, pa));
-                    if (bal) prim = __shfl_sync(FULL, pa, __ffs(bal) - 1);
-                }
+            for (int base = 0; base < plen && prim < 0; base += 32) {
+                const int pa = pan;
+                const int qn = base + 32 + lane;
+                pan = qn < plen ? __ldg(&plist[qn]).x : -1;
+                const u32 bal = __ballot_sync(FULL, pa >= 0 && sbit(sbits, pa));
+                if (bal) prim = __shfl_sync(FULL, pa, __ffs(bal) - 1);
             }
             if (lane == 0) A.pprim[pid] = (u32)prim;
-            const int2* alist = fwd ? A.g.out_e + out0 : A.g.in_e + in0;
-            const uint4* altl = fwd ? A.g.out_alt + 2 * (size_t)out0 : A.g.in_alt + 2 * (size_t)in0;
-            const int alen = fwd ? nO : nI;
             const bool fastP = fast_graph && H.big < kSmall;
             // visited record of i* without the chosen arc (PI = primary / chosen arc, PO = chosen arc / primary)
             const u64 vbase = vis_pack((u32)istar, fwd ? (u32)prim : 0u, fwd ? 0u : (u32)prim, 0u);
@@ -561,9 +592,9 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
                 const int q = base + lane;
                 int a = -1, c = 1;
                 bool adm = false, insup = false, generic = false;
-                uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
+                const uint4 r0 = r0n, r1 = r1n;   // requested one round ahead
+                if (q + 32 < alen) { r0n = __ldg(&altl[2 * (q + 32)]); r1n = __ldg(&altl[2 * (q + 32) + 1]); }
                 if (q < alen) {   // one 32-byte record per OR-alternative: arc, c, twin and the column of the arc
-                    r0 = __ldg(&altl[2 * q]); r1 = __ldg(&altl[2 * q + 1]);
                     a = (int)(r0.x & 0xffffu); c = (int)(r0.x >> 16);
                     const u32 tw = r0.y & 0xffffu;
                     generic = (r0.y >> 24) & 1u;
@@ -681,7 +712,7 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
                     // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and
                     // gcd(k, d) = 1.  An arc of the support: g = gcd(T, k f_t for t != a).
                     u64 cg = 1;
-                    if (cin) cg = common_divisor<32>(FULL, lane, flux, ns, cia, ck, cT);
+                    if (cin && H.ones - (int)(fa == 1) <= 0) cg = common_divisor<32>(FULL, lane, flux, ns, cia, ck, cT);   // a unit flux elsewhere: g = 1
                     u64 chs;
                     if (cg == 1) chs = ck * H.hs + arc_mult(A.g, (u32)ca) * (cT - ck * fa);
                     else {
@@ -996,6 +1027,7 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
     u16* arc2 = (u16*)(ef2 + nu2);
     u16* efmet2 = arc2 + n2;
     u64 mx = cin ? 0ULL : cT;   // a new arc never comes with a common divisor
+    int ones = 0;               // fluxes equal to 1 (the expansion of the child skips its gcd sweep when another arc carries 1)
     for (int t = lane; t < ns; t += G) {
         const u64 ft = t < G ? (u64)pf0 : (t < 2 * G ? (u64)pf1 : (u64)flux[t]);
         u64 F = t == cia ? cT : ck * ft;
@@ -1004,8 +1036,10 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
         flux2[pos] = (i64)F;
         arc2[pos] = (u16)(t < G ? pa0 : (t < 2 * G ? pa1 : (u32)arc[t]));
         mx = max(mx, F);
+        ones += (int)(F == 1);
     }
-    if (!cin && lane == 0) { flux2[ins] = (i64)cT; arc2[ins] = (u16)ca; }
+    if (!cin && lane == 0) { flux2[ins] = (i64)cT; arc2[ins] = (u16)ca; ones += (int)(cT == 1); }
+    ones = __reduce_add_sync(gmask, ones);
     u32 best = 0xffffffffu;   // lowest unbalanced metabolite of the child (reading G12): met << 16 | position in its list
     i64 bestE = 0;
     int vk2 = -1;
@@ -1084,7 +1118,7 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
         uint4* h4 = (uint4*)dst;
         h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2, (u32)chs, (u32)(chs >> 32));
         h4[1] = make_uint4((u32)chv, (u32)(chv >> 32), (u32)mx, (u32)(mx >> 32));
-        h4[2] = make_uint4((u32)(u64)bestE, (u32)((u64)bestE >> 32), to_cand ? 0u : ((best >> 16) | ((u32)(vk2 + 1) << 16)), 0u);
+        h4[2] = make_uint4((u32)(u64)bestE, (u32)((u64)bestE >> 32), to_cand ? 0u : ((best >> 16) | ((u32)(vk2 + 1) << 16)), (u32)ones);
     }
     }   // ok
     }
@@ -1159,7 +1193,7 @@ __global__ void __launch_bounds__(128) k_roots(const RootArgs R) {
         }
     ((u32*)e)[0] = (u32)ns; ((u32*)e)[1] = (u32)nu;
     ((u64*)e)[1] = hs; ((u64*)e)[2] = 0; ((u64*)e)[3] = big;
-    ((u64*)e)[4] = (u64)E; ((u32*)e)[10] = nu ? istar : 0u; ((u32*)e)[11] = 0u;   // no visited record yet: first visit
+    ((u64*)e)[4] = (u64)E; ((u32*)e)[10] = nu ? istar : 0u; ((u32*)e)[11] = (u32)ns;   // no visited record yet: first visit; every flux is 1
     if (nu == 0) {   // balanced at once (arbiter "Done")
         R.keys[r] = kKeySentinel;
         atomicAdd(&lv->n_done, 1ULL);
