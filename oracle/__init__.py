@@ -29,10 +29,14 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+END_CODES = {0: "none", 1: "done", 2: "not_efm_maxloop", 3: "dead_end", 4: "visited_cap", 5: "nonpos", 6: "overflow"}
+
+
 class _Params(ctypes.Structure):
     _fields_ = [("max_support", ctypes.c_int32), ("max_loop", ctypes.c_int32), ("dep_depth", ctypes.c_int32),
                 ("max_visited", ctypes.c_int32), ("frontier_cap", ctypes.c_int64), ("threads", ctypes.c_int32),
-                ("trace", ctypes.c_int32), ("shuffle_seed", ctypes.c_uint64)]
+                ("trace", ctypes.c_int32), ("shuffle_seed", ctypes.c_uint64), ("sample_count", ctypes.c_int32),
+                ("reserved", ctypes.c_int32), ("sample_seed", ctypes.c_uint64), ("allowed", ctypes.c_void_p)]
 
 
 STAT_FIELDS = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxloop", "discarded_nonpos",
@@ -66,6 +70,9 @@ def _load():
         lib.oracle_graph_info.argtypes = [ctypes.c_void_p] + [ctypes.c_void_p] * 5
         lib.oracle_graph_export.argtypes = [ctypes.c_void_p] + [ctypes.c_void_p] * 14
         lib.oracle_result_free.argtypes = [ctypes.c_void_p]
+        lib.oracle_result_steps.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.oracle_result_cand_end.restype = ctypes.c_int64
+        lib.oracle_result_cand_end.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64]
         lib.oracle_result_trace.restype = ctypes.c_int64
         lib.oracle_result_trace.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64]
         lib.oracle_state_hash.restype = ctypes.c_uint64
@@ -92,6 +99,8 @@ class OracleResult:
     # test hook (trace=True): per level the list of entries as dicts
     # {flux: {arc: f}, visited: {met: (PI, PO, cnt)}, n_unb, istar, key, kept}
     trace: Optional[List[List[dict]]] = None
+    steps: Optional[np.ndarray] = None      # per output row: expansions that built the pathway
+    cand_end: Optional[np.ndarray] = None   # sampling mode (8(f)-1): per candidate (code, steps); codes in END_CODES
 
 
 def _ptr(a: np.ndarray):
@@ -101,7 +110,8 @@ def _ptr(a: np.ndarray):
 def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarray, params: Dict[str, int],
                        seed_sets: Optional[Sequence[Sequence[int]]] = None, threads: int = 1,
                        shuffle_seed: int = 0, export_graph: bool = False,
-                       self_check: bool = True, trace: bool = False) -> OracleResult:
+                       self_check: bool = True, trace: bool = False, sample_count: int = 0, sample_seed: int = 0,
+                       allowed: Optional[np.ndarray] = None) -> OracleResult:
     """Run the oracle.  ``seed_sets`` holds arc codes 2*j + (dir < 0); None = default boundary arcs (O2)."""
     lib = _load()
     S = np.ascontiguousarray(S, dtype=np.int32)
@@ -110,7 +120,11 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
     m, n = S.shape
     p = _Params(int(params.get("max_support", 0)), int(params.get("max_loop", 8)), int(params.get("dep_depth", 4)),
                 int(params.get("max_visited", 0)), int(params.get("frontier_cap", 0)), int(threads), int(trace),
-                int(shuffle_seed))
+                int(shuffle_seed), int(sample_count), 0, int(sample_seed) & ((1 << 64) - 1), None)
+    if allowed is not None:
+        allowed = np.ascontiguousarray(allowed, dtype=np.uint8)
+        assert allowed.shape == (n,)
+        p.allowed = allowed.ctypes.data
     if seed_sets:
         ptr = np.zeros(len(seed_sets) + 1, dtype=np.int32)
         ptr[1:] = np.cumsum([len(s) for s in seed_sets])
@@ -161,6 +175,14 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
             g.update(M=M, A=A, W=W)
             graph = g
         n_roots = int(lib.oracle_result_roots(handle))
+        steps = np.zeros(k, dtype=np.int64)
+        if k:
+            lib.oracle_result_steps(handle, _ptr(steps))
+        cand_end = None
+        if sample_count > 0:
+            raw = np.zeros(max(n_roots, 1), dtype=np.int64)
+            lib.oracle_result_cand_end(handle, _ptr(raw), n_roots)
+            cand_end = np.stack([raw[:n_roots] & 0xff, raw[:n_roots] >> 8], axis=1)
         tr = None
         if trace:
             nt = int(lib.oracle_result_trace(handle, None, 0))
@@ -178,7 +200,7 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
                 tr[lvl].append(dict(flux=fl, visited=vis, n_unb=nu, istar=istar, key=key & ((1 << 64) - 1), kept=bool(kept)))
     finally:
         lib.oracle_result_free(handle)
-    res = OracleResult(flux, stats, levels, n_roots, graph, tr)
+    res = OracleResult(flux, stats, levels, n_roots, graph, tr, steps, cand_end)
     if self_check:
         from .check import check_outputs
         check_outputs(S, rev, internal, flux)
@@ -186,7 +208,8 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
 
 
 def enumerate_network(net, threads: int = 1, shuffle_seed: int = 0, export_graph: bool = False,
-                      self_check: bool = True, seed_sets="net", trace: bool = False, **param_overrides) -> OracleResult:
+                      self_check: bool = True, seed_sets="net", trace: bool = False, sample_count: int = 0,
+                      sample_seed: int = 0, allowed: Optional[np.ndarray] = None, **param_overrides) -> OracleResult:
     """Run the oracle on a ``netgen.Network`` with its own parameters (optionally overridden).
 
     ``seed_sets="net"`` uses the network's own seed sets (None there = default boundary arcs)."""
@@ -194,7 +217,7 @@ def enumerate_network(net, threads: int = 1, shuffle_seed: int = 0, export_graph
     params.update(param_overrides)
     seeds = net.seed_sets if isinstance(seed_sets, str) else seed_sets
     return enumerate_pathways(net.S, net.reversible, net.internal, params, seeds, threads, shuffle_seed,
-                              export_graph, self_check, trace)
+                              export_graph, self_check, trace, sample_count, sample_seed, allowed)
 
 
 def state_hash(arcs: Sequence[int], fluxes: Sequence[int], visited: Sequence[Sequence[int]]) -> int:

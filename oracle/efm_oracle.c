@@ -50,6 +50,16 @@ typedef struct {
     int32_t threads;       /* OpenMP threads used over the entries of a level              */
     int32_t trace;         /* 1: record every entry of every level, 2: only the balanced ones (test hook) */
     uint64_t shuffle_seed; /* != 0: permute every level before processing (pin P10)        */
+    /* SURVEY.md 8(f)-1 literal sampling mode ("each pathway is created using randomly selected output/input",
+     * PAPER.md:360 "after attempting 48 EFM candidates"): sample_count = C > 0 runs C candidate pathways, candidate c starts
+     * from seed set c mod n_sets and takes ONE admissible alternative per first visit, chosen by the counter-based
+     * generator pick(sample_seed, c, i*) below; no fan-out, no beam. */
+    int32_t sample_count;
+    int32_t reserved;
+    uint64_t sample_seed;
+    /* SURVEY.md 8(f)-2 targeted observability ("contributing reactions of each EFM were selected intentionally",
+     * PAPER.md:392-396): allowed[j] = 0 makes every OR-alternative of reaction j inadmissible; NULL = all allowed */
+    const uint8_t *allowed;
 } oracle_params;
 
 typedef struct {
@@ -188,6 +198,8 @@ static int graph_build(graph *G, const int32_t *S, int m, int n, const uint8_t *
 typedef struct { int32_t met, PI, PO, cnt; } visit;
 typedef struct {
     int32_t n_supp, n_vis;
+    int32_t cand;  /* root (seed set / sampled candidate) the pathway descends from */
+    int32_t level; /* number of expansions that built it (its "steps") */
     int32_t *arc;  /* support arcs, ascending arc id       */
     int64_t *f;    /* their fluxes, > 0, gcd = 1           */
     visit *vis;    /* visited metabolites, ascending index */
@@ -198,7 +210,7 @@ static entry *entry_new(int n_supp, int n_vis) {
     char *p = malloc(sz);
     if (!p) { fprintf(stderr, "oracle: out of memory\n"); abort(); }
     entry *e = (entry *)p;
-    e->n_supp = n_supp; e->n_vis = n_vis;
+    e->n_supp = n_supp; e->n_vis = n_vis; e->cand = 0; e->level = 0;
     e->f = (int64_t *)(p + sizeof(entry));
     e->vis = (visit *)(e->f + n_supp);
     e->arc = (int32_t *)(e->vis + n_vis);
@@ -338,7 +350,18 @@ typedef struct {
     i128 *EF, *EFs;
     int *touched, *touched2;
     uint8_t *insupp;
+    int64_t *cand_end;   /* sampling mode: how and when candidate c ended (shared array, one writer per candidate) */
 } worker;
+
+/* how a sampled candidate ended: code | steps << 8 (steps = expansions made before the end) */
+enum { END_NONE = 0, END_DONE = 1, END_NOTEFM = 2, END_DEAD = 3, END_VISITED = 4, END_NONPOS = 5, END_OVERFLOW = 6 };
+
+/* 8(f)-1: the alternative candidate c takes at the first visit of metabolite i among n admissible ones is number
+ * pick mod n in ascending arc order; a counter-based generator (no state, no order dependence), reading G23:
+ *   pick(seed, c, i) = mix( mix(seed + 0x9E3779B97F4A7C15 * (c + 1)) ^ (0x04 << 56 | i) ) */
+static uint64_t sample_pick(uint64_t seed, int32_t cand, int32_t met) {
+    return mix64(mix64(seed + 0x9E3779B97F4A7C15ULL * ((uint64_t)cand + 1ULL)) ^ (0x0400000000000000ULL | (uint64_t)met));
+}
 
 static void expand(const graph *G, const oracle_params *P, const entry *e, int istar, i128 E, worker *wk) {
     oracle_stats *st = &wk->st;
@@ -352,32 +375,50 @@ static void expand(const graph *G, const oracle_params *P, const entry *e, int i
     int64_t bytes = algo_entry_bytes(e);
     if (vk < 0) {
         /* first visit: PROC1 / PROC1' (Eq 3; readings G1, G13, G14, G15, G22) */
-        if (e->n_vis >= V) { st->discarded_visited++; goto out; }
+        if (e->n_vis >= V) { st->discarded_visited++; if (wk->cand_end) wk->cand_end[e->cand] = END_VISITED | ((int64_t)e->level << 8); goto out; }
         int prim = -1; /* forward: PI = lowest producer in the support; backward: PO = lowest consumer */
         if (fwd) { for (int q = G->in_ptr[istar]; q < G->in_ptr[istar + 1] && prim < 0; q++) if (in[G->in_arc[q]]) prim = G->in_arc[q]; }
         else     { for (int q = G->out_ptr[istar]; q < G->out_ptr[istar + 1] && prim < 0; q++) if (in[G->out_arc[q]]) prim = G->out_arc[q]; }
         int lo = fwd ? G->out_ptr[istar] : G->in_ptr[istar];
         int hi = fwd ? G->out_ptr[istar + 1] : G->in_ptr[istar + 1];
-        int n_adm = 0;
+        int n_adm = 0, pick = -1;
+        if (P->sample_count > 0) {   /* sampling: count the admissible alternatives first, then take exactly one of them */
+            for (int q = lo; q < hi; q++) {
+                int a = fwd ? G->out_arc[q] : G->in_arc[q];
+                if (G->twin[a] >= 0 && in[G->twin[a]]) continue;
+                if (!in[a] && e->n_supp >= D) continue;
+                if (P->allowed && !P->allowed[G->arc_rxn[a]]) continue;
+                n_adm++;
+            }
+            if (n_adm > 0) pick = (int)(sample_pick(P->sample_seed, e->cand, istar) % (uint64_t)n_adm);
+            n_adm = 0;
+        }
         for (int q = lo; q < hi; q++) {
             int a = fwd ? G->out_arc[q] : G->in_arc[q];
             int64_t c = fwd ? G->out_c[q] : G->in_c[q];
             if (G->twin[a] >= 0 && in[G->twin[a]]) continue;     /* G14 twin exclusion */
             if (!in[a] && e->n_supp >= D) continue;              /* G15 support cap    */
+            if (P->allowed && !P->allowed[G->arc_rxn[a]]) continue;   /* 8(f)-2: reaction outside the given subset */
             n_adm++;
+            if (pick >= 0 && n_adm - 1 != pick) continue;        /* 8(f)-1: only the sampled alternative */
             int status;
             entry *ch = bump(G, e, a, +1, absE, c, 1, wk->EFs, wk->touched2, &status);
-            if (!ch) { if (status == BUMP_OVERFLOW) st->discarded_overflow++; else st->discarded_nonpos++; continue; }
+            if (!ch) {
+                if (status == BUMP_OVERFLOW) st->discarded_overflow++; else st->discarded_nonpos++;
+                if (wk->cand_end) wk->cand_end[e->cand] = (status == BUMP_OVERFLOW ? END_OVERFLOW : END_NONPOS) | ((int64_t)e->level << 8);
+                continue;
+            }
+            ch->cand = e->cand; ch->level = e->level + 1;
             set_visit(ch, e->n_vis, istar, fwd ? prim : a, fwd ? a : prim, 0);
             evec_push(&wk->children, ch);
             st->children++;
             bytes += 8;
         }
-        if (n_adm == 0) st->dead_end++;
+        if (n_adm == 0) { st->dead_end++; if (wk->cand_end) wk->cand_end[e->cand] = END_DEAD | ((int64_t)e->level << 8); }
     } else {
         /* revisit: PROC2-4 (readings G2-G5) */
         int cnt = e->vis[vk].cnt + 1;
-        if (cnt > P->max_loop) { st->not_efm_maxloop++; goto out; }
+        if (cnt > P->max_loop) { st->not_efm_maxloop++; if (wk->cand_end) wk->cand_end[e->cand] = END_NOTEFM | ((int64_t)e->level << 8); goto out; }
         int PI = e->vis[vk].PI, PO = e->vis[vk].PO;
         int nI = G->in_ptr[istar + 1] - G->in_ptr[istar];
         int lPI = -1, lPO = -1;
@@ -398,7 +439,12 @@ static void expand(const graph *G, const oracle_params *P, const entry *e, int i
         else     { if (!dep) { a = PI; c = cPI; sign = +1; } else { a = PO; c = cPO; sign = -1; } }
         int status;
         entry *ch = bump(G, e, a, sign, absE, c, 0, wk->EFs, wk->touched2, &status);
-        if (!ch) { if (status == BUMP_OVERFLOW) st->discarded_overflow++; else st->discarded_nonpos++; goto out; }
+        if (!ch) {
+            if (status == BUMP_OVERFLOW) st->discarded_overflow++; else st->discarded_nonpos++;
+            if (wk->cand_end) wk->cand_end[e->cand] = (status == BUMP_OVERFLOW ? END_OVERFLOW : END_NONPOS) | ((int64_t)e->level << 8);
+            goto out;
+        }
+        ch->cand = e->cand; ch->level = e->level + 1;
         set_visit(ch, e->n_vis, istar, PI, PO, cnt);
         evec_push(&wk->children, ch);
         st->children++;
@@ -415,6 +461,9 @@ typedef struct {
     int64_t n_out;
     int64_t *flux;       /* n_out x n, canonical order */
     oracle_stats st;
+    int64_t *steps;      /* per output row: expansions that built the pathway (smallest over equal duplicates) */
+    int64_t n_cand_end;  /* sampling mode: candidates */
+    int64_t *cand_end;   /* code | steps << 8 per candidate */
     int64_t n_levels_rec;
     int64_t *lvl_active, *lvl_done, *lvl_expanded, *lvl_children;
     graph G;
@@ -509,7 +558,23 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
         free(mark);
     }
     free(code2arc);
+    if (P.sample_count > 0) {   /* 8(f)-1: candidate c is a copy of root c mod (number of seed sets) */
+        evec sets = level;
+        evec cl = {0};
+        for (int c = 0; c < P.sample_count && sets.n > 0; c++) {
+            const entry *src = sets.v[c % sets.n];
+            entry *e = entry_new(src->n_supp, 0);
+            for (int t = 0; t < src->n_supp; t++) { e->arc[t] = src->arc[t]; e->f[t] = 1; }
+            evec_push(&cl, e);
+        }
+        for (int64_t x = 0; x < sets.n; x++) free(sets.v[x]);
+        free(sets.v);
+        level = cl;
+        P.frontier_cap = 0;     /* a candidate has one descendant at most: nothing to cut */
+    }
+    for (int64_t x = 0; x < level.n; x++) { level.v[x]->cand = (int32_t)x; level.v[x]->level = 0; }
     R->n_roots = (int)level.n;
+    if (P.sample_count > 0) { R->n_cand_end = level.n; R->cand_end = calloc(level.n + 1, sizeof(int64_t)); }
 
     worker *wk = calloc(nthreads, sizeof(worker));
     for (int t = 0; t < nthreads; t++) {
@@ -517,6 +582,7 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
         int maxnnz = G->col_ptr[A] + 16;
         wk[t].touched = malloc(sizeof(int) * maxnnz); wk[t].touched2 = malloc(sizeof(int) * maxnnz);
         wk[t].insupp = calloc(A + 1, 1);
+        wk[t].cand_end = R->cand_end;
     }
     evec cands = {0};
     oracle_stats *st = &R->st;
@@ -623,7 +689,12 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
         R->lvl_active[R->n_levels_rec] = n_active; R->lvl_done[R->n_levels_rec] = n_done;
         R->lvl_expanded[R->n_levels_rec] = lvl_exp; R->lvl_children[R->n_levels_rec] = lvl_ch;
         R->n_levels_rec++;
-        for (int64_t x = 0; x < N; x++) { if (istar[x] < 0) evec_push(&cands, level.v[x]); else free(level.v[x]); }
+        for (int64_t x = 0; x < N; x++) {
+            if (istar[x] < 0) {
+                if (R->cand_end) R->cand_end[level.v[x]->cand] = END_DONE | ((int64_t)level.v[x]->level << 8);
+                evec_push(&cands, level.v[x]);
+            } else free(level.v[x]);
+        }
         free(istar); free(nunb); free(Estar); free(keep); free(level.v);
         level = next;
     }
@@ -642,7 +713,11 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
     evec uniq = {0};
     for (int64_t x = 0; x < cands.n;) {
         int64_t y = x; int poisoned = 0;
-        while (y < cands.n && same_support(cands.v[x], cands.v[y])) { if (cmp_cand(&cands.v[x], &cands.v[y]) != 0) poisoned = 1; y++; }
+        while (y < cands.n && same_support(cands.v[x], cands.v[y])) {
+            if (cmp_cand(&cands.v[x], &cands.v[y]) != 0) poisoned = 1;
+            if (cands.v[y]->level < cands.v[x]->level) cands.v[x]->level = cands.v[y]->level;   /* steps of the support: its quickest construction */
+            y++;
+        }
         st->unique_supports++;
         if (poisoned) st->poisoned++; else evec_push(&uniq, cands.v[x]);
         x = y;
@@ -671,18 +746,27 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
     /* (iv) reaction space v_j = f_j+ - f_j-, (v) lexicographic order */
     int64_t n_out = 0;
     for (int64_t x = 0; x < uniq.n; x++) n_out += minimal[x];
-    R->flux = calloc((size_t)(n_out + 1) * n, sizeof(int64_t));
+    /* rows carry their step count behind the n flux columns while they are sorted */
+    int64_t *rows = calloc((size_t)(n_out + 1) * (n + 1), sizeof(int64_t));
     int64_t r = 0;
     for (int64_t x = 0; x < uniq.n; x++) {
         if (!minimal[x]) continue;
         for (int k = 0; k < uniq.v[x]->n_supp; k++) {
             int a = uniq.v[x]->arc[k];
-            R->flux[r * n + G->arc_rxn[a]] += (int64_t)G->arc_dir[a] * uniq.v[x]->f[k];
+            rows[r * (n + 1) + G->arc_rxn[a]] += (int64_t)G->arc_dir[a] * uniq.v[x]->f[k];
         }
+        rows[r * (n + 1) + n] = uniq.v[x]->level;
         r++;
     }
-    g_sort_n = n;
-    qsort(R->flux, n_out, sizeof(int64_t) * n, cmp_rows);
+    g_sort_n = n;   /* the comparison looks at the n flux columns only (they are distinct) */
+    qsort(rows, n_out, sizeof(int64_t) * (n + 1), cmp_rows);
+    R->flux = calloc((size_t)(n_out + 1) * n, sizeof(int64_t));
+    R->steps = calloc((size_t)n_out + 1, sizeof(int64_t));
+    for (int64_t x = 0; x < n_out; x++) {
+        memcpy(R->flux + x * n, rows + x * (n + 1), sizeof(int64_t) * n);
+        R->steps[x] = rows[x * (n + 1) + n];
+    }
+    free(rows);
     R->n_out = n_out; st->output = n_out;
 
     free(bits); free(minimal); free(uniq.v);
@@ -698,6 +782,11 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
 int64_t oracle_result_count(const oracle_result *R) { return R->n_out; }
 void oracle_result_copy(const oracle_result *R, int64_t *dst) { memcpy(dst, R->flux, sizeof(int64_t) * R->n_out * R->n); }
 void oracle_result_stats(const oracle_result *R, oracle_stats *st) { *st = R->st; }
+void oracle_result_steps(const oracle_result *R, int64_t *dst) { memcpy(dst, R->steps, sizeof(int64_t) * R->n_out); }
+int64_t oracle_result_cand_end(const oracle_result *R, int64_t *dst, int64_t cap) {
+    for (int64_t x = 0; x < R->n_cand_end && x < cap; x++) dst[x] = R->cand_end[x];
+    return R->n_cand_end;
+}
 int64_t oracle_result_levels(const oracle_result *R, int64_t *active, int64_t *done, int64_t *expanded, int64_t *children, int64_t cap) {
     int64_t k = R->n_levels_rec < cap ? R->n_levels_rec : cap;
     for (int64_t x = 0; x < k; x++) { active[x] = R->lvl_active[x]; done[x] = R->lvl_done[x]; expanded[x] = R->lvl_expanded[x]; children[x] = R->lvl_children[x]; }
@@ -730,6 +819,7 @@ void oracle_result_free(oracle_result *R) {
     if (!R) return;
     if (R->have_graph) graph_free(&R->G);
     free(R->trace);
+    free(R->steps); free(R->cand_end);
     free(R->flux); free(R->lvl_active); free(R->lvl_done); free(R->lvl_expanded); free(R->lvl_children);
     free(R);
 }

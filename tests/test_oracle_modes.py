@@ -1,0 +1,159 @@
+"""Pins of the oracle's two extra modes (SURVEY.md 8(f)-1 literal sampling, 8(f)-2 targeted observability) and of the
+step count it reports per pathway.  Nothing here compares the oracle with itself only: the sampled choice is restated in
+Python from the formula in DESIGN.md (reading G23), the reachable states are compared with the exhaustive fan-out
+(Theorem 1: "by selecting all outputs/inputs ... all pathways are produced"), the mask and the step
+counts are derived by hand on the P1 / P2 / P5 networks of SURVEY.md 8(c)."""
+import numpy as np
+import pytest
+
+from netgen import hand_network, make_network
+
+M64 = (1 << 64) - 1
+
+
+def mix(x):   # SplitMix64 finaliser, written out (published constants; pinned against vectors in test_oracle_pins.py)
+    x &= M64
+    x ^= x >> 30; x = (x * 0xBF58476D1CE4E5B9) & M64
+    x ^= x >> 27; x = (x * 0x94D049BB133111EB) & M64
+    x ^= x >> 31
+    return x
+
+
+def pick(seed, cand, met):   # DESIGN.md reading G23
+    return mix(mix((seed + 0x9E3779B97F4A7C15 * (cand + 1)) & M64) ^ ((0x04 << 56) | met))
+
+
+P1 = ([({}, {"A": 1}, False), ({"A": 1}, {"B": 1, "C": 1}, False), ({"B": 1}, {}, False), ({"C": 1}, {}, False)], ["A", "B", "C"])
+P2 = ([({}, {"A": 1}, False), ({"A": 1}, {"B": 1, "C": 1}, False), ({"C": 2}, {"A": 1}, False), ({"B": 1}, {}, False)], ["A", "B", "C"])
+P5 = ([({}, {"A": 1}, False), ({"A": 1}, {"B": 1}, True), ({"B": 1}, {}, False), ({}, {"B": 1}, False), ({"A": 1}, {}, False)], ["A", "B"])
+
+
+def run(oracle_mod, net, seeds, **kw):
+    return oracle_mod.enumerate_pathways(net.S, net.reversible, net.internal, net.params, seeds, **kw)
+
+
+def test_steps_of_hand_traces(oracle_mod):
+    """P1: three expansions (A, B, C) build (1,1,1,1); P2: four (A, B, C, A again) build (1,2,1,2) -- SURVEY.md 8(c) P1 / P2
+    traces.  P5 with seeds {r0}, {r2}: (1,0,0,0,1) and (1,1,1,0,0) take 1 and 2 expansions from r0, (0,0,1,1,0) takes one
+    backward expansion from r2."""
+    r = run(oracle_mod, hand_network(*P1), [[0]])
+    assert r.flux.tolist() == [[1, 1, 1, 1]] and r.steps.tolist() == [3]
+    r = run(oracle_mod, hand_network(*P2), [[0]])
+    assert r.flux.tolist() == [[1, 2, 1, 2]] and r.steps.tolist() == [4]
+    r = run(oracle_mod, hand_network(*P5), [[0], [4]])
+    assert r.flux.tolist() == [[0, 0, 1, 1, 0], [1, 0, 0, 0, 1], [1, 1, 1, 0, 0]]
+    assert r.steps.tolist() == [1, 1, 2]
+
+
+def test_steps_take_the_quickest_construction(oracle_mod):
+    """Seeds {r0} and {r0, r4} of P5 both reach (1,0,0,0,1): in one expansion and in none (the seed set is balanced at
+    once); equal duplicates are one pathway and its step count is the smallest."""
+    r = run(oracle_mod, hand_network(*P5), [[0], [0, 8]])
+    rows = {tuple(v): s for v, s in zip(r.flux.tolist(), r.steps.tolist())}
+    assert rows[(1, 0, 0, 0, 1)] == 0 and rows[(1, 1, 1, 0, 0)] == 2
+
+
+def test_reaction_mask_by_hand(oracle_mod):
+    """8(f)-2 on P5 (r0: ->A, r1: A<=>B, r2: B->, r3: ->B, r4: A->), seed r0.  All reactions allowed: A first visited,
+    alternatives r1+ and r4 => (1,1,1,0,0) and (1,0,0,0,1).  Without r4: only the route through r1, r2.  Without r1:
+    only r4.  Without r1 and r4: A has no admissible alternative, a dead end.  The mask of exactly the reactions of
+    (1,1,1,0,0) constructs it in 2 expansions (the 'observability' question of PAPER.md:392-396)."""
+    net = hand_network(*P5)
+    full = run(oracle_mod, net, [[0]])
+    assert full.flux.tolist() == [[1, 0, 0, 0, 1], [1, 1, 1, 0, 0]]
+    same = run(oracle_mod, net, [[0]], allowed=np.ones(5, np.uint8))
+    assert same.flux.tolist() == full.flux.tolist() and same.stats == full.stats
+    r = run(oracle_mod, net, [[0]], allowed=np.array([1, 1, 1, 1, 0], np.uint8))
+    assert r.flux.tolist() == [[1, 1, 1, 0, 0]] and r.steps.tolist() == [2]
+    r = run(oracle_mod, net, [[0]], allowed=np.array([1, 0, 1, 1, 1], np.uint8))
+    assert r.flux.tolist() == [[1, 0, 0, 0, 1]] and r.steps.tolist() == [1]
+    r = run(oracle_mod, net, [[0]], allowed=np.array([1, 0, 1, 1, 0], np.uint8))
+    assert r.flux.tolist() == [] and r.stats["dead_end"] == 1 and r.stats["expanded"] == 1
+    r = run(oracle_mod, net, [[0]], allowed=np.array([1, 1, 1, 0, 0], np.uint8))
+    assert r.flux.tolist() == [[1, 1, 1, 0, 0]] and r.steps.tolist() == [2]
+    # the mask does not touch the seeds: a seed outside the subset still starts its pathway
+    r = run(oracle_mod, net, [[8]], allowed=np.array([1, 1, 1, 1, 0], np.uint8))
+    assert r.flux.tolist() == [[0, -1, 0, 1, 1], [1, 0, 0, 0, 1]]
+
+
+def test_mask_removes_exactly_the_pathways_through_masked_reactions_when_no_choice_depends_on_them(oracle_mod):
+    """Unimolecular networks (every node balances by choosing ONE alternative, no AND): masking reaction j can only
+    remove alternatives, so the result is the unmasked result minus the rows that use j."""
+    from netgen import unimolecular_network
+    for seed in range(6):
+        net = unimolecular_network(seed, m_int=5, n_rxn=9, n_rev=seed % 2)
+        seeds = oracle_mod.all_arc_seed_sets(net.reversible)
+        full = run(oracle_mod, net, seeds)
+        for j in range(net.S.shape[1]):
+            al = np.ones(net.S.shape[1], np.uint8); al[j] = 0
+            r = run(oracle_mod, net, [s for s in seeds if s[0] // 2 != j], allowed=al)
+            want = [row for row in full.flux.tolist() if row[j] == 0]
+            assert r.flux.tolist() == want, (seed, j)
+
+
+def test_sampled_choice_follows_the_written_generator(oracle_mod):
+    """One node with five outputs: candidate c must take alternative pick(seed, c, 0) mod 5 in ascending arc order."""
+    rx = [({}, {"A": 1}, False)] + [({"A": 1}, {}, False) for _ in range(5)]
+    net = hand_network(rx, ["A"])
+    for seed in (0, 1, 12345, M64):
+        r = run(oracle_mod, net, [[0]], sample_count=40, sample_seed=seed)
+        assert r.cand_end[:, 0].tolist() == [1] * 40 and r.cand_end[:, 1].tolist() == [1] * 40
+        used = sorted({1 + pick(seed, c, 0) % 5 for c in range(40)})
+        assert [int(np.nonzero(row[1:])[0][0]) + 1 for row in r.flux.tolist()] == sorted(used, reverse=True)
+    # the choice skips inadmissible alternatives: with r2 and r4 masked three remain, in arc order r1, r3, r5
+    al = np.array([1, 1, 0, 1, 0, 1], np.uint8)
+    r = run(oracle_mod, net, [[0]], sample_count=40, sample_seed=7, allowed=al)
+    used = {[1, 3, 5][pick(7, c, 0) % 3] for c in range(40)}
+    assert {int(np.nonzero(row[1:])[0][0]) + 1 for row in r.flux.tolist()} == used
+
+
+def _done_states(res):
+    return {tuple(sorted(e["flux"].items())) for lvl in res.trace for e in lvl if e["n_unb"] == 0}
+
+
+@pytest.mark.parametrize("name", ["toy", "P5"])
+def test_sampling_reaches_only_and_eventually_all_states_of_the_fan_out(oracle_mod, name):
+    """Theorem 1: every balanced state a sampled candidate reaches is a balanced state of the exhaustive
+    fan-out, and over enough generator seeds the union is the whole set (the lineage of a state fixes one choice per
+    visited metabolite, which some seed realises)."""
+    if name == "toy":
+        net = make_network("toy", 0)
+        seeds = None
+    else:
+        net = hand_network(*P5)
+        seeds = [[0], [4], [6]]
+    full = _done_states(run(oracle_mod, net, seeds, trace=2))
+    n_roots = run(oracle_mod, net, seeds).n_roots
+    got = set()
+    for s in range(400):
+        r = run(oracle_mod, net, seeds, trace=2, sample_count=n_roots, sample_seed=s)
+        st = _done_states(r)
+        assert st <= full
+        assert r.stats["children"] <= r.stats["expanded"]          # no fan-out: one child per expansion at most
+        got |= st
+        if got == full:
+            break
+    assert got == full
+
+
+def test_sampling_bookkeeping_and_order_independence(oracle_mod):
+    """Every candidate ends exactly once, the per-candidate records add up to the counters, and neither the thread count
+    nor the processing order changes anything (the generator is keyed on (candidate, metabolite), not on order)."""
+    net = make_network("small", 0)
+    a = oracle_mod.enumerate_network(net, sample_count=300, sample_seed=5)
+    codes = a.cand_end[:, 0]
+    assert a.n_roots == 300 and np.all(codes > 0)
+    st = a.stats
+    assert (codes == 1).sum() == st["done"] and (codes == 2).sum() == st["not_efm_maxloop"]
+    assert (codes == 3).sum() == st["dead_end"] and (codes == 4).sum() == st["discarded_visited"]
+    assert (codes == 5).sum() == st["discarded_nonpos"] and (codes == 6).sum() == st["discarded_overflow"]
+    assert st["peak_frontier"] <= 300 and st["truncated_beam"] == 0
+    # a candidate that ended Done after s expansions sits on level s
+    assert int(a.cand_end[codes == 1, 1].max()) < st["levels"]
+    b = oracle_mod.enumerate_network(net, sample_count=300, sample_seed=5, threads=3, shuffle_seed=99, frontier_cap=7)
+    assert np.array_equal(a.flux, b.flux) and a.stats == b.stats and np.array_equal(a.cand_end, b.cand_end)
+    c = oracle_mod.enumerate_network(net, sample_count=300, sample_seed=6)
+    assert not np.array_equal(a.cand_end, c.cand_end)
+    # candidate c starts from seed set c mod n_sets: with 8 default roots, candidates 3 and 11 share their seed arc
+    full = oracle_mod.enumerate_network(net)
+    assert full.n_roots >= 2
