@@ -67,6 +67,12 @@ typedef struct {
     int64_t max_child_tasks; /* 64-byte tasks per level (children on arcs of the support: every revisit, some     */
                             /* alternatives of a first visit); 0 = 4 * max_frontier + 65536 (max_child_keys with     */
                             /* EFM_F_NO_FASTPATH); EFM_E_CAPACITY when exceeded                                      */
+    int64_t sample_count;   /* SURVEY.md 8(f)-1 literal sampling mode ("each pathway is created using randomly */
+                            /* selected output/input"; "after attempting 48 EFM candidates"): C > 0 runs C     */
+                            /* candidate pathways; candidate c starts from seed set c mod n_sets and takes ONE admissible   */
+                            /* alternative per first visit (counter-based generator keyed on (sample_seed, c, metabolite),  */
+                            /* DESIGN.md reading G23); no fan-out, frontier_cap is ignored; needs C <= max_frontier         */
+    uint64_t sample_seed;
 } efm_params;
 
 typedef struct {
@@ -134,6 +140,13 @@ int efm_workspace_bytes(const efm_handle* h, size_t* bytes);
 int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_arc_code, int32_t n_sets,
                   void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* SURVEY.md 8(f)-2 targeted observability ("contributing reactions of each EFM were selected intentionally",
+ * PAPER.md:392-396): restrict the OR-alternatives to a subset of the reactions for the following efm_enumerate() calls.
+ *   allowed  host, uint8[n]; allowed[j] = 0 makes every alternative of reaction j (both directions) inadmissible;
+ *            NULL lifts the restriction.  Seed sets are the caller's choice and are not checked against the subset.
+ * Together with efm_result_steps() this answers whether, and in how many expansions, a known pathway is constructed. */
+int efm_set_reaction_mask(efm_handle* h, const uint8_t* allowed);
+
 /* The graph arrays are uploaded into the workspace by the first efm_enumerate() that sees a given workspace
  * pointer and are assumed resident afterwards (the network is an input that stays in HBM across calls).  A caller
  * that overwrites the workspace, or frees it and gets the same address back, must call this before the next run. */
@@ -151,6 +164,15 @@ int efm_result_copy(const efm_handle* h, int64_t* flux, int64_t capacity_rows);
  * efm_result_sparse_stride()), entries beyond nnz[r] are unspecified; rxn ascending within a row. */
 int efm_result_sparse_stride(const efm_handle* h, int32_t* row_capacity);
 int efm_result_copy_sparse(const efm_handle* h, int32_t* nnz, int32_t* rxn, int64_t* val, int64_t capacity_rows);
+
+/* Steps of every pathway to HOST memory (int32[count], same order as the rows): the number of expansions that built it,
+ * the smallest over its equal duplicates (the "steps" of PAPER.md:376-388, one metabolite per step, reading G12). */
+int efm_result_steps(const efm_handle* h, int32_t* steps, int64_t capacity_rows);
+
+/* Sampling mode: how every candidate ended, HOST int64[capacity]: code | steps << 8 with code 1 = balanced (Done),
+ * 2 = notEFM (MAX_LOOP), 3 = no admissible alternative, 4 = visited cap, 5 = non-positive flux (Prop 3),
+ * 6 = above the 2^62 guard; steps = expansions made.  *n_candidates receives C (0 outside sampling mode). */
+int efm_sample_ends(const efm_handle* h, int64_t* code_steps, int64_t capacity, int64_t* n_candidates);
 
 /* Compressed sparse rows to HOST memory (pinned memory makes the copies fast): row_ptr[count+1], then rxn / val with
  * efm_result_nnz() entries; row r occupies [row_ptr[r], row_ptr[r+1]), reactions ascending.  The copies are enqueued

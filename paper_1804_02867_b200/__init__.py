@@ -27,7 +27,8 @@ class efm_params(ctypes.Structure):
     _fields_ = [("max_support", ctypes.c_int32), ("max_loop", ctypes.c_int32), ("dep_depth", ctypes.c_int32),
                 ("max_visited", ctypes.c_int32), ("frontier_cap", ctypes.c_int64), ("max_frontier", ctypes.c_int64),
                 ("max_candidates", ctypes.c_int64), ("max_child_keys", ctypes.c_int64), ("device", ctypes.c_int32),
-                ("flags", ctypes.c_uint32), ("max_frontier_bytes", ctypes.c_int64), ("max_child_tasks", ctypes.c_int64)]
+                ("flags", ctypes.c_uint32), ("max_frontier_bytes", ctypes.c_int64), ("max_child_tasks", ctypes.c_int64),
+                ("sample_count", ctypes.c_int64), ("sample_seed", ctypes.c_uint64)]
 
 
 _STAT_INT = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxloop", "discarded_nonpos",
@@ -70,6 +71,9 @@ def load() -> ctypes.CDLL:
     lib.efm_workspace_bytes.argtypes = [vp, P(sz)]
     lib.efm_enumerate.argtypes = [vp, vp, vp, i32, vp, sz, vp]
     lib.efm_workspace_invalidate.argtypes = [vp]
+    lib.efm_set_reaction_mask.argtypes = [vp, vp]
+    lib.efm_result_steps.argtypes = [vp, vp, i64]
+    lib.efm_sample_ends.argtypes = [vp, vp, i64, P(i64)]
     lib.efm_result_count.argtypes = [vp, P(i64)]
     lib.efm_result_copy.argtypes = [vp, vp, i64]
     lib.efm_result_sparse_stride.argtypes = [vp, P(i32)]
@@ -98,9 +102,11 @@ def _ptr(a: Optional[np.ndarray]):
 @dataclass
 class Result:
     flux: Optional[np.ndarray]  # int64 [n_out, n], reaction space, coprime, strict lexicographic order
-    stats: Dict[str, float]
-    levels: Dict[str, np.ndarray]
-    n_out: int
+    steps: Optional[np.ndarray] = None      # int32 [n_out]: expansions that built each pathway
+    cand_end: Optional[np.ndarray] = None   # sampling mode: int64 [C, 2] (code, steps) per candidate
+    stats: Dict[str, float] = None
+    levels: Dict[str, np.ndarray] = None
+    n_out: int = 0
 
 
 class Enumerator:
@@ -122,7 +128,8 @@ class Enumerator:
                        int(params.get("max_visited", 0)), int(params.get("frontier_cap", 0)),
                        int(params.get("max_frontier", 0)), int(params.get("max_candidates", 0)),
                        int(params.get("max_child_keys", 0)), int(device), int(flags),
-                       int(params.get("max_frontier_bytes", 0)), int(params.get("max_child_tasks", 0)))
+                       int(params.get("max_frontier_bytes", 0)), int(params.get("max_child_tasks", 0)),
+                       int(params.get("sample_count", 0)), int(params.get("sample_seed", 0)) & ((1 << 64) - 1))
         self.device = int(device)
         self._check(self._lib.efm_create(_ptr(S), self.m, self.n, self.n, _ptr(rev), _ptr(internal), ctypes.byref(p),
                                          ctypes.byref(self._h)))
@@ -193,6 +200,14 @@ class Enumerator:
         self._check(self._lib.efm_enumerate(self._h, _ptr(ptr), _ptr(codes), n_sets, ctypes.c_void_p(d_workspace),
                                             ctypes.c_size_t(workspace_bytes), ctypes.c_void_p(stream)))
 
+    def set_reaction_mask(self, allowed: Optional[np.ndarray]) -> None:
+        """Restrict the OR-alternatives to the reactions with allowed[j] != 0 (None lifts the restriction)."""
+        if allowed is not None:
+            allowed = np.ascontiguousarray(allowed, dtype=np.uint8)
+            if allowed.shape != (self.n,):
+                raise ValueError("allowed must have n entries")
+        self._check(self._lib.efm_set_reaction_mask(self._h, _ptr(allowed)))
+
     def enumerate(self, seed_sets: Optional[Sequence[Sequence[int]]] = None, dense: bool = True) -> Result:
         """Allocate (once) the workspace with torch on ``cuda:device`` and run on torch's current stream."""
         import torch
@@ -214,7 +229,16 @@ class Enumerator:
         if dense:
             flux = np.zeros((k.value, self.n), dtype=np.int64)
             self._check(self._lib.efm_result_copy(self._h, _ptr(flux), k.value))
-        return Result(flux, self.stats(), self.level_stats(), int(k.value))
+        steps = np.zeros(k.value, dtype=np.int32)
+        self._check(self._lib.efm_result_steps(self._h, _ptr(steps), k.value))
+        nc = ctypes.c_int64()
+        self._check(self._lib.efm_sample_ends(self._h, None, 0, ctypes.byref(nc)))
+        cand_end = None
+        if nc.value:
+            raw = np.zeros(nc.value, dtype=np.int64)
+            self._check(self._lib.efm_sample_ends(self._h, _ptr(raw), nc.value, ctypes.byref(nc)))
+            cand_end = np.stack([raw & 0xff, raw >> 8], axis=1)
+        return Result(flux, steps, cand_end, self.stats(), self.level_stats(), int(k.value))
 
     def result_sparse(self):
         k = ctypes.c_int64()
@@ -258,13 +282,15 @@ class Enumerator:
                     children=arrs[3][: n.value])
 
 
-def enumerate_network(net, device: int = 0, flags: int = 0, seed_sets="net", dense: bool = True, **overrides) -> Result:
+def enumerate_network(net, device: int = 0, flags: int = 0, seed_sets="net", dense: bool = True, allowed=None, **overrides) -> Result:
     """Run the CUDA path on a ``netgen.Network`` with its own parameters (optionally overridden)."""
     params = dict(net.params)
     params.update(overrides)
     en = Enumerator(net.S, net.reversible, net.internal, params, device=device, flags=flags)
     try:
         seeds = net.seed_sets if isinstance(seed_sets, str) else seed_sets
+        if allowed is not None:
+            en.set_reaction_mask(allowed)
         return en.enumerate(seeds, dense=dense)
     finally:
         en.close()

@@ -23,6 +23,7 @@ struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
     Region col_ptr, col, colsig, node, in_e, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
+    Region amask, cand_end, c_steps, u_steps, r_steps;
     Region ctl, lvl, buf[2], off[2], plist, pprim, keys, tags, ckeys, tasks, surv, surv_dst, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill, vcount, vstart, vfill, tstart;
     Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, u_key, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
@@ -35,6 +36,8 @@ size_t pow2_at_least(size_t x) { size_t p = 1; while (p < x) p <<= 1; return p; 
 struct efm_handle {
     HostGraph G;
     int32_t D = 0, V = 0, max_loop = 8, L = 4;
+    int64_t sample_count = 0; uint64_t sample_seed = 0;
+    std::vector<uint32_t> amask;   // bit per arc, empty = no restriction (efm_set_reaction_mask)
     int64_t cap = 0, max_frontier = 0, max_cand = 0, max_keys = 0, max_tasks = 0, max_ckeys = 0, max_surv = 0, max_levels = 0;
     int32_t device = 0;
     uint32_t flags = 0;
@@ -83,6 +86,8 @@ void make_layout(efm_handle* h) {
     add_region(L, L.arc_rxn, sizeof(int) * (G.A + 1));
     add_region(L, L.arc_dir, sizeof(int) * (G.A + 1));
     add_region(L, L.arc_mix, sizeof(u64) * (G.A + 1));
+    add_region(L, L.amask, sizeof(u32) * ((G.A + 31) / 32 + 1));
+    add_region(L, L.cand_end, sizeof(u64) * (size_t)(h->sample_count + 1));
     add_region(L, L.ctl, sizeof(Ctl));
     add_region(L, L.lvl, sizeof(LevelStats) * (size_t)(h->max_levels + 2));
     add_region(L, L.buf[0], (size_t)h->frontier_bytes + 256);
@@ -103,6 +108,9 @@ void make_layout(efm_handle* h) {
     add_region(L, L.isrep, C + 1);
     add_region(L, L.poison, C + 1);
     add_region(L, L.uniq, C * 4);
+    add_region(L, L.c_steps, (C + 1) * 4);
+    add_region(L, L.u_steps, C * 4);
+    add_region(L, L.r_steps, C * 4);
     const size_t bins = (size_t)h->G.A + 2;   // per-arc and per-(arc, size) tables of the minimality filter
     const size_t gbins = (size_t)h->G.A * ((size_t)h->D + 1) + 2;
     add_region(L, L.freq, bins * 4);
@@ -231,7 +239,7 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     if (p) P = *p;
     if (P.max_support < 0 || P.max_loop < 0 || P.dep_depth < 0 || P.max_visited < 0 || P.frontier_cap < 0 ||
         P.max_frontier < 0 || P.max_candidates < 0 || P.max_child_keys < 0 || P.device < 0 || P.max_frontier_bytes < 0 ||
-        P.max_child_tasks < 0)
+        P.max_child_tasks < 0 || P.sample_count < 0)
         return EFM_E_INVAL;
     efm_handle* h = new (std::nothrow) efm_handle();
     if (!h) return EFM_E_NOMEM;
@@ -247,7 +255,8 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     h->V = P.max_visited ? P.max_visited : 2 * h->D;
     h->max_loop = P.max_loop ? P.max_loop : 8;
     if (h->D > 4096 || h->max_loop > 65535) { delete h; return EFM_E_INVAL; }
-    h->cap = P.frontier_cap;
+    h->cap = P.sample_count ? 0 : P.frontier_cap;   // a sampled candidate has one descendant at most: nothing to cut
+    h->sample_count = P.sample_count; h->sample_seed = P.sample_seed;
     h->device = P.device;
     h->flags = P.flags;
     const int Veff = std::min(h->V, std::max(G.M, 1));   // a pathway cannot visit more nodes than exist
@@ -257,6 +266,7 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     h->max_entry = entry_bytes((u32)h->D, (u32)Veff, (u32)Ueff);
     h->cand_stride = entry_bytes((u32)h->D, 0, 0);
     h->max_frontier = P.max_frontier ? P.max_frontier : (h->cap ? std::max<int64_t>(h->cap, 4096) : (int64_t)1 << 20);
+    if (h->sample_count > h->max_frontier) { if (P.max_frontier) { delete h; return EFM_E_INVAL; } h->max_frontier = h->sample_count; }
     if (h->max_frontier >= ((int64_t)1 << (64 - kAllocShift))) { delete h; return EFM_E_INVAL; }
     h->frontier_bytes = P.max_frontier_bytes ? ((P.max_frontier_bytes + 15) & ~(int64_t)15) : h->max_frontier * (int64_t)h->max_entry;
     if (h->frontier_bytes < (int64_t)h->max_entry) h->frontier_bytes = h->max_entry;
@@ -377,6 +387,11 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
             roots.push_back(arcs);
         }
     }
+    if (h->sample_count > 0 && !roots.empty()) {   // 8(f)-1: candidate c is a copy of seed set c mod (number of sets)
+        std::vector<std::vector<int>> cands((size_t)h->sample_count);
+        for (size_t c = 0; c < cands.size(); ++c) cands[c] = roots[c % roots.size()];
+        roots.swap(cands);
+    }
     const u64 n_roots = roots.size();
     if ((int64_t)n_roots > h->max_frontier || (int64_t)n_roots > h->max_keys) return EFM_E_CAPACITY;
     // seed sets as CSR of arc ids + the offset of every root entry in the staging buffer (16-byte units); the
@@ -459,12 +474,14 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         CK(up(ws + L.arc_mix.off, arc_mix.data(), sizeof(u64) * arc_mix.size()));
         h->graph_ws = ws;
     }
+    if (!h->amask.empty()) CK(up(ws + L.amask.off, h->amask.data(), sizeof(uint32_t) * h->amask.size()));   // a few hundred bytes
     // the seed sets travel in regions that are unused until the first level is ordered / expanded
     CK(up(ws + L.plist.off, h_seed_ptr.data(), sizeof(int) * h_seed_ptr.size()));
     CK(up(ws + L.tags.off, h_seed_arc.data(), sizeof(int) * h_seed_arc.size()));
     CK(up(ws + L.off[1].off, stage_off.data(), sizeof(u64) * stage_off.size()));
     CK(cudaMemsetAsync(ws + L.ctl.off, 0, sizeof(Ctl), s));
     CK(cudaMemsetAsync(ws + L.lvl.off, 0, sizeof(LevelStats) * 2, s));
+    if (h->sample_count > 0) CK(cudaMemsetAsync(ws + L.cand_end.off, 0, sizeof(u64) * (size_t)(h->sample_count + 1), s));
     CK(cudaStreamSynchronize(s));   // the host staging vectors above go out of scope later; keep it simple
     int host_syncs = 1;
 
@@ -491,6 +508,9 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     ea.cap = (u64)h->cap;
     ea.D = h->D; ea.V = h->V; ea.max_loop = h->max_loop;
     ea.no_fast = (h->flags & EFM_F_NO_FASTPATH) ? 1 : 0;
+    ea.sample = h->sample_count > 0 ? 1u : 0u; ea.sample_seed = h->sample_seed;
+    ea.amask = h->amask.empty() ? nullptr : (const u32*)(ws + L.amask.off);
+    ea.cand_end = h->sample_count > 0 ? (u64*)(ws + L.cand_end.off) : nullptr;
     expand_smem_layout(ea);
     ea.force_inplace = (h->flags & EFM_F_NO_STAGING) ? 1 : 0;
 
@@ -517,6 +537,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         ra.stage_off = (const u64*)(ws + L.off[1].off); ra.stage = ws + L.buf[1].off;
         ra.nxt = ws + L.buf[0].off; ra.nxt_off = (u64*)(ws + L.off[0].off);
         ra.cand = ea.cand; ra.cand_stride = h->cand_stride; ra.keys = ea.keys;
+        ra.cand_end = ea.cand_end;
         ra.max_frontier = ea.max_frontier; ra.frontier_units = ea.frontier_units; ra.max_cand = ea.max_cand; ra.cap = ea.cap;
         size_t t0 = tm.mark();
         CK(launch_roots(false, ra, s)); ++launches;
@@ -588,6 +609,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     pa.cand = ws + L.cand.off; pa.cand_stride = h->cand_stride; pa.max_cand = (u64)h->max_cand;
     pa.table = (u32*)(ws + L.table.off); pa.table_size = h->table_size;
     pa.isrep = ws + L.isrep.off; pa.poison = ws + L.poison.off; pa.uniq = (u32*)(ws + L.uniq.off);
+    pa.c_steps = (u32*)(ws + L.c_steps.off); pa.u_steps = (int*)(ws + L.u_steps.off); pa.r_steps = (int*)(ws + L.r_steps.off);
     pa.freq = (u32*)(ws + L.freq.off); pa.gcount = (u32*)(ws + L.gcount.off);
     pa.gstart = (u32*)(ws + L.gstart.off); pa.gfill = (u32*)(ws + L.gfill.off);
     // the join's row lists and row-order signatures live in regions the output stage fills only afterwards
@@ -664,6 +686,43 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     h->n_out = (int64_t)n_keep;
     h->csr_nnz = n_keep ? (int64_t)hc->csr_nnz : 0;
     h->have_result = true;
+    return EFM_OK;
+}
+
+int efm_set_reaction_mask(efm_handle* h, const uint8_t* allowed) {
+    if (!h) return EFM_E_INVAL;
+    h->amask.clear();
+    if (allowed) {
+        h->amask.assign((size_t)(h->G.A + 31) / 32 + 1, 0u);
+        for (int a = 0; a < h->G.A; ++a)
+            if (allowed[h->G.arc_rxn[a]]) h->amask[(size_t)a >> 5] |= 1u << (a & 31);
+    }
+    return EFM_OK;
+}
+
+int efm_result_steps(const efm_handle* hc, int32_t* steps, int64_t capacity_rows) {
+    efm_handle* h = const_cast<efm_handle*>(hc);
+    if (!h || (!steps && capacity_rows > 0)) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    if (capacity_rows < h->n_out) return EFM_E_INVAL;
+    if (h->n_out == 0) return EFM_OK;
+    ON_DEVICE(h);
+    CK(cudaMemcpyAsync(steps, h->ws + h->lay.r_steps.off, (size_t)h->n_out * 4, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return EFM_OK;
+}
+
+int efm_sample_ends(const efm_handle* hc, int64_t* code_steps, int64_t capacity, int64_t* n_candidates) {
+    efm_handle* h = const_cast<efm_handle*>(hc);
+    if (!h || !n_candidates || capacity < 0 || (capacity > 0 && !code_steps)) return EFM_E_INVAL;
+    if (!h->have_result) return EFM_E_STATE;
+    const int64_t n = h->sample_count > 0 ? (int64_t)h->stats.n_roots : 0;
+    *n_candidates = n;
+    const int64_t c = std::min(n, capacity);
+    if (c == 0) return EFM_OK;
+    ON_DEVICE(h);
+    CK(cudaMemcpyAsync(code_steps, h->ws + h->lay.cand_end.off, (size_t)c * 8, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
     return EFM_OK;
 }
 

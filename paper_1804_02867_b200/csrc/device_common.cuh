@@ -16,10 +16,12 @@ typedef unsigned short u16;
 // Entry format in HBM.  Frontier entries are PACKED back to back (16-byte aligned); entry
 // indices and 16-byte units come from ONE packed atomic, so entries with consecutive indices are contiguous and the
 // size of entry p is off[p + 1] - off[p].  An entry is
-//   [ 0,48)  header: u32 n_supp | n_vis << 16; u32 n_unb; u64 hs = sum of the arc terms of the state hash;
+//   [ 0,48)  header: u32 n_supp | n_vis << 16; u32 n_unb | ones << 16 (ones = number of fluxes equal to 1);
+//            u64 hs = sum of the arc terms of the state hash;
 //            u64 hv = sum of its visited terms; u64 big = max(largest flux, largest |EF|);
 //            i64 E = EF of i*; u32 i* | (vk + 1) << 16 (i* = lowest unbalanced metabolite, reading G12; vk = index of
-//            its visited record, vk + 1 = 0: first visit); u32 number of fluxes equal to 1
+//            its visited record, vk + 1 = 0: first visit); u32 root / sampled candidate the pathway descends from
+//            (candidate slots: the number of expansions that built the pathway)
 //   i64  flux[n_supp]   fluxes of the support arcs, > 0, gcd 1
 //   u64  vis[n_vis]     visited records: cnt << 48 | met << 32 | PI << 16 | PO   (unordered)
 //   i64  ef[n_unb]      the non-zero extra fluxes EF_i (Eq 2) of the state   (unordered)
@@ -124,6 +126,10 @@ struct ExpandArgs {
     u64 max_frontier, frontier_units, max_cand, max_keys, max_tasks, max_surv, max_levels;
     u64 cap;                    // beam: entries kept per level, 0 = unbounded
     int D, V, max_loop;
+    // SURVEY.md 8(f)-1 literal sampling (one alternative per first visit, chosen by sample_pick) and 8(f)-2 reaction mask
+    u64 sample_seed; u32 sample; // sample != 0: sampling mode
+    const u32* amask;           // bit per arc: its reaction is in the allowed subset (nullptr: all)
+    u64* cand_end;              // sampling mode: per candidate how and when it ended (END_* | steps << 8)
     int force_inplace;          // EFM_F_NO_STAGING: read every parent in place
     int no_fast;                // EFM_F_NO_FASTPATH: every child through the warp-cooperative general routine
     // shared-memory carve-up per warp (bytes)
@@ -144,6 +150,7 @@ struct RootArgs {
     u64 n_roots;
     u32 cand_stride;
     u64 max_frontier, frontier_units, max_cand, cap;
+    u64* cand_end;
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -166,6 +173,13 @@ __host__ __device__ inline u64 vis_pack(u32 met, u32 PI, u32 PO, u32 cnt) {
 }
 __host__ __device__ inline u64 beam_key(u32 n_unb, u64 h) { return ((u64)(n_unb > 255u ? 255u : n_unb) << 56) | (h >> 8); }
 
+// how a sampled candidate ended, code | steps << 8
+enum { END_NONE = 0, END_DONE = 1, END_NOTEFM = 2, END_DEAD = 3, END_VISITED = 4, END_NONPOS = 5, END_OVERFLOW = 6 };
+// alternative candidate c takes at the first visit of metabolite i (reading G23, written here independently of oracle/):
+//   pick(seed, c, i) = mix( mix(seed + 0x9E3779B97F4A7C15 * (c + 1)) ^ (0x04 << 56 | i) ), index = pick mod (admissible alternatives)
+__host__ __device__ inline u64 sample_pick(u64 seed, u32 cand, u32 met) {
+    return mix64(mix64(seed + 0x9E3779B97F4A7C15ULL * ((u64)cand + 1ULL)) ^ (0x0400000000000000ULL | (u64)met));
+}
 constexpr u64 kKeyDone = ~0ULL - 1ULL;   // key slot of a balanced child: always materialised, outside the beam ranking
 enum { TF_NEG = 1, TF_FIRST = 2, TF_INSUPP = 4 };   // task flags: bump subtracts (Eq 5); first visit; arc already in the support
 // child tag: [63:34] parent-list index, [33:32] kind, [31:0] payload

@@ -289,18 +289,19 @@ struct WarpAcc { u32 children, done, general; };   // warp-uniform counters kept
 // Header of an entry (three 16-byte words) decoded into registers.
 struct Hdr {
     int ns, nv, nu, istar, vk, ones;
+    u32 cand;
     u64 hs, hv, big;
     i64 E;
 };
 __device__ __forceinline__ Hdr decode_hdr(const uint4 h0, const uint4 h1, const uint4 h2) {
     Hdr H;
-    H.ns = (int)(h0.x & 0xffffu); H.nv = (int)(h0.x >> 16); H.nu = (int)h0.y;
+    H.ns = (int)(h0.x & 0xffffu); H.nv = (int)(h0.x >> 16); H.nu = (int)(h0.y & 0xffffu); H.ones = (int)(h0.y >> 16);
     H.hs = (u64)h0.z | ((u64)h0.w << 32);
     H.hv = (u64)h1.x | ((u64)h1.y << 32);
     H.big = (u64)h1.z | ((u64)h1.w << 32);
     H.E = (i64)((u64)h2.x | ((u64)h2.y << 32));
     H.istar = (int)(h2.z & 0xffffu); H.vk = (int)(h2.z >> 16) - 1;
-    H.ones = (int)h2.w;
+    H.cand = h2.w;
     return H;
 }
 __device__ __forceinline__ void write_task(const ExpandArgs& A, u64 ti, int ca, int cia, int cnu, u32 flags, u64 ck, u64 cd, u64 cT, u64 cg,
@@ -355,7 +356,7 @@ __device__ __forceinline__ void expand_revisits(const ExpandArgs& A, LevelCtl* l
         bool act = live;
         if (live && cntv > A.max_loop) {
             act = false;
-            if (gl == 0) atomicAdd(&ctl->st[ST_NOT_EFM], 1ULL);
+            if (gl == 0) { atomicAdd(&ctl->st[ST_NOT_EFM], 1ULL); if (A.cand_end) A.cand_end[H.cand] = END_NOTEFM | ((u64)A.level << 8); }
         }
         const int PI = (int)((rec >> 16) & 0xffffu), PO = (int)(rec & 0xffffu);
         // position and coefficient of PI in I[i*] and of PO in O[i*]: from the columns of the two arcs
@@ -461,7 +462,10 @@ __device__ __forceinline__ void expand_revisits(const ExpandArgs& A, LevelCtl* l
             else cnu = nu + __reduce_add_sync(gmask, delta);
         }
         if (act && status != CH_OK) {
-            if (gl == 0) atomicAdd(&ctl->st[status == CH_OVERFLOW ? ST_OVERFLOW : ST_NONPOS], 1ULL);
+            if (gl == 0) {
+                atomicAdd(&ctl->st[status == CH_OVERFLOW ? ST_OVERFLOW : ST_NONPOS], 1ULL);
+                if (A.cand_end) A.cand_end[H.cand] = (status == CH_OVERFLOW ? END_OVERFLOW : END_NONPOS) | ((u64)A.level << 8);
+            }
             act = false;
         }
         // gcd normalisation (reading G10): g = gcd(T, k f_t for t != a)
@@ -570,7 +574,7 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
         auto ef_of = [&](int met) -> i64 { const u32 u = upos[met]; return u ? ef[u - 1] : 0; };
         int n_adm = 0;
         if (nv >= A.V) {
-            if (lane == 0) atomicAdd(&ctl->st[ST_VISITED], 1ULL);
+            if (lane == 0) { atomicAdd(&ctl->st[ST_VISITED], 1ULL); if (A.cand_end) A.cand_end[H.cand] = END_VISITED | ((u64)A.level << 8); }
         } else {
             // primary on the side the flux arrives from: lowest arc of that side in the support (G13)
             int prim = -1;
@@ -587,6 +591,22 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
             // visited record of i* without the chosen arc (PI = primary / chosen arc, PO = chosen arc / primary)
             const u64 vbase = vis_pack((u32)istar, fwd ? (u32)prim : 0u, fwd ? 0u : (u32)prim, 0u);
             const int ashift = fwd ? 0 : 16;
+            auto admissible = [&](u32 a, u32 tw, bool insup) -> bool {   // readings G14, G15 and the reaction mask of 8(f)-2
+                return !(tw != 0xffffu && sbit(sbits, (int)tw)) && (insup || ns < A.D) && (!A.amask || ((__ldg(&A.amask[a >> 5]) >> (a & 31)) & 1u));
+            };
+            // 8(f)-1 sampling: count the admissible alternatives, then take exactly one of them
+            int pick_idx = -1, seen = 0;
+            if (A.sample) {
+                int tot = 0;
+#pragma unroll 1
+                for (int base = 0; base < alen; base += 32) {
+                    const int q = base + lane;
+                    bool ad = false;
+                    if (q < alen) { const uint4 r = __ldg(&altl[2 * q]); const u32 a = r.x & 0xffffu; ad = admissible(a, r.y & 0xffffu, sbit(sbits, (int)a)); }
+                    tot += __popc(__ballot_sync(FULL, ad));
+                }
+                if (tot > 0) pick_idx = (int)(sample_pick(A.sample_seed, H.cand, (u32)istar) % (u64)tot);
+            }
 #pragma unroll 1
             for (int base = 0; base < alen; base += 32) {
                 const int q = base + lane;
@@ -600,11 +620,19 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
                     generic = (r0.y >> 24) & 1u;
                     if (__builtin_expect(generic, 0)) c = __ldg(&alist[q]).y;   // the coefficient may not fit the record
                     insup = sbit(sbits, a);
-                    adm = !(tw != 0xffffu && sbit(sbits, (int)tw)) && (insup || ns < A.D);
+                    adm = admissible((u32)a, tw, insup);
                 }
-                const u32 adm_m = __ballot_sync(FULL, adm);
+                u32 adm_m = __ballot_sync(FULL, adm);
                 if (adm_m == 0) continue;
                 n_adm += __popc(adm_m);
+                if (A.sample) {   // only the sampled alternative goes on
+                    const int here = __popc(adm_m);
+                    const int sel = (pick_idx >= seen && pick_idx < seen + here) ? (int)__fns(adm_m, 0, pick_idx - seen + 1) : -1;
+                    seen += here;
+                    adm = adm && lane == sel;
+                    adm_m = sel >= 0 ? 1u << sel : 0u;
+                    if (adm_m == 0) continue;
+                }
                 // ---- lane-parallel evaluation: new arc, small integers => no overflow, no common factor
                 const bool fast = adm && !insup && fastP && !generic;
                 const u32 fast_m = __ballot_sync(FULL, fast);
@@ -706,7 +734,7 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
                         cnu = nu + __reduce_add_sync(FULL, delta);
                     }
                     if (__builtin_expect(ovf, 0)) {
-                        if (lane == 0) atomicAdd(&ctl->st[ST_OVERFLOW], 1ULL);
+                        if (lane == 0) { atomicAdd(&ctl->st[ST_OVERFLOW], 1ULL); if (A.cand_end) A.cand_end[H.cand] = END_OVERFLOW | ((u64)A.level << 8); }
                         continue;
                     }
                     // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and
@@ -739,7 +767,10 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
                     }
                 }
             }
-            if (n_adm == 0 && lane == 0) atomicAdd(&ctl->st[ST_DEAD_END], 1ULL);   // no admissible alternative
+            if (n_adm == 0 && lane == 0) {   // no admissible alternative
+                atomicAdd(&ctl->st[ST_DEAD_END], 1ULL);
+                if (A.cand_end) A.cand_end[H.cand] = END_DEAD | ((u64)A.level << 8);
+            }
         }
         // ---- restore the shared tables to zero for the next parent
         __syncwarp();
@@ -1116,9 +1147,11 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
     mx = g_max(gmask, mx);
     if (lane == 0) {
         uint4* h4 = (uint4*)dst;
-        h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2, (u32)chs, (u32)(chs >> 32));
+        h4[0] = make_uint4((u32)n2 | ((u32)nv2 << 16), (u32)nu2 | ((u32)min(ones, 0xffff) << 16), (u32)chs, (u32)(chs >> 32));
         h4[1] = make_uint4((u32)chv, (u32)(chv >> 32), (u32)mx, (u32)(mx >> 32));
-        h4[2] = make_uint4((u32)(u64)bestE, (u32)((u64)bestE >> 32), to_cand ? 0u : ((best >> 16) | ((u32)(vk2 + 1) << 16)), (u32)ones);
+        h4[2] = make_uint4((u32)(u64)bestE, (u32)((u64)bestE >> 32), to_cand ? 0u : ((best >> 16) | ((u32)(vk2 + 1) << 16)),
+                          to_cand ? A.level + 1u : P.cand);   // a balanced pathway keeps its step count, an active one its origin
+        if (to_cand && A.cand_end) A.cand_end[P.cand] = END_DONE | ((u64)(A.level + 1u) << 8);
     }
     }   // ok
     }
@@ -1145,7 +1178,7 @@ __global__ void __launch_bounds__(128) k_roots(const RootArgs R) {
         const u64 key = R.keys[r];
         const bool notrunc = R.cap == 0 || lv->n_keys <= R.cap;
         if (key == kKeySentinel || !(notrunc || key < ctl->X)) return;
-        const u32 w0 = *(const u32*)e, nu = ((const u32*)e)[1];
+        const u32 w0 = *(const u32*)e, nu = ((const u32*)e)[1] & 0xffffu;
         const u64 units = entry_bytes(w0 & 0xffffu, w0 >> 16, nu) >> 4;
         const u64 old = atomicAdd(&ctl->lv[0].alloc, (1ULL << kAllocShift) | units);
         const u64 slot = old >> kAllocShift, off = old & kAllocUnitMask;
@@ -1191,12 +1224,14 @@ __global__ void __launch_bounds__(128) k_roots(const RootArgs R) {
                 if (met < istar) { istar = met; E = s; }   // lowest unbalanced metabolite (reading G12)
             }
         }
-    ((u32*)e)[0] = (u32)ns; ((u32*)e)[1] = (u32)nu;
+    ((u32*)e)[0] = (u32)ns; ((u32*)e)[1] = (u32)nu | ((u32)ns << 16);   // every flux is 1
     ((u64*)e)[1] = hs; ((u64*)e)[2] = 0; ((u64*)e)[3] = big;
-    ((u64*)e)[4] = (u64)E; ((u32*)e)[10] = nu ? istar : 0u; ((u32*)e)[11] = (u32)ns;   // no visited record yet: first visit; every flux is 1
+    ((u64*)e)[4] = (u64)E; ((u32*)e)[10] = nu ? istar : 0u;   // no visited record yet: first visit
+    ((u32*)e)[11] = nu ? (u32)r : 0u;   // origin of the pathway; a root that is balanced at once took 0 expansions
     if (nu == 0) {   // balanced at once (arbiter "Done")
         R.keys[r] = kKeySentinel;
         atomicAdd(&lv->n_done, 1ULL);
+        if (R.cand_end) R.cand_end[r] = END_DONE;
         const u64 slot = atomicAdd(&ctl->n_cand, 1ULL);
         if (slot >= R.max_cand) { atomicOr(&ctl->error, (u32)ERR_CAND); return; }
         unsigned char* dst = R.cand + slot * R.cand_stride;

@@ -21,6 +21,7 @@ struct PostArgs {
     const unsigned char* cand; u32 cand_stride; u64 max_cand;
     u32* table; u64 table_size;        // open-addressing support hash (a-6), power of two
     unsigned char* isrep; unsigned char* poison;
+    u32* c_steps;                      // per candidate: expansions that built it; a representative ends with the minimum over its equal duplicates
     u32* uniq;                         // candidate ids of the unique, unpoisoned supports
     // minimality filter (a-7)
     u32* freq; u32* gcount; u32* gstart; u32* gfill;      // per arc: candidates using it, group size / start / fill
@@ -31,6 +32,7 @@ struct PostArgs {
     // canonical output (a-8)
     int D; int n_rxn;
     int* u_nnz; int* u_rxn; i64* u_val;   // unsorted reaction-space rows
+    int* u_steps; int* r_steps;            // step count of every row (unsorted / final order)
     ulonglong2* u_key;                     // order codes of the first two entries of every unsorted row
     u32* sort_idx; u64 n_pad;
     int* r_nnz; int* r_rxn; i64* r_val;   // final, lexicographic order

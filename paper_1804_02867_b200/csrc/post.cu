@@ -173,6 +173,8 @@ __global__ void __launch_bounds__(256) k_dedup_insert(const PostArgs a, u64 n_ca
     const int n = cand_n(e);
     const u16* arc = cand_arc(e, n);
     const i64* f = cand_flux(e);
+    const u32 own_steps = ((const u32*)e)[11];
+    atomicMin(&a.c_steps[i], own_steps);
     u64 h = 0;
     for (int t = 0; t < n; ++t) h += mix64(0x0300000000000000ULL | (u64)arc[t]);
     u64 slot = mix64(h) & (a.table_size - 1);
@@ -190,6 +192,7 @@ __global__ void __launch_bounds__(256) k_dedup_insert(const PostArgs a, u64 n_ca
                 bool eq = true;
                 for (int t = 0; t < n && eq; ++t) eq = f[t] == of[t];
                 if (!eq) a.poison[prev] = 1;
+                else atomicMin(&a.c_steps[prev], own_steps);   // equal duplicates are one pathway: its quickest construction counts
                 return;
             }
         }
@@ -211,6 +214,7 @@ cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_l
     if ((e = cudaMemsetAsync(a.table, 0xFF, a.table_size * sizeof(u32), s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(a.isrep, 0, n_cand + 1, s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(a.poison, 0, n_cand + 1, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(a.c_steps, 0xFF, (n_cand + 1) * sizeof(u32), s)) != cudaSuccess) return e;
     if (n_cand == 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((n_cand + 255) / 256);
     k_dedup_insert<<<blocks, 256, 0, s>>>(a, n_cand);
@@ -486,7 +490,7 @@ __global__ void __launch_bounds__(256) k_out_rows(const PostArgs a, u64 K) {   /
     const int n = cand_n(e);
     const u16* arc = cand_arc(e, n);
     const i64* f = cand_flux(e);
-    if (lane == 0) a.u_nnz[r] = n;
+    if (lane == 0) { a.u_nnz[r] = n; a.u_steps[r] = (int)a.c_steps[a.uniq[p]]; }
     int j01 = 0; i64 v01 = 0;   // lanes 0 and 1 keep the first two entries for the order codes
     for (int t = lane; t < n; t += 32) {   // arcs ascend => reactions ascend (twins never share a support)
         const int j = a.g.arc_rxn[arc[t]];
@@ -572,7 +576,7 @@ __global__ void __launch_bounds__(256) k_out_gather(const PostArgs a, u64 n_keep
     const int lane = threadIdx.x & 31;
     const u32 src = a.sort_idx[r];
     const int n = a.u_nnz[src];
-    if (lane == 0) a.r_nnz[r] = n;
+    if (lane == 0) { a.r_nnz[r] = n; a.r_steps[r] = a.u_steps[src]; }
     for (int t = lane; t < n; t += 32) { a.r_rxn[r * a.D + t] = a.u_rxn[(u64)src * a.D + t]; a.r_val[r * a.D + t] = a.u_val[(u64)src * a.D + t]; }
 }
 

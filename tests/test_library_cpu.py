@@ -37,7 +37,7 @@ def test_struct_sizes_match_header(lib_mod, tmp_path):
     exe = tmp_path / "sz"
     subprocess.run(["gcc", "-I", os.path.dirname(lib_mod.HEADER_PATH), str(src), "-o", str(exe)], check=True)
     c_params, c_stats = (int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split())
-    assert ctypes.sizeof(lib_mod.efm_params) == c_params == 72
+    assert ctypes.sizeof(lib_mod.efm_params) == c_params == 88
     assert ctypes.sizeof(lib_mod.efm_stats) == c_stats
 
 

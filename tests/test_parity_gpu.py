@@ -32,10 +32,11 @@ def _threads(oracle_mod):
     return max(1, min(oracle_mod.max_threads(), os.cpu_count() or 1, 64))
 
 
-def assert_parity(efm, oracle_mod, net, seeds="net", flags=0, check_levels=True, **over):
-    got = efm.enumerate_network(net, seed_sets=seeds, flags=flags, **over)
-    okeys = {k: v for k, v in over.items() if k in ("max_support", "max_loop", "dep_depth", "max_visited", "frontier_cap")}
-    ref = oracle_mod.enumerate_network(net, threads=_threads(oracle_mod), seed_sets=seeds, self_check=False, **okeys)
+def assert_parity(efm, oracle_mod, net, seeds="net", flags=0, check_levels=True, allowed=None, **over):
+    got = efm.enumerate_network(net, seed_sets=seeds, flags=flags, allowed=allowed, **over)
+    okeys = {k: v for k, v in over.items() if k in ("max_support", "max_loop", "dep_depth", "max_visited", "frontier_cap",
+                                                    "sample_count", "sample_seed")}
+    ref = oracle_mod.enumerate_network(net, threads=_threads(oracle_mod), seed_sets=seeds, self_check=False, allowed=allowed, **okeys)
     for k in STAT_KEYS:
         assert int(got.stats[k]) == int(ref.stats[k]), (k, got.stats[k], ref.stats[k])
     if check_levels:
@@ -43,7 +44,10 @@ def assert_parity(efm, oracle_mod, net, seeds="net", flags=0, check_levels=True,
             assert np.array_equal(got.levels[k], ref.levels[k]), k
     assert got.flux.shape == ref.flux.shape
     assert np.array_equal(got.flux, ref.flux)
+    assert np.array_equal(got.steps, ref.steps)          # expansions that built every pathway
     assert int(got.stats["n_roots"]) == ref.n_roots
+    if over.get("sample_count"):
+        assert np.array_equal(got.cand_end, ref.cand_end)   # how and when every sampled candidate ended
     return got, ref
 
 
@@ -368,3 +372,64 @@ def test_bench_configuration_properties(efm):
     for k in STAT_KEYS:
         assert int(again.stats[k]) == int(st[k]), k
     en.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f)-1 literal sampling mode and 8(f)-2 reaction mask
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,count,seed,over", [("toy", 48, 1, {}), ("small", 300, 5, {}), ("small", 7, 0, {}), ("core", 5000, 2, {}),
+                                                  ("mid", 20000, 3, {}), ("genome", 30000, 4, {}),
+                                                  ("genome", 2000, 9, dict(max_loop=2, max_visited=30))])
+def test_sampling_mode(efm, oracle_mod, name, count, seed, over):
+    """C candidate pathways, one sampled alternative per first visit: same pathways, same counters, and
+    the same end (code, steps) of every single candidate as the oracle."""
+    net = make_network(name, 0)
+    got, ref = assert_parity(efm, oracle_mod, net, sample_count=count, sample_seed=seed, **over)
+    assert got.cand_end.shape == (count, 2) and np.all(got.cand_end[:, 0] > 0)
+    assert int(got.stats["children"]) <= int(got.stats["expanded"]) and int(got.stats["truncated_beam"]) == 0
+    if name != "toy":
+        assert len(set(got.cand_end[:, 0].tolist())) >= 3   # several kinds of ends occur
+
+
+def test_sampling_mode_with_multi_arc_seed_sets_and_the_general_routine(efm, oracle_mod):
+    net = make_network("core", 0)
+    seeds = random_seed_sets(net, 64, 2, 3)
+    assert_parity(efm, oracle_mod, net, seeds=seeds, sample_count=4000, sample_seed=11)
+    assert_parity(efm, oracle_mod, net, seeds=seeds, sample_count=4000, sample_seed=11, flags=efm.EFM_F_NO_FASTPATH)
+
+
+def test_reaction_mask_by_hand(efm):
+    """P5 network (r0: ->A, r1: A<=>B, r2: B->, r3: ->B, r4: A->), seed r0, derived by hand (tests/test_oracle_modes.py has the
+    derivation): no oracle involved."""
+    net = hand_network([({}, {"A": 1}, False), ({"A": 1}, {"B": 1}, True), ({"B": 1}, {}, False), ({}, {"B": 1}, False),
+                        ({"A": 1}, {}, False)], ["A", "B"])
+    en = efm.Enumerator(net.S, net.reversible, net.internal, net.params)
+    r = en.enumerate([[0]])
+    assert r.flux.tolist() == [[1, 0, 0, 0, 1], [1, 1, 1, 0, 0]] and r.steps.tolist() == [1, 2]
+    en.set_reaction_mask(np.array([1, 1, 1, 1, 0], np.uint8))
+    r = en.enumerate([[0]])
+    assert r.flux.tolist() == [[1, 1, 1, 0, 0]] and r.steps.tolist() == [2]
+    en.set_reaction_mask(np.array([1, 0, 1, 1, 0], np.uint8))
+    r = en.enumerate([[0]])
+    assert r.flux.tolist() == [] and r.stats["dead_end"] == 1
+    en.set_reaction_mask(None)
+    r = en.enumerate([[0], [0, 8]])
+    assert r.flux.tolist() == [[1, 0, 0, 0, 1], [1, 1, 1, 0, 0]] and r.steps.tolist() == [0, 2]   # quickest construction counts
+    en.close()
+
+
+@pytest.mark.parametrize("name,over", [("small", {}), ("core", dict(frontier_cap=4096)), ("genome", dict(frontier_cap=2048))])
+def test_reaction_mask(efm, oracle_mod, name, over):
+    """Random subsets of the reactions (8(f)-2): the restricted traversal agrees with the oracle, and the subset made of
+    the reactions of one known output reconstructs that pathway."""
+    net = make_network(name, 0)
+    rng = np.random.default_rng(7)
+    n = net.S.shape[1]
+    for keep in (0.9, 0.6):
+        allowed = (rng.random(n) < keep).astype(np.uint8)
+        assert_parity(efm, oracle_mod, net, allowed=allowed, **over)
+    full = efm.enumerate_network(net, **over)
+    row = full.flux[len(full.flux) // 2]
+    allowed = (row != 0).astype(np.uint8)
+    got, ref = assert_parity(efm, oracle_mod, net, allowed=allowed, **over)
+    assert any(np.array_equal(row, r) for r in got.flux)
