@@ -23,7 +23,7 @@ struct Region { size_t off = 0, bytes = 0; };
 
 struct Layout {
     Region col_ptr, col, colsig, node, in_e, out_e, in_alt, out_alt, twin, dep_off, dep_bits, arc_rxn, arc_dir, arc_mix;
-    Region amask, cand_end, c_steps, u_steps, r_steps;
+    Region amask, cand_end, c_steps, u_steps, r_steps, g_sig64, r_sig64;
     Region ctl, lvl, buf[2], off[2], plist, pprim, keys, tags, ckeys, tasks, surv, surv_dst, cand, table, isrep, poison, uniq, freq, gcount, gstart, gfill, vcount, vstart, vfill, tstart;
     Region g_row, g_sig, g_size, keep, u_nnz, u_rxn, u_val, u_key, sort_idx, r_nnz, r_rxn, r_val, csr_ptr, dense;
     size_t total = 0;
@@ -123,6 +123,8 @@ void make_layout(efm_handle* h) {
     add_region(L, L.tstart, bins * 4);
     add_region(L, L.g_row, C * 4);
     add_region(L, L.g_sig, C * 16);
+    add_region(L, L.g_sig64, C * 8 + 16);
+    add_region(L, L.r_sig64, C * 8 + 16);
     add_region(L, L.g_size, C * 2);
     add_region(L, L.keep, C);
     add_region(L, L.u_nnz, C * 4);
@@ -616,6 +618,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     pa.v_row = (u32*)(ws + L.u_rxn.off); pa.r_sig = (uint4*)(ws + L.u_key.off);
     pa.vcount = (u32*)(ws + L.vcount.off); pa.vstart = (u32*)(ws + L.vstart.off); pa.vfill = (u32*)(ws + L.vfill.off); pa.tstart = (u32*)(ws + L.tstart.off);
     pa.g_row = (u32*)(ws + L.g_row.off); pa.g_sig = (uint4*)(ws + L.g_sig.off);
+    pa.g_sig64 = (uint2*)(ws + L.g_sig64.off); pa.r_sig64 = (uint2*)(ws + L.r_sig64.off);
     pa.keep = ws + L.keep.off;
     pa.D = h->D; pa.n_rxn = G.n; pa.n_sizes = h->D + 1;
     pa.u_nnz = (int*)(ws + L.u_nnz.off); pa.u_rxn = (int*)(ws + L.u_rxn.off); pa.u_val = (i64*)(ws + L.u_val.off);

@@ -26,6 +26,7 @@ struct PostArgs {
     // minimality filter (a-7)
     u32* freq; u32* gcount; u32* gstart; u32* gfill;      // per arc: candidates using it, group size / start / fill
     uint4* r_sig; u32* v_row; u32* vcount; u32* vstart; u32* vfill; u32* tstart;   // join: row-order signatures, rows per (arc, size), tile prefix per arc
+    uint2* g_sig64; uint2* r_sig64;                       // first-stage 64-bit bucket signatures, grouped order / row order
     u32* g_row; uint4* g_sig;                             // rows grouped by their rarest arc: candidate id, 112-bit signature + |supp|
     int n_sizes;                                          // D + 1: the (arc, |supp|) bins of gcount / gstart / gfill
     unsigned char* keep;                                  // per unique support (uniq order)

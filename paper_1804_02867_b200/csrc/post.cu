@@ -241,6 +241,18 @@ __device__ __forceinline__ uint4 sig_of(const u16* arc, int n, bool exact) {   /
     return make_uint4(w[0], w[1], w[2], w[3] | ((u32)n << 16));
 }
 
+// first-stage signature: arc -> one of 64 buckets.  A support of 45 arcs sets about 32 of the bits, one of 50 arcs about 35:
+// a pair passes with probability around 0.54^32, so a warp almost never leaves the straight-line loop, and two of these
+// tests cost one 16-byte shared-memory load and four LOP3.
+__device__ __forceinline__ uint2 sig64_of(const u16* arc, int n) {
+    u32 w0 = 0, w1 = 0;
+    for (int t = 0; t < n; ++t) {
+        const u32 b = ((u32)arc[t] * 0x9E3779B1u) >> 26;
+        if (b < 32) w0 |= 1u << b; else w1 |= 1u << (b - 32);
+    }
+    return make_uint2(w0, w1);
+}
+
 __global__ void __launch_bounds__(256) k_filter_freq(const PostArgs a, u64 K, int use_smem) {
     // per-block histogram in shared memory when the arcs fit (popular arcs would otherwise serialise in L2)
     extern __shared__ u32 hist[];
@@ -301,9 +313,12 @@ __global__ void __launch_bounds__(256) k_filter_scatter(const PostArgs a, u64 K)
     const u16* arc = cand_arc(e, n);
     const u32 pos = atomicAdd(&a.gfill[(size_t)rarest_arc(a, arc, n) * a.n_sizes + n], 1u);
     const uint4 sg = sig_of(arc, n, a.g.A <= kSigBits);
+    const uint2 s64 = sig64_of(arc, n);
     a.g_row[pos] = id;
     a.g_sig[pos] = sg;
-    a.r_sig[u] = sg;   // the same record in row order, for the v side of the join
+    a.g_sig64[pos] = s64;
+    a.r_sig[u] = sg;   // the same records in row order, for the v side of the join
+    a.r_sig64[u] = s64;
 }
 __device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   // supp(w) subset of supp(v), sorted lists
     const int nw = cand_n(w), nv = cand_n(v);
@@ -323,10 +338,11 @@ __device__ bool arcs_subset(const unsigned char* w, const unsigned char* v) {   
 // of once per row.  k_filter_vprep sizes V(a) (only for arcs with a non-empty group) and numbers the tiles,
 // k_filter_vscatter fills the lists, k_filter_join maps a block to (arc, tile) by binary search over the tile prefix.
 #ifndef EFM_JOIN_THREADS
-#define EFM_JOIN_THREADS 32   // rows of V(a) per block (measured: 256 -> 10.6 ms, 128 -> 9.1, 64 -> 7.8, 32 -> 6.8: most arcs list few rows)
+#define EFM_JOIN_THREADS 128   // rows of V(a) per block: four warps share every tile of W(a)
 #endif
 constexpr int kJoinThreads = EFM_JOIN_THREADS;
-// V lists are ordered by (arc, size) too: the 256 rows of a tile have about the same size, hence the same range of W
+constexpr int kWTile = 1024;   // rows of W(a) per shared-memory tile (first-stage signatures: 8 KB)
+// V lists are ordered by (arc, size) too: the rows of a tile have about the same size, hence the same range of W
 __global__ void __launch_bounds__(256) k_filter_vcount(const PostArgs a, u64 K, int fill) {
     const u64 u = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= K) return;
@@ -342,7 +358,7 @@ __global__ void __launch_bounds__(256) k_filter_vcount(const PostArgs a, u64 K, 
         }
     }
 }
-__global__ void __launch_bounds__(1024) k_filter_tiles(const PostArgs a) {   // tiles of 256 rows per arc, prefix over the arcs
+__global__ void __launch_bounds__(1024) k_filter_tiles(const PostArgs a) {   // tiles of kJoinThreads rows per arc, prefix over the arcs
     __shared__ u32 part[1024];
     const int A = a.g.A, T = blockDim.x, per = (A + T - 1) / T, b0 = threadIdx.x * per;
     u32 st = 0;
@@ -367,10 +383,13 @@ __global__ void __launch_bounds__(1024) k_filter_tiles(const PostArgs a) {   // 
     }
     if (threadIdx.x == T - 1) a.tstart[A] = part[T - 1];
 }
+// Two stages per pair (w, v): the 64-bit bucket signatures (two rows of W per 16-byte shared-memory load), then, for the
+// few pairs that pass, the 112-bit signature + size record and the exact test on the sorted arc lists.
 __global__ void __launch_bounds__(kJoinThreads) k_filter_join(const PostArgs a) {
-    __shared__ uint4 wtile[kJoinThreads];
+    __shared__ uint4 wt4[kWTile / 2];
     __shared__ u32 s_gend;
     __shared__ unsigned long long s_pairs;
+    uint2* wt = (uint2*)wt4;
     const int A = a.g.A;
     const u32 n_tiles = a.tstart[A];
     const bool exact = A <= kSigBits;
@@ -382,12 +401,13 @@ __global__ void __launch_bounds__(kJoinThreads) k_filter_join(const PostArgs a) 
         const size_t gb = (size_t)x * a.n_sizes;
         const u32 vi = a.vstart[gb] + (tile - a.tstart[x]) * kJoinThreads + threadIdx.x;
         const bool live = vi < a.vstart[gb + a.n_sizes];
-        u32 u = 0, gend = 0;
+        u32 u = 0, gend = 0, vn0 = 0, vn1 = 0;
         uint4 sv = make_uint4(0, 0, 0, 0);
         const u32 g0 = a.gstart[gb];
         if (live) {
             u = a.v_row[vi];
             sv = a.r_sig[u];
+            { const uint2 t = a.r_sig64[u]; vn0 = ~t.x; vn1 = ~t.y; }
             gend = a.gstart[gb + (sv.w >> 16)];   // group rows of size < |supp(v)|
         }
         if (threadIdx.x == 0) { s_gend = 0; s_pairs = 0; }
@@ -397,36 +417,37 @@ __global__ void __launch_bounds__(kJoinThreads) k_filter_join(const PostArgs a) 
         const u32 bend = s_gend;
         const u32 n0 = ~sv.x, n1 = ~sv.y, n2 = ~sv.z, n3 = ~sv.w & 0xffffu;
         bool found = false;
-        u32 pairs = 0;
-        for (u32 base = g0; base < bend; base += kJoinThreads) {
-            const u32 w = base + threadIdx.x;
-            if (w < bend) wtile[threadIdx.x] = a.g_sig[w];
+        for (u32 base = g0; base < bend; base += kWTile) {
+            for (u32 i = threadIdx.x; i < (u32)kWTile; i += kJoinThreads) wt[i] = base + i < bend ? a.g_sig64[base + i] : make_uint2(0xffffffffu, 0xffffffffu);
             __syncthreads();
             if (live && !found && base < gend) {
-                const int jn = (int)min((u32)kJoinThreads, gend - base);
-                pairs += (u32)jn;
-                u32 hits = 0;   // signature hits are rare: collect them four records at a time, verify afterwards
-                int j = 0;
-                for (; j + 4 <= jn; j += 4) {
-                    const uint4 r0 = wtile[j], r1 = wtile[j + 1], r2 = wtile[j + 2], r3 = wtile[j + 3];
-                    const u32 m0 = (r0.x & n0) | (r0.y & n1) | (r0.z & n2) | (r0.w & n3);
-                    const u32 m1 = (r1.x & n0) | (r1.y & n1) | (r1.z & n2) | (r1.w & n3);
-                    const u32 m2 = (r2.x & n0) | (r2.y & n1) | (r2.z & n2) | (r2.w & n3);
-                    const u32 m3 = (r3.x & n0) | (r3.y & n1) | (r3.z & n2) | (r3.w & n3);
-                    if (m0 == 0 || m1 == 0 || m2 == 0 || m3 == 0) { hits = 1; break; }
-                }
-                if (hits || j < jn) {   // verify from the first unexamined / hit group of four
-                    for (; j < jn && !found; ++j) {
-                        const uint4 r = wtile[j];
-                        if (((r.x & n0) | (r.y & n1) | (r.z & n2) | (r.w & n3)) == 0)
-                            found = exact || arcs_subset(a.cand + (u64)a.g_row[base + j] * a.cand_stride, a.cand + (u64)a.uniq[u] * a.cand_stride);
+                // eight rows of W per step, one branch: rows behind gend (or behind the tile) are filtered in the closer look
+                const u32 jn = (min((u32)kWTile, gend - base) + 7u) / 8u;
+#pragma unroll 1
+                for (u32 j = 0; j < jn; ++j) {
+                    const uint4 ra = wt4[4 * j], rb = wt4[4 * j + 1], rc = wt4[4 * j + 2], rd = wt4[4 * j + 3];
+                    u32 z = min((ra.x & vn0) | (ra.y & vn1), (ra.z & vn0) | (ra.w & vn1));
+                    z = min(z, min((rb.x & vn0) | (rb.y & vn1), (rb.z & vn0) | (rb.w & vn1)));
+                    z = min(z, min((rc.x & vn0) | (rc.y & vn1), (rc.z & vn0) | (rc.w & vn1)));
+                    z = min(z, min((rd.x & vn0) | (rd.y & vn1), (rd.z & vn0) | (rd.w & vn1)));
+                    if (__builtin_expect(z == 0, 0)) {   // rare: some row of the eight passes the first stage, look closer
+#pragma unroll 1
+                        for (u32 c = 0; c < 8 && !found; ++c) {
+                            const u32 row = base + 8 * j + c;
+                            const uint2 w = wt[8 * j + c];
+                            if (((w.x & vn0) | (w.y & vn1)) != 0 || row >= gend) continue;
+                            const uint4 sg = a.g_sig[row];
+                            if (((sg.x & n0) | (sg.y & n1) | (sg.z & n2) | (sg.w & n3)) == 0)
+                                found = exact || arcs_subset(a.cand + (u64)a.g_row[row] * a.cand_stride, a.cand + (u64)a.uniq[u] * a.cand_stride);
+                        }
+                        if (found) break;
                     }
                 }
             }
             __syncthreads();
         }
         if (found) a.keep[u] = 0;
-        if (pairs) atomicAdd(&s_pairs, (unsigned long long)pairs);
+        if (live && gend > g0) atomicAdd(&s_pairs, (unsigned long long)(gend - g0));   // pair tests this row stands for
         __syncthreads();
         if (threadIdx.x == 0 && s_pairs) atomicAdd(&a.ctl->filter_pairs, (u64)s_pairs);
         __syncthreads();
@@ -452,7 +473,7 @@ cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s
     k_filter_scan<<<1, 1024, 0, s>>>(a.vcount, a.vstart, a.vfill, a.g.A * a.n_sizes);
     k_filter_tiles<<<1, 1024, 0, s>>>(a);
     k_filter_vcount<<<blocks, 256, 0, s>>>(a, K, 1);
-    k_filter_join<<<(unsigned)(sm_count * 16 * (256 / kJoinThreads)), kJoinThreads, 0, s>>>(a);
+    k_filter_join<<<(unsigned)(sm_count * 16), kJoinThreads, 0, s>>>(a);
     *n_launches += 9;
     return cudaGetLastError();
 }
