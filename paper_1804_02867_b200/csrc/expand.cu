@@ -314,6 +314,9 @@ __device__ __forceinline__ void write_task(const ExpandArgs& A, u64 ti, int ca, 
 }
 
 // ---- revisit parents (PROC2-4; readings G2-G5): 8 lanes per parent, read in place.
+// MODES: the build with the sampling mode (8(f)-1), the reaction mask (8(f)-2) and the per-candidate end records; the
+// plain exhaustive traversal runs the build without them.
+template <bool MODES>
 __device__ __forceinline__ void expand_revisits(const ExpandArgs& A, LevelCtl* lv, u64 first, u64 nR, int lane, KeyOut& ko, TaskOut& to,
                                                 WarpAcc& acc) {
     constexpr int G = 8;
@@ -356,7 +359,7 @@ __device__ __forceinline__ void expand_revisits(const ExpandArgs& A, LevelCtl* l
         bool act = live;
         if (live && cntv > A.max_loop) {
             act = false;
-            if (gl == 0) { atomicAdd(&ctl->st[ST_NOT_EFM], 1ULL); if (A.cand_end) A.cand_end[H.cand] = END_NOTEFM | ((u64)A.level << 8); }
+            if (gl == 0) { atomicAdd(&ctl->st[ST_NOT_EFM], 1ULL); if (MODES && A.cand_end) A.cand_end[H.cand] = END_NOTEFM | ((u64)A.level << 8); }
         }
         const int PI = (int)((rec >> 16) & 0xffffu), PO = (int)(rec & 0xffffu);
         // position and coefficient of PI in I[i*] and of PO in O[i*]: from the columns of the two arcs
@@ -464,7 +467,7 @@ __device__ __forceinline__ void expand_revisits(const ExpandArgs& A, LevelCtl* l
         if (act && status != CH_OK) {
             if (gl == 0) {
                 atomicAdd(&ctl->st[status == CH_OVERFLOW ? ST_OVERFLOW : ST_NONPOS], 1ULL);
-                if (A.cand_end) A.cand_end[H.cand] = (status == CH_OVERFLOW ? END_OVERFLOW : END_NONPOS) | ((u64)A.level << 8);
+                if (MODES && A.cand_end) A.cand_end[H.cand] = (status == CH_OVERFLOW ? END_OVERFLOW : END_NONPOS) | ((u64)A.level << 8);
             }
             act = false;
         }
@@ -511,6 +514,7 @@ struct WarpSmem {
     unsigned char* stage[2]; u64* bar; u32* sbits; u16* upos;
 };
 
+template <bool MODES>
 __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCtl* lv, u64 first, u64 nF, int lane, const WarpSmem& S,
                                                     u32& phase, KeyOut& ko, TaskOut& to, WarpAcc& acc) {
     Ctl* ctl = A.ctl;
@@ -574,7 +578,7 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
         auto ef_of = [&](int met) -> i64 { const u32 u = upos[met]; return u ? ef[u - 1] : 0; };
         int n_adm = 0;
         if (nv >= A.V) {
-            if (lane == 0) { atomicAdd(&ctl->st[ST_VISITED], 1ULL); if (A.cand_end) A.cand_end[H.cand] = END_VISITED | ((u64)A.level << 8); }
+            if (lane == 0) { atomicAdd(&ctl->st[ST_VISITED], 1ULL); if (MODES && A.cand_end) A.cand_end[H.cand] = END_VISITED | ((u64)A.level << 8); }
         } else {
             // primary on the side the flux arrives from: lowest arc of that side in the support (G13)
             int prim = -1;
@@ -592,11 +596,11 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
             const u64 vbase = vis_pack((u32)istar, fwd ? (u32)prim : 0u, fwd ? 0u : (u32)prim, 0u);
             const int ashift = fwd ? 0 : 16;
             auto admissible = [&](u32 a, u32 tw, bool insup) -> bool {   // readings G14, G15 and the reaction mask of 8(f)-2
-                return !(tw != 0xffffu && sbit(sbits, (int)tw)) && (insup || ns < A.D) && (!A.amask || ((__ldg(&A.amask[a >> 5]) >> (a & 31)) & 1u));
+                return !(tw != 0xffffu && sbit(sbits, (int)tw)) && (insup || ns < A.D) && (!MODES || !A.amask || ((__ldg(&A.amask[a >> 5]) >> (a & 31)) & 1u));
             };
             // 8(f)-1 sampling: count the admissible alternatives, then take exactly one of them
             int pick_idx = -1, seen = 0;
-            if (A.sample) {
+            if (MODES && A.sample) {
                 int tot = 0;
 #pragma unroll 1
                 for (int base = 0; base < alen; base += 32) {
@@ -625,7 +629,7 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
                 u32 adm_m = __ballot_sync(FULL, adm);
                 if (adm_m == 0) continue;
                 n_adm += __popc(adm_m);
-                if (A.sample) {   // only the sampled alternative goes on
+                if (MODES && A.sample) {   // only the sampled alternative goes on
                     const int here = __popc(adm_m);
                     const int sel = (pick_idx >= seen && pick_idx < seen + here) ? (int)__fns(adm_m, 0, pick_idx - seen + 1) : -1;
                     seen += here;
@@ -734,7 +738,7 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
                         cnu = nu + __reduce_add_sync(FULL, delta);
                     }
                     if (__builtin_expect(ovf, 0)) {
-                        if (lane == 0) { atomicAdd(&ctl->st[ST_OVERFLOW], 1ULL); if (A.cand_end) A.cand_end[H.cand] = END_OVERFLOW | ((u64)A.level << 8); }
+                        if (lane == 0) { atomicAdd(&ctl->st[ST_OVERFLOW], 1ULL); if (MODES && A.cand_end) A.cand_end[H.cand] = END_OVERFLOW | ((u64)A.level << 8); }
                         continue;
                     }
                     // gcd normalisation (reading G10).  A new arc cannot introduce a common factor: gcd_t(k f_t) = k and
@@ -769,7 +773,7 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
             }
             if (n_adm == 0 && lane == 0) {   // no admissible alternative
                 atomicAdd(&ctl->st[ST_DEAD_END], 1ULL);
-                if (A.cand_end) A.cand_end[H.cand] = END_DEAD | ((u64)A.level << 8);
+                if (MODES && A.cand_end) A.cand_end[H.cand] = END_DEAD | ((u64)A.level << 8);
             }
         }
         // ---- restore the shared tables to zero for the next parent
@@ -782,6 +786,7 @@ __device__ __forceinline__ void expand_first_visits(const ExpandArgs& A, LevelCt
     }
 }
 
+template <bool MODES>
 __global__ void __launch_bounds__(32, EFM_MIN_BLOCKS) k_expand(const __grid_constant__ ExpandArgs A) {
     extern __shared__ uint4 smem4[];
     const int lane = threadIdx.x;
@@ -818,8 +823,8 @@ __global__ void __launch_bounds__(32, EFM_MIN_BLOCKS) k_expand(const __grid_cons
         if (lane == 0) w = atomicAdd(&lv->work, 1ULL);
         w = __shfl_sync(FULL, w, 0);
         if (w >= total) break;
-        if (w < nRi) expand_revisits(A, lv, w * kRevisitPerItem, nR, lane, ko, to, acc);
-        else expand_first_visits(A, lv, (w - nRi) * kParentsPerItem, nF, lane, S, phase, ko, to, acc);
+        if (w < nRi) expand_revisits<MODES>(A, lv, w * kRevisitPerItem, nR, lane, ko, to, acc);
+        else expand_first_visits<MODES>(A, lv, (w - nRi) * kParentsPerItem, nF, lane, S, phase, ko, to, acc);
     }
     ko.finish(A, lane);
     if (lane == 0) {
@@ -1273,11 +1278,14 @@ cudaError_t launch_expand(const ExpandArgs& a, int sm_count, cudaStream_t s) {
     const size_t smem = a.sm_group;
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
     // per device: the attribute belongs to the function on the current device
-    cudaError_t e = cudaFuncSetAttribute(k_expand, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    const bool modes = a.sample || a.amask || a.cand_end;
+    cudaError_t e = modes ? cudaFuncSetAttribute(k_expand<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)
+                          : cudaFuncSetAttribute(k_expand<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     int per_sm = EFM_MIN_BLOCKS;
     while (per_sm > 1 && (size_t)per_sm * (smem + 1024) > 220 * 1024) --per_sm;
-    k_expand<<<(unsigned)(sm_count * per_sm), 32, smem, s>>>(a);
+    if (modes) k_expand<true><<<(unsigned)(sm_count * per_sm), 32, smem, s>>>(a);
+    else k_expand<false><<<(unsigned)(sm_count * per_sm), 32, smem, s>>>(a);
     return cudaGetLastError();
 }
 
