@@ -28,8 +28,24 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-DEFAULT_CAP = 262144          # frontier_cap of the timed workload
+DEFAULT_CAP = 1 << 24         # frontier_cap of the timed workload: the largest power of two whose workspace fits the 180 GB of
+                              # one B200 (153 GB).  If the allocation fails the next smaller power is timed.
+PARITY_CAP = 1 << 18          # sweep point at which tests/ compares every output with the oracle (the oracle needs minutes there)
+PROPERTY_CAP = 1 << 20        # sweep point at which tests/ checks Def 2 / Def 3 / order on every output
+DEFAULT_SWEEP = "262144,1048576,4194304"
 DEFAULT_MAX_CANDIDATES = 1 << 22
+
+
+def sized_params(params, cap, max_candidates=None):
+    """Workspace sizing of the genome workload at beam `cap` (the library defaults are worst-case bounds: largest possible
+    entry x cap, largest fan-out x cap; measured needs are far smaller and an overflow is a loud EFM_E_CAPACITY)."""
+    p = dict(params)
+    p["frontier_cap"] = cap
+    p["max_candidates"] = max(max_candidates or DEFAULT_MAX_CANDIDATES, 2 * cap)
+    if cap >= (1 << 20):
+        p["max_frontier_bytes"] = 1792 * cap      # packed entries average about 1 KB
+        p["max_child_keys"] = 48 * cap            # about 17 children are evaluated per parent on average, 25 on the widest levels
+    return p
 METRIC = "partial_pathways_expanded_per_sec"
 UNIT = "expanded/s"
 
@@ -187,9 +203,6 @@ def main_ours(args):
     import paper_1804_02867_b200 as efm
 
     # rank r owns the independent problem of generator seed r (weak scaling, no collective on the data path)
-    net, params = rank_problem(args.workload, rank, args.cap)
-    params["max_candidates"] = args.max_candidates
-    en = efm.Enumerator(net.S, net.reversible, net.internal, params, device=local, flags=efm.EFM_F_TIMING)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
     def barrier():
@@ -197,7 +210,33 @@ def main_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    def make_enumerator(cap):
+        net_, params_ = rank_problem(args.workload, rank, cap)
+        if args.workload == "genome":
+            params_ = sized_params(params_, cap, args.max_candidates)
+        else:
+            params_["max_candidates"] = args.max_candidates
+        return net_, params_, efm.Enumerator(net_.S, net_.reversible, net_.internal, params_, device=local, flags=efm.EFM_F_TIMING)
+
+    # the largest beam whose workspace this GPU can hold right now: the requested one, else the next smaller powers of two
+    cap_used, fallback_note = args.cap, None
+    while True:
+        net, params, en = make_enumerator(cap_used)
+        try:
+            en.enumerate(net.seed_sets, dense=False)
+            break
+        except (torch.cuda.OutOfMemoryError, efm.EfmError) as exc:
+            if isinstance(exc, efm.EfmError) and exc.code not in (efm.EFM_E_NOMEM, efm.EFM_E_CUDA):
+                raise
+            en.close()
+            del en
+            torch.cuda.empty_cache()
+            if cap_used <= (1 << 18):
+                raise
+            fallback_note = f"frontier_cap {args.cap} did not fit ({type(exc).__name__}); timed {cap_used // 2}"
+            cap_used //= 2
+    args.cap = cap_used
+    for _ in range(max(args.warmup, 3) - 1):
         en.enumerate(net.seed_sets, dense=False)
     # ---- device-resident figure: K steps, each timed by the library with CUDA events on the launching stream
     sampler = ClockSampler(local) if rank == 0 else None
@@ -236,25 +275,65 @@ def main_ours(args):
         d2h = (row_ptr.numel() * 8 + rxn.numel() * 4 + val.numel() * 8 + int(r2.stats["levels"]) * 256)
         del row_ptr, rxn, val   # back to torch's pinned-memory cache: the next step reuses the buffers
         en2.close()
+        en2._workspace = None
     barrier()
 
     ms_max, e2e_ms_max, expanded_all, outputs_all, children_all = reduce_over_ranks(
         [ms, e2e_s * 1000.0], [float(acc["expanded"]), float(acc["output"]), float(acc["children"])],
         dist if world > 1 else None, torch.device("cuda", local))
 
+    # ---- other beam sizes of the same workload (rank 0, one warm-up + two timed steps each): the curve the headline sits on
+    sweep = []
+    if rank == 0 and args.sweep:
+        ws_bytes = en.workspace_bytes()
+        en.close()
+        en._workspace = None
+        torch.cuda.empty_cache()
+        for cap_s in [int(x) for x in args.sweep.split(",") if x]:
+            if cap_s == args.cap:
+                continue
+            try:
+                net_s, params_s, en_s = make_enumerator(cap_s)
+                en_s.enumerate(net_s.seed_sets, dense=False)
+                tot, acc_s = 0.0, {}
+                for _ in range(2):
+                    flush.fill_(1)
+                    torch.cuda.synchronize()
+                    st = en_s.enumerate(net_s.seed_sets, dense=False).stats
+                    tot += st["ms_total"]
+                    for k, v in st.items():
+                        acc_s[k] = acc_s.get(k, 0) + v
+                ms_e = acc_s["ms_order"] + acc_s["ms_expand_count"] + acc_s["ms_expand_write"]
+                sweep.append({"frontier_cap": cap_s, "ms_per_step": tot / 2, "value": acc_s["expanded"] / (tot * 1e-3),
+                              "outputs_per_step": acc_s["output"] / 2, "levels": acc_s["levels"] / 2,
+                              "roofline_frac": acc_s["algo_bytes"] / (ms_e * 1e-3) / 1e9 / _peaks()[0],
+                              "filter_share": acc_s["ms_filter"] / tot, "workspace_bytes": en_s.workspace_bytes()})
+                en_s.close()
+                del en_s
+                torch.cuda.empty_cache()
+            except Exception as exc:   # a sweep point never takes the headline down
+                sweep.append({"frontier_cap": cap_s, "error": f"{type(exc).__name__}: {exc}"[:200]})
+    else:
+        ws_bytes = en.workspace_bytes()
+
     if rank == 0:
         peak, peak_src = _peaks()
-        # one "launch" of the expansion = k_expand (evaluate) + k_compact + k_materialise of one level
-        n_exp_launch = acc["n_expand_count"]
+        # one "launch" of the expansion = k_order + k_expand (evaluate) + k_compact + k_materialise of one level
+        n_exp_launch = max(1.0, acc["levels"] - args.steps)   # the last level of a traversal has nothing to expand
         ms_expand = acc["ms_order"] + acc["ms_expand_count"] + acc["ms_expand_write"]
         achieved = acc["algo_bytes"] / (ms_expand * 1e-3) / 1e9 if ms_expand > 0 else 0.0
-        # dram__bytes_read + write per full level from the ncu --set full capture (profiles/r1_v12_expand_full.md); it was
-        # taken on the default workload only
+        # dram__bytes_read + write of the four kernels over one full level, from the committed ncu --set full capture of
+        # this workload (profiles/r2_traffic.json names the summary it was read from); null for any other configuration
         traffic, traffic_src = args.traffic, "--traffic"
-        if traffic is None and args.workload == "genome" and args.cap == DEFAULT_CAP:
-            traffic, traffic_src = 7.36e8, "profiles/r1_v12_expand_full.md: k_expand 277 MB + k_materialise 459 MB per full level (algorithmic 216 MB)"
-        elif traffic is None:
+        if traffic is None:
             traffic_src = None
+            try:
+                with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as fh:
+                    tj = json.load(fh)
+                if args.workload == tj["workload"] and args.cap == tj["frontier_cap"]:
+                    traffic, traffic_src = float(tj["dram_bytes_per_full_level"]), tj["source"]
+            except Exception:
+                pass
         roofline = {"bound": "hbm", "kernel": "expansion of one level: k_order + k_expand (evaluate) + k_compact + k_materialise", "achieved": achieved,
                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                     "peak_source": peak_src, "launches_per_step": n_exp_launch / args.steps,
@@ -274,7 +353,8 @@ def main_ours(args):
                 "vs_baseline": None, "dtype": "int64", "data": "synthetic",
                 "config": {"workload": f"{args.workload}-seed{{rank}} (BASELINE.json configs[4]: 1000+150 metabolites, 2000 reactions, "
                                        "30% reversible, depth cap 60, 8 target exchange reactions)",
-                           "frontier_cap": args.cap, "params": {k: int(v) for k, v in params.items()},
+                           "frontier_cap": args.cap, "fallback": fallback_note, "workspace_bytes": int(ws_bytes),
+                           "params": {k: int(v) for k, v in params.items()},
                            "l2": "flushed between timed iterations (256 MiB write)", "parallelism": f"replicas x{world}"},
                 "clocks": clocks,
                 "e2e": {"value": expanded_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
@@ -296,9 +376,11 @@ def main_ours(args):
                                           "ms_output": "k_out_* + k_bitonic_*"},
                           "work_profile_per_step": {k: acc[k] / args.steps for k in
                                                     ("expanded", "first_visits", "general_children", "materialised")},
+                          "sweep": sweep, "host_syncs_per_step": acc["host_syncs"] / args.steps,
                           "filter_pairs_per_s": (acc["filter_pairs"] / (acc["ms_filter"] * 1e-3)) if acc["ms_filter"] else None}}
         print(json.dumps(line))
-    en.close()
+    if en._h:
+        en.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -314,6 +396,7 @@ def main():
     ap.add_argument("--cap", type=int, default=DEFAULT_CAP, help="frontier_cap (beam) of the workload")
     ap.add_argument("--max-candidates", type=int, default=DEFAULT_MAX_CANDIDATES)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", default=DEFAULT_SWEEP, help="comma-separated frontier_cap values also timed (rank 0; '' = none)")
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram bytes per expansion of a level (default: the profiles/ capture of the default workload)")
     args = ap.parse_args()

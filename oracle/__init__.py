@@ -36,12 +36,12 @@ class _Params(ctypes.Structure):
     _fields_ = [("max_support", ctypes.c_int32), ("max_loop", ctypes.c_int32), ("dep_depth", ctypes.c_int32),
                 ("max_visited", ctypes.c_int32), ("frontier_cap", ctypes.c_int64), ("threads", ctypes.c_int32),
                 ("trace", ctypes.c_int32), ("shuffle_seed", ctypes.c_uint64), ("sample_count", ctypes.c_int32),
-                ("reserved", ctypes.c_int32), ("sample_seed", ctypes.c_uint64), ("allowed", ctypes.c_void_p)]
+                ("exact", ctypes.c_int32), ("sample_seed", ctypes.c_uint64), ("allowed", ctypes.c_void_p)]
 
 
 STAT_FIELDS = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxloop", "discarded_nonpos",
                "discarded_overflow", "discarded_visited", "truncated_beam", "unique_supports", "poisoned",
-               "output", "peak_frontier", "algo_bytes"]
+               "output", "peak_frontier", "algo_bytes", "non_elementary"]
 
 
 class _Stats(ctypes.Structure):
@@ -111,7 +111,7 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
                        seed_sets: Optional[Sequence[Sequence[int]]] = None, threads: int = 1,
                        shuffle_seed: int = 0, export_graph: bool = False,
                        self_check: bool = True, trace: bool = False, sample_count: int = 0, sample_seed: int = 0,
-                       allowed: Optional[np.ndarray] = None) -> OracleResult:
+                       allowed: Optional[np.ndarray] = None, exact: bool = False) -> OracleResult:
     """Run the oracle.  ``seed_sets`` holds arc codes 2*j + (dir < 0); None = default boundary arcs (O2)."""
     lib = _load()
     S = np.ascontiguousarray(S, dtype=np.int32)
@@ -120,7 +120,7 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
     m, n = S.shape
     p = _Params(int(params.get("max_support", 0)), int(params.get("max_loop", 8)), int(params.get("dep_depth", 4)),
                 int(params.get("max_visited", 0)), int(params.get("frontier_cap", 0)), int(threads), int(trace),
-                int(shuffle_seed), int(sample_count), 0, int(sample_seed) & ((1 << 64) - 1), None)
+                int(shuffle_seed), int(sample_count), int(bool(exact)), int(sample_seed) & ((1 << 64) - 1), None)
     if allowed is not None:
         allowed = np.ascontiguousarray(allowed, dtype=np.uint8)
         assert allowed.shape == (n,)
@@ -209,7 +209,8 @@ def enumerate_pathways(S: np.ndarray, reversible: np.ndarray, internal: np.ndarr
 
 def enumerate_network(net, threads: int = 1, shuffle_seed: int = 0, export_graph: bool = False,
                       self_check: bool = True, seed_sets="net", trace: bool = False, sample_count: int = 0,
-                      sample_seed: int = 0, allowed: Optional[np.ndarray] = None, **param_overrides) -> OracleResult:
+                      sample_seed: int = 0, allowed: Optional[np.ndarray] = None, exact: bool = False,
+                      **param_overrides) -> OracleResult:
     """Run the oracle on a ``netgen.Network`` with its own parameters (optionally overridden).
 
     ``seed_sets="net"`` uses the network's own seed sets (None there = default boundary arcs)."""
@@ -217,7 +218,7 @@ def enumerate_network(net, threads: int = 1, shuffle_seed: int = 0, export_graph
     params.update(param_overrides)
     seeds = net.seed_sets if isinstance(seed_sets, str) else seed_sets
     return enumerate_pathways(net.S, net.reversible, net.internal, params, seeds, threads, shuffle_seed,
-                              export_graph, self_check, trace, sample_count, sample_seed, allowed)
+                              export_graph, self_check, trace, sample_count, sample_seed, allowed, exact)
 
 
 def state_hash(arcs: Sequence[int], fluxes: Sequence[int], visited: Sequence[Sequence[int]]) -> int:

@@ -55,7 +55,13 @@ typedef struct {
      * from seed set c mod n_sets and takes ONE admissible alternative per first visit, chosen by the counter-based
      * generator pick(sample_seed, c, i*) below; no fan-out, no beam. */
     int32_t sample_count;
-    int32_t reserved;
+    /* SURVEY.md 8(f)-3 exact elementarity (Def 3; "recognizing the elementarity through rank
+     * test"): exact != 0 replaces step O8(iii) "minimal among the candidates found" by the rank test on every unique,
+     * unpoisoned support: it stays iff the internal rows of S restricted to its arcs have rank |supp| - 1 (nullity 1).
+     * The rank is taken over GF(p), p = 2^31 - 1: a well-defined number (any elimination order gives it), never above the
+     * rational rank, and the candidate's own flux vector bounds the rational rank by |supp| - 1 from above -- so every
+     * "elementary" verdict is exact; a "not elementary" verdict errs only if p divides a minor (reading G24). */
+    int32_t exact;
     uint64_t sample_seed;
     /* SURVEY.md 8(f)-2 targeted observability ("contributing reactions of each EFM were selected intentionally",
      * PAPER.md:392-396): allowed[j] = 0 makes every OR-alternative of reaction j inadmissible; NULL = all allowed */
@@ -67,6 +73,7 @@ typedef struct {
         discarded_overflow, discarded_visited, truncated_beam, unique_supports, poisoned, output;
     int64_t peak_frontier; /* largest number of active entries in a level (before the beam) */
     int64_t algo_bytes;    /* SURVEY.md 8(d) algorithmic bytes summed over all expansions   */
+    int64_t non_elementary; /* exact mode: unique, unpoisoned supports the rank test rejected */
 } oracle_stats;
 
 /* ------------------------------------------------------------------ O1: the MG graph */
@@ -508,6 +515,47 @@ static uint64_t rng_next(uint64_t *s) {
 /* ------------------------------------------------------------------ the whole procedure, O2 + O4 + O8 */
 #define E_INVAL (-1)
 
+/* 8(f)-3: rank over GF(2^31 - 1) of the internal rows of S restricted to the arcs of e, by plain Gaussian elimination on the
+ * dense (touched metabolites) x (arcs) matrix. */
+#define RANK_P 2147483647LL
+static int64_t inv_mod_p(int64_t a) { /* a^(p-2) mod p */
+    int64_t r = 1, b = a % RANK_P, e = RANK_P - 2;
+    while (e) { if (e & 1) r = r * b % RANK_P; b = b * b % RANK_P; e >>= 1; }
+    return r;
+}
+static int support_rank(const graph *G, const entry *e) {
+    int n = e->n_supp, M = G->M;
+    int *row_of = malloc(sizeof(int) * (M + 1));
+    for (int i = 0; i < M; i++) row_of[i] = -1;
+    int R = 0;
+    for (int k = 0; k < n; k++)
+        for (int q = G->col_ptr[e->arc[k]]; q < G->col_ptr[e->arc[k] + 1]; q++)
+            if (row_of[G->col_met[q]] < 0) row_of[G->col_met[q]] = R++;
+    int64_t *Mx = calloc((size_t)(R + 1) * (n + 1), sizeof(int64_t));
+    for (int k = 0; k < n; k++)
+        for (int q = G->col_ptr[e->arc[k]]; q < G->col_ptr[e->arc[k] + 1]; q++) {
+            int64_t v = G->col_s[q] % RANK_P;
+            if (v < 0) v += RANK_P;
+            Mx[(size_t)row_of[G->col_met[q]] * n + k] = v;
+        }
+    int rank = 0;
+    for (int c = 0; c < n && rank < R; c++) {
+        int piv = -1;
+        for (int r = rank; r < R; r++) if (Mx[(size_t)r * n + c]) { piv = r; break; }
+        if (piv < 0) continue;
+        for (int k = 0; k < n; k++) { int64_t t = Mx[(size_t)piv * n + k]; Mx[(size_t)piv * n + k] = Mx[(size_t)rank * n + k]; Mx[(size_t)rank * n + k] = t; }
+        int64_t inv = inv_mod_p(Mx[(size_t)rank * n + c]);
+        for (int r = rank + 1; r < R; r++) {
+            int64_t f = Mx[(size_t)r * n + c] * inv % RANK_P;
+            if (!f) continue;
+            for (int k = c; k < n; k++) Mx[(size_t)r * n + k] = ((Mx[(size_t)r * n + k] - f * Mx[(size_t)rank * n + k]) % RANK_P + RANK_P) % RANK_P;
+        }
+        rank++;
+    }
+    free(Mx); free(row_of);
+    return rank;
+}
+
 int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev, const uint8_t *internal,
                      const oracle_params *P0, const int32_t *seed_ptr, const int32_t *seed_code, int32_t n_sets,
                      oracle_result **out) {
@@ -730,6 +778,10 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
     uint8_t *minimal = malloc(uniq.n + 1);
 #pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
     for (int64_t x = 0; x < uniq.n; x++) {
+        if (P.exact) {   /* 8(f)-3: the rank test instead of the comparison with the other candidates */
+            minimal[x] = (uint8_t)(support_rank(G, uniq.v[x]) == uniq.v[x]->n_supp - 1);
+            continue;
+        }
         int ok = 1;
         for (int64_t y = 0; y < uniq.n && ok; y++) {
             if (y == x) continue;
@@ -746,6 +798,7 @@ int oracle_enumerate(const int32_t *S, int32_t m, int32_t n, const uint8_t *rev,
     /* (iv) reaction space v_j = f_j+ - f_j-, (v) lexicographic order */
     int64_t n_out = 0;
     for (int64_t x = 0; x < uniq.n; x++) n_out += minimal[x];
+    if (P.exact) st->non_elementary = uniq.n - n_out;
     /* rows carry their step count behind the n flux columns while they are sorted */
     int64_t *rows = calloc((size_t)(n_out + 1) * (n + 1), sizeof(int64_t));
     int64_t r = 0;

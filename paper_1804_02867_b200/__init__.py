@@ -139,7 +139,7 @@ class Enumerator:
     def _check(self, rc: int):
         if rc != EFM_OK:
             text = self._lib.efm_strerror(rc).decode()
-            if rc == EFM_E_CUDA and self._h:
+            if rc in (EFM_E_CUDA, EFM_E_CAPACITY) and self._h and self._lib.efm_last_error(self._h):
                 text += ": " + self._lib.efm_last_error(self._h).decode()
             raise EfmError(rc, text)
 

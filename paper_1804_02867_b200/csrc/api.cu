@@ -584,7 +584,16 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
             CK(cudaMemcpyAsync(recs.data() + l0, ws + L.lvl.off + sizeof(LevelStats) * l0, sizeof(LevelStats) * (size_t)(level + 1 - l0),
                                cudaMemcpyDeviceToHost, s));
             CK(read_ctl());
-            if (hc->error) return EFM_E_CAPACITY;
+            if (hc->error) {
+                char buf[160];
+                snprintf(buf, sizeof buf, "capacity exceeded near level %llu:%s%s%s%s", (unsigned long long)level,
+                         (hc->error & ERR_FRONTIER) ? " frontier (max_frontier / max_frontier_bytes)" : "",
+                         (hc->error & ERR_CAND) ? " candidates (max_candidates)" : "",
+                         (hc->error & ERR_KEYS) ? " child keys / tasks (max_child_keys / max_child_tasks)" : "",
+                         (hc->error & ERR_LEVELS) ? " levels" : "");
+                h->last_error = buf;
+                return EFM_E_CAPACITY;
+            }
             more = (hc->lv[level & 1].alloc >> kAllocShift) != 0;
             if (more && level >= (u64)h->max_levels) return EFM_E_CAPACITY;
         }

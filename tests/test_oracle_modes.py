@@ -157,3 +157,94 @@ def test_sampling_bookkeeping_and_order_independence(oracle_mod):
     # candidate c starts from seed set c mod n_sets: with 8 default roots, candidates 3 and 11 share their seed arc
     full = oracle_mod.enumerate_network(net)
     assert full.n_roots >= 2
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f)-3 exact elementarity (rank test instead of "minimal among the candidates found")
+# ---------------------------------------------------------------------------------------------------------------------
+def _rational_rank(rows):
+    """Rank over the rationals by fraction elimination (independent of the oracle's modular elimination)."""
+    from fractions import Fraction
+    Mx = [[Fraction(int(v)) for v in r] for r in rows]
+    rank, ncol = 0, len(Mx[0]) if Mx else 0
+    for c in range(ncol):
+        piv = next((r for r in range(rank, len(Mx)) if Mx[r][c] != 0), None)
+        if piv is None:
+            continue
+        Mx[rank], Mx[piv] = Mx[piv], Mx[rank]
+        for r in range(rank + 1, len(Mx)):
+            if Mx[r][c] != 0:
+                f = Mx[r][c] / Mx[rank][c]
+                Mx[r] = [x - f * y for x, y in zip(Mx[r], Mx[rank])]
+        rank += 1
+    return rank
+
+
+def test_exact_mode_by_hand(oracle_mod):
+    """H7 network r0: ->A, r1: A->, r2: ->B, r3: 2B->, seed {r0, r2}: the balanced pathway (2,2,2,1) uses all four reactions.
+    Its internal rows are A: (1,-1,0,0), B: (0,0,1,-2): rank 2 = |supp| - 2, nullity 2 -- it is the sum of the two EFMs
+    (1,1,0,0) and (0,0,2,1), not elementary (Def 3).  Alone among the candidates it passes the pairwise
+    filter; the rank test rejects it.  Seed {r0}: (1,1,0,0), one row, rank 1 = |supp| - 1: elementary."""
+    net = hand_network([({}, {"A": 1}, False), ({"A": 1}, {}, False), ({}, {"B": 1}, False), ({"B": 2}, {}, False)], ["A", "B"])
+    assert run(oracle_mod, net, [[0, 4]]).flux.tolist() == [[2, 2, 2, 1]]
+    r = run(oracle_mod, net, [[0, 4]], exact=True)
+    assert r.flux.tolist() == [] and r.stats["non_elementary"] == 1 and r.stats["unique_supports"] == 1
+    r = run(oracle_mod, net, [[0, 4], [0], [4]], exact=True)
+    assert r.flux.tolist() == [[0, 0, 2, 1], [1, 1, 0, 0]] and r.stats["non_elementary"] == 1
+    # P2 (recycle): (1,2,1,2) on r0..r3; rows A: (1,-1,1,0), B: (0,1,0,-1), C: (0,1,-2,0): rank 3 = 4 - 1
+    r = run(oracle_mod, hand_network(*P2), [[0]], exact=True)
+    assert r.flux.tolist() == [[1, 2, 1, 2]] and r.stats["non_elementary"] == 0
+
+
+@pytest.mark.parametrize("name,over,count", [("toy", {}, 0), ("small", {}, 150), ("core", dict(frontier_cap=4096), 150),
+                                             ("mid", dict(frontier_cap=2048), 200)])
+def test_exact_mode_against_rational_rank(oracle_mod, name, over, count):
+    """Every balanced state the traversal reaches (test hook), grouped by support: a support with one flux vector whose
+    internal rows have RATIONAL rank |supp| - 1 (fraction elimination, written here) must be an output of the exact
+    mode, every other one must not."""
+    from netgen import random_seed_sets
+    net = make_network(name, 0)
+    seeds = random_seed_sets(net, count, 2, 11) if count else oracle_mod.all_arc_seed_sets(net.reversible)
+    res = oracle_mod.enumerate_network(net, seed_sets=seeds, exact=True, trace=2, self_check=False, **over)
+    groups = {}
+    for lvl in res.trace:
+        for e in lvl:
+            if e["n_unb"] == 0:
+                groups.setdefault(frozenset(e["flux"]), set()).add(tuple(sorted(e["flux"].items())))
+    arcs = []
+    for j in range(net.n):
+        arcs.append((j, 1))
+        if net.reversible[j]:
+            arcs.append((j, -1))
+    Sint = net.S[net.internal.astype(bool)].astype(np.int64)
+    want, rejected = [], 0
+    for supp, vecs in groups.items():
+        if len(vecs) != 1:
+            continue
+        cols = sorted(supp)
+        sub = np.stack([Sint[:, arcs[a][0]] * arcs[a][1] for a in cols], axis=1)
+        sub = sub[np.any(sub != 0, axis=1)]
+        if _rational_rank(sub.tolist()) == len(cols) - 1:
+            v = [0] * net.n
+            for a, f in next(iter(vecs)):
+                v[arcs[a][0]] += arcs[a][1] * f
+            want.append(v)
+        else:
+            rejected += 1
+    want.sort()
+    assert res.flux.tolist() == want
+    assert res.stats["non_elementary"] == rejected and res.stats["output"] == len(want)
+    if count:
+        assert rejected > 0   # the rank test did something the data could show
+
+
+def test_exact_mode_outputs_are_true_efms_of_the_toy_network(oracle_mod):
+    """Brute force (every arc subset without a twin pair whose nullspace is one strictly positive ray) fixes the EFM set of
+    toy; the exact mode returns exactly the found candidates that are in it."""
+    from oracle.brute_force import brute_force_efms
+    net = make_network("toy", 0)
+    truth = {tuple(int(x) for x in r) for r in brute_force_efms(net.S, net.reversible, net.internal)}
+    seeds = oracle_mod.all_arc_seed_sets(net.reversible)
+    ex = oracle_mod.enumerate_network(net, seed_sets=seeds, exact=True)
+    assert {tuple(r) for r in ex.flux.tolist()} <= truth
+    assert ex.stats["output"] + ex.stats["non_elementary"] + ex.stats["poisoned"] == ex.stats["unique_supports"]

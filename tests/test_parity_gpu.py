@@ -178,11 +178,12 @@ def test_genome(efm, oracle_mod, cap):
 
 
 def test_genome_at_the_bench_configuration(efm, oracle_mod):
-    """Element-by-element parity of the configuration bench.py times (genome seed 0, frontier_cap bench.DEFAULT_CAP, the
-    bench's candidate capacity): the oracle needs a few minutes on the box's host cores."""
+    """Element-by-element parity of the bench workload (genome seed 0) at the sweep point bench.PARITY_CAP, sized as the
+    bench sizes it: the largest beam the oracle finishes in minutes on the box's host cores (about 2 ms per unit of cap)."""
     import bench
     net = make_network("genome", 0)
-    got, _ = assert_parity(efm, oracle_mod, net, frontier_cap=bench.DEFAULT_CAP, max_candidates=bench.DEFAULT_MAX_CANDIDATES)
+    sized = bench.sized_params(net.params, bench.PARITY_CAP)
+    got, _ = assert_parity(efm, oracle_mod, net, **{k: v for k, v in sized.items() if k not in net.params or k == "frontier_cap"})
     assert got.stats["truncated_beam"] > 0 and got.stats["output"] > 100000
 
 
@@ -319,15 +320,15 @@ def test_sparse_and_dense_results_agree(efm):
 
 
 def test_bench_configuration_properties(efm):
-    """The configuration bench.py times (genome seed 0, frontier_cap bench.DEFAULT_CAP) is too large for the oracle (about
-    2 ms per unit of cap), so it is held by what is true at any size: Def 2 on every output, canonical form,
-    support-minimality and lexicographic order on samples, counter identities, and run-to-run determinism (the
-    kernels allocate with atomics, the result must not depend on their order)."""
+    """The bench workload at the sweep point bench.PROPERTY_CAP is too large for the oracle (about 2 ms per unit of cap),
+    so it is held by what is true at any size: Def 2 on every output, canonical form, support-minimality and
+    lexicographic order on samples, counter identities, and run-to-run determinism (the kernels allocate with atomics,
+    the result must not depend on their order)."""
     import scipy.sparse as sp
     import bench
-    cap = bench.DEFAULT_CAP
+    cap = bench.PROPERTY_CAP
     net = make_network("genome", 0)
-    params = dict(net.params, frontier_cap=cap, max_candidates=bench.DEFAULT_MAX_CANDIDATES)
+    params = bench.sized_params(net.params, cap)
     en = efm.Enumerator(net.S, net.reversible, net.internal, params)
     res = en.enumerate(net.seed_sets, dense=False)
     nnz, rxn, val = en.result_sparse()
@@ -433,3 +434,47 @@ def test_reaction_mask(efm, oracle_mod, name, over):
     allowed = (row != 0).astype(np.uint8)
     got, ref = assert_parity(efm, oracle_mod, net, allowed=allowed, **over)
     assert any(np.array_equal(row, r) for r in got.flux)
+
+
+def test_bench_headline_configuration_sampled(efm):
+    """The configuration bench.py times by default (genome seed 0, frontier_cap bench.DEFAULT_CAP, 153 GB of workspace, or
+    the next smaller power of two this GPU can hold): Def 2, gcd 1 and strict order on sampled outputs, counter identities."""
+    import torch
+    import bench
+    net = make_network("genome", 0)
+    cap = bench.DEFAULT_CAP
+    while True:
+        en = efm.Enumerator(net.S, net.reversible, net.internal, bench.sized_params(net.params, cap))
+        try:
+            res = en.enumerate(net.seed_sets, dense=False)
+            break
+        except (torch.cuda.OutOfMemoryError, efm.EfmError):
+            en.close()
+            torch.cuda.empty_cache()
+            assert cap > (1 << 20)
+            cap //= 2
+    st, lv = res.stats, res.levels
+    K = res.n_out
+    assert K == int(st["output"]) > cap // 2 and st["truncated_beam"] > 0
+    row_ptr, rxn, val = (t.numpy() for t in en.result_csr(pinned=False))
+    assert row_ptr[0] == 0 and row_ptr[-1] == len(rxn) and np.all(np.diff(row_ptr) > 0)
+    Sint = net.S[net.internal.astype(bool)].astype(np.int64)
+    irrev = ~net.reversible.astype(bool)
+    rng = np.random.default_rng(1)
+    prev = None
+    for r in np.sort(rng.choice(K - 1, 4000, replace=False)):
+        rows = []
+        for q in (r, r + 1):
+            j, v = rxn[row_ptr[q]: row_ptr[q + 1]], val[row_ptr[q]: row_ptr[q + 1]]
+            assert np.all(np.diff(j) > 0) and np.all(v != 0) and np.gcd.reduce(np.abs(v)) == 1
+            assert np.all(v[irrev[j]] > 0)                                  # Def 2: sign on irreversible reactions
+            assert not np.any(Sint[:, j] @ v)                               # Def 2: S_int . v = 0
+            d = np.zeros(net.S.shape[1], np.int64); d[j] = v
+            rows.append(d)
+        nz = np.nonzero(rows[0] != rows[1])[0]
+        assert nz.size and rows[0][nz[0]] < rows[1][nz[0]], r               # strict lexicographic order
+    assert int(st["expanded"]) == int(lv["expanded"].sum()) and int(st["children"]) == int(lv["children"].sum())
+    assert int(st["done"]) == int(lv["done"].sum()) >= int(st["unique_supports"]) >= K
+    assert np.all(lv["expanded"] <= cap) and int(lv["expanded"].max()) > 0.9 * cap
+    assert int(st["truncated_beam"]) == int(lv["active"].sum() - lv["expanded"].sum())
+    en.close()
