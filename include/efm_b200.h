@@ -43,6 +43,10 @@ extern "C" {
 #define EFM_F_NO_STAGING 0x8u   /* read every parent in place (the route of entries larger than the   */
                                 /* shared-memory staging buffer)                                      */
 
+#define EFM_F_EXACT_ELEMENTARITY 0x10u /* replace "minimal among the candidates found" by the rank test    */
+                                /* of Def 3: a support stays iff the internal rows of S restricted */
+                                /* to it have rank |supp| - 1 over GF(2^31 - 1); needs max_support <= 128               */
+
 typedef struct efm_handle efm_handle; /* opaque: host copy of the graph + pointers INTO the workspace */
 
 /* Traversal parameters.  Alg 1's #defines M, R are taken from S; C (number of
@@ -94,6 +98,7 @@ typedef struct {
     int64_t filter_pairs;   /* signature pair tests done by the minimality filter                    */
     /* work profile of the expansion: first-visit parents, children through the general routine, children materialised */
     int64_t first_visits, general_children, materialised;
+    int64_t non_elementary; /* EFM_F_EXACT_ELEMENTARITY: unique, unpoisoned supports the rank test rejected          */
 } efm_stats;
 
 /* Build the modified AND/OR graph MG (Defs 4-6; "Convert the given matrix to the MG

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libefm_b200.so")
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "efm_b200.h")
 
 EFM_OK, EFM_E_INVAL, EFM_E_NOMEM, EFM_E_CAPACITY, EFM_E_CUDA, EFM_E_STATE = 0, -1, -2, -3, -4, -5
-EFM_F_TIMING, EFM_F_NO_FASTPATH, EFM_F_NO_STAGING = 0x1, 0x4, 0x8
+EFM_F_TIMING, EFM_F_NO_FASTPATH, EFM_F_NO_STAGING, EFM_F_EXACT_ELEMENTARITY = 0x1, 0x4, 0x8, 0x10
 
 
 class efm_params(ctypes.Structure):
@@ -37,7 +37,7 @@ _STAT_INT = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxl
              "host_syncs"]
 _STAT_MS = ["ms_build", "ms_total", "ms_order", "ms_expand_count", "ms_beam", "ms_expand_write", "ms_hash",
             "ms_filter", "ms_output"]
-_STAT_INT2 = ["n_expand_count", "filter_pairs", "first_visits", "general_children", "materialised"]
+_STAT_INT2 = ["n_expand_count", "filter_pairs", "first_visits", "general_children", "materialised", "non_elementary"]
 
 
 class efm_stats(ctypes.Structure):

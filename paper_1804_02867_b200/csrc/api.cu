@@ -257,6 +257,7 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     h->V = P.max_visited ? P.max_visited : 2 * h->D;
     h->max_loop = P.max_loop ? P.max_loop : 8;
     if (h->D > 4096 || h->max_loop > 65535) { delete h; return EFM_E_INVAL; }
+    if ((P.flags & EFM_F_EXACT_ELEMENTARITY) && h->D > 128) { delete h; return EFM_E_INVAL; }   // the basis of the rank test lives in shared memory
     h->cap = P.sample_count ? 0 : P.frontier_cap;   // a sampled candidate has one descendant at most: nothing to cut
     h->sample_count = P.sample_count; h->sample_seed = P.sample_seed;
     h->device = P.device;
@@ -646,7 +647,8 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         st.poisoned = (int64_t)hc->n_poisoned;
         if (n_uniq_ok > 0) {
             size_t t2 = tm.mark();
-            CK(launch_filter(pa, n_uniq_ok, h->sm_count, s, &launches));
+            if (h->flags & EFM_F_EXACT_ELEMENTARITY) CK(launch_rank_test(pa, n_uniq_ok, h->sm_count, s, &launches));   // 8(f)-3
+            else CK(launch_filter(pa, n_uniq_ok, h->sm_count, s, &launches));
             size_t t3 = tm.mark();
             CK(launch_output_rows(pa, n_uniq_ok, s, &launches));
             CK(read_ctl());
@@ -675,6 +677,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     st.discarded_visited = (int64_t)hc->st[ST_VISITED];
     st.truncated_beam = truncated;
     st.output = (int64_t)n_keep;
+    st.non_elementary = (h->flags & EFM_F_EXACT_ELEMENTARITY) ? (int64_t)n_uniq_ok - (int64_t)n_keep : 0;
     st.algo_bytes = (int64_t)hc->st[ST_ALGO_BYTES];
     st.general_children = (int64_t)hc->st[ST_GENERAL]; st.first_visits = (int64_t)hc->st[ST_FIRST];
     st.materialised = materialised;

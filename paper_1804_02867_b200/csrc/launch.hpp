@@ -40,6 +40,7 @@ struct PostArgs {
 };
 cudaError_t launch_select(const u64* keys, u64* ckeys /*compact buffer*/, u64 max_ckeys, Ctl* ctl, int par /*level set holding n_keys / n_slots*/, u64 cap, u64 max_keys, int sm_count, cudaStream_t s, int* n_launches);
 cudaError_t launch_dedup(const PostArgs& a, u64 n_cand, cudaStream_t s, int* n_launches);
+cudaError_t launch_rank_test(const PostArgs& a, u64 n_uniq, int sm_count, cudaStream_t s, int* n_launches);
 cudaError_t launch_filter(const PostArgs& a, u64 n_uniq, int sm_count, cudaStream_t s, int* n_launches);
 cudaError_t launch_output_rows(const PostArgs& a, u64 n_uniq, cudaStream_t s, int* n_launches);
 cudaError_t launch_output_sort(const PostArgs& a, u64 n_keep, cudaStream_t s, int* n_launches);

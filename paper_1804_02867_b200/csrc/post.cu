@@ -454,6 +454,121 @@ __global__ void __launch_bounds__(kJoinThreads) k_filter_join(const PostArgs a) 
     }
 }
 
+// =================================================================================================================
+// SURVEY.md 8(f)-3  Exact elementarity (Def 3; "recognizing the elementarity through rank
+// test"): a unique, unpoisoned support stays iff the internal rows of S restricted to its arcs have rank |supp| - 1 over
+// GF(p), p = 2^31 - 1 (reading G24).  One warp per support.  The rows (metabolites touched by the support) are
+// never materialised as a matrix: a row is gathered from the columns of the arcs (lane = arc), reduced against the basis
+// kept in shared memory (one vector per pivot column, fraction-free: v <- piv v - v_c b_c) and either vanishes or joins
+// the basis.  The rank of a matrix does not depend on the elimination order, so the result is bit-exact with any other
+// elimination over the same field.
+// =================================================================================================================
+constexpr u32 kRankP = 2147483647u;
+__device__ __forceinline__ u32 mulmod_p(u32 x, u32 y) {
+    u64 t = (u64)x * y;
+    t = (t & kRankP) + (t >> 31);
+    t = (t & kRankP) + (t >> 31);
+    return t >= kRankP ? (u32)(t - kRankP) : (u32)t;
+}
+template <int CH>   // CH chunks of 32 arcs: supports of up to 32 CH arcs
+__global__ void __launch_bounds__(128) k_rank_test(const PostArgs a, u64 K, int warps_per_block) {
+    extern __shared__ u32 rk_smem[];
+    constexpr int N = 32 * CH;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    if (wib >= warps_per_block) return;
+    u32* basis = rk_smem + (size_t)wib * N * N;   // basis[c * N + k]: the vector whose pivot column is c
+    for (u64 u = (u64)blockIdx.x * warps_per_block + wib; u < K; u += (u64)gridDim.x * warps_per_block) {
+        const unsigned char* e = a.cand + (u64)a.uniq[u] * a.cand_stride;
+        const int n = cand_n(e);
+        const u16* arc = cand_arc(e, n);
+        int my_arc[CH];
+#pragma unroll
+        for (int ch = 0; ch < CH; ++ch) my_arc[ch] = lane + 32 * ch < n ? (int)arc[lane + 32 * ch] : -1;
+        u32 has_piv[CH];
+#pragma unroll
+        for (int ch = 0; ch < CH; ++ch) has_piv[ch] = 0;
+        int rank = 0;
+#pragma unroll 1
+        for (int t = 0; t < n && rank < n - 1; ++t) {
+            const int at = arc[t];
+            const int q0 = a.g.col_ptr[at], q1 = a.g.col_ptr[at + 1];
+#pragma unroll 1
+            for (int q = q0; q < q1 && rank < n - 1; ++q) {
+                const int met = col_met(a.g.col[q]);
+                // the row of `met` over the arcs of the support
+                u32 v[CH];
+                bool earlier = false;
+#pragma unroll
+                for (int ch = 0; ch < CH; ++ch) {
+                    v[ch] = 0;
+                    const int am = my_arc[ch];
+                    if (am >= 0 && (((a.g.colsig[2 * am] | a.g.colsig[2 * am + 1]) >> (met & 63)) & 1ULL)) {
+                        for (int r = a.g.col_ptr[am]; r < a.g.col_ptr[am + 1]; ++r) {
+                            const int2 ce = a.g.col[r];
+                            if (col_met(ce) == met) { const long long sv = (long long)ce.y % (long long)kRankP; v[ch] = (u32)(sv < 0 ? sv + kRankP : sv); }
+                        }
+                    }
+                    if (v[ch] != 0 && lane + 32 * ch < t) earlier = true;
+                }
+                if (__any_sync(0xffffffffu, earlier)) continue;   // an arc before t holds this metabolite: its row was taken then
+                // reduce against the basis
+#pragma unroll 1
+                for (;;) {
+                    int c = -1;
+#pragma unroll
+                    for (int ch = CH - 1; ch >= 0; --ch) { const u32 m = __ballot_sync(0xffffffffu, v[ch] != 0); if (m) c = 32 * ch + __ffs(m) - 1; }
+                    if (c < 0) break;   // the row depends on the basis
+                    const bool have = (has_piv[c >> 5] >> (c & 31)) & 1u;
+                    if (!have) {   // a new pivot
+#pragma unroll
+                        for (int ch = 0; ch < CH; ++ch) basis[(size_t)c * N + lane + 32 * ch] = v[ch];
+                        has_piv[c >> 5] |= 1u << (c & 31);
+                        ++rank;
+                        __syncwarp();
+                        break;
+                    }
+                    const u32 piv = basis[(size_t)c * N + c];
+                    u32 vc = 0;
+#pragma unroll
+                    for (int ch = 0; ch < CH; ++ch) { const u32 x = __shfl_sync(0xffffffffu, v[ch], c & 31); if ((c >> 5) == ch) vc = x; }
+#pragma unroll
+                    for (int ch = 0; ch < CH; ++ch) {
+                        const u32 x = mulmod_p(piv, v[ch]), y = mulmod_p(vc, basis[(size_t)c * N + lane + 32 * ch]);
+                        v[ch] = x >= y ? x - y : x + kRankP - y;
+                    }
+                }
+            }
+        }
+        if (lane == 0) a.keep[u] = rank == n - 1 ? 1 : 0;
+        __syncwarp();
+    }
+}
+cudaError_t launch_rank_test(const PostArgs& a, u64 K, int sm_count, cudaStream_t s, int* n_launches) {
+    if (K == 0) return cudaSuccess;
+    const int ch = (a.D + 31) / 32;
+    if (ch > 4) return cudaErrorInvalidValue;   // efm_create refuses the flag for D > 128
+    const size_t per_warp = (size_t)(32 * ch) * (32 * ch) * 4;
+    int wpb = (int)((96 * 1024) / per_warp);
+    wpb = wpb > 4 ? 4 : (wpb < 1 ? 1 : wpb);
+    const size_t smem = per_warp * wpb;
+    u64 blocks = (K + wpb - 1) / wpb;
+    if (blocks > (u64)sm_count * 8) blocks = (u64)sm_count * 8;
+    cudaError_t e = cudaSuccess;
+#define EFM_RANK_LAUNCH(CHN)                                                                                                      \
+    do {                                                                                                                          \
+        e = cudaFuncSetAttribute(k_rank_test<CHN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);                      \
+        if (e == cudaSuccess) k_rank_test<CHN><<<(unsigned)blocks, 128, smem, s>>>(a, K, wpb);                                    \
+    } while (0)
+    if (ch <= 1) EFM_RANK_LAUNCH(1);
+    else if (ch == 2) EFM_RANK_LAUNCH(2);
+    else if (ch == 3) EFM_RANK_LAUNCH(3);
+    else EFM_RANK_LAUNCH(4);
+#undef EFM_RANK_LAUNCH
+    if (e != cudaSuccess) return e;
+    ++*n_launches;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_filter(const PostArgs& a, u64 K, int sm_count, cudaStream_t s, int* n_launches) {
     cudaError_t e;
     if ((e = cudaMemsetAsync(a.freq, 0, sizeof(u32) * (a.g.A + 2), s)) != cudaSuccess) return e;

@@ -36,7 +36,10 @@ def assert_parity(efm, oracle_mod, net, seeds="net", flags=0, check_levels=True,
     got = efm.enumerate_network(net, seed_sets=seeds, flags=flags, allowed=allowed, **over)
     okeys = {k: v for k, v in over.items() if k in ("max_support", "max_loop", "dep_depth", "max_visited", "frontier_cap",
                                                     "sample_count", "sample_seed")}
-    ref = oracle_mod.enumerate_network(net, threads=_threads(oracle_mod), seed_sets=seeds, self_check=False, allowed=allowed, **okeys)
+    exact = bool(flags & efm.EFM_F_EXACT_ELEMENTARITY)
+    ref = oracle_mod.enumerate_network(net, threads=_threads(oracle_mod), seed_sets=seeds, self_check=False, allowed=allowed,
+                                       exact=exact, **okeys)
+    assert int(got.stats["non_elementary"]) == int(ref.stats["non_elementary"])
     for k in STAT_KEYS:
         assert int(got.stats[k]) == int(ref.stats[k]), (k, got.stats[k], ref.stats[k])
     if check_levels:
@@ -478,3 +481,33 @@ def test_bench_headline_configuration_sampled(efm):
     assert np.all(lv["expanded"] <= cap) and int(lv["expanded"].max()) > 0.9 * cap
     assert int(st["truncated_beam"]) == int(lv["active"].sum() - lv["expanded"].sum())
     en.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f)-3 exact elementarity on the device
+# ---------------------------------------------------------------------------------------------------------------------
+def test_exact_elementarity_by_hand(efm):
+    """H7 network, derived by hand in tests/test_oracle_modes.py: the balanced pathway (2,2,2,1) over all four reactions has
+    nullity 2 (it is the sum of two EFMs) and goes; (1,1,0,0) and (0,0,2,1) stay.  No oracle involved."""
+    net = hand_network([({}, {"A": 1}, False), ({"A": 1}, {}, False), ({}, {"B": 1}, False), ({"B": 2}, {}, False)], ["A", "B"])
+    assert efm.enumerate_network(net, seed_sets=[[0, 4]]).flux.tolist() == [[2, 2, 2, 1]]
+    r = efm.enumerate_network(net, seed_sets=[[0, 4]], flags=efm.EFM_F_EXACT_ELEMENTARITY)
+    assert r.flux.tolist() == [] and r.stats["non_elementary"] == 1
+    r = efm.enumerate_network(net, seed_sets=[[0, 4], [0], [4]], flags=efm.EFM_F_EXACT_ELEMENTARITY)
+    assert r.flux.tolist() == [[0, 0, 2, 1], [1, 1, 0, 0]] and r.stats["non_elementary"] == 1
+
+
+@pytest.mark.parametrize("name,over,count", [("toy", {}, 0), ("small", {}, 150), ("core", dict(frontier_cap=4096), 150),
+                                             ("mid", dict(frontier_cap=4096), 300), ("genome", dict(frontier_cap=4096), 300),
+                                             ("genome", dict(frontier_cap=16384), 0)])
+def test_exact_elementarity(efm, oracle_mod, name, over, count):
+    """Rank test instead of the pairwise filter: same pathways as the oracle's plain Gaussian elimination over the same
+    field (supports of 1 to 60 arcs, one to two chunks of 32 lanes); with multi-arc seed sets the test rejects candidates."""
+    net = make_network(name, 0)
+    seeds = random_seed_sets(net, count, 2, 11) if count else "net"
+    got, ref = assert_parity(efm, oracle_mod, net, seeds=seeds, flags=efm.EFM_F_EXACT_ELEMENTARITY, **over)
+    if count:
+        assert int(got.stats["non_elementary"]) > 0
+    if net.n_arcs > 129:   # the basis of the rank test lives in shared memory: supports of at most 128 arcs
+        with pytest.raises(efm.EfmError):
+            efm.Enumerator(net.S, net.reversible, net.internal, dict(net.params, max_support=129), flags=efm.EFM_F_EXACT_ELEMENTARITY)
