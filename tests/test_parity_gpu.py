@@ -283,6 +283,8 @@ def test_degenerate_inputs(efm, oracle_mod):
     net0 = hand_network([({"X": 1}, {"Y": 2}, True)], [])
     got = efm.enumerate_network(net0)
     assert got.n_out == 0 and got.stats["levels"] == 0
+    for k in ("expanded", "children", "done", "dead_end", "algo_bytes", "unique_supports", "launches"):
+        assert int(got.stats[k]) == 0, k          # no roots: nothing ran, nothing stale is reported
     got = efm.enumerate_network(net0, seed_sets=[[0], [1]])
     assert got.flux.tolist() == [[-1], [1]]
     # capacity errors are reported, never silently truncated
