@@ -1086,20 +1086,40 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
         const int qa0 = pcol0, qa1 = pcol1;
         int wbase = 0;
         u32 seen = 0;   // bit q - qa0: metabolite of col(a)[q] is in the parent's list (columns longer than 32: see below)
+        const int nc = qa1 - qa0;
+        // the column of the arc in registers (up to six entries, the usual case): an element of the parent's list meets it
+        // with compares only, and which column entries were met is one group-wide OR at the end
+        int cm[6]; i64 cs[6];
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            cm[q] = -2; cs[q] = 0;
+            if (q < nc && nc <= 6) { const int2 e = __ldg(&A.g.col[qa0 + q]); cm[q] = col_met(e); cs[q] = (i64)e.y; }
+        }
         for (int t0 = 0; t0 < nu; t0 += G) {
             const int t = t0 + lane;
             const bool valid = t < nu;
             i64 x = 0;
             int met = -1;
-            if (valid) {
-                met = t0 == 0 ? (int)pm0 : (int)efmet[t];
+            if (nc <= 6) {
                 i64 s = 0;
-                for (int qq = qa0; qq < qa1; ++qq) { const int2 e = __ldg(&A.g.col[qq]); if (col_met(e) == met) s = e.y; }
-                x = (i64)(ck * (u64)(t0 == 0 ? pe0 : ef[t]) + sd * (u64)s);
-                if (cg > 1) x = sdiv64(x, (i64)cg);
+                if (valid) met = t0 == 0 ? (int)pm0 : (int)efmet[t];
+#pragma unroll
+                for (int q = 0; q < 6; ++q) if (met == cm[q]) { s = cs[q]; seen |= 1u << q; }
+                if (valid) {
+                    x = (i64)(ck * (u64)(t0 == 0 ? pe0 : ef[t]) + sd * (u64)s);
+                    if (cg > 1) x = sdiv64(x, (i64)cg);
+                }
+            } else {
+                if (valid) {
+                    met = t0 == 0 ? (int)pm0 : (int)efmet[t];
+                    i64 s = 0;
+                    for (int qq = qa0; qq < qa1; ++qq) { const int2 e = __ldg(&A.g.col[qq]); if (col_met(e) == met) s = e.y; }
+                    x = (i64)(ck * (u64)(t0 == 0 ? pe0 : ef[t]) + sd * (u64)s);
+                    if (cg > 1) x = sdiv64(x, (i64)cg);
+                }
+                for (int qq = qa0; qq < qa1 && qq < qa0 + 32; ++qq)
+                    if (gany(valid && col_met(__ldg(&A.g.col[qq])) == met)) seen |= 1u << (qq - qa0);
             }
-            for (int qq = qa0; qq < qa1 && qq < qa0 + 32; ++qq)
-                if (gany(valid && col_met(__ldg(&A.g.col[qq])) == met)) seen |= 1u << (qq - qa0);
             const u32 nz = gballot(valid && x != 0);
             if (valid && x != 0) {
                 const int pos = wbase + __popc(nz & lt);
@@ -1110,6 +1130,7 @@ __global__ void __launch_bounds__(kMatThreads, EFM_MAT_BLOCKS) k_materialise(con
             }
             wbase += __popc(nz);
         }
+        if (nc <= 6) seen = __reduce_or_sync(gmask, seen);   // the lanes noted their own matches
         for (int qq = qa0; qq < qa1; ++qq) {   // warp-uniform, a handful of entries
             const int2 e = __ldg(&A.g.col[qq]);
             const int emet = col_met(e);

@@ -351,7 +351,7 @@ def test_bench_configuration_properties(efm):
     assert np.all(np.gcd.reduce(np.where(mask, np.abs(val), 0), axis=1) == 1)
     # strict lexicographic order on sampled neighbours
     rng = np.random.default_rng(0)
-    for r in rng.choice(K - 1, 3000, replace=False):
+    for r in rng.choice(K - 1, 1000, replace=False):
         a, b = V[r].toarray()[0], V[r + 1].toarray()[0]
         d = np.nonzero(a != b)[0]
         assert d.size and a[d[0]] < b[d[0]], r
@@ -359,7 +359,7 @@ def test_bench_configuration_properties(efm):
     arcs = np.where(val[mask] > 0, rxn[mask], rxn[mask] + n)
     B = sp.csr_matrix((np.ones(arcs.size, np.int32), (rows, arcs)), shape=(K, 2 * n))
     size = np.asarray(B.sum(axis=1)).ravel()
-    for r in rng.choice(K, 400, replace=False):
+    for r in rng.choice(K, 150, replace=False):
         shared = np.asarray((B @ B[r].T).todense()).ravel()
         inside = (shared == size) & (size < size[r])
         assert not inside.any(), (r, int(np.nonzero(inside)[0][0]))
