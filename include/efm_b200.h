@@ -47,6 +47,10 @@ extern "C" {
                                 /* of Def 3: a support stays iff the internal rows of S restricted */
                                 /* to it have rank |supp| - 1 over GF(2^31 - 1); needs max_support <= 128               */
 
+#define EFM_F_COMPRESS 0x20u    /* SURVEY.md 8(f)-4 compression pre-pass: efm_create() leaves the reactions    */
+                                /* out of the graph that efm_blocked_reactions() reports; results stay in the caller's     */
+                                /* reaction space; a seed on such a reaction is EFM_E_INVAL                                 */
+
 typedef struct efm_handle efm_handle; /* opaque: host copy of the graph + pointers INTO the workspace */
 
 /* Traversal parameters.  Alg 1's #defines M, R are taken from S; C (number of
@@ -99,6 +103,7 @@ typedef struct {
     /* work profile of the expansion: first-visit parents, children through the general routine, children materialised */
     int64_t first_visits, general_children, materialised;
     int64_t non_elementary; /* EFM_F_EXACT_ELEMENTARITY: unique, unpoisoned supports the rank test rejected          */
+    int64_t blocked_reactions; /* EFM_F_COMPRESS: reactions left out of the graph                                    */
 } efm_stats;
 
 /* Build the modified AND/OR graph MG (Defs 4-6; "Convert the given matrix to the MG
@@ -114,6 +119,16 @@ typedef struct {
  * negative parameters. */
 int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const uint8_t* reversible,
                const uint8_t* internal, const efm_params* p, efm_handle** out);
+
+/* Compression pre-pass ("partitioning and compression preprocessing methods"): the reactions
+ * that cannot carry flux in any steady state (Def 2) for a topological reason.  An internal metabolite whose
+ * remaining reactions offer no pair (one that can produce it, another one that can consume it) forces all of them to
+ * zero; they are removed and the rule is iterated to its fixed point.  Host only, no handle needed.
+ *   S, m, n, row_stride, reversible, internal   as for efm_create()
+ *   blocked    host, uint8[n] out: 1 = blocked
+ *   n_blocked  host out (may be NULL) */
+int efm_blocked_reactions(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const uint8_t* reversible,
+                          const uint8_t* internal, uint8_t* blocked, int32_t* n_blocked);
 
 /* Sizes of the graph: internal metabolites M, arcs A, 64-bit bitset words W = ceil(A/64), nonzeros of the
  * internal arc columns, entries of the dependency table (sum over nodes of |O| * |I|).  All host. */

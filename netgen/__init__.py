@@ -15,4 +15,5 @@ from .networks import (  # noqa: F401
     mirrored,
     random_seed_sets,
     unimolecular_network,
+    with_dead_ends,
 )

@@ -588,3 +588,30 @@ def mirrored(net: Network) -> Network:
     return Network(net.name + "-mirrored", net.seed, np.ascontiguousarray(-net.S), net.reversible.copy(),
                    net.internal.copy(), dict(net.params), None if net.seed_sets is None else [list(s) for s in net.seed_sets],
                    dict(net.info))
+
+
+def with_dead_ends(net: Network, count: int, seed: int = 0) -> Network:
+    """``net`` plus ``count`` dead-end branches: an internal metabolite X feeds a chain X -> D1 -> D2 whose last metabolite
+    nothing consumes (every second branch has a reversible first step).  No steady state can use these reactions; the
+    compression pre-pass removes them by cascade, the traversal without it wastes expansions on them."""
+    rng = SplitMix64((seed * 0x9E3779B97F4A7C15 + 0x64656164) & MASK64)
+    m, n = net.S.shape
+    internal_rows = [i for i in range(m) if net.internal[i]]
+    S = np.zeros((m + 2 * count, n + 2 * count), dtype=np.int32)
+    S[:m, :n] = net.S
+    rev = np.concatenate([net.reversible, np.zeros(2 * count, dtype=np.uint8)])
+    internal = np.concatenate([net.internal, np.ones(2 * count, dtype=np.uint8)])
+    for b in range(count):
+        x = internal_rows[rng.below(len(internal_rows))]
+        d1, d2 = m + 2 * b, m + 2 * b + 1
+        j1, j2 = n + 2 * b, n + 2 * b + 1
+        S[x, j1] = -1; S[d1, j1] = 1 + b % 2
+        S[d1, j2] = -1; S[d2, j2] = 1
+        rev[j1] = b % 2
+    A = int(S.shape[1] + rev.sum())
+    p = dict(net.params)
+    if net.params.get("max_support", 0) >= net.n_arcs:
+        p["max_support"] = A
+        p["max_visited"] = 2 * A
+    return Network(net.name + f"-deadends{count}", net.seed, S, rev, internal, p,
+                   None if net.seed_sets is None else [list(s) for s in net.seed_sets], dict(net.info))

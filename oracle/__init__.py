@@ -101,6 +101,7 @@ class OracleResult:
     trace: Optional[List[List[dict]]] = None
     steps: Optional[np.ndarray] = None      # per output row: expansions that built the pathway
     cand_end: Optional[np.ndarray] = None   # sampling mode (8(f)-1): per candidate (code, steps); codes in END_CODES
+    blocked: Optional[np.ndarray] = None    # enumerate_compressed: reactions the pre-pass removed
 
 
 def _ptr(a: np.ndarray):
@@ -219,6 +220,32 @@ def enumerate_network(net, threads: int = 1, shuffle_seed: int = 0, export_graph
     seeds = net.seed_sets if isinstance(seed_sets, str) else seed_sets
     return enumerate_pathways(net.S, net.reversible, net.internal, params, seeds, threads, shuffle_seed,
                               export_graph, self_check, trace, sample_count, sample_seed, allowed, exact)
+
+
+def enumerate_compressed(S: np.ndarray, reversible: np.ndarray, internal: np.ndarray, params: Dict[str, int],
+                         seed_sets: Optional[Sequence[Sequence[int]]] = None, **kw) -> OracleResult:
+    """the traversal after the compression pre-pass of oracle/compress.py.  The blocked reactions are
+    removed from S (the arcs of the others are numbered consecutively, as always), seed codes are renumbered, and the
+    pathways are returned in the caller's reaction space (zero on the removed reactions)."""
+    from .compress import blocked_reactions
+    S = np.asarray(S)
+    blocked = blocked_reactions(S, reversible, internal)
+    keep = np.nonzero(~blocked)[0]
+    new_id = -np.ones(S.shape[1], dtype=np.int64)
+    new_id[keep] = np.arange(len(keep))
+    seeds = None
+    if seed_sets:
+        seeds = []
+        for st in seed_sets:
+            if any(blocked[c // 2] for c in st):
+                raise ValueError("seed on a blocked reaction")
+            seeds.append([int(2 * new_id[c // 2] + (c & 1)) for c in st])
+    res = enumerate_pathways(np.ascontiguousarray(S[:, keep]), np.asarray(reversible)[keep], internal, params, seeds, **kw)
+    full = np.zeros((res.flux.shape[0], S.shape[1]), dtype=np.int64)
+    full[:, keep] = res.flux
+    res.flux = full
+    res.blocked = blocked
+    return res
 
 
 def state_hash(arcs: Sequence[int], fluxes: Sequence[int], visited: Sequence[Sequence[int]]) -> int:

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libefm_b200.so")
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "efm_b200.h")
 
 EFM_OK, EFM_E_INVAL, EFM_E_NOMEM, EFM_E_CAPACITY, EFM_E_CUDA, EFM_E_STATE = 0, -1, -2, -3, -4, -5
-EFM_F_TIMING, EFM_F_NO_FASTPATH, EFM_F_NO_STAGING, EFM_F_EXACT_ELEMENTARITY = 0x1, 0x4, 0x8, 0x10
+EFM_F_TIMING, EFM_F_NO_FASTPATH, EFM_F_NO_STAGING, EFM_F_EXACT_ELEMENTARITY, EFM_F_COMPRESS = 0x1, 0x4, 0x8, 0x10, 0x20
 
 
 class efm_params(ctypes.Structure):
@@ -37,7 +37,7 @@ _STAT_INT = ["levels", "expanded", "children", "done", "dead_end", "not_efm_maxl
              "host_syncs"]
 _STAT_MS = ["ms_build", "ms_total", "ms_order", "ms_expand_count", "ms_beam", "ms_expand_write", "ms_hash",
             "ms_filter", "ms_output"]
-_STAT_INT2 = ["n_expand_count", "filter_pairs", "first_visits", "general_children", "materialised", "non_elementary"]
+_STAT_INT2 = ["n_expand_count", "filter_pairs", "first_visits", "general_children", "materialised", "non_elementary", "blocked_reactions"]
 
 
 class efm_stats(ctypes.Structure):
@@ -66,6 +66,7 @@ def load() -> ctypes.CDLL:
     vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
     P = ctypes.POINTER
     lib.efm_create.argtypes = [vp, i32, i32, i64, vp, vp, P(efm_params), P(vp)]
+    lib.efm_blocked_reactions.argtypes = [vp, i32, i32, i64, vp, vp, vp, P(i32)]
     lib.efm_graph_info.argtypes = [vp, P(i32), P(i32), P(i32), P(i64), P(i64)]
     lib.efm_graph_export.argtypes = [vp] + [vp] * 14
     lib.efm_workspace_bytes.argtypes = [vp, P(sz)]
@@ -294,6 +295,21 @@ def enumerate_network(net, device: int = 0, flags: int = 0, seed_sets="net", den
         return en.enumerate(seeds, dense=dense)
     finally:
         en.close()
+
+
+def blocked_reactions(S: np.ndarray, reversible: np.ndarray, internal: np.ndarray) -> np.ndarray:
+    """Compression pre-pass (``efm_blocked_reactions``): boolean mask of the reactions that cannot carry steady-state flux."""
+    lib = load()
+    S = np.ascontiguousarray(S, dtype=np.int32)
+    m, n = S.shape
+    rev = np.ascontiguousarray(reversible, dtype=np.uint8)
+    internal = np.ascontiguousarray(internal, dtype=np.uint8)
+    out = np.zeros(n, dtype=np.uint8)
+    nb = ctypes.c_int32()
+    rc = lib.efm_blocked_reactions(_ptr(S), m, n, n, _ptr(rev), _ptr(internal), _ptr(out), ctypes.byref(nb))
+    if rc != EFM_OK:
+        raise EfmError(rc, lib.efm_strerror(rc).decode())
+    return out.astype(bool)
 
 
 def debug_state_hash(arcs: Sequence[int], fluxes: Sequence[int], visited: Sequence[Sequence[int]], device: int = 0) -> int:

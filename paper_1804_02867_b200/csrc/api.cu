@@ -37,6 +37,7 @@ struct efm_handle {
     HostGraph G;
     int32_t D = 0, V = 0, max_loop = 8, L = 4;
     int64_t sample_count = 0; uint64_t sample_seed = 0;
+    int32_t n_blocked = 0;   // EFM_F_COMPRESS: reactions left out of the graph
     std::vector<uint32_t> amask;   // bit per arc, empty = no restriction (efm_set_reaction_mask)
     int64_t cap = 0, max_frontier = 0, max_cand = 0, max_keys = 0, max_tasks = 0, max_ckeys = 0, max_surv = 0, max_levels = 0;
     int32_t device = 0;
@@ -248,7 +249,13 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     memset(&h->stats, 0, sizeof h->stats);
     const auto c0 = std::chrono::steady_clock::now();
     h->L = P.dep_depth ? P.dep_depth : 4;
-    int rc = build_graph(h->G, S, m, n, row_stride, reversible, internal, h->L);
+    if (!S || !reversible || !internal || m <= 0 || n <= 0 || row_stride < n) { delete h; return EFM_E_INVAL; }
+    std::vector<uint8_t> skip;
+    if (P.flags & EFM_F_COMPRESS) {   // blocked reactions get no arcs
+        skip.assign((size_t)n, 0);
+        h->n_blocked = blocked_reactions(S, m, n, row_stride, reversible, internal, skip.data());
+    }
+    int rc = build_graph(h->G, S, m, n, row_stride, reversible, internal, h->L, skip.empty() ? nullptr : skip.data());
     if (rc != EFM_OK) { delete h; return rc; }
     h->ms_build = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - c0).count();   // wall time
     const HostGraph& G = h->G;
@@ -307,6 +314,14 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
     h->dense_bytes = std::max<size_t>((size_t)64 << 20, (size_t)n * 8 * 64);
     make_layout(h);
     *out = h;
+    return EFM_OK;
+}
+
+int efm_blocked_reactions(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const uint8_t* reversible,
+                          const uint8_t* internal, uint8_t* blocked, int32_t* n_blocked) {
+    if (!S || !reversible || !internal || !blocked || m <= 0 || n <= 0 || row_stride < n) return EFM_E_INVAL;
+    const int32_t nb = blocked_reactions(S, m, n, row_stride, reversible, internal, blocked);
+    if (n_blocked) *n_blocked = nb;
     return EFM_OK;
 }
 
@@ -677,6 +692,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     st.discarded_visited = (int64_t)hc->st[ST_VISITED];
     st.truncated_beam = truncated;
     st.output = (int64_t)n_keep;
+    st.blocked_reactions = h->n_blocked;
     st.non_elementary = (h->flags & EFM_F_EXACT_ELEMENTARITY) ? (int64_t)n_uniq_ok - (int64_t)n_keep : 0;
     st.algo_bytes = (int64_t)hc->st[ST_ALGO_BYTES];
     st.general_children = (int64_t)hc->st[ST_GENERAL]; st.first_visits = (int64_t)hc->st[ST_FIRST];

@@ -8,8 +8,51 @@
 
 namespace efm {
 
+int32_t blocked_reactions(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const uint8_t* reversible,
+                          const uint8_t* internal, uint8_t* blocked) {
+    // sparse rows of the internal metabolites; a work list of the metabolites whose reactions changed
+    std::vector<std::vector<int32_t>> row((size_t)m);
+    std::vector<std::vector<int32_t>> col((size_t)n);
+    for (int32_t i = 0; i < m; ++i) {
+        if (!internal[i]) continue;
+        const int32_t* r = S + (int64_t)i * row_stride;
+        for (int32_t j = 0; j < n; ++j)
+            if (r[j] != 0) { row[i].push_back(j); col[j].push_back(i); }
+    }
+    std::fill(blocked, blocked + n, (uint8_t)0);
+    std::vector<int32_t> work;
+    std::vector<char> queued((size_t)m, 0);
+    for (int32_t i = 0; i < m; ++i) if (internal[i] && !row[i].empty()) { work.push_back(i); queued[i] = 1; }
+    int32_t n_blocked = 0;
+    while (!work.empty()) {
+        const int32_t i = work.back();
+        work.pop_back();
+        queued[i] = 0;
+        // first two distinct reactions that can produce / consume i: a pair of different reactions exists iff
+        // both sides are non-empty and they are not one and the same single reaction
+        int32_t p0 = -1, p1 = -1, c0 = -1, c1 = -1, touching = 0;
+        const int32_t* r = S + (int64_t)i * row_stride;
+        for (int32_t j : row[i]) {
+            if (blocked[j]) continue;
+            ++touching;
+            if (r[j] > 0 || reversible[j]) { if (p0 < 0) p0 = j; else if (p1 < 0) p1 = j; }
+            if (r[j] < 0 || reversible[j]) { if (c0 < 0) c0 = j; else if (c1 < 0) c1 = j; }
+        }
+        if (touching == 0) continue;
+        const bool ok = p0 >= 0 && c0 >= 0 && (p1 >= 0 || c1 >= 0 || p0 != c0);
+        if (ok) continue;
+        for (int32_t j : row[i]) {
+            if (blocked[j]) continue;
+            blocked[j] = 1;
+            ++n_blocked;
+            for (int32_t i2 : col[j]) if (i2 != i && !queued[i2]) { work.push_back(i2); queued[i2] = 1; }
+        }
+    }
+    return n_blocked;
+}
+
 int build_graph(HostGraph& G, const int32_t* S, int32_t m, int32_t n, int64_t row_stride,
-                const uint8_t* reversible, const uint8_t* internal, int32_t dep_depth) {
+                const uint8_t* reversible, const uint8_t* internal, int32_t dep_depth, const uint8_t* skip_rxn) {
     if (!S || !reversible || !internal || m <= 0 || n <= 0 || row_stride < n || dep_depth < 1) return EFM_E_INVAL;
     G = HostGraph();
     G.m = m;
@@ -22,6 +65,7 @@ int build_graph(HostGraph& G, const int32_t* S, int32_t m, int32_t n, int64_t ro
     // reaction for reversible reactions").
     G.code2arc.assign((size_t)2 * n, -1);
     for (int32_t j = 0; j < n; ++j) {
+        if (skip_rxn && skip_rxn[j]) continue;   // compression pre-pass: a blocked reaction gets no arcs
         int32_t fwd = (int32_t)G.arc_rxn.size();
         G.arc_rxn.push_back(j);
         G.arc_dir.push_back(+1);

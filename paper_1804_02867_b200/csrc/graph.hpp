@@ -37,8 +37,15 @@ struct HostGraph {
     }
 };
 
-// Returns 0 or a negative EFM_E_* code.
+// Returns 0 or a negative EFM_E_* code.  skip_rxn (may be null): reactions left out of the graph (no arcs are made for them;
+// the arcs of the others keep the ORIGINAL reaction index in arc_rxn, so results stay in the caller's reaction space).
 int build_graph(HostGraph& G, const int32_t* S, int32_t m, int32_t n, int64_t row_stride,
-                const uint8_t* reversible, const uint8_t* internal, int32_t dep_depth);
+                const uint8_t* reversible, const uint8_t* internal, int32_t dep_depth, const uint8_t* skip_rxn = nullptr);
+
+// SURVEY.md 8(f)-4 compression pre-pass: reactions that cannot carry flux in any steady state for a
+// topological reason.  An internal metabolite whose remaining reactions offer no pair (producer, consumer) of two different
+// reactions forces all of them to zero; iterated to the fixed point.  blocked[n] out; returns the number blocked.
+int32_t blocked_reactions(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const uint8_t* reversible,
+                          const uint8_t* internal, uint8_t* blocked);
 
 }  // namespace efm

@@ -7,7 +7,7 @@ import os
 import numpy as np
 import pytest
 
-from netgen import hand_network, make_network, random_seed_sets, unimolecular_network
+from netgen import hand_network, make_network, random_seed_sets, unimolecular_network, with_dead_ends
 
 pytestmark = pytest.mark.gpu
 
@@ -37,8 +37,16 @@ def assert_parity(efm, oracle_mod, net, seeds="net", flags=0, check_levels=True,
     okeys = {k: v for k, v in over.items() if k in ("max_support", "max_loop", "dep_depth", "max_visited", "frontier_cap",
                                                     "sample_count", "sample_seed")}
     exact = bool(flags & efm.EFM_F_EXACT_ELEMENTARITY)
-    ref = oracle_mod.enumerate_network(net, threads=_threads(oracle_mod), seed_sets=seeds, self_check=False, allowed=allowed,
-                                       exact=exact, **okeys)
+    if flags & efm.EFM_F_COMPRESS:   # 8(f)-4: the oracle runs on the network its own pre-pass reduced
+        params = dict(net.params)
+        params.update(okeys)
+        ref = oracle_mod.enumerate_compressed(net.S, net.reversible, net.internal, params,
+                                              net.seed_sets if isinstance(seeds, str) else seeds, threads=_threads(oracle_mod),
+                                              self_check=False, exact=exact)
+        assert int(got.stats["blocked_reactions"]) == int(ref.blocked.sum())
+    else:
+        ref = oracle_mod.enumerate_network(net, threads=_threads(oracle_mod), seed_sets=seeds, self_check=False, allowed=allowed,
+                                           exact=exact, **okeys)
     assert int(got.stats["non_elementary"]) == int(ref.stats["non_elementary"])
     for k in STAT_KEYS:
         assert int(got.stats[k]) == int(ref.stats[k]), (k, got.stats[k], ref.stats[k])
@@ -513,3 +521,23 @@ def test_exact_elementarity(efm, oracle_mod, name, over, count):
     if net.n_arcs > 129:   # the basis of the rank test lives in shared memory: supports of at most 128 arcs
         with pytest.raises(efm.EfmError):
             efm.Enumerator(net.S, net.reversible, net.internal, dict(net.params, max_support=129), flags=efm.EFM_F_EXACT_ELEMENTARITY)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f)-4 compression pre-pass
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,branches,over", [("toy", 3, {}), ("small", 4, {}), ("core", 12, dict(frontier_cap=4096)),
+                                                ("genome", 200, dict(frontier_cap=4096))])
+def test_compression_prepass(efm, oracle_mod, name, branches, over):
+    """Networks with dead-end branches: with EFM_F_COMPRESS the library leaves the blocked reactions out of the graph and
+    agrees with the oracle run on the network its own pre-pass reduced; results stay in the caller's reaction space."""
+    net = with_dead_ends(make_network(name, 0), branches, 5)
+    got, ref = assert_parity(efm, oracle_mod, net, flags=efm.EFM_F_COMPRESS, **over)
+    assert int(got.stats["blocked_reactions"]) >= 2 * branches
+    assert got.flux.shape[1] == net.S.shape[1] and not got.flux[:, -2 * branches:].any()
+    plain = efm.enumerate_network(net, **over)
+    assert int(plain.stats["blocked_reactions"]) == 0
+    if not over:   # no beam: the pathways found do not depend on the pre-pass, the work does
+        assert np.array_equal(plain.flux, got.flux) and int(got.stats["expanded"]) < int(plain.stats["expanded"])
+    with pytest.raises(efm.EfmError):   # a seed on a removed reaction is refused
+        efm.enumerate_network(net, flags=efm.EFM_F_COMPRESS, seed_sets=[[2 * (net.S.shape[1] - 1)]], **over)
