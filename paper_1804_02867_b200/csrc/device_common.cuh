@@ -189,7 +189,10 @@ enum { TF_NEG = 1, TF_FIRST = 2, TF_INSUPP = 4 };   // task flags: bump subtract
 constexpr int kTagParentShift = 34;
 enum { TK_FAST = 0, TK_TASK = 1 };
 constexpr u64 kKeySentinel = ~0ULL;   // filler of reserved but unused key slots: never < X, skipped by the select
-constexpr u32 kKeyChunk = 64;         // key slots a warp reserves per atomic
+#ifndef EFM_KEYCHUNK
+#define EFM_KEYCHUNK 64
+#endif
+constexpr u32 kKeyChunk = EFM_KEYCHUNK;   // key slots a warp reserves per atomic
 
 #define EFM_GUARD (1ULL << 62)   // reading G21: any state integer above 2^62 discards the pathway
 

@@ -35,7 +35,7 @@ enum { CH_OK = 0, CH_NONPOS = 1, CH_OVERFLOW = 2 };
 constexpr int kParentsPerItem = EFM_PPI;     // first-visit parents a warp takes per work item
 constexpr int kRevisitPerItem = EFM_RPI;    // revisit parents a warp takes per work item (four at a time)
 #ifndef EFM_STAGE_BYTES
-#define EFM_STAGE_BYTES 1536
+#define EFM_STAGE_BYTES 1024
 #endif
 constexpr int kStageBytes = EFM_STAGE_BYTES;   // staging buffer per parent (larger entries are read in place)
 constexpr u32 FULL = 0xffffffffu;
