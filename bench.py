@@ -47,6 +47,8 @@ def sized_params(params, cap, max_candidates=None):
         p["max_frontier_bytes"] = 1792 * cap      # packed entries average about 1 KB
         p["max_child_keys"] = 48 * cap            # about 17 children are evaluated per parent on average, 25 on the widest levels
     return p
+WORKLOAD_TEXT = ("{name}-seed{{rank}} (BASELINE.json configs[4]: 1000+150 metabolites, 2000 reactions, 30% reversible, depth cap 60, "
+                 "8 target exchange reactions)")
 METRIC = "partial_pathways_expanded_per_sec"
 UNIT = "expanded/s"
 
@@ -156,8 +158,7 @@ def main_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1000.0 * t_sum / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-            "config": {"workload": f"{args.workload}-seed0 (BASELINE.json configs[4])", "frontier_cap": args.cap,
-                       "reference_sample_cap": cap},
+            "config": {"workload": WORKLOAD_TEXT.format(name=args.workload), "frontier_cap": args.cap, "reference_sample_cap": cap},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "extra": {"efms_per_s": outs * args.steps / t_sum}}
@@ -352,8 +353,7 @@ def main_ours(args):
         line = {"metric": METRIC, "value": expanded_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-                "config": {"workload": f"{args.workload}-seed{{rank}} (BASELINE.json configs[4]: 1000+150 metabolites, 2000 reactions, "
-                                       "30% reversible, depth cap 60, 8 target exchange reactions)",
+                "config": {"workload": WORKLOAD_TEXT.format(name=args.workload),
                            "frontier_cap": args.cap, "fallback": fallback_note, "workspace_bytes": int(ws_bytes),
                            "params": {k: int(v) for k, v in params.items()},
                            "l2": "flushed between timed iterations (256 MiB write)", "parallelism": f"replicas x{world}"},
