@@ -541,3 +541,54 @@ def test_compression_prepass(efm, oracle_mod, name, branches, over):
         assert np.array_equal(plain.flux, got.flux) and int(got.stats["expanded"]) < int(plain.stats["expanded"])
     with pytest.raises(efm.EfmError):   # a seed on a removed reaction is refused
         efm.enumerate_network(net, flags=efm.EFM_F_COMPRESS, seed_sets=[[2 * (net.S.shape[1] - 1)]], **over)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# differential test on random small networks: every mode, random parameters
+# ---------------------------------------------------------------------------------------------------------------------
+def _random_network(rng):
+    m_int, m_ext, n = int(rng.integers(2, 9)), int(rng.integers(1, 4)), int(rng.integers(4, 15))
+    m = m_int + m_ext
+    S = np.zeros((m, n), dtype=np.int32)
+    for j in range(n):
+        rows = rng.choice(m, size=int(rng.integers(1, min(m, 4) + 1)), replace=False)
+        for i in rows:
+            S[i, j] = int(rng.choice([-3, -2, -1, -1, -1, 1, 1, 1, 2, 3]))
+    rev = (rng.random(n) < 0.3).astype(np.uint8)
+    internal = np.array([1] * m_int + [0] * m_ext, dtype=np.uint8)
+    perm = rng.permutation(m)
+    return S[perm], rev, internal[perm]
+
+
+def test_random_small_networks_in_every_mode(efm, oracle_mod):
+    """150 random networks (2-8 internal metabolites, 4-14 reactions, coefficients up to 3, random reversibility) with random
+    parameters, seeds and modes (beam, sampling, reaction mask, exact elementarity, general routine only, no staging):
+    the CUDA path and the oracle agree on pathways, steps and every counter."""
+    from netgen.networks import Network
+    rng = np.random.default_rng(2024)
+    ran = {"beam": 0, "sample": 0, "mask": 0, "exact": 0, "outputs": 0}
+    for t in range(150):
+        S, rev, internal = _random_network(rng)
+        A = int(S.shape[1] + rev.sum())
+        D = int(rng.integers(2, A + 1))
+        params = dict(max_support=D, max_loop=int(rng.integers(1, 9)), dep_depth=int(rng.integers(1, 6)),
+                      max_visited=int(rng.integers(1, 2 * D + 1)), frontier_cap=0)
+        net = Network(f"random-{t}", t, S, rev, internal, params, None, {})
+        mode = t % 5
+        over, flags, allowed = {}, 0, None
+        seeds = oracle_mod.all_arc_seed_sets(rev) if t % 2 else "net"
+        if mode == 1:
+            over["frontier_cap"] = int(rng.integers(1, 40)); ran["beam"] += 1
+        elif mode == 2:
+            over.update(sample_count=int(rng.integers(1, 60)), sample_seed=int(rng.integers(0, 1 << 30))); ran["sample"] += 1
+        elif mode == 3:
+            allowed = (rng.random(S.shape[1]) < 0.8).astype(np.uint8); ran["mask"] += 1
+        elif mode == 4:
+            flags |= efm.EFM_F_EXACT_ELEMENTARITY; ran["exact"] += 1
+        if t % 7 == 0:
+            flags |= efm.EFM_F_NO_FASTPATH
+        if t % 11 == 0:
+            flags |= efm.EFM_F_NO_STAGING
+        got, ref = assert_parity(efm, oracle_mod, net, seeds=seeds, flags=flags, allowed=allowed, **over)
+        ran["outputs"] += got.n_out
+    assert min(ran["beam"], ran["sample"], ran["mask"], ran["exact"]) >= 30 and ran["outputs"] > 300
