@@ -19,6 +19,10 @@
  *   - O8(ii)/(iii) restated on the oracle's own balanced entries with multi-arc seed sets (poison and drops occur);
  *   - the state hash against published SplitMix64 vectors and its written composition; the DEP table against
  *     exhaustive chain enumeration.
+ *   - the extra modes (tests/test_oracle_modes.py, tests/test_compress.py): the sampled choice against the generator
+ *     restated in Python, states reached by sampling against the exhaustive fan-out (Theorem 1), hand-derived reaction
+ *     masks and step counts, the exact mode against rational rank by fraction elimination and brute force, the
+ *     compression pre-pass (oracle/compress.py) against brute-force EFMs and the unchanged exhaustive result.
  * Parity unpinned: the exact output sets of the configs "small".."genome" as a whole (no external truth exists; they
  * are held by the pins above, which cover every rule that produces them, and by GPU<->oracle parity).
  *
