@@ -248,3 +248,59 @@ def test_exact_mode_outputs_are_true_efms_of_the_toy_network(oracle_mod):
     ex = oracle_mod.enumerate_network(net, seed_sets=seeds, exact=True)
     assert {tuple(r) for r in ex.flux.tolist()} <= truth
     assert ex.stats["output"] + ex.stats["non_elementary"] + ex.stats["poisoned"] == ex.stats["unique_supports"]
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# sharper pins of the sampling rule: one candidate at a time, so that nothing is averaged away
+# ---------------------------------------------------------------------------------------------------------------------
+def test_each_candidate_takes_exactly_its_own_pick(oracle_mod):
+    """Node B (metabolite index 1) with five outputs behind A -> B: with C candidates the alternatives in use are exactly
+    {pick(seed, c, 1) mod 5 : c < C} -- checked for C = 1, 2, 3 and twenty generator seeds, so the candidate number, the
+    metabolite index and the modulus all matter.  With r3 and r5 masked the count runs over the three admissible ones only."""
+    rx = [({}, {"A": 1}, False), ({"A": 1}, {"B": 1}, False)] + [({"B": 1}, {}, False) for _ in range(5)]
+    net = hand_network(rx, ["A", "B"])
+    for seed in range(20):
+        for C in (1, 2, 3):
+            r = run(oracle_mod, net, [[0]], sample_count=C, sample_seed=seed)
+            got = {int(np.nonzero(row[2:])[0][0]) for row in r.flux.tolist()}
+            assert got == {pick(seed, c, 1) % 5 for c in range(C)}, (seed, C)
+            al = np.array([1, 1, 1, 0, 1, 0, 1], np.uint8)     # alternatives r2, r4, r6 remain (positions 0, 2, 4)
+            r = run(oracle_mod, net, [[0]], sample_count=C, sample_seed=seed, allowed=al)
+            got = {int(np.nonzero(row[2:])[0][0]) for row in r.flux.tolist()}
+            assert got == {[0, 2, 4][pick(seed, c, 1) % 3] for c in range(C)}, (seed, C)
+            assert r.cand_end[:, 0].tolist() == [1] * C
+
+
+def test_candidate_c_starts_from_seed_set_c_mod_n(oracle_mod):
+    """P5 with two seed sets (arcs: r0 -> 0, r2 -> 3): the roots of level 0 (test hook) show which set every candidate took."""
+    net = hand_network(*P5)
+
+    def roots(seed_sets, C, seed):
+        r = run(oracle_mod, net, seed_sets, sample_count=C, sample_seed=seed, trace=1)
+        assert r.n_roots == C
+        return sorted(tuple(sorted(e["flux"])) for e in r.trace[0])
+
+    for seed in range(4):
+        assert roots([[0], [4]], 1, seed) == [(0,)]
+        assert roots([[4], [0]], 1, seed) == [(3,)]
+        assert roots([[4], [0]], 2, seed) == [(0,), (3,)]
+        assert roots([[4], [0]], 3, seed) == [(0,), (3,), (3,)]      # candidates 0 and 2 start from {r2}, candidate 1 from {r0}
+        assert roots([[0], [4], [0, 4]], 5, seed) == [(0,), (0,), (0, 3), (3,), (3,)]
+
+
+def test_step_count_is_the_minimum_over_all_equal_duplicates(oracle_mod):
+    """P5: (1,1,1,0,0) is reached from {r0} in 2 expansions, from {r0, r1+} in 1 and from {r0, r1+, r2} in 0; (1,0,0,0,1) from
+    {r0} in 1 and from {r0, r4} in 0.  Whatever order the duplicates are grouped in, the smallest count is reported."""
+    net = hand_network(*P5)
+    sets = [[0], [0, 2], [0, 2, 4], [0, 8]]
+    import itertools
+    for perm in itertools.permutations(sets):
+        r = run(oracle_mod, net, list(perm))
+        rows = {tuple(v): s for v, s in zip(r.flux.tolist(), r.steps.tolist())}
+        assert rows[(1, 1, 1, 0, 0)] == 0 and rows[(1, 0, 0, 0, 1)] == 0
+    r = run(oracle_mod, net, [[0], [0, 2]])
+    rows = {tuple(v): s for v, s in zip(r.flux.tolist(), r.steps.tolist())}
+    assert rows[(1, 1, 1, 0, 0)] == 1 and rows[(1, 0, 0, 0, 1)] == 1
+    r = run(oracle_mod, net, [[0, 2], [0]])
+    rows = {tuple(v): s for v, s in zip(r.flux.tolist(), r.steps.tolist())}
+    assert rows[(1, 1, 1, 0, 0)] == 1 and rows[(1, 0, 0, 0, 1)] == 1
