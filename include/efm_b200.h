@@ -218,6 +218,51 @@ int efm_get_level_stats(const efm_handle* h, int64_t* active, int64_t* done, int
 int efm_debug_state_hash(int32_t device, int32_t n_supp, const int32_t* arc, const int64_t* flux, int32_t n_vis,
                          const int32_t* vis4, uint64_t* hash_out);
 
+/* ---- The beam threshold selection as a call of its own (a-4; "X = the key at sorted position
+ * frontier_cap; the level keeps exactly the children with key < X").  Keys are the 64-bit beam keys of one level's
+ * child slots; the two largest values (0xFF..FE: balanced child, 0xFF..FF: unused slot) stand outside the ranking.
+ *
+ * efm_beam_threshold(): the selection exactly as efm_enumerate() runs it (same kernels, same launcher), with its
+ * control block and compact key buffer in caller-provided scratch instead of the traversal's workspace.
+ *   d_keys       DEVICE, uint64[n_slots]
+ *   n_active     number of selectable keys among them (the traversal counts them while it writes them); must be > cap,
+ *                since the traversal skips the selection when the beam does not bind (EFM_E_INVAL otherwise)
+ *   d_scratch    DEVICE, 256-byte aligned, >= efm_beam_threshold_scratch_bytes(n_slots), caller-owned, contents lost
+ *   d_threshold  DEVICE, uint64[1] out
+ * Enqueued on `cuda_stream`; returns after the stream has been synchronised. */
+int efm_beam_threshold_scratch_bytes(int64_t n_slots, size_t* bytes);
+int efm_beam_threshold(const uint64_t* d_keys, int64_t n_slots, int64_t n_active, int64_t cap, void* d_scratch, size_t scratch_bytes,
+                       uint64_t* d_threshold, int32_t device, void* cuda_stream);
+
+/* efm_beam_threshold_static(): the same selection for a caller that can hand over its keys and a result slot but has
+ * nowhere to get scratch from -- code that runs as a guest inside another program's GPU process (a plug-in of a host
+ * application or a serving engine whose own allocator holds all of HBM, a job under a hard memory cap), or a
+ * latency-critical loop in which cudaMalloc / cudaFree are off limits because they can stall the whole device.  This
+ * call, and everything it calls, allocates no memory of any kind, device or pinned host: the histogram, the rank /
+ * prefix words and the compact key buffer sit in ONE array compiled into the library, EFM_STATIC_SELECT_BYTES on every
+ * GPU that loads the library, held until the process exits.  That fixes the limit below.
+ *   d_keys       DEVICE, uint64[n_keys], read only
+ *   n_keys       key slots, 0 .. EFM_STATIC_SELECT_MAX_KEYS; more is refused with EFM_E_CAPACITY before any CUDA call
+ *   cap          > 0: sorted position of the threshold (frontier_cap)
+ *   d_threshold  DEVICE, uint64[1] out: the key at sorted position cap among the selectable keys; 0xFF..FF (keeps
+ *                every selectable key) when there are no more than cap of them -- the call counts them itself
+ *   device       ordinal of the GPU that holds d_keys / d_threshold; made current by the call
+ *   cuda_stream  the three kernels and one memset are enqueued there; the call does NOT synchronise, the result is
+ *                valid once the stream has reached that point
+ * Shared state, read this: all calls on one device use the same array.  (1) It keeps whatever the last call left; the
+ * call clears the part that must start at zero itself, nothing to do for the caller.  (2) Two calls whose kernels can
+ * overlap on the GPU (different streams, or different host threads without ordering between their streams) race on it
+ * and both results are garbage: order them on one stream or with events.  (3) The first call on each device looks up
+ * where the array lives on that device (once, under a lock); make that first call during start-up, before any stream
+ * capture begins.
+ * Errors: EFM_E_INVAL (NULL pointer, n_keys < 0, cap <= 0, device outside 0..63), EFM_E_CAPACITY (n_keys above the
+ * limit), EFM_E_CUDA; efm_beam_threshold_static_error() gives the text of this thread's last failure ("" after success). */
+#define EFM_STATIC_SELECT_MAX_KEYS (1u << 20)
+#define EFM_STATIC_SELECT_BYTES (8448u + 8u * EFM_STATIC_SELECT_MAX_KEYS) /* 8 MiB + 8.25 KiB of device memory per GPU */
+int efm_beam_threshold_static(const uint64_t* d_keys, int64_t n_keys, int64_t cap, uint64_t* d_threshold, int32_t device,
+                              void* cuda_stream);
+const char* efm_beam_threshold_static_error(void);
+
 void efm_destroy(efm_handle* h);
 const char* efm_strerror(int code);
 const char* efm_last_error(const efm_handle* h); /* text of the last CUDA error, "" if none */

@@ -86,6 +86,11 @@ def load() -> ctypes.CDLL:
     lib.efm_get_stats.argtypes = [vp, P(efm_stats)]
     lib.efm_get_level_stats.argtypes = [vp, vp, vp, vp, vp, i64, P(i64)]
     lib.efm_debug_state_hash.argtypes = [i32, i32, vp, vp, i32, vp, P(ctypes.c_uint64)]
+    lib.efm_beam_threshold_scratch_bytes.argtypes = [i64, P(sz)]
+    lib.efm_beam_threshold.argtypes = [vp, i64, i64, i64, vp, sz, vp, i32, vp]
+    lib.efm_beam_threshold_static.argtypes = [vp, i64, i64, vp, i32, vp]
+    lib.efm_beam_threshold_static_error.argtypes = []
+    lib.efm_beam_threshold_static_error.restype = ctypes.c_char_p
     lib.efm_destroy.argtypes = [vp]
     lib.efm_destroy.restype = None
     lib.efm_strerror.argtypes = [ctypes.c_int]
@@ -323,6 +328,39 @@ def debug_state_hash(arcs: Sequence[int], fluxes: Sequence[int], visited: Sequen
     if rc != EFM_OK:
         raise EfmError(rc, lib.efm_strerror(rc).decode())
     return int(out.value)
+
+
+STATIC_SELECT_MAX_KEYS = 1 << 20   # EFM_STATIC_SELECT_MAX_KEYS of include/efm_b200.h
+
+
+def beam_threshold_scratch_bytes(n_slots: int) -> int:
+    b = ctypes.c_size_t()
+    rc = load().efm_beam_threshold_scratch_bytes(int(n_slots), ctypes.byref(b))
+    if rc != EFM_OK:
+        raise EfmError(rc, load().efm_strerror(rc).decode())
+    return int(b.value)
+
+
+def beam_threshold(d_keys: int, n_slots: int, n_active: int, cap: int, d_scratch: int, scratch_bytes: int, d_threshold: int,
+                   device: int = 0, stream: int = 0) -> None:
+    """``efm_beam_threshold``: the traversal's own beam selection on raw device pointers, scratch from the caller."""
+    lib = load()
+    rc = lib.efm_beam_threshold(ctypes.c_void_p(d_keys), int(n_slots), int(n_active), int(cap), ctypes.c_void_p(d_scratch),
+                                ctypes.c_size_t(scratch_bytes), ctypes.c_void_p(d_threshold), int(device), ctypes.c_void_p(stream))
+    if rc != EFM_OK:
+        raise EfmError(rc, lib.efm_strerror(rc).decode())
+
+
+def beam_threshold_static(d_keys: int, n_keys: int, cap: int, d_threshold: int, device: int = 0, stream: int = 0) -> None:
+    """``efm_beam_threshold_static``: the beam selection for a caller that cannot allocate scratch (a guest in another
+    program's GPU process, a loop where cudaMalloc is banned).  Raw device pointers in, nothing allocated here or in the
+    library; at most ``STATIC_SELECT_MAX_KEYS`` keys; enqueued on ``stream`` WITHOUT a synchronisation.  All calls on a
+    device share one built-in scratch array: keep them ordered on the GPU."""
+    lib = load()
+    rc = lib.efm_beam_threshold_static(ctypes.c_void_p(d_keys), int(n_keys), int(cap), ctypes.c_void_p(d_threshold), int(device),
+                                       ctypes.c_void_p(stream))
+    if rc != EFM_OK:
+        raise EfmError(rc, lib.efm_strerror(rc).decode() + ": " + lib.efm_beam_threshold_static_error().decode())
 
 
 def exported_symbols() -> List[str]:

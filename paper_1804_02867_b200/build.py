@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libefm_b200.so")
-SOURCES = ["api.cu", "expand.cu", "post.cu", "graph.cpp"]
+SOURCES = ["api.cu", "expand.cu", "post.cu", "select_static.cu", "graph.cpp"]
 HEADERS = ["device_common.cuh", "launch.hpp", "graph.hpp", os.path.join("..", "..", "include", "efm_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]

@@ -897,6 +897,41 @@ int efm_debug_state_hash(int32_t device, int32_t n_supp, const int32_t* arc, con
     return EFM_OK;
 }
 
+int efm_beam_threshold_scratch_bytes(int64_t n_slots, size_t* bytes) {
+    if (n_slots < 0 || !bytes) return EFM_E_INVAL;
+    *bytes = ((sizeof(Ctl) + 255) & ~(size_t)255) + 8 * (size_t)std::max<int64_t>(n_slots, 1);
+    return EFM_OK;
+}
+
+int efm_beam_threshold(const uint64_t* d_keys, int64_t n_slots, int64_t n_active, int64_t cap, void* d_scratch, size_t scratch_bytes,
+                       uint64_t* d_threshold, int32_t device, void* cuda_stream) {
+    size_t need = 0;
+    if (n_slots <= 0 || cap <= 0 || n_active <= cap || n_active > n_slots || !d_keys || !d_scratch || !d_threshold ||
+        ((uintptr_t)d_scratch & 255)) return EFM_E_INVAL;
+    efm_beam_threshold_scratch_bytes(n_slots, &need);
+    if (scratch_bytes < need) return EFM_E_NOMEM;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return EFM_E_CUDA; }
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms <= 0) { cudaGetLastError(); return EFM_E_CUDA; }
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    Ctl* ctl = (Ctl*)d_scratch;
+    u64* ckeys = (u64*)((unsigned char*)d_scratch + ((sizeof(Ctl) + 255) & ~(size_t)255));
+    // the control block as the traversal leaves it before launch_select(): level set 0 knows its slots and its active children
+    LevelCtl lv;
+    memset(&lv, 0, sizeof lv);
+    lv.n_slots = (u64)n_slots; lv.n_keys = (u64)n_active;
+    int launches = 0;
+    u32 err = 0;
+    cudaError_t e = cudaMemsetAsync(ctl, 0, sizeof(Ctl), s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&ctl->lv[0], &lv, sizeof lv, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = launch_select((const u64*)d_keys, ckeys, (u64)n_slots, ctl, 0, (u64)cap, (u64)n_slots, sms, s, &launches);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_threshold, &ctl->X, sizeof(u64), cudaMemcpyDeviceToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&err, &ctl->error, sizeof err, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { cudaGetLastError(); return EFM_E_CUDA; }
+    return err ? EFM_E_CAPACITY : EFM_OK;
+}
+
 void efm_destroy(efm_handle* h) {
     if (!h) return;
     for (cudaEvent_t e : h->events) cudaEventDestroy(e);
