@@ -179,6 +179,17 @@ def reduce_over_ranks(times_ms, counts, dist, device):
     return t.tolist() + c.tolist()
 
 
+def agreed_cap(cap_used: int, dist, device) -> int:
+    """The beam every replica times: the smallest one any rank had to fall back to (MIN over ranks), so that the summed
+    throughput describes ONE configuration.  `dist` is torch.distributed or None."""
+    import torch
+    if dist is None:
+        return int(cap_used)
+    t = torch.tensor([int(cap_used)], dtype=torch.int64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MIN)
+    return int(t.item())
+
+
 def rank_problem(workload: str, rank: int, cap: int):
     """The independent problem rank `rank` owns: the synthetic network of generator seed `rank`."""
     return _workload(workload, rank, cap)
@@ -237,6 +248,17 @@ def main_ours(args):
                 raise
             fallback_note = f"frontier_cap {args.cap} did not fit ({type(exc).__name__}); timed {cap_used // 2}"
             cap_used //= 2
+    if world > 1:
+        # replicas time ONE configuration: every rank takes the smallest beam any rank had to fall back to
+        agreed = agreed_cap(cap_used, dist, torch.device("cuda"))
+        if agreed != cap_used:
+            en.close()
+            del en
+            torch.cuda.empty_cache()
+            cap_used = agreed
+            fallback_note = f"frontier_cap {args.cap} did not fit on every rank; all ranks timed {cap_used}"
+            net, params, en = make_enumerator(cap_used)
+            en.enumerate(net.seed_sets, dense=False)
     args.cap = cap_used
     for _ in range(max(args.warmup, 3) - 1):
         en.enumerate(net.seed_sets, dense=False)

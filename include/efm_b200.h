@@ -65,8 +65,10 @@ typedef struct {
     int64_t max_frontier;   /* entries per frontier buffer; 0 = max(frontier_cap, 4096), 2^20 when cap == 0 */
     int64_t max_candidates; /* capacity of the candidate buffer / support hash; 0 = 2^20             */
     int64_t max_child_keys; /* child slots per level (8-byte beam key + 8-byte tag each, < 2^32);    */
-                            /* 0 = frontier_cap * the largest fan-out of a node (never overflows);   */
-                            /* a smaller value saves HBM and reports EFM_E_CAPACITY when exceeded    */
+                            /* 0 = max(frontier_cap * the largest fan-out of a node, sample_count,   */
+                            /* 65536): never overflows with a beam or in sampling mode; an unbounded */
+                            /* run (frontier_cap 0) with more children in a level, or a smaller      */
+                            /* explicit value, reports EFM_E_CAPACITY when exceeded                  */
     int32_t device;         /* CUDA device ordinal the workspace lives on                            */
     uint32_t flags;         /* EFM_F_*                                                               */
     int64_t max_frontier_bytes; /* bytes of one frontier buffer (entries are packed, variable size);         */

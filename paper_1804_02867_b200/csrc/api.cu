@@ -294,8 +294,10 @@ int efm_create(const int32_t* S, int32_t m, int32_t n, int64_t row_stride, const
         if (cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, P.device) == cudaSuccess && smc > 0) kSlackSMs = smc;
         else cudaGetLastError();
     }
-    h->max_keys = (P.max_child_keys ? P.max_child_keys : std::max<int64_t>(h->cap * (int64_t)G.max_fanout, 65536)) +
-                  (int64_t)expand_key_slack(kSlackSMs);
+    // default: a capped level has at most cap * fan-out children; a sampled candidate has one child at most; an unbounded
+    // run (cap == 0) gets 65536 slots and reports EFM_E_CAPACITY beyond (the caller sizes max_child_keys for its network)
+    const int64_t dflt_keys = std::max<int64_t>(std::max<int64_t>(h->cap * (int64_t)G.max_fanout, h->sample_count), 65536);
+    h->max_keys = (P.max_child_keys ? P.max_child_keys : dflt_keys) + (int64_t)expand_key_slack(kSlackSMs);
     if (h->max_keys > 0xFFFFFFF0LL) {   // slots are addressed with 32 bits; the default is clamped, an explicit request is refused
         if (P.max_child_keys) { delete h; return EFM_E_INVAL; }
         h->max_keys = 0xFFFFFFF0LL;
@@ -411,7 +413,10 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         roots.swap(cands);
     }
     const u64 n_roots = roots.size();
-    if ((int64_t)n_roots > h->max_frontier || (int64_t)n_roots > h->max_keys) return EFM_E_CAPACITY;
+    if ((int64_t)n_roots > h->max_frontier || (int64_t)n_roots > h->max_keys) {
+        h->last_error = "more roots than max_frontier / max_child_keys hold";
+        return EFM_E_CAPACITY;
+    }
     // seed sets as CSR of arc ids + the offset of every root entry in the staging buffer (16-byte units); the
     // entries themselves are built on the device (k_roots)
     std::vector<int> h_seed_ptr(n_roots + 1, 0), h_seed_arc;
@@ -424,8 +429,10 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
         stage_off[r] = stage_units;
         stage_units += entry_bytes((u32)roots[r].size(), 0, (u32)std::min<int64_t>(touched, G.M)) >> 4;
     }
-    if ((int64_t)(stage_units << 4) > h->frontier_bytes || h_seed_arc.size() * sizeof(int) > (size_t)h->max_keys * 8)
+    if ((int64_t)(stage_units << 4) > h->frontier_bytes || h_seed_arc.size() * sizeof(int) > (size_t)h->max_keys * 8) {
+        h->last_error = "the root entries / seed arcs do not fit max_frontier_bytes / max_child_keys";
         return EFM_E_CAPACITY;
+    }
 
     ON_DEVICE(h);
     if (!h->h_ctl) {
@@ -498,7 +505,8 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
     CK(up(ws + L.tags.off, h_seed_arc.data(), sizeof(int) * h_seed_arc.size()));
     CK(up(ws + L.off[1].off, stage_off.data(), sizeof(u64) * stage_off.size()));
     CK(cudaMemsetAsync(ws + L.ctl.off, 0, sizeof(Ctl), s));
-    CK(cudaMemsetAsync(ws + L.lvl.off, 0, sizeof(LevelStats) * 2, s));
+    // every record the host may walk: k_materialise skips record level + 1 at the last level, which must then read as empty
+    CK(cudaMemsetAsync(ws + L.lvl.off, 0, sizeof(LevelStats) * (size_t)(h->max_levels + 2), s));
     if (h->sample_count > 0) CK(cudaMemsetAsync(ws + L.cand_end.off, 0, sizeof(u64) * (size_t)(h->sample_count + 1), s));
     CK(cudaStreamSynchronize(s));   // the host staging vectors above go out of scope later; keep it simple
     int host_syncs = 1;
@@ -611,7 +619,7 @@ int efm_enumerate(efm_handle* h, const int32_t* seed_ptr, const int32_t* seed_ar
                 return EFM_E_CAPACITY;
             }
             more = (hc->lv[level & 1].alloc >> kAllocShift) != 0;
-            if (more && level >= (u64)h->max_levels) return EFM_E_CAPACITY;
+            if (more && level >= (u64)h->max_levels) { h->last_error = "active entries left after max_levels levels"; return EFM_E_CAPACITY; }
         }
         // per-level figures: record r holds the children of level r - 1 = the entries of level r
         for (size_t r = 0; r < recs.size(); ++r) {

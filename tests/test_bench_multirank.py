@@ -22,8 +22,9 @@ def _worker(rank, world, port, out):
     times = [10.0 + rank, 100.0 - rank]               # rank-dependent so that MAX and SUM are distinguishable
     counts = [float(net.S.shape[1]), float(rank + 1), 7.0]
     red = bench.reduce_over_ranks(times, counts, dist, torch.device("cpu"))
+    cap = bench.agreed_cap(1 << (24 - rank), dist, torch.device("cpu"))   # rank 1 "fell back" one size
     dist.barrier()
-    out[rank] = (red, int(np.abs(net.S).sum()), params["frontier_cap"])
+    out[rank] = (red, int(np.abs(net.S).sum()), params["frontier_cap"], cap)
     dist.destroy_process_group()
 
 
@@ -39,9 +40,11 @@ def test_replica_reduction_world_size_2():
     assert (c_a, c_b, c_c) == (64.0, 3.0, 14.0)        # SUM over ranks (32 reactions per small network)
     assert r0[1] != r1[1]                              # different generator seeds: independent problems
     assert r0[2] == r1[2] == 512
+    assert r0[3] == r1[3] == 1 << 23                   # every rank times the smallest beam any rank fell back to
 
 
 def test_single_rank_is_identity():
     sys.path.insert(0, ROOT)
     import bench
     assert bench.reduce_over_ranks([1.5, 2.5], [3.0], None, torch.device("cpu")) == [1.5, 2.5, 3.0]
+    assert bench.agreed_cap(1 << 22, None, torch.device("cpu")) == 1 << 22

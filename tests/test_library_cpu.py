@@ -1,8 +1,8 @@
-import os
 """CPU-side checks of the CUDA library: it builds, loads, exports the C ABI of include/efm_b200.h, its host-side
 graph builder (SURVEY.md 8(a) a-1) agrees with the oracle's graph, seeds are validated, and without a GPU the
 product path fails loudly instead of falling back to anything."""
 import ctypes
+import os
 
 import numpy as np
 import pytest
