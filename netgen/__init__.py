@@ -7,6 +7,7 @@ and the parameter sets of the five ``BASELINE.json`` configs.
 """
 from .networks import (  # noqa: F401
     CONFIGS,
+    chain_pair_network,
     Network,
     SplitMix64,
     config_names,
@@ -15,5 +16,6 @@ from .networks import (  # noqa: F401
     mirrored,
     random_seed_sets,
     unimolecular_network,
+    wide_fan_network,
     with_dead_ends,
 )

@@ -523,6 +523,32 @@ def hand_network(reactions: Sequence[Tuple[Dict[str, int], Dict[str, int], bool]
     return Network(name, 0, S, rev, internal, p, None, {})
 
 
+def wide_fan_network(n_p: int = 300, n_q: int = 200, **params) -> Network:
+    """r0 -> P_0 .. P_{n_p-1} and r1 -> Q_0 .. Q_{n_q-1}, every product with two consumers: a pathway grown from r0 has
+    n_p - k unbalanced metabolites after k steps (with n_p = 300: more than the 255 the top byte of a beam key can hold), one
+    grown from r1 has n_q - k, and both families double their number of entries with every level."""
+    mets = [f"P{i}" for i in range(n_p)] + [f"Q{i}" for i in range(n_q)]
+    rx = [({}, {f"P{i}": 1 for i in range(n_p)}, False), ({}, {f"Q{i}": 1 for i in range(n_q)}, False)]
+    for m in mets:
+        rx += [({m: 1}, {}, False), ({m: 1}, {}, False)]
+    return hand_network(rx, mets, **params)
+
+
+def chain_pair_network(len_a: int, len_b: int, **params) -> Network:
+    """Two disjoint linear chains a0: -> A_0, a_i: A_{i-1} -> A_i, a_len: A_{len-1} -> (and the same with B); every tenth step
+    produces two molecules so that the fluxes are not all 1.  Each chain is one EFM with len + 1 reactions; a pathway seeded on
+    both a0 and b0 balances to their sum (len_a + len_b + 2 reactions), which is not elementary."""
+    rx, mets = [], []
+    for tag, ln in (("A", len_a), ("B", len_b)):
+        names = [f"{tag}{i}" for i in range(ln)]
+        mets += names
+        rx.append(({}, {names[0]: 1}, False))
+        for i in range(1, ln):
+            rx.append(({names[i - 1]: 1}, {names[i]: 2 if i % 10 == 0 else 1}, False))
+        rx.append(({names[-1]: 1}, {}, False))
+    return hand_network(rx, mets, **params)
+
+
 def unimolecular_network(seed: int, m_int: int, n_rxn: int, n_rev: int = 0) -> Network:
     """Unit-coefficient network with at most one internal substrate and one internal product per
     reaction (sources, sinks and internal A->B links).  On such networks the EFM set is exactly

@@ -6,7 +6,7 @@ counts are derived by hand on the P1 / P2 / P5 networks of SURVEY.md 8(c)."""
 import numpy as np
 import pytest
 
-from netgen import hand_network, make_network
+from netgen import chain_pair_network, hand_network, make_network
 
 M64 = (1 << 64) - 1
 
@@ -238,6 +238,29 @@ def test_exact_mode_against_rational_rank(oracle_mod, name, over, count):
         assert rejected > 0   # the rank test did something the data could show
 
 
+def chain_flux(length):
+    """Closed form of netgen.chain_pair_network's single chain: step i (1 <= i < length) turns one A_{i-1} into 2 A_i when
+    i % 10 == 0, else into one; balancing node by node, reaction i + 1 runs at the rate A_i is produced."""
+    f = [1, 1]
+    for i in range(1, length):
+        f.append(f[-1] * (2 if i % 10 == 0 else 1))
+    return f
+
+
+@pytest.mark.parametrize("len_a,len_b,D", [(70, 20, 96), (100, 24, 128)])
+def test_exact_mode_on_supports_wider_than_64_arcs(oracle_mod, len_a, len_b, D):
+    """Def 3 on supports of 71 / 101 arcs: each chain alone is elementary (closed-form fluxes above), the
+    pathway seeded on both chain heads balances to their sum over len_a + len_b + 2 arcs and has nullity 2."""
+    net = chain_pair_network(len_a, len_b, max_support=D)
+    na = len_a + 1
+    fa, fb = chain_flux(len_a), chain_flux(len_b)
+    r = run(oracle_mod, net, [[0], [2 * na], [0, 2 * na]], exact=True)
+    assert r.flux.tolist() == sorted([fa + [0] * (len_b + 1), [0] * na + fb])
+    assert (r.stats["unique_supports"], r.stats["non_elementary"], r.stats["output"]) == (3, 1, 2)
+    plain = run(oracle_mod, net, [[0, 2 * na]])          # the pairwise filter alone cannot see it: nothing smaller was found
+    assert plain.flux.tolist() == [fa + fb]
+
+
 def test_exact_mode_outputs_are_true_efms_of_the_toy_network(oracle_mod):
     """Brute force (every arc subset without a twin pair whose nullspace is one strictly positive ray) fixes the EFM set of
     toy; the exact mode returns exactly the found candidates that are in it."""
@@ -269,6 +292,35 @@ def test_each_candidate_takes_exactly_its_own_pick(oracle_mod):
             got = {int(np.nonzero(row[2:])[0][0]) for row in r.flux.tolist()}
             assert got == {[0, 2, 4][pick(seed, c, 1) % 3] for c in range(C)}, (seed, C)
             assert r.cand_end[:, 0].tolist() == [1] * C
+
+
+def test_sampled_choice_counts_only_what_the_support_cap_admits(oracle_mod):
+    """Reading G23 with a binding D (reading G15): r0 -> A, r1 A -> 3 B, r2 .. r6 B ->; one candidate from the seed set
+    {r0, r3, r5} with max_support = 4.  A (first visit) adds r1: the support {r0, r1, r3, r5} is full.  B: EF = 3 - 2 = +1,
+    first visit; of its five outputs only r3 and r5 (already in the support) are admissible, so the candidate takes
+    [r3, r5][pick(seed, 0, 1) mod 2] -- not mod 5 -- bumps it to 2 and is balanced after two expansions."""
+    rx = [({}, {"A": 1}, False), ({"A": 1}, {"B": 3}, False)] + [({"B": 1}, {}, False) for _ in range(5)]
+    net = hand_network(rx, ["A", "B"], max_support=4)
+    free = hand_network(rx, ["A", "B"])
+    seen = set()
+    differs = 0
+    for seed in range(24):
+        r = run(oracle_mod, net, [[0, 6, 10]], sample_count=1, sample_seed=seed)
+        k = pick(seed, 0, 1) % 2
+        seen.add(k)
+        differs += [3, 5][k] != 2 + pick(seed, 0, 1) % 5
+        want = [1, 1, 0, 1, 0, 1, 0]
+        want[[3, 5][k]] = 2
+        assert r.flux.tolist() == [want], seed
+        assert r.cand_end.tolist() == [[1, 2]] and r.steps.tolist() == [2]
+    assert seen == {0, 1} and differs >= 12
+    # without the cap all five are admissible again and the modulus is 5
+    for seed in range(24):
+        r = run(oracle_mod, free, [[0, 6, 10]], sample_count=1, sample_seed=seed)
+        j = 2 + pick(seed, 0, 1) % 5
+        want = [1, 1, 0, 1, 0, 1, 0]
+        want[j] += 1
+        assert r.flux.tolist() == [want], seed
 
 
 def test_candidate_c_starts_from_seed_set_c_mod_n(oracle_mod):

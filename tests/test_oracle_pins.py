@@ -12,7 +12,8 @@ from math import gcd
 import numpy as np
 import pytest
 
-from netgen import SplitMix64, hand_network, make_network, mirrored, random_seed_sets, unimolecular_network
+from netgen import (SplitMix64, chain_pair_network, hand_network, make_network, mirrored, random_seed_sets, unimolecular_network,
+                    wide_fan_network)
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "hand_pins.json")
 
@@ -418,9 +419,32 @@ def test_beam_against_sorted_definition(oracle_mod, name, cap):
     h >> 8 with n_unb counted here from S_int . v; the level keeps exactly the entries with key <= T*, T* the largest
     value such that #{key <= T*} <= cap (sort-based, ties stand or fall together)."""
     net = make_network(name, 0)
-    res = oracle_mod.enumerate_network(net, self_check=False, trace=True, frontier_cap=cap)
+    _beam_restatement(oracle_mod, net, cap, object)
+
+
+def test_beam_key_clamps_the_unbalanced_count_at_255(oracle_mod):
+    """key = min(n_unb, 255) << 56 | h >> 8.  On netgen.wide_fan_network (r0 -> P_0 .. P_299, r1 -> Q_0 .. Q_199,
+    two consumers per product) with seeds {r0}, {r1} level k holds 2^k
+    entries with n_unb = 300 - k (clamped: top byte 0xff) and 2^k with n_unb = 200 - k (top byte 200 - k < 0xff).  cap 40 binds
+    from level 5 on (32 + 32 entries): every entry of the r1 family ranks before every entry of the r0 family, which are ranked
+    among themselves by the hash bits alone.  A clamp at 127 would mix the families, no clamp would wrap 295 to 39 and put the r0
+    family first; the restatement (n_unb recounted from S . v) fails on either."""
+    net = wide_fan_network()
+    levels = _beam_restatement(oracle_mod, net, 40, np.int64, seed_sets=[[0], [2]], max_visited=7)
+    lvl5 = levels[5]
+    big = [e for e in lvl5 if e["n_unb"] == 295]
+    small = [e for e in lvl5 if e["n_unb"] == 195]
+    assert len(big) == 32 and len(small) == 32
+    assert all(e["key"] >> 56 == 0xff for e in big) and all(e["key"] >> 56 == 195 for e in small)
+    assert all(e["kept"] for e in small) and sum(e["kept"] for e in big) == 8
+    kept_big = sorted(e["key"] for e in big if e["kept"])
+    assert kept_big == sorted(e["key"] for e in big)[:8]          # ... by the 56 hash bits
+
+
+def _beam_restatement(oracle_mod, net, cap, dtype, **over):
+    res = oracle_mod.enumerate_network(net, self_check=False, trace=True, frontier_cap=cap, **over)
     assert res.stats["truncated_beam"] > 0
-    Sint = net.S[net.internal.astype(bool)].astype(object)
+    Sint = net.S[net.internal.astype(bool)].astype(dtype)
     arc_col = []
     for j in range(net.n):
         arc_col.append((j, 1))
@@ -431,7 +455,7 @@ def test_beam_against_sorted_definition(oracle_mod, name, cap):
     for lvl in res.trace:
         keys = []
         for e in lvl:
-            v = np.zeros(net.n, dtype=object)
+            v = np.zeros(net.n, dtype=dtype)
             for a, f in e["flux"].items():
                 v[arc_col[a][0]] += arc_col[a][1] * f
             n_unb = int(np.count_nonzero(Sint.dot(v)))
@@ -462,6 +486,7 @@ def test_beam_against_sorted_definition(oracle_mod, name, cap):
         assert count <= cap
         truncated += len(keys) - count
     assert cut_levels > 0 and truncated == res.stats["truncated_beam"]
+    return res.trace
 
 
 def test_beam_ties_stand_or_fall_together(oracle_mod):

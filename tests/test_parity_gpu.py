@@ -7,7 +7,8 @@ import os
 import numpy as np
 import pytest
 
-from netgen import hand_network, make_network, random_seed_sets, unimolecular_network, with_dead_ends
+from netgen import (chain_pair_network, hand_network, make_network, random_seed_sets, unimolecular_network, wide_fan_network,
+                    with_dead_ends)
 
 pytestmark = pytest.mark.gpu
 
@@ -529,6 +530,59 @@ def test_exact_elementarity(efm, oracle_mod, name, over, count):
     if net.n_arcs > 129:   # the basis of the rank test lives in shared memory: supports of at most 128 arcs
         with pytest.raises(efm.EfmError):
             efm.Enumerator(net.S, net.reversible, net.internal, dict(net.params, max_support=129), flags=efm.EFM_F_EXACT_ELEMENTARITY)
+
+
+@pytest.mark.parametrize("len_a,len_b,D", [(70, 20, 96), (100, 24, 128)])
+def test_exact_elementarity_three_and_four_chunks_by_hand(efm, oracle_mod, len_a, len_b, D):
+    """k_rank_test<3> (D 65..96) and <4> (D 97..128) on supports that really are that wide: two disjoint chains of 71 / 101 and
+    21 / 25 reactions.  Each chain is elementary; the pathway seeded on both heads is their sum (92 / 126 arcs, nullity 2) and
+    goes.  Expected values are the closed form of the chain (tests/test_oracle_modes.py), then parity with the oracle."""
+    from test_oracle_modes import chain_flux
+    net = chain_pair_network(len_a, len_b, max_support=D)
+    na = len_a + 1
+    seeds = [[0], [2 * na], [0, 2 * na]]
+    got = efm.enumerate_network(net, seed_sets=seeds, flags=efm.EFM_F_EXACT_ELEMENTARITY)
+    assert got.flux.tolist() == sorted([chain_flux(len_a) + [0] * (len_b + 1), [0] * na + chain_flux(len_b)])
+    assert (got.stats["unique_supports"], got.stats["non_elementary"], got.stats["output"]) == (3, 1, 2)
+    assert_parity(efm, oracle_mod, net, seeds=seeds, flags=efm.EFM_F_EXACT_ELEMENTARITY)
+
+
+@pytest.mark.parametrize("over", [dict(frontier_cap=2048, max_support=96), dict(frontier_cap=1024, max_support=128, max_visited=200)])
+def test_exact_elementarity_three_and_four_chunks_on_genome(efm, oracle_mod, over):
+    """The same two instantiations on the genome-scale network with multi-arc seed sets: thousands of candidate supports of
+    up to D arcs, most of them rejected, on both sides."""
+    net = make_network("genome", 0)
+    seeds = random_seed_sets(net, 300, 2, 11)
+    got, ref = assert_parity(efm, oracle_mod, net, seeds=seeds, flags=efm.EFM_F_EXACT_ELEMENTARITY, **over)
+    assert int(got.stats["non_elementary"]) > 1000 and int(got.stats["output"]) > 100
+    assert int((got.flux != 0).sum(axis=1).max()) > 64
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# SURVEY.md 8(c)-B key clamp and reading G23 under a binding support cap, on the device
+# ---------------------------------------------------------------------------------------------------------------------
+def test_more_than_255_unbalanced_metabolites(efm, oracle_mod):
+    """netgen.wide_fan_network: entries with 300 - k unbalanced metabolites (key top byte clamped to 0xff) next to entries with
+    200 - k, a beam of 40 that binds from level 5 on (tests/test_oracle_pins.py restates which entries stay)."""
+    net = wide_fan_network()
+    got, ref = assert_parity(efm, oracle_mod, net, seeds=[[0], [2]], frontier_cap=40, max_visited=7)
+    assert int(got.stats["truncated_beam"]) > 0 and int(got.stats["discarded_visited"]) > 0
+    assert_parity(efm, oracle_mod, net, seeds=[[0]], frontier_cap=16, max_visited=12)   # every key of every level has the top byte 0xff
+
+
+def test_sampled_choice_under_a_binding_support_cap(efm, oracle_mod):
+    """Reading G23 with D binding (hand-derived in tests/test_oracle_modes.py): r0 -> A, r1 A -> 3 B, r2 .. r6 B ->; seed set
+    {r0, r3, r5}, max_support 4: the candidate chooses among r3 and r5 only.  No oracle needed for the expected row."""
+    from test_oracle_modes import pick
+    rx = [({}, {"A": 1}, False), ({"A": 1}, {"B": 3}, False)] + [({"B": 1}, {}, False) for _ in range(5)]
+    net = hand_network(rx, ["A", "B"], max_support=4)
+    for seed in range(24):
+        got = efm.enumerate_network(net, seed_sets=[[0, 6, 10]], sample_count=1, sample_seed=seed)
+        want = [1, 1, 0, 1, 0, 1, 0]
+        want[[3, 5][pick(seed, 0, 1) % 2]] = 2
+        assert got.flux.tolist() == [want], seed
+        assert got.cand_end.tolist() == [[1, 2]]
+    assert_parity(efm, oracle_mod, net, seeds=[[0, 6, 10], [0, 8]], sample_count=7, sample_seed=5)
 
 
 # ---------------------------------------------------------------------------------------------------------------------
