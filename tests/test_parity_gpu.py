@@ -199,6 +199,43 @@ def test_genome_at_the_bench_configuration(efm, oracle_mod):
     assert got.stats["truncated_beam"] > 0 and got.stats["output"] > 100000
 
 
+def _digest_cases():
+    path = os.path.join(os.path.dirname(GOLDEN), "digests.json")
+    with open(path) as fh:
+        return json.load(fh)["cases"]
+
+
+@pytest.mark.parametrize("case", _digest_cases(), ids=lambda c: f"{c['workload']}-{c['frontier_cap']}")
+def test_digests_at_large_beams(efm, case):
+    """The CUDA path against what the oracle returned at beams the oracle needs tens of minutes for (tests/golden/digests.json,
+    written by tests/golden/make_digests.py from oracle/ alone): every counter, the per-level series, and SHA-256 of the
+    canonical output rows (CSR, strict lexicographic order) and of their step counts."""
+    import importlib.util
+    import bench
+    spec = importlib.util.spec_from_file_location("make_digests", os.path.join(os.path.dirname(GOLDEN), "make_digests.py"))
+    md = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(md)
+    net = make_network(case["workload"], case["generator_seed"])
+    cap = case["frontier_cap"]
+    assert dict(net.params, frontier_cap=cap) == case["params"]
+    if case["workload"] == "genome":
+        params = bench.sized_params(net.params, cap)
+    else:   # capacity only (an overflow would be a loud EFM_E_CAPACITY): room for twice the balanced pathways the oracle counted
+        params = dict(net.params, frontier_cap=cap, max_candidates=max(1 << 20, 2 * case["counters"]["done"]))
+    en = efm.Enumerator(net.S, net.reversible, net.internal, params)
+    res = en.enumerate(net.seed_sets, dense=False)
+    for k, v in case["counters"].items():
+        assert int(res.stats[k]) == v, (k, res.stats[k], v)
+    assert int(res.stats["n_roots"]) == case["n_roots"]
+    for k, v in case["levels"].items():
+        assert res.levels[k].tolist() == v, k
+    row_ptr, rxn, val = (t.numpy() for t in en.result_csr(pinned=False))
+    got = md.digest_csr(row_ptr, rxn, val, res.steps)
+    for k in ("rows", "nnz", "steps_sha256", "rows_sha256"):
+        assert got[k] == case[k], k
+    en.close()
+
+
 def test_general_routine_only(efm, oracle_mod):
     """EFM_F_NO_FASTPATH sends every child through the warp-cooperative general routine: both routes must agree
     with the oracle (and hence with each other)."""
