@@ -417,12 +417,14 @@ __global__ void __launch_bounds__(kJoinThreads) k_filter_join(const PostArgs a) 
         const u32 bend = s_gend;
         const u32 n0 = ~sv.x, n1 = ~sv.y, n2 = ~sv.z, n3 = ~sv.w & 0xffffu;
         bool found = false;
+        u32 tested = 0;   // first-stage pair tests this row really made (a hit ends its scan)
         for (u32 base = g0; base < bend; base += kWTile) {
             for (u32 i = threadIdx.x; i < (u32)kWTile; i += kJoinThreads) wt[i] = base + i < bend ? a.g_sig64[base + i] : make_uint2(0xffffffffu, 0xffffffffu);
             __syncthreads();
             if (live && !found && base < gend) {
                 // eight rows of W per step, one branch: rows behind gend (or behind the tile) are filtered in the closer look
                 const u32 jn = (min((u32)kWTile, gend - base) + 7u) / 8u;
+                u32 jstop = jn;
 #pragma unroll 1
                 for (u32 j = 0; j < jn; ++j) {
                     const uint4 ra = wt4[4 * j], rb = wt4[4 * j + 1], rc = wt4[4 * j + 2], rd = wt4[4 * j + 3];
@@ -440,14 +442,15 @@ __global__ void __launch_bounds__(kJoinThreads) k_filter_join(const PostArgs a) 
                             if (((sg.x & n0) | (sg.y & n1) | (sg.z & n2) | (sg.w & n3)) == 0)
                                 found = exact || arcs_subset(a.cand + (u64)a.g_row[row] * a.cand_stride, a.cand + (u64)a.uniq[u] * a.cand_stride);
                         }
-                        if (found) break;
+                        if (found) { jstop = j + 1; break; }
                     }
                 }
+                tested += min(8u * jstop, min((u32)kWTile, gend - base));
             }
             __syncthreads();
         }
         if (found) a.keep[u] = 0;
-        if (live && gend > g0) atomicAdd(&s_pairs, (unsigned long long)(gend - g0));   // pair tests this row stands for
+        if (tested) atomicAdd(&s_pairs, (unsigned long long)tested);
         __syncthreads();
         if (threadIdx.x == 0 && s_pairs) atomicAdd(&a.ctl->filter_pairs, (u64)s_pairs);
         __syncthreads();
